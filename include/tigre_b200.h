@@ -1,0 +1,152 @@
+/*
+ * tigre_b200.h — C ABI of libtigre_b200: the cone-beam projector pair of TIGRE-style
+ * iterative CT reconstruction (arxiv 2412.10129), hand-written CUDA for sm_100a.
+ *
+ * Citations are to /root/reference/PAPER.md (line, section) and to the readings P1..P19
+ * in DESIGN.md where the paper is silent.
+ *
+ * Conventions (all entry points)
+ *   units      mm and radians
+ *   volume     float32, vol[iz][iy][ix], x fastest, nVoxel = (nx,ny,nz)
+ *   projections float32, proj[ia][iv][iu], u fastest, nDetector = (nu,nv)
+ *   pointers   "dev" = CUDA device memory of the current device; "host" = ordinary host memory
+ *              read during the call only; "pinned" = page-locked host memory (chunked path).
+ *              The library keeps no pointer after a call returns.
+ *   stream     `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *              Kernels are enqueued on it; calls that return host scalars synchronise it.
+ *   memory     The library owns no persistent device memory.  Temporaries (per-view parameter
+ *              tables; driver work buffers) come from the device's stream-ordered pool
+ *              (cudaMallocAsync / cudaFreeAsync on `cuda_stream`); tigre_workspace_bytes()
+ *              reports how much a call will take so the caller can budget HBM.
+ *   errors     0 on success, negative tigre_status otherwise.  No exception crosses the ABI.
+ *              There is no CPU fallback: without a CUDA device every compute call fails.
+ */
+#ifndef TIGRE_B200_H
+#define TIGRE_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define TIGRE_API __attribute__((visibility("default")))
+#else
+#define TIGRE_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Geometry descriptor: App. B Table B1; §2.4 lines 179-197.
+ * sVoxel / sDetector are derived (n*d) (reading P1).  The `_a` pointers are optional host
+ * arrays of length nAngles ("defined individually for each projection"); when
+ * NULL the scalar member is used for every view. */
+typedef struct tigre_geo {
+    uint32_t struct_size;       /* = sizeof(tigre_geo); checked                              */
+    int32_t  nVoxel[3];         /* x, y, z                                                    */
+    double   dVoxel[3];         /* mm                                                         */
+    int32_t  nDetector[2];      /* u, v                                                       */
+    double   dDetector[2];      /* mm                                                         */
+    double   DSD, DSO, COR;     /* source-detector, source-origin distance; axis shift (Oy)   */
+    double   offOrigin[3];      /* volume centre w.r.t. O (Oxyz)                              */
+    double   offDetector[2];    /* detector centre shift (uv)                                 */
+    double   rotDetector[3];    /* in-place detector rotation (phi, theta, psi)               */
+    const double *DSD_a, *DSO_a, *COR_a;        /* [nA]     or NULL                           */
+    const double *offOrigin_a;                  /* [nA][3]  or NULL                           */
+    const double *offDetector_a;                /* [nA][2]  or NULL                           */
+    const double *rotDetector_a;                /* [nA][3]  or NULL                           */
+    double   accuracy;          /* interpolated-mode step in voxels (0.5 in configs C2, C4)   */
+} tigre_geo;
+
+typedef enum tigre_status {
+    TIGRE_OK = 0,
+    TIGRE_ERR_ARG = -1,       /* NULL pointer, bad mode, bad struct_size, bad sizes            */
+    TIGRE_ERR_GEOMETRY = -2,  /* DSO<=0, DSD<=0, non-positive sizes, or a volume corner at or  */
+                              /* behind the source plane of some view (voxel-driven calls)     */
+    TIGRE_ERR_MEMSPACE = -3,  /* a data pointer is in the wrong memory space                   */
+    TIGRE_ERR_WORKSPACE = -4, /* a temporary allocation failed                                 */
+    TIGRE_ERR_CUDA = -5,      /* any other CUDA error (tigre_last_cuda_error() gives the text) */
+    TIGRE_ERR_NO_DEVICE = -6  /* no CUDA device: there is no CPU fallback                      */
+} tigre_status;
+
+enum { TIGRE_AX_SIDDON = 0, TIGRE_AX_INTERP = 1 };
+enum { TIGRE_ATB_MATCHED = 0, TIGRE_ATB_FDK = 1 };
+enum { TIGRE_OP_AX = 0, TIGRE_OP_ATB = 1, TIGRE_OP_OSSART = 2, TIGRE_OP_CGLS = 3, TIGRE_OP_FDK = 4 };
+
+/* ---- the projector pair ------------------------------------------------------------------
+ * tigre_Ax: forward projection b = A x, line integrals of the volume along the source->pixel
+ * segments (§2.1 eq. 1).  Ray-driven, one thread per detector pixel.
+ *   mode TIGRE_AX_SIDDON  exact intersection lengths with the voxel grid (DESIGN.md O-A)
+ *   mode TIGRE_AX_INTERP  fixed-step trilinear sampling, step geo->accuracy voxels (O-B, P9)
+ *   vol   dev, [nz][ny][nx], read      proj  dev, [nA][nv][nu], overwritten
+ *   angles host, [nA][3] Euler ZYZ (z1,y1,z2); a circular scan is (theta,0,0)
+ * If both vol and proj are PINNED HOST pointers the call takes the single-GPU host-chunking
+ * path (z-slabs of the volume and angle batches stream through HBM) and
+ * synchronises before returning.  Pageable host data pointers give TIGRE_ERR_MEMSPACE. */
+TIGRE_API int tigre_Ax(const float *vol, const tigre_geo *geo, const double *angles, int nA, int mode,
+             float *proj, void *cuda_stream);
+
+/* tigre_Atb: voxel-driven backprojection x = A^T b used by eqs. 4 and 6;
+ * bilinear detector interpolation with zero border, weight per voxel-view
+ *   mode TIGRE_ATB_MATCHED  w = (dx dy dz)/(du dv) * R^2/(r^2 cos gamma)   (P10)
+ *   mode TIGRE_ATB_FDK      w = (DSO/(DSO - X'_x))^2
+ *   proj dev, [nA][nv][nu], read       vol  dev, [nz][ny][nx], OVERWRITTEN
+ * Pinned-host pointers select the chunked path as for tigre_Ax. */
+TIGRE_API int tigre_Atb(const float *proj, const tigre_geo *geo, const double *angles, int nA, int mode,
+              float *vol, void *cuda_stream);
+
+/* ---- SIRT / OS-SART weights and elementwise updates (eq. 6 at 135) ----------
+ * W = 1/(A 1) where (A 1) > 1e-2*min(dVoxel), else 0   (row sums; proj-shaped, dev)
+ * V = 1/(A^T 1) where (A^T 1) > 1e-6*max(A^T 1), else 0 (column sums; vol-shaped, dev)  (P13) */
+TIGRE_API int tigre_row_weights(const tigre_geo *geo, const double *angles, int nA, int ax_mode, float *W,
+                      void *cuda_stream);
+TIGRE_API int tigre_col_weights(const tigre_geo *geo, const double *angles, int nA, int atb_mode, float *V,
+                      void *cuda_stream);
+/* r = W .* (b - Ax)  (W may be NULL = ones); *nrm2 (host, may be NULL) = ||b - Ax||_2^2.
+ * All arrays dev, n elements.  Synchronises only when nrm2 != NULL. */
+TIGRE_API int tigre_residual(const float *b, const float *Ax, const float *W, float *r, size_t n, double *nrm2,
+                   void *cuda_stream);
+/* x <- x + lambda * V .* g, then x <- max(x,0) if nonneg  (V may be NULL = ones).  dev, n elements */
+TIGRE_API int tigre_update(float *x, const float *g, const float *V, float lambda, int nonneg, size_t n,
+                 void *cuda_stream);
+
+/* ---- drivers ------------------------------------------------------------------------------
+ * OS-SART (eq. 6; DESIGN.md O-E): for it, for subset s:
+ *   r = W_s .* (b_s - A_s x);  x += lambda * V_s .* A_s^T r;  x = max(x,0) if nonneg.
+ * Subsets are CSR lists of view indices: subset s = subset_idx[subset_off[s] .. subset_off[s+1]).
+ * One subset holding all views is SIRT.  resid_hist[it] (host, may be NULL) = running
+ * ||b - A x||_2 over the sweep.  b dev [nA][nv][nu]; x_inout dev (initial iterate in, result out). */
+TIGRE_API int tigre_ossart(const float *b, const tigre_geo *geo, const double *angles, int nA,
+                 const int32_t *subset_idx, const int32_t *subset_off, int nSubsets, int n_iter,
+                 float lambda, int nonneg, int ax_mode, int atb_mode, float *x_inout,
+                 double *resid_hist, void *cuda_stream);
+/* CGLS (textbook recurrences, DESIGN.md O-F), x0 = 0; x_out dev. */
+TIGRE_API int tigre_cgls(const float *b, const tigre_geo *geo, const double *angles, int nA, int n_iter,
+               int ax_mode, int atb_mode, float *x_out, double *resid_hist, void *cuda_stream);
+/* FDK (DESIGN.md O-D): cosine weight, Ram-Lak ramp filter along u, FDK-weighted
+ * backprojection scaled by pi/nA (full 2 pi orbit).  b dev, x_out dev. */
+TIGRE_API int tigre_fdk(const float *b, const tigre_geo *geo, const double *angles, int nA, float *x_out,
+              void *cuda_stream);
+/* the FDK pre-filter alone: q = tau * ((b * cos) conv h), per detector row.  dev -> dev */
+TIGRE_API int tigre_fdk_filter(const float *b, const tigre_geo *geo, const double *angles, int nA, float *q,
+                     void *cuda_stream);
+
+/* ---- measurement helpers -------------------------------------------------------------------
+ * Exact count of ray-samples of one tigre_Ax call without marching the data (BASELINE metric:
+ * Siddon = non-zero voxel segments; interpolated = samples K inside the grown box).
+ * counts: dev uint32 [nA][nv][nu] or NULL; *total (host) = sum.  Synchronises. */
+TIGRE_API int tigre_Ax_count(const tigre_geo *geo, const double *angles, int nA, int mode, uint32_t *counts,
+                   uint64_t *total, void *cuda_stream);
+/* bytes of stream-ordered temporaries a call of kind `op` will allocate */
+TIGRE_API size_t tigre_workspace_bytes(const tigre_geo *geo, int nA, int op);
+/* tuning knobs of the chunked path: device bytes it may use for slabs (0 = default 3/4 of free) */
+TIGRE_API int tigre_set_chunk_budget(size_t bytes);
+
+TIGRE_API const char *tigre_strerror(int code);
+TIGRE_API const char *tigre_last_cuda_error(void);
+TIGRE_API int tigre_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TIGRE_B200_H */

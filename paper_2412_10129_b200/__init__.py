@@ -1,0 +1,288 @@
+"""Thin Python binding of libtigre_b200 (include/tigre_b200.h): argument marshalling only.
+
+Every step of the hot path runs inside the CUDA library; PyTorch is used for device memory
+and streams.  There is no CPU fallback and no import of oracle/: if the shared library is
+missing or no CUDA device is present, calls raise.
+
+Functions mirror the C ABI names: Ax, Atb, row_weights, col_weights, residual, update,
+ossart, sirt, cgls, fdk, fdk_filter, Ax_count.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtigre_b200.so")
+
+AX_SIDDON, AX_INTERP = 0, 1
+ATB_MATCHED, ATB_FDK = 0, 1
+_AX_MODES = {"siddon": 0, "interp": 1, "interpolated": 1, 0: 0, 1: 1}
+_ATB_MODES = {"matched": 0, "fdk": 1, "FDK": 1, 0: 0, 1: 1}
+
+_dp = C.POINTER(C.c_double)
+
+
+class tigre_geo(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_uint32),
+        ("nVoxel", C.c_int32 * 3), ("dVoxel", C.c_double * 3),
+        ("nDetector", C.c_int32 * 2), ("dDetector", C.c_double * 2),
+        ("DSD", C.c_double), ("DSO", C.c_double), ("COR", C.c_double),
+        ("offOrigin", C.c_double * 3), ("offDetector", C.c_double * 2), ("rotDetector", C.c_double * 3),
+        ("DSD_a", _dp), ("DSO_a", _dp), ("COR_a", _dp),
+        ("offOrigin_a", _dp), ("offDetector_a", _dp), ("rotDetector_a", _dp),
+        ("accuracy", C.c_double),
+    ]
+
+
+class TigreError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        msg = _lib().tigre_strerror(code).decode()
+        if code == -5:
+            msg += ": " + _lib().tigre_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} [{code}]")
+
+
+_LIB = None
+EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_row_weights", "tigre_col_weights", "tigre_residual",
+           "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_fdk", "tigre_fdk_filter",
+           "tigre_Ax_count", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_strerror",
+           "tigre_last_cuda_error", "tigre_version"]
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2412_10129_b200.build` "
+                              "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        lib.tigre_strerror.restype = C.c_char_p
+        lib.tigre_last_cuda_error.restype = C.c_char_p
+        lib.tigre_workspace_bytes.restype = C.c_size_t
+        for name in EXPORTS:
+            getattr(lib, name)
+        _LIB = lib
+    return _LIB
+
+
+def _check(code, where):
+    if code != 0:
+        raise TigreError(code, where)
+
+
+class _Geo:
+    """Marshals a workloads.Geometry (or anything with the same attributes) to the C struct and
+    keeps the numpy arrays behind the optional per-angle pointers alive."""
+
+    def __init__(self, geo, nA):
+        g = tigre_geo()
+        g.struct_size = C.sizeof(tigre_geo)
+        g.nVoxel[:] = [int(v) for v in geo.nVoxel]
+        g.dVoxel[:] = [float(v) for v in geo.dVoxel]
+        g.nDetector[:] = [int(v) for v in geo.nDetector]
+        g.dDetector[:] = [float(v) for v in geo.dDetector]
+        g.DSD, g.DSO, g.COR = float(geo.DSD), float(geo.DSO), float(geo.COR)
+        g.offOrigin[:] = [float(v) for v in geo.offOrigin]
+        g.offDetector[:] = [float(v) for v in geo.offDetector]
+        g.rotDetector[:] = [float(v) for v in geo.rotDetector]
+        g.accuracy = float(geo.accuracy)
+        self.keep = []
+        for name, width in (("DSD_a", 1), ("DSO_a", 1), ("COR_a", 1), ("offOrigin_a", 3),
+                            ("offDetector_a", 2), ("rotDetector_a", 3)):
+            a = getattr(geo, name, None)
+            if a is not None:
+                a = np.ascontiguousarray(a, dtype=np.float64).reshape(nA, width)
+                self.keep.append(a)
+                setattr(g, name, a.ctypes.data_as(_dp))
+        self.c = g
+
+    @property
+    def ref(self):
+        return C.byref(self.c)
+
+
+def _angles(angles):
+    a = np.ascontiguousarray(angles, dtype=np.float64)
+    if a.ndim == 1:
+        a = np.stack([a, np.zeros_like(a), np.zeros_like(a)], 1)
+    a = np.ascontiguousarray(a.reshape(-1, 3))
+    return a, a.shape[0]
+
+
+def _stream(t=None):
+    import torch
+    if t is not None and t.is_cuda:
+        return C.c_void_p(torch.cuda.current_stream(t.device).cuda_stream)
+    if torch.cuda.is_available():
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return C.c_void_p(0)
+
+
+def _f32(t, shape=None, name="tensor"):
+    import torch
+    if not isinstance(t, torch.Tensor):
+        raise TypeError(f"{name}: expected a torch.Tensor (device memory), got {type(t)}")
+    if t.dtype != torch.float32 or not t.is_contiguous():
+        raise ValueError(f"{name}: need contiguous float32")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: shape {tuple(t.shape)} != {tuple(shape)}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _new(shape, like=None, device=None):
+    import torch
+    if like is not None:
+        if like.is_cuda:
+            return torch.empty(shape, dtype=torch.float32, device=like.device)
+        return torch.empty(shape, dtype=torch.float32, pin_memory=True)   # chunked path: pinned in, pinned out
+    return torch.empty(shape, dtype=torch.float32, device=device or "cuda")
+
+
+def vol_shape(geo):
+    return (geo.nVoxel[2], geo.nVoxel[1], geo.nVoxel[0])
+
+
+def proj_shape(geo, nA):
+    return (nA, geo.nDetector[1], geo.nDetector[0])
+
+
+# ------------------------------------------------------------------ the projector pair
+def Ax(vol, geo, angles, mode="siddon", out=None):
+    """b = A x.  vol: float32 [nz][ny][nx] CUDA tensor (or pinned host tensor -> chunked path)."""
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    pv = _f32(vol, vol_shape(geo), "vol")
+    if out is None:
+        out = _new(proj_shape(geo, nA), like=vol)
+    po = _f32(out, proj_shape(geo, nA), "out")
+    _check(_lib().tigre_Ax(pv, G.ref, a.ctypes.data_as(_dp), nA, _AX_MODES[mode], po, _stream(vol)), "tigre_Ax")
+    return out
+
+
+def Atb(proj, geo, angles, mode="matched", out=None):
+    """x = A^T b (voxel-driven).  proj: float32 [nA][nv][nu]."""
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    pp = _f32(proj, proj_shape(geo, nA), "proj")
+    if out is None:
+        out = _new(vol_shape(geo), like=proj)
+    po = _f32(out, vol_shape(geo), "out")
+    _check(_lib().tigre_Atb(pp, G.ref, a.ctypes.data_as(_dp), nA, _ATB_MODES[mode], po, _stream(proj)), "tigre_Atb")
+    return out
+
+
+def row_weights(geo, angles, ax_mode="siddon", device="cuda"):
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    W = _new(proj_shape(geo, nA), device=device)
+    _check(_lib().tigre_row_weights(G.ref, a.ctypes.data_as(_dp), nA, _AX_MODES[ax_mode], _f32(W), _stream(W)),
+           "tigre_row_weights")
+    return W
+
+
+def col_weights(geo, angles, atb_mode="matched", device="cuda"):
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    V = _new(vol_shape(geo), device=device)
+    _check(_lib().tigre_col_weights(G.ref, a.ctypes.data_as(_dp), nA, _ATB_MODES[atb_mode], _f32(V), _stream(V)),
+           "tigre_col_weights")
+    return V
+
+
+def residual(b, ax, W=None, return_norm=False):
+    r = _new(tuple(b.shape), like=b)
+    nrm = C.c_double(0.0)
+    _check(_lib().tigre_residual(_f32(b), _f32(ax, b.shape, "Ax"), _f32(W, b.shape, "W") if W is not None else None,
+                                 _f32(r), C.c_size_t(b.numel()), C.byref(nrm) if return_norm else None, _stream(b)),
+           "tigre_residual")
+    return (r, nrm.value) if return_norm else r
+
+
+def update(x, g, V=None, lam=1.0, nonneg=True):
+    """In place: x <- max(0, x + lam * V .* g)."""
+    _check(_lib().tigre_update(_f32(x), _f32(g, x.shape, "g"), _f32(V, x.shape, "V") if V is not None else None,
+                               C.c_float(lam), int(bool(nonneg)), C.c_size_t(x.numel()), _stream(x)), "tigre_update")
+    return x
+
+
+# ------------------------------------------------------------------ drivers
+def ossart(b, geo, angles, subsets, n_iter, lam=1.0, nonneg=True, ax_mode="siddon", atb_mode="matched", x0=None):
+    """OS-SART; `subsets` is a list of view-index lists.  Returns (x, resid_hist)."""
+    import torch
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    idx = np.ascontiguousarray(np.concatenate([np.asarray(s, dtype=np.int32) for s in subsets]))
+    off = np.zeros(len(subsets) + 1, dtype=np.int32)
+    off[1:] = np.cumsum([len(s) for s in subsets])
+    x = torch.zeros(vol_shape(geo), dtype=torch.float32, device=b.device) if x0 is None else x0.clone()
+    hist = np.zeros(max(n_iter, 1), dtype=np.float64)
+    _check(_lib().tigre_ossart(_f32(b, proj_shape(geo, nA), "b"), G.ref, a.ctypes.data_as(_dp), nA,
+                               idx.ctypes.data_as(C.POINTER(C.c_int32)), off.ctypes.data_as(C.POINTER(C.c_int32)),
+                               len(subsets), int(n_iter), C.c_float(lam), int(bool(nonneg)), _AX_MODES[ax_mode],
+                               _ATB_MODES[atb_mode], _f32(x), hist.ctypes.data_as(_dp), _stream(b)), "tigre_ossart")
+    return x, hist[:n_iter]
+
+
+def sirt(b, geo, angles, n_iter, **kw):
+    _, nA = _angles(angles)
+    return ossart(b, geo, angles, [np.arange(nA)], n_iter, **kw)
+
+
+def cgls(b, geo, angles, n_iter, ax_mode="siddon", atb_mode="matched"):
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    x = _new(vol_shape(geo), like=b)
+    hist = np.zeros(max(n_iter, 1), dtype=np.float64)
+    _check(_lib().tigre_cgls(_f32(b, proj_shape(geo, nA), "b"), G.ref, a.ctypes.data_as(_dp), nA, int(n_iter),
+                             _AX_MODES[ax_mode], _ATB_MODES[atb_mode], _f32(x), hist.ctypes.data_as(_dp), _stream(b)),
+           "tigre_cgls")
+    return x, hist[:n_iter]
+
+
+def fdk(b, geo, angles):
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    x = _new(vol_shape(geo), like=b)
+    _check(_lib().tigre_fdk(_f32(b, proj_shape(geo, nA), "b"), G.ref, a.ctypes.data_as(_dp), nA, _f32(x), _stream(b)),
+           "tigre_fdk")
+    return x
+
+
+def fdk_filter(b, geo, angles):
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    q = _new(tuple(b.shape), like=b)
+    _check(_lib().tigre_fdk_filter(_f32(b, proj_shape(geo, nA), "b"), G.ref, a.ctypes.data_as(_dp), nA, _f32(q),
+                                   _stream(b)), "tigre_fdk_filter")
+    return q
+
+
+def Ax_count(geo, angles, mode="siddon", return_counts=False, device="cuda"):
+    """Exact number of ray-samples of one Ax call (the BASELINE metric's unit)."""
+    import torch
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    total = C.c_uint64(0)
+    counts = torch.empty(proj_shape(geo, nA), dtype=torch.int32, device=device) if return_counts else None
+    _check(_lib().tigre_Ax_count(G.ref, a.ctypes.data_as(_dp), nA, _AX_MODES[mode],
+                                 C.c_void_p(counts.data_ptr()) if return_counts else None, C.byref(total),
+                                 _stream(counts)), "tigre_Ax_count")
+    return (total.value, counts) if return_counts else total.value
+
+
+def workspace_bytes(geo, nA, op):
+    G = _Geo(geo, nA)
+    return int(_lib().tigre_workspace_bytes(G.ref, int(nA), int(op)))
+
+
+def set_chunk_budget(nbytes):
+    _check(_lib().tigre_set_chunk_budget(C.c_size_t(int(nbytes))), "tigre_set_chunk_budget")
+
+
+def version():
+    return int(_lib().tigre_version())

@@ -1,0 +1,406 @@
+// api.cu — the C ABI of libtigre_b200 (include/tigre_b200.h): argument checks, per-view table
+// upload, kernel launches and the SIRT/OS-SART, CGLS and FDK drivers (DESIGN.md O-D..O-F).
+// No CPU fallback anywhere: without a device every compute call returns TIGRE_ERR_NO_DEVICE.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <string>
+#include <vector>
+#include "common.cuh"
+
+namespace tg {
+
+static thread_local std::string g_last_cuda_error;
+void set_cuda_error(cudaError_t e, const char* file, int line) {
+    char buf[512];
+    snprintf(buf, sizeof buf, "%s (%s) at %s:%d", cudaGetErrorName(e), cudaGetErrorString(e), file, line);
+    g_last_cuda_error = buf;
+    (void)cudaGetLastError();  // clear the non-sticky error state
+}
+
+int TempBuf::alloc(size_t bytes, cudaStream_t st) {
+    release();
+    s = st;
+    if (bytes == 0) bytes = 16;
+    cudaError_t e = cudaMallocAsync(&p, bytes, st);
+    if (e != cudaSuccess) {
+        p = nullptr;
+        set_cuda_error(e, __FILE__, __LINE__);
+        return TIGRE_ERR_WORKSPACE;
+    }
+    return TIGRE_OK;
+}
+void TempBuf::release() {
+    if (p) cudaFreeAsync(p, s);
+    p = nullptr;
+}
+int upload(TempBuf& buf, const void* host, size_t bytes, cudaStream_t st) {
+    TG_TRY(buf.alloc(bytes, st));
+    // pageable source: the runtime stages the bytes before returning, so `host` may die afterwards
+    TG_CUDA(cudaMemcpyAsync(buf.p, host, bytes, cudaMemcpyHostToDevice, st));
+    return TIGRE_OK;
+}
+
+static int ensure_device() {
+    static std::once_flag once;
+    static int status = TIGRE_OK;
+    std::call_once(once, [] {
+        int n = 0;
+        if (cudaGetDeviceCount(&n) != cudaSuccess || n <= 0) {
+            (void)cudaGetLastError();
+            status = TIGRE_ERR_NO_DEVICE;
+            return;
+        }
+        // keep freed temporaries in the pool instead of returning them to the OS at every sync
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            unsigned long long thr = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+        }
+        (void)cudaGetLastError();
+    });
+    return status;
+}
+
+enum MemKind { MEM_DEVICE, MEM_PINNED, MEM_PAGEABLE };
+static MemKind mem_kind(const void* p) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return MEM_PAGEABLE;
+    }
+    if (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged) return MEM_DEVICE;
+    if (at.type == cudaMemoryTypeHost) return MEM_PINNED;
+    return MEM_PAGEABLE;
+}
+
+// ---------------------------------------------------------------- per-view tables on the device
+struct Tables {
+    std::vector<ViewH> views;
+    Grid g;
+    TempBuf ray, vox;
+    int build_ray(const int32_t* idx, int n, cudaStream_t st) {
+        std::vector<RayView> h(n);
+        for (int i = 0; i < n; ++i) build_ray_view(g, views[idx ? idx[i] : i], h[i]);
+        return upload(ray, h.data(), sizeof(RayView) * n, st);
+    }
+    int build_vox(const int32_t* idx, int n, cudaStream_t st) {
+        std::vector<VoxView> h(n);
+        for (int i = 0; i < n; ++i) TG_TRY(build_vox_view(g, views[idx ? idx[i] : i], h[i]));
+        return upload(vox, h.data(), sizeof(VoxView) * n, st);
+    }
+};
+
+static int prep(const tigre_geo* geo, const double* angles, int nA, Tables& t) {
+    TG_TRY(validate_geo(geo, angles, nA));
+    TG_TRY(ensure_device());
+    t.g = make_grid(geo);
+    resolve_views(geo, angles, nA, t.views);
+    return TIGRE_OK;
+}
+
+static int device_ax(const float* vol, Tables& t, const int32_t* idx, int n, int mode, bool unit, float* proj,
+                     cudaStream_t st) {
+    TG_TRY(t.build_ray(idx, n, st));
+    return launch_ax(vol, t.g, t.ray.as<RayView>(), n, mode, unit, false, proj, nullptr, st);
+}
+static int device_atb(const float* proj, Tables& t, const int32_t* idx, int n, int mode, bool unit, float* vol,
+                      cudaStream_t st) {
+    TG_TRY(t.build_vox(idx, n, st));
+    return launch_atb(proj, t.g, t.vox.as<VoxView>(), n, mode, unit, vol, 0, t.g.nz, false, 0, t.g.nv, st);
+}
+
+}  // namespace tg
+
+using namespace tg;
+
+extern "C" {
+
+int tigre_version(void) { return 100; }
+
+const char* tigre_strerror(int code) {
+    switch (code) {
+        case TIGRE_OK: return "ok";
+        case TIGRE_ERR_ARG: return "invalid argument";
+        case TIGRE_ERR_GEOMETRY: return "invalid geometry (non-positive size/distance, or volume at/behind the source)";
+        case TIGRE_ERR_MEMSPACE: return "data pointer in the wrong memory space (need device, or pinned host for the chunked path)";
+        case TIGRE_ERR_WORKSPACE: return "temporary device allocation failed";
+        case TIGRE_ERR_CUDA: return "CUDA error (see tigre_last_cuda_error)";
+        case TIGRE_ERR_NO_DEVICE: return "no CUDA device (libtigre_b200 has no CPU fallback)";
+    }
+    return "unknown error";
+}
+const char* tigre_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
+
+int tigre_Ax(const float* vol, const tigre_geo* geo, const double* angles, int nA, int mode, float* proj,
+             void* cuda_stream) {
+    if (!vol || !proj) return TIGRE_ERR_ARG;
+    if (mode != TIGRE_AX_SIDDON && mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const MemKind kv = mem_kind(vol), kp = mem_kind(proj);
+    if (kv == MEM_PINNED && kp == MEM_PINNED) return chunked_ax(vol, geo, angles, nA, mode, proj, st);
+    if (kv != MEM_DEVICE || kp != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    return device_ax(vol, t, nullptr, nA, mode, false, proj, st);
+}
+
+int tigre_Atb(const float* proj, const tigre_geo* geo, const double* angles, int nA, int mode, float* vol,
+              void* cuda_stream) {
+    if (!vol || !proj) return TIGRE_ERR_ARG;
+    if (mode != TIGRE_ATB_MATCHED && mode != TIGRE_ATB_FDK) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const MemKind kv = mem_kind(vol), kp = mem_kind(proj);
+    if (kv == MEM_PINNED && kp == MEM_PINNED) return chunked_atb(proj, geo, angles, nA, mode, vol, st);
+    if (kv != MEM_DEVICE || kp != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    return device_atb(proj, t, nullptr, nA, mode, false, vol, st);
+}
+
+int tigre_row_weights(const tigre_geo* geo, const double* angles, int nA, int ax_mode, float* W, void* cuda_stream) {
+    if (!W) return TIGRE_ERR_ARG;
+    if (ax_mode != TIGRE_AX_SIDDON && ax_mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    if (mem_kind(W) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    TG_TRY(device_ax(nullptr, t, nullptr, nA, ax_mode, true, W, st));
+    const double eps = 1e-2 * std::min(t.g.dx, std::min(t.g.dy, t.g.dz));
+    return launch_invert_rows(W, (size_t)nA * t.g.nu * t.g.nv, (float)eps, st);
+}
+
+int tigre_col_weights(const tigre_geo* geo, const double* angles, int nA, int atb_mode, float* V, void* cuda_stream) {
+    if (!V) return TIGRE_ERR_ARG;
+    if (atb_mode != TIGRE_ATB_MATCHED && atb_mode != TIGRE_ATB_FDK) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    if (mem_kind(V) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    TG_TRY(device_atb(nullptr, t, nullptr, nA, atb_mode, true, V, st));
+    return launch_invert_cols(V, (size_t)t.g.nx * t.g.ny * t.g.nz, 1e-6f, st);
+}
+
+int tigre_residual(const float* b, const float* Ax, const float* W, float* r, size_t n, double* nrm2, void* cuda_stream) {
+    if (!b || !Ax || !r) return TIGRE_ERR_ARG;
+    TG_TRY(ensure_device());
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    TempBuf acc;
+    if (nrm2) {
+        TG_TRY(acc.alloc(sizeof(double), st));
+        TG_CUDA(cudaMemsetAsync(acc.p, 0, sizeof(double), st));
+    }
+    TG_TRY(launch_residual(b, nullptr, Ax, W, r, n, 1, nrm2 ? acc.as<double>() : nullptr, st));
+    if (nrm2) {
+        TG_CUDA(cudaMemcpyAsync(nrm2, acc.p, sizeof(double), cudaMemcpyDeviceToHost, st));
+        TG_CUDA(cudaStreamSynchronize(st));
+    }
+    return TIGRE_OK;
+}
+
+int tigre_update(float* x, const float* g, const float* V, float lambda, int nonneg, size_t n, void* cuda_stream) {
+    if (!x || !g) return TIGRE_ERR_ARG;
+    TG_TRY(ensure_device());
+    return launch_update(x, g, V, lambda, nonneg, n, (cudaStream_t)cuda_stream);
+}
+
+int tigre_Ax_count(const tigre_geo* geo, const double* angles, int nA, int mode, uint32_t* counts, uint64_t* total,
+                   void* cuda_stream) {
+    if (mode != TIGRE_AX_SIDDON && mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n = (size_t)nA * t.g.nu * t.g.nv;
+    TempBuf own, tot;
+    uint32_t* c = counts;
+    if (!c) {
+        TG_TRY(own.alloc(n * sizeof(uint32_t), st));
+        c = own.as<uint32_t>();
+    } else if (mem_kind(counts) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    TG_TRY(t.build_ray(nullptr, nA, st));
+    TG_TRY(launch_ax(nullptr, t.g, t.ray.as<RayView>(), nA, mode, false, false, nullptr, c, st));
+    if (total) {
+        TG_TRY(tot.alloc(sizeof(unsigned long long), st));
+        TG_TRY(launch_count_reduce(c, n, tot.as<unsigned long long>(), st));
+        unsigned long long h = 0;
+        TG_CUDA(cudaMemcpyAsync(&h, tot.p, sizeof h, cudaMemcpyDeviceToHost, st));
+        TG_CUDA(cudaStreamSynchronize(st));
+        *total = h;
+    }
+    return TIGRE_OK;
+}
+
+// ---------------------------------------------------------------- OS-SART / SIRT
+int tigre_ossart(const float* b, const tigre_geo* geo, const double* angles, int nA, const int32_t* subset_idx,
+                 const int32_t* subset_off, int nSubsets, int n_iter, float lambda, int nonneg, int ax_mode,
+                 int atb_mode, float* x, double* resid_hist, void* cuda_stream) {
+    if (!b || !x || !subset_idx || !subset_off || nSubsets <= 0 || n_iter < 0) return TIGRE_ERR_ARG;
+    if (ax_mode != TIGRE_AX_SIDDON && ax_mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
+    if (atb_mode != TIGRE_ATB_MATCHED && atb_mode != TIGRE_ATB_FDK) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    if (mem_kind(b) != MEM_DEVICE || mem_kind(x) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int maxs = 0;
+    for (int s = 0; s < nSubsets; ++s) {
+        const int n = subset_off[s + 1] - subset_off[s];
+        if (n <= 0) return TIGRE_ERR_ARG;
+        maxs = std::max(maxs, n);
+        for (int k = subset_off[s]; k < subset_off[s + 1]; ++k)
+            if (subset_idx[k] < 0 || subset_idx[k] >= nA) return TIGRE_ERR_ARG;
+    }
+    const Grid& g = t.g;
+    const size_t per = (size_t)g.nu * g.nv, nvox = (size_t)g.nx * g.ny * g.nz;
+    const int nIdx = subset_off[nSubsets];
+    // Temporaries: W for every view listed (subset-major), V per subset, one subset's Ax/residual, A^T r.
+    TempBuf W, V, Axb, grad, d_idx, d_acc;
+    TG_TRY(W.alloc(sizeof(float) * per * nIdx, st));
+    TG_TRY(V.alloc(sizeof(float) * nvox * nSubsets, st));
+    TG_TRY(Axb.alloc(sizeof(float) * per * maxs, st));
+    TG_TRY(grad.alloc(sizeof(float) * nvox, st));
+    TG_TRY(upload(d_idx, subset_idx, sizeof(int32_t) * nIdx, st));
+    TG_TRY(d_acc.alloc(sizeof(double) * std::max(n_iter, 1), st));
+    TG_CUDA(cudaMemsetAsync(d_acc.p, 0, sizeof(double) * std::max(n_iter, 1), st));
+    // per-subset tables and weights (P13, P16)
+    std::vector<TempBuf> ray(nSubsets), vox(nSubsets);
+    const double epsW = 1e-2 * std::min(g.dx, std::min(g.dy, g.dz));
+    for (int s = 0; s < nSubsets; ++s) {
+        const int32_t* idx = subset_idx + subset_off[s];
+        const int n = subset_off[s + 1] - subset_off[s];
+        std::vector<RayView> hr(n);
+        std::vector<VoxView> hv(n);
+        for (int i = 0; i < n; ++i) {
+            build_ray_view(g, t.views[idx[i]], hr[i]);
+            TG_TRY(build_vox_view(g, t.views[idx[i]], hv[i]));
+        }
+        TG_TRY(upload(ray[s], hr.data(), sizeof(RayView) * n, st));
+        TG_TRY(upload(vox[s], hv.data(), sizeof(VoxView) * n, st));
+        float* Ws = W.as<float>() + per * subset_off[s];
+        float* Vs = V.as<float>() + nvox * s;
+        TG_TRY(launch_ax(nullptr, g, ray[s].as<RayView>(), n, ax_mode, true, false, Ws, nullptr, st));
+        TG_TRY(launch_invert_rows(Ws, per * n, (float)epsW, st));
+        TG_TRY(launch_atb(nullptr, g, vox[s].as<VoxView>(), n, atb_mode, true, Vs, 0, g.nz, false, 0, g.nv, st));
+        TG_TRY(launch_invert_cols(Vs, nvox, 1e-6f, st));
+    }
+    for (int it = 0; it < n_iter; ++it) {
+        for (int s = 0; s < nSubsets; ++s) {
+            const int n = subset_off[s + 1] - subset_off[s];
+            float* Ws = W.as<float>() + per * subset_off[s];
+            float* Vs = V.as<float>() + nvox * s;
+            float* A = Axb.as<float>();
+            TG_TRY(launch_ax(x, g, ray[s].as<RayView>(), n, ax_mode, false, false, A, nullptr, st));
+            // r = W_s .* (b_s - A_s x), in place over A; b gathered through the subset's view list,
+            // W stored subset-major so it is read with the local view index
+            TG_TRY(launch_residual(b, d_idx.as<int32_t>() + subset_off[s], A, Ws, A, per, n, d_acc.as<double>() + it, st));
+            TG_TRY(launch_atb(A, g, vox[s].as<VoxView>(), n, atb_mode, false, grad.as<float>(), 0, g.nz, false, 0, g.nv, st));
+            TG_TRY(launch_update(x, grad.as<float>(), Vs, lambda, nonneg, nvox, st));
+        }
+    }
+    if (resid_hist && n_iter > 0) {
+        std::vector<double> h(n_iter);
+        TG_CUDA(cudaMemcpyAsync(h.data(), d_acc.p, sizeof(double) * n_iter, cudaMemcpyDeviceToHost, st));
+        TG_CUDA(cudaStreamSynchronize(st));
+        for (int it = 0; it < n_iter; ++it) resid_hist[it] = std::sqrt(h[it]);
+    }
+    return TIGRE_OK;
+}
+
+
+// ---------------------------------------------------------------- CGLS (textbook recurrences, O-F)
+int tigre_cgls(const float* b, const tigre_geo* geo, const double* angles, int nA, int n_iter, int ax_mode,
+               int atb_mode, float* x, double* resid_hist, void* cuda_stream) {
+    if (!b || !x || n_iter < 0) return TIGRE_ERR_ARG;
+    if (ax_mode != TIGRE_AX_SIDDON && ax_mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
+    if (atb_mode != TIGRE_ATB_MATCHED && atb_mode != TIGRE_ATB_FDK) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    if (mem_kind(b) != MEM_DEVICE || mem_kind(x) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const Grid& g = t.g;
+    const size_t np = (size_t)nA * g.nu * g.nv, nvox = (size_t)g.nx * g.ny * g.nz;
+    TempBuf r, q, s, p, sc;
+    TG_TRY(r.alloc(sizeof(float) * np, st));
+    TG_TRY(q.alloc(sizeof(float) * np, st));
+    TG_TRY(s.alloc(sizeof(float) * nvox, st));
+    TG_TRY(p.alloc(sizeof(float) * nvox, st));
+    // device scalars: [0]=gamma [1]=gamma_new [2]=||q||^2 [3+it]=||r||^2 history
+    TG_TRY(sc.alloc(sizeof(double) * (3 + std::max(n_iter, 1)), st));
+    double* d = sc.as<double>();
+    TG_TRY(t.build_ray(nullptr, nA, st));
+    TG_TRY(t.build_vox(nullptr, nA, st));
+    const RayView* rv = t.ray.as<RayView>();
+    const VoxView* vv = t.vox.as<VoxView>();
+    TG_CUDA(cudaMemsetAsync(x, 0, sizeof(float) * nvox, st));
+    TG_CUDA(cudaMemcpyAsync(r.p, b, sizeof(float) * np, cudaMemcpyDeviceToDevice, st));              // r = b - A 0
+    TG_TRY(launch_atb(r.as<float>(), g, vv, nA, atb_mode, false, s.as<float>(), 0, g.nz, false, 0, g.nv, st));
+    TG_CUDA(cudaMemcpyAsync(p.p, s.p, sizeof(float) * nvox, cudaMemcpyDeviceToDevice, st));          // p = s
+    TG_TRY(launch_dot(s.as<float>(), s.as<float>(), nvox, d + 0, st));                               // gamma
+    for (int it = 0; it < n_iter; ++it) {
+        TG_TRY(launch_ax(p.as<float>(), g, rv, nA, ax_mode, false, false, q.as<float>(), nullptr, st));   // q = A p
+        TG_TRY(launch_dot(q.as<float>(), q.as<float>(), np, d + 2, st));
+        TG_TRY(launch_axpy(x, p.as<float>(), d + 0, d + 2, 1.f, nvox, st));                          // x += alpha p
+        TG_TRY(launch_axpy(r.as<float>(), q.as<float>(), d + 0, d + 2, -1.f, np, st));               // r -= alpha q
+        TG_TRY(launch_atb(r.as<float>(), g, vv, nA, atb_mode, false, s.as<float>(), 0, g.nz, false, 0, g.nv, st));
+        TG_TRY(launch_dot(s.as<float>(), s.as<float>(), nvox, d + 1, st));                           // gamma'
+        TG_TRY(launch_xpby(p.as<float>(), s.as<float>(), d + 1, d + 0, nvox, st));                   // p = s + beta p
+        TG_CUDA(cudaMemcpyAsync(d + 0, d + 1, sizeof(double), cudaMemcpyDeviceToDevice, st));        // gamma = gamma'
+        TG_TRY(launch_dot(r.as<float>(), r.as<float>(), np, d + 3 + it, st));
+    }
+    if (resid_hist && n_iter > 0) {
+        std::vector<double> h(n_iter);
+        TG_CUDA(cudaMemcpyAsync(h.data(), d + 3, sizeof(double) * n_iter, cudaMemcpyDeviceToHost, st));
+        TG_CUDA(cudaStreamSynchronize(st));
+        for (int it = 0; it < n_iter; ++it) resid_hist[it] = std::sqrt(h[it]);
+    }
+    return TIGRE_OK;
+}
+
+// ---------------------------------------------------------------- FDK (O-D)
+static int fdk_filter_impl(const float* b, Tables& t, int nA, float* q, cudaStream_t st) {
+    std::vector<double> dd(2 * (size_t)nA);
+    for (int a = 0; a < nA; ++a) dd[a] = t.views[a].DSD, dd[nA + a] = t.views[a].DSO;
+    TempBuf tb;
+    TG_TRY(upload(tb, dd.data(), sizeof(double) * dd.size(), st));
+    return launch_fdk_filter(b, t.g, tb.as<double>(), tb.as<double>() + nA, nA, q, st);
+}
+int tigre_fdk_filter(const float* b, const tigre_geo* geo, const double* angles, int nA, float* q, void* cuda_stream) {
+    if (!b || !q) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    if (mem_kind(b) != MEM_DEVICE || mem_kind(q) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    return fdk_filter_impl(b, t, nA, q, (cudaStream_t)cuda_stream);
+}
+int tigre_fdk(const float* b, const tigre_geo* geo, const double* angles, int nA, float* x, void* cuda_stream) {
+    if (!b || !x) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    if (mem_kind(b) != MEM_DEVICE || mem_kind(x) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const Grid& g = t.g;
+    TempBuf q;
+    TG_TRY(q.alloc(sizeof(float) * (size_t)nA * g.nu * g.nv, st));
+    TG_TRY(fdk_filter_impl(b, t, nA, q.as<float>(), st));
+    TG_TRY(device_atb(q.as<float>(), t, nullptr, nA, TIGRE_ATB_FDK, false, x, st));
+    return launch_scale(x, (float)(M_PI / (double)nA), (size_t)g.nx * g.ny * g.nz, st);
+}
+
+size_t tigre_workspace_bytes(const tigre_geo* geo, int nA, int op) {
+    if (!geo || nA <= 0) return 0;
+    const size_t per = (size_t)geo->nDetector[0] * geo->nDetector[1] * sizeof(float);
+    const size_t vol = (size_t)geo->nVoxel[0] * geo->nVoxel[1] * geo->nVoxel[2] * sizeof(float);
+    const size_t tab = (size_t)nA * (sizeof(RayView) + sizeof(VoxView));
+    switch (op) {
+        case TIGRE_OP_AX:
+        case TIGRE_OP_ATB: return tab;
+        case TIGRE_OP_OSSART: return tab + per * nA * 2 + vol * 2;   // + vol per subset for V (caller adds nSubsets-1)
+        case TIGRE_OP_CGLS: return tab + per * nA * 2 + vol * 2;
+        case TIGRE_OP_FDK: return tab + per * nA;
+    }
+    return 0;
+}
+
+}  // extern "C"

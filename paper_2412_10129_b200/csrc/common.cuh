@@ -1,0 +1,120 @@
+// common.cuh — shared declarations of libtigre_b200 (CUDA path only; nothing here is used by,
+// or taken from, oracle/).  Geometry follows PAPER.md:543-566 (App. B Table B1) and §2.4
+// (lines 179-197) under the readings P1-P6 listed in DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <vector>
+#include "../../include/tigre_b200.h"
+
+namespace tg {
+
+// ---------------------------------------------------------------- errors
+void set_cuda_error(cudaError_t e, const char* file, int line);
+#define TG_CUDA(expr)                                                     \
+    do {                                                                  \
+        cudaError_t _e = (expr);                                          \
+        if (_e != cudaSuccess) {                                          \
+            tg::set_cuda_error(_e, __FILE__, __LINE__);                   \
+            return (_e == cudaErrorMemoryAllocation) ? TIGRE_ERR_WORKSPACE : TIGRE_ERR_CUDA; \
+        }                                                                 \
+    } while (0)
+#define TG_TRY(expr)                 \
+    do {                             \
+        int _s = (expr);             \
+        if (_s != TIGRE_OK) return _s; \
+    } while (0)
+
+// ---------------------------------------------------------------- host geometry (fp64)
+struct ViewH {  // one projection's resolved parameters (everything but sizes per view)
+    double DSD, DSO, COR;
+    double offO[3], offD[2], rotD[3], ang[3];
+};
+
+// Ray-driven per-view table, in VOXEL-INDEX coordinates xi = (X - volume_min)/dVoxel, so voxel
+// (ix,iy,iz) is the cube [ix,ix+1) x [iy,iy+1) x [iz,iz+1).  fp64: per-ray set-up is done in
+// double on the device (about 1/600 of the work of a ray).
+struct RayView {
+    double S[3];    // source
+    double P0[3];   // centre of pixel (0,0)
+    double dU[3];   // step per pixel along u
+    double dV[3];   // step per pixel along v
+};
+
+// Voxel-driven per-view table (fp32, built in fp64).  With c = centred voxel index
+// (ix-(nx-1)/2, iy-(ny-1)/2, iz-(nz-1)/2):
+//   W  = rowW.c + rowW[3]   (normalised detector-normal depth, t = 1/W is the magnification)
+//   fu - nu/2 = (rowU.c + rowU[3]) / W ,  fv - nv/2 likewise   (integer shifts: floor() commutes)
+//   G  = rowG.c + rowG[3]   = (DSO - X'_x)/DSO   (FDK distance weight = 1/G^2)
+//   matched weight = km * t^2 * sqrt(sx2 + du^2*(fuh-fus)^2 + dv^2*(fvh-fvs)^2), fuh = fu - nu/2
+struct alignas(16) VoxView {
+    float rowU[4], rowV[4], rowW[4], rowG[4];
+    float km, sx2, fus, fvs;
+};
+
+struct Grid {
+    int nx, ny, nz, nu, nv;
+    double dx, dy, dz, du, dv, accuracy;
+};
+
+int validate_geo(const tigre_geo* geo, const double* angles, int nA);
+Grid make_grid(const tigre_geo* geo);
+void resolve_views(const tigre_geo* geo, const double* angles, int nA, std::vector<ViewH>& out);
+void build_ray_view(const Grid& g, const ViewH& v, RayView& r);
+// returns TIGRE_ERR_GEOMETRY if a corner of the (z-restricted) volume is at/behind the source
+int build_vox_view(const Grid& g, const ViewH& v, VoxView& o);
+
+// ---------------------------------------------------------------- stream-ordered temporaries
+struct TempBuf {  // RAII: cudaMallocAsync / cudaFreeAsync on one stream
+    void* p = nullptr;
+    cudaStream_t s = nullptr;
+    TempBuf() {}
+    TempBuf(const TempBuf&) = delete;
+    TempBuf& operator=(const TempBuf&) = delete;
+    ~TempBuf() { release(); }
+    int alloc(size_t bytes, cudaStream_t st);
+    void release();
+    template <class T> T* as() { return reinterpret_cast<T*>(p); }
+};
+// copy a small host table to a fresh device buffer on the stream (host data is staged before return)
+int upload(TempBuf& buf, const void* host, size_t bytes, cudaStream_t st);
+
+// ---------------------------------------------------------------- kernel launchers (device pointers)
+// forward projection of nViews views given their RayView table (device), out contiguous [nViews][nv][nu]
+//   unit_vol: treat the volume as all ones (row sums A 1), vol may be NULL
+//   count_out: if non-NULL, write per-ray sample counts instead of projecting (measurement helper)
+//   accumulate: proj += instead of proj = (partial projections of a z-slab, chunked path)
+int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nViews, int mode, bool unit_vol,
+              bool accumulate, float* proj, uint32_t* count_out, cudaStream_t st);
+// backprojection of nViews views given their VoxView table (device) into z-slices [z0, z0+nzs) of a
+// volume whose full height is g.nz; vol points at slice z0.  accumulate: vol += instead of vol =.
+//   unit_proj: treat projections as all ones (column sums A^T 1), proj may be NULL
+//   row0/nrows: the projection buffer holds detector rows [row0,row0+nrows) only (chunked path)
+int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nViews, int mode, bool unit_proj,
+               float* vol, int z0, int nzs, bool accumulate, int row0, int nrows, cudaStream_t st);
+
+// elementwise
+int launch_residual(const float* b, const int32_t* view_idx, const float* Ax, const float* W, float* r,
+                    size_t per_view, int nViews, double* d_nrm2_accum, cudaStream_t st);
+int launch_update(float* x, const float* g, const float* V, float lambda, int nonneg, size_t n, cudaStream_t st);
+int launch_invert_rows(float* w, size_t n, float eps, cudaStream_t st);                 // w = w>eps ? 1/w : 0
+int launch_invert_cols(float* v, size_t n, float rel_eps, cudaStream_t st);             // eps = rel_eps*max(v)
+int launch_dot(const float* a, const float* b, size_t n, double* d_out, cudaStream_t st);   // *d_out = sum a*b
+int launch_axpy(float* y, const float* x, const double* d_num, const double* d_den, float sign, size_t n,
+                cudaStream_t st);                                                       // y += sign*(num/den)*x
+int launch_xpby(float* p, const float* s, const double* d_num, const double* d_den, size_t n,
+                cudaStream_t st);                                                       // p = s + (num/den)*p
+int launch_scale(float* x, float a, size_t n, cudaStream_t st);
+int launch_fdk_filter(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, int nViews,
+                      float* q, cudaStream_t st);
+int launch_count_reduce(const uint32_t* c, size_t n, unsigned long long* d_total, cudaStream_t st);
+
+// chunked (pinned host) path
+int chunked_ax(const float* h_vol, const tigre_geo* geo, const double* angles, int nA, int mode, float* h_proj,
+               cudaStream_t st);
+int chunked_atb(const float* h_proj, const tigre_geo* geo, const double* angles, int nA, int mode, float* h_vol,
+                cudaStream_t st);
+size_t chunk_budget();
+
+}  // namespace tg

@@ -1,0 +1,266 @@
+// elementwise.cu — the HBM-bound half of the Kaczmarz family (eq. 6 at 135):
+// residual r = W.*(b - Ax), update x = max(0, x + lambda V.*g), weight inversion, the CGLS
+// vector recurrences and the FDK pre-filter (DESIGN.md O-D).
+// Grid-stride kernels, float4 where alignment allows, grids sized as a multiple of the SM count.
+// Reductions: fp32 products accumulated in fp64 per thread, block tree, one fp64 atomic per block.
+#include <cmath>
+#include "common.cuh"
+
+namespace tg {
+
+static int ew_blocks(size_t n, int per_thread = 4) {
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    size_t want = (n + (size_t)256 * per_thread - 1) / ((size_t)256 * per_thread);
+    size_t cap = (size_t)sms * 8;
+    if (want < 1) want = 1;
+    return (int)(want < cap ? want : cap);
+}
+
+__device__ __forceinline__ double block_sum(double v) {
+    __shared__ double sh[32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) sh[w] = v;
+    __syncthreads();
+    v = (threadIdx.x < (blockDim.x >> 5)) ? sh[threadIdx.x] : 0.0;
+    if (w == 0) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    }
+    return v;
+}
+
+// r[j][i] = W[j][i] * (b[view_idx[j]][i] - Ax[j][i]);  nrm2 += sum (b - Ax)^2
+__global__ void __launch_bounds__(256)
+residual_kernel(const float* __restrict__ b, const int32_t* __restrict__ view_idx, const float* __restrict__ Ax,
+                const float* __restrict__ W, float* __restrict__ r, size_t per_view, int nViews,
+                double* __restrict__ nrm2) {
+    const size_t n4 = per_view >> 2;  // per_view % 4 == 0 guaranteed by the launcher (else scalar path)
+    double s = 0.0;
+    const size_t total = n4 * nViews;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int j = (int)(i / n4);
+        const size_t k = i - (size_t)j * n4;
+        const size_t src = (size_t)(view_idx ? view_idx[j] : j) * n4 + k;
+        const float4 bb = __ldg(reinterpret_cast<const float4*>(b) + src);
+        const float4 aa = __ldg(reinterpret_cast<const float4*>(Ax) + i);
+        float4 d = make_float4(bb.x - aa.x, bb.y - aa.y, bb.z - aa.z, bb.w - aa.w);
+        s += (double)d.x * d.x + (double)d.y * d.y + (double)d.z * d.z + (double)d.w * d.w;
+        if (W) {   // W is laid out like Ax / r (view-list order)
+            const float4 ww = __ldg(reinterpret_cast<const float4*>(W) + i);
+            d.x *= ww.x, d.y *= ww.y, d.z *= ww.z, d.w *= ww.w;
+        }
+        reinterpret_cast<float4*>(r)[i] = d;
+    }
+    if (nrm2) {
+        s = block_sum(s);
+        if (threadIdx.x == 0) atomicAdd(nrm2, s);
+    }
+}
+__global__ void __launch_bounds__(256)
+residual_kernel_scalar(const float* __restrict__ b, const int32_t* __restrict__ view_idx, const float* __restrict__ Ax,
+                       const float* __restrict__ W, float* __restrict__ r, size_t per_view, int nViews,
+                       double* __restrict__ nrm2) {
+    double s = 0.0;
+    const size_t total = per_view * nViews;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int j = (int)(i / per_view);
+        const size_t src = (size_t)(view_idx ? view_idx[j] : j) * per_view + (i - (size_t)j * per_view);
+        float d = b[src] - Ax[i];
+        s += (double)d * d;
+        if (W) d *= W[i];
+        r[i] = d;
+    }
+    if (nrm2) {
+        s = block_sum(s);
+        if (threadIdx.x == 0) atomicAdd(nrm2, s);
+    }
+}
+
+int launch_residual(const float* b, const int32_t* view_idx, const float* Ax, const float* W, float* r,
+                    size_t per_view, int nViews, double* d_nrm2, cudaStream_t st) {
+    const size_t total = per_view * nViews;
+    if (total == 0) return TIGRE_OK;
+    const bool al = ((per_view & 3) == 0) && ((((uintptr_t)b | (uintptr_t)Ax | (uintptr_t)r | (uintptr_t)W) & 15) == 0);
+    if (al) residual_kernel<<<ew_blocks(total / 4), 256, 0, st>>>(b, view_idx, Ax, W, r, per_view, nViews, d_nrm2);
+    else residual_kernel_scalar<<<ew_blocks(total), 256, 0, st>>>(b, view_idx, Ax, W, r, per_view, nViews, d_nrm2);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+
+__global__ void __launch_bounds__(256)
+update_kernel(float* __restrict__ x, const float* __restrict__ g, const float* __restrict__ V, float lambda, int nonneg,
+              size_t n, int vec) {
+    if (vec) {
+        const size_t n4 = n >> 2;
+        for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
+            float4 xx = reinterpret_cast<float4*>(x)[i];
+            const float4 gg = __ldg(reinterpret_cast<const float4*>(g) + i);
+            float4 vv = make_float4(1.f, 1.f, 1.f, 1.f);
+            if (V) vv = __ldg(reinterpret_cast<const float4*>(V) + i);
+            xx.x = fmaf(lambda * vv.x, gg.x, xx.x), xx.y = fmaf(lambda * vv.y, gg.y, xx.y);
+            xx.z = fmaf(lambda * vv.z, gg.z, xx.z), xx.w = fmaf(lambda * vv.w, gg.w, xx.w);
+            if (nonneg) xx.x = fmaxf(xx.x, 0.f), xx.y = fmaxf(xx.y, 0.f), xx.z = fmaxf(xx.z, 0.f), xx.w = fmaxf(xx.w, 0.f);
+            reinterpret_cast<float4*>(x)[i] = xx;
+        }
+        // tail
+        for (size_t i = (n4 << 2) + blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+            float xx = fmaf(lambda * (V ? V[i] : 1.f), g[i], x[i]);
+            x[i] = nonneg ? fmaxf(xx, 0.f) : xx;
+        }
+    } else {
+        for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+            float xx = fmaf(lambda * (V ? V[i] : 1.f), g[i], x[i]);
+            x[i] = nonneg ? fmaxf(xx, 0.f) : xx;
+        }
+    }
+}
+int launch_update(float* x, const float* g, const float* V, float lambda, int nonneg, size_t n, cudaStream_t st) {
+    if (n == 0) return TIGRE_OK;
+    const int vec = ((((uintptr_t)x | (uintptr_t)g | (uintptr_t)V) & 15) == 0) ? 1 : 0;
+    update_kernel<<<ew_blocks(n / 4 + 1), 256, 0, st>>>(x, g, V, lambda, nonneg, n, vec);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+
+__global__ void __launch_bounds__(256) invert_kernel(float* __restrict__ w, size_t n, float eps, const float* __restrict__ d_max, float rel) {
+    const float e = d_max ? rel * (*d_max) : eps;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const float v = w[i];
+        w[i] = v > e ? 1.0f / v : 0.f;
+    }
+}
+__global__ void __launch_bounds__(256) max_kernel(const float* __restrict__ v, size_t n, float* __restrict__ out) {
+    float m = 0.f;   // column sums are non-negative
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) m = fmaxf(m, v[i]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_down_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<int*>(out), __float_as_int(m));   // valid for m >= 0
+}
+int launch_invert_rows(float* w, size_t n, float eps, cudaStream_t st) {
+    if (n == 0) return TIGRE_OK;
+    invert_kernel<<<ew_blocks(n), 256, 0, st>>>(w, n, eps, nullptr, 0.f);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+int launch_invert_cols(float* v, size_t n, float rel_eps, cudaStream_t st) {
+    if (n == 0) return TIGRE_OK;
+    TempBuf mx;
+    TG_TRY(mx.alloc(sizeof(float), st));
+    TG_CUDA(cudaMemsetAsync(mx.p, 0, sizeof(float), st));
+    max_kernel<<<ew_blocks(n), 256, 0, st>>>(v, n, mx.as<float>());
+    invert_kernel<<<ew_blocks(n), 256, 0, st>>>(v, n, 0.f, mx.as<float>(), rel_eps);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+
+__global__ void __launch_bounds__(256) dot_kernel(const float* __restrict__ a, const float* __restrict__ b, size_t n, double* __restrict__ out) {
+    double s = 0.0;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        s += (double)a[i] * (double)b[i];
+    s = block_sum(s);
+    if (threadIdx.x == 0) atomicAdd(out, s);
+}
+int launch_dot(const float* a, const float* b, size_t n, double* d_out, cudaStream_t st) {
+    TG_CUDA(cudaMemsetAsync(d_out, 0, sizeof(double), st));
+    if (n == 0) return TIGRE_OK;
+    dot_kernel<<<ew_blocks(n), 256, 0, st>>>(a, b, n, d_out);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+__global__ void __launch_bounds__(256) axpy_kernel(float* __restrict__ y, const float* __restrict__ x, const double* num, const double* den, float sign, size_t n) {
+    const float a = sign * (float)(*num / *den);
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) y[i] = fmaf(a, x[i], y[i]);
+}
+int launch_axpy(float* y, const float* x, const double* d_num, const double* d_den, float sign, size_t n, cudaStream_t st) {
+    if (n == 0) return TIGRE_OK;
+    axpy_kernel<<<ew_blocks(n), 256, 0, st>>>(y, x, d_num, d_den, sign, n);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+__global__ void __launch_bounds__(256) xpby_kernel(float* __restrict__ p, const float* __restrict__ s, const double* num, const double* den, size_t n) {
+    const float bta = (float)(*num / *den);
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = fmaf(bta, p[i], s[i]);
+}
+int launch_xpby(float* p, const float* s, const double* d_num, const double* d_den, size_t n, cudaStream_t st) {
+    if (n == 0) return TIGRE_OK;
+    xpby_kernel<<<ew_blocks(n), 256, 0, st>>>(p, s, d_num, d_den, n);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+__global__ void __launch_bounds__(256) scale_kernel(float* __restrict__ x, float a, size_t n) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) x[i] *= a;
+}
+int launch_scale(float* x, float a, size_t n, cudaStream_t st) {
+    if (n == 0) return TIGRE_OK;
+    scale_kernel<<<ew_blocks(n), 256, 0, st>>>(x, a, n);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+
+__global__ void __launch_bounds__(256) count_reduce_kernel(const uint32_t* __restrict__ c, size_t n, unsigned long long* __restrict__ out) {
+    unsigned long long s = 0;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) s += c[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) atomicAdd(out, s);
+}
+int launch_count_reduce(const uint32_t* c, size_t n, unsigned long long* d_total, cudaStream_t st) {
+    TG_CUDA(cudaMemsetAsync(d_total, 0, sizeof(unsigned long long), st));
+    if (n == 0) return TIGRE_OK;
+    count_reduce_kernel<<<ew_blocks(n), 256, 0, st>>>(c, n, d_total);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+
+// ---------------------------------------------------------------- FDK pre-filter (reading P12)
+// One CTA per detector row: the cosine-weighted row is staged in shared memory, then each thread
+// forms q[iu] = tau * ( row[iu] h[0] + sum_{odd n} row[iu-n] h[n] ),  h[0] = 1/(4 tau^2),
+// h[n] = -1/(pi n tau)^2 (n odd), tau = du*DSO/DSD: a direct linear convolution with zero padding
+// (no FFT, so no circular wrap).  The tap table 1/n^2 is built once per CTA in shared memory.
+__global__ void __launch_bounds__(256)
+fdk_filter_kernel(const float* __restrict__ b, int nu, int nv, float du, float dv, const double* __restrict__ dsd_a,
+                  const double* __restrict__ dso_a, float* __restrict__ q) {
+    extern __shared__ float sm[];
+    float* row = sm;            // [nu]
+    float* tap = sm + nu;       // [nu]  tap[n] = 1/n^2 for odd n, 0 for even n
+    const int iv = blockIdx.x, ia = blockIdx.y;
+    const float DSD = (float)dsd_a[ia], DSO = (float)dso_a[ia];
+    const float tau = du * DSO / DSD;
+    const float v = ((float)iv + 0.5f) * dv - 0.5f * (float)nv * dv;
+    const size_t base = ((size_t)ia * nv + iv) * nu;
+    for (int iu = threadIdx.x; iu < nu; iu += blockDim.x) {
+        const float u = ((float)iu + 0.5f) * du - 0.5f * (float)nu * du;
+        row[iu] = __ldg(b + base + iu) * DSD * rsqrtf(DSD * DSD + u * u + v * v);
+        tap[iu] = (iu & 1) ? 1.0f / ((float)iu * (float)iu) : 0.f;
+    }
+    __syncthreads();
+    const float c0 = 1.0f / (4.0f * tau), c1 = -1.0f / (9.8696044010893586f * tau);   // tau*h[0], tau*h[n]*n^2
+    for (int iu = threadIdx.x; iu < nu; iu += blockDim.x) {
+        float s = 0.f;
+        // odd offsets only: n = 1,3,5,... on both sides
+        for (int n = 1; n < nu; n += 2) {
+            const int l = iu - n, r = iu + n;
+            float t = 0.f;
+            if (l >= 0) t += row[l];
+            if (r < nu) t += row[r];
+            s = fmaf(t, tap[n], s);
+        }
+        q[base + iu] = fmaf(c1, s, c0 * row[iu]);
+    }
+}
+int launch_fdk_filter(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, int nViews,
+                      float* q, cudaStream_t st) {
+    const size_t smem = 2 * (size_t)g.nu * sizeof(float);
+    if (smem > 200 * 1024) return TIGRE_ERR_ARG;
+    if (smem > 48 * 1024) TG_CUDA(cudaFuncSetAttribute(fdk_filter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    dim3 grid(g.nv, nViews);
+    fdk_filter_kernel<<<grid, 256, smem, st>>>(b, g.nu, g.nv, (float)g.du, (float)g.dv, d_dsd, d_dso, q);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+
+}  // namespace tg

@@ -1,0 +1,275 @@
+"""GPU parity: libtigre_b200 (through the C ABI binding) against the fp64 oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json north_star's:
+  rel-L2 <= 1e-5  Siddon Ax, matched A^T b        rel-L2 <= 1e-4  interpolated Ax, FDK A^T b
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from tests import helpers as H
+from workloads import Geometry, circular_angles, make_config, phantom_for
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def tg():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2412_10129_b200 as m
+    m.version()          # fails loudly if the .so is missing
+    return m
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def host(t):
+    return t.detach().cpu().numpy().astype(np.float64)
+
+
+def odd_geometry(nA=5, seed=11, n=(37, 29, 23), det=(45, 31)):
+    rng = np.random.default_rng(seed)
+    geo = Geometry(nVoxel=n, dVoxel=(1.0, 1.3, 0.8), nDetector=det, dDetector=(2.1, 2.6),
+                   DSD=400.0, DSO=250.0, COR=0.7, offOrigin=(0.4, -0.6, 0.3), offDetector=(1.1, -0.9),
+                   rotDetector=(0.05, -0.04, 0.08))
+    angles = np.stack([rng.uniform(0, 2 * np.pi, nA), rng.uniform(-0.4, 0.4, nA), rng.uniform(-0.5, 0.5, nA)], 1)
+    geo.offOrigin_a = np.asarray(geo.offOrigin) + 0.2 * rng.standard_normal((nA, 3))
+    geo.rotDetector_a = np.asarray(geo.rotDetector) + 0.03 * rng.standard_normal((nA, 3))
+    geo.DSD_a = geo.DSD + rng.uniform(-3, 3, nA)
+    return geo, angles
+
+
+@pytest.fixture(scope="module")
+def c1():
+    geo, ang, rec = make_config("C1")
+    vol = phantom_for(rec, geo)
+    return geo, ang, vol
+
+
+# ------------------------------------------------------------------ Ax
+def test_c1_siddon_ax(tg, c1):
+    geo, ang, vol = c1
+    ref = orc.ax(vol, geo, ang, orc.SIDDON)
+    got = host(tg.Ax(dev(vol), geo, ang, "siddon"))
+    assert H.rel_l2(got, ref) <= 1e-5
+    assert np.array_equal(got == 0, ref == 0)          # same rays miss the volume
+
+
+def test_siddon_random_volume_all_octants(tg):
+    # uniform-random voxels (worst case for fp32 split positions), 16 views around the circle so
+    # every dominant-axis / direction-sign combination occurs, ragged sizes
+    geo = Geometry(nVoxel=(70, 61, 53), dVoxel=(1.0, 1.0, 1.0), nDetector=(101, 67), dDetector=(1.5, 1.5),
+                   DSD=600.0, DSO=380.0)
+    ang = circular_angles(16, start=0.05)
+    vol = np.random.default_rng(0).random(geo.vol_shape, dtype=np.float32)
+    ref = orc.ax(vol, geo, ang, orc.SIDDON)
+    got = host(tg.Ax(dev(vol), geo, ang, "siddon"))
+    assert H.rel_l2(got, ref) <= 1e-5
+
+
+def test_siddon_general_geometry(tg):
+    geo, ang = odd_geometry()
+    vol = np.random.default_rng(1).random(geo.vol_shape, dtype=np.float32)
+    ref = orc.ax(vol, geo, ang, orc.SIDDON)
+    got = host(tg.Ax(dev(vol), geo, ang, "siddon"))
+    assert H.rel_l2(got, ref) <= 1e-5
+
+
+def test_siddon_z_dominant_rays_and_source_inside(tg):
+    # gantry tilted by ~80 degrees: rays run mostly along z; and a short DSO puts the source inside
+    geo = Geometry(nVoxel=(24, 24, 24), dVoxel=(1, 1, 1), nDetector=(20, 20), dDetector=(1.0, 1.0), DSD=60.0, DSO=40.0)
+    ang = np.array([[0.3, 1.4, 0.2], [2.0, -1.45, 0.0]])
+    vol = np.random.default_rng(2).random(geo.vol_shape, dtype=np.float32)
+    assert H.rel_l2(host(tg.Ax(dev(vol), geo, ang, "siddon")), orc.ax(vol, geo, ang)) <= 1e-5
+    geo2 = geo.copy(DSO=6.0, DSD=14.0)                 # source and detector inside the volume (P7)
+    assert H.rel_l2(host(tg.Ax(dev(vol), geo2, circular_angles(3, start=0.2), "siddon")),
+                    orc.ax(vol, geo2, circular_angles(3, start=0.2))) <= 1e-5
+
+
+def test_interp_ax_scaled_c2(tg):
+    geo, ang, rec = make_config("C2", scale=4, n_angles=24)
+    vol = phantom_for(rec, geo)
+    ref = orc.ax(vol, geo, ang, orc.INTERP)
+    got = host(tg.Ax(dev(vol), geo, ang, "interp"))
+    assert H.rel_l2(got, ref) <= 1e-4
+
+
+def test_interp_general_geometry_random_volume(tg):
+    geo, ang = odd_geometry()
+    vol = np.random.default_rng(3).random(geo.vol_shape, dtype=np.float32)
+    ref = orc.ax(vol, geo, ang, orc.INTERP)
+    got = host(tg.Ax(dev(vol), geo, ang, "interp"))
+    assert H.rel_l2(got, ref) <= 1e-4
+
+
+def test_ax_counts_match_oracle_segments(tg):
+    geo, ang = odd_geometry()
+    _, info = orc.ax(np.ones(geo.vol_shape, dtype=np.float32), geo, ang, orc.SIDDON, info=True)
+    total, counts = tg.Ax_count(geo, ang, "siddon", return_counts=True)
+    c = counts.cpu().numpy().astype(np.int64)
+    assert total == int(c.sum())
+    # identical except on knife-edge rays (a crossing pair closer than the oracle resolves, P19)
+    assert np.mean(c != info["nseg"]) < 2e-3
+    assert np.max(np.abs(c - info["nseg"])) <= 2
+    _, info = orc.ax(np.ones(geo.vol_shape, dtype=np.float32), geo, ang, orc.INTERP, info=True)
+    total_i, counts_i = tg.Ax_count(geo, ang, "interp", return_counts=True)
+    ci = counts_i.cpu().numpy().astype(np.int64)
+    assert np.max(np.abs(ci - info["nseg"])) <= 1 and np.mean(ci != info["nseg"]) < 1e-3
+
+
+# ------------------------------------------------------------------ Atb
+def test_c1_matched_atb(tg, c1):
+    geo, ang, vol = c1
+    proj = orc.ax(vol, geo, ang, orc.SIDDON).astype(np.float32)
+    ref = orc.atb(proj, geo, ang, orc.MATCHED)
+    got = host(tg.Atb(dev(proj), geo, ang, "matched"))
+    assert H.rel_l2(got, ref) <= 1e-5
+
+
+@pytest.mark.parametrize("mode,tol", [("matched", 1e-5), ("fdk", 1e-4)])
+def test_atb_random_projections(tg, mode, tol):
+    # noise-like projections (worst case for fp32 tap weights); detector smaller than the footprint so
+    # the zero border is exercised; ragged sizes
+    geo = Geometry(nVoxel=(70, 61, 53), dVoxel=(1.0, 1.0, 1.0), nDetector=(90, 50), dDetector=(1.5, 1.5),
+                   DSD=600.0, DSO=380.0, offDetector=(7.0, -3.0))
+    ang = circular_angles(19, start=0.05)
+    proj = np.random.default_rng(4).random((19, 50, 90), dtype=np.float32)
+    ref = orc.atb(proj, geo, ang, orc.MATCHED if mode == "matched" else orc.FDK)
+    got = host(tg.Atb(dev(proj), geo, ang, mode))
+    assert H.rel_l2(got, ref) <= tol
+
+
+@pytest.mark.parametrize("mode,tol", [("matched", 1e-5), ("fdk", 1e-4)])
+def test_atb_general_geometry(tg, mode, tol):
+    geo, ang = odd_geometry()
+    proj = np.random.default_rng(5).random((5, 31, 45), dtype=np.float32)
+    ref = orc.atb(proj, geo, ang, orc.MATCHED if mode == "matched" else orc.FDK)
+    got = host(tg.Atb(dev(proj), geo, ang, mode))
+    assert H.rel_l2(got, ref) <= tol
+
+
+def test_atb_tap_indices_match_oracle(tg):
+    # P19(b): delta projections make the tap index observable: backproject an image whose value is its
+    # own u index, and one whose value is its v index, at a single view -> bilinear returns (fu, fv)
+    geo = Geometry(nVoxel=(40, 36, 20), dVoxel=(1.0, 1.0, 1.0), nDetector=(128, 96), dDetector=(1.0, 1.0),
+                   DSD=600.0, DSO=380.0)
+    ang = circular_angles(1, start=0.7)
+    iu, iv = np.meshgrid(np.arange(128, dtype=np.float32), np.arange(96, dtype=np.float32))
+    _, fuv = orc.atb(np.ones((1, 96, 128), np.float32), geo, ang, orc.FDK, vox_ids=np.arange(40 * 36 * 20), return_fuv=True)
+    w = orc.atb(None, geo, ang, orc.FDK).ravel()
+    gu = host(tg.Atb(dev(iu[None]), geo, ang, "fdk")).ravel() / w
+    gv = host(tg.Atb(dev(iv[None]), geo, ang, "fdk")).ravel() / w
+    assert np.max(np.abs(gu - fuv[:, 0, 0])) < 2e-3 and np.max(np.abs(gv - fuv[:, 0, 1])) < 2e-3
+    frac = fuv[:, 0, :] - np.floor(fuv[:, 0, :])
+    safe = np.all((frac > 1e-3) & (frac < 1 - 1e-3), axis=1)
+    assert np.array_equal(np.floor(gu[safe]), np.floor(fuv[safe, 0, 0]))
+    assert np.array_equal(np.floor(gv[safe]), np.floor(fuv[safe, 0, 1]))
+
+
+def test_atb_behind_source_is_geometry_error(tg):
+    geo = Geometry(nVoxel=(8, 8, 8), dVoxel=(1, 1, 1), nDetector=(4, 4), dDetector=(1, 1), DSD=20, DSO=3.0)
+    with pytest.raises(tg.TigreError) as e:
+        tg.Atb(torch.ones((1, 4, 4), device="cuda"), geo, circular_angles(1), "fdk")
+    assert e.value.code == -2
+
+
+def test_fdk_atb_and_filter_scaled_c2(tg):
+    geo, ang, rec = make_config("C2", scale=4, n_angles=45)
+    vol = phantom_for(rec, geo)
+    proj = orc.ax(vol, geo, ang, orc.INTERP).astype(np.float32)
+    qref = orc.fdk_filter(proj, geo, ang)
+    q = host(tg.fdk_filter(dev(proj), geo, ang))
+    assert H.rel_l2(q, qref) <= 1e-4
+    xref = orc.fdk(proj, geo, ang)
+    x = host(tg.fdk(dev(proj), geo, ang))
+    assert H.rel_l2(x, xref) <= 1e-4
+    ref = orc.atb(qref.astype(np.float32), geo, ang, orc.FDK)
+    got = host(tg.Atb(dev(qref), geo, ang, "fdk"))
+    assert H.rel_l2(got, ref) <= 1e-4
+
+
+# ------------------------------------------------------------------ adjoint gap (P11)
+def test_inner_products_match_oracle(tg, c1):
+    geo, ang, vol = c1
+    y = np.random.default_rng(6).random((64, 96, 96), dtype=np.float32)
+    ax_o, aty_o = orc.ax(vol, geo, ang), orc.atb(y, geo, ang, orc.MATCHED)
+    lhs_o, rhs_o = float(np.sum(ax_o * y)), float(np.sum(vol * aty_o))
+    lhs_g = float(np.sum(host(tg.Ax(dev(vol), geo, ang, "siddon")) * y))
+    rhs_g = float(np.sum(vol * host(tg.Atb(dev(y), geo, ang, "matched"))))
+    assert abs(lhs_g - lhs_o) <= 1e-4 * abs(lhs_o) and abs(rhs_g - rhs_o) <= 1e-4 * abs(rhs_o)
+    gap_o = abs(lhs_o - rhs_o) / abs(lhs_o)
+    gap_g = abs(lhs_g - rhs_g) / abs(lhs_g)
+    assert abs(gap_g - gap_o) <= 2e-4          # the intrinsic gap of the voxel-driven pair is reported, not gated
+
+
+# ------------------------------------------------------------------ weights / elementwise / drivers
+def test_weights(tg, c1):
+    geo, ang, _ = c1
+    Wr = orc.row_weights(geo, ang, orc.SIDDON)
+    Wg = host(tg.row_weights(geo, ang, "siddon"))
+    assert np.array_equal(Wg == 0, Wr == 0) and H.rel_l2(Wg, Wr) <= 1e-5
+    Vr = orc.col_weights(geo, ang, orc.MATCHED)
+    Vg = host(tg.col_weights(geo, ang, "matched"))
+    assert np.array_equal(Vg == 0, Vr == 0) and H.rel_l2(Vg, Vr) <= 1e-5
+    geo2, ang2, _ = make_config("C2", scale=8, n_angles=12)
+    assert H.rel_l2(host(tg.row_weights(geo2, ang2, "interp")), orc.row_weights(geo2, ang2, orc.INTERP)) <= 1e-4
+    assert H.rel_l2(host(tg.col_weights(geo2, ang2, "fdk")), orc.col_weights(geo2, ang2, orc.FDK)) <= 1e-4
+
+
+def test_residual_and_update(tg):
+    rng = np.random.default_rng(7)
+    for n in (1, 5, 4096, 100003):
+        b, a, w = (rng.random(n, dtype=np.float32) for _ in range(3))
+        r, nrm = tg.residual(dev(b), dev(a), dev(w), return_norm=True)
+        assert np.array_equal(r.cpu().numpy(), w * (b - a))
+        assert abs(nrm - float(np.sum((b.astype(np.float64) - a) ** 2))) <= 1e-6 * max(nrm, 1e-30)
+        x, g, v = (rng.standard_normal(n).astype(np.float32) for _ in range(3))
+        out = tg.update(dev(x), dev(g), dev(v), lam=0.7, nonneg=True).cpu().numpy()
+        ref = np.maximum(x.astype(np.float64) + np.float32(0.7) * v.astype(np.float64) * g, 0)
+        assert np.allclose(out, ref, rtol=1e-6, atol=1e-6)
+    assert tg.residual(dev(np.zeros(0)), dev(np.zeros(0))).numel() == 0      # empty input
+
+
+def test_c1_sirt_iteration(tg, c1):
+    geo, ang, vol = c1
+    b = orc.ax(vol, geo, ang, orc.SIDDON).astype(np.float32)
+    xr, rr = orc.sirt(b, geo, ang, 1, lam=1.0)
+    xg, rg = tg.sirt(dev(b), geo, ang, 1, lam=1.0)
+    assert H.rel_l2(host(xg), xr) <= 1e-5
+    assert abs(rg[0] - rr[0]) <= 1e-5 * rr[0]
+
+
+def test_ossart_scaled_c3(tg):
+    geo, ang, rec = make_config("C3", scale=16, n_angles=40)         # 32^3, 64x48, half-fan offset
+    vol = phantom_for(rec, geo)
+    b = orc.ax(vol, geo, ang, orc.SIDDON).astype(np.float32)
+    subsets = [np.arange(s, 40, 5) for s in range(5)]
+    xr, rr = orc.ossart(b, geo, ang, subsets, 3)
+    xg, rg = tg.ossart(dev(b), geo, ang, subsets, 3)
+    assert H.rel_l2(host(xg), xr) <= 1e-4
+    assert np.allclose(rg, rr, rtol=1e-4)
+
+
+def test_cgls_small(tg):
+    geo, ang, rec = make_config("C4", scale=32, n_angles=24)         # 32^3, 48x48, tilted detector + COR
+    vol = phantom_for(dict(rec, phantom="rand32"), geo)
+    b = orc.ax(vol, geo, ang, orc.INTERP).astype(np.float32)
+    xr, rr = orc.cgls(b, geo, ang, 4, orc.INTERP, orc.MATCHED)
+    xg, rg = tg.cgls(dev(b), geo, ang, 4, "interp", "matched")
+    assert H.rel_l2(host(xg), xr) <= 1e-3
+    assert np.allclose(rg, rr, rtol=1e-3)
+
+
+def test_wrong_memory_space_and_args(tg):
+    geo, ang, _ = make_config("C1")
+    with pytest.raises(tg.TigreError) as e:
+        tg.Ax(torch.zeros(geo.vol_shape), geo, ang)        # pageable host tensor
+    assert e.value.code == -3
+    bad = geo.copy(dVoxel=(0.0, 1.0, 1.0))
+    with pytest.raises(tg.TigreError) as e:
+        tg.Ax(torch.zeros(geo.vol_shape, device="cuda"), bad, ang)
+    assert e.value.code == -2
