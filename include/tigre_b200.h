@@ -120,6 +120,19 @@ TIGRE_API int tigre_ossart(const float *b, const tigre_geo *geo, const double *a
                  const int32_t *subset_idx, const int32_t *subset_off, int nSubsets, int n_iter,
                  float lambda, int nonneg, int ax_mode, int atb_mode, float *x_inout,
                  double *resid_hist, void *cuda_stream);
+/* The same iteration with the per-geometry set-up (view tables, W_s, V_s, scratch) done once in a
+ * plan.  tigre_plan_create computes the weights on `cuda_stream`; the plan owns its device buffers
+ * (stream-ordered pool) until tigre_plan_destroy.  tigre_plan_ossart runs n_iter sweeps starting from
+ * x_inout; b and x_inout are both dev, or both PINNED HOST (then they are copied in, and x copied
+ * back, on the stream: the end-to-end path bench.py times). */
+typedef struct tigre_plan tigre_plan;
+TIGRE_API int tigre_plan_create(const tigre_geo *geo, const double *angles, int nA, const int32_t *subset_idx,
+                      const int32_t *subset_off, int nSubsets, int ax_mode, int atb_mode,
+                      void *cuda_stream, tigre_plan **plan_out);
+TIGRE_API int tigre_plan_ossart(tigre_plan *plan, const float *b, float *x_inout, int n_iter, float lambda,
+                      int nonneg, double *resid_hist, void *cuda_stream);
+TIGRE_API int tigre_plan_destroy(tigre_plan *plan);
+TIGRE_API size_t tigre_plan_bytes(const tigre_plan *plan);
 /* CGLS (textbook recurrences, DESIGN.md O-F), x0 = 0; x_out dev. */
 TIGRE_API int tigre_cgls(const float *b, const tigre_geo *geo, const double *angles, int nA, int n_iter,
                int ax_mode, int atb_mode, float *x_out, double *resid_hist, void *cuda_stream);
@@ -137,6 +150,13 @@ TIGRE_API int tigre_fdk_filter(const float *b, const tigre_geo *geo, const doubl
  * counts: dev uint32 [nA][nv][nu] or NULL; *total (host) = sum.  Synchronises. */
 TIGRE_API int tigre_Ax_count(const tigre_geo *geo, const double *angles, int nA, int mode, uint32_t *counts,
                    uint64_t *total, void *cuda_stream);
+/* In-library timing for bench.py's roofline leg.  tigre_profile(1) resets and starts recording a CUDA
+ * event pair around every kernel group the launchers enqueue (on the launching stream); tigre_profile(0)
+ * stops.  tigre_profile_read waits for the recorded events and returns, per kind k = 0 (Ax kernels),
+ * 1 (A^T b kernels), 2 (elementwise / reduction / filter kernels): ms[k] = summed device time,
+ * launches[k] = kernels launched since the last tigre_profile call (counted even when not recording). */
+TIGRE_API int tigre_profile(int enable);
+TIGRE_API int tigre_profile_read(double *ms /*[3]*/, uint64_t *launches /*[3]*/);
 /* bytes of stream-ordered temporaries a call of kind `op` will allocate */
 TIGRE_API size_t tigre_workspace_bytes(const tigre_geo *geo, int nA, int op);
 /* tuning knobs of the chunked path: device bytes it may use for slabs (0 = default 3/4 of free) */

@@ -50,7 +50,8 @@ class TigreError(RuntimeError):
 _LIB = None
 EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_row_weights", "tigre_col_weights", "tigre_residual",
            "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_fdk", "tigre_fdk_filter",
-           "tigre_Ax_count", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_strerror",
+           "tigre_Ax_count", "tigre_plan_create", "tigre_plan_ossart", "tigre_plan_destroy",
+           "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version"]
 
 
@@ -64,6 +65,9 @@ def _lib():
         lib.tigre_strerror.restype = C.c_char_p
         lib.tigre_last_cuda_error.restype = C.c_char_p
         lib.tigre_workspace_bytes.restype = C.c_size_t
+        lib.tigre_plan_bytes.restype = C.c_size_t
+        lib.tigre_plan_bytes.argtypes = [C.c_void_p]
+        lib.tigre_plan_destroy.argtypes = [C.c_void_p]
         for name in EXPORTS:
             getattr(lib, name)
         _LIB = lib
@@ -228,6 +232,46 @@ def ossart(b, geo, angles, subsets, n_iter, lam=1.0, nonneg=True, ax_mode="siddo
     return x, hist[:n_iter]
 
 
+class OssartPlan:
+    """tigre_plan_*: view tables and the SART weights computed once; iterate() runs sweeps."""
+
+    def __init__(self, geo, angles, subsets, ax_mode="siddon", atb_mode="matched"):
+        a, nA = _angles(angles)
+        G = _Geo(geo, nA)
+        idx = np.ascontiguousarray(np.concatenate([np.asarray(s, dtype=np.int32) for s in subsets]))
+        off = np.zeros(len(subsets) + 1, dtype=np.int32)
+        off[1:] = np.cumsum([len(s) for s in subsets])
+        self.geo, self.nA = geo, nA
+        self._h = C.c_void_p(None)
+        _check(_lib().tigre_plan_create(G.ref, a.ctypes.data_as(_dp), nA, idx.ctypes.data_as(C.POINTER(C.c_int32)),
+                                        off.ctypes.data_as(C.POINTER(C.c_int32)), len(subsets), _AX_MODES[ax_mode],
+                                        _ATB_MODES[atb_mode], _stream(), C.byref(self._h)), "tigre_plan_create")
+
+    @property
+    def nbytes(self):
+        return int(_lib().tigre_plan_bytes(self._h))
+
+    def iterate(self, b, x, n_iter=1, lam=1.0, nonneg=True, want_resid=True):
+        """In place on x.  b, x: CUDA tensors, or both pinned host tensors (end-to-end path)."""
+        hist = np.zeros(max(n_iter, 1), dtype=np.float64)
+        _check(_lib().tigre_plan_ossart(self._h, _f32(b, proj_shape(self.geo, self.nA), "b"),
+                                        _f32(x, vol_shape(self.geo), "x"), int(n_iter), C.c_float(lam),
+                                        int(bool(nonneg)), hist.ctypes.data_as(_dp) if want_resid else None,
+                                        _stream(b)), "tigre_plan_ossart")
+        return hist[:n_iter]
+
+    def close(self):
+        if self._h:
+            _lib().tigre_plan_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
 def sirt(b, geo, angles, n_iter, **kw):
     _, nA = _angles(angles)
     return ossart(b, geo, angles, [np.arange(nA)], n_iter, **kw)
@@ -282,6 +326,19 @@ def workspace_bytes(geo, nA, op):
 
 def set_chunk_budget(nbytes):
     _check(_lib().tigre_set_chunk_budget(C.c_size_t(int(nbytes))), "tigre_set_chunk_budget")
+
+
+def profile(enable=True):
+    _check(_lib().tigre_profile(int(bool(enable))), "tigre_profile")
+
+
+def profile_read():
+    """{'ms': {'ax','atb','ew'}, 'launches': {...}} accumulated since profile(True)."""
+    ms = (C.c_double * 3)()
+    n = (C.c_uint64 * 3)()
+    _check(_lib().tigre_profile_read(ms, n), "tigre_profile_read")
+    k = ("ax", "atb", "ew")
+    return dict(ms=dict(zip(k, [float(v) for v in ms])), launches=dict(zip(k, [int(v) for v in n])))
 
 
 def version():

@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <memory>
 #include <mutex>
 #include <string>
 #include <vector>
@@ -18,6 +19,38 @@ void set_cuda_error(cudaError_t e, const char* file, int line) {
     snprintf(buf, sizeof buf, "%s (%s) at %s:%d", cudaGetErrorName(e), cudaGetErrorString(e), file, line);
     g_last_cuda_error = buf;
     (void)cudaGetLastError();  // clear the non-sticky error state
+}
+
+// ---------------------------------------------------------------- profiling hook
+struct ProfRec {
+    cudaEvent_t a, b;
+    int kind;
+};
+static std::mutex g_prof_mu;
+static bool g_prof_on = false;
+static std::vector<ProfRec*> g_prof_recs;
+static unsigned long long g_prof_launches[PK_N] = {0, 0, 0};
+
+ProfScope::ProfScope(int k, cudaStream_t s, int launches) : kind(k), st(s), rec(nullptr) {
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    g_prof_launches[k] += launches;
+    if (!g_prof_on) return;
+    ProfRec* r = new ProfRec;
+    r->kind = k;
+    if (cudaEventCreate(&r->a) != cudaSuccess || cudaEventCreate(&r->b) != cudaSuccess) {
+        (void)cudaGetLastError();
+        delete r;
+        return;
+    }
+    cudaEventRecord(r->a, s);
+    rec = r;
+}
+ProfScope::~ProfScope() {
+    if (!rec) return;
+    ProfRec* r = (ProfRec*)rec;
+    cudaEventRecord(r->b, st);
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    g_prof_recs.push_back(r);
 }
 
 int TempBuf::alloc(size_t bytes, cudaStream_t st) {
@@ -122,6 +155,34 @@ extern "C" {
 
 int tigre_version(void) { return 100; }
 
+int tigre_profile(int enable) {
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    for (ProfRec* r : g_prof_recs) {
+        cudaEventDestroy(r->a);
+        cudaEventDestroy(r->b);
+        delete r;
+    }
+    g_prof_recs.clear();
+    for (int k = 0; k < PK_N; ++k) g_prof_launches[k] = 0;
+    g_prof_on = enable != 0;
+    return TIGRE_OK;
+}
+int tigre_profile_read(double* ms, uint64_t* launches) {
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    double acc[PK_N] = {0, 0, 0};
+    for (ProfRec* r : g_prof_recs) {
+        TG_CUDA(cudaEventSynchronize(r->b));
+        float t = 0.f;
+        TG_CUDA(cudaEventElapsedTime(&t, r->a, r->b));
+        acc[r->kind] += t;
+    }
+    for (int k = 0; k < PK_N; ++k) {
+        if (ms) ms[k] = acc[k];
+        if (launches) launches[k] = g_prof_launches[k];
+    }
+    return TIGRE_OK;
+}
+
 const char* tigre_strerror(int code) {
     switch (code) {
         case TIGRE_OK: return "ok";
@@ -186,6 +247,10 @@ int tigre_col_weights(const tigre_geo* geo, const double* angles, int nA, int at
 }
 
 int tigre_residual(const float* b, const float* Ax, const float* W, float* r, size_t n, double* nrm2, void* cuda_stream) {
+    if (n == 0) {
+        if (nrm2) *nrm2 = 0.0;
+        return TIGRE_OK;
+    }
     if (!b || !Ax || !r) return TIGRE_ERR_ARG;
     TG_TRY(ensure_device());
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -203,6 +268,7 @@ int tigre_residual(const float* b, const float* Ax, const float* W, float* r, si
 }
 
 int tigre_update(float* x, const float* g, const float* V, float lambda, int nonneg, size_t n, void* cuda_stream) {
+    if (n == 0) return TIGRE_OK;
     if (!x || !g) return TIGRE_ERR_ARG;
     TG_TRY(ensure_device());
     return launch_update(x, g, V, lambda, nonneg, n, (cudaStream_t)cuda_stream);
@@ -235,38 +301,48 @@ int tigre_Ax_count(const tigre_geo* geo, const double* angles, int nA, int mode,
 }
 
 // ---------------------------------------------------------------- OS-SART / SIRT
-int tigre_ossart(const float* b, const tigre_geo* geo, const double* angles, int nA, const int32_t* subset_idx,
-                 const int32_t* subset_off, int nSubsets, int n_iter, float lambda, int nonneg, int ax_mode,
-                 int atb_mode, float* x, double* resid_hist, void* cuda_stream) {
-    if (!b || !x || !subset_idx || !subset_off || nSubsets <= 0 || n_iter < 0) return TIGRE_ERR_ARG;
+// A plan holds what does not change between iterations: the per-subset view tables, the row weights
+// W_s = 1/(A_s 1) and column weights V_s = 1/(A_s^T 1) (P13, P16) and the scratch buffers.
+struct tigre_plan {
+    Tables t;
+    int nA = 0, nSubsets = 0, maxs = 0, ax_mode = 0, atb_mode = 0;
+    std::vector<int32_t> idx, off;
+    std::vector<TempBuf> ray, vox;
+    TempBuf W, V, Axb, grad, d_idx, d_acc;
+    size_t bytes = 0;
+};
+
+int tigre_plan_create(const tigre_geo* geo, const double* angles, int nA, const int32_t* subset_idx,
+                      const int32_t* subset_off, int nSubsets, int ax_mode, int atb_mode, void* cuda_stream,
+                      tigre_plan** out) {
+    if (!out || !subset_idx || !subset_off || nSubsets <= 0) return TIGRE_ERR_ARG;
+    *out = nullptr;
     if (ax_mode != TIGRE_AX_SIDDON && ax_mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
     if (atb_mode != TIGRE_ATB_MATCHED && atb_mode != TIGRE_ATB_FDK) return TIGRE_ERR_ARG;
-    Tables t;
-    TG_TRY(prep(geo, angles, nA, t));
-    if (mem_kind(b) != MEM_DEVICE || mem_kind(x) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    std::unique_ptr<tigre_plan> P(new tigre_plan);
+    TG_TRY(prep(geo, angles, nA, P->t));
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    int maxs = 0;
+    P->nA = nA, P->nSubsets = nSubsets, P->ax_mode = ax_mode, P->atb_mode = atb_mode;
     for (int s = 0; s < nSubsets; ++s) {
         const int n = subset_off[s + 1] - subset_off[s];
         if (n <= 0) return TIGRE_ERR_ARG;
-        maxs = std::max(maxs, n);
+        P->maxs = std::max(P->maxs, n);
         for (int k = subset_off[s]; k < subset_off[s + 1]; ++k)
             if (subset_idx[k] < 0 || subset_idx[k] >= nA) return TIGRE_ERR_ARG;
     }
-    const Grid& g = t.g;
-    const size_t per = (size_t)g.nu * g.nv, nvox = (size_t)g.nx * g.ny * g.nz;
     const int nIdx = subset_off[nSubsets];
-    // Temporaries: W for every view listed (subset-major), V per subset, one subset's Ax/residual, A^T r.
-    TempBuf W, V, Axb, grad, d_idx, d_acc;
-    TG_TRY(W.alloc(sizeof(float) * per * nIdx, st));
-    TG_TRY(V.alloc(sizeof(float) * nvox * nSubsets, st));
-    TG_TRY(Axb.alloc(sizeof(float) * per * maxs, st));
-    TG_TRY(grad.alloc(sizeof(float) * nvox, st));
-    TG_TRY(upload(d_idx, subset_idx, sizeof(int32_t) * nIdx, st));
-    TG_TRY(d_acc.alloc(sizeof(double) * std::max(n_iter, 1), st));
-    TG_CUDA(cudaMemsetAsync(d_acc.p, 0, sizeof(double) * std::max(n_iter, 1), st));
-    // per-subset tables and weights (P13, P16)
-    std::vector<TempBuf> ray(nSubsets), vox(nSubsets);
+    P->idx.assign(subset_idx, subset_idx + nIdx);
+    P->off.assign(subset_off, subset_off + nSubsets + 1);
+    const Grid& g = P->t.g;
+    const size_t per = (size_t)g.nu * g.nv, nvox = (size_t)g.nx * g.ny * g.nz;
+    TG_TRY(P->W.alloc(sizeof(float) * per * nIdx, st));
+    TG_TRY(P->V.alloc(sizeof(float) * nvox * nSubsets, st));
+    TG_TRY(P->Axb.alloc(sizeof(float) * per * P->maxs, st));
+    TG_TRY(P->grad.alloc(sizeof(float) * nvox, st));
+    TG_TRY(upload(P->d_idx, subset_idx, sizeof(int32_t) * nIdx, st));
+    P->bytes = sizeof(float) * (per * nIdx + nvox * nSubsets + per * P->maxs + nvox);
+    P->ray = std::vector<TempBuf>(nSubsets);
+    P->vox = std::vector<TempBuf>(nSubsets);
     const double epsW = 1e-2 * std::min(g.dx, std::min(g.dy, g.dz));
     for (int s = 0; s < nSubsets; ++s) {
         const int32_t* idx = subset_idx + subset_off[s];
@@ -274,41 +350,85 @@ int tigre_ossart(const float* b, const tigre_geo* geo, const double* angles, int
         std::vector<RayView> hr(n);
         std::vector<VoxView> hv(n);
         for (int i = 0; i < n; ++i) {
-            build_ray_view(g, t.views[idx[i]], hr[i]);
-            TG_TRY(build_vox_view(g, t.views[idx[i]], hv[i]));
+            build_ray_view(g, P->t.views[idx[i]], hr[i]);
+            TG_TRY(build_vox_view(g, P->t.views[idx[i]], hv[i]));
         }
-        TG_TRY(upload(ray[s], hr.data(), sizeof(RayView) * n, st));
-        TG_TRY(upload(vox[s], hv.data(), sizeof(VoxView) * n, st));
-        float* Ws = W.as<float>() + per * subset_off[s];
-        float* Vs = V.as<float>() + nvox * s;
-        TG_TRY(launch_ax(nullptr, g, ray[s].as<RayView>(), n, ax_mode, true, false, Ws, nullptr, st));
+        TG_TRY(upload(P->ray[s], hr.data(), sizeof(RayView) * n, st));
+        TG_TRY(upload(P->vox[s], hv.data(), sizeof(VoxView) * n, st));
+        float* Ws = P->W.as<float>() + per * subset_off[s];
+        float* Vs = P->V.as<float>() + nvox * s;
+        TG_TRY(launch_ax(nullptr, g, P->ray[s].as<RayView>(), n, ax_mode, true, false, Ws, nullptr, st));
         TG_TRY(launch_invert_rows(Ws, per * n, (float)epsW, st));
-        TG_TRY(launch_atb(nullptr, g, vox[s].as<VoxView>(), n, atb_mode, true, Vs, 0, g.nz, false, 0, g.nv, st));
+        TG_TRY(launch_atb(nullptr, g, P->vox[s].as<VoxView>(), n, atb_mode, true, Vs, 0, g.nz, false, 0, g.nv, st));
         TG_TRY(launch_invert_cols(Vs, nvox, 1e-6f, st));
     }
+    *out = P.release();
+    return TIGRE_OK;
+}
+
+int tigre_plan_destroy(tigre_plan* plan) {
+    delete plan;   // TempBuf destructors return the buffers to the stream-ordered pool
+    return TIGRE_OK;
+}
+
+size_t tigre_plan_bytes(const tigre_plan* plan) { return plan ? plan->bytes : 0; }
+
+int tigre_plan_ossart(tigre_plan* P, const float* b, float* x, int n_iter, float lambda, int nonneg,
+                      double* resid_hist, void* cuda_stream) {
+    if (!P || !b || !x || n_iter < 0) return TIGRE_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const Grid& g = P->t.g;
+    const size_t per = (size_t)g.nu * g.nv, nvox = (size_t)g.nx * g.ny * g.nz;
+    // b and x may live in device memory, or both in pinned host memory (end-to-end path: the
+    // projections and the iterate are copied in, the iterate is copied back, all on `st`)
+    const MemKind kb = mem_kind(b), kx = mem_kind(x);
+    TempBuf db, dx;
+    const float* bd = b;
+    float* xd = x;
+    if (kb == MEM_PINNED && kx == MEM_PINNED) {
+        TG_TRY(db.alloc(sizeof(float) * per * P->nA, st));
+        TG_TRY(dx.alloc(sizeof(float) * nvox, st));
+        TG_CUDA(cudaMemcpyAsync(db.p, b, sizeof(float) * per * P->nA, cudaMemcpyHostToDevice, st));
+        TG_CUDA(cudaMemcpyAsync(dx.p, x, sizeof(float) * nvox, cudaMemcpyHostToDevice, st));
+        bd = db.as<float>(), xd = dx.as<float>();
+    } else if (kb != MEM_DEVICE || kx != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    TG_TRY(P->d_acc.alloc(sizeof(double) * std::max(n_iter, 1), st));
+    TG_CUDA(cudaMemsetAsync(P->d_acc.p, 0, sizeof(double) * std::max(n_iter, 1), st));
     for (int it = 0; it < n_iter; ++it) {
-        for (int s = 0; s < nSubsets; ++s) {
-            const int n = subset_off[s + 1] - subset_off[s];
-            float* Ws = W.as<float>() + per * subset_off[s];
-            float* Vs = V.as<float>() + nvox * s;
-            float* A = Axb.as<float>();
-            TG_TRY(launch_ax(x, g, ray[s].as<RayView>(), n, ax_mode, false, false, A, nullptr, st));
-            // r = W_s .* (b_s - A_s x), in place over A; b gathered through the subset's view list,
-            // W stored subset-major so it is read with the local view index
-            TG_TRY(launch_residual(b, d_idx.as<int32_t>() + subset_off[s], A, Ws, A, per, n, d_acc.as<double>() + it, st));
-            TG_TRY(launch_atb(A, g, vox[s].as<VoxView>(), n, atb_mode, false, grad.as<float>(), 0, g.nz, false, 0, g.nv, st));
-            TG_TRY(launch_update(x, grad.as<float>(), Vs, lambda, nonneg, nvox, st));
+        for (int s = 0; s < P->nSubsets; ++s) {
+            const int n = P->off[s + 1] - P->off[s];
+            float* Ws = P->W.as<float>() + per * P->off[s];
+            float* Vs = P->V.as<float>() + nvox * s;
+            float* A = P->Axb.as<float>();
+            TG_TRY(launch_ax(xd, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st));
+            // r = W_s .* (b_s - A_s x) in place over A; b is gathered through the subset's view list
+            TG_TRY(launch_residual(bd, P->d_idx.as<int32_t>() + P->off[s], A, Ws, A, per, n, P->d_acc.as<double>() + it, st));
+            TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>(), 0, g.nz, false, 0, g.nv, st));
+            TG_TRY(launch_update(xd, P->grad.as<float>(), Vs, lambda, nonneg, nvox, st));
         }
     }
+    if (xd != x) TG_CUDA(cudaMemcpyAsync(x, xd, sizeof(float) * nvox, cudaMemcpyDeviceToHost, st));
     if (resid_hist && n_iter > 0) {
         std::vector<double> h(n_iter);
-        TG_CUDA(cudaMemcpyAsync(h.data(), d_acc.p, sizeof(double) * n_iter, cudaMemcpyDeviceToHost, st));
+        TG_CUDA(cudaMemcpyAsync(h.data(), P->d_acc.p, sizeof(double) * n_iter, cudaMemcpyDeviceToHost, st));
         TG_CUDA(cudaStreamSynchronize(st));
         for (int it = 0; it < n_iter; ++it) resid_hist[it] = std::sqrt(h[it]);
+    } else if (xd != x) {
+        TG_CUDA(cudaStreamSynchronize(st));
     }
     return TIGRE_OK;
 }
 
+int tigre_ossart(const float* b, const tigre_geo* geo, const double* angles, int nA, const int32_t* subset_idx,
+                 const int32_t* subset_off, int nSubsets, int n_iter, float lambda, int nonneg, int ax_mode,
+                 int atb_mode, float* x, double* resid_hist, void* cuda_stream) {
+    if (!b || !x) return TIGRE_ERR_ARG;
+    tigre_plan* P = nullptr;
+    TG_TRY(tigre_plan_create(geo, angles, nA, subset_idx, subset_off, nSubsets, ax_mode, atb_mode, cuda_stream, &P));
+    const int rc = tigre_plan_ossart(P, b, x, n_iter, lambda, nonneg, resid_hist, cuda_stream);
+    tigre_plan_destroy(P);
+    return rc;
+}
 
 // ---------------------------------------------------------------- CGLS (textbook recurrences, O-F)
 int tigre_cgls(const float* b, const tigre_geo* geo, const double* angles, int nA, int n_iter, int ax_mode,

@@ -108,6 +108,7 @@ int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nVi
     dim3 block(ATB_BX, ATB_BY);
     dim3 grid((g.nx + ATB_BX - 1) / ATB_BX, (g.ny + ATB_BY - 1) / ATB_BY, (nzs + ZR - 1) / ZR);
     if (grid.y > 65535 || grid.z > 65535) return TIGRE_ERR_ARG;
+    ProfScope ps(PK_ATB, st);
     if (unit_proj) {
         if (mode == TIGRE_ATB_FDK) atb_gather_kernel<TIGRE_ATB_FDK, true, ZR><<<grid, block, 0, st>>>(proj, d_views, nViews, p, vol);
         else atb_gather_kernel<TIGRE_ATB_MATCHED, true, ZR><<<grid, block, 0, st>>>(proj, d_views, nViews, p, vol);

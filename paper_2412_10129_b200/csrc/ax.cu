@@ -100,42 +100,66 @@ ax_siddon_kernel(const float* __restrict__ vol, const RayView* __restrict__ view
                 i0 = max(i0, 0), i1 = min(i1, nD);
                 const int nslab = i1 - i0;
                 const int hE = nE >> 1, hF = nF >> 1;   // volume-centred coordinates: |e| <= n/2
-                const float eref = (float)(SE + ((double)i0 - SD) * mE - (double)hE);
-                const float fref = (float)(SF + ((double)i0 - SD) * mF - (double)hF);
+                // state at the START of slab i0 (s = 0), fp64: position, cell index, next plane ahead
+                const double eS = SE + ((double)i0 - SD) * mE, fS = SF + ((double)i0 - SD) * mF;
+                int ie = (int)floor(eS), jf = (int)floor(fS);
+                const bool upE = mE > 0.0, upF = mF > 0.0;
+                const float eref = (float)(eS - (double)hE), fref = (float)(fS - (double)hF);
                 const float mEf = (float)mE, mFf = (float)mF;
-                const float imE = mE != 0.0 ? (float)(1.0 / mE) : 0.f, imF = mF != 0.0 ? (float)(1.0 / mF) : 0.f;
+                // slab-local parameter of the next E / F plane: s = (next - e0) / m, saturated to [0,1];
+                // a ray parallel to the planes (m = 0) never crosses: next = +huge, 1/m := 1
+                const float imE = mE != 0.0 ? (float)(1.0 / mE) : 1.f, imF = mF != 0.0 ? (float)(1.0 / mF) : 1.f;
+                float nextE = mE != 0.0 ? (float)((upE ? ie + 1 : ie) - hE) : 3.0e38f;
+                float nextF = mF != 0.0 ? (float)((upF ? jf + 1 : jf) - hF) : 3.0e38f;
+                const float sgE = upE ? 1.f : -1.f, sgF = upF ? 1.f : -1.f;
                 const float slo0 = (float)(lo - (double)i0), shiN = (float)(hi - (double)(i1 - 1));
                 const IdxT sD = D == 0 ? 1 : (D == 1 ? (IdxT)p.nx : (IdxT)p.nx * p.ny);
                 const IdxT sE = E == 0 ? 1 : (E == 1 ? (IdxT)p.nx : (IdxT)p.nx * p.ny);
                 const IdxT sF = F == 0 ? 1 : (F == 1 ? (IdxT)p.nx : (IdxT)p.nx * p.ny);
-                float e0 = eref, f0 = fref;
-                float fe0 = floorf(e0), ff0 = floorf(f0);
+                const IdxT stE = upE ? sE : -sE, stF = upF ? sF : -sF;
+                const int diE = upE ? 1 : -1, diF = upF ? 1 : -1;
+                IdxT off = (IdxT)i0 * sD + (IdxT)ie * sE + (IdxT)jf * sF;   // may be out of range: guarded below
                 float acc = 0.f;
-                IdxT base = (IdxT)i0 * sD;
+                float kf = 0.f;
+                const int last = nslab - 1;
                 for (int k = 0; k < nslab; ++k) {
-                    const float e1 = fmaf((float)(k + 1), mEf, eref);
-                    const float f1 = fmaf((float)(k + 1), mFf, fref);
-                    const float fe1 = floorf(e1), ff1 = floorf(f1);
-                    const float slo = (k == 0) ? slo0 : 0.f;
-                    const float shi = (k == nslab - 1) ? shiN : 1.f;
-                    // slab-local parameter of the E / F plane crossing (2 = none in this slab)
-                    const float se = (fe0 != fe1) ? (fmaxf(fe0, fe1) - e0) * imE : 2.f;
-                    const float sf = (ff0 != ff1) ? (fmaxf(ff0, ff1) - f0) * imF : 2.f;
-                    const float s1 = fminf(fmaxf(fminf(se, sf), slo), shi);
-                    const float s2 = fminf(fmaxf(fmaxf(se, sf), slo), shi);
-                    const float lenA = s1 - slo, lenB = s2 - s1, lenC = shi - s2;
-                    const int ieA = (int)fe0 + hE, ifA = (int)ff0 + hF;
-                    const int ieC = (int)fe1 + hE, ifC = (int)ff1 + hF;
-                    const bool eFirst = se < sf;
-                    const int ieB = eFirst ? ieC : ieA, ifB = eFirst ? ifA : ifC;
-                    if (lenA > 0.f && (unsigned)ieA < (unsigned)nE && (unsigned)ifA < (unsigned)nF)
-                        acc = fmaf(lenA, UNIT ? 1.f : __ldg(vol + base + (IdxT)ieA * sE + (IdxT)ifA * sF), acc);
-                    if (lenB > 0.f && (unsigned)ieB < (unsigned)nE && (unsigned)ifB < (unsigned)nF)
-                        acc = fmaf(lenB, UNIT ? 1.f : __ldg(vol + base + (IdxT)ieB * sE + (IdxT)ifB * sF), acc);
-                    if (lenC > 0.f && (unsigned)ieC < (unsigned)nE && (unsigned)ifC < (unsigned)nF)
-                        acc = fmaf(lenC, UNIT ? 1.f : __ldg(vol + base + (IdxT)ieC * sE + (IdxT)ifC * sF), acc);
-                    e0 = e1, f0 = f1, fe0 = fe1, ff0 = ff1;
-                    base += sD;
+                    const float e0 = fmaf(kf, mEf, eref), f0 = fmaf(kf, mFf, fref);
+                    kf += 1.0f;
+                    const float se = __saturatef((nextE - e0) * imE);
+                    const float sf = __saturatef((nextF - f0) * imF);
+                    const bool cE = se < 1.0f, cF = sf < 1.0f;
+                    float s1 = fminf(se, sf), s2 = fmaxf(se, sf);
+                    float slo = 0.f, shi = 1.f;
+                    if (k == 0 || k == last) {   // only the end slabs are clipped to the segment / box
+                        slo = (k == 0) ? slo0 : 0.f;
+                        shi = (k == last) ? shiN : 1.f;
+                        s1 = fminf(fmaxf(s1, slo), shi);
+                        s2 = fminf(fmaxf(s2, slo), shi);
+                    }
+                    const bool vEA = (unsigned)ie < (unsigned)nE, vFA = (unsigned)jf < (unsigned)nF;
+                    const int ieC = cE ? ie + diE : ie, jfC = cF ? jf + diF : jf;
+                    const IdxT offC = off + (cE ? stE : (IdxT)0) + (cF ? stF : (IdxT)0);
+                    const bool vEC = (unsigned)ieC < (unsigned)nE, vFC = (unsigned)jfC < (unsigned)nF;
+                    const float lenA = s1 - slo, lenC = shi - s2;
+                    if (lenA > 0.f && vEA && vFA) acc = fmaf(lenA, UNIT ? 1.f : __ldg(vol + off), acc);
+                    if (__any_sync(__activemask(), cE && cF)) {
+                        // some lane crosses both planes inside this slab: a middle voxel between the two crossings
+                        // (for a lane with one crossing the middle voxel IS the end voxel and lenC = 0)
+                        const float lenB = s2 - s1;
+                        const bool eFirst = se < sf;
+                        const IdxT offB = eFirst ? off + stE : off + stF;
+                        const bool vB = eFirst ? (vEC && vFA) : (vEA && vFC);
+                        if (lenB > 0.f && vB) acc = fmaf(lenB, UNIT ? 1.f : __ldg(vol + offB), acc);
+                        if (lenC > 0.f && vEC && vFC) acc = fmaf(lenC, UNIT ? 1.f : __ldg(vol + offC), acc);
+                    } else {
+                        // at most one crossing: [s1, shi] lies in the end voxel (s2 == shi when nothing else crosses)
+                        const float lenBC = shi - s1;
+                        if (lenBC > 0.f && vEC && vFC) acc = fmaf(lenBC, UNIT ? 1.f : __ldg(vol + offC), acc);
+                    }
+                    if (cE) nextE += sgE;
+                    if (cF) nextF += sgF;
+                    ie = ieC, jf = jfC;
+                    off = offC + sD;
                 }
                 result = acc * (float)(Lmm / fabs(dD));
             }
@@ -274,6 +298,7 @@ int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nView
     const long long nblk = (long long)p.nUt * p.nVt * nViews;
     if (nblk <= 0 || nblk > 0x7fffffffLL) return TIGRE_ERR_ARG;
     const size_t nvox = (size_t)g.nx * g.ny * g.nz;
+    ProfScope ps(PK_AX, st);
     if (nvox < (1ull << 31)) ax_dispatch<int>(vol, d_views, nViews, p, mode, unit_vol, proj, count_out, st);
     else ax_dispatch<long long>(vol, d_views, nViews, p, mode, unit_vol, proj, count_out, st);
     TG_CUDA(cudaGetLastError());

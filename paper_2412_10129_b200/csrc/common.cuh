@@ -80,6 +80,18 @@ struct TempBuf {  // RAII: cudaMallocAsync / cudaFreeAsync on one stream
 // copy a small host table to a fresh device buffer on the stream (host data is staged before return)
 int upload(TempBuf& buf, const void* host, size_t bytes, cudaStream_t st);
 
+// ---------------------------------------------------------------- in-library timing (bench.py's roofline leg)
+// When enabled with tigre_profile(1) every launcher brackets its kernels with CUDA events on the
+// launching stream; tigre_profile_read() sums the elapsed times per kind.  Launch counts are kept always.
+enum ProfKind { PK_AX = 0, PK_ATB = 1, PK_EW = 2, PK_N = 3 };
+struct ProfScope {
+    int kind;
+    cudaStream_t st;
+    void* rec;
+    ProfScope(int kind, cudaStream_t st, int launches = 1);
+    ~ProfScope();
+};
+
 // ---------------------------------------------------------------- kernel launchers (device pointers)
 // forward projection of nViews views given their RayView table (device), out contiguous [nViews][nv][nu]
 //   unit_vol: treat the volume as all ones (row sums A 1), vol may be NULL

@@ -82,6 +82,7 @@ residual_kernel_scalar(const float* __restrict__ b, const int32_t* __restrict__ 
 
 int launch_residual(const float* b, const int32_t* view_idx, const float* Ax, const float* W, float* r,
                     size_t per_view, int nViews, double* d_nrm2, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
     const size_t total = per_view * nViews;
     if (total == 0) return TIGRE_OK;
     const bool al = ((per_view & 3) == 0) && ((((uintptr_t)b | (uintptr_t)Ax | (uintptr_t)r | (uintptr_t)W) & 15) == 0);
@@ -119,6 +120,7 @@ update_kernel(float* __restrict__ x, const float* __restrict__ g, const float* _
     }
 }
 int launch_update(float* x, const float* g, const float* V, float lambda, int nonneg, size_t n, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
     if (n == 0) return TIGRE_OK;
     const int vec = ((((uintptr_t)x | (uintptr_t)g | (uintptr_t)V) & 15) == 0) ? 1 : 0;
     update_kernel<<<ew_blocks(n / 4 + 1), 256, 0, st>>>(x, g, V, lambda, nonneg, n, vec);
@@ -141,12 +143,14 @@ __global__ void __launch_bounds__(256) max_kernel(const float* __restrict__ v, s
     if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<int*>(out), __float_as_int(m));   // valid for m >= 0
 }
 int launch_invert_rows(float* w, size_t n, float eps, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
     if (n == 0) return TIGRE_OK;
     invert_kernel<<<ew_blocks(n), 256, 0, st>>>(w, n, eps, nullptr, 0.f);
     TG_CUDA(cudaGetLastError());
     return TIGRE_OK;
 }
 int launch_invert_cols(float* v, size_t n, float rel_eps, cudaStream_t st) {
+    ProfScope ps(PK_EW, st, 2);
     if (n == 0) return TIGRE_OK;
     TempBuf mx;
     TG_TRY(mx.alloc(sizeof(float), st));
@@ -165,6 +169,7 @@ __global__ void __launch_bounds__(256) dot_kernel(const float* __restrict__ a, c
     if (threadIdx.x == 0) atomicAdd(out, s);
 }
 int launch_dot(const float* a, const float* b, size_t n, double* d_out, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
     TG_CUDA(cudaMemsetAsync(d_out, 0, sizeof(double), st));
     if (n == 0) return TIGRE_OK;
     dot_kernel<<<ew_blocks(n), 256, 0, st>>>(a, b, n, d_out);
@@ -176,6 +181,7 @@ __global__ void __launch_bounds__(256) axpy_kernel(float* __restrict__ y, const 
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) y[i] = fmaf(a, x[i], y[i]);
 }
 int launch_axpy(float* y, const float* x, const double* d_num, const double* d_den, float sign, size_t n, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
     if (n == 0) return TIGRE_OK;
     axpy_kernel<<<ew_blocks(n), 256, 0, st>>>(y, x, d_num, d_den, sign, n);
     TG_CUDA(cudaGetLastError());
@@ -186,6 +192,7 @@ __global__ void __launch_bounds__(256) xpby_kernel(float* __restrict__ p, const 
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = fmaf(bta, p[i], s[i]);
 }
 int launch_xpby(float* p, const float* s, const double* d_num, const double* d_den, size_t n, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
     if (n == 0) return TIGRE_OK;
     xpby_kernel<<<ew_blocks(n), 256, 0, st>>>(p, s, d_num, d_den, n);
     TG_CUDA(cudaGetLastError());
@@ -195,6 +202,7 @@ __global__ void __launch_bounds__(256) scale_kernel(float* __restrict__ x, float
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) x[i] *= a;
 }
 int launch_scale(float* x, float a, size_t n, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
     if (n == 0) return TIGRE_OK;
     scale_kernel<<<ew_blocks(n), 256, 0, st>>>(x, a, n);
     TG_CUDA(cudaGetLastError());
@@ -209,6 +217,7 @@ __global__ void __launch_bounds__(256) count_reduce_kernel(const uint32_t* __res
     if ((threadIdx.x & 31) == 0) atomicAdd(out, s);
 }
 int launch_count_reduce(const uint32_t* c, size_t n, unsigned long long* d_total, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
     TG_CUDA(cudaMemsetAsync(d_total, 0, sizeof(unsigned long long), st));
     if (n == 0) return TIGRE_OK;
     count_reduce_kernel<<<ew_blocks(n), 256, 0, st>>>(c, n, d_total);
@@ -254,6 +263,7 @@ fdk_filter_kernel(const float* __restrict__ b, int nu, int nv, float du, float d
 }
 int launch_fdk_filter(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, int nViews,
                       float* q, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
     const size_t smem = 2 * (size_t)g.nu * sizeof(float);
     if (smem > 200 * 1024) return TIGRE_ERR_ARG;
     if (smem > 48 * 1024) TG_CUDA(cudaFuncSetAttribute(fdk_filter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -60,30 +60,34 @@ def concat_ellipsoids(*lists):
 
 
 def voxelise_slab(ell, geo, z0: int, z1: int, dtype=np.float32):
-    """Voxelise z-slices [z0, z1) of the volume described by geo (offOrigin scalar form)."""
-    nx, ny, _ = geo.nVoxel
+    """Voxelise z-slices [z0, z1) of the volume described by geo (offOrigin scalar form).
+    Membership ((Q^T (X-c)) / axes)^2 summed <= 1 is evaluated in float64 at voxel centres, inside
+    each ellipsoid's axis-aligned bounding box only."""
+    nx, ny, nz = geo.nVoxel
     dx, dy, dz = geo.dVoxel
     ox, oy, oz = geo.offOrigin
     x = ox + (np.arange(nx) + 0.5) * dx - 0.5 * nx * dx
     y = oy + (np.arange(ny) + 0.5) * dy - 0.5 * ny * dy
-    z = oz + (np.arange(z0, z1) + 0.5) * dz - 0.5 * geo.nVoxel[2] * dz
-    out = np.zeros((z1 - z0, ny, nx), dtype=np.float64)
+    z = oz + (np.arange(z0, z1) + 0.5) * dz - 0.5 * nz * dz
+    out = np.zeros((z1 - z0, ny, nx), dtype=dtype)
     for c, ax, Q, rho in zip(ell["centre"], ell["axes"], ell["Q"], ell["rho"]):
-        # bounding radius cull along z
-        rmax = float(np.max(ax))
-        zsel = np.nonzero(np.abs(z - c[2]) <= rmax)[0]
-        if zsel.size == 0:
+        ext = np.sqrt(((Q * ax[None, :]) ** 2).sum(axis=1))      # half-extent of the bounding box per world axis
+        sel = []
+        for coord, ck, ek in ((x, c[0], ext[0]), (y, c[1], ext[1]), (z, c[2], ext[2])):
+            k = np.nonzero(np.abs(coord - ck) <= ek)[0]
+            sel.append(k)
+        if any(k.size == 0 for k in sel):
             continue
-        za, zb = zsel[0], zsel[-1] + 1
-        X = x[None, None, :] - c[0]
-        Y = y[None, :, None] - c[1]
-        Z = z[za:zb, None, None] - c[2]
+        sx, sy, sz = (slice(k[0], k[-1] + 1) for k in sel)
+        X = x[sx][None, None, :] - c[0]
+        Y = y[sy][None, :, None] - c[1]
+        Z = z[sz][:, None, None] - c[2]
         s = 0.0
         for k in range(3):
             lk = (Q[0, k] * X + Q[1, k] * Y + Q[2, k] * Z) / ax[k]
             s = s + lk * lk
-        out[za:zb] += rho * (s <= 1.0)
-    return out.astype(dtype)
+        out[sz, sy, sx] += (rho * (s <= 1.0)).astype(dtype)
+    return out
 
 
 def voxelise(ell, geo, dtype=np.float32, slab: int = 64):
