@@ -1,0 +1,288 @@
+#!/usr/bin/env python
+"""bench.py — one JSON line for the driver.
+
+A step = one pass of the whole hot path over the workload: one OS-SART iteration
+(all ordered subsets: Ax on every view, residual with row weights, A^T b on every view,
+column-weighted update) through libtigre_b200's plan API.  Default workload: BASELINE.json
+configs[2] "C3" (512^3, 720 views of 1024x768, half-fan, Poisson noise, 20 ordered subsets,
+Siddon Ax / matched A^T b) — the configuration north_star's target is quoted on.
+
+  python bench.py --gpus N --steps K --warmup W [--config C3] [--impl reference]
+
+N > 1 (torchrun): the path does not shard in this build (north_star: one GPU, no collectives),
+so every rank runs an independent replica of the same workload; value = N * units / max time.
+--impl reference times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from workloads import make_config, phantom_for  # noqa: E402
+
+METRIC = "Ax ray-samples/s + A^T b voxel-updates/s (one OS-SART iteration)"
+UNIT = "G(samples+updates)/s"
+
+# issue-slot model of the dominant kernel: thread-instructions per unit of work
+# measured by ncu (smsp__inst_executed.sum * 32 / units), see profiles/.
+INSTR_PER_UNIT = {"ax_siddon": 30.0, "ax_interp": 75.0, "atb": 34.0}
+SM_COUNT, LANES_PER_CLK = 148, 128          # 4 schedulers x 32 lanes per SM per clock
+
+
+def subsets_for(rec, nA):
+    n = 20 if rec["name"] == "C3" else 1
+    n = min(n, nA)
+    return [np.arange(s, nA, n) for s in range(n)]        # interleaved, visited in order (P15)
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([c.strip() for c in out.strip().split(",")])
+            except Exception:
+                pass
+            time.sleep(0.2)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in self.rows if len(r) >= 7 for n, v in zip(names, r[3:7]) if v.lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def cpu_baseline(geo, ang, rec, vol_h, b_h, samples_per_step, updates_per_step, budget_s=20.0):
+    """The oracle as it stands, timed on this box's host cores on a bounded sample of the same workload:
+    seeded random rays for Ax and seeded random voxels (all views) for A^T b."""
+    from oracle import oracle as orc
+    ax_mode = orc.SIDDON if rec["ax"] == "siddon" else orc.INTERP
+    atb_mode = orc.MATCHED if rec["atb"] == "matched" else orc.FDK
+    nA = len(ang)
+    rng = np.random.default_rng(12345)
+    n_rays_total = nA * geo.nDetector[0] * geo.nDetector[1]
+    n_vox_total = int(np.prod(geo.nVoxel))
+    # calibrate on a small sample, then size the real one to ~budget/2 each
+    def run_ax(n):
+        ids = rng.integers(0, n_rays_total, n)
+        t = time.perf_counter()
+        _, info = orc.ax(vol_h, geo, ang, ax_mode, ray_ids=ids, info=True)
+        return time.perf_counter() - t, int(info["nseg"].sum())
+
+    def run_atb(n):
+        ids = rng.integers(0, n_vox_total, n)
+        t = time.perf_counter()
+        orc.atb(b_h, geo, ang, atb_mode, vox_ids=ids)
+        return time.perf_counter() - t, n * nA
+
+    t0, s0 = run_ax(2000)
+    n_ax = int(max(2000, min(5e6, 2000 * (budget_s / 2) / max(t0, 1e-3))))
+    t_ax, s_ax = run_ax(n_ax)
+    t0, u0 = run_atb(200)
+    n_atb = int(max(200, min(5e6, 200 * (budget_s / 2) / max(t0, 1e-3))))
+    t_atb, u_atb = run_atb(n_atb)
+    rate_ax, rate_atb = s_ax / t_ax, u_atb / t_atb
+    t_step = samples_per_step / rate_ax + updates_per_step / rate_atb
+    return {"value": (samples_per_step + updates_per_step) / t_step / 1e9, "unit": UNIT, "cores": orc.num_threads(),
+            "kind": "oracle",
+            "sample": f"{n_ax} seeded random rays ({s_ax} ray-samples, {t_ax:.1f} s) + {n_atb} seeded random voxels x "
+                      f"{nA} views ({u_atb} updates, {t_atb:.1f} s) of the same workload; full-step time extrapolated "
+                      f"linearly from the two rates",
+            "ax_gsamples_per_s": rate_ax / 1e9, "atb_gups": rate_atb / 1e9}, t_ax + t_atb
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C3")
+    ap.add_argument("--scale", type=int, default=1, help="geometric down-scaling of the config (debug only)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    K, W = max(1, args.steps), max(0, args.warmup)
+
+    geo, ang, rec = make_config(args.config, scale=args.scale)
+    nA = len(ang)
+    subsets = subsets_for(rec, nA)
+    workload = (f"{rec['name']}{'' if args.scale == 1 else '/' + str(args.scale)}: {geo.nVoxel[0]}^3 fp32 volume, {nA} views of "
+                f"{geo.nDetector[0]}x{geo.nDetector[1]}, {rec['ax']} Ax / {rec['atb']} A^T b, OS-SART with {len(subsets)} ordered subsets")
+    config = {"workload": workload, "phantom": rec["phantom"], "seed": rec["seed"],
+              "l2": "inputs larger than L2 (no flush needed)", "parallelism": "replicas only" if world > 1 else "single GPU"}
+
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        vol_h = phantom_for(rec, geo)
+        from oracle import oracle as orc
+        # projections for the A^T b sample: the oracle's own Ax is too slow at full size, so the sample uses
+        # seeded uniform-random projections of the right shape (timing does not depend on the values)
+        b_h = np.random.default_rng(rec["seed"]).random((nA, geo.nDetector[1], geo.nDetector[0]), dtype=np.float32)
+        n_rays = nA * geo.nDetector[0] * geo.nDetector[1]
+        ids = np.random.default_rng(1).integers(0, n_rays, 20000)
+        _, info = orc.ax(vol_h, geo, ang, orc.SIDDON if rec["ax"] == "siddon" else orc.INTERP, ray_ids=ids, info=True)
+        samples = float(info["nseg"].mean()) * n_rays
+        updates = float(np.prod(geo.nVoxel)) * nA
+        vals, t_all = [], 0.0
+        for i in range(W + K):
+            cb, t = cpu_baseline(geo, ang, rec, vol_h, b_h, samples, updates, budget_s=8.0)
+            if i >= W:
+                vals.append(cb)
+                t_all += t
+        v = float(np.mean([c["value"] for c in vals]))
+        cb = dict(vals[-1], value=v)
+        line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
+                "warmup": W, "ms_per_step": (samples + updates) / (v * 1e9) * 1e3, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config,
+                "cpu_baseline": cb, "gpu_launches": 0,
+                "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+        print(json.dumps(line))
+        return
+
+    import torch
+    import paper_2412_10129_b200 as tg
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (libtigre_b200 has no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    # ---- synthetic inputs (seeded)
+    vol_h = phantom_for(rec, geo)
+    vol = torch.from_numpy(vol_h).cuda()
+    b = tg.Ax(vol, geo, ang, rec["ax"])
+    if rec["name"] == "C3":           # Poisson noise on I0 = 1e5 then -log (configs[2]); timing input only
+        g = torch.Generator(device="cuda").manual_seed(rec["seed"])
+        counts = torch.poisson(1e5 * torch.exp(-b), generator=g)
+        b = -torch.log(torch.clamp(counts, min=1.0) / 1e5)
+        del counts
+    samples = tg.Ax_count(geo, ang, rec["ax"])
+    updates = int(np.prod(geo.nVoxel)) * nA
+    units = samples + updates
+
+    plan = tg.OssartPlan(geo, ang, subsets, rec["ax"], rec["atb"])
+    x = torch.zeros(geo.vol_shape, dtype=torch.float32, device="cuda")
+    for _ in range(W):
+        plan.iterate(b, x, 1, want_resid=False)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    barrier()
+    tg.profile(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(K):
+        plan.iterate(b, x, 1, want_resid=False)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    prof = tg.profile_read()
+    tg.profile(False)
+    sampler.stop_flag = True
+    sampler.join(timeout=2)
+    if world > 1:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_step = ms / K
+    value = world * units / (ms_step * 1e-3) / 1e9
+
+    # ---- end to end through the C ABI with HOST buffers: b and x in pinned host memory, copied in / out per step
+    e2e = None
+    if not args.no_e2e:
+        b_h = torch.empty(b.shape, dtype=torch.float32, pin_memory=True)
+        b_h.copy_(b)
+        x_h = torch.zeros(geo.vol_shape, dtype=torch.float32, pin_memory=True)
+        plan.iterate(b_h, x_h, 1, want_resid=False)
+        barrier()
+        t0 = torch.cuda.Event(enable_timing=True)
+        t1 = torch.cuda.Event(enable_timing=True)
+        t0.record()
+        for _ in range(K):
+            plan.iterate(b_h, x_h, 1, want_resid=False)
+        t1.record()
+        barrier()
+        ems = t0.elapsed_time(t1)
+        if world > 1:
+            t = torch.tensor([ems], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ems = float(t.item())
+        e2e = {"value": world * units / (ems / K * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ems / K,
+               "h2d_bytes_per_step": int(b_h.numel() * 4 + x_h.numel() * 4), "d2h_bytes_per_step": int(x_h.numel() * 4)}
+        del b_h
+
+    if rank != 0:
+        return
+    clocks = sampler.summary()
+    # ---- roofline of the dominant kernel (in-library CUDA events around every launch of the timed region)
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    kind = "ax" if prof["ms"]["ax"] >= prof["ms"]["atb"] else "atb"
+    kname = ("ax_" + rec["ax"]) if kind == "ax" else "atb"
+    k_units = samples if kind == "ax" else updates
+    k_ms = prof["ms"][kind] / K                       # per full pass over all views
+    achieved = k_units / (k_ms * 1e-3) / 1e9
+    peak = SM_COUNT * LANES_PER_CLK * sm_max * 1e6 / INSTR_PER_UNIT[kname] / 1e9
+    hbm_bytes = (vol.numel() + b.numel()) * 4         # compulsory: volume once + projections once
+    roofline = {"kernel": kname, "bound": "alu", "achieved": achieved, "peak": peak,
+                "unit": "Gsamples/s" if kind == "ax" else "Gupdates/s", "frac": achieved / peak, "traffic": None,
+                "peak_source": f"issue slots: {SM_COUNT} SMs x {LANES_PER_CLK} lanes/clk x {sm_max:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz) / "
+                               f"{INSTR_PER_UNIT[kname]} thread-instr per unit (ncu, profiles/)",
+                "share_of_step": prof["ms"][kind] / ms, "ms_per_pass": k_ms,
+                "hbm": {"algorithmic_bytes_per_pass": hbm_bytes, "achieved_gbs": hbm_bytes / (k_ms * 1e-3) / 1e9,
+                        "peak_gbs": peaks.get("hbm_gbs"), "note": "compulsory HBM traffic is ~1% of the time: not the bound"}}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic", "config": config, "clocks": clocks,
+            "ax_gsamples_per_s": samples / (prof["ms"]["ax"] / K * 1e-3) / 1e9,
+            "atb_gups": updates / (prof["ms"]["atb"] / K * 1e-3) / 1e9,
+            "kernel_ms_per_step": {k: v / K for k, v in prof["ms"].items()},
+            "units_per_step": {"ray_samples": samples, "voxel_updates": updates},
+            "gpu_launches": int(sum(prof["launches"].values())), "roofline": roofline}
+    if e2e:
+        line["e2e"] = e2e
+    if world == 1 and not args.no_cpu_baseline:
+        b_host = b.cpu().numpy()
+        line["cpu_baseline"], _ = cpu_baseline(geo, ang, rec, vol_h, b_host, samples, updates)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -44,10 +44,82 @@ __device__ __forceinline__ bool ax_decode(const AxP& p, int nViews, int& view, i
     return iu < p.nu && iv < p.nv;
 }
 
+// Per-ray marching state shared by the checked (end slabs) and unchecked (interior) slab steps.
+template <typename IdxT>
+struct SidRay {
+    float eref, fref, mE, mF, imE, imF, sgE, sgF;   // positions are volume-centred: e = xi_E - nE/2
+    IdxT stE, stF, sD;                              // signed element strides of one step along E, F, D
+    float nextE, nextF;                             // next E / F plane ahead of the ray
+    float kf, acc;
+    IdxT off;                                       // element offset of the current voxel
+};
+
+// One D-slab, interior of the volume: the whole slab [0,1] lies inside the ray's clipped range and at
+// least 1e-3 voxel away from the lateral faces, so no clipping and no bounds checks are needed.
+template <typename IdxT, bool UNIT>
+__device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base, SidRay<IdxT>& r) {
+    const float e0 = fmaf(r.kf, r.mE, r.eref), f0 = fmaf(r.kf, r.mF, r.fref);
+    r.kf += 1.0f;
+    // slab-local parameter of the next E / F plane crossing, saturated to [0,1] (1 = not in this slab)
+    const float se = __saturatef((r.nextE - e0) * r.imE);
+    const float sf = __saturatef((r.nextF - f0) * r.imF);
+    const bool cE = se < 1.0f, cF = sf < 1.0f;
+    const float s1 = fminf(se, sf);
+    const IdxT offC = r.off + (cE ? r.stE : (IdxT)0) + (cF ? r.stF : (IdxT)0);
+    const float vA = UNIT ? 1.f : __ldg(base + r.off);
+    const float vC = UNIT ? 1.f : __ldg(base + offC);
+    r.acc = fmaf(s1, vA, r.acc);
+    if (__any_sync(__activemask(), cE && cF)) {
+        // some lane crosses both planes inside this slab: a middle voxel between the two crossings
+        // (for a lane with a single crossing the middle voxel is the end voxel, so nothing changes)
+        const float s2 = fmaxf(se, sf);
+        const IdxT offB = r.off + ((se < sf) ? r.stE : r.stF);
+        const float vB = UNIT ? 1.f : __ldg(base + ((cE && cF) ? offB : offC));
+        r.acc = fmaf(s2 - s1, vB, r.acc);
+        r.acc = fmaf(1.0f - s2, vC, r.acc);
+    } else {
+        r.acc = fmaf(1.0f - s1, vC, r.acc);
+    }
+    if (cE) r.nextE += r.sgE;
+    if (cF) r.nextF += r.sgF;
+    r.off = offC + r.sD;
+}
+
+// One D-slab with clipping to [slo, shi] and per-voxel bounds checks (first / last slabs of a ray and
+// slabs that run within 1e-3 voxel of a lateral face).
+template <typename IdxT, bool UNIT>
+__device__ __forceinline__ void siddon_slab_checked(const float* __restrict__ base, SidRay<IdxT>& r, int& ie, int& jf,
+                                                    int diE, int diF, int nE, int nF, float slo, float shi) {
+    const float e0 = fmaf(r.kf, r.mE, r.eref), f0 = fmaf(r.kf, r.mF, r.fref);
+    r.kf += 1.0f;
+    const float se = __saturatef((r.nextE - e0) * r.imE);
+    const float sf = __saturatef((r.nextF - f0) * r.imF);
+    const bool cE = se < 1.0f, cF = sf < 1.0f;
+    const float s1 = fminf(fmaxf(fminf(se, sf), slo), shi);
+    const float s2 = fminf(fmaxf(fmaxf(se, sf), slo), shi);
+    const bool vEA = (unsigned)ie < (unsigned)nE, vFA = (unsigned)jf < (unsigned)nF;
+    const int ieC = cE ? ie + diE : ie, jfC = cF ? jf + diF : jf;
+    const IdxT offC = r.off + (cE ? r.stE : (IdxT)0) + (cF ? r.stF : (IdxT)0);
+    const bool vEC = (unsigned)ieC < (unsigned)nE, vFC = (unsigned)jfC < (unsigned)nF;
+    const bool eFirst = se < sf;
+    const IdxT offB = eFirst ? r.off + r.stE : r.off + r.stF;
+    const bool vB = eFirst ? (vEC && vFA) : (vEA && vFC);
+    const float lenA = s1 - slo, lenB = s2 - s1, lenC = shi - s2;
+    if (lenA > 0.f && vEA && vFA) r.acc = fmaf(lenA, UNIT ? 1.f : __ldg(base + r.off), r.acc);
+    if (cE && cF && lenB > 0.f && vB) r.acc = fmaf(lenB, UNIT ? 1.f : __ldg(base + offB), r.acc);
+    // with a single crossing [s1, shi] lies in the end voxel: lenB + lenC = shi - s1
+    const float lenE = (cE && cF) ? lenC : lenB + lenC;
+    if (lenE > 0.f && vEC && vFC) r.acc = fmaf(lenE, UNIT ? 1.f : __ldg(base + offC), r.acc);
+    if (cE) r.nextE += r.sgE;
+    if (cF) r.nextF += r.sgF;
+    ie = ieC, jf = jfC;
+    r.off = offC + r.sD;
+}
+
 template <typename IdxT, bool UNIT, bool COUNT>
 __global__ void __launch_bounds__(AX_TU* AX_TV)
-ax_siddon_kernel(const float* __restrict__ vol, const RayView* __restrict__ views, int nViews, AxP p,
-                 float* __restrict__ proj, uint32_t* __restrict__ counts) {
+ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, const RayView* __restrict__ views,
+                 int nViews, AxP p, float* __restrict__ proj, uint32_t* __restrict__ counts) {
     int view, iu, iv;
     if (!ax_decode(p, nViews, view, iu, iv)) return;
     const RayView& rv = views[view];
@@ -73,18 +145,31 @@ ax_siddon_kernel(const float* __restrict__ vol, const RayView* __restrict__ view
     uint32_t cnt = 0;
     if (dD != 0.0) {
         const double mE = dE / dD, mF = dF / dD;
-        // range of xi_D covered by the segment S->P, clipped to the volume box on all three axes
+        // range of xi_D covered by the segment S->P, clipped to the volume box on all three axes;
+        // [sa, sb]: sub-range that also stays >= margin away from the lateral faces (unchecked slabs)
+        const double margin = 1e-3;
         double lo = fmin(SD, SD + dD), hi = fmax(SD, SD + dD);
         lo = fmax(lo, 0.0), hi = fmin(hi, (double)nD);
+        double sa = lo, sb = hi;
         bool miss = false;
         if (mE != 0.0) {
             const double t1 = SD + (0.0 - SE) / mE, t2 = SD + ((double)nE - SE) / mE;
             lo = fmax(lo, fmin(t1, t2)), hi = fmin(hi, fmax(t1, t2));
-        } else if (SE < 0.0 || SE > (double)nE) miss = true;
+            const double u1 = SD + (margin - SE) / mE, u2 = SD + ((double)nE - margin - SE) / mE;
+            sa = fmax(sa, fmin(u1, u2)), sb = fmin(sb, fmax(u1, u2));
+        } else {
+            if (SE < 0.0 || SE > (double)nE) miss = true;
+            if (SE < margin || SE > (double)nE - margin) sb = sa - 1.0;
+        }
         if (mF != 0.0) {
             const double t1 = SD + (0.0 - SF) / mF, t2 = SD + ((double)nF - SF) / mF;
             lo = fmax(lo, fmin(t1, t2)), hi = fmin(hi, fmax(t1, t2));
-        } else if (SF < 0.0 || SF > (double)nF) miss = true;
+            const double u1 = SD + (margin - SF) / mF, u2 = SD + ((double)nF - margin - SF) / mF;
+            sa = fmax(sa, fmin(u1, u2)), sb = fmin(sb, fmax(u1, u2));
+        } else {
+            if (SF < 0.0 || SF > (double)nF) miss = true;
+            if (SF < margin || SF > (double)nF - margin) sb = sa - 1.0;
+        }
         if (!miss && hi > lo) {
             if (COUNT) {
                 // exact number of voxels met = |dix|+|diy|+|diz|+1 between entry and exit voxel
@@ -99,69 +184,50 @@ ax_siddon_kernel(const float* __restrict__ vol, const RayView* __restrict__ view
                 int i0 = (int)floor(lo), i1 = (int)ceil(hi);
                 i0 = max(i0, 0), i1 = min(i1, nD);
                 const int nslab = i1 - i0;
+                // unchecked slabs: k in [kA, kB), each fully inside [max(lo,sa), min(hi,sb)]
+                int kA = (int)ceil(fmax(lo, sa)) - i0, kB = (int)floor(fmin(hi, sb)) - i0;
+                kA = min(max(kA, 0), nslab), kB = min(max(kB, kA), nslab);
                 const int hE = nE >> 1, hF = nF >> 1;   // volume-centred coordinates: |e| <= n/2
                 // state at the START of slab i0 (s = 0), fp64: position, cell index, next plane ahead
                 const double eS = SE + ((double)i0 - SD) * mE, fS = SF + ((double)i0 - SD) * mF;
                 int ie = (int)floor(eS), jf = (int)floor(fS);
                 const bool upE = mE > 0.0, upF = mF > 0.0;
-                const float eref = (float)(eS - (double)hE), fref = (float)(fS - (double)hF);
-                const float mEf = (float)mE, mFf = (float)mF;
-                // slab-local parameter of the next E / F plane: s = (next - e0) / m, saturated to [0,1];
+                // x-dominant rays read the (x,y)-transposed copy so that neighbouring lanes (which differ
+                // mostly in y) touch neighbouring addresses
+                const bool useT = (D == 0) && (volT != nullptr);
+                const float* __restrict__ base = useT ? volT : vol;
+                const IdxT pX = useT ? (IdxT)p.ny : (IdxT)1, pY = useT ? (IdxT)1 : (IdxT)p.nx, pZ = (IdxT)p.nx * p.ny;
+                const IdxT sD = D == 0 ? pX : (D == 1 ? pY : pZ);
+                const IdxT sE = E == 0 ? pX : (E == 1 ? pY : pZ);
+                const IdxT sF = F == 0 ? pX : (F == 1 ? pY : pZ);
+                SidRay<IdxT> r;
+                r.eref = (float)(eS - (double)hE), r.fref = (float)(fS - (double)hF);
+                r.mE = (float)mE, r.mF = (float)mF;
                 // a ray parallel to the planes (m = 0) never crosses: next = +huge, 1/m := 1
-                const float imE = mE != 0.0 ? (float)(1.0 / mE) : 1.f, imF = mF != 0.0 ? (float)(1.0 / mF) : 1.f;
-                float nextE = mE != 0.0 ? (float)((upE ? ie + 1 : ie) - hE) : 3.0e38f;
-                float nextF = mF != 0.0 ? (float)((upF ? jf + 1 : jf) - hF) : 3.0e38f;
-                const float sgE = upE ? 1.f : -1.f, sgF = upF ? 1.f : -1.f;
-                const float slo0 = (float)(lo - (double)i0), shiN = (float)(hi - (double)(i1 - 1));
-                const IdxT sD = D == 0 ? 1 : (D == 1 ? (IdxT)p.nx : (IdxT)p.nx * p.ny);
-                const IdxT sE = E == 0 ? 1 : (E == 1 ? (IdxT)p.nx : (IdxT)p.nx * p.ny);
-                const IdxT sF = F == 0 ? 1 : (F == 1 ? (IdxT)p.nx : (IdxT)p.nx * p.ny);
-                const IdxT stE = upE ? sE : -sE, stF = upF ? sF : -sF;
+                r.imE = mE != 0.0 ? (float)(1.0 / mE) : 1.f, r.imF = mF != 0.0 ? (float)(1.0 / mF) : 1.f;
+                r.nextE = mE != 0.0 ? (float)((upE ? ie + 1 : ie) - hE) : 3.0e38f;
+                r.nextF = mF != 0.0 ? (float)((upF ? jf + 1 : jf) - hF) : 3.0e38f;
+                r.sgE = upE ? 1.f : -1.f, r.sgF = upF ? 1.f : -1.f;
+                r.stE = upE ? sE : -sE, r.stF = upF ? sF : -sF, r.sD = sD;
+                r.off = (IdxT)i0 * sD + (IdxT)ie * sE + (IdxT)jf * sF;   // may be out of range in checked slabs
+                r.kf = 0.f, r.acc = 0.f;
                 const int diE = upE ? 1 : -1, diF = upF ? 1 : -1;
-                IdxT off = (IdxT)i0 * sD + (IdxT)ie * sE + (IdxT)jf * sF;   // may be out of range: guarded below
-                float acc = 0.f;
-                float kf = 0.f;
+                const float slo0 = (float)(lo - (double)i0), shiN = (float)(hi - (double)(i1 - 1));
                 const int last = nslab - 1;
-                for (int k = 0; k < nslab; ++k) {
-                    const float e0 = fmaf(kf, mEf, eref), f0 = fmaf(kf, mFf, fref);
-                    kf += 1.0f;
-                    const float se = __saturatef((nextE - e0) * imE);
-                    const float sf = __saturatef((nextF - f0) * imF);
-                    const bool cE = se < 1.0f, cF = sf < 1.0f;
-                    float s1 = fminf(se, sf), s2 = fmaxf(se, sf);
-                    float slo = 0.f, shi = 1.f;
-                    if (k == 0 || k == last) {   // only the end slabs are clipped to the segment / box
-                        slo = (k == 0) ? slo0 : 0.f;
-                        shi = (k == last) ? shiN : 1.f;
-                        s1 = fminf(fmaxf(s1, slo), shi);
-                        s2 = fminf(fmaxf(s2, slo), shi);
+                int k = 0;
+                for (; k < kA; ++k)
+                    siddon_slab_checked<IdxT, UNIT>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
+                for (; k < kB; ++k) siddon_slab_fast<IdxT, UNIT>(base, r);
+                if (k < nslab) {
+                    // recover the cell indices from the plane state for the checked tail
+                    if (kB > kA) {
+                        if (mE != 0.0) ie = (int)r.nextE + hE - (upE ? 1 : 0);
+                        if (mF != 0.0) jf = (int)r.nextF + hF - (upF ? 1 : 0);
                     }
-                    const bool vEA = (unsigned)ie < (unsigned)nE, vFA = (unsigned)jf < (unsigned)nF;
-                    const int ieC = cE ? ie + diE : ie, jfC = cF ? jf + diF : jf;
-                    const IdxT offC = off + (cE ? stE : (IdxT)0) + (cF ? stF : (IdxT)0);
-                    const bool vEC = (unsigned)ieC < (unsigned)nE, vFC = (unsigned)jfC < (unsigned)nF;
-                    const float lenA = s1 - slo, lenC = shi - s2;
-                    if (lenA > 0.f && vEA && vFA) acc = fmaf(lenA, UNIT ? 1.f : __ldg(vol + off), acc);
-                    if (__any_sync(__activemask(), cE && cF)) {
-                        // some lane crosses both planes inside this slab: a middle voxel between the two crossings
-                        // (for a lane with one crossing the middle voxel IS the end voxel and lenC = 0)
-                        const float lenB = s2 - s1;
-                        const bool eFirst = se < sf;
-                        const IdxT offB = eFirst ? off + stE : off + stF;
-                        const bool vB = eFirst ? (vEC && vFA) : (vEA && vFC);
-                        if (lenB > 0.f && vB) acc = fmaf(lenB, UNIT ? 1.f : __ldg(vol + offB), acc);
-                        if (lenC > 0.f && vEC && vFC) acc = fmaf(lenC, UNIT ? 1.f : __ldg(vol + offC), acc);
-                    } else {
-                        // at most one crossing: [s1, shi] lies in the end voxel (s2 == shi when nothing else crosses)
-                        const float lenBC = shi - s1;
-                        if (lenBC > 0.f && vEC && vFC) acc = fmaf(lenBC, UNIT ? 1.f : __ldg(vol + offC), acc);
-                    }
-                    if (cE) nextE += sgE;
-                    if (cF) nextF += sgF;
-                    ie = ieC, jf = jfC;
-                    off = offC + sD;
+                    for (; k < nslab; ++k)
+                        siddon_slab_checked<IdxT, UNIT>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
                 }
-                result = acc * (float)(Lmm / fabs(dD));
+                result = r.acc * (float)(Lmm / fabs(dD));
             }
         }
     }
@@ -169,6 +235,22 @@ ax_siddon_kernel(const float* __restrict__ vol, const RayView* __restrict__ view
         counts[out] = cnt;
     } else {
         proj[out] = p.accumulate ? proj[out] + result : result;
+    }
+}
+
+// (x,y) transpose of every z-slice: volT[z][x][y] = vol[z][y][x]
+__global__ void __launch_bounds__(256) transpose_xy_kernel(const float* __restrict__ in, float* __restrict__ out, int nx, int ny) {
+    __shared__ float tile[32][33];
+    const size_t slice = (size_t)nx * ny * blockIdx.z;
+    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
+    for (int j = threadIdx.y; j < 32; j += 8) {
+        const int x = x0 + threadIdx.x, y = y0 + j;
+        if (x < nx && y < ny) tile[j][threadIdx.x] = in[slice + (size_t)y * nx + x];
+    }
+    __syncthreads();
+    for (int j = threadIdx.y; j < 32; j += 8) {
+        const int y = y0 + threadIdx.x, x = x0 + j;
+        if (x < nx && y < ny) out[slice + (size_t)x * ny + y] = tile[threadIdx.x][j];
     }
 }
 
@@ -269,15 +351,15 @@ ax_interp_kernel(const float* __restrict__ vol, const RayView* __restrict__ view
 }
 
 template <typename IdxT>
-static void ax_dispatch(const float* vol, const RayView* v, int nViews, const AxP& p, int mode, bool unit,
+static void ax_dispatch(const float* vol, const float* volT, const RayView* v, int nViews, const AxP& p, int mode, bool unit,
                         float* proj, uint32_t* counts, cudaStream_t st) {
     dim3 block(AX_TU, AX_TV);
     const long long nblk = (long long)p.nUt * p.nVt * nViews;
     dim3 grid((unsigned)nblk);
     if (mode == TIGRE_AX_SIDDON) {
-        if (counts) ax_siddon_kernel<IdxT, false, true><<<grid, block, 0, st>>>(vol, v, nViews, p, proj, counts);
-        else if (unit) ax_siddon_kernel<IdxT, true, false><<<grid, block, 0, st>>>(vol, v, nViews, p, proj, counts);
-        else ax_siddon_kernel<IdxT, false, false><<<grid, block, 0, st>>>(vol, v, nViews, p, proj, counts);
+        if (counts) ax_siddon_kernel<IdxT, false, true><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
+        else if (unit) ax_siddon_kernel<IdxT, true, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
+        else ax_siddon_kernel<IdxT, false, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
     } else {
         if (counts) ax_interp_kernel<IdxT, false, true><<<grid, block, 0, st>>>(vol, v, nViews, p, proj, counts);
         else if (unit) ax_interp_kernel<IdxT, true, false><<<grid, block, 0, st>>>(vol, v, nViews, p, proj, counts);
@@ -298,9 +380,20 @@ int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nView
     const long long nblk = (long long)p.nUt * p.nVt * nViews;
     if (nblk <= 0 || nblk > 0x7fffffffLL) return TIGRE_ERR_ARG;
     const size_t nvox = (size_t)g.nx * g.ny * g.nz;
-    ProfScope ps(PK_AX, st);
-    if (nvox < (1ull << 31)) ax_dispatch<int>(vol, d_views, nViews, p, mode, unit_vol, proj, count_out, st);
-    else ax_dispatch<long long>(vol, d_views, nViews, p, mode, unit_vol, proj, count_out, st);
+    // Siddon on real data: an (x,y)-transposed copy of the volume serves the x-dominant rays
+    TempBuf vt;
+    const float* volT = nullptr;
+    int launches = 1;
+    const bool wantT = (mode == TIGRE_AX_SIDDON) && !unit_vol && !count_out && vol && g.nx > 1 && g.ny > 1;
+    if (wantT && vt.alloc(nvox * sizeof(float), st) == TIGRE_OK) volT = vt.as<float>(), launches = 2;
+    ProfScope ps(PK_AX, st, launches);
+    if (volT) {
+        dim3 tb(32, 8), tg_((g.nx + 31) / 32, (g.ny + 31) / 32, g.nz);
+        if (tg_.y > 65535 || tg_.z > 65535) volT = nullptr;
+        else transpose_xy_kernel<<<tg_, tb, 0, st>>>(vol, vt.as<float>(), g.nx, g.ny);
+    }
+    if (nvox < (1ull << 31)) ax_dispatch<int>(vol, volT, d_views, nViews, p, mode, unit_vol, proj, count_out, st);
+    else ax_dispatch<long long>(vol, volT, d_views, nViews, p, mode, unit_vol, proj, count_out, st);
     TG_CUDA(cudaGetLastError());
     return TIGRE_OK;
 }
