@@ -116,6 +116,7 @@ struct Tables {
     std::vector<ViewH> views;
     Grid g;
     TempBuf ray, vox;
+    bool clamp = false;
     int build_ray(const int32_t* idx, int n, cudaStream_t st) {
         std::vector<RayView> h(n);
         for (int i = 0; i < n; ++i) build_ray_view(g, views[idx ? idx[i] : i], h[i]);
@@ -124,6 +125,7 @@ struct Tables {
     int build_vox(const int32_t* idx, int n, cudaStream_t st) {
         std::vector<VoxView> h(n);
         for (int i = 0; i < n; ++i) TG_TRY(build_vox_view(g, views[idx ? idx[i] : i], h[i]));
+        clamp = vox_needs_clamp(g, h.data(), n);
         return upload(vox, h.data(), sizeof(VoxView) * n, st);
     }
 };
@@ -144,7 +146,7 @@ static int device_ax(const float* vol, Tables& t, const int32_t* idx, int n, int
 static int device_atb(const float* proj, Tables& t, const int32_t* idx, int n, int mode, bool unit, float* vol,
                       cudaStream_t st) {
     TG_TRY(t.build_vox(idx, n, st));
-    return launch_atb(proj, t.g, t.vox.as<VoxView>(), n, mode, unit, vol, 0, t.g.nz, false, 0, t.g.nv, st);
+    return launch_atb(proj, t.g, t.vox.as<VoxView>(), n, mode, unit, vol, 0, t.g.nz, false, 0, t.g.nv, t.clamp, st);
 }
 
 }  // namespace tg
@@ -310,6 +312,7 @@ struct tigre_plan {
     std::vector<TempBuf> ray, vox;
     TempBuf W, V, Axb, grad, d_idx, d_acc;
     size_t bytes = 0;
+    bool clamp = false;
 };
 
 int tigre_plan_create(const tigre_geo* geo, const double* angles, int nA, const int32_t* subset_idx,
@@ -354,12 +357,13 @@ int tigre_plan_create(const tigre_geo* geo, const double* angles, int nA, const 
             TG_TRY(build_vox_view(g, P->t.views[idx[i]], hv[i]));
         }
         TG_TRY(upload(P->ray[s], hr.data(), sizeof(RayView) * n, st));
+        P->clamp = P->clamp || vox_needs_clamp(g, hv.data(), n);
         TG_TRY(upload(P->vox[s], hv.data(), sizeof(VoxView) * n, st));
         float* Ws = P->W.as<float>() + per * subset_off[s];
         float* Vs = P->V.as<float>() + nvox * s;
         TG_TRY(launch_ax(nullptr, g, P->ray[s].as<RayView>(), n, ax_mode, true, false, Ws, nullptr, st));
         TG_TRY(launch_invert_rows(Ws, per * n, (float)epsW, st));
-        TG_TRY(launch_atb(nullptr, g, P->vox[s].as<VoxView>(), n, atb_mode, true, Vs, 0, g.nz, false, 0, g.nv, st));
+        TG_TRY(launch_atb(nullptr, g, P->vox[s].as<VoxView>(), n, atb_mode, true, Vs, 0, g.nz, false, 0, g.nv, P->clamp, st));
         TG_TRY(launch_invert_cols(Vs, nvox, 1e-6f, st));
     }
     *out = P.release();
@@ -403,7 +407,7 @@ int tigre_plan_ossart(tigre_plan* P, const float* b, float* x, int n_iter, float
             TG_TRY(launch_ax(xd, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st));
             // r = W_s .* (b_s - A_s x) in place over A; b is gathered through the subset's view list
             TG_TRY(launch_residual(bd, P->d_idx.as<int32_t>() + P->off[s], A, Ws, A, per, n, P->d_acc.as<double>() + it, st));
-            TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>(), 0, g.nz, false, 0, g.nv, st));
+            TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>(), 0, g.nz, false, 0, g.nv, P->clamp, st));
             TG_TRY(launch_update(xd, P->grad.as<float>(), Vs, lambda, nonneg, nvox, st));
         }
     }
@@ -456,7 +460,7 @@ int tigre_cgls(const float* b, const tigre_geo* geo, const double* angles, int n
     const VoxView* vv = t.vox.as<VoxView>();
     TG_CUDA(cudaMemsetAsync(x, 0, sizeof(float) * nvox, st));
     TG_CUDA(cudaMemcpyAsync(r.p, b, sizeof(float) * np, cudaMemcpyDeviceToDevice, st));              // r = b - A 0
-    TG_TRY(launch_atb(r.as<float>(), g, vv, nA, atb_mode, false, s.as<float>(), 0, g.nz, false, 0, g.nv, st));
+    TG_TRY(launch_atb(r.as<float>(), g, vv, nA, atb_mode, false, s.as<float>(), 0, g.nz, false, 0, g.nv, t.clamp, st));
     TG_CUDA(cudaMemcpyAsync(p.p, s.p, sizeof(float) * nvox, cudaMemcpyDeviceToDevice, st));          // p = s
     TG_TRY(launch_dot(s.as<float>(), s.as<float>(), nvox, d + 0, st));                               // gamma
     for (int it = 0; it < n_iter; ++it) {
@@ -464,7 +468,7 @@ int tigre_cgls(const float* b, const tigre_geo* geo, const double* angles, int n
         TG_TRY(launch_dot(q.as<float>(), q.as<float>(), np, d + 2, st));
         TG_TRY(launch_axpy(x, p.as<float>(), d + 0, d + 2, 1.f, nvox, st));                          // x += alpha p
         TG_TRY(launch_axpy(r.as<float>(), q.as<float>(), d + 0, d + 2, -1.f, np, st));               // r -= alpha q
-        TG_TRY(launch_atb(r.as<float>(), g, vv, nA, atb_mode, false, s.as<float>(), 0, g.nz, false, 0, g.nv, st));
+        TG_TRY(launch_atb(r.as<float>(), g, vv, nA, atb_mode, false, s.as<float>(), 0, g.nz, false, 0, g.nv, t.clamp, st));
         TG_TRY(launch_dot(s.as<float>(), s.as<float>(), nvox, d + 1, st));                           // gamma'
         TG_TRY(launch_xpby(p.as<float>(), s.as<float>(), d + 1, d + 0, nvox, st));                   // p = s + beta p
         TG_CUDA(cudaMemcpyAsync(d + 0, d + 1, sizeof(double), cudaMemcpyDeviceToDevice, st));        // gamma = gamma'

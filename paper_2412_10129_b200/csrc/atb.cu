@@ -10,6 +10,7 @@
 //   atb_gather_kernel   any geometry; detector taps gathered through L1/L2 (general fall-back and
 //                       the path used when a view's footprint does not fit the staged box)
 //   atb_tma_kernel      (atb_tma.cu) footprints staged into shared memory by TMA
+#include <cmath>
 #include "common.cuh"
 
 namespace tg {
@@ -27,7 +28,57 @@ struct AtbP {
 
 constexpr int ATB_BX = 32, ATB_BY = 8;
 
-template <int MODE, bool UNIT, int ZR>
+// ---- arithmetic shared by the gather and the TMA kernels -------------------------------------
+// 1/x and sqrt(x) from the SFU approximations (max rel. error ~1 ulp / ~2 ulp): the IEEE sequences
+// cost 8-10 issue slots each and the kernels are issue-bound (profiles/r1_baseline_ncu_full.md).
+__device__ __forceinline__ float rcp_fast(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float sqrt_fast(float x) {
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+// floor(x) and its integer value for |x| < 2^21 without the conversion pipe: adding 1.5*2^23 leaves
+// round-to-nearest(x - 1/2) in the low mantissa bits.  At exact integers the result may be x-1 with
+// fraction 1, which gives the same bilinear value.  Callers clamp x when the geometry allows |x| >= 2^21.
+__device__ __forceinline__ float floor_magic(float x, int& i) {
+    const float m = 12582912.0f;   // 1.5 * 2^23 = 0x4B400000
+    const float t = (x - 0.5f) + m;
+    i = __float_as_int(t) - 0x4B400000;
+    return t - m;
+}
+
+struct TapW {   // per voxel-view: bilinear fractions, integer tap (detector index), weight
+    float au, av, w;
+    int iu, iv;
+};
+template <int MODE, bool CLAMP>
+__device__ __forceinline__ TapW voxel_view(float U, float V, float W, float G, const float4& cst, const AtbP& p) {
+    TapW o;
+    const float t = rcp_fast(W);
+    float fu = U * t, fv = V * t;   // detector index minus nu/2, nv/2
+    if (MODE == TIGRE_ATB_FDK) {
+        const float ig = rcp_fast(G);
+        o.w = ig * ig;
+    } else {
+        const float eu = fu - cst.z, ev = fv - cst.w;
+        o.w = (cst.x * t) * t * sqrt_fast(fmaf(p.du2 * eu, eu, fmaf(p.dv2 * ev, ev, cst.y)));
+    }
+    if (CLAMP) {
+        fu = fminf(fmaxf(fu, -2.0e6f), 2.0e6f);
+        fv = fminf(fmaxf(fv, -2.0e6f), 2.0e6f);
+    }
+    int iu, iv;
+    const float flu = floor_magic(fu, iu), flv = floor_magic(fv, iv);
+    o.au = fu - flu, o.av = fv - flv;
+    o.iu = iu + p.hu, o.iv = iv + p.hv;
+    return o;
+}
+
+template <int MODE, bool UNIT, bool CLAMP, int ZR>
 __global__ void __launch_bounds__(ATB_BX* ATB_BY)
 atb_gather_kernel(const float* __restrict__ proj, const VoxView* __restrict__ views, int nViews, AtbP p,
                   float* __restrict__ vol) {
@@ -40,6 +91,7 @@ atb_gather_kernel(const float* __restrict__ proj, const VoxView* __restrict__ vi
 #pragma unroll
     for (int k = 0; k < ZR; ++k) acc[k] = 0.f;
     const size_t per = (size_t)p.nu * p.nrows;
+    const unsigned nu1 = (unsigned)(p.nu - 1), nr1 = (unsigned)(p.nrows - 1);
     for (int a = 0; a < nViews; ++a) {
         const float4* vp = reinterpret_cast<const float4*>(views + a);
         const float4 rU = __ldg(vp), rV = __ldg(vp + 1), rW = __ldg(vp + 2), rG = __ldg(vp + 3), cst = __ldg(vp + 4);
@@ -51,37 +103,33 @@ atb_gather_kernel(const float* __restrict__ proj, const VoxView* __restrict__ vi
 #pragma unroll
         for (int k = 0; k < ZR; ++k) {
             const float kf = (float)k;
-            const float W = fmaf(kf, rW.z, W0);
-            const float t = 1.0f / W;
-            const float fu = fmaf(kf, rU.z, U0) * t, fv = fmaf(kf, rV.z, V0) * t;   // minus nu/2, nv/2
-            float w;
-            if (MODE == TIGRE_ATB_FDK) {
-                const float G = fmaf(kf, rG.z, G0);
-                const float ig = 1.0f / G;
-                w = ig * ig;
-            } else {
-                const float eu = fu - cst.z, ev = fv - cst.w;
-                w = cst.x * t * t * sqrtf(fmaf(p.du2 * eu, eu, fmaf(p.dv2 * ev, ev, cst.y)));
-            }
-            const float flu = floorf(fu), flv = floorf(fv);
-            const float au = fu - flu, av = fv - flv;
-            const int iu = (int)flu + p.hu, iv = (int)flv + p.hv;
-            // zero border on the true detector bounds
-            const bool u0 = (unsigned)iu < (unsigned)p.nu, u1 = (unsigned)(iu + 1) < (unsigned)p.nu;
-            const bool v0 = (unsigned)iv < (unsigned)p.nv, v1 = (unsigned)(iv + 1) < (unsigned)p.nv;
+            const TapW tw = voxel_view<MODE, CLAMP>(fmaf(kf, rU.z, U0), fmaf(kf, rV.z, V0), fmaf(kf, rW.z, W0),
+                                                    fmaf(kf, rG.z, G0), cst, p);
+            const int iu = tw.iu, iv = tw.iv;
             float val;
             if (UNIT) {
-                val = ((u0 ? 1.f - au : 0.f) + (u1 ? au : 0.f)) * ((v0 ? 1.f - av : 0.f) + (v1 ? av : 0.f));
+                // zero border on the true detector bounds: sum of the in-range tap weights
+                const bool u0 = (unsigned)iu < (unsigned)p.nu, u1 = (unsigned)(iu + 1) < (unsigned)p.nu;
+                const bool v0 = (unsigned)iv < (unsigned)p.nv, v1 = (unsigned)(iv + 1) < (unsigned)p.nv;
+                val = ((u0 ? 1.f - tw.au : 0.f) + (u1 ? tw.au : 0.f)) * ((v0 ? 1.f - tw.av : 0.f) + (v1 ? tw.av : 0.f));
             } else {
-                const float* q = pa + (ptrdiff_t)(iv - p.row0) * p.nu + iu;
-                const float p00 = (u0 && v0) ? __ldg(q) : 0.f;
-                const float p10 = (u1 && v0) ? __ldg(q + 1) : 0.f;
-                const float p01 = (u0 && v1) ? __ldg(q + p.nu) : 0.f;
-                const float p11 = (u1 && v1) ? __ldg(q + p.nu + 1) : 0.f;
-                const float r0 = fmaf(au, p10 - p00, p00), r1 = fmaf(au, p11 - p01, p01);
-                val = fmaf(av, r1 - r0, r0);
+                const int lv = iv - p.row0;
+                const float* q = pa + (ptrdiff_t)lv * p.nu + iu;
+                float p00, p10, p01, p11;
+                if ((unsigned)iu < nu1 && (unsigned)lv < nr1) {   // all four taps inside
+                    p00 = __ldg(q), p10 = __ldg(q + 1), p01 = __ldg(q + p.nu), p11 = __ldg(q + p.nu + 1);
+                } else {
+                    const bool u0 = (unsigned)iu < (unsigned)p.nu, u1 = (unsigned)(iu + 1) < (unsigned)p.nu;
+                    const bool v0 = (unsigned)lv < (unsigned)p.nrows, v1 = (unsigned)(lv + 1) < (unsigned)p.nrows;
+                    p00 = (u0 && v0) ? __ldg(q) : 0.f;
+                    p10 = (u1 && v0) ? __ldg(q + 1) : 0.f;
+                    p01 = (u0 && v1) ? __ldg(q + p.nu) : 0.f;
+                    p11 = (u1 && v1) ? __ldg(q + p.nu + 1) : 0.f;
+                }
+                const float r0 = fmaf(tw.au, p10 - p00, p00), r1 = fmaf(tw.au, p11 - p01, p01);
+                val = fmaf(tw.av, r1 - r0, r0);
             }
-            acc[k] = fmaf(w, val, acc[k]);
+            acc[k] = fmaf(tw.w, val, acc[k]);
         }
     }
     const size_t slice = (size_t)p.nx * p.ny;
@@ -94,8 +142,32 @@ atb_gather_kernel(const float* __restrict__ proj, const VoxView* __restrict__ vi
     }
 }
 
+// largest |fu|, |fv| any voxel of the box can reach (projective map with W > 0: extrema at the corners)
+bool vox_needs_clamp(const Grid& g, const VoxView* hv, int n) {
+    const double cx = 0.5 * g.nx, cy = 0.5 * g.ny, cz = 0.5 * g.nz;
+    for (int a = 0; a < n; ++a) {
+        const VoxView& v = hv[a];
+        for (int i = 0; i < 8; ++i) {
+            const double c[3] = {(i & 1) ? cx : -cx, (i & 2) ? cy : -cy, (i & 4) ? cz : -cz};
+            const double W = v.rowW[0] * c[0] + v.rowW[1] * c[1] + v.rowW[2] * c[2] + v.rowW[3];
+            const double U = v.rowU[0] * c[0] + v.rowU[1] * c[1] + v.rowU[2] * c[2] + v.rowU[3];
+            const double V = v.rowV[0] * c[0] + v.rowV[1] * c[1] + v.rowV[2] * c[2] + v.rowV[3];
+            if (!(W > 0.0) || std::fabs(U / W) > 1.0e6 || std::fabs(V / W) > 1.0e6) return true;
+        }
+    }
+    return false;
+}
+
+template <int MODE, bool UNIT>
+static void atb_gather_launch(dim3 grid, dim3 block, cudaStream_t st, bool clamp, const float* proj, const VoxView* v,
+                              int nViews, const AtbP& p, float* vol) {
+    constexpr int ZR = 8;
+    if (clamp) atb_gather_kernel<MODE, UNIT, true, ZR><<<grid, block, 0, st>>>(proj, v, nViews, p, vol);
+    else atb_gather_kernel<MODE, UNIT, false, ZR><<<grid, block, 0, st>>>(proj, v, nViews, p, vol);
+}
+
 int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nViews, int mode, bool unit_proj,
-               float* vol, int z0, int nzs, bool accumulate, int row0, int nrows, cudaStream_t st) {
+               float* vol, int z0, int nzs, bool accumulate, int row0, int nrows, bool clamp, cudaStream_t st) {
     if (mode != TIGRE_ATB_MATCHED && mode != TIGRE_ATB_FDK) return TIGRE_ERR_ARG;
     AtbP p;
     p.nx = g.nx, p.ny = g.ny, p.nz = g.nz, p.nu = g.nu, p.nv = g.nv;
@@ -110,11 +182,11 @@ int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nVi
     if (grid.y > 65535 || grid.z > 65535) return TIGRE_ERR_ARG;
     ProfScope ps(PK_ATB, st);
     if (unit_proj) {
-        if (mode == TIGRE_ATB_FDK) atb_gather_kernel<TIGRE_ATB_FDK, true, ZR><<<grid, block, 0, st>>>(proj, d_views, nViews, p, vol);
-        else atb_gather_kernel<TIGRE_ATB_MATCHED, true, ZR><<<grid, block, 0, st>>>(proj, d_views, nViews, p, vol);
+        if (mode == TIGRE_ATB_FDK) atb_gather_launch<TIGRE_ATB_FDK, true>(grid, block, st, clamp, proj, d_views, nViews, p, vol);
+        else atb_gather_launch<TIGRE_ATB_MATCHED, true>(grid, block, st, clamp, proj, d_views, nViews, p, vol);
     } else {
-        if (mode == TIGRE_ATB_FDK) atb_gather_kernel<TIGRE_ATB_FDK, false, ZR><<<grid, block, 0, st>>>(proj, d_views, nViews, p, vol);
-        else atb_gather_kernel<TIGRE_ATB_MATCHED, false, ZR><<<grid, block, 0, st>>>(proj, d_views, nViews, p, vol);
+        if (mode == TIGRE_ATB_FDK) atb_gather_launch<TIGRE_ATB_FDK, false>(grid, block, st, clamp, proj, d_views, nViews, p, vol);
+        else atb_gather_launch<TIGRE_ATB_MATCHED, false>(grid, block, st, clamp, proj, d_views, nViews, p, vol);
     }
     TG_CUDA(cudaGetLastError());
     return TIGRE_OK;

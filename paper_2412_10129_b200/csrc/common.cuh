@@ -104,7 +104,9 @@ int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nView
 //   unit_proj: treat projections as all ones (column sums A^T 1), proj may be NULL
 //   row0/nrows: the projection buffer holds detector rows [row0,row0+nrows) only (chunked path)
 int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nViews, int mode, bool unit_proj,
-               float* vol, int z0, int nzs, bool accumulate, int row0, int nrows, cudaStream_t st);
+               float* vol, int z0, int nzs, bool accumulate, int row0, int nrows, bool clamp, cudaStream_t st);
+// true if some voxel of the box can project beyond |index| 1e6 in some view (then the kernels clamp)
+bool vox_needs_clamp(const Grid& g, const VoxView* host_views, int n);
 
 // elementwise
 int launch_residual(const float* b, const int32_t* view_idx, const float* Ax, const float* W, float* r,
