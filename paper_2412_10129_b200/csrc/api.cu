@@ -130,12 +130,15 @@ struct Tables {
     }
 };
 
-static int prep(const tigre_geo* geo, const double* angles, int nA, Tables& t) {
+int tables_prep(const tigre_geo* geo, const double* angles, int nA, Grid& g, std::vector<ViewH>& views) {
     TG_TRY(validate_geo(geo, angles, nA));
     TG_TRY(ensure_device());
-    t.g = make_grid(geo);
-    resolve_views(geo, angles, nA, t.views);
+    g = make_grid(geo);
+    resolve_views(geo, angles, nA, views);
     return TIGRE_OK;
+}
+static int prep(const tigre_geo* geo, const double* angles, int nA, Tables& t) {
+    return tables_prep(geo, angles, nA, t.g, t.views);
 }
 
 static int device_ax(const float* vol, Tables& t, const int32_t* idx, int n, int mode, bool unit, float* proj,

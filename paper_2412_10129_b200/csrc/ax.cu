@@ -24,6 +24,8 @@ struct AxP {
     double hxd, hyd, hzd;
     double delta;         // interpolated step, mm
     int nUt, nVt;         // tiles per view
+    int iv0, iv1;         // detector rows computed: [iv0, iv1)
+    int zs0, zs1;         // interpolated mode: z-slices present in `vol` (which points at slice zs0)
     int accumulate;
 };
 
@@ -40,8 +42,8 @@ __device__ __forceinline__ bool ax_decode(const AxP& p, int nViews, int& view, i
     view = (int)(t % nViews);
     int vt = (int)(t / nViews);
     iu = ut * AX_TU + threadIdx.x;
-    iv = vt * AX_TV + threadIdx.y;
-    return iu < p.nu && iv < p.nv;
+    iv = p.iv0 + vt * AX_TV + threadIdx.y;
+    return iu < p.nu && iv < p.iv1;
 }
 
 // Per-ray marching state shared by the checked (end slabs) and unchecked (interior) slab steps.
@@ -303,9 +305,23 @@ ax_interp_kernel(const float* __restrict__ vol, const RayView* __restrict__ view
                 const IdxT pitchY = p.nx, pitchZ = (IdxT)p.nx * p.ny;
                 // samples beyond the detector end of the segment are dropped (l_k > |p-S|)
                 const long long Kmax = (long long)floor((Lmm - lin) / p.delta - 0.5) + 1;
-                const int Kuse = (int)min(K, max(Kmax, 0LL));
+                int Kuse = (int)min(K, max(Kmax, 0LL)), k0 = 0;
+                if (p.zs0 > 0 || p.zs1 < p.nz) {
+                    // only a z-slab of the volume is present: skip the samples none of whose taps can lie in
+                    // it (conservative by one sample and 0.01 voxel; taps are bounds-checked anyway)
+                    const float za = (float)(p.zs0 - hz) - 1.01f, zb = (float)(p.zs1 - hz) + 0.01f;
+                    if (fabsf(sz) > 1e-9f) {
+                        const float ka = (za - z0) / sz - 0.5f, kb = (zb - z0) / sz - 0.5f;
+                        const float klo = fminf(fmaxf(fminf(ka, kb), -1.f), (float)Kuse + 1.f);
+                        const float khi = fminf(fmaxf(fmaxf(ka, kb), -1.f), (float)Kuse + 1.f);
+                        k0 = max((int)floorf(klo) - 1, 0);
+                        Kuse = min((int)ceilf(khi) + 2, Kuse);
+                    } else if (z0 < za - 1.f || z0 > zb + 1.f) {
+                        Kuse = 0;
+                    }
+                }
                 float acc = 0.f;
-                for (int k = 0; k < Kuse; ++k) {
+                for (int k = k0; k < Kuse; ++k) {
                     const float t = (float)k + 0.5f;
                     const float x = fmaf(t, sx, x0), y = fmaf(t, sy, y0), z = fmaf(t, sz, z0);
                     const float fx = floorf(x), fy = floorf(y), fz = floorf(z);
@@ -315,10 +331,11 @@ ax_interp_kernel(const float* __restrict__ vol, const RayView* __restrict__ view
                     if (UNIT) {
                         const float wx = ((unsigned)ix < (unsigned)p.nx ? 1.f - ax : 0.f) + ((unsigned)(ix + 1) < (unsigned)p.nx ? ax : 0.f);
                         const float wy = ((unsigned)iy < (unsigned)p.ny ? 1.f - ay : 0.f) + ((unsigned)(iy + 1) < (unsigned)p.ny ? ay : 0.f);
-                        const float wz = ((unsigned)iz < (unsigned)p.nz ? 1.f - az : 0.f) + ((unsigned)(iz + 1) < (unsigned)p.nz ? az : 0.f);
+                        const float wz = ((unsigned)(iz - p.zs0) < (unsigned)(p.zs1 - p.zs0) ? 1.f - az : 0.f) +
+                                         ((unsigned)(iz + 1 - p.zs0) < (unsigned)(p.zs1 - p.zs0) ? az : 0.f);
                         v = wx * wy * wz;
-                    } else if (ix >= 0 && ix + 1 < p.nx && iy >= 0 && iy + 1 < p.ny && iz >= 0 && iz + 1 < p.nz) {
-                        const float* q = vol + ((IdxT)iz * pitchZ + (IdxT)iy * pitchY + ix);
+                    } else if (ix >= 0 && ix + 1 < p.nx && iy >= 0 && iy + 1 < p.ny && iz >= p.zs0 && iz + 1 < p.zs1) {
+                        const float* q = vol + ((IdxT)(iz - p.zs0) * pitchZ + (IdxT)iy * pitchY + ix);
                         const float v000 = __ldg(q), v100 = __ldg(q + 1);
                         const float v010 = __ldg(q + pitchY), v110 = __ldg(q + pitchY + 1);
                         const float v001 = __ldg(q + pitchZ), v101 = __ldg(q + pitchZ + 1);
@@ -331,9 +348,10 @@ ax_interp_kernel(const float* __restrict__ vol, const RayView* __restrict__ view
 #pragma unroll
                         for (int c = 0; c < 8; ++c) {
                             const int jx = ix + (c & 1), jy = iy + ((c >> 1) & 1), jz = iz + (c >> 2);
-                            if ((unsigned)jx < (unsigned)p.nx && (unsigned)jy < (unsigned)p.ny && (unsigned)jz < (unsigned)p.nz) {
+                            if ((unsigned)jx < (unsigned)p.nx && (unsigned)jy < (unsigned)p.ny &&
+                                (unsigned)(jz - p.zs0) < (unsigned)(p.zs1 - p.zs0)) {
                                 const float w = ((c & 1) ? ax : 1.f - ax) * ((c & 2) ? ay : 1.f - ay) * ((c & 4) ? az : 1.f - az);
-                                v = fmaf(w, __ldg(vol + ((IdxT)jz * pitchZ + (IdxT)jy * pitchY + jx)), v);
+                                v = fmaf(w, __ldg(vol + ((IdxT)(jz - p.zs0) * pitchZ + (IdxT)jy * pitchY + jx)), v);
                             }
                         }
                     }
@@ -368,14 +386,19 @@ static void ax_dispatch(const float* vol, const float* volT, const RayView* v, i
 }
 
 int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nViews, int mode, bool unit_vol,
-              bool accumulate, float* proj, uint32_t* count_out, cudaStream_t st) {
+              bool accumulate, float* proj, uint32_t* count_out, cudaStream_t st, const AxSub* sub) {
     if (mode != TIGRE_AX_SIDDON && mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
+    if (sub && (sub->row0 < 0 || sub->row0 + sub->nrows > g.nv || sub->zs0 < 0 || sub->zs0 + sub->nzs > g.nz)) return TIGRE_ERR_ARG;
+    if (sub && (sub->nrows <= 0 || sub->nzs <= 0)) return TIGRE_OK;   // nothing of this slab reaches the detector
     AxP p;
     p.nx = g.nx, p.ny = g.ny, p.nz = g.nz, p.nu = g.nu, p.nv = g.nv;
     p.hx = (float)g.dx, p.hy = (float)g.dy, p.hz = (float)g.dz;
     p.hxd = g.dx, p.hyd = g.dy, p.hzd = g.dz;
     p.delta = g.accuracy * fmin(g.dx, fmin(g.dy, g.dz));
-    p.nUt = (g.nu + AX_TU - 1) / AX_TU, p.nVt = (g.nv + AX_TV - 1) / AX_TV;
+    p.iv0 = sub ? sub->row0 : 0, p.iv1 = sub ? sub->row0 + sub->nrows : g.nv;
+    p.zs0 = sub ? sub->zs0 : 0, p.zs1 = sub ? sub->zs0 + sub->nzs : g.nz;
+    if (mode == TIGRE_AX_SIDDON && (p.zs0 != 0 || p.zs1 != g.nz)) return TIGRE_ERR_ARG;   // Siddon slabs are sub-grids
+    p.nUt = (g.nu + AX_TU - 1) / AX_TU, p.nVt = (p.iv1 - p.iv0 + AX_TV - 1) / AX_TV;
     p.accumulate = accumulate ? 1 : 0;
     const long long nblk = (long long)p.nUt * p.nVt * nViews;
     if (nblk <= 0 || nblk > 0x7fffffffLL) return TIGRE_ERR_ARG;

@@ -64,6 +64,8 @@ void resolve_views(const tigre_geo* geo, const double* angles, int nA, std::vect
 void build_ray_view(const Grid& g, const ViewH& v, RayView& r);
 // returns TIGRE_ERR_GEOMETRY if a corner of the (z-restricted) volume is at/behind the source
 int build_vox_view(const Grid& g, const ViewH& v, VoxView& o);
+// detector rows the z-slices [z0,z0+nzs) can reach in view v (with the interpolation support and slack)
+void row_band(const Grid& g, const ViewH& v, int z0, int nzs, int& row0, int& nrows);
 
 // ---------------------------------------------------------------- stream-ordered temporaries
 struct TempBuf {  // RAII: cudaMallocAsync / cudaFreeAsync on one stream
@@ -97,8 +99,13 @@ struct ProfScope {
 //   unit_vol: treat the volume as all ones (row sums A 1), vol may be NULL
 //   count_out: if non-NULL, write per-ray sample counts instead of projecting (measurement helper)
 //   accumulate: proj += instead of proj = (partial projections of a z-slab, chunked path)
+//   sub (chunked path): compute detector rows [row0,row0+nrows) only; interpolated mode: `vol` holds the
+//   z-slices [zs0,zs0+nzs) of a volume of height g.nz and points at slice zs0 (other slices count as 0)
+struct AxSub {
+    int row0, nrows, zs0, nzs;
+};
 int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nViews, int mode, bool unit_vol,
-              bool accumulate, float* proj, uint32_t* count_out, cudaStream_t st);
+              bool accumulate, float* proj, uint32_t* count_out, cudaStream_t st, const AxSub* sub = nullptr);
 // backprojection of nViews views given their VoxView table (device) into z-slices [z0, z0+nzs) of a
 // volume whose full height is g.nz; vol points at slice z0.  accumulate: vol += instead of vol =.
 //   unit_proj: treat projections as all ones (column sums A^T 1), proj may be NULL
@@ -130,5 +137,6 @@ int chunked_ax(const float* h_vol, const tigre_geo* geo, const double* angles, i
 int chunked_atb(const float* h_proj, const tigre_geo* geo, const double* angles, int nA, int mode, float* h_vol,
                 cudaStream_t st);
 size_t chunk_budget();
+int tables_prep(const tigre_geo* geo, const double* angles, int nA, Grid& g, std::vector<ViewH>& views);
 
 }  // namespace tg

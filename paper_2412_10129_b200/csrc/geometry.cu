@@ -107,7 +107,12 @@ void build_ray_view(const Grid& g, const ViewH& v, RayView& r) {
     }
 }
 
-int build_vox_view(const Grid& g, const ViewH& v, VoxView& o) {
+// fp64 rows of the voxel -> detector map of one view (see VoxView in common.cuh); also the detector-frame
+// source s (s[0] = distance source -> detector plane) and the scanner-frame x of the volume centre.
+struct VoxRows {
+    double rowU[4], rowV[4], rowW[4], rowG[4], s[3];
+};
+static int build_vox_rows(const Grid& g, const ViewH& v, VoxRows& R) {
     const M3 RgT = transpose(gantry(v)), RdT = transpose(detrot(v));
     const double h[3] = {g.dx, g.dy, g.dz};
     // q(c) = M c + q0 : detector-frame position of the voxel with centred index c
@@ -120,10 +125,11 @@ int build_vox_view(const Grid& g, const ViewH& v, VoxView& o) {
     const double Dc[3] = {v.DSO - v.DSD, v.offD[0], v.offD[1]};
     double a0[3] = {xo[0] - Dc[0], xo[1] - Dc[1], xo[2] - Dc[2]}, q0[3];
     apply(RdT, a0, q0);
-    double b0[3] = {v.DSO - Dc[0], -Dc[1], -Dc[2]}, s[3];
+    double b0[3] = {v.DSO - Dc[0], -Dc[1], -Dc[2]};
+    double* s = R.s;
     apply(RdT, b0, s);
     if (!(s[0] > 0.0)) return TIGRE_ERR_GEOMETRY;
-    double rowW[4], rowU[4], rowV[4], rowG[4];
+    double *rowW = R.rowW, *rowU = R.rowU, *rowV = R.rowV, *rowG = R.rowG;
     for (int k = 0; k < 3; ++k) rowW[k] = -M.m[0][k] / s[0];
     rowW[3] = 1.0 - q0[0] / s[0];
     // u*W = s_y*W + (q_y - s_y);  fu = u/du + (nu-1)/2;  fuh = fu - nu/2 = u/du + offU
@@ -134,6 +140,37 @@ int build_vox_view(const Grid& g, const ViewH& v, VoxView& o) {
     rowV[3] = (s[2] * rowW[3] + q0[2] - s[2]) / g.dv + offV * rowW[3];
     for (int k = 0; k < 3; ++k) rowG[k] = -A.m[0][k] / v.DSO;
     rowG[3] = (v.DSO - xo[0]) / v.DSO;
+    return TIGRE_OK;
+}
+
+// Detector rows [row0, row0+nrows) that the z-slices [z0, z0+nzs) of the volume can reach in view v:
+// the projective map is quasi-linear where W > 0, so the extrema of fv over the slab box (grown by one
+// voxel: trilinear support, bilinear taps) are at its corners.  Any corner at W <= 0: all rows.
+void row_band(const Grid& g, const ViewH& v, int z0, int nzs, int& row0, int& nrows) {
+    row0 = 0, nrows = g.nv;
+    VoxRows R;
+    if (build_vox_rows(g, v, R) != TIGRE_OK) return;
+    const double cx = 0.5 * g.nx + 1.0, cy = 0.5 * g.ny + 1.0;
+    const double za = (double)z0 - 0.5 * g.nz - 1.0, zb = (double)(z0 + nzs) - 0.5 * g.nz + 1.0;
+    double lo = 1e300, hi = -1e300;
+    for (int i = 0; i < 8; ++i) {
+        const double c[3] = {(i & 1) ? cx : -cx, (i & 2) ? cy : -cy, (i & 4) ? zb : za};
+        const double W = R.rowW[0] * c[0] + R.rowW[1] * c[1] + R.rowW[2] * c[2] + R.rowW[3];
+        const double V = R.rowV[0] * c[0] + R.rowV[1] * c[1] + R.rowV[2] * c[2] + R.rowV[3];
+        if (!(W > 1e-9)) return;
+        lo = std::fmin(lo, V / W), hi = std::fmax(hi, V / W);
+    }
+    // fv = (V/W) + nv/2 is the continuous row index; taps floor(fv), floor(fv)+1; one row of slack
+    const double a = std::floor(lo + (double)(g.nv / 2)) - 1.0, b = std::ceil(hi + (double)(g.nv / 2)) + 2.0;
+    const int r0 = (int)std::fmax(0.0, std::fmin(a, (double)g.nv)), r1 = (int)std::fmax(0.0, std::fmin(b, (double)g.nv));
+    row0 = r0, nrows = r1 > r0 ? r1 - r0 : 0;
+}
+
+int build_vox_view(const Grid& g, const ViewH& v, VoxView& o) {
+    VoxRows R;
+    TG_TRY(build_vox_rows(g, v, R));
+    const double *rowW = R.rowW, *rowU = R.rowU, *rowV = R.rowV, *rowG = R.rowG, *s = R.s;
+    const double offU = 0.5 * (g.nu - 1) - (double)(g.nu / 2), offV = 0.5 * (g.nv - 1) - (double)(g.nv / 2);
     // every corner of the volume box must be in front of the source (W>0, G>0)
     const double cx = 0.5 * g.nx, cy = 0.5 * g.ny, cz = 0.5 * g.nz;
     for (int i = 0; i < 8; ++i) {
