@@ -120,6 +120,7 @@ def main():
     ap.add_argument("--config", default="C3")
     ap.add_argument("--scale", type=int, default=1, help="geometric down-scaling of the config (debug only)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--atb-kernel", default="tma", choices=["tma", "gather"], help="A/B switch of the A^T b kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -169,6 +170,8 @@ def main():
     import paper_2412_10129_b200 as tg
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (libtigre_b200 has no CPU fallback)"
     torch.cuda.set_device(local_rank)
+    tg.set_atb_path(0 if args.atb_kernel == "tma" else 1)
+    config["atb_kernel"] = args.atb_kernel
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))

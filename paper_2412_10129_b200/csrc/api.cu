@@ -116,6 +116,7 @@ struct Tables {
     std::vector<ViewH> views;
     Grid g;
     TempBuf ray, vox;
+    std::vector<VoxView> hvox;   // host copy of the table in `vox` (sizes the TMA boxes)
     bool clamp = false;
     int build_ray(const int32_t* idx, int n, cudaStream_t st) {
         std::vector<RayView> h(n);
@@ -123,7 +124,8 @@ struct Tables {
         return upload(ray, h.data(), sizeof(RayView) * n, st);
     }
     int build_vox(const int32_t* idx, int n, cudaStream_t st) {
-        std::vector<VoxView> h(n);
+        std::vector<VoxView>& h = hvox;
+        h.resize(n);
         for (int i = 0; i < n; ++i) TG_TRY(build_vox_view(g, views[idx ? idx[i] : i], h[i]));
         clamp = vox_needs_clamp(g, h.data(), n);
         return upload(vox, h.data(), sizeof(VoxView) * n, st);
@@ -149,7 +151,8 @@ static int device_ax(const float* vol, Tables& t, const int32_t* idx, int n, int
 static int device_atb(const float* proj, Tables& t, const int32_t* idx, int n, int mode, bool unit, float* vol,
                       cudaStream_t st) {
     TG_TRY(t.build_vox(idx, n, st));
-    return launch_atb(proj, t.g, t.vox.as<VoxView>(), n, mode, unit, vol, 0, t.g.nz, false, 0, t.g.nv, t.clamp, st);
+    return launch_atb(proj, t.g, t.vox.as<VoxView>(), n, mode, unit, vol, 0, t.g.nz, false, 0, t.g.nv, t.clamp, st,
+                      t.hvox.data());
 }
 
 }  // namespace tg
@@ -313,6 +316,7 @@ struct tigre_plan {
     int nA = 0, nSubsets = 0, maxs = 0, ax_mode = 0, atb_mode = 0;
     std::vector<int32_t> idx, off;
     std::vector<TempBuf> ray, vox;
+    std::vector<std::vector<VoxView>> hvox;
     TempBuf W, V, Axb, grad, d_idx, d_acc;
     size_t bytes = 0;
     bool clamp = false;
@@ -349,12 +353,14 @@ int tigre_plan_create(const tigre_geo* geo, const double* angles, int nA, const 
     P->bytes = sizeof(float) * (per * nIdx + nvox * nSubsets + per * P->maxs + nvox);
     P->ray = std::vector<TempBuf>(nSubsets);
     P->vox = std::vector<TempBuf>(nSubsets);
+    P->hvox.resize(nSubsets);
     const double epsW = 1e-2 * std::min(g.dx, std::min(g.dy, g.dz));
     for (int s = 0; s < nSubsets; ++s) {
         const int32_t* idx = subset_idx + subset_off[s];
         const int n = subset_off[s + 1] - subset_off[s];
         std::vector<RayView> hr(n);
-        std::vector<VoxView> hv(n);
+        std::vector<VoxView>& hv = P->hvox[s];
+        hv.resize(n);
         for (int i = 0; i < n; ++i) {
             build_ray_view(g, P->t.views[idx[i]], hr[i]);
             TG_TRY(build_vox_view(g, P->t.views[idx[i]], hv[i]));
@@ -410,7 +416,8 @@ int tigre_plan_ossart(tigre_plan* P, const float* b, float* x, int n_iter, float
             TG_TRY(launch_ax(xd, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st));
             // r = W_s .* (b_s - A_s x) in place over A; b is gathered through the subset's view list
             TG_TRY(launch_residual(bd, P->d_idx.as<int32_t>() + P->off[s], A, Ws, A, per, n, P->d_acc.as<double>() + it, st));
-            TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>(), 0, g.nz, false, 0, g.nv, P->clamp, st));
+            TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>(), 0, g.nz, false, 0, g.nv, P->clamp, st,
+                              P->hvox[s].data()));
             TG_TRY(launch_update(xd, P->grad.as<float>(), Vs, lambda, nonneg, nvox, st));
         }
     }
@@ -463,7 +470,7 @@ int tigre_cgls(const float* b, const tigre_geo* geo, const double* angles, int n
     const VoxView* vv = t.vox.as<VoxView>();
     TG_CUDA(cudaMemsetAsync(x, 0, sizeof(float) * nvox, st));
     TG_CUDA(cudaMemcpyAsync(r.p, b, sizeof(float) * np, cudaMemcpyDeviceToDevice, st));              // r = b - A 0
-    TG_TRY(launch_atb(r.as<float>(), g, vv, nA, atb_mode, false, s.as<float>(), 0, g.nz, false, 0, g.nv, t.clamp, st));
+    TG_TRY(launch_atb(r.as<float>(), g, vv, nA, atb_mode, false, s.as<float>(), 0, g.nz, false, 0, g.nv, t.clamp, st, t.hvox.data()));
     TG_CUDA(cudaMemcpyAsync(p.p, s.p, sizeof(float) * nvox, cudaMemcpyDeviceToDevice, st));          // p = s
     TG_TRY(launch_dot(s.as<float>(), s.as<float>(), nvox, d + 0, st));                               // gamma
     for (int it = 0; it < n_iter; ++it) {
@@ -471,7 +478,7 @@ int tigre_cgls(const float* b, const tigre_geo* geo, const double* angles, int n
         TG_TRY(launch_dot(q.as<float>(), q.as<float>(), np, d + 2, st));
         TG_TRY(launch_axpy(x, p.as<float>(), d + 0, d + 2, 1.f, nvox, st));                          // x += alpha p
         TG_TRY(launch_axpy(r.as<float>(), q.as<float>(), d + 0, d + 2, -1.f, np, st));               // r -= alpha q
-        TG_TRY(launch_atb(r.as<float>(), g, vv, nA, atb_mode, false, s.as<float>(), 0, g.nz, false, 0, g.nv, t.clamp, st));
+        TG_TRY(launch_atb(r.as<float>(), g, vv, nA, atb_mode, false, s.as<float>(), 0, g.nz, false, 0, g.nv, t.clamp, st, t.hvox.data()));
         TG_TRY(launch_dot(s.as<float>(), s.as<float>(), nvox, d + 1, st));                           // gamma'
         TG_TRY(launch_xpby(p.as<float>(), s.as<float>(), d + 1, d + 0, nvox, st));                   // p = s + beta p
         TG_CUDA(cudaMemcpyAsync(d + 0, d + 1, sizeof(double), cudaMemcpyDeviceToDevice, st));        // gamma = gamma'

@@ -11,72 +11,9 @@
 //                       the path used when a view's footprint does not fit the staged box)
 //   atb_tma_kernel      (atb_tma.cu) footprints staged into shared memory by TMA
 #include <cmath>
-#include "common.cuh"
+#include "atb_common.cuh"
 
 namespace tg {
-
-struct AtbP {
-    int nx, ny, nz;       // full volume size (centred coordinates refer to it)
-    int nu, nv;
-    int z0, nzs;          // z-slices written: [z0, z0+nzs); vol points at slice z0
-    int row0, nrows;      // detector rows present in the projection buffer
-    float cx, cy, cz;     // (n-1)/2
-    float du2, dv2;       // pixel pitch squared, mm^2
-    int hu, hv;           // nu/2, nv/2
-    int accumulate;
-};
-
-constexpr int ATB_BX = 32, ATB_BY = 8;
-
-// ---- arithmetic shared by the gather and the TMA kernels -------------------------------------
-// 1/x and sqrt(x) from the SFU approximations (max rel. error ~1 ulp / ~2 ulp): the IEEE sequences
-// cost 8-10 issue slots each and the kernels are issue-bound (profiles/r1_baseline_ncu_full.md).
-__device__ __forceinline__ float rcp_fast(float x) {
-    float r;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-__device__ __forceinline__ float sqrt_fast(float x) {
-    float r;
-    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-// floor(x) and its integer value for |x| < 2^21 without the conversion pipe: adding 1.5*2^23 leaves
-// round-to-nearest(x - 1/2) in the low mantissa bits.  At exact integers the result may be x-1 with
-// fraction 1, which gives the same bilinear value.  Callers clamp x when the geometry allows |x| >= 2^21.
-__device__ __forceinline__ float floor_magic(float x, int& i) {
-    const float m = 12582912.0f;   // 1.5 * 2^23 = 0x4B400000
-    const float t = (x - 0.5f) + m;
-    i = __float_as_int(t) - 0x4B400000;
-    return t - m;
-}
-
-struct TapW {   // per voxel-view: bilinear fractions, integer tap (detector index), weight
-    float au, av, w;
-    int iu, iv;
-};
-template <int MODE, bool CLAMP>
-__device__ __forceinline__ TapW voxel_view(float U, float V, float W, float G, const float4& cst, const AtbP& p) {
-    TapW o;
-    const float t = rcp_fast(W);
-    float fu = U * t, fv = V * t;   // detector index minus nu/2, nv/2
-    if (MODE == TIGRE_ATB_FDK) {
-        const float ig = rcp_fast(G);
-        o.w = ig * ig;
-    } else {
-        const float eu = fu - cst.z, ev = fv - cst.w;
-        o.w = (cst.x * t) * t * sqrt_fast(fmaf(p.du2 * eu, eu, fmaf(p.dv2 * ev, ev, cst.y)));
-    }
-    if (CLAMP) {
-        fu = fminf(fmaxf(fu, -2.0e6f), 2.0e6f);
-        fv = fminf(fmaxf(fv, -2.0e6f), 2.0e6f);
-    }
-    int iu, iv;
-    const float flu = floor_magic(fu, iu), flv = floor_magic(fv, iv);
-    o.au = fu - flu, o.av = fv - flv;
-    o.iu = iu + p.hu, o.iv = iv + p.hv;
-    return o;
-}
 
 template <int MODE, bool UNIT, bool CLAMP, int ZR>
 __global__ void __launch_bounds__(ATB_BX* ATB_BY)
@@ -166,8 +103,13 @@ static void atb_gather_launch(dim3 grid, dim3 block, cudaStream_t st, bool clamp
     else atb_gather_kernel<MODE, UNIT, false, ZR><<<grid, block, 0, st>>>(proj, v, nViews, p, vol);
 }
 
+int launch_atb_tma(const float* proj, const Grid& g, const VoxView* d_views, const VoxView* h_views, int nViews, int mode,
+                   const AtbP& p, float* vol, cudaStream_t st);   // atb_tma.cu
+int g_atb_path = 0;   // 0 = TMA-staged kernel when the problem qualifies, 1 = gather kernel only, 2 = TMA, box undersized
+
 int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nViews, int mode, bool unit_proj,
-               float* vol, int z0, int nzs, bool accumulate, int row0, int nrows, bool clamp, cudaStream_t st) {
+               float* vol, int z0, int nzs, bool accumulate, int row0, int nrows, bool clamp, cudaStream_t st,
+               const VoxView* h_views) {
     if (mode != TIGRE_ATB_MATCHED && mode != TIGRE_ATB_FDK) return TIGRE_ERR_ARG;
     AtbP p;
     p.nx = g.nx, p.ny = g.ny, p.nz = g.nz, p.nu = g.nu, p.nv = g.nv;
@@ -181,6 +123,10 @@ int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nVi
     dim3 grid((g.nx + ATB_BX - 1) / ATB_BX, (g.ny + ATB_BY - 1) / ATB_BY, (nzs + ZR - 1) / ZR);
     if (grid.y > 65535 || grid.z > 65535) return TIGRE_ERR_ARG;
     ProfScope ps(PK_ATB, st);
+    if (!unit_proj && h_views && g_atb_path != 1) {
+        const int rc = launch_atb_tma(proj, g, d_views, h_views, nViews, mode, p, vol, st);
+        if (rc <= 0) return rc;   // launched, or a CUDA error; rc > 0: does not qualify
+    }
     if (unit_proj) {
         if (mode == TIGRE_ATB_FDK) atb_gather_launch<TIGRE_ATB_FDK, true>(grid, block, st, clamp, proj, d_views, nViews, p, vol);
         else atb_gather_launch<TIGRE_ATB_MATCHED, true>(grid, block, st, clamp, proj, d_views, nViews, p, vol);
@@ -193,3 +139,9 @@ int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nVi
 }
 
 }  // namespace tg
+
+extern "C" int tigre_set_atb_path(int path) {
+    if (path < 0 || path > 2) return TIGRE_ERR_ARG;
+    tg::g_atb_path = path;
+    return TIGRE_OK;
+}

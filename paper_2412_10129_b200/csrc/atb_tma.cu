@@ -1,0 +1,331 @@
+// atb_tma.cu — voxel-driven backprojection with the detector footprints staged into shared memory by
+// TMA (BASELINE.json north_star: "each batch's detector footprint is staged into shared memory by TMA,
+// and accumulation stays in registers"; DESIGN.md O-C for what is computed).
+//
+// A CTA owns a tile of 32 x BY x ZR voxels; thread (tx,ty) owns the ZR voxels along z at one (x,y) and
+// keeps their sums in registers over all views.  One extra PRODUCER warp walks the views ahead of the
+// consumers: for each view it projects the 8 corner voxels of the tile (the projective map is quasi-
+// linear, so they bound the footprint), and issues ONE cp.async.bulk.tensor load of the BU x BV pixel box
+// around it into a ring of shared-memory stages (mbarrier full/empty pairs).  TMA zero-fills whatever
+// lies outside the detector, which IS the zero border of the bilinear interpolation, so the consumers
+// read their four taps from shared memory with no bounds checks.  A view whose footprint does not fit
+// the box (extreme magnification / tilt) is flagged and its taps are gathered through L1/L2 instead.
+//
+// Views whose detector columns are parallel to the volume's z axis (every circular-orbit view without
+// detector tilt: rowU.z = rowW.z = rowG.z = 0) take a cheaper inner loop: the magnification, the
+// column pair, its fraction and the u-part of the weight are constant along the thread's z-run.
+#include <cuda.h>
+#include <cmath>
+#include <mutex>
+#include "atb_common.cuh"
+
+namespace tg {
+
+namespace {
+
+constexpr int TMA_STAGES_MAX = 4;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+            smem_u32(dst)),
+        "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
+        : "memory");
+}
+
+struct StageInfo {   // written by the producer before it arms the stage's full barrier
+    int c0, c1;      // absolute detector index of the box origin (u, v)
+    int fits, pad;
+};
+
+}  // namespace
+
+extern int g_atb_path;   // atb.cu
+
+template <int MODE, int BY, int ZR>
+__global__ void __launch_bounds__(32 * (BY + 1))
+atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict__ proj, const VoxView* __restrict__ views,
+               int nViews, AtbP p, int BU, int BV, int nStages, float* __restrict__ vol) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int stageElems = (BU * BV + 31) & ~31;   // 128-byte multiple
+    float* tiles = reinterpret_cast<float*>(smem_raw);
+    uint64_t* full = reinterpret_cast<uint64_t*>(tiles + (size_t)nStages * stageElems);
+    uint64_t* empty = full + TMA_STAGES_MAX;
+    StageInfo* info = reinterpret_cast<StageInfo*>(empty + TMA_STAGES_MAX);
+
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * BY, zb = blockIdx.z * ZR;   // zb relative to p.z0
+    if (tx == 0 && ty == 0) {
+        for (int s = 0; s < nStages; ++s) {
+            mbar_init(full + s, 1);
+            mbar_init(empty + s, BY);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (ty == BY) {
+        // ------------------------------------------------------------ producer warp
+        const int c = tx & 7;   // corner of the tile's box of voxel centres
+        const float cxf = (float)(x0 + ((c & 1) ? 31 : 0)) - p.cx;
+        const float cyf = (float)(y0 + ((c & 2) ? BY - 1 : 0)) - p.cy;
+        const float czf = (float)(p.z0 + zb + ((c & 4) ? ZR - 1 : 0)) - p.cz;
+        for (int a = 0; a < nViews; ++a) {
+            const int s = a % nStages;
+            const float4* vp = reinterpret_cast<const float4*>(views + a);
+            const float4 rU = __ldg(vp), rV = __ldg(vp + 1), rW = __ldg(vp + 2);
+            const float U = fmaf(rU.x, cxf, fmaf(rU.y, cyf, fmaf(rU.z, czf, rU.w)));
+            const float V = fmaf(rV.x, cxf, fmaf(rV.y, cyf, fmaf(rV.z, czf, rV.w)));
+            const float W = fmaf(rW.x, cxf, fmaf(rW.y, cyf, fmaf(rW.z, czf, rW.w)));
+            const float t = rcp_fast(W);
+            float ulo = U * t, vlo = V * t, uhi = ulo, vhi = vlo;
+#pragma unroll
+            for (int o = 4; o > 0; o >>= 1) {
+                ulo = fminf(ulo, __shfl_xor_sync(0xffffffffu, ulo, o)), uhi = fmaxf(uhi, __shfl_xor_sync(0xffffffffu, uhi, o));
+                vlo = fminf(vlo, __shfl_xor_sync(0xffffffffu, vlo, o)), vhi = fmaxf(vhi, __shfl_xor_sync(0xffffffffu, vhi, o));
+            }
+            if (tx == 0) {
+                // box origin one pixel below the smallest tap; taps reach floor(max)+1, one more of slack for
+                // the consumers' own rounding: extent floor(max) - floor(min) + 4 must fit
+                const bool finite = fabsf(ulo) < 1.0e6f && fabsf(uhi) < 1.0e6f && fabsf(vlo) < 1.0e6f && fabsf(vhi) < 1.0e6f;
+                int fits = 0, c0 = 0, c1 = 0;
+                if (finite) {
+                    // TMA wants the box to start on a 16-byte boundary of the row: round u down to a multiple of 4
+                    const int u0 = (((int)floorf(ulo) - 1 + p.hu) & ~3) - p.hu, v0 = (int)floorf(vlo) - 1;
+                    fits = ((int)floorf(uhi) + 3 - u0 <= BU) && ((int)floorf(vhi) + 3 - v0 <= BV);
+                    c0 = u0 + p.hu, c1 = v0 + p.hv;
+                }
+                if (a >= nStages) mbar_wait(empty + s, ((a / nStages) - 1) & 1);
+                info[s].c0 = c0, info[s].c1 = c1, info[s].fits = fits;
+                if (fits) {
+                    mbar_arrive_expect_tx(full + s, (uint32_t)(BU * BV * sizeof(float)));
+                    tma_load_3d(tiles + (size_t)s * stageElems, &tmap, c0, c1 - p.row0, a, full + s);
+                } else {
+                    mbar_arrive(full + s);
+                }
+            }
+            __syncwarp();
+        }
+        return;
+    }
+
+    // ---------------------------------------------------------------- consumer warps
+    const int ix = x0 + tx, iy = y0 + ty;
+    const bool active = ix < p.nx && iy < p.ny;
+    const float cxf = (float)ix - p.cx, cyf = (float)iy - p.cy, czf = (float)(p.z0 + zb) - p.cz;
+    float acc[ZR];
+#pragma unroll
+    for (int k = 0; k < ZR; ++k) acc[k] = 0.f;
+    const size_t per = (size_t)p.nu * p.nrows;
+    for (int a = 0; a < nViews; ++a) {
+        const int s = a % nStages;
+        const float4* vp = reinterpret_cast<const float4*>(views + a);
+        const float4 rU = __ldg(vp), rV = __ldg(vp + 1), rW = __ldg(vp + 2), rG = __ldg(vp + 3), cst = __ldg(vp + 4);
+        const float U0 = fmaf(rU.x, cxf, fmaf(rU.y, cyf, fmaf(rU.z, czf, rU.w)));
+        const float V0 = fmaf(rV.x, cxf, fmaf(rV.y, cyf, fmaf(rV.z, czf, rV.w)));
+        const float W0 = fmaf(rW.x, cxf, fmaf(rW.y, cyf, fmaf(rW.z, czf, rW.w)));
+        const float G0 = fmaf(rG.x, cxf, fmaf(rG.y, cyf, fmaf(rG.z, czf, rG.w)));
+        mbar_wait(full + s, (a / nStages) & 1);
+        const int c0 = info[s].c0, c1 = info[s].c1, fits = info[s].fits;
+        const float* tile = tiles + (size_t)s * stageElems;
+        if (!fits) {
+            // footprint larger than the staged box: gather this view through L1/L2 (bounds-checked, clamped)
+            if (active) {
+                const float* pa = proj + (size_t)a * per;
+#pragma unroll
+                for (int k = 0; k < ZR; ++k) {
+                    const float kf = (float)k;
+                    const TapW tw = voxel_view<MODE, true>(fmaf(kf, rU.z, U0), fmaf(kf, rV.z, V0), fmaf(kf, rW.z, W0),
+                                                           fmaf(kf, rG.z, G0), cst, p);
+                    acc[k] = fmaf(tw.w, bilinear_global(pa, tw.iu, tw.iv, tw.au, tw.av, p), acc[k]);
+                }
+            }
+        } else if (!active) {
+            // voxels outside the volume (ragged tile): nothing to add, but the warp still releases the stage
+        } else if (rU.z == 0.f && rW.z == 0.f && rG.z == 0.f) {
+            // detector columns parallel to z: per view and thread, one reciprocal, one column pair
+            const float t = rcp_fast(W0);
+            const float fu = U0 * t;
+            int iu;
+            const float flu = floor_magic(fu, iu);
+            const float au = fu - flu;
+            const float fv0 = V0 * t, dfv = rV.z * t;
+            float wu, wk;   // matched: w = wk * sqrt(wu + dv2*ev^2); FDK: w = wk
+            if (MODE == TIGRE_ATB_FDK) {
+                const float ig = rcp_fast(G0);
+                wk = ig * ig, wu = 0.f;
+            } else {
+                const float eu = fu - cst.z;
+                wk = (cst.x * t) * t, wu = fmaf(p.du2 * eu, eu, cst.y);
+            }
+            const float* col = tile + (iu + p.hu - c0);
+            const int vshift = p.hv - c1;
+#pragma unroll
+            for (int k = 0; k < ZR; ++k) {
+                const float fv = fmaf((float)k, dfv, fv0);
+                int iv;
+                const float flv = floor_magic(fv, iv);
+                const float av = fv - flv;
+                const float* q = col + (iv + vshift) * BU;
+                const float p00 = q[0], p10 = q[1], p01 = q[BU], p11 = q[BU + 1];
+                const float r0 = fmaf(au, p10 - p00, p00), r1 = fmaf(au, p11 - p01, p01);
+                const float val = fmaf(av, r1 - r0, r0);
+                float w = wk;
+                if (MODE != TIGRE_ATB_FDK) {
+                    const float ev = fv - cst.w;
+                    w = wk * sqrt_fast(fmaf(p.dv2 * ev, ev, wu));
+                }
+                acc[k] = fmaf(w, val, acc[k]);
+            }
+        } else {
+            const int ushift = -c0, vshift = -c1;   // voxel_view returns absolute detector indices
+#pragma unroll
+            for (int k = 0; k < ZR; ++k) {
+                const float kf = (float)k;
+                const TapW tw = voxel_view<MODE, false>(fmaf(kf, rU.z, U0), fmaf(kf, rV.z, V0), fmaf(kf, rW.z, W0),
+                                                        fmaf(kf, rG.z, G0), cst, p);
+                const float* q = tile + (tw.iv + vshift) * BU + (tw.iu + ushift);
+                const float p00 = q[0], p10 = q[1], p01 = q[BU], p11 = q[BU + 1];
+                const float r0 = fmaf(tw.au, p10 - p00, p00), r1 = fmaf(tw.au, p11 - p01, p01);
+                acc[k] = fmaf(tw.w, fmaf(tw.av, r1 - r0, r0), acc[k]);
+            }
+        }
+        __syncwarp();
+        if (tx == 0) mbar_arrive(empty + s);
+    }
+    if (active) {
+        const size_t slice = (size_t)p.nx * p.ny;
+#pragma unroll
+        for (int k = 0; k < ZR; ++k) {
+            if (zb + k < p.nzs) {
+                float* o = vol + (size_t)(zb + k) * slice + (size_t)iy * p.nx + ix;
+                *o = p.accumulate ? *o + acc[k] : acc[k];
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------ host side
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)f;
+        (void)cudaGetLastError();
+    });
+    return fn;
+}
+
+// footprint extent (pixels) of the tile of voxel centres [x0,x0+bx-1] x [y0,..] x [z0,..] in one view
+void tile_extent(const VoxView& v, double cx, double cy, double cz, int x0, int y0, int z0, int bx, int by, int bz, double& eu,
+                 double& ev) {
+    double ulo = 1e300, uhi = -1e300, vlo = 1e300, vhi = -1e300;
+    for (int c = 0; c < 8; ++c) {
+        const double x = x0 + ((c & 1) ? bx - 1 : 0) - cx, y = y0 + ((c & 2) ? by - 1 : 0) - cy, z = z0 + ((c & 4) ? bz - 1 : 0) - cz;
+        const double W = v.rowW[0] * x + v.rowW[1] * y + v.rowW[2] * z + v.rowW[3];
+        const double U = v.rowU[0] * x + v.rowU[1] * y + v.rowU[2] * z + v.rowU[3];
+        const double V = v.rowV[0] * x + v.rowV[1] * y + v.rowV[2] * z + v.rowV[3];
+        if (!(W > 1e-12)) {
+            eu = ev = 1e9;
+            return;
+        }
+        ulo = std::fmin(ulo, U / W), uhi = std::fmax(uhi, U / W), vlo = std::fmin(vlo, V / W), vhi = std::fmax(vhi, V / W);
+    }
+    eu = uhi - ulo, ev = vhi - vlo;
+}
+
+template <int MODE, int BY, int ZR>
+int tma_launch(const CUtensorMap& map, const float* proj, const VoxView* d_views, int nViews, const AtbP& p, int BU, int BV,
+               int nStages, float* vol, int nzs, cudaStream_t st) {
+    const size_t stageElems = ((size_t)BU * BV + 31) & ~(size_t)31;
+    const size_t smem = nStages * stageElems * sizeof(float) + 2 * TMA_STAGES_MAX * sizeof(uint64_t) + TMA_STAGES_MAX * sizeof(StageInfo);
+    auto kern = atb_tma_kernel<MODE, BY, ZR>;
+    TG_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    dim3 block(32, BY + 1), grid((p.nx + 31) / 32, (p.ny + BY - 1) / BY, (nzs + ZR - 1) / ZR);
+    if (grid.y > 65535 || grid.z > 65535) return TIGRE_ERR_ARG;
+    kern<<<grid, block, smem, st>>>(map, proj, d_views, nViews, p, BU, BV, nStages, vol);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+
+}  // namespace
+
+// Returns TIGRE_OK if the TMA kernel was launched, 1 if this problem does not qualify (caller falls back to the
+// gather kernel), a negative status on a CUDA error.
+int launch_atb_tma(const float* proj, const Grid& g, const VoxView* d_views, const VoxView* h_views, int nViews, int mode,
+                   const AtbP& p, float* vol, cudaStream_t st) {
+    constexpr int BY = 16, ZR = 8;
+    EncodeTiledFn enc = encode_fn();
+    if (!enc || !h_views || !proj) return 1;
+    if ((g.nu & 3) || (reinterpret_cast<uintptr_t>(proj) & 15) || p.nrows < 1) return 1;   // TMA: 16-byte rows and base
+    if (g.nx < 32 || g.ny < BY || nViews < 2) return 1;                                      // not worth staging
+    // box size: the largest footprint of a tile over a sample of tile positions (the 8 corner tiles of the
+    // slab and its centre) and all views; tiles that still do not fit fall back per view inside the kernel
+    const double cx = 0.5 * (g.nx - 1), cy = 0.5 * (g.ny - 1), cz = 0.5 * (g.nz - 1);
+    double eu = 0, ev = 0;
+    const int xs[3] = {0, std::max(0, (g.nx / 2 / 32) * 32), std::max(0, ((g.nx - 1) / 32) * 32)};
+    const int ys[3] = {0, std::max(0, (g.ny / 2 / BY) * BY), std::max(0, ((g.ny - 1) / BY) * BY)};
+    const int zs[3] = {p.z0, p.z0 + std::max(0, (p.nzs / 2 / ZR) * ZR), p.z0 + std::max(0, ((p.nzs - 1) / ZR) * ZR)};
+    for (int a = 0; a < nViews; ++a)
+        for (int i = 0; i < 27; ++i) {
+            double e1, e2;
+            tile_extent(h_views[a], cx, cy, cz, xs[i % 3], ys[(i / 3) % 3], zs[i / 9], 32, BY, ZR, e1, e2);
+            eu = std::fmax(eu, e1), ev = std::fmax(ev, e2);
+        }
+    if (!(eu < 240.0) || !(ev < 240.0)) return 1;
+    if (g_atb_path == 2) eu *= 0.7, ev *= 0.7;   // test hook: most views no longer fit and take the in-kernel fallback
+    const int BU = (((int)std::ceil(eu) + 5 + 3) + 3) & ~3, BV = (int)std::ceil(ev) + 5;   // +3: 16-byte aligned origin
+    if (BU > 256 || BV > 256) return 1;
+    const size_t stageB = (((size_t)BU * BV + 31) & ~(size_t)31) * sizeof(float);
+    int nStages = TMA_STAGES_MAX;
+    while (nStages > 2 && nStages * stageB > 100 * 1024) --nStages;
+    if (nStages * stageB > 200 * 1024) return 1;
+    nStages = std::min(nStages, std::max(2, nViews));
+
+    CUtensorMap map;
+    const cuuint64_t gdim[3] = {(cuuint64_t)g.nu, (cuuint64_t)p.nrows, (cuuint64_t)nViews};
+    const cuuint64_t gstr[2] = {(cuuint64_t)g.nu * sizeof(float), (cuuint64_t)g.nu * p.nrows * sizeof(float)};
+    const cuuint32_t box[3] = {(cuuint32_t)BU, (cuuint32_t)BV, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    if (enc(&map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(proj), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return 1;
+    if (mode == TIGRE_ATB_FDK) return tma_launch<TIGRE_ATB_FDK, BY, ZR>(map, proj, d_views, nViews, p, BU, BV, nStages, vol, p.nzs, st);
+    return tma_launch<TIGRE_ATB_MATCHED, BY, ZR>(map, proj, d_views, nViews, p, BU, BV, nStages, vol, p.nzs, st);
+}
+
+}  // namespace tg

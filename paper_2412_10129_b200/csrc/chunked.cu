@@ -215,7 +215,7 @@ int chunked_atb(const float* h_proj, const tigre_geo* geo, const double* angles,
                                           (size_t)na, cudaMemcpyHostToDevice, sd.h2d));
                 TG_CUDA(cudaEventRecord(sd.ready[ib % nPb], sd.h2d));
                 TG_CUDA(cudaStreamWaitEvent(st, sd.ready[ib % nPb], 0));
-                TG_TRY(launch_atb(P, g, tab.as<VoxView>() + a0, na, mode, false, V, z0, nz_s, b > 0, row0, nrows, clamp, st));
+                TG_TRY(launch_atb(P, g, tab.as<VoxView>() + a0, na, mode, false, V, z0, nz_s, b > 0, row0, nrows, clamp, st, hv.data() + a0));
                 TG_CUDA(cudaEventRecord(sd.freed[ib % nPb], st));
             }
         }

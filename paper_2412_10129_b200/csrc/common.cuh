@@ -110,8 +110,11 @@ int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nView
 // volume whose full height is g.nz; vol points at slice z0.  accumulate: vol += instead of vol =.
 //   unit_proj: treat projections as all ones (column sums A^T 1), proj may be NULL
 //   row0/nrows: the projection buffer holds detector rows [row0,row0+nrows) only (chunked path)
+//   h_views: host copy of the same table; when given (and the problem qualifies) the TMA-staged kernel of
+//   atb_tma.cu runs, otherwise the L1/L2 gather kernel of atb.cu
 int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nViews, int mode, bool unit_proj,
-               float* vol, int z0, int nzs, bool accumulate, int row0, int nrows, bool clamp, cudaStream_t st);
+               float* vol, int z0, int nzs, bool accumulate, int row0, int nrows, bool clamp, cudaStream_t st,
+               const VoxView* h_views = nullptr);
 // true if some voxel of the box can project beyond |index| 1e6 in some view (then the kernels clamp)
 bool vox_needs_clamp(const Grid& g, const VoxView* host_views, int n);
 

@@ -38,7 +38,7 @@ def host(t):
 def cone_geometry():
     # wide cone (volume close to the source) so that z-slabs map to clearly different detector-row bands;
     # ragged sizes; detector offset so some rows see nothing
-    return Geometry(nVoxel=(45, 38, 53), dVoxel=(1.0, 1.1, 0.9), nDetector=(70, 90), dDetector=(1.4, 1.2),
+    return Geometry(nVoxel=(45, 38, 53), dVoxel=(1.0, 1.1, 0.9), nDetector=(72, 90), dDetector=(1.4, 1.2),
                     DSD=330.0, DSO=200.0, offDetector=(3.0, -6.0), offOrigin=(1.0, -2.0, 3.0))
 
 
@@ -65,7 +65,7 @@ def test_chunked_ax_matches_oracle(tg, mode, tol, budget_kb):
 def test_chunked_atb_matches_oracle(tg, mode, tol, budget_kb):
     geo = cone_geometry()
     ang = circular_angles(11, start=0.1)
-    proj = np.random.default_rng(22).random((11, 90, 70), dtype=np.float32)
+    proj = np.random.default_rng(22).random((11, 90, 72), dtype=np.float32)
     ref = orc.atb(proj, geo, ang, orc.MATCHED if mode == "matched" else orc.FDK)
     tg.set_chunk_budget(budget_kb * 1024)
     got = tg.Atb(pinned(proj), geo, ang, mode)
@@ -131,5 +131,5 @@ def test_chunked_budget_too_small_and_mixed_memory(tg):
     finally:
         tg.set_chunk_budget(0)
     with pytest.raises(tg.TigreError) as e:               # pinned in, device out: not a supported mix
-        tg.Ax(vol, geo, ang, "siddon", out=torch.empty((3, 90, 70), device="cuda"))
+        tg.Ax(vol, geo, ang, "siddon", out=torch.empty((3, 90, 72), device="cuda"))
     assert e.value.code == -3
