@@ -66,10 +66,13 @@ struct StageInfo {   // written by the producer before it arms the stage's full 
 
 extern int g_atb_path;   // atb.cu
 
-template <int MODE, int BY, int ZR>
+// BU (box width, pixels) is a template parameter so that the second tap row is an immediate offset; the
+// launcher picks the smallest of 48, 80, ... 240 (all = 16 mod 32: with the 8 x 4 lane layout below, the taps
+// of one warp span < 16 columns of at most a few adjacent rows, and rows 16 banks apart do not collide).
+template <int MODE, int BY, int ZR, int BU>
 __global__ void __launch_bounds__(32 * (BY + 1))
 atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict__ proj, const VoxView* __restrict__ views,
-               int nViews, AtbP p, int BU, int BV, int nStages, float* __restrict__ vol) {
+               int nViews, AtbP p, int BV, int nStages, float* __restrict__ vol) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int stageElems = (BU * BV + 31) & ~31;   // 128-byte multiple
     float* tiles = reinterpret_cast<float*>(smem_raw);
@@ -77,9 +80,9 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
     uint64_t* empty = full + TMA_STAGES_MAX;
     StageInfo* info = reinterpret_cast<StageInfo*>(empty + TMA_STAGES_MAX);
 
-    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int lane = threadIdx.x, warp = threadIdx.y;
     const int x0 = blockIdx.x * 32, y0 = blockIdx.y * BY, zb = blockIdx.z * ZR;   // zb relative to p.z0
-    if (tx == 0 && ty == 0) {
+    if (lane == 0 && warp == 0) {
         for (int s = 0; s < nStages; ++s) {
             mbar_init(full + s, 1);
             mbar_init(empty + s, BY);
@@ -88,9 +91,9 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
     }
     __syncthreads();
 
-    if (ty == BY) {
+    if (warp == BY) {
         // ------------------------------------------------------------ producer warp
-        const int c = tx & 7;   // corner of the tile's box of voxel centres
+        const int c = lane & 7;   // corner of the tile's box of voxel centres
         const float cxf = (float)(x0 + ((c & 1) ? 31 : 0)) - p.cx;
         const float cyf = (float)(y0 + ((c & 2) ? BY - 1 : 0)) - p.cy;
         const float czf = (float)(p.z0 + zb + ((c & 4) ? ZR - 1 : 0)) - p.cz;
@@ -108,7 +111,7 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
                 ulo = fminf(ulo, __shfl_xor_sync(0xffffffffu, ulo, o)), uhi = fmaxf(uhi, __shfl_xor_sync(0xffffffffu, uhi, o));
                 vlo = fminf(vlo, __shfl_xor_sync(0xffffffffu, vlo, o)), vhi = fmaxf(vhi, __shfl_xor_sync(0xffffffffu, vhi, o));
             }
-            if (tx == 0) {
+            if (lane == 0) {
                 // box origin one pixel below the smallest tap; taps reach floor(max)+1, one more of slack for
                 // the consumers' own rounding: extent floor(max) - floor(min) + 4 must fit
                 const bool finite = fabsf(ulo) < 1.0e6f && fabsf(uhi) < 1.0e6f && fabsf(vlo) < 1.0e6f && fabsf(vhi) < 1.0e6f;
@@ -134,13 +137,16 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
     }
 
     // ---------------------------------------------------------------- consumer warps
-    const int ix = x0 + tx, iy = y0 + ty;
+    // a warp owns 8 (x) x 4 (y) columns of voxels: a compact detector footprint (few shared-memory bank
+    // conflicts) and still 32-byte store segments
+    const int ix = x0 + (warp & 3) * 8 + (lane & 7), iy = y0 + (warp >> 2) * 4 + (lane >> 3);
     const bool active = ix < p.nx && iy < p.ny;
     const float cxf = (float)ix - p.cx, cyf = (float)iy - p.cy, czf = (float)(p.z0 + zb) - p.cz;
     float acc[ZR];
 #pragma unroll
     for (int k = 0; k < ZR; ++k) acc[k] = 0.f;
     const size_t per = (size_t)p.nu * p.nrows;
+    const uint32_t tiles_s = smem_u32(tiles);
     for (int a = 0; a < nViews; ++a) {
         const int s = a % nStages;
         const float4* vp = reinterpret_cast<const float4*>(views + a);
@@ -167,39 +173,48 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
         } else if (!active) {
             // voxels outside the volume (ragged tile): nothing to add, but the warp still releases the stage
         } else if (rU.z == 0.f && rW.z == 0.f && rG.z == 0.f) {
-            // detector columns parallel to z: per view and thread, one reciprocal, one column pair
+            // detector columns parallel to z: per view and thread, one reciprocal, one column pair; the weight
+            // w = wk * sqrt(q(k)) with q quadratic in k (matched) or w = wk (FDK); wk is folded into the
+            // u-interpolation weights
             const float t = rcp_fast(W0);
             const float fu = U0 * t;
             int iu;
             const float flu = floor_magic(fu, iu);
             const float au = fu - flu;
             const float fv0 = V0 * t, dfv = rV.z * t;
-            float wu, wk;   // matched: w = wk * sqrt(wu + dv2*ev^2); FDK: w = wk
+            float wk, qA = 0.f, qB = 0.f, qC = 0.f;
             if (MODE == TIGRE_ATB_FDK) {
                 const float ig = rcp_fast(G0);
-                wk = ig * ig, wu = 0.f;
+                wk = ig * ig;
             } else {
-                const float eu = fu - cst.z;
-                wk = (cst.x * t) * t, wu = fmaf(p.du2 * eu, eu, cst.y);
+                const float eu = fu - cst.z, ev0 = fv0 - cst.w;
+                wk = (cst.x * t) * t;
+                qA = fmaf(p.dv2 * ev0, ev0, fmaf(p.du2 * eu, eu, cst.y));
+                qB = 2.f * p.dv2 * ev0 * dfv, qC = p.dv2 * dfv * dfv;
             }
-            const float* col = tile + (iu + p.hu - c0);
-            const int vshift = p.hv - c1;
+            const float wa = wk * (1.f - au), wb = wk * au;
+            // byte address (shared window) of the tap column in row 0 of the stage; rows via one IMAD
+            const uint32_t col = tiles_s + (uint32_t)(s * stageElems + (iu + p.hu - c0) + (p.hv - c1) * BU) * 4u;
 #pragma unroll
             for (int k = 0; k < ZR; ++k) {
                 const float fv = fmaf((float)k, dfv, fv0);
                 int iv;
                 const float flv = floor_magic(fv, iv);
                 const float av = fv - flv;
-                const float* q = col + (iv + vshift) * BU;
-                const float p00 = q[0], p10 = q[1], p01 = q[BU], p11 = q[BU + 1];
-                const float r0 = fmaf(au, p10 - p00, p00), r1 = fmaf(au, p11 - p01, p01);
+                const uint32_t q = col + (uint32_t)(iv * (BU * 4));
+                float p00, p10, p01, p11;
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(p00) : "r"(q));
+                asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(p10) : "r"(q));
+                asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(p01) : "r"(q), "n"(BU * 4));
+                asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(p11) : "r"(q), "n"(BU * 4 + 4));
+                const float r0 = fmaf(p10, wb, p00 * wa), r1 = fmaf(p11, wb, p01 * wa);
                 const float val = fmaf(av, r1 - r0, r0);
-                float w = wk;
-                if (MODE != TIGRE_ATB_FDK) {
-                    const float ev = fv - cst.w;
-                    w = wk * sqrt_fast(fmaf(p.dv2 * ev, ev, wu));
+                if (MODE == TIGRE_ATB_FDK) {
+                    acc[k] += val;
+                } else {
+                    const float kf = (float)k;
+                    acc[k] = fmaf(sqrt_fast(fmaf(fmaf(qC, kf, qB), kf, qA)), val, acc[k]);
                 }
-                acc[k] = fmaf(w, val, acc[k]);
             }
         } else {
             const int ushift = -c0, vshift = -c1;   // voxel_view returns absolute detector indices
@@ -215,7 +230,7 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
             }
         }
         __syncwarp();
-        if (tx == 0) mbar_arrive(empty + s);
+        if (lane == 0) mbar_arrive(empty + s);
     }
     if (active) {
         const size_t slice = (size_t)p.nx * p.ny;
@@ -268,18 +283,31 @@ void tile_extent(const VoxView& v, double cx, double cy, double cz, int x0, int 
     eu = uhi - ulo, ev = vhi - vlo;
 }
 
-template <int MODE, int BY, int ZR>
-int tma_launch(const CUtensorMap& map, const float* proj, const VoxView* d_views, int nViews, const AtbP& p, int BU, int BV,
-               int nStages, float* vol, int nzs, cudaStream_t st) {
+template <int MODE, int BY, int ZR, int BU>
+int tma_launch(const CUtensorMap& map, const float* proj, const VoxView* d_views, int nViews, const AtbP& p, int BV,
+               int nStages, float* vol, cudaStream_t st) {
     const size_t stageElems = ((size_t)BU * BV + 31) & ~(size_t)31;
     const size_t smem = nStages * stageElems * sizeof(float) + 2 * TMA_STAGES_MAX * sizeof(uint64_t) + TMA_STAGES_MAX * sizeof(StageInfo);
-    auto kern = atb_tma_kernel<MODE, BY, ZR>;
+    auto kern = atb_tma_kernel<MODE, BY, ZR, BU>;
     TG_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    dim3 block(32, BY + 1), grid((p.nx + 31) / 32, (p.ny + BY - 1) / BY, (nzs + ZR - 1) / ZR);
+    dim3 block(32, BY + 1), grid((p.nx + 31) / 32, (p.ny + BY - 1) / BY, (p.nzs + ZR - 1) / ZR);
     if (grid.y > 65535 || grid.z > 65535) return TIGRE_ERR_ARG;
-    kern<<<grid, block, smem, st>>>(map, proj, d_views, nViews, p, BU, BV, nStages, vol);
+    kern<<<grid, block, smem, st>>>(map, proj, d_views, nViews, p, BV, nStages, vol);
     TG_CUDA(cudaGetLastError());
     return TIGRE_OK;
+}
+template <int MODE, int BY, int ZR>
+int tma_launch_bu(int BU, const CUtensorMap& map, const float* proj, const VoxView* d_views, int nViews, const AtbP& p, int BV,
+                  int nStages, float* vol, cudaStream_t st) {
+    switch (BU) {
+        case 48: return tma_launch<MODE, BY, ZR, 48>(map, proj, d_views, nViews, p, BV, nStages, vol, st);
+        case 80: return tma_launch<MODE, BY, ZR, 80>(map, proj, d_views, nViews, p, BV, nStages, vol, st);
+        case 112: return tma_launch<MODE, BY, ZR, 112>(map, proj, d_views, nViews, p, BV, nStages, vol, st);
+        case 144: return tma_launch<MODE, BY, ZR, 144>(map, proj, d_views, nViews, p, BV, nStages, vol, st);
+        case 176: return tma_launch<MODE, BY, ZR, 176>(map, proj, d_views, nViews, p, BV, nStages, vol, st);
+        case 240: return tma_launch<MODE, BY, ZR, 240>(map, proj, d_views, nViews, p, BV, nStages, vol, st);
+    }
+    return 1;
 }
 
 }  // namespace
@@ -307,9 +335,16 @@ int launch_atb_tma(const float* proj, const Grid& g, const VoxView* d_views, con
             eu = std::fmax(eu, e1), ev = std::fmax(ev, e2);
         }
     if (!(eu < 240.0) || !(ev < 240.0)) return 1;
-    if (g_atb_path == 2) eu *= 0.7, ev *= 0.7;   // test hook: most views no longer fit and take the in-kernel fallback
-    const int BU = (((int)std::ceil(eu) + 5 + 3) + 3) & ~3, BV = (int)std::ceil(ev) + 5;   // +3: 16-byte aligned origin
-    if (BU > 256 || BV > 256) return 1;
+    if (g_atb_path == 2) eu *= 0.45, ev *= 0.7;   // test hook: most views no longer fit and take the in-kernel fallback
+    const int need = (int)std::ceil(eu) + 5 + 3;   // +3: 16-byte aligned origin
+    const int BV = (int)std::ceil(ev) + 5;
+    int BU = 0;
+    for (int c : {48, 80, 112, 144, 176, 240})
+        if (c >= need) {
+            BU = c;
+            break;
+        }
+    if (!BU || BV > 256) return 1;
     const size_t stageB = (((size_t)BU * BV + 31) & ~(size_t)31) * sizeof(float);
     int nStages = TMA_STAGES_MAX;
     while (nStages > 2 && nStages * stageB > 100 * 1024) --nStages;
@@ -324,8 +359,8 @@ int launch_atb_tma(const float* proj, const Grid& g, const VoxView* d_views, con
     if (enc(&map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(proj), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return 1;
-    if (mode == TIGRE_ATB_FDK) return tma_launch<TIGRE_ATB_FDK, BY, ZR>(map, proj, d_views, nViews, p, BU, BV, nStages, vol, p.nzs, st);
-    return tma_launch<TIGRE_ATB_MATCHED, BY, ZR>(map, proj, d_views, nViews, p, BU, BV, nStages, vol, p.nzs, st);
+    if (mode == TIGRE_ATB_FDK) return tma_launch_bu<TIGRE_ATB_FDK, BY, ZR>(BU, map, proj, d_views, nViews, p, BV, nStages, vol, st);
+    return tma_launch_bu<TIGRE_ATB_MATCHED, BY, ZR>(BU, map, proj, d_views, nViews, p, BV, nStages, vol, st);
 }
 
 }  // namespace tg
