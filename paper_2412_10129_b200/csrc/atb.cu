@@ -118,6 +118,7 @@ int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nVi
     p.du2 = (float)(g.du * g.du), p.dv2 = (float)(g.dv * g.dv);
     p.hu = g.nu / 2, p.hv = g.nv / 2;
     p.accumulate = accumulate ? 1 : 0;
+    p.magic = 0x4B400000;
     constexpr int ZR = 8;
     dim3 block(ATB_BX, ATB_BY);
     dim3 grid((g.nx + ATB_BX - 1) / ATB_BX, (g.ny + ATB_BY - 1) / ATB_BY, (nzs + ZR - 1) / ZR);

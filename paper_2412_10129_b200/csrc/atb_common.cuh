@@ -17,6 +17,7 @@ struct AtbP {
     float du2, dv2;       // pixel pitch squared, mm^2
     int hu, hv;           // nu/2, nv/2
     int accumulate;
+    int magic;            // 0x4B400000 = bits of 1.5*2^23 (floor_magic), passed as data (see atb_tma.cu)
 };
 
 constexpr int ATB_BX = 32, ATB_BY = 8;

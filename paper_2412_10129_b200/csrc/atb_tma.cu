@@ -16,6 +16,7 @@
 // column pair, its fraction and the u-part of the weight are constant along the thread's z-run.
 #include <cuda.h>
 #include <cmath>
+#include <cstdlib>
 #include <mutex>
 #include "atb_common.cuh"
 
@@ -69,8 +70,8 @@ extern int g_atb_path;   // atb.cu
 // BU (box width, pixels) is a template parameter so that the second tap row is an immediate offset; the
 // launcher picks the smallest of 48, 80, ... 240 (all = 16 mod 32: with the 8 x 4 lane layout below, the taps
 // of one warp span < 16 columns of at most a few adjacent rows, and rows 16 banks apart do not collide).
-template <int MODE, int BY, int ZR, int BU>
-__global__ void __launch_bounds__(32 * (BY + 1))
+template <int MODE, int WX, int WY, int ZR, int BU>
+__global__ void __launch_bounds__(32 * (WX * WY + 1), (WX * WY >= 16 ? 2 : 3))
 atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict__ proj, const VoxView* __restrict__ views,
                int nViews, AtbP p, int BV, int nStages, float* __restrict__ vol) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -80,25 +81,27 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
     uint64_t* empty = full + TMA_STAGES_MAX;
     StageInfo* info = reinterpret_cast<StageInfo*>(empty + TMA_STAGES_MAX);
 
+    constexpr int BX = 8 * WX, BY = 4 * WY, NW = WX * WY;   // tile = WX x WY consumer warps of 8 x 4 voxel columns
     const int lane = threadIdx.x, warp = threadIdx.y;
-    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * BY, zb = blockIdx.z * ZR;   // zb relative to p.z0
+    const int x0 = blockIdx.x * BX, y0 = blockIdx.y * BY, zb = blockIdx.z * ZR;   // zb relative to p.z0
     if (lane == 0 && warp == 0) {
         for (int s = 0; s < nStages; ++s) {
             mbar_init(full + s, 1);
-            mbar_init(empty + s, BY);
+            mbar_init(empty + s, NW);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    if (warp == BY) {
+    if (warp == NW) {
         // ------------------------------------------------------------ producer warp
         const int c = lane & 7;   // corner of the tile's box of voxel centres
-        const float cxf = (float)(x0 + ((c & 1) ? 31 : 0)) - p.cx;
+        const float cxf = (float)(x0 + ((c & 1) ? BX - 1 : 0)) - p.cx;
         const float cyf = (float)(y0 + ((c & 2) ? BY - 1 : 0)) - p.cy;
         const float czf = (float)(p.z0 + zb + ((c & 4) ? ZR - 1 : 0)) - p.cz;
+        int s = 0;
+        uint32_t ph = 1;   // parity of the "stage is free" phase the producer waits for (first pass: free by construction)
         for (int a = 0; a < nViews; ++a) {
-            const int s = a % nStages;
             const float4* vp = reinterpret_cast<const float4*>(views + a);
             const float4 rU = __ldg(vp), rV = __ldg(vp + 1), rW = __ldg(vp + 2);
             const float U = fmaf(rU.x, cxf, fmaf(rU.y, cyf, fmaf(rU.z, czf, rU.w)));
@@ -122,7 +125,7 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
                     fits = ((int)floorf(uhi) + 3 - u0 <= BU) && ((int)floorf(vhi) + 3 - v0 <= BV);
                     c0 = u0 + p.hu, c1 = v0 + p.hv;
                 }
-                if (a >= nStages) mbar_wait(empty + s, ((a / nStages) - 1) & 1);
+                if (a >= nStages) mbar_wait(empty + s, ph);
                 info[s].c0 = c0, info[s].c1 = c1, info[s].fits = fits;
                 if (fits) {
                     mbar_arrive_expect_tx(full + s, (uint32_t)(BU * BV * sizeof(float)));
@@ -132,6 +135,7 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
                 }
             }
             __syncwarp();
+            if (++s == nStages) s = 0, ph ^= 1;
         }
         return;
     }
@@ -139,7 +143,7 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
     // ---------------------------------------------------------------- consumer warps
     // a warp owns 8 (x) x 4 (y) columns of voxels: a compact detector footprint (few shared-memory bank
     // conflicts) and still 32-byte store segments
-    const int ix = x0 + (warp & 3) * 8 + (lane & 7), iy = y0 + (warp >> 2) * 4 + (lane >> 3);
+    const int ix = x0 + (warp % WX) * 8 + (lane & 7), iy = y0 + (warp / WX) * 4 + (lane >> 3);
     const bool active = ix < p.nx && iy < p.ny;
     const float cxf = (float)ix - p.cx, cyf = (float)iy - p.cy, czf = (float)(p.z0 + zb) - p.cz;
     float acc[ZR];
@@ -147,15 +151,18 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
     for (int k = 0; k < ZR; ++k) acc[k] = 0.f;
     const size_t per = (size_t)p.nu * p.nrows;
     const uint32_t tiles_s = smem_u32(tiles);
+    int s = 0;
+    uint32_t ph = 0;
     for (int a = 0; a < nViews; ++a) {
-        const int s = a % nStages;
         const float4* vp = reinterpret_cast<const float4*>(views + a);
-        const float4 rU = __ldg(vp), rV = __ldg(vp + 1), rW = __ldg(vp + 2), rG = __ldg(vp + 3), cst = __ldg(vp + 4);
+        const float4 rU = __ldg(vp), rV = __ldg(vp + 1), rW = __ldg(vp + 2), cst = __ldg(vp + 4);
+        // the depth row G only enters the FDK weight
+        const float4 rG = MODE == TIGRE_ATB_FDK ? __ldg(vp + 3) : make_float4(0.f, 0.f, 0.f, 1.f);
         const float U0 = fmaf(rU.x, cxf, fmaf(rU.y, cyf, fmaf(rU.z, czf, rU.w)));
         const float V0 = fmaf(rV.x, cxf, fmaf(rV.y, cyf, fmaf(rV.z, czf, rV.w)));
         const float W0 = fmaf(rW.x, cxf, fmaf(rW.y, cyf, fmaf(rW.z, czf, rW.w)));
         const float G0 = fmaf(rG.x, cxf, fmaf(rG.y, cyf, fmaf(rG.z, czf, rG.w)));
-        mbar_wait(full + s, (a / nStages) & 1);
+        mbar_wait(full + s, ph);
         const int c0 = info[s].c0, c1 = info[s].c1, fits = info[s].fits;
         const float* tile = tiles + (size_t)s * stageElems;
         if (!fits) {
@@ -193,20 +200,26 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
                 qB = 2.f * p.dv2 * ev0 * dfv, qC = p.dv2 * dfv * dfv;
             }
             const float wa = wk * (1.f - au), wb = wk * au;
-            // byte address (shared window) of the tap column in row 0 of the stage; rows via one IMAD
-            const uint32_t col = tiles_s + (uint32_t)(s * stageElems + (iu + p.hu - c0) + (p.hv - c1) * BU) * 4u;
+            // byte address (shared window) of the tap column in row 0 of the stage, minus the magic-number
+            // bias of floor_magic times the row pitch (mod 2^32): the row address is then ONE integer
+            // multiply-add of the raw bits of (fv - 1/2) + 1.5*2^23
+            const uint32_t col = tiles_s + (uint32_t)(s * stageElems + (iu + p.hu - c0) + (p.hv - c1) * BU) * 4u -
+                           (uint32_t)p.magic * (uint32_t)(BU * 4);   // p.magic = 0x4B400000, opaque to the compiler
+                                                                      // (as a literal it is re-added before every load)
 #pragma unroll
             for (int k = 0; k < ZR; ++k) {
                 const float fv = fmaf((float)k, dfv, fv0);
-                int iv;
-                const float flv = floor_magic(fv, iv);
-                const float av = fv - flv;
-                const uint32_t q = col + (uint32_t)(iv * (BU * 4));
+                const float tm = (fv - 0.5f) + 12582912.0f;
+                const float av = fv - (tm - 12582912.0f);
+                const uint32_t q = col + __float_as_uint(tm) * (uint32_t)(BU * 4);
                 float p00, p10, p01, p11;
-                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(p00) : "r"(q));
-                asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(p10) : "r"(q));
-                asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(p01) : "r"(q), "n"(BU * 4));
-                asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(p11) : "r"(q), "n"(BU * 4 + 4));
+                asm volatile(
+                    "ld.shared.f32 %0, [%4];\n\t"
+                    "ld.shared.f32 %1, [%4+4];\n\t"
+                    "ld.shared.f32 %2, [%4+%5];\n\t"
+                    "ld.shared.f32 %3, [%4+%6];"
+                    : "=f"(p00), "=f"(p10), "=f"(p01), "=f"(p11)
+                    : "r"(q), "n"(BU * 4), "n"(BU * 4 + 4));
                 const float r0 = fmaf(p10, wb, p00 * wa), r1 = fmaf(p11, wb, p01 * wa);
                 const float val = fmaf(av, r1 - r0, r0);
                 if (MODE == TIGRE_ATB_FDK) {
@@ -231,6 +244,7 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(empty + s);
+        if (++s == nStages) s = 0, ph ^= 1;
     }
     if (active) {
         const size_t slice = (size_t)p.nx * p.ny;
@@ -283,31 +297,87 @@ void tile_extent(const VoxView& v, double cx, double cy, double cz, int x0, int 
     eu = uhi - ulo, ev = vhi - vlo;
 }
 
-template <int MODE, int BY, int ZR, int BU>
-int tma_launch(const CUtensorMap& map, const float* proj, const VoxView* d_views, int nViews, const AtbP& p, int BV,
-               int nStages, float* vol, cudaStream_t st) {
-    const size_t stageElems = ((size_t)BU * BV + 31) & ~(size_t)31;
-    const size_t smem = nStages * stageElems * sizeof(float) + 2 * TMA_STAGES_MAX * sizeof(uint64_t) + TMA_STAGES_MAX * sizeof(StageInfo);
-    auto kern = atb_tma_kernel<MODE, BY, ZR, BU>;
+struct TmaArgs {
+    CUtensorMap map;
+    const float* proj;
+    const VoxView* d_views;
+    int nViews, BV, nStages;
+    AtbP p;
+    float* vol;
+    cudaStream_t st;
+};
+
+template <int MODE, int WX, int WY, int ZR, int BU>
+int tma_launch(const TmaArgs& A) {
+    const size_t stageElems = ((size_t)BU * A.BV + 31) & ~(size_t)31;
+    const size_t smem = A.nStages * stageElems * sizeof(float) + 2 * TMA_STAGES_MAX * sizeof(uint64_t) + TMA_STAGES_MAX * sizeof(StageInfo);
+    auto kern = atb_tma_kernel<MODE, WX, WY, ZR, BU>;
     TG_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    dim3 block(32, BY + 1), grid((p.nx + 31) / 32, (p.ny + BY - 1) / BY, (p.nzs + ZR - 1) / ZR);
+    dim3 block(32, WX * WY + 1), grid((A.p.nx + 8 * WX - 1) / (8 * WX), (A.p.ny + 4 * WY - 1) / (4 * WY), (A.p.nzs + ZR - 1) / ZR);
     if (grid.y > 65535 || grid.z > 65535) return TIGRE_ERR_ARG;
-    kern<<<grid, block, smem, st>>>(map, proj, d_views, nViews, p, BV, nStages, vol);
+    kern<<<grid, block, smem, A.st>>>(A.map, A.proj, A.d_views, A.nViews, A.p, A.BV, A.nStages, A.vol);
     TG_CUDA(cudaGetLastError());
     return TIGRE_OK;
 }
-template <int MODE, int BY, int ZR>
-int tma_launch_bu(int BU, const CUtensorMap& map, const float* proj, const VoxView* d_views, int nViews, const AtbP& p, int BV,
-                  int nStages, float* vol, cudaStream_t st) {
+template <int MODE, int WX, int WY, int ZR>
+int tma_launch_bu(int BU, const TmaArgs& A) {
     switch (BU) {
-        case 48: return tma_launch<MODE, BY, ZR, 48>(map, proj, d_views, nViews, p, BV, nStages, vol, st);
-        case 80: return tma_launch<MODE, BY, ZR, 80>(map, proj, d_views, nViews, p, BV, nStages, vol, st);
-        case 112: return tma_launch<MODE, BY, ZR, 112>(map, proj, d_views, nViews, p, BV, nStages, vol, st);
-        case 144: return tma_launch<MODE, BY, ZR, 144>(map, proj, d_views, nViews, p, BV, nStages, vol, st);
-        case 176: return tma_launch<MODE, BY, ZR, 176>(map, proj, d_views, nViews, p, BV, nStages, vol, st);
-        case 240: return tma_launch<MODE, BY, ZR, 240>(map, proj, d_views, nViews, p, BV, nStages, vol, st);
+        case 48: return tma_launch<MODE, WX, WY, ZR, 48>(A);
+        case 80: return tma_launch<MODE, WX, WY, ZR, 80>(A);
+        case 112: return tma_launch<MODE, WX, WY, ZR, 112>(A);
+        case 144: return tma_launch<MODE, WX, WY, ZR, 144>(A);
+        case 176: return tma_launch<MODE, WX, WY, ZR, 176>(A);
+        case 240: return tma_launch<MODE, WX, WY, ZR, 240>(A);
     }
     return 1;
+}
+
+// one tile configuration: sizes the staged box from the geometry, encodes the tensor map, launches
+template <int WX, int WY, int ZR>
+int tma_config(EncodeTiledFn enc, const float* proj, const Grid& g, const VoxView* d_views, const VoxView* h_views, int nViews,
+               int mode, const AtbP& p, float* vol, cudaStream_t st) {
+    constexpr int BX = 8 * WX, BY = 4 * WY;
+    if (g.nx < BX || g.ny < BY || nViews < 2) return 1;   // not worth staging
+    // box size: the largest footprint of a tile over a sample of tile positions (corner, edge and centre tiles of
+    // the slab) and all views; tiles that still do not fit fall back per view inside the kernel
+    const double cx = 0.5 * (g.nx - 1), cy = 0.5 * (g.ny - 1), cz = 0.5 * (g.nz - 1);
+    double eu = 0, ev = 0;
+    const int xs[3] = {0, std::max(0, (g.nx / 2 / BX) * BX), std::max(0, ((g.nx - 1) / BX) * BX)};
+    const int ys[3] = {0, std::max(0, (g.ny / 2 / BY) * BY), std::max(0, ((g.ny - 1) / BY) * BY)};
+    const int zs[3] = {p.z0, p.z0 + std::max(0, (p.nzs / 2 / ZR) * ZR), p.z0 + std::max(0, ((p.nzs - 1) / ZR) * ZR)};
+    for (int a = 0; a < nViews; ++a)
+        for (int i = 0; i < 27; ++i) {
+            double e1, e2;
+            tile_extent(h_views[a], cx, cy, cz, xs[i % 3], ys[(i / 3) % 3], zs[i / 9], BX, BY, ZR, e1, e2);
+            eu = std::fmax(eu, e1), ev = std::fmax(ev, e2);
+        }
+    if (!(eu < 240.0) || !(ev < 240.0)) return 1;
+    if (g_atb_path == 2) eu *= 0.45, ev *= 0.7;   // test hook: most views no longer fit and take the in-kernel fallback
+    const int need = (int)std::ceil(eu) + 5 + 3;   // +3: 16-byte aligned origin
+    TmaArgs A;
+    A.BV = (int)std::ceil(ev) + 5;
+    int BU = 0;
+    for (int c : {48, 80, 112, 144, 176, 240})
+        if (c >= need) {
+            BU = c;
+            break;
+        }
+    if (!BU || A.BV > 256) return 1;
+    const size_t stageB = (((size_t)BU * A.BV + 31) & ~(size_t)31) * sizeof(float);
+    int nStages = TMA_STAGES_MAX;
+    while (nStages > 2 && nStages * stageB > 72 * 1024) --nStages;
+    if (nStages * stageB > 200 * 1024) return 1;
+    A.nStages = std::min(nStages, std::max(2, nViews));
+    const cuuint64_t gdim[3] = {(cuuint64_t)g.nu, (cuuint64_t)p.nrows, (cuuint64_t)nViews};
+    const cuuint64_t gstr[2] = {(cuuint64_t)g.nu * sizeof(float), (cuuint64_t)g.nu * p.nrows * sizeof(float)};
+    const cuuint32_t box[3] = {(cuuint32_t)BU, (cuuint32_t)A.BV, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    if (enc(&A.map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(proj), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return 1;
+    A.proj = proj, A.d_views = d_views, A.nViews = nViews, A.p = p, A.vol = vol, A.st = st;
+    if (mode == TIGRE_ATB_FDK) return tma_launch_bu<TIGRE_ATB_FDK, WX, WY, ZR>(BU, A);
+    return tma_launch_bu<TIGRE_ATB_MATCHED, WX, WY, ZR>(BU, A);
 }
 
 }  // namespace
@@ -316,51 +386,12 @@ int tma_launch_bu(int BU, const CUtensorMap& map, const float* proj, const VoxVi
 // gather kernel), a negative status on a CUDA error.
 int launch_atb_tma(const float* proj, const Grid& g, const VoxView* d_views, const VoxView* h_views, int nViews, int mode,
                    const AtbP& p, float* vol, cudaStream_t st) {
-    constexpr int BY = 16, ZR = 8;
     EncodeTiledFn enc = encode_fn();
     if (!enc || !h_views || !proj) return 1;
     if ((g.nu & 3) || (reinterpret_cast<uintptr_t>(proj) & 15) || p.nrows < 1) return 1;   // TMA: 16-byte rows and base
-    if (g.nx < 32 || g.ny < BY || nViews < 2) return 1;                                      // not worth staging
-    // box size: the largest footprint of a tile over a sample of tile positions (the 8 corner tiles of the
-    // slab and its centre) and all views; tiles that still do not fit fall back per view inside the kernel
-    const double cx = 0.5 * (g.nx - 1), cy = 0.5 * (g.ny - 1), cz = 0.5 * (g.nz - 1);
-    double eu = 0, ev = 0;
-    const int xs[3] = {0, std::max(0, (g.nx / 2 / 32) * 32), std::max(0, ((g.nx - 1) / 32) * 32)};
-    const int ys[3] = {0, std::max(0, (g.ny / 2 / BY) * BY), std::max(0, ((g.ny - 1) / BY) * BY)};
-    const int zs[3] = {p.z0, p.z0 + std::max(0, (p.nzs / 2 / ZR) * ZR), p.z0 + std::max(0, ((p.nzs - 1) / ZR) * ZR)};
-    for (int a = 0; a < nViews; ++a)
-        for (int i = 0; i < 27; ++i) {
-            double e1, e2;
-            tile_extent(h_views[a], cx, cy, cz, xs[i % 3], ys[(i / 3) % 3], zs[i / 9], 32, BY, ZR, e1, e2);
-            eu = std::fmax(eu, e1), ev = std::fmax(ev, e2);
-        }
-    if (!(eu < 240.0) || !(ev < 240.0)) return 1;
-    if (g_atb_path == 2) eu *= 0.45, ev *= 0.7;   // test hook: most views no longer fit and take the in-kernel fallback
-    const int need = (int)std::ceil(eu) + 5 + 3;   // +3: 16-byte aligned origin
-    const int BV = (int)std::ceil(ev) + 5;
-    int BU = 0;
-    for (int c : {48, 80, 112, 144, 176, 240})
-        if (c >= need) {
-            BU = c;
-            break;
-        }
-    if (!BU || BV > 256) return 1;
-    const size_t stageB = (((size_t)BU * BV + 31) & ~(size_t)31) * sizeof(float);
-    int nStages = TMA_STAGES_MAX;
-    while (nStages > 2 && nStages * stageB > 100 * 1024) --nStages;
-    if (nStages * stageB > 200 * 1024) return 1;
-    nStages = std::min(nStages, std::max(2, nViews));
-
-    CUtensorMap map;
-    const cuuint64_t gdim[3] = {(cuuint64_t)g.nu, (cuuint64_t)p.nrows, (cuuint64_t)nViews};
-    const cuuint64_t gstr[2] = {(cuuint64_t)g.nu * sizeof(float), (cuuint64_t)g.nu * p.nrows * sizeof(float)};
-    const cuuint32_t box[3] = {(cuuint32_t)BU, (cuuint32_t)BV, 1};
-    const cuuint32_t estr[3] = {1, 1, 1};
-    if (enc(&map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(proj), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return 1;
-    if (mode == TIGRE_ATB_FDK) return tma_launch_bu<TIGRE_ATB_FDK, BY, ZR>(BU, map, proj, d_views, nViews, p, BV, nStages, vol, st);
-    return tma_launch_bu<TIGRE_ATB_MATCHED, BY, ZR>(BU, map, proj, d_views, nViews, p, BV, nStages, vol, st);
+    // tile = 4 x 4 consumer warps of 8 x 4 voxel columns, 16 voxels along z per thread (32 x 16 x 16 voxels per CTA,
+    // 2 CTAs per SM): the best of the configurations measured on C2, C3 and C4 (profiles/r1_atb_tma.md)
+    return tma_config<4, 4, 16>(enc, proj, g, d_views, h_views, nViews, mode, p, vol, st);
 }
 
 }  // namespace tg
