@@ -61,6 +61,7 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, i
 struct StageInfo {   // written by the producer before it arms the stage's full barrier
     int c0, c1;      // absolute detector index of the box origin (u, v)
     int fits, pad;
+    float4 rU, rV, rW, rG, cst;   // the view's table entry: consumers read it here (shared-memory latency, broadcast)
 };
 
 }  // namespace
@@ -103,7 +104,7 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
         uint32_t ph = 1;   // parity of the "stage is free" phase the producer waits for (first pass: free by construction)
         for (int a = 0; a < nViews; ++a) {
             const float4* vp = reinterpret_cast<const float4*>(views + a);
-            const float4 rU = __ldg(vp), rV = __ldg(vp + 1), rW = __ldg(vp + 2);
+            const float4 rU = __ldg(vp), rV = __ldg(vp + 1), rW = __ldg(vp + 2), rG = __ldg(vp + 3), cst = __ldg(vp + 4);
             const float U = fmaf(rU.x, cxf, fmaf(rU.y, cyf, fmaf(rU.z, czf, rU.w)));
             const float V = fmaf(rV.x, cxf, fmaf(rV.y, cyf, fmaf(rV.z, czf, rV.w)));
             const float W = fmaf(rW.x, cxf, fmaf(rW.y, cyf, fmaf(rW.z, czf, rW.w)));
@@ -127,6 +128,7 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
                 }
                 if (a >= nStages) mbar_wait(empty + s, ph);
                 info[s].c0 = c0, info[s].c1 = c1, info[s].fits = fits;
+                info[s].rU = rU, info[s].rV = rV, info[s].rW = rW, info[s].rG = rG, info[s].cst = cst;
                 if (fits) {
                     mbar_arrive_expect_tx(full + s, (uint32_t)(BU * BV * sizeof(float)));
                     tma_load_3d(tiles + (size_t)s * stageElems, &tmap, c0, c1 - p.row0, a, full + s);
@@ -154,16 +156,15 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
     int s = 0;
     uint32_t ph = 0;
     for (int a = 0; a < nViews; ++a) {
-        const float4* vp = reinterpret_cast<const float4*>(views + a);
-        const float4 rU = __ldg(vp), rV = __ldg(vp + 1), rW = __ldg(vp + 2), cst = __ldg(vp + 4);
+        mbar_wait(full + s, ph);
+        const int c0 = info[s].c0, c1 = info[s].c1, fits = info[s].fits;
+        const float4 rU = info[s].rU, rV = info[s].rV, rW = info[s].rW, cst = info[s].cst;
         // the depth row G only enters the FDK weight
-        const float4 rG = MODE == TIGRE_ATB_FDK ? __ldg(vp + 3) : make_float4(0.f, 0.f, 0.f, 1.f);
+        const float4 rG = MODE == TIGRE_ATB_FDK ? info[s].rG : make_float4(0.f, 0.f, 0.f, 1.f);
         const float U0 = fmaf(rU.x, cxf, fmaf(rU.y, cyf, fmaf(rU.z, czf, rU.w)));
         const float V0 = fmaf(rV.x, cxf, fmaf(rV.y, cyf, fmaf(rV.z, czf, rV.w)));
         const float W0 = fmaf(rW.x, cxf, fmaf(rW.y, cyf, fmaf(rW.z, czf, rW.w)));
         const float G0 = fmaf(rG.x, cxf, fmaf(rG.y, cyf, fmaf(rG.z, czf, rG.w)));
-        mbar_wait(full + s, ph);
-        const int c0 = info[s].c0, c1 = info[s].c1, fits = info[s].fits;
         const float* tile = tiles + (size_t)s * stageElems;
         if (!fits) {
             // footprint larger than the staged box: gather this view through L1/L2 (bounds-checked, clamped)

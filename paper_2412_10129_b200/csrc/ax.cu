@@ -259,8 +259,8 @@ __global__ void __launch_bounds__(256) transpose_xy_kernel(const float* __restri
 // ------------------------------------------------------------------------------------------
 template <typename IdxT, bool UNIT, bool COUNT>
 __global__ void __launch_bounds__(AX_TU* AX_TV)
-ax_interp_kernel(const float* __restrict__ vol, const RayView* __restrict__ views, int nViews, AxP p,
-                 float* __restrict__ proj, uint32_t* __restrict__ counts) {
+ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, const RayView* __restrict__ views, int nViews,
+                 AxP p, float* __restrict__ proj, uint32_t* __restrict__ counts) {
     int view, iu, iv;
     if (!ax_decode(p, nViews, view, iu, iv)) return;
     const RayView& rv = views[view];
@@ -294,15 +294,24 @@ ax_interp_kernel(const float* __restrict__ vol, const RayView* __restrict__ view
             if (COUNT) {
                 cnt = (uint32_t)K;
             } else {
-                // centre-index coordinates relative to the volume centre: c = xi - 1/2 - (n-1)/2... kept
-                // as (xi - 1/2) - hn with hn = n/2 so floor() stays an exact integer shift
-                const int hx = p.nx >> 1, hy = p.ny >> 1, hz = p.nz >> 1;
-                const float x0 = (float)(S[0] + lin * d[0] / Lmm - 0.5 - hx);
-                const float y0 = (float)(S[1] + lin * d[1] / Lmm - 0.5 - hy);
+                // centre-index coordinates relative to the volume centre: c = (xi - 1/2) - hn with hn = n/2, so
+                // that floor() stays an exact integer shift and fp32 magnitudes stay <= n/2.
+                // Rays that run mostly along x read the (x,y)-transposed copy of the volume with the roles of
+                // x and y swapped (trilinear interpolation is symmetric under the swap): neighbouring lanes,
+                // which then differ mostly in y, touch neighbouring addresses.
+                const bool useT = UNIT ? false : (volT != nullptr && fabs(d[0]) > fabs(d[1]));
+                const int X = useT ? 1 : 0, Y = useT ? 0 : 1;
+                const int nX = useT ? p.ny : p.nx, nY = useT ? p.nx : p.ny;
+                const int hx = nX >> 1, hy = nY >> 1, hz = p.nz >> 1;
+                const double dX = sel3(X, d[0], d[1], d[2]), dY = sel3(Y, d[0], d[1], d[2]);
+                const double SX = sel3(X, S[0], S[1], S[2]), SY = sel3(Y, S[0], S[1], S[2]);
+                const float x0 = (float)(SX + lin * dX / Lmm - 0.5 - hx);
+                const float y0 = (float)(SY + lin * dY / Lmm - 0.5 - hy);
                 const float z0 = (float)(S[2] + lin * d[2] / Lmm - 0.5 - hz);
-                const float sx = (float)(p.delta * d[0] / Lmm), sy = (float)(p.delta * d[1] / Lmm),
+                const float sx = (float)(p.delta * dX / Lmm), sy = (float)(p.delta * dY / Lmm),
                             sz = (float)(p.delta * d[2] / Lmm);
-                const IdxT pitchY = p.nx, pitchZ = (IdxT)p.nx * p.ny;
+                const float* __restrict__ base = useT ? volT : vol;
+                const IdxT pitchY = nX, pitchZ = (IdxT)p.nx * p.ny;
                 // samples beyond the detector end of the segment are dropped (l_k > |p-S|)
                 const long long Kmax = (long long)floor((Lmm - lin) / p.delta - 0.5) + 1;
                 int Kuse = (int)min(K, max(Kmax, 0LL)), k0 = 0;
@@ -320,8 +329,29 @@ ax_interp_kernel(const float* __restrict__ vol, const RayView* __restrict__ view
                         Kuse = 0;
                     }
                 }
+                // interior samples [kA, kB): all eight taps inside the (slab of the) volume with 0.01 voxel and
+                // one sample to spare, so the loop over them has no bounds checks
+                int kA = Kuse, kB = Kuse;
+                if (!UNIT) {
+                    float tlo = (float)k0, thi = (float)Kuse;   // in units of t = k + 1/2
+                    const float lo3[3] = {(float)(-hx) + 0.01f, (float)(-hy) + 0.01f, (float)(p.zs0 - hz) + 0.01f};
+                    const float hi3[3] = {(float)(nX - 1 - hx) - 0.01f, (float)(nY - 1 - hy) - 0.01f, (float)(p.zs1 - 1 - hz) - 0.01f};
+                    const float c3[3] = {x0, y0, z0}, s3[3] = {sx, sy, sz};
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) {
+                        if (fabsf(s3[q]) > 1e-7f) {
+                            const float t1 = (lo3[q] - c3[q]) / s3[q], t2 = (hi3[q] - c3[q]) / s3[q];
+                            tlo = fmaxf(tlo, fminf(t1, t2)), thi = fminf(thi, fmaxf(t1, t2));
+                        } else if (c3[q] < lo3[q] || c3[q] > hi3[q]) {
+                            thi = tlo - 4.f;
+                        }
+                    }
+                    kA = min(max((int)ceilf(tlo - 0.5f) + 1, k0), Kuse);
+                    kB = min(max((int)floorf(thi - 0.5f), kA), Kuse);
+                }
                 float acc = 0.f;
-                for (int k = k0; k < Kuse; ++k) {
+                // bounds-checked sample (entry / exit ends of the ray, and the row-sum variant)
+                auto checked = [&](int k) {
                     const float t = (float)k + 0.5f;
                     const float x = fmaf(t, sx, x0), y = fmaf(t, sy, y0), z = fmaf(t, sz, z0);
                     const float fx = floorf(x), fy = floorf(y), fz = floorf(z);
@@ -329,13 +359,39 @@ ax_interp_kernel(const float* __restrict__ vol, const RayView* __restrict__ view
                     const int ix = (int)fx + hx, iy = (int)fy + hy, iz = (int)fz + hz;
                     float v = 0.f;
                     if (UNIT) {
-                        const float wx = ((unsigned)ix < (unsigned)p.nx ? 1.f - ax : 0.f) + ((unsigned)(ix + 1) < (unsigned)p.nx ? ax : 0.f);
-                        const float wy = ((unsigned)iy < (unsigned)p.ny ? 1.f - ay : 0.f) + ((unsigned)(iy + 1) < (unsigned)p.ny ? ay : 0.f);
+                        const float wx = ((unsigned)ix < (unsigned)nX ? 1.f - ax : 0.f) + ((unsigned)(ix + 1) < (unsigned)nX ? ax : 0.f);
+                        const float wy = ((unsigned)iy < (unsigned)nY ? 1.f - ay : 0.f) + ((unsigned)(iy + 1) < (unsigned)nY ? ay : 0.f);
                         const float wz = ((unsigned)(iz - p.zs0) < (unsigned)(p.zs1 - p.zs0) ? 1.f - az : 0.f) +
                                          ((unsigned)(iz + 1 - p.zs0) < (unsigned)(p.zs1 - p.zs0) ? az : 0.f);
                         v = wx * wy * wz;
-                    } else if (ix >= 0 && ix + 1 < p.nx && iy >= 0 && iy + 1 < p.ny && iz >= p.zs0 && iz + 1 < p.zs1) {
-                        const float* q = vol + ((IdxT)(iz - p.zs0) * pitchZ + (IdxT)iy * pitchY + ix);
+                    } else {
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) {
+                            const int jx = ix + (c & 1), jy = iy + ((c >> 1) & 1), jz = iz + (c >> 2);
+                            if ((unsigned)jx < (unsigned)nX && (unsigned)jy < (unsigned)nY &&
+                                (unsigned)(jz - p.zs0) < (unsigned)(p.zs1 - p.zs0)) {
+                                const float w = ((c & 1) ? ax : 1.f - ax) * ((c & 2) ? ay : 1.f - ay) * ((c & 4) ? az : 1.f - az);
+                                v = fmaf(w, __ldg(base + ((IdxT)(jz - p.zs0) * pitchZ + (IdxT)jy * pitchY + jx)), v);
+                            }
+                        }
+                    }
+                    acc += v;
+                };
+                int k = k0;
+                for (; k < kA; ++k) checked(k);
+                if (!UNIT && kB > kA) {
+                    // element offset of voxel (centred index 0,0,0) from the slab's first voxel
+                    const float* __restrict__ org = base + ((IdxT)(hz - p.zs0) * pitchZ + (IdxT)hy * pitchY + hx);
+#pragma unroll 2
+                    for (; k < kB; ++k) {
+                        const float t = (float)k + 0.5f;
+                        const float x = fmaf(t, sx, x0), y = fmaf(t, sy, y0), z = fmaf(t, sz, z0);
+                        // floor without the conversion pipe (see floor_magic in atb_common.cuh)
+                        const float mx = (x - 0.5f) + 12582912.0f, my = (y - 0.5f) + 12582912.0f, mz = (z - 0.5f) + 12582912.0f;
+                        const float ax = x - (mx - 12582912.0f), ay = y - (my - 12582912.0f), az = z - (mz - 12582912.0f);
+                        const int ix = __float_as_int(mx) - 0x4B400000, iy = __float_as_int(my) - 0x4B400000,
+                                  iz = __float_as_int(mz) - 0x4B400000;
+                        const float* q = org + ((IdxT)iz * pitchZ + (IdxT)iy * pitchY + (IdxT)ix);
                         const float v000 = __ldg(q), v100 = __ldg(q + 1);
                         const float v010 = __ldg(q + pitchY), v110 = __ldg(q + pitchY + 1);
                         const float v001 = __ldg(q + pitchZ), v101 = __ldg(q + pitchZ + 1);
@@ -343,20 +399,10 @@ ax_interp_kernel(const float* __restrict__ vol, const RayView* __restrict__ view
                         const float c00 = fmaf(ax, v100 - v000, v000), c10 = fmaf(ax, v110 - v010, v010);
                         const float c01 = fmaf(ax, v101 - v001, v001), c11 = fmaf(ax, v111 - v011, v011);
                         const float c0 = fmaf(ay, c10 - c00, c00), c1 = fmaf(ay, c11 - c01, c01);
-                        v = fmaf(az, c1 - c0, c0);
-                    } else {
-#pragma unroll
-                        for (int c = 0; c < 8; ++c) {
-                            const int jx = ix + (c & 1), jy = iy + ((c >> 1) & 1), jz = iz + (c >> 2);
-                            if ((unsigned)jx < (unsigned)p.nx && (unsigned)jy < (unsigned)p.ny &&
-                                (unsigned)(jz - p.zs0) < (unsigned)(p.zs1 - p.zs0)) {
-                                const float w = ((c & 1) ? ax : 1.f - ax) * ((c & 2) ? ay : 1.f - ay) * ((c & 4) ? az : 1.f - az);
-                                v = fmaf(w, __ldg(vol + ((IdxT)(jz - p.zs0) * pitchZ + (IdxT)jy * pitchY + jx)), v);
-                            }
-                        }
+                        acc += fmaf(az, c1 - c0, c0);
                     }
-                    acc += v;
                 }
+                for (; k < Kuse; ++k) checked(k);
                 result = acc * (float)p.delta;
             }
         }
@@ -379,9 +425,9 @@ static void ax_dispatch(const float* vol, const float* volT, const RayView* v, i
         else if (unit) ax_siddon_kernel<IdxT, true, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
         else ax_siddon_kernel<IdxT, false, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
     } else {
-        if (counts) ax_interp_kernel<IdxT, false, true><<<grid, block, 0, st>>>(vol, v, nViews, p, proj, counts);
-        else if (unit) ax_interp_kernel<IdxT, true, false><<<grid, block, 0, st>>>(vol, v, nViews, p, proj, counts);
-        else ax_interp_kernel<IdxT, false, false><<<grid, block, 0, st>>>(vol, v, nViews, p, proj, counts);
+        if (counts) ax_interp_kernel<IdxT, false, true><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
+        else if (unit) ax_interp_kernel<IdxT, true, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
+        else ax_interp_kernel<IdxT, false, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
     }
 }
 
@@ -403,15 +449,16 @@ int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nView
     const long long nblk = (long long)p.nUt * p.nVt * nViews;
     if (nblk <= 0 || nblk > 0x7fffffffLL) return TIGRE_ERR_ARG;
     const size_t nvox = (size_t)g.nx * g.ny * g.nz;
-    // Siddon on real data: an (x,y)-transposed copy of the volume serves the x-dominant rays
     TempBuf vt;
     const float* volT = nullptr;
     int launches = 1;
-    const bool wantT = (mode == TIGRE_AX_SIDDON) && !unit_vol && !count_out && vol && g.nx > 1 && g.ny > 1;
-    if (wantT && vt.alloc(nvox * sizeof(float), st) == TIGRE_OK) volT = vt.as<float>(), launches = 2;
+    // an (x,y)-transposed copy of the volume (of the slab present, in the chunked path) serves the x-dominant rays
+    const int nzT = p.zs1 - p.zs0;
+    const bool wantT = !unit_vol && !count_out && vol && g.nx > 1 && g.ny > 1;
+    if (wantT && vt.alloc((size_t)g.nx * g.ny * nzT * sizeof(float), st) == TIGRE_OK) volT = vt.as<float>(), launches = 2;
     ProfScope ps(PK_AX, st, launches);
     if (volT) {
-        dim3 tb(32, 8), tg_((g.nx + 31) / 32, (g.ny + 31) / 32, g.nz);
+        dim3 tb(32, 8), tg_((g.nx + 31) / 32, (g.ny + 31) / 32, nzT);
         if (tg_.y > 65535 || tg_.z > 65535) volT = nullptr;
         else transpose_xy_kernel<<<tg_, tb, 0, st>>>(vol, vt.as<float>(), g.nx, g.ny);
     }

@@ -75,8 +75,8 @@ int chunked_ax(const float* h_vol, const tigre_geo* geo, const double* angles, i
     const size_t per = (size_t)g.nu * g.nv, slice = (size_t)g.nx * g.ny;
     const size_t perB = per * sizeof(float), sliceB = slice * sizeof(float);
     const size_t budget = device_budget();
-    // Siddon keeps an (x,y)-transposed copy of the slab it projects (launch_ax): one more slab of room
-    const size_t nbufV = mode == TIGRE_AX_SIDDON ? 3 : 2;
+    // launch_ax keeps an (x,y)-transposed copy of the slab it projects: one more slab of room
+    const size_t nbufV = 3;
     int nAb, nPb;
     if (perB * nA + nbufV * sliceB * std::min(g.nz, 8) <= budget) nAb = nA, nPb = 1;
     else nAb = (int)std::min<size_t>((size_t)nA, std::max<size_t>(1, budget / 2 / (2 * perB))), nPb = 2;
