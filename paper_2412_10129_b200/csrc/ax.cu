@@ -257,12 +257,21 @@ __global__ void __launch_bounds__(256) transpose_xy_kernel(const float* __restri
 }
 
 // ------------------------------------------------------------------------------------------
+// Interpolated mode.  Per-ray state produced by the fp64 set-up; all coordinates are centre-index
+// coordinates relative to the volume centre, c = (xi - 1/2) - n/2, in the (possibly swapped) axes X, Y, z.
+struct InterpRay {
+    float x0, y0, z0, sx, sy, sz;   // position at l_in and step per sample
+    int k0, kA, kB, Kuse;           // samples [k0,Kuse); [kA,kB) need no bounds checks
+    bool useT;
+};
+
 template <typename IdxT, bool UNIT, bool COUNT>
 __global__ void __launch_bounds__(AX_TU* AX_TV)
 ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, const RayView* __restrict__ views, int nViews,
                  AxP p, float* __restrict__ proj, uint32_t* __restrict__ counts) {
     int view, iu, iv;
     if (!ax_decode(p, nViews, view, iu, iv)) return;
+    const unsigned wmask = __activemask();   // lanes of this warp that own a pixel (converged here)
     const RayView& rv = views[view];
     const size_t out = ((size_t)view * p.nv + iv) * p.nu + iu;
     // fp64 set-up in voxel-index coordinates (voxel centres at integer + 1/2)
@@ -275,8 +284,16 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     const double h[3] = {p.hxd, p.hyd, p.hzd};
     const int n[3] = {p.nx, p.ny, p.nz};
     const double Lmm = sqrt(d[0] * h[0] * d[0] * h[0] + d[1] * h[1] * d[1] * h[1] + d[2] * h[2] * d[2] * h[2]);
-    float result = 0.f;
     uint32_t cnt = 0;
+    InterpRay r;
+    r.x0 = r.y0 = r.z0 = r.sx = r.sy = r.sz = 0.f;
+    r.k0 = r.kA = r.kB = r.Kuse = 0;
+    // Rays that run mostly along x read the (x,y)-transposed copy of the volume with the roles of x and y
+    // swapped (trilinear interpolation is symmetric under the swap): neighbouring lanes, which then differ
+    // mostly in y, touch neighbouring addresses.
+    r.useT = UNIT ? false : (volT != nullptr && fabs(d[0]) > fabs(d[1]));
+    const int nX = r.useT ? p.ny : p.nx, nY = r.useT ? p.nx : p.ny;
+    const int hx = nX >> 1, hy = nY >> 1, hz = p.nz >> 1;
     if (Lmm > 0.0) {
         // slab clip against B+ = box grown by half a voxel, in mm along the ray
         double lin = 0.0, lout = Lmm;
@@ -291,52 +308,41 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
         }
         if (!miss && lout > lin) {
             const long long K = (long long)ceil((lout - lin) / p.delta);
-            if (COUNT) {
-                cnt = (uint32_t)K;
-            } else {
-                // centre-index coordinates relative to the volume centre: c = (xi - 1/2) - hn with hn = n/2, so
-                // that floor() stays an exact integer shift and fp32 magnitudes stay <= n/2.
-                // Rays that run mostly along x read the (x,y)-transposed copy of the volume with the roles of
-                // x and y swapped (trilinear interpolation is symmetric under the swap): neighbouring lanes,
-                // which then differ mostly in y, touch neighbouring addresses.
-                const bool useT = UNIT ? false : (volT != nullptr && fabs(d[0]) > fabs(d[1]));
-                const int X = useT ? 1 : 0, Y = useT ? 0 : 1;
-                const int nX = useT ? p.ny : p.nx, nY = useT ? p.nx : p.ny;
-                const int hx = nX >> 1, hy = nY >> 1, hz = p.nz >> 1;
+            cnt = (uint32_t)K;
+            if (!COUNT) {
+                const int X = r.useT ? 1 : 0, Y = r.useT ? 0 : 1;
                 const double dX = sel3(X, d[0], d[1], d[2]), dY = sel3(Y, d[0], d[1], d[2]);
                 const double SX = sel3(X, S[0], S[1], S[2]), SY = sel3(Y, S[0], S[1], S[2]);
-                const float x0 = (float)(SX + lin * dX / Lmm - 0.5 - hx);
-                const float y0 = (float)(SY + lin * dY / Lmm - 0.5 - hy);
-                const float z0 = (float)(S[2] + lin * d[2] / Lmm - 0.5 - hz);
-                const float sx = (float)(p.delta * dX / Lmm), sy = (float)(p.delta * dY / Lmm),
-                            sz = (float)(p.delta * d[2] / Lmm);
-                const float* __restrict__ base = useT ? volT : vol;
-                const IdxT pitchY = nX, pitchZ = (IdxT)p.nx * p.ny;
+                r.x0 = (float)(SX + lin * dX / Lmm - 0.5 - hx);
+                r.y0 = (float)(SY + lin * dY / Lmm - 0.5 - hy);
+                r.z0 = (float)(S[2] + lin * d[2] / Lmm - 0.5 - hz);
+                r.sx = (float)(p.delta * dX / Lmm), r.sy = (float)(p.delta * dY / Lmm), r.sz = (float)(p.delta * d[2] / Lmm);
                 // samples beyond the detector end of the segment are dropped (l_k > |p-S|)
                 const long long Kmax = (long long)floor((Lmm - lin) / p.delta - 0.5) + 1;
-                int Kuse = (int)min(K, max(Kmax, 0LL)), k0 = 0;
+                r.Kuse = (int)min(K, max(Kmax, 0LL));
                 if (p.zs0 > 0 || p.zs1 < p.nz) {
                     // only a z-slab of the volume is present: skip the samples none of whose taps can lie in
                     // it (conservative by one sample and 0.01 voxel; taps are bounds-checked anyway)
                     const float za = (float)(p.zs0 - hz) - 1.01f, zb = (float)(p.zs1 - hz) + 0.01f;
-                    if (fabsf(sz) > 1e-9f) {
-                        const float ka = (za - z0) / sz - 0.5f, kb = (zb - z0) / sz - 0.5f;
-                        const float klo = fminf(fmaxf(fminf(ka, kb), -1.f), (float)Kuse + 1.f);
-                        const float khi = fminf(fmaxf(fmaxf(ka, kb), -1.f), (float)Kuse + 1.f);
-                        k0 = max((int)floorf(klo) - 1, 0);
-                        Kuse = min((int)ceilf(khi) + 2, Kuse);
-                    } else if (z0 < za - 1.f || z0 > zb + 1.f) {
-                        Kuse = 0;
+                    if (fabsf(r.sz) > 1e-9f) {
+                        const float ka = (za - r.z0) / r.sz - 0.5f, kb = (zb - r.z0) / r.sz - 0.5f;
+                        const float klo = fminf(fmaxf(fminf(ka, kb), -1.f), (float)r.Kuse + 1.f);
+                        const float khi = fminf(fmaxf(fmaxf(ka, kb), -1.f), (float)r.Kuse + 1.f);
+                        r.k0 = max((int)floorf(klo) - 1, 0);
+                        r.Kuse = min((int)ceilf(khi) + 2, r.Kuse);
+                    } else if (r.z0 < za - 1.f || r.z0 > zb + 1.f) {
+                        r.Kuse = 0;
                     }
+                    r.k0 = min(r.k0, r.Kuse);
                 }
                 // interior samples [kA, kB): all eight taps inside the (slab of the) volume with 0.01 voxel and
-                // one sample to spare, so the loop over them has no bounds checks
-                int kA = Kuse, kB = Kuse;
+                // one sample to spare, so they need no bounds checks
+                r.kA = r.kB = r.Kuse;
                 if (!UNIT) {
-                    float tlo = (float)k0, thi = (float)Kuse;   // in units of t = k + 1/2
+                    float tlo = (float)r.k0, thi = (float)r.Kuse;   // in units of t = k + 1/2
                     const float lo3[3] = {(float)(-hx) + 0.01f, (float)(-hy) + 0.01f, (float)(p.zs0 - hz) + 0.01f};
                     const float hi3[3] = {(float)(nX - 1 - hx) - 0.01f, (float)(nY - 1 - hy) - 0.01f, (float)(p.zs1 - 1 - hz) - 0.01f};
-                    const float c3[3] = {x0, y0, z0}, s3[3] = {sx, sy, sz};
+                    const float c3[3] = {r.x0, r.y0, r.z0}, s3[3] = {r.sx, r.sy, r.sz};
 #pragma unroll
                     for (int q = 0; q < 3; ++q) {
                         if (fabsf(s3[q]) > 1e-7f) {
@@ -346,72 +352,98 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
                             thi = tlo - 4.f;
                         }
                     }
-                    kA = min(max((int)ceilf(tlo - 0.5f) + 1, k0), Kuse);
-                    kB = min(max((int)floorf(thi - 0.5f), kA), Kuse);
+                    r.kA = min(max((int)ceilf(tlo - 0.5f) + 1, r.k0), r.Kuse);
+                    r.kB = min(max((int)floorf(thi - 0.5f), r.kA), r.Kuse);
                 }
-                float acc = 0.f;
-                // bounds-checked sample (entry / exit ends of the ray, and the row-sum variant)
-                auto checked = [&](int k) {
-                    const float t = (float)k + 0.5f;
-                    const float x = fmaf(t, sx, x0), y = fmaf(t, sy, y0), z = fmaf(t, sz, z0);
-                    const float fx = floorf(x), fy = floorf(y), fz = floorf(z);
-                    const float ax = x - fx, ay = y - fy, az = z - fz;
-                    const int ix = (int)fx + hx, iy = (int)fy + hy, iz = (int)fz + hz;
-                    float v = 0.f;
-                    if (UNIT) {
-                        const float wx = ((unsigned)ix < (unsigned)nX ? 1.f - ax : 0.f) + ((unsigned)(ix + 1) < (unsigned)nX ? ax : 0.f);
-                        const float wy = ((unsigned)iy < (unsigned)nY ? 1.f - ay : 0.f) + ((unsigned)(iy + 1) < (unsigned)nY ? ay : 0.f);
-                        const float wz = ((unsigned)(iz - p.zs0) < (unsigned)(p.zs1 - p.zs0) ? 1.f - az : 0.f) +
-                                         ((unsigned)(iz + 1 - p.zs0) < (unsigned)(p.zs1 - p.zs0) ? az : 0.f);
-                        v = wx * wy * wz;
-                    } else {
-#pragma unroll
-                        for (int c = 0; c < 8; ++c) {
-                            const int jx = ix + (c & 1), jy = iy + ((c >> 1) & 1), jz = iz + (c >> 2);
-                            if ((unsigned)jx < (unsigned)nX && (unsigned)jy < (unsigned)nY &&
-                                (unsigned)(jz - p.zs0) < (unsigned)(p.zs1 - p.zs0)) {
-                                const float w = ((c & 1) ? ax : 1.f - ax) * ((c & 2) ? ay : 1.f - ay) * ((c & 4) ? az : 1.f - az);
-                                v = fmaf(w, __ldg(base + ((IdxT)(jz - p.zs0) * pitchZ + (IdxT)jy * pitchY + jx)), v);
-                            }
-                        }
-                    }
-                    acc += v;
-                };
-                int k = k0;
-                for (; k < kA; ++k) checked(k);
-                if (!UNIT && kB > kA) {
-                    // element offset of voxel (centred index 0,0,0) from the slab's first voxel
-                    const float* __restrict__ org = base + ((IdxT)(hz - p.zs0) * pitchZ + (IdxT)hy * pitchY + hx);
-#pragma unroll 2
-                    for (; k < kB; ++k) {
-                        const float t = (float)k + 0.5f;
-                        const float x = fmaf(t, sx, x0), y = fmaf(t, sy, y0), z = fmaf(t, sz, z0);
-                        // floor without the conversion pipe (see floor_magic in atb_common.cuh)
-                        const float mx = (x - 0.5f) + 12582912.0f, my = (y - 0.5f) + 12582912.0f, mz = (z - 0.5f) + 12582912.0f;
-                        const float ax = x - (mx - 12582912.0f), ay = y - (my - 12582912.0f), az = z - (mz - 12582912.0f);
-                        const int ix = __float_as_int(mx) - 0x4B400000, iy = __float_as_int(my) - 0x4B400000,
-                                  iz = __float_as_int(mz) - 0x4B400000;
-                        const float* q = org + ((IdxT)iz * pitchZ + (IdxT)iy * pitchY + (IdxT)ix);
-                        const float v000 = __ldg(q), v100 = __ldg(q + 1);
-                        const float v010 = __ldg(q + pitchY), v110 = __ldg(q + pitchY + 1);
-                        const float v001 = __ldg(q + pitchZ), v101 = __ldg(q + pitchZ + 1);
-                        const float v011 = __ldg(q + pitchZ + pitchY), v111 = __ldg(q + pitchZ + pitchY + 1);
-                        const float c00 = fmaf(ax, v100 - v000, v000), c10 = fmaf(ax, v110 - v010, v010);
-                        const float c01 = fmaf(ax, v101 - v001, v001), c11 = fmaf(ax, v111 - v011, v011);
-                        const float c0 = fmaf(ay, c10 - c00, c00), c1 = fmaf(ay, c11 - c01, c01);
-                        acc += fmaf(az, c1 - c0, c0);
-                    }
-                }
-                for (; k < Kuse; ++k) checked(k);
-                result = acc * (float)p.delta;
             }
         }
     }
     if (COUNT) {
         counts[out] = cnt;
-    } else {
-        proj[out] = p.accumulate ? proj[out] + result : result;
+        return;
     }
+    const float* __restrict__ base = r.useT ? volT : vol;
+    const IdxT pitchY = nX, pitchZ = (IdxT)p.nx * p.ny;
+    // address of the voxel with centred index (0,0,0), relative to the first slice present
+    const float* __restrict__ org = base + ((IdxT)(hz - p.zs0) * pitchZ + (IdxT)hy * pitchY + hx);
+    float acc = 0.f;
+    // bounds-checked sample (entry / exit ends of the ray, and the row-sum variant)
+    auto checked = [&](int k) {
+        const float t = (float)k + 0.5f;
+        const float x = fmaf(t, r.sx, r.x0), y = fmaf(t, r.sy, r.y0), z = fmaf(t, r.sz, r.z0);
+        const float fx = floorf(x), fy = floorf(y), fz = floorf(z);
+        const float ax = x - fx, ay = y - fy, az = z - fz;
+        const int ix = (int)fx + hx, iy = (int)fy + hy, iz = (int)fz + hz;
+        float v = 0.f;
+        if (UNIT) {
+            const float wx = ((unsigned)ix < (unsigned)nX ? 1.f - ax : 0.f) + ((unsigned)(ix + 1) < (unsigned)nX ? ax : 0.f);
+            const float wy = ((unsigned)iy < (unsigned)nY ? 1.f - ay : 0.f) + ((unsigned)(iy + 1) < (unsigned)nY ? ay : 0.f);
+            const float wz = ((unsigned)(iz - p.zs0) < (unsigned)(p.zs1 - p.zs0) ? 1.f - az : 0.f) +
+                             ((unsigned)(iz + 1 - p.zs0) < (unsigned)(p.zs1 - p.zs0) ? az : 0.f);
+            v = wx * wy * wz;
+        } else {
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                const int jx = ix + (c & 1), jy = iy + ((c >> 1) & 1), jz = iz + (c >> 2);
+                if ((unsigned)jx < (unsigned)nX && (unsigned)jy < (unsigned)nY && (unsigned)(jz - p.zs0) < (unsigned)(p.zs1 - p.zs0)) {
+                    const float w = ((c & 1) ? ax : 1.f - ax) * ((c & 2) ? ay : 1.f - ay) * ((c & 4) ? az : 1.f - az);
+                    v = fmaf(w, __ldg(base + ((IdxT)(jz - p.zs0) * pitchZ + (IdxT)jy * pitchY + jx)), v);
+                }
+            }
+        }
+        acc += v;
+    };
+    // interior sample: no bounds checks; floor without the conversion pipe (see floor_magic in atb_common.cuh)
+    auto interior = [&](int k) {
+        const float t = (float)k + 0.5f;
+        const float x = fmaf(t, r.sx, r.x0), y = fmaf(t, r.sy, r.y0), z = fmaf(t, r.sz, r.z0);
+        const float mx = (x - 0.5f) + 12582912.0f, my = (y - 0.5f) + 12582912.0f, mz = (z - 0.5f) + 12582912.0f;
+        const float ax = x - (mx - 12582912.0f), ay = y - (my - 12582912.0f), az = z - (mz - 12582912.0f);
+        const int ix = __float_as_int(mx) - 0x4B400000, iy = __float_as_int(my) - 0x4B400000, iz = __float_as_int(mz) - 0x4B400000;
+        const float* q = org + ((IdxT)iz * pitchZ + (IdxT)iy * pitchY + (IdxT)ix);
+        const float v000 = __ldg(q), v100 = __ldg(q + 1);
+        const float v010 = __ldg(q + pitchY), v110 = __ldg(q + pitchY + 1);
+        const float v001 = __ldg(q + pitchZ), v101 = __ldg(q + pitchZ + 1);
+        const float v011 = __ldg(q + pitchZ + pitchY), v111 = __ldg(q + pitchZ + pitchY + 1);
+        const float c00 = fmaf(ax, v100 - v000, v000), c10 = fmaf(ax, v110 - v010, v010);
+        const float c01 = fmaf(ax, v101 - v001, v001), c11 = fmaf(ax, v111 - v011, v011);
+        const float c0 = fmaf(ay, c10 - c00, c00), c1 = fmaf(ay, c11 - c01, c01);
+        acc += fmaf(az, c1 - c0, c0);
+    };
+    auto sample = [&](int k) {
+        if (!UNIT && (unsigned)(k - r.kA) < (unsigned)(r.kB - r.kA)) interior(k);
+        else checked(k);
+    };
+
+    // The samples of a ray are fixed by the definition (l_in + (k+1/2) delta from ITS entry point), but the
+    // order in which a warp visits them is free.  Neighbouring rays enter the volume at different depths, so
+    // visiting sample k of every lane together scatters the warp over many rows of the volume.  Instead the
+    // warp advances row by row along Y (the in-plane axis the rays run along): in each step every lane
+    // takes the samples of its own ray that fall into the current row, and all lanes stay within the same
+    // two rows of the (transposed) volume.
+    int k = r.k0;
+    const bool live = r.Kuse > r.k0, up = r.sy >= 0.f;
+    const unsigned liveM = __ballot_sync(wmask, live), upM = __ballot_sync(wmask, live && up);
+    const bool steep = fabsf(r.sy) > 0.05f * (fabsf(r.sx) + fabsf(r.sz));
+    const bool lock = liveM != 0 && (upM == liveM || upM == 0) && __ballot_sync(wmask, live && !steep) == 0;
+    if (lock) {
+        const bool wup = upM != 0;
+        const float isy = live ? 1.0f / r.sy : 0.f, cc = live ? fmaf(-r.y0, isy, -0.5f) : 0.f;
+        const int j0 = live ? (int)floorf(fmaf((float)r.k0 + 0.5f, r.sy, r.y0)) : (wup ? 0x7fffffff : (int)0x80000000);
+        const int jw = wup ? __reduce_min_sync(wmask, j0) : __reduce_max_sync(wmask, j0);
+        float Yb = wup ? (float)jw + 1.f : (float)jw;   // far side of the current row in the direction of travel
+        const float dY = wup ? 1.f : -1.f;
+        for (int it = 0; it < nY + 8; ++it) {
+            const float kf = ceilf(fmaf(Yb, isy, cc));
+            const int kend = live ? (int)fminf(fmaxf(kf, (float)k), (float)r.Kuse) : k;
+            for (; k < kend; ++k) sample(k);
+            Yb += dY;
+            if (!__any_sync(wmask, k < r.Kuse)) break;
+        }
+    }
+    for (; k < r.Kuse; ++k) sample(k);   // rays not marched in lockstep (mixed directions, rays across Y), leftovers
+    const float result = acc * (float)p.delta;
+    proj[out] = p.accumulate ? proj[out] + result : result;
 }
 
 template <typename IdxT>
