@@ -393,34 +393,61 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
         }
         acc += v;
     };
-    // interior sample: no bounds checks; floor without the conversion pipe (see floor_magic in atb_common.cuh)
-    auto interior = [&](int k) {
-        const float t = (float)k + 0.5f;
+    // interior sample: no bounds checks; floor without the conversion pipe (see floor_magic in atb_common.cuh).
+    // The element index is formed from the raw bits of (c - 1/2) + 1.5*2^23 (two integer multiply-adds, the
+    // bias of the magic number is folded into `bias`), and the four tap rows are four fixed base pointers.
+    const float *org0 = org, *orgY = org + pitchY, *orgZ = org + pitchZ, *orgYZ = org + pitchZ + pitchY;
+    // keep them four independent 64-bit bases (one IMAD.WIDE per tap row); left to itself the compiler folds
+    // them back into one base plus 64-bit index arithmetic with carry chains in the loop
+    asm volatile("" : "+l"(org0), "+l"(orgY), "+l"(orgZ), "+l"(orgYZ));
+    const uint32_t upY = (uint32_t)pitchY, upZ = (uint32_t)pitchZ, bias = 0x4B400000u * (upZ + upY + 1u);
+    auto interior = [&](float t) {
         const float x = fmaf(t, r.sx, r.x0), y = fmaf(t, r.sy, r.y0), z = fmaf(t, r.sz, r.z0);
         const float mx = (x - 0.5f) + 12582912.0f, my = (y - 0.5f) + 12582912.0f, mz = (z - 0.5f) + 12582912.0f;
         const float ax = x - (mx - 12582912.0f), ay = y - (my - 12582912.0f), az = z - (mz - 12582912.0f);
-        const int ix = __float_as_int(mx) - 0x4B400000, iy = __float_as_int(my) - 0x4B400000, iz = __float_as_int(mz) - 0x4B400000;
-        const float* q = org + ((IdxT)iz * pitchZ + (IdxT)iy * pitchY + (IdxT)ix);
-        const float v000 = __ldg(q), v100 = __ldg(q + 1);
-        const float v010 = __ldg(q + pitchY), v110 = __ldg(q + pitchY + 1);
-        const float v001 = __ldg(q + pitchZ), v101 = __ldg(q + pitchZ + 1);
-        const float v011 = __ldg(q + pitchZ + pitchY), v111 = __ldg(q + pitchZ + pitchY + 1);
+        float v000, v100, v010, v110, v001, v101, v011, v111;
+        if (sizeof(IdxT) == 4) {
+            const int idx = (int)(__float_as_uint(mz) * upZ + __float_as_uint(my) * upY + __float_as_uint(mx) - bias);
+            v000 = __ldg(org0 + idx), v100 = __ldg(org0 + idx + 1);
+            v010 = __ldg(orgY + idx), v110 = __ldg(orgY + idx + 1);
+            v001 = __ldg(orgZ + idx), v101 = __ldg(orgZ + idx + 1);
+            v011 = __ldg(orgYZ + idx), v111 = __ldg(orgYZ + idx + 1);
+        } else {
+            const int ix = __float_as_int(mx) - 0x4B400000, iy = __float_as_int(my) - 0x4B400000, iz = __float_as_int(mz) - 0x4B400000;
+            const float* q = org + ((IdxT)iz * pitchZ + (IdxT)iy * pitchY + (IdxT)ix);
+            v000 = __ldg(q), v100 = __ldg(q + 1);
+            v010 = __ldg(q + pitchY), v110 = __ldg(q + pitchY + 1);
+            v001 = __ldg(q + pitchZ), v101 = __ldg(q + pitchZ + 1);
+            v011 = __ldg(q + pitchZ + pitchY), v111 = __ldg(q + pitchZ + pitchY + 1);
+        }
         const float c00 = fmaf(ax, v100 - v000, v000), c10 = fmaf(ax, v110 - v010, v010);
         const float c01 = fmaf(ax, v101 - v001, v001), c11 = fmaf(ax, v111 - v011, v011);
         const float c0 = fmaf(ay, c10 - c00, c00), c1 = fmaf(ay, c11 - c01, c01);
         acc += fmaf(az, c1 - c0, c0);
     };
-    auto sample = [&](int k) {
-        if (!UNIT && (unsigned)(k - r.kA) < (unsigned)(r.kB - r.kA)) interior(k);
-        else checked(k);
+    // samples [k, kend): the checked ends of the ray around the unchecked interior [kA, kB)
+    auto run = [&](int& k, int kend) {
+        if (UNIT) {
+            for (; k < kend; ++k) checked(k);
+            return;
+        }
+        const int e1 = min(kend, r.kA);
+        for (; k < e1; ++k) checked(k);
+        const int e2 = min(kend, r.kB);
+        if (k < e2) {
+            float t = (float)k + 0.5f;
+            for (; k < e2; ++k, t += 1.f) interior(t);
+        }
+        for (; k < kend; ++k) checked(k);
     };
 
     // The samples of a ray are fixed by the definition (l_in + (k+1/2) delta from ITS entry point), but the
     // order in which a warp visits them is free.  Neighbouring rays enter the volume at different depths, so
     // visiting sample k of every lane together scatters the warp over many rows of the volume.  Instead the
-    // warp advances row by row along Y (the in-plane axis the rays run along): in each step every lane
-    // takes the samples of its own ray that fall into the current row, and all lanes stay within the same
-    // two rows of the (transposed) volume.
+    // warp advances along Y (the in-plane axis the rays run along) two rows at a time: in each step every
+    // lane takes the samples of its own ray that fall into the current pair of rows (4 or 5 of them at a
+    // step of half a voxel, so the lanes' trip counts differ by at most one in five), and all lanes stay
+    // within three adjacent rows of the (transposed) volume.
     int k = r.k0;
     const bool live = r.Kuse > r.k0, up = r.sy >= 0.f;
     const unsigned liveM = __ballot_sync(wmask, live), upM = __ballot_sync(wmask, live && up);
@@ -431,17 +458,17 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
         const float isy = live ? 1.0f / r.sy : 0.f, cc = live ? fmaf(-r.y0, isy, -0.5f) : 0.f;
         const int j0 = live ? (int)floorf(fmaf((float)r.k0 + 0.5f, r.sy, r.y0)) : (wup ? 0x7fffffff : (int)0x80000000);
         const int jw = wup ? __reduce_min_sync(wmask, j0) : __reduce_max_sync(wmask, j0);
-        float Yb = wup ? (float)jw + 1.f : (float)jw;   // far side of the current row in the direction of travel
-        const float dY = wup ? 1.f : -1.f;
-        for (int it = 0; it < nY + 8; ++it) {
+        float Yb = wup ? (float)jw + 2.f : (float)jw - 1.f;   // far side of the current rows in the direction of travel
+        const float dY = wup ? 2.f : -2.f;
+        for (int it = 0; it < nY / 2 + 8; ++it) {
             const float kf = ceilf(fmaf(Yb, isy, cc));
             const int kend = live ? (int)fminf(fmaxf(kf, (float)k), (float)r.Kuse) : k;
-            for (; k < kend; ++k) sample(k);
+            run(k, kend);
             Yb += dY;
             if (!__any_sync(wmask, k < r.Kuse)) break;
         }
     }
-    for (; k < r.Kuse; ++k) sample(k);   // rays not marched in lockstep (mixed directions, rays across Y), leftovers
+    run(k, r.Kuse);   // rays not marched in lockstep (mixed directions, rays across Y), leftovers
     const float result = acc * (float)p.delta;
     proj[out] = p.accumulate ? proj[out] + result : result;
 }
