@@ -32,10 +32,30 @@ from workloads import make_config, phantom_for  # noqa: E402
 METRIC = "Ax ray-samples/s + A^T b voxel-updates/s (one OS-SART iteration)"
 UNIT = "G(samples+updates)/s"
 
-# issue-slot model of the dominant kernel: thread-instructions per unit of work
-# measured by ncu (smsp__inst_executed.sum * 32 / units), see profiles/.
-INSTR_PER_UNIT = {"ax_siddon": 30.0, "ax_interp": 75.0, "atb": 34.0}
+# Roofline of the projector kernels.  They are gather kernels with hundreds of updates per
+# HBM byte: the binding resource is plain-ALU issue slots (and the L1 gather path for the interpolated
+# projector), not HBM.  peak = issue slots per second / ALGORITHMIC thread-instructions per unit of work, the
+# instruction count being the a-priori minimum derived in DESIGN.md (not the kernel's own count):
+#   A^T b          22 per voxel-update   (projective map or its z-incremental form, floor, 4 taps, bilinear, weight)
+#   Ax Siddon      min(18 per segment on the ALUs, 6 L1 wavefronts per warp-step) = 1.5e12 segments/s at 1965 MHz
+#   Ax interpolated  24 L1 wavefronts per warp-sample (8 taps) = 3.9e11 samples/s at 1965 MHz
 SM_COUNT, LANES_PER_CLK = 148, 128          # 4 schedulers x 32 lanes per SM per clock
+
+
+def model_peak(kname, sm_mhz):
+    """G units/s the model allows at the given SM clock."""
+    slots = SM_COUNT * LANES_PER_CLK * sm_mhz * 1e6            # thread-instructions per second
+    wavefronts = SM_COUNT * sm_mhz * 1e6                       # L1 wavefronts per second (1 per clk per SM)
+    if kname == "atb":
+        return slots / 22.0 / 1e9
+    if kname == "ax_siddon":
+        return min(slots / 18.0, wavefronts / 6.0 * 32) / 1e9
+    return min(slots / 40.0, wavefronts / 24.0 * 32) / 1e9    # ax_interp
+
+
+# dram__bytes_read+write per launch of the dominant kernel from the committed ncu captures (profiles/), for
+# the default workload only (C3, one ordered subset = 36 views per launch)
+NCU_TRAFFIC_PER_LAUNCH = {("C3", "ax_siddon"): 1.695e9, ("C3", "atb"): 5.99e8}
 
 
 def subsets_for(rec, nA):
@@ -260,13 +280,21 @@ def main():
     k_units = samples if kind == "ax" else updates
     k_ms = prof["ms"][kind] / K                       # per full pass over all views
     achieved = k_units / (k_ms * 1e-3) / 1e9
-    peak = SM_COUNT * LANES_PER_CLK * sm_max * 1e6 / INSTR_PER_UNIT[kname] / 1e9
+    peak = model_peak(kname, sm_max)
+    n_launch = len(subsets)                           # launches of the dominant kernel per step (one per subset)
     hbm_bytes = (vol.numel() + b.numel()) * 4         # compulsory: volume once + projections once
     roofline = {"kernel": kname, "bound": "alu", "achieved": achieved, "peak": peak,
-                "unit": "Gsamples/s" if kind == "ax" else "Gupdates/s", "frac": achieved / peak, "traffic": None,
-                "peak_source": f"issue slots: {SM_COUNT} SMs x {LANES_PER_CLK} lanes/clk x {sm_max:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz) / "
-                               f"{INSTR_PER_UNIT[kname]} thread-instr per unit (ncu, profiles/)",
+                "unit": "Gsamples/s" if kind == "ax" else "Gupdates/s", "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_PER_LAUNCH.get((rec["name"], kname)) if args.scale == 1 else None,
+                "peak_source": f"model (DESIGN.md section 6): {SM_COUNT} SMs x {LANES_PER_CLK} lanes/clk x {sm_max:.0f} MHz "
+                               f"(MEASURED_PEAKS.json sm_max_mhz) / algorithmic thread-instructions per unit, or the L1 "
+                               f"wavefront bound where lower; HBM is not the bound (see hbm)",
+                "launches_per_step": n_launch, "ms_per_launch": k_ms / n_launch,
+                "units_per_launch": k_units / n_launch,
                 "share_of_step": prof["ms"][kind] / ms, "ms_per_pass": k_ms,
+                "other_kernel": {"kernel": "atb" if kind == "ax" else "ax_" + rec["ax"],
+                                 "achieved": (updates if kind == "ax" else samples) / (prof["ms"]["atb" if kind == "ax" else "ax"] / K * 1e-3) / 1e9,
+                                 "peak": model_peak("atb" if kind == "ax" else "ax_" + rec["ax"], sm_max)},
                 "hbm": {"algorithmic_bytes_per_pass": hbm_bytes, "achieved_gbs": hbm_bytes / (k_ms * 1e-3) / 1e9,
                         "peak_gbs": peaks.get("hbm_gbs"), "note": "compulsory HBM traffic is ~1% of the time: not the bound"}}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,

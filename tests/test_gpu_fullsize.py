@@ -1,0 +1,125 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (C3: one ordered
+subset = 36 interleaved views per launch; C2: all 360 views in one launch), on SAMPLED outputs the fp64
+oracle computes one by one: seeded random rays for Ax, seeded random voxels (all views of the launch) for
+A^T b.  Inputs are seeded uniform-random volumes / projections (no smoothness for fp32 error to hide
+behind).  Tolerances are north_star's: 1e-5 Siddon and matched, 1e-4 interpolated and FDK (rel-L2 over the
+sample).
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from tests import helpers as H
+from workloads import make_config
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+N_RAYS, N_VOX = 200_000, 20_000
+
+
+@pytest.fixture(scope="module")
+def tg():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2412_10129_b200 as m
+    m.version()
+    return m
+
+
+def subset_geometry(name, view_ids):
+    geo, ang, rec = make_config(name)
+    view_ids = np.asarray(view_ids)
+    if geo.rotDetector_a is not None:
+        geo.rotDetector_a = geo.rotDetector_a[view_ids]
+    return geo, ang[view_ids], rec
+
+
+def random_volume(geo, seed):
+    g = torch.Generator(device="cuda").manual_seed(seed)
+    v = torch.rand(geo.vol_shape, generator=g, device="cuda", dtype=torch.float32)
+    return v, v.cpu().numpy()
+
+
+def random_projections(geo, nA, seed):
+    g = torch.Generator(device="cuda").manual_seed(seed)
+    p = torch.rand((nA,) + geo.proj_shape, generator=g, device="cuda", dtype=torch.float32)
+    return p, p.cpu().numpy()
+
+
+def check_ax(tg, geo, ang, vol_d, vol_h, mode, tol, seed):
+    got = tg.Ax(vol_d, geo, ang, mode)
+    ids = np.random.default_rng(seed).integers(0, got.numel(), N_RAYS)
+    ref = orc.ax(vol_h, geo, ang, orc.SIDDON if mode == "siddon" else orc.INTERP, ray_ids=ids)
+    g = got.reshape(-1)[torch.from_numpy(ids).cuda()].cpu().numpy().astype(np.float64)
+    assert np.count_nonzero(ref) > N_RAYS // 10
+    assert H.rel_l2(g, ref) <= tol
+    if mode == "siddon":
+        assert np.array_equal(g == 0, ref == 0)            # the same rays miss the volume
+
+
+def check_atb(tg, geo, ang, proj_d, proj_h, mode, tol, seed):
+    got = tg.Atb(proj_d, geo, ang, mode)
+    ids = np.random.default_rng(seed).integers(0, got.numel(), N_VOX)
+    ref = orc.atb(proj_h, geo, ang, orc.MATCHED if mode == "matched" else orc.FDK, vox_ids=ids)
+    g = got.reshape(-1)[torch.from_numpy(ids).cuda()].cpu().numpy().astype(np.float64)
+    assert H.rel_l2(g, ref) <= tol
+
+
+def test_c3_full_size_siddon_and_matched(tg):
+    # 512^3, 1024x768 half-fan detector; ordered subset 3 of 20 = views 3, 23, 43, ... (36 views per launch)
+    geo, ang, _ = subset_geometry("C3", np.arange(3, 720, 20))
+    vol_d, vol_h = random_volume(geo, 101)
+    check_ax(tg, geo, ang, vol_d, vol_h, "siddon", 1e-5, 1)
+    del vol_d
+    proj_d, proj_h = random_projections(geo, len(ang), 102)
+    for path in (0, 1):                                     # TMA-staged kernel (bench default) and gather kernel
+        tg.set_atb_path(path)
+        try:
+            check_atb(tg, geo, ang, proj_d, proj_h, "matched", 1e-5, 2)
+        finally:
+            tg.set_atb_path(0)
+
+
+def test_c3_full_size_weights_sampled(tg):
+    # row weights 1/(A 1) of one subset at sampled rays; column weights 1/(A^T 1) at sampled voxels (P13)
+    geo, ang, _ = subset_geometry("C3", np.arange(0, 720, 20))
+    W = tg.row_weights(geo, ang, "siddon")
+    ids = np.random.default_rng(3).integers(0, W.numel(), N_RAYS)
+    a1 = orc.ax(np.ones(geo.vol_shape, np.float32), geo, ang, orc.SIDDON, ray_ids=ids)
+    eps = 1e-2 * min(geo.dVoxel)
+    w_ref = np.where(a1 > eps, 1.0 / np.maximum(a1, 1e-300), 0.0)
+    w = W.reshape(-1)[torch.from_numpy(ids).cuda()].cpu().numpy().astype(np.float64)
+    safe = np.abs(a1 - eps) > 1e-3 * eps                    # hard threshold: skip knife-edge rays
+    assert np.array_equal((w == 0)[safe], (w_ref == 0)[safe])
+    nz = safe & (w_ref != 0)
+    assert H.rel_l2(1.0 / w[nz], 1.0 / w_ref[nz]) <= 1e-5
+    V = tg.col_weights(geo, ang, "matched")
+    vid = np.random.default_rng(4).integers(0, V.numel(), N_VOX)
+    at1 = orc.atb(None, geo, ang, orc.MATCHED, vox_ids=vid)
+    v = V.reshape(-1)[torch.from_numpy(vid).cuda()].cpu().numpy().astype(np.float64)
+    assert np.all(v[at1 > 0] > 0) and H.rel_l2(1.0 / v[at1 > 0], at1[at1 > 0]) <= 1e-5
+
+
+def test_c2_full_size_interp_and_fdk(tg):
+    # 256^3, 512x512 detector: interpolated Ax on 36 of the 360 views, FDK-weighted A^T b over all 360 views
+    geo, ang, _ = subset_geometry("C2", np.arange(0, 360, 10))
+    vol_d, vol_h = random_volume(geo, 201)
+    check_ax(tg, geo, ang, vol_d, vol_h, "interp", 1e-4, 5)
+    geo, ang, _ = subset_geometry("C2", np.arange(360))
+    proj_d, proj_h = random_projections(geo, 360, 202)
+    check_atb(tg, geo, ang, proj_d, proj_h, "fdk", 1e-4, 6)
+
+
+def test_c4_full_size_tilted_detectors(tg):
+    # 1024^3 (4.3 GB), 1536^2 detector, per-view detector roll/pitch/yaw and COR offset: interpolated Ax on 4
+    # views, matched A^T b on 16 views (the general, non z-aligned inner loop of the TMA kernel)
+    geo, ang, _ = subset_geometry("C4", np.arange(0, 1600, 400))
+    vol_d, vol_h = random_volume(geo, 301)
+    check_ax(tg, geo, ang, vol_d, vol_h, "interp", 1e-4, 7)
+    del vol_d, vol_h
+    torch.cuda.empty_cache()
+    geo, ang, _ = subset_geometry("C4", np.arange(0, 1600, 100))
+    proj_d, proj_h = random_projections(geo, len(ang), 302)
+    check_atb(tg, geo, ang, proj_d, proj_h, "matched", 1e-5, 8)
