@@ -58,6 +58,22 @@ def model_peak(kname, sm_mhz):
 NCU_TRAFFIC_PER_LAUNCH = {("C3", "ax_siddon"): 1.695e9, ("C3", "atb"): 5.99e8}
 
 
+def max_over_ranks(ms, device="cpu"):
+    """Device time of the slowest rank (the contract's max over ranks); identity without a process group."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms)
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(units_per_rank, ms_step, world):
+    """Replicas only: every rank processes the same units; G units/s over all ranks."""
+    return world * units_per_rank / (ms_step * 1e-3) / 1e9
+
+
 def subsets_for(rec, nA):
     n = 20 if rec["name"] == "C3" else 1
     n = min(n, nA)
@@ -234,12 +250,9 @@ def main():
     tg.profile(False)
     sampler.stop_flag = True
     sampler.join(timeout=2)
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, "cuda")
     ms_step = ms / K
-    value = world * units / (ms_step * 1e-3) / 1e9
+    value = whole_job_value(units, ms_step, world)
 
     # ---- end to end through the C ABI with HOST buffers: b and x in pinned host memory, copied in / out per step
     e2e = None
@@ -257,11 +270,8 @@ def main():
         t1.record()
         barrier()
         ems = t0.elapsed_time(t1)
-        if world > 1:
-            t = torch.tensor([ems], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ems = float(t.item())
-        e2e = {"value": world * units / (ems / K * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ems / K,
+        ems = max_over_ranks(ems, "cuda")
+        e2e = {"value": whole_job_value(units, ems / K, world), "unit": UNIT, "ms_per_step": ems / K,
                "h2d_bytes_per_step": int(b_h.numel() * 4 + x_h.numel() * 4), "d2h_bytes_per_step": int(x_h.numel() * 4)}
         del b_h
 

@@ -318,3 +318,18 @@ def test_atb_tma_and_gather_kernels_match_oracle(tg, case, mode, tol):
     finally:
         tg.set_atb_path(0)
     assert H.rel_l2(out[0], out[1]) <= 2e-6 and H.rel_l2(out[2], out[1]) <= 2e-6
+
+
+def test_c1_against_golden_samples(tg, c1):
+    # the stored oracle values of tests/golden (written by make_golden.py from oracle/ alone)
+    from tests.test_oracle_pins import _golden
+    geo, ang, vol = c1
+    g = _golden()
+    rid, vid = g["ray"][:, 0].astype(np.int64), g["vox"][:, 0].astype(np.int64)
+    sid = host(tg.Ax(dev(vol), geo, ang, "siddon")).ravel()[rid]
+    itp = host(tg.Ax(dev(vol), geo, ang, "interp")).ravel()[rid]
+    assert H.rel_l2(sid, g["ray"][:, 1]) <= 1e-5 and H.rel_l2(itp, g["ray"][:, 2]) <= 1e-4
+    proj = orc.ax(vol, geo, ang, orc.SIDDON).astype(np.float32)
+    mat = host(tg.Atb(dev(proj), geo, ang, "matched")).ravel()[vid]
+    fdk = host(tg.Atb(dev(proj), geo, ang, "fdk")).ravel()[vid]
+    assert H.rel_l2(mat, g["vox"][:, 1]) <= 1e-5 and H.rel_l2(fdk, g["vox"][:, 2]) <= 1e-4

@@ -411,3 +411,33 @@ def test_cgls_with_exact_adjoint_solves_normal_equations():
     ref = np.linalg.lstsq(A, b, rcond=None)[0]
     x, _ = orc.cgls(b.reshape(6, 5, 6), geo, ang, nvox, exact_adjoint=True)
     assert H.rel_l2(x.ravel(), ref) < 1e-4          # finite termination up to conditioning
+
+
+# ------------------------------------------------------------------ regression anchor (tests/golden)
+def _golden():
+    import os
+    rows = {"ray": [], "vox": []}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "c1_oracle_samples.txt")) as f:
+        for line in f:
+            if line.startswith("#"):
+                continue
+            kind, i, a, b = line.split()
+            rows[kind].append((int(i), float(a), float(b)))
+    return {k: np.array(v) for k, v in rows.items()}
+
+
+def test_oracle_reproduces_golden_c1_samples():
+    # values written by tests/golden/make_golden.py from the oracle alone; guards against silent changes of the
+    # oracle's arithmetic (a deliberate change must regenerate the file and say why in the commit message)
+    from workloads import make_config, phantom_for
+    geo, ang, rec = make_config("C1")
+    vol = phantom_for(rec, geo)
+    g = _golden()
+    rid = g["ray"][:, 0].astype(np.int64)
+    assert np.allclose(orc.ax(vol, geo, ang, orc.SIDDON, ray_ids=rid), g["ray"][:, 1], rtol=1e-12, atol=1e-12)
+    assert np.allclose(orc.ax(vol, geo, ang, orc.INTERP, ray_ids=rid), g["ray"][:, 2], rtol=1e-12, atol=1e-12)
+    proj = orc.ax(vol, geo, ang, orc.SIDDON).astype(np.float32)
+    vid = g["vox"][:, 0].astype(np.int64)
+    assert np.allclose(orc.atb(proj, geo, ang, orc.MATCHED, vox_ids=vid), g["vox"][:, 1], rtol=1e-12)
+    assert np.allclose(orc.atb(proj, geo, ang, orc.FDK, vox_ids=vid), g["vox"][:, 2], rtol=1e-12)
+    assert np.count_nonzero(g["ray"][:, 1]) > 24            # the sample is not trivially empty
