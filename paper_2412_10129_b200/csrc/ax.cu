@@ -52,7 +52,7 @@ struct SidRay {
     float eref, fref, mE, mF, imE, imF, sgE, sgF;   // positions are volume-centred: e = xi_E - nE/2
     IdxT stE, stF, sD;                              // signed element strides of one step along E, F, D
     float nextE, nextF;                             // next E / F plane ahead of the ray
-    float kf, acc;
+    float kf, acc, vB;
     IdxT off;                                       // element offset of the current voxel
 };
 
@@ -71,17 +71,13 @@ __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base,
     const float vA = UNIT ? 1.f : __ldg(base + r.off);
     const float vC = UNIT ? 1.f : __ldg(base + offC);
     r.acc = fmaf(s1, vA, r.acc);
-    if (__any_sync(__activemask(), cE && cF)) {
-        // some lane crosses both planes inside this slab: a middle voxel between the two crossings
-        // (for a lane with a single crossing the middle voxel is the end voxel, so nothing changes)
-        const float s2 = fmaxf(se, sf);
-        const IdxT offB = r.off + ((se < sf) ? r.stE : r.stF);
-        const float vB = UNIT ? 1.f : __ldg(base + ((cE && cF) ? offB : offC));
-        r.acc = fmaf(s2 - s1, vB, r.acc);
-        r.acc = fmaf(1.0f - s2, vC, r.acc);
-    } else {
-        r.acc = fmaf(1.0f - s1, vC, r.acc);
-    }
+    // a lane that crosses both planes inside this slab meets a middle voxel between the two crossings; for
+    // the other lanes the middle piece has zero length (its weight multiplies the last value loaded)
+    const bool both = cE && cF;
+    const float s2 = both ? fmaxf(se, sf) : s1;
+    if (both && !UNIT) r.vB = __ldg(base + (r.off + ((se < sf) ? r.stE : r.stF)));
+    r.acc = fmaf(s2 - s1, UNIT ? 1.f : r.vB, r.acc);
+    r.acc = fmaf(1.0f - s2, vC, r.acc);
     if (cE) r.nextE += r.sgE;
     if (cF) r.nextF += r.sgF;
     r.off = offC + r.sD;
@@ -212,7 +208,7 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
                 r.sgE = upE ? 1.f : -1.f, r.sgF = upF ? 1.f : -1.f;
                 r.stE = upE ? sE : -sE, r.stF = upF ? sF : -sF, r.sD = sD;
                 r.off = (IdxT)i0 * sD + (IdxT)ie * sE + (IdxT)jf * sF;   // may be out of range in checked slabs
-                r.kf = 0.f, r.acc = 0.f;
+                r.kf = 0.f, r.acc = 0.f, r.vB = 0.f;
                 const int diE = upE ? 1 : -1, diF = upF ? 1 : -1;
                 const float slo0 = (float)(lo - (double)i0), shiN = (float)(hi - (double)(i1 - 1));
                 const int last = nslab - 1;
