@@ -49,9 +49,12 @@ __device__ __forceinline__ bool ax_decode(const AxP& p, int nViews, int& view, i
 // Per-ray marching state shared by the checked (end slabs) and unchecked (interior) slab steps.
 template <typename IdxT>
 struct SidRay {
-    float eref, fref, mE, mF, imE, imF, sgE, sgF;   // positions are volume-centred: e = xi_E - nE/2
+    float imE, imF, sgE, sgF;                       // 1/mE, 1/mF (1 if the ray never crosses), plane step +-1
     IdxT stE, stF, sD;                              // signed element strides of one step along E, F, D
-    float nextE, nextF;                             // next E / F plane ahead of the ray
+    // distance (in voxels along E / F) from the ray's position at the start of slab 0 to the next E / F plane
+    // ahead of it.  Grows by exactly +-1 per crossing (magnitudes <= n: the adds are exact up to one ulp of the
+    // largest value, they do not accumulate); the crossing's position inside slab k is hE/mE - k, one FFMA.
+    float hE, hF;
     float kf, acc, vB;
     IdxT off;                                       // element offset of the current voxel
 };
@@ -60,11 +63,9 @@ struct SidRay {
 // least 1e-3 voxel away from the lateral faces, so no clipping and no bounds checks are needed.
 template <typename IdxT, bool UNIT>
 __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base, SidRay<IdxT>& r) {
-    const float e0 = fmaf(r.kf, r.mE, r.eref), f0 = fmaf(r.kf, r.mF, r.fref);
-    r.kf += 1.0f;
     // slab-local parameter of the next E / F plane crossing, saturated to [0,1] (1 = not in this slab)
-    const float se = __saturatef((r.nextE - e0) * r.imE);
-    const float sf = __saturatef((r.nextF - f0) * r.imF);
+    const float se = __saturatef(fmaf(r.hE, r.imE, -r.kf)), sf = __saturatef(fmaf(r.hF, r.imF, -r.kf));
+    r.kf += 1.0f;
     const bool cE = se < 1.0f, cF = sf < 1.0f;
     const float s1 = fminf(se, sf);
     const IdxT offC = r.off + (cE ? r.stE : (IdxT)0) + (cF ? r.stF : (IdxT)0);
@@ -78,8 +79,8 @@ __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base,
     if (both && !UNIT) r.vB = __ldg(base + (r.off + ((se < sf) ? r.stE : r.stF)));
     r.acc = fmaf(s2 - s1, UNIT ? 1.f : r.vB, r.acc);
     r.acc = fmaf(1.0f - s2, vC, r.acc);
-    if (cE) r.nextE += r.sgE;
-    if (cF) r.nextF += r.sgF;
+    if (cE) r.hE += r.sgE;
+    if (cF) r.hF += r.sgF;
     r.off = offC + r.sD;
 }
 
@@ -88,10 +89,8 @@ __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base,
 template <typename IdxT, bool UNIT>
 __device__ __forceinline__ void siddon_slab_checked(const float* __restrict__ base, SidRay<IdxT>& r, int& ie, int& jf,
                                                     int diE, int diF, int nE, int nF, float slo, float shi) {
-    const float e0 = fmaf(r.kf, r.mE, r.eref), f0 = fmaf(r.kf, r.mF, r.fref);
+    const float se = __saturatef(fmaf(r.hE, r.imE, -r.kf)), sf = __saturatef(fmaf(r.hF, r.imF, -r.kf));
     r.kf += 1.0f;
-    const float se = __saturatef((r.nextE - e0) * r.imE);
-    const float sf = __saturatef((r.nextF - f0) * r.imF);
     const bool cE = se < 1.0f, cF = sf < 1.0f;
     const float s1 = fminf(fmaxf(fminf(se, sf), slo), shi);
     const float s2 = fminf(fmaxf(fmaxf(se, sf), slo), shi);
@@ -108,8 +107,8 @@ __device__ __forceinline__ void siddon_slab_checked(const float* __restrict__ ba
     // with a single crossing [s1, shi] lies in the end voxel: lenB + lenC = shi - s1
     const float lenE = (cE && cF) ? lenC : lenB + lenC;
     if (lenE > 0.f && vEC && vFC) r.acc = fmaf(lenE, UNIT ? 1.f : __ldg(base + offC), r.acc);
-    if (cE) r.nextE += r.sgE;
-    if (cF) r.nextF += r.sgF;
+    if (cE) r.hE += r.sgE;
+    if (cF) r.hF += r.sgF;
     ie = ieC, jf = jfC;
     r.off = offC + r.sD;
 }
@@ -185,26 +184,25 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
                 // unchecked slabs: k in [kA, kB), each fully inside [max(lo,sa), min(hi,sb)]
                 int kA = (int)ceil(fmax(lo, sa)) - i0, kB = (int)floor(fmin(hi, sb)) - i0;
                 kA = min(max(kA, 0), nslab), kB = min(max(kB, kA), nslab);
-                const int hE = nE >> 1, hF = nF >> 1;   // volume-centred coordinates: |e| <= n/2
                 // state at the START of slab i0 (s = 0), fp64: position, cell index, next plane ahead
                 const double eS = SE + ((double)i0 - SD) * mE, fS = SF + ((double)i0 - SD) * mF;
-                int ie = (int)floor(eS), jf = (int)floor(fS);
+                const int ie0 = (int)floor(eS), jf0 = (int)floor(fS);
+                int ie = ie0, jf = jf0;
                 const bool upE = mE > 0.0, upF = mF > 0.0;
                 // x-dominant rays read the (x,y)-transposed copy so that neighbouring lanes (which differ
                 // mostly in y) touch neighbouring addresses
                 const bool useT = (D == 0) && (volT != nullptr);
-                const float* __restrict__ base = useT ? volT : vol;
+                const float* base = useT ? volT : vol;
+                asm volatile("" : "+l"(base));   // keep the selected pointer in registers (else it is re-selected per slab)
                 const IdxT pX = useT ? (IdxT)p.ny : (IdxT)1, pY = useT ? (IdxT)1 : (IdxT)p.nx, pZ = (IdxT)p.nx * p.ny;
                 const IdxT sD = D == 0 ? pX : (D == 1 ? pY : pZ);
                 const IdxT sE = E == 0 ? pX : (E == 1 ? pY : pZ);
                 const IdxT sF = F == 0 ? pX : (F == 1 ? pY : pZ);
                 SidRay<IdxT> r;
-                r.eref = (float)(eS - (double)hE), r.fref = (float)(fS - (double)hF);
-                r.mE = (float)mE, r.mF = (float)mF;
-                // a ray parallel to the planes (m = 0) never crosses: next = +huge, 1/m := 1
+                // a ray parallel to the planes (m = 0) never crosses: next plane at +huge, 1/m := 1
                 r.imE = mE != 0.0 ? (float)(1.0 / mE) : 1.f, r.imF = mF != 0.0 ? (float)(1.0 / mF) : 1.f;
-                r.nextE = mE != 0.0 ? (float)((upE ? ie + 1 : ie) - hE) : 3.0e38f;
-                r.nextF = mF != 0.0 ? (float)((upF ? jf + 1 : jf) - hF) : 3.0e38f;
+                r.hE = mE != 0.0 ? (float)((double)(upE ? ie0 + 1 : ie0) - eS) : 3.0e38f;
+                r.hF = mF != 0.0 ? (float)((double)(upF ? jf0 + 1 : jf0) - fS) : 3.0e38f;
                 r.sgE = upE ? 1.f : -1.f, r.sgF = upF ? 1.f : -1.f;
                 r.stE = upE ? sE : -sE, r.stF = upF ? sF : -sF, r.sD = sD;
                 r.off = (IdxT)i0 * sD + (IdxT)ie * sE + (IdxT)jf * sF;   // may be out of range in checked slabs
@@ -217,10 +215,11 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
                     siddon_slab_checked<IdxT, UNIT>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
                 for (; k < kB; ++k) siddon_slab_fast<IdxT, UNIT>(base, r);
                 if (k < nslab) {
-                    // recover the cell indices from the plane state for the checked tail
+                    // recover the cell indices from the plane state for the checked tail: hE has moved by
+                    // one per crossing since the start
                     if (kB > kA) {
-                        if (mE != 0.0) ie = (int)r.nextE + hE - (upE ? 1 : 0);
-                        if (mF != 0.0) jf = (int)r.nextF + hF - (upF ? 1 : 0);
+                        if (mE != 0.0) ie = ie0 + (int)rint((double)r.hE - ((double)(upE ? ie0 + 1 : ie0) - eS));
+                        if (mF != 0.0) jf = jf0 + (int)rint((double)r.hF - ((double)(upF ? jf0 + 1 : jf0) - fS));
                     }
                     for (; k < nslab; ++k)
                         siddon_slab_checked<IdxT, UNIT>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
