@@ -114,11 +114,12 @@ __device__ __forceinline__ void siddon_slab_checked(const float* __restrict__ ba
 }
 
 template <typename IdxT, bool UNIT, bool COUNT>
-__global__ void __launch_bounds__(AX_TU* AX_TV)
+__global__ void __launch_bounds__(AX_TU* AX_TV, 8)
 ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, const RayView* __restrict__ views,
                  int nViews, AxP p, float* __restrict__ proj, uint32_t* __restrict__ counts) {
     int view, iu, iv;
     if (!ax_decode(p, nViews, view, iu, iv)) return;
+    const unsigned wmask = __activemask();   // lanes of this warp that own a pixel (converged here)
     const RayView& rv = views[view];
     const size_t out = ((size_t)view * p.nv + iv) * p.nu + iu;
 
@@ -138,8 +139,15 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     const int nD = D == 0 ? p.nx : (D == 1 ? p.ny : p.nz);
     const int nE = E == 0 ? p.nx : (E == 1 ? p.ny : p.nz);
     const int nF = F == 0 ? p.nx : (F == 1 ? p.ny : p.nz);
-    float result = 0.f;
     uint32_t cnt = 0;
+    // marching state, filled by the set-up below; a ray that misses the volume keeps nslab = 0
+    SidRay<IdxT> r;
+    r.imE = r.imF = 1.f, r.sgE = r.sgF = 1.f, r.hE = r.hF = 3.0e38f, r.stE = r.stF = r.sD = 0;
+    r.kf = 0.f, r.acc = 0.f, r.vB = 0.f, r.off = 0;
+    const float* base = vol;
+    int i0 = 0, nslab = 0, kA = 0, kB = 0, ie = 0, jf = 0, ie0 = 0, jf0 = 0, diE = 1, diF = 1;
+    float slo0 = 0.f, shiN = 1.f, scale = 0.f;
+    double hE0 = 0.0, hF0 = 0.0;   // fp64 values r.hE / r.hF start from (0 for a ray that never crosses)
     if (dD != 0.0) {
         const double mE = dE / dD, mF = dF / dD;
         // range of xi_D covered by the segment S->P, clipped to the volume box on all three axes;
@@ -178,61 +186,70 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
                 c += abs((int)floor(SF + (l1 - SD) * mF) - (int)floor(SF + (l0 - SD) * mF));
                 cnt = (uint32_t)c;
             } else {
-                int i0 = (int)floor(lo), i1 = (int)ceil(hi);
-                i0 = max(i0, 0), i1 = min(i1, nD);
-                const int nslab = i1 - i0;
+                int i1 = (int)ceil(hi);
+                i0 = max((int)floor(lo), 0), i1 = min(i1, nD);
+                nslab = i1 - i0;
                 // unchecked slabs: k in [kA, kB), each fully inside [max(lo,sa), min(hi,sb)]
-                int kA = (int)ceil(fmax(lo, sa)) - i0, kB = (int)floor(fmin(hi, sb)) - i0;
+                kA = (int)ceil(fmax(lo, sa)) - i0, kB = (int)floor(fmin(hi, sb)) - i0;
                 kA = min(max(kA, 0), nslab), kB = min(max(kB, kA), nslab);
                 // state at the START of slab i0 (s = 0), fp64: position, cell index, next plane ahead
                 const double eS = SE + ((double)i0 - SD) * mE, fS = SF + ((double)i0 - SD) * mF;
-                const int ie0 = (int)floor(eS), jf0 = (int)floor(fS);
-                int ie = ie0, jf = jf0;
+                ie0 = (int)floor(eS), jf0 = (int)floor(fS);
+                ie = ie0, jf = jf0;
                 const bool upE = mE > 0.0, upF = mF > 0.0;
                 // x-dominant rays read the (x,y)-transposed copy so that neighbouring lanes (which differ
                 // mostly in y) touch neighbouring addresses
                 const bool useT = (D == 0) && (volT != nullptr);
-                const float* base = useT ? volT : vol;
-                asm volatile("" : "+l"(base));   // keep the selected pointer in registers (else it is re-selected per slab)
+                base = useT ? volT : vol;
                 const IdxT pX = useT ? (IdxT)p.ny : (IdxT)1, pY = useT ? (IdxT)1 : (IdxT)p.nx, pZ = (IdxT)p.nx * p.ny;
                 const IdxT sD = D == 0 ? pX : (D == 1 ? pY : pZ);
                 const IdxT sE = E == 0 ? pX : (E == 1 ? pY : pZ);
                 const IdxT sF = F == 0 ? pX : (F == 1 ? pY : pZ);
-                SidRay<IdxT> r;
                 // a ray parallel to the planes (m = 0) never crosses: next plane at +huge, 1/m := 1
                 r.imE = mE != 0.0 ? (float)(1.0 / mE) : 1.f, r.imF = mF != 0.0 ? (float)(1.0 / mF) : 1.f;
-                r.hE = mE != 0.0 ? (float)((double)(upE ? ie0 + 1 : ie0) - eS) : 3.0e38f;
-                r.hF = mF != 0.0 ? (float)((double)(upF ? jf0 + 1 : jf0) - fS) : 3.0e38f;
+                hE0 = mE != 0.0 ? (double)(upE ? ie0 + 1 : ie0) - eS : 0.0;
+                hF0 = mF != 0.0 ? (double)(upF ? jf0 + 1 : jf0) - fS : 0.0;
+                r.hE = mE != 0.0 ? (float)hE0 : 3.0e38f, r.hF = mF != 0.0 ? (float)hF0 : 3.0e38f;
                 r.sgE = upE ? 1.f : -1.f, r.sgF = upF ? 1.f : -1.f;
                 r.stE = upE ? sE : -sE, r.stF = upF ? sF : -sF, r.sD = sD;
                 r.off = (IdxT)i0 * sD + (IdxT)ie * sE + (IdxT)jf * sF;   // may be out of range in checked slabs
-                r.kf = 0.f, r.acc = 0.f, r.vB = 0.f;
-                const int diE = upE ? 1 : -1, diF = upF ? 1 : -1;
-                const float slo0 = (float)(lo - (double)i0), shiN = (float)(hi - (double)(i1 - 1));
-                const int last = nslab - 1;
-                int k = 0;
-                for (; k < kA; ++k)
-                    siddon_slab_checked<IdxT, UNIT>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
-                for (; k < kB; ++k) siddon_slab_fast<IdxT, UNIT>(base, r);
-                if (k < nslab) {
-                    // recover the cell indices from the plane state for the checked tail: hE has moved by
-                    // one per crossing since the start
-                    if (kB > kA) {
-                        if (mE != 0.0) ie = ie0 + (int)rint((double)r.hE - ((double)(upE ? ie0 + 1 : ie0) - eS));
-                        if (mF != 0.0) jf = jf0 + (int)rint((double)r.hF - ((double)(upF ? jf0 + 1 : jf0) - fS));
-                    }
-                    for (; k < nslab; ++k)
-                        siddon_slab_checked<IdxT, UNIT>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
-                }
-                result = r.acc * (float)(Lmm / fabs(dD));
+                diE = upE ? 1 : -1, diF = upF ? 1 : -1;
+                slo0 = (float)(lo - (double)i0), shiN = (float)(hi - (double)(i1 - 1));
+                scale = (float)(Lmm / fabs(dD));
             }
         }
     }
     if (COUNT) {
         counts[out] = cnt;
-    } else {
-        proj[out] = p.accumulate ? proj[out] + result : result;
+        return;
     }
+    asm volatile("" : "+l"(base));   // keep the selected pointer in registers (else it is re-selected per slab)
+    // ---- the march.  Neighbouring rays enter the volume at different depths; if every lane started its
+    // unchecked slabs at its own first one, the warp would be spread over many rows of the volume.  So the head
+    // (clipped, bounds-checked slabs) of each lane is stretched to the deepest start in the warp: from there on
+    // all lanes are in the SAME absolute slab in every iteration of the interior loop.
+    {
+        const bool any = kB > kA;
+        const int jmax = __reduce_max_sync(wmask, any ? i0 + kA : (int)0x80000000);
+        if (any) kA = min(max(kA, jmax - i0), kB);
+    }
+    const int last = nslab - 1;
+    int k = 0;
+    for (; k < kA; ++k)
+        siddon_slab_checked<IdxT, UNIT>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
+    const bool ranFast = kB > k;
+    for (; k < kB; ++k) siddon_slab_fast<IdxT, UNIT>(base, r);
+    if (k < nslab) {
+        // recover the cell indices from the plane state for the checked tail: hE has moved by one per crossing
+        if (ranFast) {
+            if (r.hE < 1.0e38f) ie = ie0 + (int)rint((double)r.hE - hE0);
+            if (r.hF < 1.0e38f) jf = jf0 + (int)rint((double)r.hF - hF0);
+        }
+        for (; k < nslab; ++k)
+            siddon_slab_checked<IdxT, UNIT>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
+    }
+    const float result = r.acc * scale;
+    proj[out] = p.accumulate ? proj[out] + result : result;
 }
 
 // (x,y) transpose of every z-slice: volT[z][x][y] = vol[z][y][x]
