@@ -161,6 +161,9 @@ TIGRE_API int tigre_profile_read(double *ms /*[3]*/, uint64_t *launches /*[3]*/)
 TIGRE_API size_t tigre_workspace_bytes(const tigre_geo *geo, int nA, int op);
 /* tuning knobs of the chunked path: device bytes it may use for slabs (0 = default 3/4 of free) */
 TIGRE_API int tigre_set_chunk_budget(size_t bytes);
+/* what the most recent chunked tigre_Ax / tigre_Atb call of this process moved: bytes copied host->device and
+ * device->host, number of z-slabs and of view batches (any pointer may be NULL) */
+TIGRE_API int tigre_chunk_stats(uint64_t *h2d_bytes, uint64_t *d2h_bytes, int *n_slabs, int *n_batches);
 /* which A^T b kernel runs: 0 (default) = detector footprints staged into shared memory by TMA whenever the
  * problem qualifies (16-byte aligned rows, tiles >= 32x16 voxels), 1 = always the L1/L2 gather kernel.  Both
  * compute the same sums (DESIGN.md O-C); the switch exists for A/B measurement.  2 = the TMA kernel with its

@@ -51,7 +51,7 @@ _LIB = None
 EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_row_weights", "tigre_col_weights", "tigre_residual",
            "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_fdk", "tigre_fdk_filter",
            "tigre_Ax_count", "tigre_plan_create", "tigre_plan_ossart", "tigre_plan_destroy",
-           "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_set_atb_path", "tigre_strerror",
+           "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version"]
 
 
@@ -348,3 +348,10 @@ def version():
 def set_atb_path(path):
     """0 = TMA-staged A^T b kernel when the problem qualifies (default), 1 = gather kernel only."""
     _check(_lib().tigre_set_atb_path(int(path)), "tigre_set_atb_path")
+
+
+def chunk_stats():
+    """(h2d_bytes, d2h_bytes, n_slabs, n_batches) of the most recent chunked Ax / Atb call."""
+    a, b, c, d = C.c_uint64(0), C.c_uint64(0), C.c_int(0), C.c_int(0)
+    _check(_lib().tigre_chunk_stats(C.byref(a), C.byref(b), C.byref(c), C.byref(d)), "tigre_chunk_stats")
+    return a.value, b.value, c.value, d.value

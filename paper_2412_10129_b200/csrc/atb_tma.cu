@@ -2,14 +2,15 @@
 // TMA (BASELINE.json north_star: "each batch's detector footprint is staged into shared memory by TMA,
 // and accumulation stays in registers"; DESIGN.md O-C for what is computed).
 //
-// A CTA owns a tile of 32 x BY x ZR voxels; thread (tx,ty) owns the ZR voxels along z at one (x,y) and
-// keeps their sums in registers over all views.  One extra PRODUCER warp walks the views ahead of the
-// consumers: for each view it projects the 8 corner voxels of the tile (the projective map is quasi-
-// linear, so they bound the footprint), and issues ONE cp.async.bulk.tensor load of the BU x BV pixel box
-// around it into a ring of shared-memory stages (mbarrier full/empty pairs).  TMA zero-fills whatever
-// lies outside the detector, which IS the zero border of the bilinear interpolation, so the consumers
-// read their four taps from shared memory with no bounds checks.  A view whose footprint does not fit
-// the box (extreme magnification / tilt) is flagged and its taps are gathered through L1/L2 instead.
+// A CTA owns a tile of 32 x 16 x 16 voxels: 4 x 4 consumer warps, each 8 (x) x 4 (y) columns of voxels, every
+// thread the 16 voxels along z of one column, their sums in registers over all views.  One extra PRODUCER
+// warp walks the views ahead of the consumers: for each view it projects the 8 corner voxels of the tile (the
+// projective map is quasi-linear, so they bound the footprint), and issues ONE cp.async.bulk.tensor load of
+// the BU x BV pixel box around it into a ring of shared-memory stages (mbarrier full/empty pairs), together
+// with the view's table entry.  TMA zero-fills whatever lies outside the detector, which IS the zero border
+// of the bilinear interpolation, so the consumers read their four taps from shared memory with no bounds
+// checks.  A view whose footprint does not fit the box (extreme magnification / tilt) is flagged and its
+// taps are gathered through L1/L2 instead.
 //
 // Views whose detector columns are parallel to the volume's z axis (every circular-orbit view without
 // detector tilt: rowU.z = rowW.z = rowG.z = 0) take a cheaper inner loop: the magnification, the

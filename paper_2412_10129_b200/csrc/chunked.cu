@@ -21,6 +21,9 @@ namespace tg {
 
 static size_t g_budget = 0;
 size_t chunk_budget() { return g_budget; }
+// bytes copied and chunk counts of the most recent chunked call (tigre_chunk_stats)
+static unsigned long long g_h2d = 0, g_d2h = 0;
+static int g_nslabs = 0, g_nbatches = 0;
 
 namespace {
 
@@ -77,17 +80,26 @@ int chunked_ax(const float* h_vol, const tigre_geo* geo, const double* angles, i
     const size_t budget = device_budget();
     // launch_ax keeps an (x,y)-transposed copy of the slab it projects: one more slab of room
     const size_t nbufV = 3;
+    // Even when everything would fit, large problems are cut into a few pieces so that the pipeline has
+    // something to overlap: >= 2 view batches (the D2H of one hides behind the kernels of the next; the price is
+    // one more H2D pass over the volume, itself hidden) and >= 4 z-slabs (the first upload is the only exposed one).
+    const size_t big = (size_t)256 << 20;
     int nAb, nPb;
-    if (perB * nA + nbufV * sliceB * std::min(g.nz, 8) <= budget) nAb = nA, nPb = 1;
-    else nAb = (int)std::min<size_t>((size_t)nA, std::max<size_t>(1, budget / 2 / (2 * perB))), nPb = 2;
+    if (perB * nA + nbufV * sliceB * std::min(g.nz, 8) <= budget && perB * nA <= big) nAb = nA, nPb = 1;
+    else {
+        nAb = (int)std::min<size_t>((size_t)nA, std::max<size_t>(1, budget / 2 / (2 * perB))), nPb = 2;
+        nAb = std::min(nAb, std::max(1, (nA + 1) / 2));
+    }
     const size_t projB = (size_t)nPb * nAb * perB;
     if (projB + nbufV * sliceB > budget) return TIGRE_ERR_WORKSPACE;
     int nzs = (int)std::min<size_t>((size_t)g.nz, (budget - projB) / (nbufV * sliceB));
+    if ((size_t)g.nz * sliceB > big) nzs = std::min(nzs, std::max(1, (g.nz + 3) / 4));
     const int nSlabs = (g.nz + nzs - 1) / nzs;
     nzs = (g.nz + nSlabs - 1) / nSlabs;   // even slabs
     const int nBatches = (nA + nAb - 1) / nAb;
     const int nVb = nSlabs > 1 ? 2 : 1;
 
+    g_h2d = g_d2h = 0, g_nslabs = nSlabs, g_nbatches = nBatches;
     Side sd;
     TG_TRY(sd.init());
     TempBuf vb[2], pb[2];
@@ -113,6 +125,7 @@ int chunked_ax(const float* h_vol, const tigre_geo* geo, const double* angles, i
             if (nSlabs > 1 || b == 0) {   // a volume that fits in one slab is uploaded once
                 if (islab >= nVb) TG_CUDA(cudaStreamWaitEvent(sd.h2d, sd.freed[islab % nVb], 0));
                 TG_CUDA(cudaMemcpyAsync(V, h_vol + (size_t)z0 * slice, (size_t)nz_s * sliceB, cudaMemcpyHostToDevice, sd.h2d));
+                g_h2d += (unsigned long long)nz_s * sliceB;
                 TG_CUDA(cudaEventRecord(sd.ready[islab % nVb], sd.h2d));
                 TG_CUDA(cudaStreamWaitEvent(st, sd.ready[islab % nVb], 0));
             }
@@ -140,6 +153,7 @@ int chunked_ax(const float* h_vol, const tigre_geo* geo, const double* angles, i
         TG_CUDA(cudaEventRecord(sd.done, st));
         TG_CUDA(cudaStreamWaitEvent(sd.d2h, sd.done, 0));
         TG_CUDA(cudaMemcpyAsync(h_proj + (size_t)a0 * per, P, (size_t)na * perB, cudaMemcpyDeviceToHost, sd.d2h));
+        g_d2h += (unsigned long long)na * perB;
         TG_CUDA(cudaEventRecord(sd.out[b % nPb], sd.d2h));
     }
     for (int i = 0; i < std::min(nPb, nBatches); ++i) TG_CUDA(cudaStreamWaitEvent(st, sd.out[i], 0));
@@ -166,9 +180,11 @@ int chunked_atb(const float* h_proj, const tigre_geo* geo, const double* angles,
     TG_TRY(upload(tab, hv.data(), sizeof(VoxView) * nA, st));
 
     // volume slabs: the whole volume if it fits in half of the budget, else two buffers in that half
+    // (large volumes are cut into >= 2 slabs even if they fit, so that the D2H of one hides behind the next)
+    const size_t big = (size_t)256 << 20;
     int nzs;
-    if ((size_t)g.nz * sliceB <= budget / 2) nzs = g.nz;
-    else nzs = (int)(budget / 2 / (2 * sliceB));
+    if ((size_t)g.nz * sliceB <= budget / 2 && (size_t)g.nz * sliceB <= big) nzs = g.nz;
+    else nzs = (int)std::min<size_t>(budget / 2 / (2 * sliceB), (size_t)std::max(1, (g.nz + 1) / 2));
     if (nzs < 1) return TIGRE_ERR_WORKSPACE;
     const int nSlabs = (g.nz + nzs - 1) / nzs;
     nzs = (g.nz + nSlabs - 1) / nSlabs;
@@ -184,10 +200,12 @@ int chunked_atb(const float* h_proj, const tigre_geo* geo, const double* angles,
     }
     const size_t bandB = (size_t)nrMax * g.nu * sizeof(float);
     if (volB + 2 * bandB > budget) return TIGRE_ERR_WORKSPACE;
-    const int nAb = (int)std::min<size_t>((size_t)nA, (budget - volB) / (2 * bandB));
+    int nAb = (int)std::min<size_t>((size_t)nA, (budget - volB) / (2 * bandB));
+    if (bandB * nA > ((size_t)64 << 20)) nAb = std::min(nAb, std::max(1, (nA + 3) / 4));   // >= 4 batches to overlap
     const int nBatches = (nA + nAb - 1) / nAb;
     const int nPb = nBatches * nSlabs > 1 ? 2 : 1;
 
+    g_h2d = g_d2h = 0, g_nslabs = nSlabs, g_nbatches = nBatches;
     Side sd;
     TG_TRY(sd.init());
     TempBuf vb[2], pb[2];
@@ -213,6 +231,7 @@ int chunked_atb(const float* h_proj, const tigre_geo* geo, const double* angles,
                 const size_t rowBytes = (size_t)nrows * g.nu * sizeof(float);
                 TG_CUDA(cudaMemcpy2DAsync(P, rowBytes, h_proj + ((size_t)a0 * g.nv + row0) * g.nu, per * sizeof(float), rowBytes,
                                           (size_t)na, cudaMemcpyHostToDevice, sd.h2d));
+                g_h2d += (unsigned long long)rowBytes * na;
                 TG_CUDA(cudaEventRecord(sd.ready[ib % nPb], sd.h2d));
                 TG_CUDA(cudaStreamWaitEvent(st, sd.ready[ib % nPb], 0));
                 TG_TRY(launch_atb(P, g, tab.as<VoxView>() + a0, na, mode, false, V, z0, nz_s, b > 0, row0, nrows, clamp, st, hv.data() + a0));
@@ -222,6 +241,7 @@ int chunked_atb(const float* h_proj, const tigre_geo* geo, const double* angles,
         TG_CUDA(cudaEventRecord(sd.done, st));
         TG_CUDA(cudaStreamWaitEvent(sd.d2h, sd.done, 0));
         TG_CUDA(cudaMemcpyAsync(h_vol + (size_t)z0 * slice, V, (size_t)nz_s * sliceB, cudaMemcpyDeviceToHost, sd.d2h));
+        g_d2h += (unsigned long long)nz_s * sliceB;
         TG_CUDA(cudaEventRecord(sd.out[s % nVb], sd.d2h));
     }
     for (int i = 0; i < std::min(nVb, nSlabs); ++i) TG_CUDA(cudaStreamWaitEvent(st, sd.out[i], 0));
@@ -233,6 +253,14 @@ int chunked_atb(const float* h_proj, const tigre_geo* geo, const double* angles,
 }
 
 }  // namespace tg
+
+extern "C" int tigre_chunk_stats(uint64_t* h2d_bytes, uint64_t* d2h_bytes, int* n_slabs, int* n_batches) {
+    if (h2d_bytes) *h2d_bytes = tg::g_h2d;
+    if (d2h_bytes) *d2h_bytes = tg::g_d2h;
+    if (n_slabs) *n_slabs = tg::g_nslabs;
+    if (n_batches) *n_batches = tg::g_nbatches;
+    return TIGRE_OK;
+}
 
 extern "C" int tigre_set_chunk_budget(size_t bytes) {
     tg::g_budget = bytes;
