@@ -25,7 +25,7 @@ namespace tg {
 
 namespace {
 
-constexpr int TMA_STAGES_MAX = 4;
+constexpr int TMA_STAGES_MAX = 8;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
@@ -367,7 +367,7 @@ int tma_config(EncodeTiledFn enc, const float* proj, const Grid& g, const VoxVie
     if (!BU || A.BV > 256) return 1;
     const size_t stageB = (((size_t)BU * A.BV + 31) & ~(size_t)31) * sizeof(float);
     int nStages = TMA_STAGES_MAX;
-    while (nStages > 2 && nStages * stageB > 72 * 1024) --nStages;
+    while (nStages > 2 && nStages * stageB > 100 * 1024) --nStages;
     if (nStages * stageB > 200 * 1024) return 1;
     A.nStages = std::min(nStages, std::max(2, nViews));
     const cuuint64_t gdim[3] = {(cuuint64_t)g.nu, (cuuint64_t)p.nrows, (cuuint64_t)nViews};
