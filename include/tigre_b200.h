@@ -70,7 +70,9 @@ typedef enum tigre_status {
 } tigre_status;
 
 enum { TIGRE_AX_SIDDON = 0, TIGRE_AX_INTERP = 1 };
-enum { TIGRE_ATB_MATCHED = 0, TIGRE_ATB_FDK = 1 };
+enum { TIGRE_ATB_MATCHED = 0, TIGRE_ATB_FDK = 1,
+       /* exact transposes of tigre_Ax (ray-driven scatter of the very same weights) */
+       TIGRE_ATB_EXACT_SIDDON = 2, TIGRE_ATB_EXACT_INTERP = 3 };
 enum { TIGRE_OP_AX = 0, TIGRE_OP_ATB = 1, TIGRE_OP_OSSART = 2, TIGRE_OP_CGLS = 3, TIGRE_OP_FDK = 4 };
 
 /* ---- the projector pair ------------------------------------------------------------------
@@ -90,8 +92,13 @@ TIGRE_API int tigre_Ax(const float *vol, const tigre_geo *geo, const double *ang
  * bilinear detector interpolation with zero border, weight per voxel-view
  *   mode TIGRE_ATB_MATCHED  w = (dx dy dz)/(du dv) * R^2/(r^2 cos gamma)   (P10)
  *   mode TIGRE_ATB_FDK      w = (DSO/(DSO - X'_x))^2
+ *   mode TIGRE_ATB_EXACT_SIDDON / _INTERP   the exact transpose A^T of tigre_Ax in that mode: every ray adds
+ *        (intersection length | trilinear weight x step) x its value to the voxels it meets, so that
+ *        <Ax, y> = <x, A^T y> up to fp32 rounding (the Krylov family wants a matched pair).
+ *        Sums are formed with floating-point atomics: the result is reproducible only up to summation order.
  *   proj dev, [nA][nv][nu], read       vol  dev, [nz][ny][nx], OVERWRITTEN
- * Pinned-host pointers select the chunked path as for tigre_Ax. */
+ * Pinned-host pointers select the chunked path as for tigre_Ax (voxel-driven modes only: the exact modes return
+ * TIGRE_ERR_MEMSPACE for host pointers). */
 TIGRE_API int tigre_Atb(const float *proj, const tigre_geo *geo, const double *angles, int nA, int mode,
               float *vol, void *cuda_stream);
 
@@ -133,7 +140,8 @@ TIGRE_API int tigre_plan_ossart(tigre_plan *plan, const float *b, float *x_inout
                       int nonneg, double *resid_hist, void *cuda_stream);
 TIGRE_API int tigre_plan_destroy(tigre_plan *plan);
 TIGRE_API size_t tigre_plan_bytes(const tigre_plan *plan);
-/* CGLS (textbook recurrences, DESIGN.md O-F), x0 = 0; x_out dev. */
+/* CGLS (textbook recurrences, DESIGN.md O-F), x0 = 0; x_out dev.  atb_mode may be any of the
+ * four tigre_Atb modes (the exact ones must match ax_mode); tigre_ossart / tigre_plan_* take the voxel-driven two. */
 TIGRE_API int tigre_cgls(const float *b, const tigre_geo *geo, const double *angles, int nA, int n_iter,
                int ax_mode, int atb_mode, float *x_out, double *resid_hist, void *cuda_stream);
 /* FDK (DESIGN.md O-D): cosine weight, Ram-Lak ramp filter along u, FDK-weighted

@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libtigre_b200.so")
 AX_SIDDON, AX_INTERP = 0, 1
 ATB_MATCHED, ATB_FDK = 0, 1
 _AX_MODES = {"siddon": 0, "interp": 1, "interpolated": 1, 0: 0, 1: 1}
-_ATB_MODES = {"matched": 0, "fdk": 1, "FDK": 1, 0: 0, 1: 1}
+_ATB_MODES = {"matched": 0, "fdk": 1, "FDK": 1, "exact_siddon": 2, "exact_interp": 3, 0: 0, 1: 1, 2: 2, 3: 3}
 
 _dp = C.POINTER(C.c_double)
 
@@ -169,7 +169,8 @@ def Ax(vol, geo, angles, mode="siddon", out=None):
 
 
 def Atb(proj, geo, angles, mode="matched", out=None):
-    """x = A^T b (voxel-driven).  proj: float32 [nA][nv][nu]."""
+    """x = A^T b.  mode: "matched" / "fdk" (voxel-driven) or "exact_siddon" / "exact_interp" (the exact transpose of
+    Ax in that mode, ray-driven scatter).  proj: float32 [nA][nv][nu]."""
     a, nA = _angles(angles)
     G = _Geo(geo, nA)
     pp = _f32(proj, proj_shape(geo, nA), "proj")

@@ -221,11 +221,16 @@ int tigre_Ax(const float* vol, const tigre_geo* geo, const double* angles, int n
 int tigre_Atb(const float* proj, const tigre_geo* geo, const double* angles, int nA, int mode, float* vol,
               void* cuda_stream) {
     if (!vol || !proj) return TIGRE_ERR_ARG;
-    if (mode != TIGRE_ATB_MATCHED && mode != TIGRE_ATB_FDK) return TIGRE_ERR_ARG;
+    if (mode < TIGRE_ATB_MATCHED || mode > TIGRE_ATB_EXACT_INTERP) return TIGRE_ERR_ARG;
     Tables t;
     TG_TRY(prep(geo, angles, nA, t));
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const MemKind kv = mem_kind(vol), kp = mem_kind(proj);
+    if (mode >= TIGRE_ATB_EXACT_SIDDON) {   // ray-driven exact transpose: device arrays only
+        if (kv != MEM_DEVICE || kp != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+        TG_TRY(t.build_ray(nullptr, nA, st));
+        return launch_ax_adjoint(proj, t.g, t.ray.as<RayView>(), nA, mode - TIGRE_ATB_EXACT_SIDDON, vol, st);
+    }
     if (kv == MEM_PINNED && kp == MEM_PINNED) return chunked_atb(proj, geo, angles, nA, mode, vol, st);
     if (kv != MEM_DEVICE || kp != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
     return device_atb(proj, t, nullptr, nA, mode, false, vol, st);
@@ -449,7 +454,9 @@ int tigre_cgls(const float* b, const tigre_geo* geo, const double* angles, int n
                int atb_mode, float* x, double* resid_hist, void* cuda_stream) {
     if (!b || !x || n_iter < 0) return TIGRE_ERR_ARG;
     if (ax_mode != TIGRE_AX_SIDDON && ax_mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
-    if (atb_mode != TIGRE_ATB_MATCHED && atb_mode != TIGRE_ATB_FDK) return TIGRE_ERR_ARG;
+    if (atb_mode < TIGRE_ATB_MATCHED || atb_mode > TIGRE_ATB_EXACT_INTERP) return TIGRE_ERR_ARG;
+    const bool exact = atb_mode >= TIGRE_ATB_EXACT_SIDDON;
+    if (exact && atb_mode - TIGRE_ATB_EXACT_SIDDON != ax_mode) return TIGRE_ERR_ARG;   // the transpose of THIS Ax
     Tables t;
     TG_TRY(prep(geo, angles, nA, t));
     if (mem_kind(b) != MEM_DEVICE || mem_kind(x) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
@@ -465,12 +472,16 @@ int tigre_cgls(const float* b, const tigre_geo* geo, const double* angles, int n
     TG_TRY(sc.alloc(sizeof(double) * (3 + std::max(n_iter, 1)), st));
     double* d = sc.as<double>();
     TG_TRY(t.build_ray(nullptr, nA, st));
-    TG_TRY(t.build_vox(nullptr, nA, st));
+    if (!exact) TG_TRY(t.build_vox(nullptr, nA, st));
     const RayView* rv = t.ray.as<RayView>();
     const VoxView* vv = t.vox.as<VoxView>();
+    auto AT = [&](const float* y, float* out) -> int {
+        if (exact) return launch_ax_adjoint(y, g, rv, nA, ax_mode, out, st);
+        return launch_atb(y, g, vv, nA, atb_mode, false, out, 0, g.nz, false, 0, g.nv, t.clamp, st, t.hvox.data());
+    };
     TG_CUDA(cudaMemsetAsync(x, 0, sizeof(float) * nvox, st));
     TG_CUDA(cudaMemcpyAsync(r.p, b, sizeof(float) * np, cudaMemcpyDeviceToDevice, st));              // r = b - A 0
-    TG_TRY(launch_atb(r.as<float>(), g, vv, nA, atb_mode, false, s.as<float>(), 0, g.nz, false, 0, g.nv, t.clamp, st, t.hvox.data()));
+    TG_TRY(AT(r.as<float>(), s.as<float>()));
     TG_CUDA(cudaMemcpyAsync(p.p, s.p, sizeof(float) * nvox, cudaMemcpyDeviceToDevice, st));          // p = s
     TG_TRY(launch_dot(s.as<float>(), s.as<float>(), nvox, d + 0, st));                               // gamma
     for (int it = 0; it < n_iter; ++it) {
@@ -478,7 +489,7 @@ int tigre_cgls(const float* b, const tigre_geo* geo, const double* angles, int n
         TG_TRY(launch_dot(q.as<float>(), q.as<float>(), np, d + 2, st));
         TG_TRY(launch_axpy(x, p.as<float>(), d + 0, d + 2, 1.f, nvox, st));                          // x += alpha p
         TG_TRY(launch_axpy(r.as<float>(), q.as<float>(), d + 0, d + 2, -1.f, np, st));               // r -= alpha q
-        TG_TRY(launch_atb(r.as<float>(), g, vv, nA, atb_mode, false, s.as<float>(), 0, g.nz, false, 0, g.nv, t.clamp, st, t.hvox.data()));
+        TG_TRY(AT(r.as<float>(), s.as<float>()));
         TG_TRY(launch_dot(s.as<float>(), s.as<float>(), nvox, d + 1, st));                           // gamma'
         TG_TRY(launch_xpby(p.as<float>(), s.as<float>(), d + 1, d + 0, nvox, st));                   // p = s + beta p
         TG_CUDA(cudaMemcpyAsync(d + 0, d + 1, sizeof(double), cudaMemcpyDeviceToDevice, st));        // gamma = gamma'

@@ -56,12 +56,13 @@ struct SidRay {
     // largest value, they do not accumulate); the crossing's position inside slab k is hE/mE - k, one FFMA.
     float hE, hF;
     float kf, acc, vB;
+    float ys;                                       // scatter (exact adjoint): ray value times the length scale
     IdxT off;                                       // element offset of the current voxel
 };
 
 // One D-slab, interior of the volume: the whole slab [0,1] lies inside the ray's clipped range and at
 // least 1e-3 voxel away from the lateral faces, so no clipping and no bounds checks are needed.
-template <typename IdxT, bool UNIT>
+template <typename IdxT, bool UNIT, bool SCATTER>
 __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base, SidRay<IdxT>& r) {
     // slab-local parameter of the next E / F plane crossing, saturated to [0,1] (1 = not in this slab)
     const float se = __saturatef(fmaf(r.hE, r.imE, -r.kf)), sf = __saturatef(fmaf(r.hF, r.imF, -r.kf));
@@ -69,16 +70,25 @@ __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base,
     const bool cE = se < 1.0f, cF = sf < 1.0f;
     const float s1 = fminf(se, sf);
     const IdxT offC = r.off + (cE ? r.stE : (IdxT)0) + (cF ? r.stF : (IdxT)0);
-    const float vA = UNIT ? 1.f : __ldg(base + r.off);
-    const float vC = UNIT ? 1.f : __ldg(base + offC);
-    r.acc = fmaf(s1, vA, r.acc);
     // a lane that crosses both planes inside this slab meets a middle voxel between the two crossings; for
-    // the other lanes the middle piece has zero length (its weight multiplies the last value loaded)
+    // the other lanes the middle piece has zero length
     const bool both = cE && cF;
     const float s2 = both ? fmaxf(se, sf) : s1;
-    if (both && !UNIT) r.vB = __ldg(base + (r.off + ((se < sf) ? r.stE : r.stF)));
-    r.acc = fmaf(s2 - s1, UNIT ? 1.f : r.vB, r.acc);
-    r.acc = fmaf(1.0f - s2, vC, r.acc);
+    if (SCATTER) {
+        // exact adjoint: the same three lengths, added to the voxels instead of gathered from them
+        float* out = const_cast<float*>(base);
+        atomicAdd(out + r.off, s1 * r.ys);
+        if (both) atomicAdd(out + (r.off + ((se < sf) ? r.stE : r.stF)), (s2 - s1) * r.ys);
+        atomicAdd(out + offC, (1.0f - s2) * r.ys);
+    } else {
+        const float vA = UNIT ? 1.f : __ldg(base + r.off);
+        const float vC = UNIT ? 1.f : __ldg(base + offC);
+        r.acc = fmaf(s1, vA, r.acc);
+        // (the middle weight multiplies the last value loaded when this lane has no middle voxel: times zero)
+        if (both && !UNIT) r.vB = __ldg(base + (r.off + ((se < sf) ? r.stE : r.stF)));
+        r.acc = fmaf(s2 - s1, UNIT ? 1.f : r.vB, r.acc);
+        r.acc = fmaf(1.0f - s2, vC, r.acc);
+    }
     if (cE) r.hE += r.sgE;
     if (cF) r.hF += r.sgF;
     r.off = offC + r.sD;
@@ -86,7 +96,7 @@ __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base,
 
 // One D-slab with clipping to [slo, shi] and per-voxel bounds checks (first / last slabs of a ray and
 // slabs that run within 1e-3 voxel of a lateral face).
-template <typename IdxT, bool UNIT>
+template <typename IdxT, bool UNIT, bool SCATTER>
 __device__ __forceinline__ void siddon_slab_checked(const float* __restrict__ base, SidRay<IdxT>& r, int& ie, int& jf,
                                                     int diE, int diF, int nE, int nF, float slo, float shi) {
     const float se = __saturatef(fmaf(r.hE, r.imE, -r.kf)), sf = __saturatef(fmaf(r.hF, r.imF, -r.kf));
@@ -102,18 +112,25 @@ __device__ __forceinline__ void siddon_slab_checked(const float* __restrict__ ba
     const IdxT offB = eFirst ? r.off + r.stE : r.off + r.stF;
     const bool vB = eFirst ? (vEC && vFA) : (vEA && vFC);
     const float lenA = s1 - slo, lenB = s2 - s1, lenC = shi - s2;
-    if (lenA > 0.f && vEA && vFA) r.acc = fmaf(lenA, UNIT ? 1.f : __ldg(base + r.off), r.acc);
-    if (cE && cF && lenB > 0.f && vB) r.acc = fmaf(lenB, UNIT ? 1.f : __ldg(base + offB), r.acc);
     // with a single crossing [s1, shi] lies in the end voxel: lenB + lenC = shi - s1
     const float lenE = (cE && cF) ? lenC : lenB + lenC;
-    if (lenE > 0.f && vEC && vFC) r.acc = fmaf(lenE, UNIT ? 1.f : __ldg(base + offC), r.acc);
+    if (SCATTER) {
+        float* out = const_cast<float*>(base);
+        if (lenA > 0.f && vEA && vFA) atomicAdd(out + r.off, lenA * r.ys);
+        if (cE && cF && lenB > 0.f && vB) atomicAdd(out + offB, lenB * r.ys);
+        if (lenE > 0.f && vEC && vFC) atomicAdd(out + offC, lenE * r.ys);
+    } else {
+        if (lenA > 0.f && vEA && vFA) r.acc = fmaf(lenA, UNIT ? 1.f : __ldg(base + r.off), r.acc);
+        if (cE && cF && lenB > 0.f && vB) r.acc = fmaf(lenB, UNIT ? 1.f : __ldg(base + offB), r.acc);
+        if (lenE > 0.f && vEC && vFC) r.acc = fmaf(lenE, UNIT ? 1.f : __ldg(base + offC), r.acc);
+    }
     if (cE) r.hE += r.sgE;
     if (cF) r.hF += r.sgF;
     ie = ieC, jf = jfC;
     r.off = offC + r.sD;
 }
 
-template <typename IdxT, bool UNIT, bool COUNT>
+template <typename IdxT, bool UNIT, bool COUNT, bool SCATTER>
 __global__ void __launch_bounds__(AX_TU* AX_TV, 8)
 ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, const RayView* __restrict__ views,
                  int nViews, AxP p, float* __restrict__ proj, uint32_t* __restrict__ counts) {
@@ -143,7 +160,7 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     // marching state, filled by the set-up below; a ray that misses the volume keeps nslab = 0
     SidRay<IdxT> r;
     r.imE = r.imF = 1.f, r.sgE = r.sgF = 1.f, r.hE = r.hF = 3.0e38f, r.stE = r.stF = r.sD = 0;
-    r.kf = 0.f, r.acc = 0.f, r.vB = 0.f, r.off = 0;
+    r.kf = 0.f, r.acc = 0.f, r.vB = 0.f, r.ys = 0.f, r.off = 0;
     const float* base = vol;
     int i0 = 0, nslab = 0, kA = 0, kB = 0, ie = 0, jf = 0, ie0 = 0, jf0 = 0, diE = 1, diF = 1;
     float slo0 = 0.f, shiN = 1.f, scale = 0.f;
@@ -224,6 +241,11 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
         return;
     }
     asm volatile("" : "+l"(base));   // keep the selected pointer in registers (else it is re-selected per slab)
+    if (SCATTER) {
+        // exact adjoint (vol / volT are the OUTPUTS, proj the input): every length of this ray times its value
+        r.ys = proj[out] * scale;
+        if (r.ys == 0.f) nslab = 0, kA = 0, kB = 0;
+    }
     // ---- the march.  Neighbouring rays enter the volume at different depths; if every lane started its
     // unchecked slabs at its own first one, the warp would be spread over many rows of the volume.  So the head
     // (clipped, bounds-checked slabs) of each lane is stretched to the deepest start in the warp: from there on
@@ -236,9 +258,9 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     const int last = nslab - 1;
     int k = 0;
     for (; k < kA; ++k)
-        siddon_slab_checked<IdxT, UNIT>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
+        siddon_slab_checked<IdxT, UNIT, SCATTER>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
     const bool ranFast = kB > k;
-    for (; k < kB; ++k) siddon_slab_fast<IdxT, UNIT>(base, r);
+    for (; k < kB; ++k) siddon_slab_fast<IdxT, UNIT, SCATTER>(base, r);
     if (k < nslab) {
         // recover the cell indices from the plane state for the checked tail: hE has moved by one per crossing
         if (ranFast) {
@@ -246,10 +268,12 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
             if (r.hF < 1.0e38f) jf = jf0 + (int)rint((double)r.hF - hF0);
         }
         for (; k < nslab; ++k)
-            siddon_slab_checked<IdxT, UNIT>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
+            siddon_slab_checked<IdxT, UNIT, SCATTER>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
     }
-    const float result = r.acc * scale;
-    proj[out] = p.accumulate ? proj[out] + result : result;
+    if (!SCATTER) {
+        const float result = r.acc * scale;
+        proj[out] = p.accumulate ? proj[out] + result : result;
+    }
 }
 
 // (x,y) transpose of every z-slice: volT[z][x][y] = vol[z][y][x]
@@ -277,7 +301,7 @@ struct InterpRay {
     bool useT;
 };
 
-template <typename IdxT, bool UNIT, bool COUNT>
+template <typename IdxT, bool UNIT, bool COUNT, bool SCATTER>
 __global__ void __launch_bounds__(AX_TU* AX_TV)
 ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, const RayView* __restrict__ views, int nViews,
                  AxP p, float* __restrict__ proj, uint32_t* __restrict__ counts) {
@@ -379,6 +403,8 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     // address of the voxel with centred index (0,0,0), relative to the first slice present
     const float* __restrict__ org = base + ((IdxT)(hz - p.zs0) * pitchZ + (IdxT)hy * pitchY + hx);
     float acc = 0.f;
+    const float ys = SCATTER ? proj[out] * (float)p.delta : 0.f;   // exact adjoint: vol / volT are outputs, proj the input
+    if (SCATTER && ys == 0.f) r.k0 = r.kA = r.kB = r.Kuse = 0;
     // bounds-checked sample (entry / exit ends of the ray, and the row-sum variant)
     auto checked = [&](int k) {
         const float t = (float)k + 0.5f;
@@ -399,7 +425,9 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
                 const int jx = ix + (c & 1), jy = iy + ((c >> 1) & 1), jz = iz + (c >> 2);
                 if ((unsigned)jx < (unsigned)nX && (unsigned)jy < (unsigned)nY && (unsigned)(jz - p.zs0) < (unsigned)(p.zs1 - p.zs0)) {
                     const float w = ((c & 1) ? ax : 1.f - ax) * ((c & 2) ? ay : 1.f - ay) * ((c & 4) ? az : 1.f - az);
-                    v = fmaf(w, __ldg(base + ((IdxT)(jz - p.zs0) * pitchZ + (IdxT)jy * pitchY + jx)), v);
+                    const IdxT at = (IdxT)(jz - p.zs0) * pitchZ + (IdxT)jy * pitchY + jx;
+                    if (SCATTER) atomicAdd(const_cast<float*>(base) + at, w * ys);   // exact adjoint: same weight, added
+                    else v = fmaf(w, __ldg(base + at), v);
                 }
             }
         }
@@ -437,6 +465,20 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
         const float c0 = fmaf(ay, c10 - c00, c00), c1 = fmaf(ay, c11 - c01, c01);
         acc += fmaf(az, c1 - c0, c0);
     };
+    // the same sample, scattered (exact adjoint): the eight trilinear weights times the ray's value
+    auto interior_scatter = [&](float t) {
+        const float x = fmaf(t, r.sx, r.x0), y = fmaf(t, r.sy, r.y0), z = fmaf(t, r.sz, r.z0);
+        const float mx = (x - 0.5f) + 12582912.0f, my = (y - 0.5f) + 12582912.0f, mz = (z - 0.5f) + 12582912.0f;
+        const float ax = x - (mx - 12582912.0f), ay = y - (my - 12582912.0f), az = z - (mz - 12582912.0f);
+        const int ix = __float_as_int(mx) - 0x4B400000, iy = __float_as_int(my) - 0x4B400000, iz = __float_as_int(mz) - 0x4B400000;
+        float* q = const_cast<float*>(org) + ((IdxT)iz * pitchZ + (IdxT)iy * pitchY + (IdxT)ix);
+        const float w0 = (1.f - az) * ys, w1 = az * ys;
+        const float w00 = (1.f - ay) * w0, w10 = ay * w0, w01 = (1.f - ay) * w1, w11 = ay * w1;
+        atomicAdd(q, (1.f - ax) * w00), atomicAdd(q + 1, ax * w00);
+        atomicAdd(q + pitchY, (1.f - ax) * w10), atomicAdd(q + pitchY + 1, ax * w10);
+        atomicAdd(q + pitchZ, (1.f - ax) * w01), atomicAdd(q + pitchZ + 1, ax * w01);
+        atomicAdd(q + pitchZ + pitchY, (1.f - ax) * w11), atomicAdd(q + pitchZ + pitchY + 1, ax * w11);
+    };
     // samples [k, kend): the checked ends of the ray around the unchecked interior [kA, kB)
     auto run = [&](int& k, int kend) {
         if (UNIT) {
@@ -448,7 +490,10 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
         const int e2 = min(kend, r.kB);
         if (k < e2) {
             float t = (float)k + 0.5f;
-            for (; k < e2; ++k, t += 1.f) interior(t);
+            for (; k < e2; ++k, t += 1.f) {
+                if (SCATTER) interior_scatter(t);
+                else interior(t);
+            }
         }
         for (; k < kend; ++k) checked(k);
     };
@@ -481,8 +526,10 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
         }
     }
     run(k, r.Kuse);   // rays not marched in lockstep (mixed directions, rays across Y), leftovers
-    const float result = acc * (float)p.delta;
-    proj[out] = p.accumulate ? proj[out] + result : result;
+    if (!SCATTER) {
+        const float result = acc * (float)p.delta;
+        proj[out] = p.accumulate ? proj[out] + result : result;
+    }
 }
 
 template <typename IdxT>
@@ -492,13 +539,13 @@ static void ax_dispatch(const float* vol, const float* volT, const RayView* v, i
     const long long nblk = (long long)p.nUt * p.nVt * nViews;
     dim3 grid((unsigned)nblk);
     if (mode == TIGRE_AX_SIDDON) {
-        if (counts) ax_siddon_kernel<IdxT, false, true><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
-        else if (unit) ax_siddon_kernel<IdxT, true, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
-        else ax_siddon_kernel<IdxT, false, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
+        if (counts) ax_siddon_kernel<IdxT, false, true, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
+        else if (unit) ax_siddon_kernel<IdxT, true, false, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
+        else ax_siddon_kernel<IdxT, false, false, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
     } else {
-        if (counts) ax_interp_kernel<IdxT, false, true><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
-        else if (unit) ax_interp_kernel<IdxT, true, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
-        else ax_interp_kernel<IdxT, false, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
+        if (counts) ax_interp_kernel<IdxT, false, true, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
+        else if (unit) ax_interp_kernel<IdxT, true, false, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
+        else ax_interp_kernel<IdxT, false, false, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
     }
 }
 
@@ -535,6 +582,60 @@ int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nView
     }
     if (nvox < (1ull << 31)) ax_dispatch<int>(vol, volT, d_views, nViews, p, mode, unit_vol, proj, count_out, st);
     else ax_dispatch<long long>(vol, volT, d_views, nViews, p, mode, unit_vol, proj, count_out, st);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+
+// vol[z][y][x] += volT[z][x][y]
+__global__ void __launch_bounds__(256) transpose_add_kernel(const float* __restrict__ inT, float* __restrict__ out, int nx, int ny) {
+    __shared__ float tile[32][33];
+    const size_t slice = (size_t)nx * ny * blockIdx.z;
+    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
+    for (int j = threadIdx.y; j < 32; j += 8) {
+        const int y = y0 + threadIdx.x, x = x0 + j;
+        if (x < nx && y < ny) tile[j][threadIdx.x] = inT[slice + (size_t)x * ny + y];
+    }
+    __syncthreads();
+    for (int j = threadIdx.y; j < 32; j += 8) {
+        const int x = x0 + threadIdx.x, y = y0 + j;
+        if (x < nx && y < ny) out[slice + (size_t)y * nx + x] += tile[threadIdx.x][j];
+    }
+}
+
+// Exact adjoint of launch_ax ("matched" pairs for the Krylov family): the
+// same ray march, every (length or trilinear weight) x ray value ADDED to its voxel (red.global.add.f32).
+// x-dominant rays scatter into a transposed scratch volume that is added back at the end.
+int launch_ax_adjoint(const float* proj, const Grid& g, const RayView* d_views, int nViews, int mode, float* vol,
+                      cudaStream_t st) {
+    if (mode != TIGRE_AX_SIDDON && mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
+    AxP p;
+    p.nx = g.nx, p.ny = g.ny, p.nz = g.nz, p.nu = g.nu, p.nv = g.nv;
+    p.hx = (float)g.dx, p.hy = (float)g.dy, p.hz = (float)g.dz;
+    p.hxd = g.dx, p.hyd = g.dy, p.hzd = g.dz;
+    p.delta = g.accuracy * fmin(g.dx, fmin(g.dy, g.dz));
+    p.iv0 = 0, p.iv1 = g.nv, p.zs0 = 0, p.zs1 = g.nz;
+    p.nUt = (g.nu + AX_TU - 1) / AX_TU, p.nVt = (g.nv + AX_TV - 1) / AX_TV;
+    p.accumulate = 0;
+    const long long nblk = (long long)p.nUt * p.nVt * nViews;
+    if (nblk <= 0 || nblk > 0x7fffffffLL) return TIGRE_ERR_ARG;
+    const size_t nvox = (size_t)g.nx * g.ny * g.nz;
+    TempBuf vt;
+    float* volT = nullptr;
+    dim3 tb(32, 8), tgd((g.nx + 31) / 32, (g.ny + 31) / 32, g.nz);
+    if (g.nx > 1 && g.ny > 1 && tgd.y <= 65535 && tgd.z <= 65535 && vt.alloc(nvox * sizeof(float), st) == TIGRE_OK) volT = vt.as<float>();
+    ProfScope ps(PK_ATB, st, volT ? 2 : 1);
+    TG_CUDA(cudaMemsetAsync(vol, 0, nvox * sizeof(float), st));
+    if (volT) TG_CUDA(cudaMemsetAsync(volT, 0, nvox * sizeof(float), st));
+    dim3 block(AX_TU, AX_TV), grid((unsigned)nblk);
+    float* pin = const_cast<float*>(proj);   // read only by the SCATTER instantiations
+    if (nvox < (1ull << 31)) {
+        if (mode == TIGRE_AX_SIDDON) ax_siddon_kernel<int, false, false, true><<<grid, block, 0, st>>>(vol, volT, d_views, nViews, p, pin, nullptr);
+        else ax_interp_kernel<int, false, false, true><<<grid, block, 0, st>>>(vol, volT, d_views, nViews, p, pin, nullptr);
+    } else {
+        if (mode == TIGRE_AX_SIDDON) ax_siddon_kernel<long long, false, false, true><<<grid, block, 0, st>>>(vol, volT, d_views, nViews, p, pin, nullptr);
+        else ax_interp_kernel<long long, false, false, true><<<grid, block, 0, st>>>(vol, volT, d_views, nViews, p, pin, nullptr);
+    }
+    if (volT) transpose_add_kernel<<<tgd, tb, 0, st>>>(volT, vol, g.nx, g.ny);
     TG_CUDA(cudaGetLastError());
     return TIGRE_OK;
 }

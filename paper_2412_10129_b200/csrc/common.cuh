@@ -106,6 +106,9 @@ struct AxSub {
 };
 int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nViews, int mode, bool unit_vol,
               bool accumulate, float* proj, uint32_t* count_out, cudaStream_t st, const AxSub* sub = nullptr);
+// exact adjoint of launch_ax (ray-driven scatter of the same weights); vol [nz][ny][nx] is overwritten
+int launch_ax_adjoint(const float* proj, const Grid& g, const RayView* d_views, int nViews, int mode, float* vol,
+                      cudaStream_t st);
 // backprojection of nViews views given their VoxView table (device) into z-slices [z0, z0+nzs) of a
 // volume whose full height is g.nz; vol points at slice z0.  accumulate: vol += instead of vol =.
 //   unit_proj: treat projections as all ones (column sums A^T 1), proj may be NULL
