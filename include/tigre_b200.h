@@ -152,6 +152,21 @@ TIGRE_API int tigre_fdk(const float *b, const tigre_geo *geo, const double *angl
 TIGRE_API int tigre_fdk_filter(const float *b, const tigre_geo *geo, const double *angles, int nA, float *q,
                      void *cuda_stream);
 
+/* ---- total variation (section 2.2.3 eqs. 7-8; P20-P22) ----------
+ * AwTV(x) = sum_p sqrt(w_x dx^2 + w_y dy^2 + w_z dz^2 + eps), backward differences d_a = x[p] - x[p - e_a], weights
+ * w_a = exp(-(d_a/delta)^2), over the voxels that have all their backward neighbours (an axis of length 1 drops
+ * out: nz = 1 is the paper's 2-D formula).  delta <= 0 or infinite selects the plain TV norm (w = 1).
+ * x dev [nz][ny][nx].  tigre_awtv: *value (host) = AwTV(x); synchronises.  tigre_awtv_gradient: g dev (same
+ * shape) = dAwTV/dx, the weights differentiated too; *value and *grad_norm2 (host, each may be NULL) receive
+ * AwTV(x) and ||g||_2^2 from the same pass (the call synchronises only if one of them is asked for).
+ * tigre_minimize_awtv: n_steps of x <- x - alpha g/||g||_2 in place (the "gradient descent minimizer" of PAPER.md:169;
+ * stops moving when the gradient vanishes); asynchronous. */
+TIGRE_API int tigre_awtv(const float *x, int nx, int ny, int nz, float delta, float eps, double *value, void *cuda_stream);
+TIGRE_API int tigre_awtv_gradient(const float *x, int nx, int ny, int nz, float delta, float eps, float *g, double *value,
+                        double *grad_norm2, void *cuda_stream);
+TIGRE_API int tigre_minimize_awtv(float *x_inout, int nx, int ny, int nz, float delta, float eps, float alpha, int n_steps,
+                        void *cuda_stream);
+
 /* ---- measurement helpers -------------------------------------------------------------------
  * Exact count of ray-samples of one tigre_Ax call without marching the data (BASELINE metric:
  * Siddon = non-zero voxel segments; interpolated = samples K inside the grown box).

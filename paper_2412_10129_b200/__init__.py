@@ -50,7 +50,7 @@ class TigreError(RuntimeError):
 _LIB = None
 EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_row_weights", "tigre_col_weights", "tigre_residual",
            "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_fdk", "tigre_fdk_filter",
-           "tigre_Ax_count", "tigre_plan_create", "tigre_plan_ossart", "tigre_plan_destroy",
+           "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_ossart", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version"]
 
@@ -356,3 +356,41 @@ def chunk_stats():
     a, b, c, d = C.c_uint64(0), C.c_uint64(0), C.c_int(0), C.c_int(0)
     _check(_lib().tigre_chunk_stats(C.byref(a), C.byref(b), C.byref(c), C.byref(d)), "tigre_chunk_stats")
     return a.value, b.value, c.value, d.value
+
+
+# ------------------------------------------------------------------ TV / AwTV
+def _dims(x):
+    if x.dim() != 3:
+        raise ValueError("expected a [nz][ny][nx] volume")
+    return int(x.shape[2]), int(x.shape[1]), int(x.shape[0])
+
+
+def _delta(delta):
+    return C.c_float(0.0 if delta is None or not np.isfinite(delta) else float(delta))
+
+
+def awtv(x, delta=None, eps=0.0):
+    """AwTV(x) of PAPER.md eq. 7 in 3-D (delta None / inf: the TV norm)."""
+    nx, ny, nz = _dims(x)
+    v = C.c_double(0.0)
+    _check(_lib().tigre_awtv(_f32(x), nx, ny, nz, _delta(delta), C.c_float(eps), C.byref(v), _stream(x)), "tigre_awtv")
+    return v.value
+
+
+def awtv_gradient(x, delta=None, eps=1e-8, return_scalars=False):
+    """dAwTV/dx; with return_scalars also (AwTV(x), ||g||^2) from the same pass."""
+    nx, ny, nz = _dims(x)
+    g = _new(tuple(x.shape), like=x)
+    v, n2 = C.c_double(0.0), C.c_double(0.0)
+    _check(_lib().tigre_awtv_gradient(_f32(x), nx, ny, nz, _delta(delta), C.c_float(eps), _f32(g),
+                                      C.byref(v) if return_scalars else None, C.byref(n2) if return_scalars else None,
+                                      _stream(x)), "tigre_awtv_gradient")
+    return (g, v.value, n2.value) if return_scalars else g
+
+
+def minimize_awtv(x, n_steps, alpha, delta=None, eps=1e-8):
+    """In place: n_steps of x <- x - alpha g/||g||_2."""
+    nx, ny, nz = _dims(x)
+    _check(_lib().tigre_minimize_awtv(_f32(x), nx, ny, nz, _delta(delta), C.c_float(eps), C.c_float(alpha), int(n_steps),
+                                      _stream(x)), "tigre_minimize_awtv")
+    return x

@@ -533,6 +533,53 @@ int tigre_fdk(const float* b, const tigre_geo* geo, const double* angles, int nA
     return launch_scale(x, (float)(M_PI / (double)nA), (size_t)g.nx * g.ny * g.nz, st);
 }
 
+// ---------------------------------------------------------------- TV / AwTV (tv.cu)
+int tigre_awtv_gradient(const float* x, int nx, int ny, int nz, float delta, float eps, float* g, double* value,
+                        double* grad_norm2, void* cuda_stream) {
+    if (!x || nx <= 0 || ny <= 0 || nz <= 0 || !(eps >= 0.f)) return TIGRE_ERR_ARG;
+    TG_TRY(ensure_device());
+    if (mem_kind(x) != MEM_DEVICE || (g && mem_kind(g) != MEM_DEVICE)) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    TempBuf acc;
+    const bool scal = value || grad_norm2;
+    if (scal) {
+        TG_TRY(acc.alloc(2 * sizeof(double), st));
+        TG_CUDA(cudaMemsetAsync(acc.p, 0, 2 * sizeof(double), st));
+    }
+    double* d = acc.as<double>();
+    TG_TRY(launch_tv_gradient(x, nx, ny, nz, delta, eps, g, value ? d : nullptr, (grad_norm2 && g) ? d + 1 : nullptr, st));
+    if (scal) {
+        double h[2] = {0, 0};
+        TG_CUDA(cudaMemcpyAsync(h, d, sizeof h, cudaMemcpyDeviceToHost, st));
+        TG_CUDA(cudaStreamSynchronize(st));
+        if (value) *value = h[0];
+        if (grad_norm2) *grad_norm2 = h[1];
+    }
+    return TIGRE_OK;
+}
+
+int tigre_awtv(const float* x, int nx, int ny, int nz, float delta, float eps, double* value, void* cuda_stream) {
+    if (!value) return TIGRE_ERR_ARG;
+    return tigre_awtv_gradient(x, nx, ny, nz, delta, eps, nullptr, value, nullptr, cuda_stream);
+}
+
+int tigre_minimize_awtv(float* x, int nx, int ny, int nz, float delta, float eps, float alpha, int n_steps, void* cuda_stream) {
+    if (!x || nx <= 0 || ny <= 0 || nz <= 0 || n_steps < 0 || !(eps >= 0.f)) return TIGRE_ERR_ARG;
+    TG_TRY(ensure_device());
+    if (mem_kind(x) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n = (size_t)nx * ny * nz;
+    TempBuf g, acc;
+    TG_TRY(g.alloc(n * sizeof(float), st));
+    TG_TRY(acc.alloc(sizeof(double) * std::max(n_steps, 1), st));
+    TG_CUDA(cudaMemsetAsync(acc.p, 0, sizeof(double) * std::max(n_steps, 1), st));
+    for (int it = 0; it < n_steps; ++it) {
+        TG_TRY(launch_tv_gradient(x, nx, ny, nz, delta, eps, g.as<float>(), nullptr, acc.as<double>() + it, st));
+        TG_TRY(launch_tv_step(x, g.as<float>(), alpha, acc.as<double>() + it, n, st));
+    }
+    return TIGRE_OK;
+}
+
 size_t tigre_workspace_bytes(const tigre_geo* geo, int nA, int op) {
     if (!geo || nA <= 0) return 0;
     const size_t per = (size_t)geo->nDetector[0] * geo->nDetector[1] * sizeof(float);

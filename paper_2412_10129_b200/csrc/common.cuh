@@ -137,6 +137,12 @@ int launch_fdk_filter(const float* b, const Grid& g, const double* d_dsd, const 
                       float* q, cudaStream_t st);
 int launch_count_reduce(const uint32_t* c, size_t n, unsigned long long* d_total, cudaStream_t st);
 
+// TV / AwTV (tv.cu): value and/or gradient in one pass (g, d_val, d_gg may be NULL; accumulators pre-zeroed);
+// normalised descent step x -= alpha g / sqrt(*d_gg)
+int launch_tv_gradient(const float* x, int nx, int ny, int nz, float delta, float eps, float* g, double* d_val, double* d_gg,
+                       cudaStream_t st);
+int launch_tv_step(float* x, const float* g, float alpha, const double* d_gg, size_t n, cudaStream_t st);
+
 // chunked (pinned host) path
 int chunked_ax(const float* h_vol, const tigre_geo* geo, const double* angles, int nA, int mode, float* h_proj,
                cudaStream_t st);
