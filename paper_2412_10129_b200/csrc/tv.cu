@@ -6,11 +6,10 @@
 //   T_p = sqrt(.),  a_a(p) = dT_p/dd_a = d_a w_a (1 - d_a^2/delta^2) / T_p
 // the gradient is  g[p] = a_x(p) + a_y(p) + a_z(p) - a_x(p+e_x) - a_y(p+e_y) - a_z(p+e_z).
 //
-// A stencil, HBM-bound by its bytes (read x once, write g once = 8 B per voxel) — and close to the SFU limit in
-// the adaptive case (3 exp + 1 rsqrt per voxel), which is why the a_a are computed ONCE per voxel into shared
-// memory (tile plus a one-voxel forward halo) instead of once per use: a CTA stages the x tile with its halo,
-// forms T and the three a_a for (TX+1)(TY+1)(TZ+1) voxels, then writes TX*TY*TZ gradients.  The same pass
-// returns sum T (the value) and sum g^2 (the minimiser's normalisation) in fp64.
+// A stencil, HBM-bound by its bytes (read x once, write g once = 8 B per voxel) and, in the adaptive case, close
+// to the SFU limit (3 exp + 1 rsqrt per voxel): so T and the a_a are computed ONCE per voxel and handed to the
+// three neighbours that need them (shuffle, shared memory, the next plane) instead of once per use.  The same
+// pass returns sum T (the value) and sum g^2 (the minimiser's normalisation) in fp64.
 #include <algorithm>
 #include <cmath>
 #include "common.cuh"
@@ -19,9 +18,8 @@ namespace tg {
 
 namespace {
 
-constexpr int TV_TX = 32, TV_TY = 8, TV_TZ = 8;
-constexpr int XS_X = TV_TX + 2, XS_Y = TV_TY + 2, XS_Z = TV_TZ + 2;   // x tile with a halo of one on both sides
-constexpr int AS_X = TV_TX + 1, AS_Y = TV_TY + 1, AS_Z = TV_TZ + 1;   // a tile with a forward halo of one
+constexpr int TV_BX = 32, TV_BY = 16;   // threads per CTA; it owns (BX-1) x (BY-1) columns, the last column / row is halo
+constexpr int TV_ZCHUNK = 64;           // planes per CTA along z
 
 __device__ __forceinline__ float ex2_fast(float x) {
     float r;
@@ -34,91 +32,97 @@ __device__ __forceinline__ float rsqrt_fast(float x) {
     return r;
 }
 
-__device__ __forceinline__ double block_sum256(double v, double* sh) {
+__device__ __forceinline__ double block_sum512(double v, double* sh) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
     const int t = threadIdx.y * blockDim.x + threadIdx.x;
     if ((t & 31) == 0) sh[t >> 5] = v;
     __syncthreads();
-    v = t < 8 ? sh[t] : 0.0;
+    v = t < 16 ? sh[t] : 0.0;
     if (t < 32) {
 #pragma unroll
-        for (int o = 4; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        for (int o = 8; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
     }
     return v;
 }
 
 // AW: adaptive weights (finite delta).  nl2 = -log2(e)/delta^2, id2 = 1/delta^2.
+// Streaming along z: a CTA of 32 x 16 threads owns 31 x 15 columns of voxels and walks TV_ZCHUNK planes; a thread
+// forms T and the three a_a of ITS voxel once per plane (x[p - e_z] is the previous plane's value, kept in a
+// register; x[p - e_x], x[p - e_y] are L1 hits), gets a_x(p + e_x) from the next lane (shuffle), a_y(p + e_y) from
+// the next row (shared memory, double buffered: one barrier per plane) and a_z(p + e_z) one plane later, which is
+// when the gradient of the previous plane is written.
 template <bool AW>
-__global__ void __launch_bounds__(TV_TX* TV_TY)
+__global__ void __launch_bounds__(TV_BX* TV_BY)
 tv_gradient_kernel(const float* __restrict__ x, int nx, int ny, int nz, float nl2, float id2, float eps,
                    float* __restrict__ g, double* __restrict__ d_val, double* __restrict__ d_gg) {
-    __shared__ float xs[XS_Z][XS_Y][XS_X];
-    __shared__ float ax[AS_Z][AS_Y][AS_X], ay[AS_Z][AS_Y][AS_X], az[AS_Z][AS_Y][AS_X];
-    __shared__ double red[8];
-    const int x0 = blockIdx.x * TV_TX, y0 = blockIdx.y * TV_TY, z0 = blockIdx.z * TV_TZ;
-    const int tid = threadIdx.y * TV_TX + threadIdx.x;
-    // ---- 1. the x tile, halo of one voxel on every side (zero outside the volume: never used there)
-    for (int i = tid; i < XS_Z * XS_Y * XS_X; i += TV_TX * TV_TY) {
-        const int lx = i % XS_X, ly = (i / XS_X) % XS_Y, lz = i / (XS_X * XS_Y);
-        const int gx = x0 + lx - 1, gy = y0 + ly - 1, gz = z0 + lz - 1;
-        float v = 0.f;
-        if ((unsigned)gx < (unsigned)nx && (unsigned)gy < (unsigned)ny && (unsigned)gz < (unsigned)nz)
-            v = __ldg(x + ((size_t)gz * ny + gy) * nx + gx);
-        xs[lz][ly][lx] = v;
-    }
-    __syncthreads();
-    // ---- 2. T and the three derivatives a_a for the tile and its forward halo
+    __shared__ float say[2][TV_BY][TV_BX];
+    __shared__ double red[16];
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int gx = blockIdx.x * (TV_BX - 1) + tx, gy = blockIdx.y * (TV_BY - 1) + ty;
+    const int zs = blockIdx.z * TV_ZCHUNK, ze = min(zs + TV_ZCHUNK, nz);
     const bool hx = nx > 1, hy = ny > 1, hz = nz > 1;   // an axis of length 1 drops out (P20)
-    double val = 0.0;
-    for (int i = tid; i < AS_Z * AS_Y * AS_X; i += TV_TX * TV_TY) {
-        const int lx = i % AS_X, ly = (i / AS_X) % AS_Y, lz = i / (AS_X * AS_Y);
-        const int gx = x0 + lx, gy = y0 + ly, gz = z0 + lz;
-        float fx = 0.f, fy = 0.f, fz = 0.f;
-        // summation domain: inside the volume, index >= 1 along every axis that exists
-        if (gx < nx && gy < ny && gz < nz && (!hx || gx >= 1) && (!hy || gy >= 1) && (!hz || gz >= 1)) {
-            const float c = xs[lz + 1][ly + 1][lx + 1];
-            const float dx = hx ? c - xs[lz + 1][ly + 1][lx] : 0.f;
-            const float dy = hy ? c - xs[lz + 1][ly][lx + 1] : 0.f;
-            const float dz = hz ? c - xs[lz][ly + 1][lx + 1] : 0.f;
-            const float qx = dx * dx, qy = dy * dy, qz = dz * dz;
-            float wx = 1.f, wy = 1.f, wz = 1.f;
-            if (AW) wx = ex2_fast(qx * nl2), wy = ex2_fast(qy * nl2), wz = ex2_fast(qz * nl2);
-            const float q = fmaf(wx, qx, fmaf(wy, qy, fmaf(wz, qz, eps)));
-            const float it = q > 0.f ? rsqrt_fast(q) : 0.f;
-            if (AW) wx *= fmaf(-qx, id2, 1.f), wy *= fmaf(-qy, id2, 1.f), wz *= fmaf(-qz, id2, 1.f);
-            fx = dx * wx * it, fy = dy * wy * it, fz = dz * wz * it;
-            if (lx < TV_TX && ly < TV_TY && lz < TV_TZ) val += (double)(q * it);   // T_p of the tile's own voxels
-        }
-        ax[lz][ly][lx] = fx, ay[lz][ly][lx] = fy, az[lz][ly][lx] = fz;
-    }
-    __syncthreads();
-    // ---- 3. gradients of the tile's own voxels
-    double gg = 0.0;
-    if (g) {
-        const int lx = threadIdx.x, ly = threadIdx.y;
-        const int gx = x0 + lx, gy = y0 + ly;
-        if (gx < nx && gy < ny) {
-#pragma unroll
-            for (int lz = 0; lz < TV_TZ; ++lz) {
-                const int gz = z0 + lz;
-                if (gz < nz) {
-                    const float v = ax[lz][ly][lx] + ay[lz][ly][lx] + az[lz][ly][lx] - ax[lz][ly][lx + 1] - ay[lz][ly + 1][lx] -
-                                    az[lz + 1][ly][lx];
-                    g[((size_t)gz * ny + gy) * nx + gx] = v;
-                    gg += (double)v * v;
-                }
+    const bool inside = gx < nx && gy < ny;
+    const bool owner = inside && tx < TV_BX - 1 && ty < TV_BY - 1;
+    const bool dom_xy = inside && (!hx || gx >= 1) && (!hy || gy >= 1);
+    const size_t plane = (size_t)nx * ny;
+    size_t idx = ((size_t)zs * ny + gy) * nx + gx;
+    const float* px = x + idx;                 // this thread's voxel in the current plane
+    float* pg = g ? g + idx : nullptr;
+    float xprev = (inside && hz && zs >= 1) ? __ldg(px - plane) : 0.f;
+    float Sprev = 0.f;
+    // partial sums in fp32 over 16 planes at a time, then into fp64 (fp64 arithmetic per voxel would dominate the
+    // instruction count: the fp64 pipe of this part is narrow)
+    float vacc = 0.f, gacc = 0.f;
+    double val = 0.0, gg = 0.0;
+    int buf = 0;
+    const bool ldx = hx && gx >= 1, ldy = hy && gy >= 1;
+    for (int z = zs; z <= ze; ++z) {          // plane ze is visited for its a_z only (nothing beyond the volume)
+        float c = 0.f, fx = 0.f, fy = 0.f, fz = 0.f, T = 0.f;
+        if (inside && z < nz) {
+            c = __ldg(px);
+            if (dom_xy && (!hz || z >= 1)) {   // summation domain: index >= 1 along every axis that exists
+                const float dx = ldx ? c - __ldg(px - 1) : 0.f;
+                const float dy = ldy ? c - __ldg(px - nx) : 0.f;
+                const float dz = hz ? c - xprev : 0.f;
+                const float qx = dx * dx, qy = dy * dy, qz = dz * dz;
+                float wx = 1.f, wy = 1.f, wz = 1.f;
+                if (AW) wx = ex2_fast(qx * nl2), wy = ex2_fast(qy * nl2), wz = ex2_fast(qz * nl2);
+                const float q = fmaf(wx, qx, fmaf(wy, qy, fmaf(wz, qz, eps)));
+                const float it = q > 0.f ? rsqrt_fast(q) : 0.f;
+                if (AW) wx *= fmaf(-qx, id2, 1.f), wy *= fmaf(-qy, id2, 1.f), wz *= fmaf(-qz, id2, 1.f);
+                fx = dx * wx * it, fy = dy * wy * it, fz = dz * wz * it;
+                T = q * it;
             }
         }
+        const float fxn = __shfl_down_sync(0xffffffffu, fx, 1);      // a_x(p + e_x); lane 31 is halo, never an owner
+        say[buf][ty][tx] = fy;
+        __syncthreads();
+        const float fyn = ty + 1 < TV_BY ? say[buf][ty + 1][tx] : 0.f;   // a_y(p + e_y)
+        buf ^= 1;
+        if (owner) {
+            if (z > zs && pg) {                 // the previous plane is complete now: its a_z(p + e_z) is this fz
+                const float v = Sprev - fz;
+                pg[-(ptrdiff_t)plane] = v;
+                gacc = fmaf(v, v, gacc);
+            }
+            if (z < ze) vacc += T;
+        }
+        if (((z - zs) & 15) == 15) val += (double)vacc, gg += (double)gacc, vacc = 0.f, gacc = 0.f;
+        Sprev = fx + fy + fz - fxn - fyn;
+        xprev = c;
+        px += plane;
+        if (pg) pg += plane;
     }
+    val += (double)vacc, gg += (double)gacc;
     if (d_val) {
-        val = block_sum256(val, red);
-        if (tid == 0) atomicAdd(d_val, val);
+        val = block_sum512(val, red);
+        if (tx == 0 && ty == 0) atomicAdd(d_val, val);
         __syncthreads();
     }
     if (d_gg && g) {
-        gg = block_sum256(gg, red);
-        if (tid == 0) atomicAdd(d_gg, gg);
+        gg = block_sum512(gg, red);
+        if (tx == 0 && ty == 0) atomicAdd(d_gg, gg);
     }
 }
 
@@ -146,7 +150,7 @@ __global__ void __launch_bounds__(256) tv_step_kernel(float* __restrict__ x, con
 int launch_tv_gradient(const float* x, int nx, int ny, int nz, float delta, float eps, float* g, double* d_val, double* d_gg,
                        cudaStream_t st) {
     if (nx <= 0 || ny <= 0 || nz <= 0) return TIGRE_ERR_ARG;
-    dim3 block(TV_TX, TV_TY), grid((nx + TV_TX - 1) / TV_TX, (ny + TV_TY - 1) / TV_TY, (nz + TV_TZ - 1) / TV_TZ);
+    dim3 block(TV_BX, TV_BY), grid((nx + TV_BX - 2) / (TV_BX - 1), (ny + TV_BY - 2) / (TV_BY - 1), (nz + TV_ZCHUNK - 1) / TV_ZCHUNK);
     if (grid.y > 65535 || grid.z > 65535) return TIGRE_ERR_ARG;
     ProfScope ps(PK_EW, st);
     const bool aw = delta > 0.f && std::isfinite(delta);
