@@ -51,7 +51,7 @@ _LIB = None
 EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_row_weights", "tigre_col_weights", "tigre_residual",
            "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_fdk", "tigre_fdk_filter",
            "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_ossart", "tigre_plan_destroy",
-           "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_strerror",
+           "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version"]
 
 
@@ -344,6 +344,11 @@ def profile_read():
 
 def version():
     return int(_lib().tigre_version())
+
+
+def set_tv_path(path):
+    """0 = float4 TV gradient kernel when the shape qualifies (default), 1 = scalar kernel only."""
+    _check(_lib().tigre_set_tv_path(int(path)), "tigre_set_tv_path")
 
 
 def set_atb_path(path):
