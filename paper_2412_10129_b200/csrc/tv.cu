@@ -10,8 +10,10 @@
 // to the SFU limit (3 exp + 1 rsqrt per voxel): so T and the a_a are computed ONCE per voxel and handed to the
 // three neighbours that need them (shuffle, shared memory, the next plane) instead of once per use.  The same
 // pass returns sum T (the value) and sum g^2 (the minimiser's normalisation) in fp64.
+#include <cuda.h>
 #include <algorithm>
 #include <cmath>
+#include <mutex>
 #include "common.cuh"
 
 namespace tg {
@@ -19,7 +21,10 @@ namespace tg {
 namespace {
 
 constexpr int TV_BX = 32, TV_BY = 16;   // threads per CTA; it owns (BX-1) x (BY-1) columns, the last column / row is halo
-constexpr int TV_ZCHUNK = 64;           // planes per CTA along z
+#ifndef TVZ
+#define TVZ 64
+#endif
+constexpr int TV_ZCHUNK = TVZ;           // planes per CTA along z
 #define TV_PF 4                         // planes of x loaded ahead of the one being worked on
 
 __device__ __forceinline__ float ex2_fast(float x) {
@@ -42,7 +47,7 @@ __device__ __forceinline__ double block_sum512(double v, double* sh) {
     v = t < (int)(blockDim.x * blockDim.y) >> 5 ? sh[t] : 0.0;
     if (t < 32) {
 #pragma unroll
-        for (int o = 8; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
     }
     return v;
 }
@@ -58,7 +63,7 @@ __global__ void __launch_bounds__(TV_BX* TV_BY)
 tv_gradient_kernel(const float* __restrict__ x, int nx, int ny, int nz, float nl2, float id2, float eps,
                    float* __restrict__ g, double* __restrict__ d_val, double* __restrict__ d_gg) {
     __shared__ float say[2][TV_BY][TV_BX];
-    __shared__ double red[16];
+    __shared__ double red[32];
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int gx = blockIdx.x * (TV_BX - 1) + tx, gy = blockIdx.y * (TV_BY - 1) + ty;
     const int zs = blockIdx.z * TV_ZCHUNK, ze = min(zs + TV_ZCHUNK, nz);
@@ -138,18 +143,26 @@ tv_gradient_kernel(const float* __restrict__ x, int nx, int ny, int nz, float nl
     }
 }
 
-// The same streaming walk with FOUR voxels along x per thread (rows of nx % 4 == 0 floats, 16-byte aligned): the scalar
-// kernel above spends ~100 thread-instructions per voxel on addresses, predicates, the barrier and the exchange, which
-// makes it issue-bound at a quarter of the HBM rate; here one float4 load / store / shared-memory exchange and one
-// shuffle serve four voxels, a_x(p + e_x) of three of them is the thread's own register, and the domain tests are a
-// per-voxel threshold under the rsqrt (thr = 0 on the summation domain, +inf outside: it = 0 there).
-// CTA = 32 x 16 threads = 31 x 4 columns by 15 rows of owned voxels (last lane / row are halo).
-constexpr int V4_BY = 12;
-constexpr int V4_PF = 4;
-#ifndef V4_UNROLL
-#define V4_UNROLL 1
+// The same streaming walk with FOUR voxels along x per thread and the planes of x staged into shared memory by TMA
+// (rows of nx % 4 == 0 floats, 16-byte aligned).  History of this kernel on 512^3 (profiles/r1_tv.md): the scalar kernel
+// above spends ~100 thread-instructions per voxel on addresses, predicates, the barrier and the exchange (issue-bound,
+// 1.7 TB/s); four voxels per thread with register prefetch queues cut that to ~40, but then the walk waits, at every
+// plane's barrier, for the slowest load (3.3 TB/s).  Here one elected thread issues ONE cp.async.bulk.tensor per plane:
+// the tile's rows with a 4-float apron on both sides and the row above ((TM_BY + 1) x 136 floats; TMA's zero fill is
+// the outside of the volume) into a ring of TM_D planes, so TM_D planes per CTA are in flight with no registers held,
+// and x[p - e_x], x[p - e_y] are shared-memory reads of the same tile.  Domain tests are a per-voxel threshold under
+// the rsqrt (thr = 0 on the summation domain, +inf outside: it = 0 there).
+// CTA = TM_BY row warps (a tile of 128 x TM_BY voxels, its last row halo: its a_y feeds the row above) + one edge warp
+// (lane r forms a_x of the voxel just right of the tile in row r, which the last lane of that row subtracts; lane 0 is
+// also the TMA producer).
+#ifndef TMBY
+#define TMBY 15
+#define TMD 6
 #endif
-constexpr int V4_UNR = V4_UNROLL;
+constexpr int TM_BY = TMBY;
+constexpr int TM_D = TMD;
+constexpr int TM_W = 136;                       // floats per staged row: 4 apron + 128 + 4 apron
+constexpr int TM_PLANE = (TM_BY + 1) * TM_W;    // floats per staged plane
 
 template <bool AW>
 __device__ __forceinline__ void tv_voxel(float dx, float dy, float dz, float thr, float nl2, float id2, float eps, float& fx,
@@ -165,81 +178,161 @@ __device__ __forceinline__ void tv_voxel(float dx, float dy, float dz, float thr
     T = q * it;
 }
 
+__device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0;" ::: "memory"); }   // same barrier from two code paths
 __device__ __forceinline__ float4 ld4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+            smem_u32(dst)),
+        "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
+        : "memory");
+}
+
+static_assert((TM_BY + 1) % 4 == 0, "a staged plane must be a multiple of 128 bytes (TMA destination alignment)");
+constexpr size_t TM_SMEM = (size_t)TM_D * TM_PLANE * 4 + 2 * TM_BY * 32 * 16 + 64 * 4 + TM_D * 8;
 
 template <bool AW>
-__global__ void __launch_bounds__(32 * V4_BY, 2)
-tv_gradient_v4_kernel(const float* __restrict__ x, int nx, int ny, int nz, float nl2, float id2, float eps,
-                      float* __restrict__ g, double* __restrict__ d_val, double* __restrict__ d_gg) {
-    __shared__ float4 say[2][V4_BY][32];
-    __shared__ double red[16];
+__global__ void __launch_bounds__(32 * (TM_BY + 1), 2)
+tv_gradient_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict__ x, int nx, int ny, int nz, float nl2,
+                       float id2, float eps, float* __restrict__ g, double* __restrict__ d_val, double* __restrict__ d_gg) {
+    extern __shared__ __align__(128) unsigned char tv_smem[];
+    float* ring = reinterpret_cast<float*>(tv_smem);                 // [TM_D][TM_BY + 1][TM_W]
+    float4* say = reinterpret_cast<float4*>(ring + TM_D * TM_PLANE);  // [2][TM_BY][32]   a_y of the plane, for the row above
+    float* sedge = reinterpret_cast<float*>(say + 2 * TM_BY * 32);    // [2][32]          a_x right of the tile, per row
+    uint64_t* full = reinterpret_cast<uint64_t*>(sedge + 64);         // [TM_D]
+    __shared__ double red[32];
     const int tx = threadIdx.x, ty = threadIdx.y;
-    const int gx = blockIdx.x * (31 * 4) + tx * 4, gy = blockIdx.y * (V4_BY - 1) + ty;
+    const int gx0 = blockIdx.x * 128, gy0 = blockIdx.y * (TM_BY - 1);
     const int zs = blockIdx.z * TV_ZCHUNK, ze = min(zs + TV_ZCHUNK, nz);
-    const bool inside = gx < nx && gy < ny;
-    const bool owner = inside && tx < 31 && ty < V4_BY - 1;
-    const float inf = __int_as_float(0x7f800000);
-    const float thr_a = (inside && gy >= 1 && gx >= 1) ? 0.f : inf;   // voxel 0 of the four
-    const float thr_b = (inside && gy >= 1) ? 0.f : inf;              // voxels 1..3
-    const bool ldy = inside && gy >= 1, ldl = inside && tx == 0 && gx >= 1;
+    const int nplanes = ze - zs + 1;          // planes zs..ze are visited; plane ze for its a_z only (plane nz does not exist)
+    const int nreal = min(ze, nz - 1) - zs + 1;   // planes that are loaded
     const size_t plane = (size_t)nx * ny;
-    const size_t idx = ((size_t)zs * ny + gy) * nx + gx;
-    const float* px = x + idx;
-    float* pg = g ? g + idx : nullptr;
-    const int zlast = min(ze, nz - 1);        // last plane this CTA reads
-    const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
-    float4 xprev = (inside && zs >= 1) ? ld4(px - plane) : zero4;
-    float4 cq[V4_PF];
-#pragma unroll
-    for (int i = 0; i < V4_PF; ++i) cq[i] = (inside && zs + i <= zlast) ? ld4(px + (size_t)i * plane) : zero4;
-    float4 uq = (ldy && zs <= zlast) ? ld4(px - nx) : zero4;          // row above, this plane
-    float lq = (ldl && zs <= zlast) ? __ldg(px - 1) : 0.f;            // left neighbour of lane 0's first voxel
-    float4 Sprev = zero4;
-    float vacc = 0.f, gacc = 0.f;
-    double val = 0.0, gg = 0.0;
-    int buf = 0;
-#pragma unroll(V4_UNR)
-    for (int z = zs; z <= ze; ++z) {
-        const float4 c = cq[0], u = uq;
-        const float lft = lq;
-#pragma unroll
-        for (int i = 0; i + 1 < V4_PF; ++i) cq[i] = cq[i + 1];
-        cq[V4_PF - 1] = (inside && z + V4_PF <= zlast) ? ld4(px + (size_t)V4_PF * plane) : zero4;
-        uq = (ldy && z + 1 <= zlast) ? ld4(px + plane - nx) : zero4;
-        lq = (ldl && z + 1 <= zlast) ? __ldg(px + plane - 1) : 0.f;
-        const bool zin = z >= 1 && z < nz;
-        const float ta = zin ? thr_a : inf, tb = zin ? thr_b : inf;
-        float l = __shfl_up_sync(0xffffffffu, c.w, 1);
-        if (tx == 0) l = lft;
-        float4 fx, fy, fz, T;
-        tv_voxel<AW>(c.x - l, c.x - u.x, c.x - xprev.x, ta, nl2, id2, eps, fx.x, fy.x, fz.x, T.x);
-        tv_voxel<AW>(c.y - c.x, c.y - u.y, c.y - xprev.y, tb, nl2, id2, eps, fx.y, fy.y, fz.y, T.y);
-        tv_voxel<AW>(c.z - c.y, c.z - u.z, c.z - xprev.z, tb, nl2, id2, eps, fx.z, fy.z, fz.z, T.z);
-        tv_voxel<AW>(c.w - c.z, c.w - u.w, c.w - xprev.w, tb, nl2, id2, eps, fx.w, fy.w, fz.w, T.w);
-        const float fxr = __shfl_down_sync(0xffffffffu, fx.x, 1);     // a_x of the next lane's first voxel
-        say[buf][ty][tx] = fy;
-        __syncthreads();
-        const float4 fyn = ty + 1 < V4_BY ? say[buf][ty + 1][tx] : zero4;
-        buf ^= 1;
-        if (owner) {
-            if (z > zs && pg) {
-                float4 v;
-                v.x = Sprev.x - fz.x, v.y = Sprev.y - fz.y, v.z = Sprev.z - fz.z, v.w = Sprev.w - fz.w;
-                *reinterpret_cast<float4*>(pg - plane) = v;
-                gacc = fmaf(v.x, v.x, fmaf(v.y, v.y, fmaf(v.z, v.z, fmaf(v.w, v.w, gacc))));
-            }
-            if (z < ze) vacc += (T.x + T.y) + (T.z + T.w);
-        }
-        if (((z - zs) & 15) == 15) val += (double)vacc, gg += (double)gacc, vacc = 0.f, gacc = 0.f;
-        Sprev.x = fx.x + fy.x + fz.x - fx.y - fyn.x;
-        Sprev.y = fx.y + fy.y + fz.y - fx.z - fyn.y;
-        Sprev.z = fx.z + fy.z + fz.z - fx.w - fyn.z;
-        Sprev.w = fx.w + fy.w + fz.w - fxr - fyn.w;
-        xprev = c;
-        px += plane;
-        if (pg) pg += plane;
+    const float inf = __int_as_float(0x7f800000);
+    const bool producer = ty == TM_BY && tx == 0;
+    if (producer) {
+        for (int s = 0; s < TM_D; ++s) mbar_init(full + s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    val += (double)vacc, gg += (double)gacc;
+    __syncthreads();
+    if (producer) {
+        for (int i = 0; i < TM_D && i < nreal; ++i) {
+            mbar_arrive_expect_tx(full + i, TM_PLANE * 4);
+            tma_load_3d(ring + i * TM_PLANE, &tmap, gx0 - 4, gy0 - 1, zs + i, full + i);
+        }
+    }
+    double val = 0.0, gg = 0.0;
+    int s = 0;
+    uint32_t parity = 0;
+    if (ty == TM_BY) {
+        // ---- edge warp: one voxel per row and plane, the column right of the tile; lane 0 refills the ring
+        const int ex = gx0 + 128, ey = gy0 + tx;
+        const bool on = tx < TM_BY && ex < nx && ey < ny && ey >= 1;
+        const int rr = min(tx, TM_BY - 1);
+        float xprev = zs >= 1 ? __ldg(x + ((size_t)(zs - 1) * ny + min(ey, ny - 1)) * nx + min(ex, nx - 1)) : 0.f;
+        for (int i = 0; i < nplanes; ++i) {
+            const int z = zs + i;
+            float c = 0.f, l = 0.f, u = 0.f;
+            if (i < nreal) {
+                mbar_wait(full + s, parity);
+                const float* T = ring + s * TM_PLANE;
+                c = T[(rr + 1) * TM_W + 132], l = T[(rr + 1) * TM_W + 131], u = T[rr * TM_W + 132];
+            }
+            const float thr = (on && z >= 1 && z < nz) ? 0.f : inf;
+            float fx, fy, fz, Tq;
+            tv_voxel<AW>(c - l, c - u, c - xprev, thr, nl2, id2, eps, fx, fy, fz, Tq);
+            sedge[(i & 1) * 32 + tx] = fx;
+            cta_sync();
+            // every thread has read plane i: its slot takes plane i + TM_D
+            if (producer && i + TM_D < nreal) {
+                mbar_arrive_expect_tx(full + s, TM_PLANE * 4);
+                tma_load_3d(ring + s * TM_PLANE, &tmap, gx0 - 4, gy0 - 1, z + TM_D, full + s);
+            }
+            xprev = c;
+            if (++s == TM_D) s = 0, parity ^= 1;
+        }
+    } else {
+        const int gx = gx0 + 4 * tx, gy = gy0 + ty;
+        const bool inside = gx < nx && gy < ny;
+        const bool owner = inside && ty < TM_BY - 1;
+        const bool hasg = g != nullptr;
+        const float thr_a = (inside && gy >= 1 && gx >= 1) ? 0.f : inf;   // voxel 0 of the four
+        const float thr_b = (inside && gy >= 1) ? 0.f : inf;              // voxels 1..3
+        // threads outside the volume address a clamped column (never stored to; their terms are switched off by thr)
+        const size_t idx = ((size_t)zs * ny + min(gy, ny - 1)) * nx + min(gx, nx - 4);
+        const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        float4 xprev = zs >= 1 ? ld4(x + idx - plane) : zero4;
+        float* pg = g + idx;                  // never dereferenced when g is NULL
+        float4 Sprev = zero4;
+        float vacc = 0.f, gacc = 0.f;
+        const int oc = (ty + 1) * TM_W + 4 + 4 * tx, ou = ty * TM_W + 4 + 4 * tx;
+        for (int i = 0; i < nplanes; ++i) {
+            const int z = zs + i;
+            float4 c = zero4, u = zero4;
+            float l = 0.f;
+            if (i < nreal) {
+                mbar_wait(full + s, parity);
+                const float* T = ring + s * TM_PLANE;
+                c = *reinterpret_cast<const float4*>(T + oc);
+                u = *reinterpret_cast<const float4*>(T + ou);
+                l = __shfl_up_sync(0xffffffffu, c.w, 1);
+                if (tx == 0) l = T[oc - 1];
+            }
+            const bool zin = z >= 1 && z < nz;
+            const float ta = zin ? thr_a : inf, tb = zin ? thr_b : inf;
+            float4 fx, fy, fz, T4;
+            tv_voxel<AW>(c.x - l, c.x - u.x, c.x - xprev.x, ta, nl2, id2, eps, fx.x, fy.x, fz.x, T4.x);
+            tv_voxel<AW>(c.y - c.x, c.y - u.y, c.y - xprev.y, tb, nl2, id2, eps, fx.y, fy.y, fz.y, T4.y);
+            tv_voxel<AW>(c.z - c.y, c.z - u.z, c.z - xprev.z, tb, nl2, id2, eps, fx.z, fy.z, fz.z, T4.z);
+            tv_voxel<AW>(c.w - c.z, c.w - u.w, c.w - xprev.w, tb, nl2, id2, eps, fx.w, fy.w, fz.w, T4.w);
+            float fxr = __shfl_down_sync(0xffffffffu, fx.x, 1);       // a_x of the next lane's first voxel
+            float4* sb = say + (i & 1) * (TM_BY * 32);
+            sb[ty * 32 + tx] = fy;
+            cta_sync();
+            float4 fyn = zero4;
+            if (ty + 1 < TM_BY) fyn = sb[(ty + 1) * 32 + tx];         // a_y(p + e_y)
+            if (tx == 31) fxr = sedge[(i & 1) * 32 + ty];             // the last lane's neighbour is the edge warp's voxel
+            if (owner) {
+                if (i > 0 && hasg) {          // the previous plane is complete now: its a_z(p + e_z) is this fz
+                    float4 v;
+                    v.x = Sprev.x - fz.x, v.y = Sprev.y - fz.y, v.z = Sprev.z - fz.z, v.w = Sprev.w - fz.w;
+                    *reinterpret_cast<float4*>(pg - plane) = v;
+                    gacc = fmaf(v.x, v.x, fmaf(v.y, v.y, fmaf(v.z, v.z, fmaf(v.w, v.w, gacc))));
+                }
+                if (z < ze) vacc += (T4.x + T4.y) + (T4.z + T4.w);
+            }
+            // partial sums in fp32 over 16 planes at a time, then into fp64
+            if ((i & 15) == 15) val += (double)vacc, gg += (double)gacc, vacc = 0.f, gacc = 0.f;
+            Sprev.x = fx.x + fy.x + fz.x - fx.y - fyn.x;
+            Sprev.y = fx.y + fy.y + fz.y - fx.z - fyn.y;
+            Sprev.z = fx.z + fy.z + fz.z - fx.w - fyn.z;
+            Sprev.w = fx.w + fy.w + fz.w - fxr - fyn.w;
+            xprev = c;
+            pg += plane;
+            if (++s == TM_D) s = 0, parity ^= 1;
+        }
+        val += (double)vacc, gg += (double)gacc;
+    }
     if (d_val) {
         val = block_sum512(val, red);
         if (tx == 0 && ty == 0) atomicAdd(d_val, val);
@@ -270,6 +363,25 @@ __global__ void __launch_bounds__(256) tv_step_kernel(float* __restrict__ x, con
 
 }  // namespace
 
+namespace {
+typedef CUresult (*TvEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+TvEncodeFn tv_encode_fn() {
+    static TvEncodeFn fn = nullptr;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (TvEncodeFn)f;
+        (void)cudaGetLastError();
+    });
+    return fn;
+}
+}  // namespace
+
 bool g_tv_scalar = false;   // test hook (tigre_set_tv_path): force the one-voxel-per-thread kernel
 
 // value and/or gradient of AwTV (delta <= 0 or infinite: TV).  g, d_val, d_gg may each be NULL; the two
@@ -281,14 +393,28 @@ int launch_tv_gradient(const float* x, int nx, int ny, int nz, float delta, floa
     if (grid.y > 65535 || grid.z > 65535) return TIGRE_ERR_ARG;
     ProfScope ps(PK_EW, st);
     const bool aw = delta > 0.f && std::isfinite(delta);
+    TvEncodeFn enc = tv_encode_fn();
     const bool vec4 = (nx & 3) == 0 && ny > 1 && nz > 1 && !(reinterpret_cast<uintptr_t>(x) & 15) &&
-                      !(reinterpret_cast<uintptr_t>(g) & 15) && !g_tv_scalar;
+                      !(reinterpret_cast<uintptr_t>(g) & 15) && !g_tv_scalar && enc;
     if (vec4) {
-        dim3 b4(32, V4_BY), g4((nx + 123) / 124, (ny + V4_BY - 2) / (V4_BY - 1), grid.z);
+        CUtensorMap map;
+        const cuuint64_t gdim[3] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz};
+        const cuuint64_t gstr[2] = {(cuuint64_t)nx * sizeof(float), (cuuint64_t)nx * ny * sizeof(float)};
+        const cuuint32_t box[3] = {(cuuint32_t)TM_W, (cuuint32_t)(TM_BY + 1), 1};
+        const cuuint32_t estr[3] = {1, 1, 1};
+        if (enc(&map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(x), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return TIGRE_ERR_ARG;
+        static std::once_flag once;
+        std::call_once(once, [] {
+            cudaFuncSetAttribute(tv_gradient_tma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TM_SMEM);
+            cudaFuncSetAttribute(tv_gradient_tma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TM_SMEM);
+        });
+        dim3 b4(32, TM_BY + 1), g4((nx + 127) / 128, (ny + TM_BY - 2) / (TM_BY - 1), grid.z);
         if (g4.y > 65535) return TIGRE_ERR_ARG;
         const float id2 = aw ? 1.0f / (delta * delta) : 0.f;
-        if (aw) tv_gradient_v4_kernel<true><<<g4, b4, 0, st>>>(x, nx, ny, nz, -1.4426950408889634f * id2, id2, eps, g, d_val, d_gg);
-        else tv_gradient_v4_kernel<false><<<g4, b4, 0, st>>>(x, nx, ny, nz, 0.f, 0.f, eps, g, d_val, d_gg);
+        if (aw) tv_gradient_tma_kernel<true><<<g4, b4, TM_SMEM, st>>>(map, x, nx, ny, nz, -1.4426950408889634f * id2, id2, eps, g, d_val, d_gg);
+        else tv_gradient_tma_kernel<false><<<g4, b4, TM_SMEM, st>>>(map, x, nx, ny, nz, 0.f, 0.f, eps, g, d_val, d_gg);
     } else if (aw) {
         const float id2 = 1.0f / (delta * delta);
         tv_gradient_kernel<true><<<grid, block, 0, st>>>(x, nx, ny, nz, -1.4426950408889634f * id2, id2, eps, g, d_val, d_gg);

@@ -30,7 +30,9 @@ def host(t):
     return t.detach().cpu().numpy().astype(np.float64)
 
 
-SHAPES = [(53, 61, 70), (8, 8, 32), (1, 45, 37), (9, 1, 33), (17, 20, 1), (1, 1, 5), (3, 9, 100)]   # (nz, ny, nx): ragged, 2-D, 1-D
+SHAPES = [(53, 61, 70), (8, 8, 32), (1, 45, 37), (9, 1, 33), (17, 20, 1), (1, 1, 5), (3, 9, 100),   # (nz, ny, nx): ragged, 2-D, 1-D
+          # nx % 4 == 0: the four-voxels-per-thread kernel; several x tiles (edge warp), ragged y tiles, three z chunks
+          (70, 37, 264), (5, 23, 128), (130, 12, 132), (2, 2, 4)]
 
 
 @pytest.mark.parametrize("delta", [None, 0.25, 0.02])
@@ -89,6 +91,22 @@ def test_full_size_properties_512(tg):
     ref = otv.awtv_gradient(blk, 0.2, eps=1e-8)[1:-1, 1:-1, 1:-1]
     got = host(grad[101:139, 201:239, 301:363])
     assert H.rel_l2(got, ref) <= 1e-5
+
+
+def test_vector_and_scalar_kernels_agree_at_full_size(tg):
+    # the two gradient kernels (tigre_set_tv_path) form the same sums; compared on the whole 512^3 volume
+    g = torch.Generator(device="cuda").manual_seed(11)
+    x = torch.rand((512, 512, 512), generator=g, device="cuda") * 0.3
+    try:
+        for delta in (None, 0.2):
+            tg.set_tv_path(0)
+            g4, v4, n4 = tg.awtv_gradient(x, delta, eps=1e-8, return_scalars=True)
+            tg.set_tv_path(1)
+            g1, v1, n1 = tg.awtv_gradient(x, delta, eps=1e-8, return_scalars=True)
+            assert float((g4 - g1).double().norm()) <= 1e-6 * float(g1.double().norm())
+            assert v4 == pytest.approx(v1, rel=1e-6) and n4 == pytest.approx(n1, rel=1e-6)
+    finally:
+        tg.set_tv_path(0)
 
 
 def test_argument_errors(tg):
