@@ -140,6 +140,19 @@ TIGRE_API int tigre_plan_ossart(tigre_plan *plan, const float *b, float *x_inout
                       int nonneg, double *resid_hist, void *cuda_stream);
 TIGRE_API int tigre_plan_destroy(tigre_plan *plan);
 TIGRE_API size_t tigre_plan_bytes(const tigre_plan *plan);
+/* ASD-POCS / OS-ASD-POCS / AwASD-POCS ("Projection Onto Convex Sets ... ASD-POCS [30] ... Adaptive weighed TV
+ * norm [32, 33] ... OS versions", 141-149 Snippet 1, 169; reading P23 spells the loop out).  Per iteration:
+ *   x0 = x;  one OS-SART sweep of the plan's subsets with relaxation beta (nonnegativity on);  beta *= beta_red;
+ *   dd = ||A x - b||_2 (fresh forward projection);  dp = ||x - x0||_2;  first iteration: dtvg = alpha * dp;
+ *   xp = x;  ng steps of x <- x - dtvg g/||g||_2 with g the gradient of TV (delta <= 0 or inf) or AwTV (delta > 0);
+ *   dg = ||x - xp||_2;  if dg > r_max*dp and dd > epsilon: dtvg *= alpha_red;  c = cos(x - xp, xp - x0);
+ *   stop after the iteration if (c < -0.99 and dd <= epsilon) or beta < 0.005.
+ * Single-view subsets in the plan give ASD-POCS, blocks give OS-ASD-POCS.  b, x_inout dev.  hist (host, may be NULL)
+ * [n_iter][5] = dd, dp, dg, the dtvg this iteration used, c;  *n_done (host, may be NULL) = iterations run.
+ * Synchronises the stream twice per iteration (the step-length rule runs on the host). */
+TIGRE_API int tigre_plan_asd_pocs(tigre_plan *plan, const float *b, float *x_inout, int n_iter, float beta, float beta_red,
+                        int ng, float alpha, float alpha_red, float r_max, float epsilon, float delta, float tv_eps,
+                        double *hist, int *n_done, void *cuda_stream);
 /* CGLS (textbook recurrences, DESIGN.md O-F), x0 = 0; x_out dev.  atb_mode may be any of the
  * four tigre_Atb modes (the exact ones must match ax_mode); tigre_ossart / tigre_plan_* take the voxel-driven two. */
 TIGRE_API int tigre_cgls(const float *b, const tigre_geo *geo, const double *angles, int nA, int n_iter,

@@ -50,7 +50,7 @@ class TigreError(RuntimeError):
 _LIB = None
 EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_row_weights", "tigre_col_weights", "tigre_residual",
            "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_fdk", "tigre_fdk_filter",
-           "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_ossart", "tigre_plan_destroy",
+           "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version"]
 
@@ -260,6 +260,19 @@ class OssartPlan:
                                         int(bool(nonneg)), hist.ctypes.data_as(_dp) if want_resid else None,
                                         _stream(b)), "tigre_plan_ossart")
         return hist[:n_iter]
+
+    def asd_pocs(self, b, x, n_iter, beta=1.0, beta_red=0.99, ng=20, alpha=0.002, alpha_red=0.95, r_max=0.95,
+                 epsilon=0.0, delta=None, tv_eps=1e-8):
+        """ASD-POCS family in place on x (single-view subsets: ASD-POCS; blocks: OS-ASD-POCS; delta: AwTV).
+        Returns hist[n_done][5] = dd, dp, dg, dtvg, c."""
+        hist = np.zeros((max(n_iter, 1), 5), dtype=np.float64)
+        done = C.c_int(0)
+        _check(_lib().tigre_plan_asd_pocs(self._h, _f32(b, proj_shape(self.geo, self.nA), "b"),
+                                          _f32(x, vol_shape(self.geo), "x"), int(n_iter), C.c_float(beta),
+                                          C.c_float(beta_red), int(ng), C.c_float(alpha), C.c_float(alpha_red),
+                                          C.c_float(r_max), C.c_float(epsilon), _delta(delta), C.c_float(tv_eps),
+                                          hist.ctypes.data_as(_dp), C.byref(done), _stream(b)), "tigre_plan_asd_pocs")
+        return hist[:done.value]
 
     def close(self):
         if self._h:

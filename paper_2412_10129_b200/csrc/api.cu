@@ -449,6 +449,75 @@ int tigre_ossart(const float* b, const tigre_geo* geo, const double* angles, int
     return rc;
 }
 
+// ---------------------------------------------------------------- ASD-POCS family (reading P23; oracle/pocs.py)
+// Data step = one OS-SART sweep of the plan with relaxation beta; regulariser step = ng normalised steepest-descent
+// steps on (Aw)TV.  The control scalars (dd, dp, dg) decide the next step length on the host: two stream
+// synchronisations per iteration, against hundreds of kernel launches.
+int tigre_plan_asd_pocs(tigre_plan* P, const float* b, float* x, int n_iter, float beta, float beta_red, int ng, float alpha,
+                        float alpha_red, float r_max, float epsilon, float delta, float tv_eps, double* hist, int* n_done,
+                        void* cuda_stream) {
+    if (n_done) *n_done = 0;
+    if (!P || !b || !x || n_iter < 0 || ng < 0 || !(tv_eps >= 0.f)) return TIGRE_ERR_ARG;
+    if (mem_kind(b) != MEM_DEVICE || mem_kind(x) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const Grid& g = P->t.g;
+    const size_t per = (size_t)g.nu * g.nv, nvox = (size_t)g.nx * g.ny * g.nz;
+    TempBuf x0, xp, acc, tvacc;
+    TG_TRY(x0.alloc(sizeof(float) * nvox, st));
+    TG_TRY(xp.alloc(sizeof(float) * nvox, st));
+    TG_TRY(acc.alloc(sizeof(double) * 4, st));
+    TG_TRY(tvacc.alloc(sizeof(double) * std::max(ng, 1), st));
+    double* d = acc.as<double>();
+    float* G = P->grad.as<float>();
+    double dtvg = 0.0;
+    for (int it = 0; it < n_iter; ++it) {
+        TG_CUDA(cudaMemcpyAsync(x0.p, x, sizeof(float) * nvox, cudaMemcpyDeviceToDevice, st));
+        // ---- data step
+        for (int s = 0; s < P->nSubsets; ++s) {
+            const int n = P->off[s + 1] - P->off[s];
+            float* A = P->Axb.as<float>();
+            TG_TRY(launch_ax(x, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st));
+            TG_TRY(launch_residual(b, P->d_idx.as<int32_t>() + P->off[s], A, P->W.as<float>() + per * P->off[s], A, per, n, nullptr, st));
+            TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, G, 0, g.nz, false, 0, g.nv, P->clamp, st,
+                              P->hvox[s].data()));
+            TG_TRY(launch_update(x, G, P->V.as<float>() + nvox * s, beta, 1, nvox, st));
+        }
+        beta *= beta_red;
+        // ---- dd = ||A x - b||, dp = ||x - x0||
+        TG_CUDA(cudaMemsetAsync(d + 3, 0, sizeof(double), st));
+        for (int s = 0; s < P->nSubsets; ++s) {
+            const int n = P->off[s + 1] - P->off[s];
+            float* A = P->Axb.as<float>();
+            TG_TRY(launch_ax(x, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st));
+            TG_TRY(launch_residual(b, P->d_idx.as<int32_t>() + P->off[s], A, nullptr, A, per, n, d + 3, st));
+        }
+        TG_TRY(launch_diff_stats(x, x0.as<float>(), x0.as<float>(), nvox, d, st));
+        double h[4];
+        TG_CUDA(cudaMemcpyAsync(h, d, sizeof h, cudaMemcpyDeviceToHost, st));
+        TG_CUDA(cudaStreamSynchronize(st));
+        const double dd = std::sqrt(h[3]), dp = std::sqrt(h[0]);
+        if (it == 0) dtvg = (double)alpha * dp;
+        TG_CUDA(cudaMemcpyAsync(xp.p, x, sizeof(float) * nvox, cudaMemcpyDeviceToDevice, st));
+        // ---- regulariser step
+        const double used = dtvg;
+        if (ng > 0) TG_CUDA(cudaMemsetAsync(tvacc.p, 0, sizeof(double) * ng, st));
+        for (int k = 0; k < ng; ++k) {
+            TG_TRY(launch_tv_gradient(x, g.nx, g.ny, g.nz, delta, tv_eps, G, nullptr, tvacc.as<double>() + k, st));
+            TG_TRY(launch_tv_step(x, G, (float)dtvg, tvacc.as<double>() + k, nvox, st));
+        }
+        TG_TRY(launch_diff_stats(x, xp.as<float>(), x0.as<float>(), nvox, d, st));
+        TG_CUDA(cudaMemcpyAsync(h, d, 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        TG_CUDA(cudaStreamSynchronize(st));
+        const double dg = std::sqrt(h[0]);
+        if (dg > (double)r_max * dp && dd > (double)epsilon) dtvg *= (double)alpha_red;
+        const double c = (dg > 0.0 && dp > 0.0) ? h[1] / (dg * dp) : 0.0;
+        if (hist) hist[5 * it] = dd, hist[5 * it + 1] = dp, hist[5 * it + 2] = dg, hist[5 * it + 3] = used, hist[5 * it + 4] = c;
+        if (n_done) *n_done = it + 1;
+        if ((c < -0.99 && dd <= (double)epsilon) || beta < 0.005f) break;
+    }
+    return TIGRE_OK;
+}
+
 // ---------------------------------------------------------------- CGLS (textbook recurrences, O-F)
 int tigre_cgls(const float* b, const tigre_geo* geo, const double* angles, int nA, int n_iter, int ax_mode,
                int atb_mode, float* x, double* resid_hist, void* cuda_stream) {

@@ -176,6 +176,30 @@ int launch_dot(const float* a, const float* b, size_t n, double* d_out, cudaStre
     TG_CUDA(cudaGetLastError());
     return TIGRE_OK;
 }
+// ASD-POCS step statistics (reading P23): out[0] += ||a - b||^2, out[1] += <a - b, b - c>, out[2] += ||b - c||^2
+__global__ void __launch_bounds__(256) diff_stats_kernel(const float* __restrict__ a, const float* __restrict__ b,
+                                                         const float* __restrict__ c, size_t n, double* __restrict__ out) {
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const float bb = b[i];
+        const double u = (double)(a[i] - bb), v = (double)(bb - c[i]);
+        s0 += u * u, s1 += u * v, s2 += v * v;
+    }
+    s0 = block_sum(s0);
+    __syncthreads();
+    s1 = block_sum(s1);
+    __syncthreads();
+    s2 = block_sum(s2);
+    if (threadIdx.x == 0) atomicAdd(out, s0), atomicAdd(out + 1, s1), atomicAdd(out + 2, s2);
+}
+int launch_diff_stats(const float* a, const float* b, const float* c, size_t n, double* d_out3, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
+    TG_CUDA(cudaMemsetAsync(d_out3, 0, 3 * sizeof(double), st));
+    if (n == 0) return TIGRE_OK;
+    diff_stats_kernel<<<ew_blocks(n), 256, 0, st>>>(a, b, c, n, d_out3);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
 __global__ void __launch_bounds__(256) axpy_kernel(float* __restrict__ y, const float* __restrict__ x, const double* num, const double* den, float sign, size_t n) {
     const float a = sign * (float)(*num / *den);
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) y[i] = fmaf(a, x[i], y[i]);
