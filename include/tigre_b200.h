@@ -180,6 +180,19 @@ TIGRE_API int tigre_awtv_gradient(const float *x, int nx, int ny, int nz, float 
 TIGRE_API int tigre_minimize_awtv(float *x_inout, int nx, int ny, int nz, float delta, float eps, float alpha, int n_steps,
                         void *cuda_stream);
 
+/* ---- TV proximal operator and FISTA ("For the 2-norm and TV proximal operators, TIGRE provides ... FISTA [42]";
+ * used at 308-314 and 377-393: FISTA(proj, geo, angles, 20, 'hyper', 2e2, ..., 'tviter', 50); readings P24, P25) -----
+ * tigre_tv_prox: u = argmin 1/2||u - f||^2 + lambda TV(u), isotropic TV with forward differences, by n_iter steps of the dual
+ * projection iteration p <- (p + tau grad(div p - f/lambda)) / (1 + tau |grad(div p - f/lambda)|), u = f - lambda div p
+ * (tau <= 1/12 in three dimensions).  f, u dev [nz][ny][nx] (u may alias f); lambda = 0 copies.  Asynchronous.
+ * tigre_fista: x_{k+1} = prox_{tv_lambda}(y_k + (2/L) A^T(b - A y_k)), t_{k+1} = (1 + sqrt(1 + 4 t_k^2))/2,
+ * y_{k+1} = x_{k+1} + ((t_k - 1)/t_{k+1})(x_{k+1} - x_k); y_0 = x_0 = x_inout (the 'init'), t_0 = 1; L = 'hyper'.
+ * resid_hist[k] (host, may be NULL) = ||b - A y_k||_2.  atb_mode: any of the four tigre_Atb modes (exact ones must match
+ * ax_mode).  b dev, x_inout dev. */
+TIGRE_API int tigre_tv_prox(const float *f, int nx, int ny, int nz, float lambda, int n_iter, float tau, float *u, void *cuda_stream);
+TIGRE_API int tigre_fista(const float *b, const tigre_geo *geo, const double *angles, int nA, int n_iter, float L, float tv_lambda,
+                int tv_iter, float tau, int ax_mode, int atb_mode, float *x_inout, double *resid_hist, void *cuda_stream);
+
 /* ---- measurement helpers -------------------------------------------------------------------
  * Exact count of ray-samples of one tigre_Ax call without marching the data (BASELINE metric:
  * Siddon = non-zero voxel segments; interpolated = samples K inside the grown box).

@@ -50,7 +50,7 @@ class TigreError(RuntimeError):
 _LIB = None
 EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_row_weights", "tigre_col_weights", "tigre_residual",
            "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_fdk", "tigre_fdk_filter",
-           "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_destroy",
+           "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version"]
 
@@ -404,6 +404,31 @@ def awtv_gradient(x, delta=None, eps=1e-8, return_scalars=False):
                                       C.byref(v) if return_scalars else None, C.byref(n2) if return_scalars else None,
                                       _stream(x)), "tigre_awtv_gradient")
     return (g, v.value, n2.value) if return_scalars else g
+
+
+def tv_prox(f, lam, n_iter, tau=1.0 / 12.0, out=None):
+    """TV proximal operator (ROF denoising by the dual projection iteration); out may be f itself."""
+    nx, ny, nz = _dims(f)
+    u = _new(tuple(f.shape), like=f) if out is None else out
+    _check(_lib().tigre_tv_prox(_f32(f), nx, ny, nz, C.c_float(lam), int(n_iter), C.c_float(tau), _f32(u), _stream(f)),
+           "tigre_tv_prox")
+    return u
+
+
+def fista(b, geo, angles, n_iter, L, tv_lambda, tv_iter, ax_mode="siddon", atb_mode="matched", x0=None, tau=1.0 / 12.0):
+    """FISTA with the TV prox; returns (x, resid)."""
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    x = _new(vol_shape(geo), like=b)
+    if x0 is None:
+        x.zero_()
+    else:
+        x.copy_(x0)
+    hist = np.zeros(max(n_iter, 1), dtype=np.float64)
+    _check(_lib().tigre_fista(_f32(b, proj_shape(geo, nA), "b"), G.ref, a.ctypes.data_as(_dp), nA, int(n_iter), C.c_float(L),
+                              C.c_float(tv_lambda), int(tv_iter), C.c_float(tau), _AX_MODES[ax_mode], _ATB_MODES[atb_mode],
+                              _f32(x), hist.ctypes.data_as(_dp), _stream(b)), "tigre_fista")
+    return x, hist[:n_iter]
 
 
 def minimize_awtv(x, n_steps, alpha, delta=None, eps=1e-8):

@@ -142,6 +142,10 @@ int launch_count_reduce(const uint32_t* c, size_t n, unsigned long long* d_total
 // normalised descent step x -= alpha g / sqrt(*d_gg)
 int launch_tv_gradient(const float* x, int nx, int ny, int nz, float delta, float eps, float* g, double* d_val, double* d_gg,
                        cudaStream_t st);
+int launch_prox_div(const float* px, const float* py, const float* pz, const float* f, float lam, bool final, float* out, int nx,
+                    int ny, int nz, cudaStream_t st);
+int launch_prox_update(float* px, float* py, float* pz, const float* d, float tau, int nx, int ny, int nz, cudaStream_t st);
+int launch_momentum(float* y, float* x, const float* xn, float c, size_t n, cudaStream_t st);
 int launch_tv_step(float* x, const float* g, float alpha, const double* d_gg, size_t n, cudaStream_t st);
 
 // chunked (pinned host) path
