@@ -239,14 +239,25 @@ def run_tv(args, tg, geo, rec, K, W, rank, world, local_rank):
     gradient kernel reads x and writes g (8 B), the step kernel reads x and g and writes x (12 B)."""
     import torch
     n_tv, delta = args.tv_steps, (args.tv_delta if args.tv_delta > 0 else None)
+    prox = args.tv_op == "prox"
+    bpv = 48 if prox else 20                  # algorithmic bytes per voxel and inner step (DESIGN.md section 6)
     shape = tuple(geo.vol_shape)
     nvox = int(np.prod(shape))
     gen = torch.Generator(device="cuda").manual_seed(rec["seed"])
     x0 = torch.from_numpy(phantom_for(rec, geo)).cuda() if nvox <= 512 ** 3 else torch.zeros(shape, device="cuda")
     x0 += 1e-3 * torch.rand(shape, generator=gen, device="cuda")          # noisy phantom: what the minimiser is for
     x = x0.clone()
+    if prox:
+        class _P:                              # same call shape as the minimiser: in place on x
+            @staticmethod
+            def minimize_awtv(x, n, alpha, delta):
+                return tg.tv_prox(x, 0.05, n, out=x)
+            awtv_gradient = staticmethod(lambda x, delta: tg.tv_prox(x, 0.05, 1))
+        run = _P
+    else:
+        run = tg
     for _ in range(W):
-        tg.minimize_awtv(x, n_tv, 1e-3, delta)
+        run.minimize_awtv(x, n_tv, 1e-3, delta)
     sampler = ClockSampler(local_rank)
     sampler.start()
     tg.profile(True)
@@ -254,7 +265,7 @@ def run_tv(args, tg, geo, rec, K, W, rank, world, local_rank):
     torch.cuda.synchronize()
     e0.record()
     for _ in range(K):
-        tg.minimize_awtv(x, n_tv, 1e-3, delta)
+        run.minimize_awtv(x, n_tv, 1e-3, delta)
     e1.record()
     torch.cuda.synchronize()
     ms = max_over_ranks(e0.elapsed_time(e1), "cuda")
@@ -262,11 +273,11 @@ def run_tv(args, tg, geo, rec, K, W, rank, world, local_rank):
     tg.profile(False)
     # the gradient kernel alone (value and ||g||^2 from the same pass), K * n_tv launches
     g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    tg.awtv_gradient(x, delta)
+    run.awtv_gradient(x, delta)
     torch.cuda.synchronize()
     g0.record()
     for _ in range(K * n_tv):
-        tg.awtv_gradient(x, delta)
+        run.awtv_gradient(x, delta)
     g1.record()
     torch.cuda.synchronize()
     gms = g0.elapsed_time(g1) / (K * n_tv)
@@ -278,7 +289,7 @@ def run_tv(args, tg, geo, rec, K, W, rank, world, local_rank):
     t0.record()
     for _ in range(K):
         x.copy_(x_h, non_blocking=True)
-        tg.minimize_awtv(x, n_tv, 1e-3, delta)
+        run.minimize_awtv(x, n_tv, 1e-3, delta)
         x_h.copy_(x, non_blocking=True)
     t1.record()
     torch.cuda.synchronize()
@@ -296,19 +307,20 @@ def run_tv(args, tg, geo, rec, K, W, rank, world, local_rank):
     ms_step = ms / K
     unit = "Gvoxel-steps/s"
     value = whole_job_value(nvox * n_tv, ms_step, world)
-    ach = nvox * n_tv * 20 / (ms_step * 1e-3) / 1e9
-    line = {"metric": "TV minimiser voxel-steps/s", "value": value, "unit": unit, "n_gpus": world, "steps": K, "warmup": W,
+    ach = nvox * n_tv * bpv / (ms_step * 1e-3) / 1e9
+    line = {"metric": "TV proximal operator voxel-iterations/s" if prox else "TV minimiser voxel-steps/s", "value": value, "unit": unit, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
             "config": {"workload": f"{rec['name']}-sized volume {shape[2]}x{shape[1]}x{shape[0]} fp32, {n_tv} descent steps of "
-                                   f"{'TV' if delta is None else 'AwTV delta=%g' % delta} per step", "seed": rec["seed"],
+                                   f"{'the TV prox (dual projection iterations)' if prox else 'TV' if delta is None else 'AwTV delta=%g' % delta} per step", "seed": rec["seed"],
                        "l2": "volume + gradient larger than L2" if nvox * 8 > 126e6 else "fits L2", "parallelism": "single GPU"},
             "clocks": sampler.summary(), "gpu_launches": int(sum(prof["launches"].values())),
-            "roofline": {"kernel": "tv_gradient_kernel + tv_step_kernel", "bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s",
-                         "frac": ach / hbm, "traffic": None, "bytes_per_voxel_step": 20,
+            "roofline": {"kernel": "prox_div_kernel + prox_update_kernel" if prox else "tv_gradient_kernel + tv_step_kernel",
+                         "bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s",
+                         "frac": ach / hbm, "traffic": None, "bytes_per_voxel_step": bpv,
                          "peak_source": "MEASURED_PEAKS.json hbm_gbs (copy bandwidth)",
-                         "gradient_kernel": {"ms_per_launch": gms, "achieved": nvox * 8 / (gms * 1e-3) / 1e9, "bytes_per_voxel": 8,
-                                             "frac": nvox * 8 / (gms * 1e-3) / 1e9 / hbm}},
+                         **({} if prox else {"gradient_kernel": {"ms_per_launch": gms, "achieved": nvox * 8 / (gms * 1e-3) / 1e9,
+                                                                  "bytes_per_voxel": 8, "frac": nvox * 8 / (gms * 1e-3) / 1e9 / hbm}})},
             "e2e": {"value": whole_job_value(nvox * n_tv, ems, world), "unit": unit, "ms_per_step": ems,
                     "h2d_bytes_per_step": nvox * 4, "d2h_bytes_per_step": nvox * 4}}
     if world == 1 and not args.no_cpu_baseline:
@@ -316,7 +328,11 @@ def run_tv(args, tg, geo, rec, K, W, rank, world, local_rank):
         m = 160
         xs = x0[:m, :m, :m].double().cpu().numpy()
         t = time.perf_counter()
-        otv.minimize_awtv(xs, 2, 1e-3, np.inf if delta is None else delta)
+        if prox:
+            from oracle import prox as oprox
+            oprox.tv_prox(xs, 0.05, 2)
+        else:
+            otv.minimize_awtv(xs, 2, 1e-3, np.inf if delta is None else delta)
         dt = time.perf_counter() - t
         line["cpu_baseline"] = {"value": m ** 3 * 2 / dt / 1e9, "unit": unit, "cores": 1, "kind": "oracle",
                                 "sample": f"2 descent steps on the {m}^3 corner of the same volume ({dt:.1f} s, numpy fp64)"}
@@ -334,6 +350,8 @@ def main():
     ap.add_argument("--atb-kernel", default="tma", choices=["tma", "gather"], help="A/B switch of the A^T b kernel")
     ap.add_argument("--tv-steps", type=int, default=20, help="tv mode: descent steps per timed step")
     ap.add_argument("--tv-delta", type=float, default=0.0, help="tv mode: AwTV delta (0 = plain TV)")
+    ap.add_argument("--tv-op", default="minimise", choices=["minimise", "prox"],
+                    help="tv mode: the gradient-descent minimiser (tigre_minimize_awtv) or the TV proximal operator of FISTA (tigre_tv_prox)")
     ap.add_argument("--mode", default="plan", choices=["plan", "chunked", "tv"],
                     help="plan: OS-SART iteration in HBM (default); chunked: Ax + A^T b with all arrays in pinned host memory (S8)")
     ap.add_argument("--budget-gb", type=float, default=0.0, help="chunked mode: device bytes the chunked path may use (0 = 3/4 of free)")
