@@ -73,6 +73,9 @@ enum { TIGRE_AX_SIDDON = 0, TIGRE_AX_INTERP = 1 };
 enum { TIGRE_ATB_MATCHED = 0, TIGRE_ATB_FDK = 1,
        /* exact transposes of tigre_Ax (ray-driven scatter of the very same weights) */
        TIGRE_ATB_EXACT_SIDDON = 2, TIGRE_ATB_EXACT_INTERP = 3 };
+enum { TIGRE_FILTER_RAM_LAK = 0, TIGRE_FILTER_SHEPP_LOGAN = 1, TIGRE_FILTER_COSINE = 2, TIGRE_FILTER_HAMMING = 3,
+       TIGRE_FILTER_HANN = 4 };
+enum { TIGRE_FDK_FULL = 0, TIGRE_FDK_PARKER = 1, TIGRE_FDK_WANG = 2 };
 enum { TIGRE_OP_AX = 0, TIGRE_OP_ATB = 1, TIGRE_OP_OSSART = 2, TIGRE_OP_CGLS = 3, TIGRE_OP_FDK = 4 };
 
 /* ---- the projector pair ------------------------------------------------------------------
@@ -164,6 +167,21 @@ TIGRE_API int tigre_fdk(const float *b, const tigre_geo *geo, const double *angl
 /* the FDK pre-filter alone: q = tau * ((b * cos) conv h), per detector row.  dev -> dev */
 TIGRE_API int tigre_fdk_filter(const float *b, const tigre_geo *geo, const double *angles, int nA, float *q,
                      void *cuda_stream);
+
+/* FDK variants ("various filter types and geometric correction methods, such as Wang [25]
+ * and Parker [26] weights for detector displacement and angular range corrections", 281, 359; readings P26-P28).
+ * filter: the Ram-Lak taps windowed in frequency on L = 2^ceil(log2(2 nDetector_u)) samples, omega in [0, pi]:
+ *   RAM_LAK 1, SHEPP_LOGAN sin(omega/2)/(omega/2), COSINE cos(omega/2), HAMMING 0.54 + 0.46 cos(omega), HANN 0.5 + 0.5 cos(omega),
+ * applied as a linear convolution of the zero-padded row (equal to the FFT formulation).
+ * weighting: FULL = full circle (tigre_fdk); PARKER = short scan over |theta_last - theta_first| = pi + 2 eps < 2 pi with
+ * monotone angles, sum scaled by the angular step; WANG = detector displaced along u over a full circle, projections
+ * multiplied by 2 w(u).  TIGRE_ERR_ARG if the scan does not fit the weighting.
+ * tigre_fdk_weights: the weight table alone, w host [nA][nDetector_u] fp64 (WANG without the factor 2); no device needed. */
+TIGRE_API int tigre_fdk_ex(const float *b, const tigre_geo *geo, const double *angles, int nA, int filter, int weighting,
+                 float *x_out, void *cuda_stream);
+TIGRE_API int tigre_fdk_filter_ex(const float *b, const tigre_geo *geo, const double *angles, int nA, int filter, int weighting,
+                        float *q, void *cuda_stream);
+TIGRE_API int tigre_fdk_weights(const tigre_geo *geo, const double *angles, int nA, int weighting, double *w);
 
 /* ---- total variation (section 2.2.3 eqs. 7-8; P20-P22) ----------
  * AwTV(x) = sum_p sqrt(w_x dx^2 + w_y dy^2 + w_z dz^2 + eps), backward differences d_a = x[p] - x[p - e_a], weights

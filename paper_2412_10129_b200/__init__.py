@@ -49,7 +49,7 @@ class TigreError(RuntimeError):
 
 _LIB = None
 EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_row_weights", "tigre_col_weights", "tigre_residual",
-           "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_fdk", "tigre_fdk_filter",
+           "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_fdk", "tigre_fdk_filter", "tigre_fdk_ex", "tigre_fdk_filter_ex", "tigre_fdk_weights",
            "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version"]
@@ -300,6 +300,39 @@ def cgls(b, geo, angles, n_iter, ax_mode="siddon", atb_mode="matched"):
                              _AX_MODES[ax_mode], _ATB_MODES[atb_mode], _f32(x), hist.ctypes.data_as(_dp), _stream(b)),
            "tigre_cgls")
     return x, hist[:n_iter]
+
+
+_FILTERS = {"ram_lak": 0, "shepp_logan": 1, "cosine": 2, "hamming": 3, "hann": 4}
+_WEIGHTINGS = {None: 0, "full": 0, "parker": 1, "wang": 2}
+
+
+def fdk_ex(b, geo, angles, filt="ram_lak", weighting=None):
+    """FDK with a windowed ramp filter and Parker (short scan) or Wang (displaced detector) weights."""
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    x = _new(vol_shape(geo), like=b)
+    _check(_lib().tigre_fdk_ex(_f32(b, proj_shape(geo, nA), "b"), G.ref, a.ctypes.data_as(_dp), nA, _FILTERS[filt],
+                               _WEIGHTINGS[weighting], _f32(x), _stream(b)), "tigre_fdk_ex")
+    return x
+
+
+def fdk_filter_ex(b, geo, angles, filt="ram_lak", weighting=None):
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    q = _new(proj_shape(geo, nA), like=b)
+    _check(_lib().tigre_fdk_filter_ex(_f32(b, proj_shape(geo, nA), "b"), G.ref, a.ctypes.data_as(_dp), nA, _FILTERS[filt],
+                                      _WEIGHTINGS[weighting], _f32(q), _stream(b)), "tigre_fdk_filter_ex")
+    return q
+
+
+def fdk_weights(geo, angles, weighting):
+    """Parker / Wang weight table [nA][nu] (host, fp64; Wang without the factor 2)."""
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    w = np.zeros((nA, geo.nDetector[0]), dtype=np.float64)
+    _check(_lib().tigre_fdk_weights(G.ref, a.ctypes.data_as(_dp), nA, _WEIGHTINGS[weighting], w.ctypes.data_as(_dp)),
+           "tigre_fdk_weights")
+    return w
 
 
 def fdk(b, geo, angles):

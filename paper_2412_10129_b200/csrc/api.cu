@@ -602,6 +602,65 @@ int tigre_fdk(const float* b, const tigre_geo* geo, const double* angles, int nA
     return launch_scale(x, (float)(M_PI / (double)nA), (size_t)g.nx * g.ny * g.nz, st);
 }
 
+// ---------------------------------------------------------------- FDK variants (fdk.cu; P26-P28)
+static int fdk_filter_ex_impl(const float* b, Tables& t, int nA, int filter, int weighting, float* q, cudaStream_t st) {
+    if (filter < TIGRE_FILTER_RAM_LAK || filter > TIGRE_FILTER_HANN) return TIGRE_ERR_ARG;
+    if (weighting < TIGRE_FDK_FULL || weighting > TIGRE_FDK_WANG) return TIGRE_ERR_ARG;
+    if (filter == TIGRE_FILTER_RAM_LAK && weighting == TIGRE_FDK_FULL) return fdk_filter_impl(b, t, nA, q, st);
+    const int nu = t.g.nu;
+    std::vector<double> dd(2 * (size_t)nA), taps, w;
+    for (int a = 0; a < nA; ++a) dd[a] = t.views[a].DSD, dd[nA + a] = t.views[a].DSO;
+    fdk_filter_taps(nu, filter, taps);
+    std::vector<float> ft(taps.begin(), taps.end()), fw;
+    TempBuf tb, tt, tw;
+    TG_TRY(upload(tb, dd.data(), sizeof(double) * dd.size(), st));
+    TG_TRY(upload(tt, ft.data(), sizeof(float) * ft.size(), st));
+    if (weighting != TIGRE_FDK_FULL) {
+        TG_TRY(fdk_weights(t.g, t.views, weighting, w));
+        fw.resize(w.size());
+        const double k = weighting == TIGRE_FDK_WANG ? 2.0 : 1.0;
+        for (size_t i = 0; i < w.size(); ++i) fw[i] = (float)(k * w[i]);
+        TG_TRY(upload(tw, fw.data(), sizeof(float) * fw.size(), st));
+    }
+    return launch_fdk_filter_taps(b, t.g, tb.as<double>(), tb.as<double>() + nA, nA, tt.as<float>(),
+                                  weighting != TIGRE_FDK_FULL ? tw.as<float>() : nullptr, q, st);
+}
+int tigre_fdk_filter_ex(const float* b, const tigre_geo* geo, const double* angles, int nA, int filter, int weighting, float* q,
+                        void* cuda_stream) {
+    if (!b || !q) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    if (mem_kind(b) != MEM_DEVICE || mem_kind(q) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    return fdk_filter_ex_impl(b, t, nA, filter, weighting, q, (cudaStream_t)cuda_stream);
+}
+int tigre_fdk_ex(const float* b, const tigre_geo* geo, const double* angles, int nA, int filter, int weighting, float* x,
+                 void* cuda_stream) {
+    if (!b || !x) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    if (mem_kind(b) != MEM_DEVICE || mem_kind(x) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const Grid& g = t.g;
+    TempBuf q;
+    TG_TRY(q.alloc(sizeof(float) * (size_t)nA * g.nu * g.nv, st));
+    TG_TRY(fdk_filter_ex_impl(b, t, nA, filter, weighting, q.as<float>(), st));
+    TG_TRY(device_atb(q.as<float>(), t, nullptr, nA, TIGRE_ATB_FDK, false, x, st));
+    double scale = M_PI / (double)nA;
+    if (weighting == TIGRE_FDK_PARKER) scale = std::fabs(t.views[nA - 1].ang[0] - t.views[0].ang[0]) / (double)(nA - 1);
+    return launch_scale(x, (float)scale, (size_t)g.nx * g.ny * g.nz, st);
+}
+int tigre_fdk_weights(const tigre_geo* geo, const double* angles, int nA, int weighting, double* w) {
+    if (!w) return TIGRE_ERR_ARG;
+    TG_TRY(validate_geo(geo, angles, nA));      // host arithmetic only: no device needed
+    Grid g = make_grid(geo);
+    std::vector<ViewH> views;
+    resolve_views(geo, angles, nA, views);
+    std::vector<double> v;
+    TG_TRY(fdk_weights(g, views, weighting, v));
+    std::copy(v.begin(), v.end(), w);
+    return TIGRE_OK;
+}
+
 // ---------------------------------------------------------------- TV / AwTV (tv.cu)
 int tigre_awtv_gradient(const float* x, int nx, int ny, int nz, float delta, float eps, float* g, double* value,
                         double* grad_norm2, void* cuda_stream) {

@@ -1,0 +1,148 @@
+// fdk.cu — FDK variants ("various filter types and geometric correction methods,
+// such as Wang [25] and Parker [26] weights", 281, 359; readings P26-P28).
+//
+// Filters: the Ram-Lak taps (P12) windowed in frequency on L = 2^ceil(log2(2 nu)) samples.  The product of the taps'
+// spectrum with the window is transformed back ON THE HOST (fp64, direct cosine sums: the spectrum is real and even) into
+// nu spatial taps for tau = 1; the device then applies them as a direct linear convolution of the zero-padded row, which
+// equals the FFT formulation exactly (L >= 2 nu: no wrap) and keeps the kernel free of an FFT dependency.
+// Weights: Parker (short scan) and Wang (displaced detector) are per-view, per-column factors built on the host in
+// fp64 and multiplied into the cosine-weighted row before the convolution.
+#include <cmath>
+#include <vector>
+#include "common.cuh"
+
+namespace tg {
+
+namespace {
+
+// q[iu] = (1/tau) * sum_n row[iu - n] * taps[|n|],  row = b * cosine weight * colw
+__global__ void __launch_bounds__(256)
+fdk_filter_taps_kernel(const float* __restrict__ b, int nu, int nv, float du, float dv, const double* __restrict__ dsd_a,
+                       const double* __restrict__ dso_a, const float* __restrict__ taps, const float* __restrict__ colw,
+                       float* __restrict__ q) {
+    extern __shared__ float sm[];
+    float* row = sm;            // [nu]
+    float* tap = sm + nu;       // [nu]
+    const int iv = blockIdx.x, ia = blockIdx.y;
+    const float DSD = (float)dsd_a[ia], DSO = (float)dso_a[ia];
+    const float itau = DSD / (du * DSO);
+    const float v = ((float)iv + 0.5f) * dv - 0.5f * (float)nv * dv;
+    const size_t base = ((size_t)ia * nv + iv) * nu;
+    for (int iu = threadIdx.x; iu < nu; iu += blockDim.x) {
+        const float u = ((float)iu + 0.5f) * du - 0.5f * (float)nu * du;
+        float r = __ldg(b + base + iu) * DSD * rsqrtf(DSD * DSD + u * u + v * v);
+        if (colw) r *= __ldg(colw + (size_t)ia * nu + iu);
+        row[iu] = r;
+        tap[iu] = __ldg(taps + iu);
+    }
+    __syncthreads();
+    for (int iu = threadIdx.x; iu < nu; iu += blockDim.x) {
+        float s0 = row[iu] * tap[0], s1 = 0.f;
+        // left side: row[iu - n], n = 1..iu;  right side: row[iu + n], n = 1..nu-1-iu  (two chains for ILP)
+        for (int n = 1; n <= iu; ++n) s0 = fmaf(row[iu - n], tap[n], s0);
+        for (int n = 1; n < nu - iu; ++n) s1 = fmaf(row[iu + n], tap[n], s1);
+        q[base + iu] = (s0 + s1) * itau;
+    }
+}
+
+double window_at(int filter, double om) {
+    switch (filter) {
+        case TIGRE_FILTER_SHEPP_LOGAN: return om > 0.0 ? std::sin(0.5 * om) / (0.5 * om) : 1.0;
+        case TIGRE_FILTER_COSINE: return std::cos(0.5 * om);
+        case TIGRE_FILTER_HAMMING: return 0.54 + 0.46 * std::cos(om);
+        case TIGRE_FILTER_HANN: return 0.5 + 0.5 * std::cos(om);
+        default: return 1.0;
+    }
+}
+
+}  // namespace
+
+// taps for tau = 1 (the kernel scales by 1/tau: h ~ 1/tau^2, times the tau of the quadrature)
+void fdk_filter_taps(int nu, int filter, std::vector<double>& g) {
+    g.assign(nu, 0.0);
+    if (filter == TIGRE_FILTER_RAM_LAK) {
+        g[0] = 0.25;
+        for (int n = 1; n < nu; n += 2) g[n] = -1.0 / (M_PI * M_PI * (double)n * (double)n);
+        return;
+    }
+    int L = 1;
+    while (L < 2 * nu) L <<= 1;
+    const int half = L / 2;
+    std::vector<double> ct(L);
+    for (int j = 0; j < L; ++j) ct[j] = std::cos(2.0 * M_PI * (double)j / (double)L);
+    std::vector<double> HW(half + 1);
+    for (int k = 0; k <= half; ++k) {
+        double s = 0.0;
+        for (int n = 1; n < half; n += 2) s += -1.0 / (M_PI * M_PI * (double)n * (double)n) * ct[(size_t)((long long)k * n % L)];
+        HW[k] = (0.25 + 2.0 * s) * window_at(filter, 2.0 * M_PI * (double)k / (double)L);
+    }
+    for (int m = 0; m < nu; ++m) {
+        double s = 0.0;
+        for (int k = 1; k < half; ++k) s += HW[k] * ct[(size_t)((long long)k * m % L)];
+        g[m] = (HW[0] + 2.0 * s + HW[half] * ((m & 1) ? -1.0 : 1.0)) / (double)L;
+    }
+}
+
+// Parker (P27) / Wang (P28, without the factor 2) weights, [nA][nu]; returns TIGRE_ERR_ARG for a scan they do not apply to
+int fdk_weights(const Grid& g, const std::vector<ViewH>& views, int weighting, std::vector<double>& w) {
+    const int nA = (int)views.size(), nu = g.nu;
+    w.assign((size_t)nA * nu, 1.0);
+    if (weighting == TIGRE_FDK_FULL) return TIGRE_OK;
+    if (weighting == TIGRE_FDK_PARKER) {
+        if (nA < 2) return TIGRE_ERR_ARG;
+        const double t0 = views[0].ang[0], t1 = views[nA - 1].ang[0];
+        const double dir = t1 > t0 ? 1.0 : -1.0;
+        for (int a = 1; a < nA; ++a)
+            if (!((views[a].ang[0] - views[a - 1].ang[0]) * dir > 0.0)) return TIGRE_ERR_ARG;   // monotone angles only
+        const double Theta = std::fabs(t1 - t0), eps = 0.5 * (Theta - M_PI);
+        if (!(Theta < 2.0 * M_PI)) return TIGRE_ERR_ARG;
+        for (int a = 0; a < nA; ++a) {
+            const double beta = std::fabs(views[a].ang[0] - t0);
+            for (int iu = 0; iu < nu; ++iu) {
+                const double u = (iu + 0.5) * g.du - 0.5 * nu * g.du + views[a].offD[0];
+                const double gamma = -dir * std::atan(u / views[a].DSD);
+                double v = 1.0;
+                if (beta < 2.0 * eps - 2.0 * gamma) {
+                    const double s = std::sin(0.25 * M_PI * beta / (eps - gamma));
+                    v = s * s;
+                } else if (beta > M_PI - 2.0 * gamma) {
+                    const double s = std::sin(0.25 * M_PI * (M_PI + 2.0 * eps - beta) / (eps + gamma));
+                    v = s * s;
+                }
+                w[(size_t)a * nu + iu] = v;
+            }
+        }
+        return TIGRE_OK;
+    }
+    if (weighting == TIGRE_FDK_WANG) {
+        for (int a = 0; a < nA; ++a) {
+            const double off = views[a].offD[0], s = off >= 0.0 ? 1.0 : -1.0;
+            const double u_ov = 0.5 * nu * g.du - std::fabs(off);
+            if (!(u_ov > 0.0)) return TIGRE_ERR_ARG;
+            const double den = std::atan(u_ov / views[a].DSD);
+            for (int iu = 0; iu < nu; ++iu) {
+                const double t = ((iu + 0.5) * g.du - 0.5 * nu * g.du + off) * s;
+                double v = 0.5 * (std::sin(0.5 * M_PI * std::atan(t / views[a].DSD) / den) + 1.0);
+                if (t > u_ov) v = 1.0;
+                if (t < -u_ov) v = 0.0;
+                w[(size_t)a * nu + iu] = v;
+            }
+        }
+        return TIGRE_OK;
+    }
+    return TIGRE_ERR_ARG;
+}
+
+int launch_fdk_filter_taps(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, int nViews, const float* d_taps,
+                           const float* d_colw, float* q, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
+    const size_t smem = 2 * (size_t)g.nu * sizeof(float);
+    if (smem > 200 * 1024) return TIGRE_ERR_ARG;
+    if (smem > 48 * 1024) TG_CUDA(cudaFuncSetAttribute(fdk_filter_taps_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    dim3 grid(g.nv, nViews);
+    fdk_filter_taps_kernel<<<grid, 256, smem, st>>>(b, g.nu, g.nv, (float)g.du, (float)g.dv, d_dsd, d_dso, d_taps, d_colw, q);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+
+}  // namespace tg
