@@ -105,6 +105,22 @@ TIGRE_API int tigre_Ax(const float *vol, const tigre_geo *geo, const double *ang
 TIGRE_API int tigre_Atb(const float *proj, const tigre_geo *geo, const double *angles, int nA, int mode,
               float *vol, void *cuda_stream);
 
+/* ---- z-slab entry points: the building blocks of multi-GPU sharding (PAPER.md:201-203
+ * "split ... by image slabs").  The volume is cut into slabs of z-slices [z0, z0 + nzs); geo describes the FULL volume.
+ * tigre_Ax_slab: proj (dev, full size [nA][nv][nu], overwritten) = the slab's PARTIAL line integrals; the sum over a
+ * partition into slabs is tigre_Ax of the whole volume (Siddon: intersection lengths are additive; interpolated: the sample
+ * positions are those of the full volume and taps outside the slab count as zero).  Rows outside the slab's detector-row
+ * band are zero.  vol_slab dev [nzs][ny][nx].
+ * tigre_Atb_slab: vol_slab (dev [nzs][ny][nx]) = slices [z0, z0 + nzs) of tigre_Atb (voxel-driven modes); it reads only
+ * the slab's row band of proj (dev, full size).
+ * tigre_slab_row_band: the band [row0, row0 + nrows) of detector rows the slab can reach in any of the views (corner
+ * projection in fp64, one row of margin); host arithmetic, no device needed. */
+TIGRE_API int tigre_Ax_slab(const float *vol_slab, const tigre_geo *geo, const double *angles, int nA, int mode, int z0, int nzs,
+                  float *proj, void *cuda_stream);
+TIGRE_API int tigre_Atb_slab(const float *proj, const tigre_geo *geo, const double *angles, int nA, int mode, int z0, int nzs,
+                   float *vol_slab, void *cuda_stream);
+TIGRE_API int tigre_slab_row_band(const tigre_geo *geo, const double *angles, int nA, int z0, int nzs, int *row0, int *nrows);
+
 /* ---- SIRT / OS-SART weights and elementwise updates (eq. 6 at 135) ----------
  * W = 1/(A 1) where (A 1) > 1e-2*min(dVoxel), else 0   (row sums; proj-shaped, dev)
  * V = 1/(A^T 1) where (A^T 1) > 1e-6*max(A^T 1), else 0 (column sums; vol-shaped, dev)  (P13) */

@@ -48,7 +48,7 @@ class TigreError(RuntimeError):
 
 
 _LIB = None
-EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_row_weights", "tigre_col_weights", "tigre_residual",
+EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_Ax_slab", "tigre_Atb_slab", "tigre_slab_row_band", "tigre_row_weights", "tigre_col_weights", "tigre_residual",
            "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_fdk", "tigre_fdk_filter", "tigre_fdk_ex", "tigre_fdk_filter_ex", "tigre_fdk_weights",
            "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
@@ -165,6 +165,44 @@ def Ax(vol, geo, angles, mode="siddon", out=None):
         out = _new(proj_shape(geo, nA), like=vol)
     po = _f32(out, proj_shape(geo, nA), "out")
     _check(_lib().tigre_Ax(pv, G.ref, a.ctypes.data_as(_dp), nA, _AX_MODES[mode], po, _stream(vol)), "tigre_Ax")
+    return out
+
+
+def slab_row_band(geo, angles, z0, nzs):
+    """(row0, nrows): detector rows the z-slab [z0, z0 + nzs) can reach in any view (host arithmetic)."""
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    r0, nr = C.c_int(0), C.c_int(0)
+    _check(_lib().tigre_slab_row_band(G.ref, a.ctypes.data_as(_dp), nA, int(z0), int(nzs), C.byref(r0), C.byref(nr)),
+           "tigre_slab_row_band")
+    return r0.value, nr.value
+
+
+def Ax_slab(vol_slab, geo, angles, z0, mode="siddon", out=None):
+    """Partial line integrals of the z-slices [z0, z0 + vol_slab.shape[0]) of a volume described by geo (full size)."""
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    nzs = int(vol_slab.shape[0])
+    pv = _f32(vol_slab, (nzs,) + tuple(vol_shape(geo)[1:]), "vol_slab")
+    if out is None:
+        out = _new(proj_shape(geo, nA), like=vol_slab)
+    po = _f32(out, proj_shape(geo, nA), "out")
+    _check(_lib().tigre_Ax_slab(pv, G.ref, a.ctypes.data_as(_dp), nA, _AX_MODES[mode], int(z0), nzs, po, _stream(vol_slab)),
+           "tigre_Ax_slab")
+    return out
+
+
+def Atb_slab(proj, geo, angles, z0, nzs, mode="matched", out=None):
+    """Slices [z0, z0 + nzs) of A^T b (voxel-driven modes)."""
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    pp = _f32(proj, proj_shape(geo, nA), "proj")
+    shape = (int(nzs),) + tuple(vol_shape(geo)[1:])
+    if out is None:
+        out = _new(shape, like=proj)
+    po = _f32(out, shape, "out")
+    _check(_lib().tigre_Atb_slab(pp, G.ref, a.ctypes.data_as(_dp), nA, _ATB_MODES[mode], int(z0), int(nzs), po, _stream(proj)),
+           "tigre_Atb_slab")
     return out
 
 

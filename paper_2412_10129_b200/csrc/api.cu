@@ -236,6 +236,78 @@ int tigre_Atb(const float* proj, const tigre_geo* geo, const double* angles, int
     return device_atb(proj, t, nullptr, nA, mode, false, vol, st);
 }
 
+// ---------------------------------------------------------------- z-slab entry points (multi-GPU sharding)
+int tigre_slab_row_band(const tigre_geo* geo, const double* angles, int nA, int z0, int nzs, int* row0, int* nrows) {
+    if (!row0 || !nrows) return TIGRE_ERR_ARG;
+    TG_TRY(validate_geo(geo, angles, nA));      // host arithmetic only: no device needed
+    const Grid g = make_grid(geo);
+    if (z0 < 0 || nzs <= 0 || z0 + nzs > g.nz) return TIGRE_ERR_ARG;
+    std::vector<ViewH> views;
+    resolve_views(geo, angles, nA, views);
+    int lo = g.nv, hi = 0;
+    for (int a = 0; a < nA; ++a) {
+        int r0, nr;
+        row_band(g, views[a], z0, nzs, r0, nr);
+        if (nr > 0) lo = std::min(lo, r0), hi = std::max(hi, r0 + nr);
+    }
+    *row0 = hi > lo ? lo : 0, *nrows = hi > lo ? hi - lo : 0;
+    return TIGRE_OK;
+}
+
+int tigre_Ax_slab(const float* vol_slab, const tigre_geo* geo, const double* angles, int nA, int mode, int z0, int nzs,
+                  float* proj, void* cuda_stream) {
+    if (!vol_slab || !proj) return TIGRE_ERR_ARG;
+    if (mode != TIGRE_AX_SIDDON && mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    const Grid& g = t.g;
+    if (z0 < 0 || nzs <= 0 || z0 + nzs > g.nz) return TIGRE_ERR_ARG;
+    if (mem_kind(vol_slab) != MEM_DEVICE || mem_kind(proj) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    TG_CUDA(cudaMemsetAsync(proj, 0, sizeof(float) * (size_t)nA * g.nu * g.nv, st));
+    AxSub sub;
+    {
+        int lo = g.nv, hi = 0;
+        for (int a = 0; a < nA; ++a) {
+            int r0, nr;
+            row_band(g, t.views[a], z0, nzs, r0, nr);
+            if (nr > 0) lo = std::min(lo, r0), hi = std::max(hi, r0 + nr);
+        }
+        sub.row0 = hi > lo ? lo : 0, sub.nrows = hi > lo ? hi - lo : 0;
+    }
+    if (sub.nrows == 0) return TIGRE_OK;
+    std::vector<RayView> hr(nA);
+    for (int i = 0; i < nA; ++i) build_ray_view(g, t.views[i], hr[i]);
+    if (mode == TIGRE_AX_SIDDON) {
+        // the slab as its own grid: same voxels, z origin moved to its first slice (intersection lengths are additive)
+        Grid gs = g;
+        gs.nz = nzs;
+        for (RayView& r : hr) r.S[2] -= (double)z0, r.P0[2] -= (double)z0;
+        TG_TRY(upload(t.ray, hr.data(), sizeof(RayView) * nA, st));
+        sub.zs0 = 0, sub.nzs = nzs;
+        return launch_ax(vol_slab, gs, t.ray.as<RayView>(), nA, mode, false, true, proj, nullptr, st, &sub);
+    }
+    // interpolated: the sample positions are those of the full volume; taps outside the slab count as zero
+    TG_TRY(upload(t.ray, hr.data(), sizeof(RayView) * nA, st));
+    sub.zs0 = z0, sub.nzs = nzs;
+    return launch_ax(vol_slab, g, t.ray.as<RayView>(), nA, mode, false, true, proj, nullptr, st, &sub);
+}
+
+int tigre_Atb_slab(const float* proj, const tigre_geo* geo, const double* angles, int nA, int mode, int z0, int nzs,
+                   float* vol_slab, void* cuda_stream) {
+    if (!vol_slab || !proj) return TIGRE_ERR_ARG;
+    if (mode != TIGRE_ATB_MATCHED && mode != TIGRE_ATB_FDK) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    const Grid& g = t.g;
+    if (z0 < 0 || nzs <= 0 || z0 + nzs > g.nz) return TIGRE_ERR_ARG;
+    if (mem_kind(vol_slab) != MEM_DEVICE || mem_kind(proj) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    TG_TRY(t.build_vox(nullptr, nA, st));
+    return launch_atb(proj, g, t.vox.as<VoxView>(), nA, mode, false, vol_slab, z0, nzs, false, 0, g.nv, t.clamp, st,
+                      t.hvox.data());
+}
+
 int tigre_row_weights(const tigre_geo* geo, const double* angles, int nA, int ax_mode, float* W, void* cuda_stream) {
     if (!W) return TIGRE_ERR_ARG;
     if (ax_mode != TIGRE_AX_SIDDON && ax_mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
