@@ -155,6 +155,12 @@ typedef struct tigre_plan tigre_plan;
 TIGRE_API int tigre_plan_create(const tigre_geo *geo, const double *angles, int nA, const int32_t *subset_idx,
                       const int32_t *subset_off, int nSubsets, int ax_mode, int atb_mode,
                       void *cuda_stream, tigre_plan **plan_out);
+/* tigre_plan_create with data-redundancy weighting for displaced detectors inside the iteration (DESIGN.md
+ * readings P17, P28): redundancy != 0 multiplies the row weights W of view a, column u by the Wang weight w_a(u) (1 on the
+ * singly measured side, a smooth ramp over the doubly measured columns); TIGRE_ERR_ARG if the displacement leaves no overlap. */
+TIGRE_API int tigre_plan_create_ex(const tigre_geo *geo, const double *angles, int nA, const int32_t *subset_idx,
+                         const int32_t *subset_off, int nSubsets, int ax_mode, int atb_mode, int redundancy,
+                         void *cuda_stream, tigre_plan **plan_out);
 TIGRE_API int tigre_plan_ossart(tigre_plan *plan, const float *b, float *x_inout, int n_iter, float lambda,
                       int nonneg, double *resid_hist, void *cuda_stream);
 TIGRE_API int tigre_plan_destroy(tigre_plan *plan);

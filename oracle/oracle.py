@@ -236,7 +236,7 @@ def _sub_geo(geo, idx):
 
 
 def ossart(b, geo, angles, subsets, n_iter, lam=1.0, nonneg=True, ax_mode=SIDDON, atb_mode=MATCHED,
-           x0=None, trace=None):
+           x0=None, trace=None, row_scale=None):
     """for it, for s:  r = W_s*(b_s - A_s x);  x += lam * V_s * A_s^T r;  x = max(x,0).
     SIRT is one subset holding all views.  resid[it] = sqrt(sum_s ||b_s - A_s x||^2) from the
     A_s x computed during the sweep (running residual).  Returns (x, resid)."""
@@ -245,6 +245,11 @@ def ossart(b, geo, angles, subsets, n_iter, lam=1.0, nonneg=True, ax_mode=SIDDON
     x = np.zeros(geo.vol_shape) if x0 is None else np.array(x0, dtype=np.float64)
     subsets = [np.asarray(s, dtype=np.int64) for s in subsets]
     Ws = [row_weights(_sub_geo(geo, s), angles[s], ax_mode) for s in subsets]
+    if row_scale is not None:
+        # data-redundancy weighting (reading P17): the row weights of view a, column u are multiplied
+        # by row_scale[a][u] (the displaced-detector weights of oracle/fdk_ext.py, P28)
+        rs = np.asarray(row_scale, dtype=np.float64)
+        Ws = [W * rs[s][:, None, :] for W, s in zip(Ws, subsets)]
     Vs = [col_weights(_sub_geo(geo, s), angles[s], atb_mode) for s in subsets]
     resid = np.zeros(n_iter)
     for it in range(n_iter):

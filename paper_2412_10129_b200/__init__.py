@@ -50,7 +50,7 @@ class TigreError(RuntimeError):
 _LIB = None
 EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_Ax_slab", "tigre_Atb_slab", "tigre_slab_row_band", "tigre_row_weights", "tigre_col_weights", "tigre_residual",
            "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_fdk", "tigre_fdk_filter", "tigre_fdk_ex", "tigre_fdk_filter_ex", "tigre_fdk_weights",
-           "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_destroy",
+           "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_create_ex", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version"]
 
@@ -274,7 +274,7 @@ def ossart(b, geo, angles, subsets, n_iter, lam=1.0, nonneg=True, ax_mode="siddo
 class OssartPlan:
     """tigre_plan_*: view tables and the SART weights computed once; iterate() runs sweeps."""
 
-    def __init__(self, geo, angles, subsets, ax_mode="siddon", atb_mode="matched"):
+    def __init__(self, geo, angles, subsets, ax_mode="siddon", atb_mode="matched", redundancy=False):
         a, nA = _angles(angles)
         G = _Geo(geo, nA)
         idx = np.ascontiguousarray(np.concatenate([np.asarray(s, dtype=np.int32) for s in subsets]))
@@ -282,9 +282,10 @@ class OssartPlan:
         off[1:] = np.cumsum([len(s) for s in subsets])
         self.geo, self.nA = geo, nA
         self._h = C.c_void_p(None)
-        _check(_lib().tigre_plan_create(G.ref, a.ctypes.data_as(_dp), nA, idx.ctypes.data_as(C.POINTER(C.c_int32)),
-                                        off.ctypes.data_as(C.POINTER(C.c_int32)), len(subsets), _AX_MODES[ax_mode],
-                                        _ATB_MODES[atb_mode], _stream(), C.byref(self._h)), "tigre_plan_create")
+        _check(_lib().tigre_plan_create_ex(G.ref, a.ctypes.data_as(_dp), nA, idx.ctypes.data_as(C.POINTER(C.c_int32)),
+                                           off.ctypes.data_as(C.POINTER(C.c_int32)), len(subsets), _AX_MODES[ax_mode],
+                                           _ATB_MODES[atb_mode], int(bool(redundancy)), _stream(), C.byref(self._h)),
+               "tigre_plan_create_ex")
 
     @property
     def nbytes(self):

@@ -402,6 +402,12 @@ struct tigre_plan {
 int tigre_plan_create(const tigre_geo* geo, const double* angles, int nA, const int32_t* subset_idx,
                       const int32_t* subset_off, int nSubsets, int ax_mode, int atb_mode, void* cuda_stream,
                       tigre_plan** out) {
+    return tigre_plan_create_ex(geo, angles, nA, subset_idx, subset_off, nSubsets, ax_mode, atb_mode, 0, cuda_stream, out);
+}
+
+int tigre_plan_create_ex(const tigre_geo* geo, const double* angles, int nA, const int32_t* subset_idx,
+                         const int32_t* subset_off, int nSubsets, int ax_mode, int atb_mode, int redundancy,
+                         void* cuda_stream, tigre_plan** out) {
     if (!out || !subset_idx || !subset_off || nSubsets <= 0) return TIGRE_ERR_ARG;
     *out = nullptr;
     if (ax_mode != TIGRE_AX_SIDDON && ax_mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
@@ -432,6 +438,8 @@ int tigre_plan_create(const tigre_geo* geo, const double* angles, int nA, const 
     P->vox = std::vector<TempBuf>(nSubsets);
     P->hvox.resize(nSubsets);
     const double epsW = 1e-2 * std::min(g.dx, std::min(g.dy, g.dz));
+    std::vector<double> red;
+    if (redundancy) TG_TRY(fdk_weights(g, P->t.views, TIGRE_FDK_WANG, red));   // [nA][nu], reading P17 / P28
     for (int s = 0; s < nSubsets; ++s) {
         const int32_t* idx = subset_idx + subset_off[s];
         const int n = subset_off[s + 1] - subset_off[s];
@@ -449,6 +457,14 @@ int tigre_plan_create(const tigre_geo* geo, const double* angles, int nA, const 
         float* Vs = P->V.as<float>() + nvox * s;
         TG_TRY(launch_ax(nullptr, g, P->ray[s].as<RayView>(), n, ax_mode, true, false, Ws, nullptr, st));
         TG_TRY(launch_invert_rows(Ws, per * n, (float)epsW, st));
+        if (redundancy) {
+            std::vector<float> cw((size_t)n * g.nu);
+            for (int i = 0; i < n; ++i)
+                for (int iu = 0; iu < g.nu; ++iu) cw[(size_t)i * g.nu + iu] = (float)red[(size_t)idx[i] * g.nu + iu];
+            TempBuf tc;
+            TG_TRY(upload(tc, cw.data(), sizeof(float) * cw.size(), st));
+            TG_TRY(launch_scale_columns(Ws, tc.as<float>(), n, g.nv, g.nu, st));
+        }
         TG_TRY(launch_atb(nullptr, g, P->vox[s].as<VoxView>(), n, atb_mode, true, Vs, 0, g.nz, false, 0, g.nv, P->clamp, st));
         TG_TRY(launch_invert_cols(Vs, nvox, 1e-6f, st));
     }

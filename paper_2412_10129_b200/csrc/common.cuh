@@ -133,6 +133,7 @@ int launch_axpy(float* y, const float* x, const double* d_num, const double* d_d
 int launch_xpby(float* p, const float* s, const double* d_num, const double* d_den, size_t n,
                 cudaStream_t st);                                                       // p = s + (num/den)*p
 int launch_scale(float* x, float a, size_t n, cudaStream_t st);
+int launch_scale_columns(float* W, const float* colw, int nViews, int nv, int nu, cudaStream_t st);
 int launch_diff_stats(const float* a, const float* b, const float* c, size_t n, double* d_out3, cudaStream_t st);
 int launch_fdk_filter(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, int nViews,
                       float* q, cudaStream_t st);

@@ -161,6 +161,23 @@ int launch_invert_cols(float* v, size_t n, float rel_eps, cudaStream_t st) {
     return TIGRE_OK;
 }
 
+// W[j][iv][iu] *= colw[j][iu]   (data-redundancy weighting of the row weights, reading P17)
+__global__ void __launch_bounds__(256) scale_columns_kernel(float* __restrict__ W, const float* __restrict__ colw, int nu, size_t per,
+                                                            size_t total) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t j = i / per;
+        const int iu = (int)((i - j * per) % (size_t)nu);
+        W[i] *= __ldg(colw + j * nu + iu);
+    }
+}
+int launch_scale_columns(float* W, const float* colw, int nViews, int nv, int nu, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
+    const size_t per = (size_t)nv * nu, total = per * nViews;
+    if (total == 0) return TIGRE_OK;
+    scale_columns_kernel<<<ew_blocks(total), 256, 0, st>>>(W, colw, nu, per, total);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
 __global__ void __launch_bounds__(256) dot_kernel(const float* __restrict__ a, const float* __restrict__ b, size_t n, double* __restrict__ out) {
     double s = 0.0;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)

@@ -49,3 +49,28 @@ def test_weighting_errors():
                     offDetector=(9.0, 0.0))                          # displaced by more than half the detector: no overlap
     with pytest.raises(tg.TigreError):
         tg.fdk_weights(wide, full, "wang")
+
+
+def test_oracle_ossart_row_scale_pins():
+    # the redundancy weighting of the iterative methods (reading P17) enters oracle.ossart as a scale of the row weights:
+    # ones change nothing (bitwise); a constant c scales the first SIRT step by c (the update is linear in W); a scale
+    # that zeroes some columns equals running on data whose residual is zeroed there
+    from oracle import oracle as orc
+    from workloads import make_config, phantom_for
+    geo, ang, rec = make_config("C3", scale=32, n_angles=8)           # 16^3, 32x24 detector displaced by +20 mm
+    vol = phantom_for(rec, geo).astype(np.float64)
+    b = orc.ax(vol, geo, ang, orc.SIDDON)
+    subsets = [list(range(0, 8, 2)), list(range(1, 8, 2))]
+    nu = geo.nDetector[0]
+    x_plain, _ = orc.ossart(b, geo, ang, subsets, 2)
+    x_ones, _ = orc.ossart(b, geo, ang, subsets, 2, row_scale=np.ones((8, nu)))
+    assert np.array_equal(x_plain, x_ones)
+    x1, _ = orc.ossart(b, geo, ang, [list(range(8))], 1, nonneg=False)
+    xc, _ = orc.ossart(b, geo, ang, [list(range(8))], 1, nonneg=False, row_scale=np.full((8, nu), 0.25))
+    assert np.allclose(xc, 0.25 * x1, rtol=1e-13, atol=0)
+    mask = np.ones((8, nu))
+    mask[:, : nu // 3] = 0.0
+    xm, _ = orc.ossart(b, geo, ang, [list(range(8))], 1, nonneg=False, row_scale=mask)
+    W = orc.row_weights(geo, ang, orc.SIDDON) * mask[:, None, :]
+    ref = orc.col_weights(geo, ang, orc.MATCHED) * orc.atb(W * b, geo, ang, orc.MATCHED)
+    assert np.allclose(xm, ref, rtol=1e-13, atol=1e-18)

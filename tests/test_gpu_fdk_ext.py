@@ -111,3 +111,22 @@ def test_argument_errors(tg):
     with pytest.raises(tg.TigreError) as e:
         tg.fdk_ex(b.cpu(), geo, ang, "hann", None)
     assert e.value.code == -3
+
+
+def test_redundancy_weighting_inside_ossart_matches_oracle(tg):
+    # the displaced-detector weights inside the iteration (plan created with redundancy on; reading P17)
+    geo, ang, rec = make_config("C3", scale=16, n_angles=40)           # 32^3, 64x48 detector displaced by +20 mm (the case of test_ossart_scaled_c3)
+    vol = phantom_for(rec, geo).astype(np.float64)
+    b = orc.ax(vol, geo, ang, orc.SIDDON).astype(np.float32)
+    nA = len(ang)
+    subsets = [list(range(s, nA, 5)) for s in range(5)]
+    w = fx.wang_weights(geo, nA)
+    ref, rres = orc.ossart(b, geo, ang, subsets, 3, row_scale=w)
+    plan = tg.OssartPlan(geo, ang, subsets, "siddon", "matched", redundancy=True)
+    x = torch.zeros(geo.vol_shape, dtype=torch.float32, device="cuda")
+    res = plan.iterate(dev(b), x, 3)
+    plan.close()
+    assert H.rel_l2(host(x), ref) <= 1e-4
+    assert np.allclose(res, rres, rtol=1e-4)
+    plain, _ = orc.ossart(b, geo, ang, subsets, 3)
+    assert H.rel_l2(host(x), plain) > 1e-3                             # and it is not the unweighted iteration
