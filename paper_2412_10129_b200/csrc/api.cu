@@ -491,12 +491,42 @@ int tigre_plan_ossart(tigre_plan* P, const float* b, float* x, int n_iter, float
     TempBuf db, dx;
     const float* bd = b;
     float* xd = x;
+    // end-to-end path: the projections go up on a side stream in the order the subsets need them (one event per subset:
+    // the first sweep's residual of subset s waits for its views only), so all but the first subset's upload hides
+    // behind the kernels; the iterate goes up first on the caller's stream
+    cudaStream_t up = nullptr;
+    std::vector<cudaEvent_t> ev;
+    struct Cleanup {
+        cudaStream_t& s;
+        std::vector<cudaEvent_t>& e;
+        ~Cleanup() {
+            for (cudaEvent_t x : e) cudaEventDestroy(x);
+            if (s) cudaStreamDestroy(s);
+        }
+    } cleanup{up, ev};
     if (kb == MEM_PINNED && kx == MEM_PINNED) {
         TG_TRY(db.alloc(sizeof(float) * per * P->nA, st));
         TG_TRY(dx.alloc(sizeof(float) * nvox, st));
-        TG_CUDA(cudaMemcpyAsync(db.p, b, sizeof(float) * per * P->nA, cudaMemcpyHostToDevice, st));
-        TG_CUDA(cudaMemcpyAsync(dx.p, x, sizeof(float) * nvox, cudaMemcpyHostToDevice, st));
         bd = db.as<float>(), xd = dx.as<float>();
+        TG_CUDA(cudaMemcpyAsync(dx.p, x, sizeof(float) * nvox, cudaMemcpyHostToDevice, st));
+        if (n_iter > 0) {
+            TG_CUDA(cudaStreamCreateWithFlags(&up, cudaStreamNonBlocking));
+            cudaEvent_t start;
+            TG_CUDA(cudaEventCreateWithFlags(&start, cudaEventDisableTiming));
+            ev.push_back(start);
+            TG_CUDA(cudaEventRecord(start, st));               // the buffer exists from here on in stream order
+            TG_CUDA(cudaStreamWaitEvent(up, start, 0));
+            for (int s = 0; s < P->nSubsets; ++s) {
+                for (int k = P->off[s]; k < P->off[s + 1]; ++k) {
+                    const size_t o = per * (size_t)P->idx[k];
+                    TG_CUDA(cudaMemcpyAsync(db.as<float>() + o, b + o, sizeof(float) * per, cudaMemcpyHostToDevice, up));
+                }
+                cudaEvent_t e;
+                TG_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+                ev.push_back(e);
+                TG_CUDA(cudaEventRecord(e, up));
+            }
+        }
     } else if (kb != MEM_DEVICE || kx != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
     TG_TRY(P->d_acc.alloc(sizeof(double) * std::max(n_iter, 1), st));
     TG_CUDA(cudaMemsetAsync(P->d_acc.p, 0, sizeof(double) * std::max(n_iter, 1), st));
@@ -507,6 +537,7 @@ int tigre_plan_ossart(tigre_plan* P, const float* b, float* x, int n_iter, float
             float* Vs = P->V.as<float>() + nvox * s;
             float* A = P->Axb.as<float>();
             TG_TRY(launch_ax(xd, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st));
+            if (up && it == 0) TG_CUDA(cudaStreamWaitEvent(st, ev[1 + s], 0));   // this subset's projections have arrived
             // r = W_s .* (b_s - A_s x) in place over A; b is gathered through the subset's view list
             TG_TRY(launch_residual(bd, P->d_idx.as<int32_t>() + P->off[s], A, Ws, A, per, n, P->d_acc.as<double>() + it, st));
             TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>(), 0, g.nz, false, 0, g.nv, P->clamp, st,
