@@ -212,6 +212,67 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, i
 static_assert((TM_BY + 1) % 4 == 0, "a staged plane must be a multiple of 128 bytes (TMA destination alignment)");
 constexpr size_t TM_SMEM = (size_t)TM_D * TM_PLANE * 4 + 2 * TM_BY * 32 * 16 + 64 * 4 + TM_D * 8;
 
+struct TmRow {   // a row-warp thread's walk state
+    float4 xprev, Sprev;
+    float* pg;
+    float vacc, gacc;
+    double val, gg;
+};
+
+// One plane of a row-warp thread.  EDGE = false: 1 <= i <= nplanes - 2, i.e. the plane exists (1 <= z < nz, z < ze) and the
+// previous plane has been visited: nothing is tested.
+template <bool AW, bool EDGE>
+__device__ __forceinline__ void tm_plane(TmRow& w, int i, int zs, int ze, int nz, int nreal, int& s, uint32_t& parity, uint64_t* full,
+                                         const float* ring, float4* say, const float* sedge, int oc, int ou, int tx, int ty,
+                                         float thr_a, float thr_b, bool owner, bool hasg, size_t plane, float nl2, float id2,
+                                         float eps) {
+    const float inf = __int_as_float(0x7f800000);
+    const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    const int z = zs + i;
+    float4 c = zero4, u = zero4;
+    float l = 0.f;
+    if (!EDGE || i < nreal) {
+        mbar_wait(full + s, parity);
+        const float* T = ring + s * TM_PLANE;
+        c = *reinterpret_cast<const float4*>(T + oc);
+        u = *reinterpret_cast<const float4*>(T + ou);
+        l = __shfl_up_sync(0xffffffffu, c.w, 1);
+        if (tx == 0) l = T[oc - 1];
+    }
+    float ta = thr_a, tb = thr_b;
+    if (EDGE && !(z >= 1 && z < nz)) ta = inf, tb = inf;
+    float4 fx, fy, fz, T4;
+    tv_voxel<AW>(c.x - l, c.x - u.x, c.x - w.xprev.x, ta, nl2, id2, eps, fx.x, fy.x, fz.x, T4.x);
+    tv_voxel<AW>(c.y - c.x, c.y - u.y, c.y - w.xprev.y, tb, nl2, id2, eps, fx.y, fy.y, fz.y, T4.y);
+    tv_voxel<AW>(c.z - c.y, c.z - u.z, c.z - w.xprev.z, tb, nl2, id2, eps, fx.z, fy.z, fz.z, T4.z);
+    tv_voxel<AW>(c.w - c.z, c.w - u.w, c.w - w.xprev.w, tb, nl2, id2, eps, fx.w, fy.w, fz.w, T4.w);
+    float fxr = __shfl_down_sync(0xffffffffu, fx.x, 1);       // a_x of the next lane's first voxel
+    float4* sb = say + (i & 1) * (TM_BY * 32);
+    sb[ty * 32 + tx] = fy;
+    cta_sync();
+    float4 fyn = zero4;
+    if (ty + 1 < TM_BY) fyn = sb[(ty + 1) * 32 + tx];         // a_y(p + e_y)
+    if (tx == 31) fxr = sedge[(i & 1) * 32 + ty];             // the last lane's neighbour is the edge warp's voxel
+    if (owner) {
+        if ((!EDGE || i > 0) && hasg) {       // the previous plane is complete now: its a_z(p + e_z) is this fz
+            float4 v;
+            v.x = w.Sprev.x - fz.x, v.y = w.Sprev.y - fz.y, v.z = w.Sprev.z - fz.z, v.w = w.Sprev.w - fz.w;
+            *reinterpret_cast<float4*>(w.pg - plane) = v;
+            w.gacc = fmaf(v.x, v.x, fmaf(v.y, v.y, fmaf(v.z, v.z, fmaf(v.w, v.w, w.gacc))));
+        }
+        if (!EDGE || z < ze) w.vacc += (T4.x + T4.y) + (T4.z + T4.w);
+    }
+    // partial sums in fp32 over 16 planes at a time, then into fp64
+    if ((i & 15) == 15) w.val += (double)w.vacc, w.gg += (double)w.gacc, w.vacc = 0.f, w.gacc = 0.f;
+    w.Sprev.x = fx.x + fy.x + fz.x - fx.y - fyn.x;
+    w.Sprev.y = fx.y + fy.y + fz.y - fx.z - fyn.y;
+    w.Sprev.z = fx.z + fy.z + fz.z - fx.w - fyn.z;
+    w.Sprev.w = fx.w + fy.w + fz.w - fxr - fyn.w;
+    w.xprev = c;
+    w.pg += plane;
+    if (++s == TM_D) s = 0, parity ^= 1;
+}
+
 template <bool AW>
 __global__ void __launch_bounds__(32 * (TM_BY + 1), 2)
 tv_gradient_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict__ x, int nx, int ny, int nz, float nl2,
@@ -286,51 +347,17 @@ tv_gradient_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __
         float4 Sprev = zero4;
         float vacc = 0.f, gacc = 0.f;
         const int oc = (ty + 1) * TM_W + 4 + 4 * tx, ou = ty * TM_W + 4 + 4 * tx;
-        for (int i = 0; i < nplanes; ++i) {
-            const int z = zs + i;
-            float4 c = zero4, u = zero4;
-            float l = 0.f;
-            if (i < nreal) {
-                mbar_wait(full + s, parity);
-                const float* T = ring + s * TM_PLANE;
-                c = *reinterpret_cast<const float4*>(T + oc);
-                u = *reinterpret_cast<const float4*>(T + ou);
-                l = __shfl_up_sync(0xffffffffu, c.w, 1);
-                if (tx == 0) l = T[oc - 1];
-            }
-            const bool zin = z >= 1 && z < nz;
-            const float ta = zin ? thr_a : inf, tb = zin ? thr_b : inf;
-            float4 fx, fy, fz, T4;
-            tv_voxel<AW>(c.x - l, c.x - u.x, c.x - xprev.x, ta, nl2, id2, eps, fx.x, fy.x, fz.x, T4.x);
-            tv_voxel<AW>(c.y - c.x, c.y - u.y, c.y - xprev.y, tb, nl2, id2, eps, fx.y, fy.y, fz.y, T4.y);
-            tv_voxel<AW>(c.z - c.y, c.z - u.z, c.z - xprev.z, tb, nl2, id2, eps, fx.z, fy.z, fz.z, T4.z);
-            tv_voxel<AW>(c.w - c.z, c.w - u.w, c.w - xprev.w, tb, nl2, id2, eps, fx.w, fy.w, fz.w, T4.w);
-            float fxr = __shfl_down_sync(0xffffffffu, fx.x, 1);       // a_x of the next lane's first voxel
-            float4* sb = say + (i & 1) * (TM_BY * 32);
-            sb[ty * 32 + tx] = fy;
-            cta_sync();
-            float4 fyn = zero4;
-            if (ty + 1 < TM_BY) fyn = sb[(ty + 1) * 32 + tx];         // a_y(p + e_y)
-            if (tx == 31) fxr = sedge[(i & 1) * 32 + ty];             // the last lane's neighbour is the edge warp's voxel
-            if (owner) {
-                if (i > 0 && hasg) {          // the previous plane is complete now: its a_z(p + e_z) is this fz
-                    float4 v;
-                    v.x = Sprev.x - fz.x, v.y = Sprev.y - fz.y, v.z = Sprev.z - fz.z, v.w = Sprev.w - fz.w;
-                    *reinterpret_cast<float4*>(pg - plane) = v;
-                    gacc = fmaf(v.x, v.x, fmaf(v.y, v.y, fmaf(v.z, v.z, fmaf(v.w, v.w, gacc))));
-                }
-                if (z < ze) vacc += (T4.x + T4.y) + (T4.z + T4.w);
-            }
-            // partial sums in fp32 over 16 planes at a time, then into fp64
-            if ((i & 15) == 15) val += (double)vacc, gg += (double)gacc, vacc = 0.f, gacc = 0.f;
-            Sprev.x = fx.x + fy.x + fz.x - fx.y - fyn.x;
-            Sprev.y = fx.y + fy.y + fz.y - fx.z - fyn.y;
-            Sprev.z = fx.z + fy.z + fz.z - fx.w - fyn.z;
-            Sprev.w = fx.w + fy.w + fz.w - fxr - fyn.w;
-            xprev = c;
-            pg += plane;
-            if (++s == TM_D) s = 0, parity ^= 1;
-        }
+        TmRow w{xprev, Sprev, pg, vacc, gacc, val, gg};
+        // first and last plane of the chunk carry the tests (z = 0, z = nz, nothing to write yet, no T to count);
+        // the planes between are interior to the volume and run without them
+        tm_plane<AW, true>(w, 0, zs, ze, nz, nreal, s, parity, full, ring, say, sedge, oc, ou, tx, ty, thr_a, thr_b, owner, hasg,
+                           plane, nl2, id2, eps);
+        for (int i = 1; i < nplanes - 1; ++i)
+            tm_plane<AW, false>(w, i, zs, ze, nz, nreal, s, parity, full, ring, say, sedge, oc, ou, tx, ty, thr_a, thr_b, owner, hasg,
+                                plane, nl2, id2, eps);
+        tm_plane<AW, true>(w, nplanes - 1, zs, ze, nz, nreal, s, parity, full, ring, say, sedge, oc, ou, tx, ty, thr_a, thr_b, owner,
+                           hasg, plane, nl2, id2, eps);
+        vacc = w.vacc, gacc = w.gacc, val = w.val, gg = w.gg;
         val += (double)vacc, gg += (double)gacc;
     }
     if (d_val) {
