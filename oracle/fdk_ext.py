@@ -136,9 +136,10 @@ def fdk_filter(proj, geo, angles, filt="ram_lak", colw=None):
     p = np.asarray(proj, dtype=np.float64).reshape(nA, nv, nu)
     out = np.zeros_like(p)
     L = pad_length(nu)
+    par = getattr(geo, "mode", "cone") == "parallel"       # P29: no magnification, no cosine weight
     for a in range(nA):
-        tau = du * DSO[a] / DSD[a]
-        cosw = DSD[a] / np.sqrt(DSD[a] ** 2 + u[None, :] ** 2 + v[:, None] ** 2)
+        tau = du if par else du * DSO[a] / DSD[a]
+        cosw = 1.0 if par else DSD[a] / np.sqrt(DSD[a] ** 2 + u[None, :] ** 2 + v[:, None] ** 2)
         row = p[a] * cosw
         if colw is not None:
             row = row * colw[a][None, :]

@@ -25,7 +25,7 @@ MATCHED, FDK = 0, 1
 
 class _Grid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
-                ("nu", C.c_int32), ("nv", C.c_int32),
+                ("nu", C.c_int32), ("nv", C.c_int32), ("parallel", C.c_int32),
                 ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double),
                 ("du", C.c_double), ("dv", C.c_double), ("accuracy", C.c_double)]
 
@@ -53,6 +53,7 @@ def num_threads() -> int:
 
 def _grid(geo) -> _Grid:
     return _Grid(geo.nVoxel[0], geo.nVoxel[1], geo.nVoxel[2], geo.nDetector[0], geo.nDetector[1],
+                 1 if getattr(geo, "mode", "cone") == "parallel" else 0,
                  geo.dVoxel[0], geo.dVoxel[1], geo.dVoxel[2], geo.dDetector[0], geo.dDetector[1],
                  geo.accuracy)
 

@@ -40,6 +40,7 @@
 typedef struct {
     int32_t nx, ny, nz;
     int32_t nu, nv;
+    int32_t parallel; /* 0 = cone beam; 1 = parallel beam (reading P29): rays along the S-O line */
     double dx, dy, dz;
     double du, dv;
     double accuracy;
@@ -129,6 +130,17 @@ static void pixel_pos(const orc_grid *g, const orc_view *w, const double Rg[9], 
     double p1[3] = {w->DSO - w->DSD + r[0], w->offD[0] + r[1] - w->COR, w->offD[1] + r[2]};
     mv(Rg, p1, P);
 }
+/* P29 parallel beam: every ray runs along the gantry-rotated x axis (the S-O line); its segment starts DSD in front of
+ * its pixel.  Cone beam: all rays start at the source. */
+static void ray_start(const orc_grid *g, const orc_view *w, const double Rg[9], const double P[3], double S[3]) {
+    if (g->parallel) {
+        double e[3] = {w->DSD, 0.0, 0.0}, r[3];
+        mv(Rg, e, r);
+        for (int k = 0; k < 3; k++) S[k] = P[k] + r[k];
+    } else {
+        source_pos(w, Rg, S);
+    }
+}
 /* voxel centre X (world) -> continuous detector index (fu,fv) and the weight terms */
 typedef struct {
     double fu, fv;
@@ -149,6 +161,20 @@ static vox_map voxel_to_det(const orc_grid *g, const orc_view *w, const double R
     double q[3], s[3];
     mtv(Rd, a, q);
     mtv(Rd, b, s);
+    if (g->parallel) {
+        /* slide the voxel along the ray direction e = R_det^T e_x onto the detector plane q_x = 0 */
+        double ex[3] = {1.0, 0.0, 0.0}, e[3];
+        mtv(Rd, ex, e);
+        double t = q[0] / e[0];
+        double u = q[1] - t * e[1], v = q[2] - t * e[2];
+        m.fu = (u + 0.5 * g->nu * g->du) / g->du - 0.5;
+        m.fv = (v + 0.5 * g->nv * g->dv) / g->dv - 0.5;
+        m.depth = w->DSO; /* FDK distance weight (DSO/depth)^2 = 1 */
+        m.R = m.r = 1.0;  /* no magnification */
+        m.cosg = fabs(e[0]);
+        m.ok = 1;
+        return m;
+    }
     m.depth = w->DSO - Xp[0];
     double den = s[0] - q[0];
     m.ok = (den > 0.0) && (m.depth > 0.0);
@@ -349,8 +375,8 @@ int orc_ax(const void *vol, int vol_f32, const orc_grid *g, const orc_view *view
             const orc_view *w = &views[ia];
             double Rg[9], Rd[9], S[3], P[3];
             frames(w, Rg, Rd);
-            source_pos(w, Rg, S);
             pixel_pos(g, w, Rg, Rd, iu, iv, P);
+            ray_start(g, w, Rg, P, S);
             if (mode == 0) {
                 int ns = siddon_ray(g, w, S, P, ts, idx, len);
                 double s = 0.0;
@@ -381,8 +407,8 @@ int orc_siddon_segments(const orc_grid *g, const orc_view *views, int ia, int iu
     const orc_view *w = &views[ia];
     double Rg[9], Rd[9], S[3], P[3];
     frames(w, Rg, Rd);
-    source_pos(w, Rg, S);
     pixel_pos(g, w, Rg, Rd, iu, iv, P);
+    ray_start(g, w, Rg, P, S);
     int ns = siddon_ray(g, w, S, P, ts, idx, len);
     free(ts);
     return ns;
@@ -403,11 +429,11 @@ int orc_atb_exact(const void *proj, int proj_f32, const orc_grid *g, const orc_v
         const orc_view *w = &views[ia];
         double Rg[9], Rd[9], S[3], P[3];
         frames(w, Rg, Rd);
-        source_pos(w, Rg, S);
         for (int iv = 0; iv < g->nv; iv++)
             for (int iu = 0; iu < g->nu; iu++) {
                 double yv = LD(Y, ((size_t)ia * g->nv + iv) * g->nu + iu);
                 pixel_pos(g, w, Rg, Rd, iu, iv, P);
+                ray_start(g, w, Rg, P, S);
                 if (mode == 0) {
                     int ns = siddon_ray(g, w, S, P, ts, idx, len);
                     for (int j = 0; j < ns; j++) vol_out[idx[j]] += len[j] * yv;
@@ -511,12 +537,12 @@ int orc_fdk_filter(const void *proj, int proj_f32, const orc_grid *g, const orc_
         for (int ia = 0; ia < nA; ia++)
             for (int iv = 0; iv < nv; iv++) {
                 const orc_view *w = &views[ia];
-                double tau = g->du * w->DSO / w->DSD;
+                double tau = g->parallel ? g->du : g->du * w->DSO / w->DSD; /* P29: no magnification */
                 double v = (iv + 0.5) * g->dv - 0.5 * nv * g->dv;
                 size_t base = ((size_t)ia * nv + iv) * nu;
                 for (int iu = 0; iu < nu; iu++) {
                     double u = (iu + 0.5) * g->du - 0.5 * nu * g->du;
-                    row[iu] = LD(Y, base + iu) * w->DSD / sqrt(w->DSD * w->DSD + u * u + v * v);
+                    row[iu] = LD(Y, base + iu) * (g->parallel ? 1.0 : w->DSD / sqrt(w->DSD * w->DSD + u * u + v * v));
                 }
                 for (int iu = 0; iu < nu; iu++) {
                     double s = row[iu] / (4.0 * tau * tau);
@@ -538,8 +564,8 @@ void orc_source_pixel(const orc_grid *g, const orc_view *views, int ia, double i
                       double S[3], double P[3]) {
     double Rg[9], Rd[9];
     frames(&views[ia], Rg, Rd);
-    source_pos(&views[ia], Rg, S);
     pixel_pos(g, &views[ia], Rg, Rd, iu, iv, P);
+    ray_start(g, &views[ia], Rg, P, S);
 }
 void orc_voxel_map(const orc_grid *g, const orc_view *views, int ia, int ix, int iy, int iz,
                    double X[3], double fuv[2]) {

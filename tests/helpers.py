@@ -42,6 +42,29 @@ def pixel_world(geo, angles, ia, iu, iv):
     return S, Dc + np.multiply.outer(u, eu) + np.multiply.outer(v, ev)
 
 
+def parallel_rays(geo, angles, ia, iu, iv):
+    """Parallel-beam mode (reading P29), independently of the oracle: start and end points of the rays of pixels
+    (iu, iv): every ray runs along the gantry-rotated x axis and ends at its pixel, starting DSD in front of it."""
+    S, Dc, eu, ev, n, p = world_frame(geo, angles, ia)
+    u = (np.asarray(iu) + 0.5) * geo.dDetector[0] - 0.5 * geo.nDetector[0] * geo.dDetector[0]
+    v = (np.asarray(iv) + 0.5) * geo.dDetector[1] - 0.5 * geo.nDetector[1] * geo.dDetector[1]
+    P = Dc + np.multiply.outer(u, eu) + np.multiply.outer(v, ev)
+    ex = Rot.from_euler("ZYZ", p["ang"]).as_matrix() @ np.array([1.0, 0.0, 0.0])
+    return P + p["DSD"] * ex, P
+
+
+def parallel_voxel_to_detector(geo, angles, ia, X):
+    """Parallel-beam mode: continuous pixel index of the point where the ray through X (direction: gantry x axis) meets
+    the detector plane, and the cosine between ray and detector normal."""
+    S, Dc, eu, ev, n, p = world_frame(geo, angles, ia)
+    ex = Rot.from_euler("ZYZ", p["ang"]).as_matrix() @ np.array([1.0, 0.0, 0.0])
+    t = ((Dc - X) @ n) / (ex @ n)
+    hit = X + t[..., None] * ex
+    fu = ((hit - Dc) @ eu + 0.5 * geo.nDetector[0] * geo.dDetector[0]) / geo.dDetector[0] - 0.5
+    fv = ((hit - Dc) @ ev + 0.5 * geo.nDetector[1] * geo.dDetector[1]) / geo.dDetector[1] - 0.5
+    return fu, fv, abs(float(ex @ n))
+
+
 def vol_box(geo, offO):
     s = np.array(geo.nVoxel) * np.array(geo.dVoxel)
     b0 = np.asarray(offO) - 0.5 * s

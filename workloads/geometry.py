@@ -26,6 +26,7 @@ class Geometry:
     offDetector: tuple = (0.0, 0.0)
     rotDetector: tuple = (0.0, 0.0, 0.0)     # (phi, theta, psi)
     accuracy: float = 0.5                    # interpolated-mode step, in voxels
+    mode: str = "cone"                       # "cone" or "parallel" (synchrotron parallel-beam data)
     # optional per-angle overrides ("defined individually for each projection")
     DSD_a: Optional[np.ndarray] = None       # [nA]
     DSO_a: Optional[np.ndarray] = None       # [nA]
