@@ -56,7 +56,12 @@ typedef struct tigre_geo {
     const double *offDetector_a;                /* [nA][2]  or NULL                           */
     const double *rotDetector_a;                /* [nA][3]  or NULL                           */
     double   accuracy;          /* interpolated-mode step in voxels (0.5 in configs C2, C4)   */
+    int32_t  mode;              /* TIGRE_GEO_CONE (0) or TIGRE_GEO_PARALLEL (1): PAPER.md:296-306 (synchrotron parallel-beam
+                                 * data); reading P29: every ray runs along the S-O line (the gantry-rotated x axis)
+                                 * and is the segment of length DSD that ends at its pixel; the voxel-driven map is affine,
+                                 * the matched weight dVoxel^3/(du dv cos), the FDK weight 1 (tigre_fdk = FBP)             */
 } tigre_geo;
+enum { TIGRE_GEO_CONE = 0, TIGRE_GEO_PARALLEL = 1 };
 
 typedef enum tigre_status {
     TIGRE_OK = 0,

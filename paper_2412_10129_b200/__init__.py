@@ -34,7 +34,7 @@ class tigre_geo(C.Structure):
         ("offOrigin", C.c_double * 3), ("offDetector", C.c_double * 2), ("rotDetector", C.c_double * 3),
         ("DSD_a", _dp), ("DSO_a", _dp), ("COR_a", _dp),
         ("offOrigin_a", _dp), ("offDetector_a", _dp), ("rotDetector_a", _dp),
-        ("accuracy", C.c_double),
+        ("accuracy", C.c_double), ("mode", C.c_int32),
     ]
 
 
@@ -95,6 +95,7 @@ class _Geo:
         g.offDetector[:] = [float(v) for v in geo.offDetector]
         g.rotDetector[:] = [float(v) for v in geo.rotDetector]
         g.accuracy = float(geo.accuracy)
+        g.mode = 1 if getattr(geo, "mode", "cone") == "parallel" else 0
         self.keep = []
         for name, width in (("DSD_a", 1), ("DSO_a", 1), ("COR_a", 1), ("offOrigin_a", 3),
                             ("offDetector_a", 2), ("rotDetector_a", 3)):

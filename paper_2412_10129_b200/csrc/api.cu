@@ -696,6 +696,8 @@ int tigre_cgls(const float* b, const tigre_geo* geo, const double* angles, int n
 static int fdk_filter_impl(const float* b, Tables& t, int nA, float* q, cudaStream_t st) {
     std::vector<double> dd(2 * (size_t)nA);
     for (int a = 0; a < nA; ++a) dd[a] = t.views[a].DSD, dd[nA + a] = t.views[a].DSO;
+    // parallel beam (P29): no magnification (tau = du) and no cosine weight: the kernels' DSO/DSD = 1, DSD/sqrt(DSD^2 + u^2 + v^2) = 1
+    if (t.views[0].parallel) std::fill(dd.begin(), dd.end(), 1e15);
     TempBuf tb;
     TG_TRY(upload(tb, dd.data(), sizeof(double) * dd.size(), st));
     return launch_fdk_filter(b, t.g, tb.as<double>(), tb.as<double>() + nA, nA, q, st);
@@ -725,10 +727,13 @@ int tigre_fdk(const float* b, const tigre_geo* geo, const double* angles, int nA
 static int fdk_filter_ex_impl(const float* b, Tables& t, int nA, int filter, int weighting, float* q, cudaStream_t st) {
     if (filter < TIGRE_FILTER_RAM_LAK || filter > TIGRE_FILTER_HANN) return TIGRE_ERR_ARG;
     if (weighting < TIGRE_FDK_FULL || weighting > TIGRE_FDK_WANG) return TIGRE_ERR_ARG;
+    if (weighting != TIGRE_FDK_FULL && t.views[0].parallel) return TIGRE_ERR_ARG;   // cone-beam redundancy weights
     if (filter == TIGRE_FILTER_RAM_LAK && weighting == TIGRE_FDK_FULL) return fdk_filter_impl(b, t, nA, q, st);
     const int nu = t.g.nu;
     std::vector<double> dd(2 * (size_t)nA), taps, w;
     for (int a = 0; a < nA; ++a) dd[a] = t.views[a].DSD, dd[nA + a] = t.views[a].DSO;
+    // parallel beam (P29): no magnification (tau = du) and no cosine weight: the kernels' DSO/DSD = 1, DSD/sqrt(DSD^2 + u^2 + v^2) = 1
+    if (t.views[0].parallel) std::fill(dd.begin(), dd.end(), 1e15);
     fdk_filter_taps(nu, filter, taps);
     std::vector<float> ft(taps.begin(), taps.end()), fw;
     TempBuf tb, tt, tw;

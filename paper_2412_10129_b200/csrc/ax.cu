@@ -144,7 +144,7 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     double S[3], d[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        S[k] = rv.S[k];
+        S[k] = rv.S[k] + iu * rv.dSU[k] + iv * rv.dSV[k];   // parallel beam: every ray has its own start (P29)
         d[k] = rv.P0[k] + iu * rv.dU[k] + iv * rv.dV[k] - S[k];
     }
     const double Lmm = sqrt(d[0] * p.hxd * d[0] * p.hxd + d[1] * p.hyd * d[1] * p.hyd + d[2] * p.hzd * d[2] * p.hzd);
@@ -314,7 +314,7 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     double S[3], d[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        S[k] = rv.S[k];
+        S[k] = rv.S[k] + iu * rv.dSU[k] + iv * rv.dSV[k];   // parallel beam: every ray has its own start (P29)
         d[k] = rv.P0[k] + iu * rv.dU[k] + iv * rv.dV[k] - S[k];
     }
     const double h[3] = {p.hxd, p.hyd, p.hzd};

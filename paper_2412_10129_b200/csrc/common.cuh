@@ -30,6 +30,7 @@ void set_cuda_error(cudaError_t e, const char* file, int line);
 struct ViewH {  // one projection's resolved parameters (everything but sizes per view)
     double DSD, DSO, COR;
     double offO[3], offD[2], rotD[3], ang[3];
+    int parallel;   // tigre_geo.mode == TIGRE_GEO_PARALLEL (reading P29)
 };
 
 // Ray-driven per-view table, in VOXEL-INDEX coordinates xi = (X - volume_min)/dVoxel, so voxel
@@ -40,6 +41,8 @@ struct RayView {
     double P0[3];   // centre of pixel (0,0)
     double dU[3];   // step per pixel along u
     double dV[3];   // step per pixel along v
+    double dSU[3];  // step of the ray's START per pixel along u / v: zero for cone beam (all rays start at S),
+    double dSV[3];  // = dU / dV for parallel beam (S is then the start of pixel (0,0)'s ray)
 };
 
 // Voxel-driven per-view table (fp32, built in fp64).  With c = centred voxel index

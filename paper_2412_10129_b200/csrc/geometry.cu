@@ -60,6 +60,7 @@ void resolve_views(const tigre_geo* geo, const double* angles, int nA, std::vect
         for (int k = 0; k < 2; ++k) v.offD[k] = geo->offDetector_a ? geo->offDetector_a[2 * a + k] : geo->offDetector[k];
         for (int k = 0; k < 3; ++k) v.rotD[k] = geo->rotDetector_a ? geo->rotDetector_a[3 * a + k] : geo->rotDetector[k];
         for (int k = 0; k < 3; ++k) v.ang[k] = angles[3 * a + k];
+        v.parallel = geo->mode == TIGRE_GEO_PARALLEL;
     }
 }
 
@@ -71,6 +72,7 @@ int validate_geo(const tigre_geo* geo, const double* angles, int nA) {
     for (int k = 0; k < 2; ++k)
         if (geo->nDetector[k] <= 0 || !(geo->dDetector[k] > 0.0)) return TIGRE_ERR_GEOMETRY;
     if (!(geo->accuracy > 0.0)) return TIGRE_ERR_GEOMETRY;
+    if (geo->mode != TIGRE_GEO_CONE && geo->mode != TIGRE_GEO_PARALLEL) return TIGRE_ERR_GEOMETRY;
     for (int a = 0; a < nA; ++a) {
         double dsd = geo->DSD_a ? geo->DSD_a[a] : geo->DSD;
         double dso = geo->DSO_a ? geo->DSO_a[a] : geo->DSO;
@@ -99,11 +101,19 @@ void build_ray_view(const Grid& g, const ViewH& v, RayView& r) {
     apply(Rg, p1, P);
     apply(Rg, ru, dU);
     apply(Rg, rv, dV);
+    if (v.parallel) {   // P29: the ray of a pixel starts DSD in front of it along the gantry-rotated x axis
+        const double e1[3] = {v.DSD, 0.0, 0.0};
+        double e[3];
+        apply(Rg, e1, e);
+        for (int k = 0; k < 3; ++k) S[k] = P[k] + e[k];
+    }
     for (int k = 0; k < 3; ++k) {
         r.S[k] = (S[k] - vmin[k]) / h[k];
         r.P0[k] = (P[k] - vmin[k]) / h[k];
         r.dU[k] = dU[k] / h[k];
         r.dV[k] = dV[k] / h[k];
+        r.dSU[k] = v.parallel ? r.dU[k] : 0.0;
+        r.dSV[k] = v.parallel ? r.dV[k] : 0.0;
     }
 }
 
@@ -128,8 +138,26 @@ static int build_vox_rows(const Grid& g, const ViewH& v, VoxRows& R) {
     double b0[3] = {v.DSO - Dc[0], -Dc[1], -Dc[2]};
     double* s = R.s;
     apply(RdT, b0, s);
-    if (!(s[0] > 0.0)) return TIGRE_ERR_GEOMETRY;
     double *rowW = R.rowW, *rowU = R.rowU, *rowV = R.rowV, *rowG = R.rowG;
+    if (v.parallel) {
+        // P29: slide the voxel along the ray direction e = R_det^T e_x onto the detector plane q_x = 0: an affine map (W = 1)
+        const double ex[3] = {1.0, 0.0, 0.0};
+        double e[3];
+        apply(RdT, ex, e);
+        if (!(std::fabs(e[0]) > 1e-9)) return TIGRE_ERR_GEOMETRY;
+        const double oU = 0.5 * (g.nu - 1) - (double)(g.nu / 2), oV = 0.5 * (g.nv - 1) - (double)(g.nv / 2);
+        for (int k = 0; k < 3; ++k) {
+            rowW[k] = 0.0, rowG[k] = 0.0;
+            rowU[k] = (M.m[1][k] - e[1] / e[0] * M.m[0][k]) / g.du;
+            rowV[k] = (M.m[2][k] - e[2] / e[0] * M.m[0][k]) / g.dv;
+        }
+        rowW[3] = 1.0, rowG[3] = 1.0;
+        rowU[3] = (q0[1] - e[1] / e[0] * q0[0]) / g.du + oU;
+        rowV[3] = (q0[2] - e[2] / e[0] * q0[0]) / g.dv + oV;
+        s[0] = std::fabs(e[0]), s[1] = 0.0, s[2] = 0.0;   // s[0] carries the cosine between ray and detector normal
+        return TIGRE_OK;
+    }
+    if (!(s[0] > 0.0)) return TIGRE_ERR_GEOMETRY;
     for (int k = 0; k < 3; ++k) rowW[k] = -M.m[0][k] / s[0];
     rowW[3] = 1.0 - q0[0] / s[0];
     // u*W = s_y*W + (q_y - s_y);  fu = u/du + (nu-1)/2;  fuh = fu - nu/2 = u/du + offU
@@ -184,6 +212,14 @@ int build_vox_view(const Grid& g, const ViewH& v, VoxView& o) {
         o.rowV[k] = (float)rowV[k];
         o.rowW[k] = (float)rowW[k];
         o.rowG[k] = (float)rowG[k];
+    }
+    if (v.parallel) {
+        // constant matched weight dVoxel^3 / (du dv cos) through the SAME kernel arithmetic  km t^2 sqrt(sx2 + du^2 eu^2 +
+        // dv^2 ev^2)  (t = 1): sx2 = 2^100 absorbs the other terms exactly in fp32, sqrt(2^100) = 2^50
+        o.km = (float)((g.dx * g.dy * g.dz) / (g.du * g.dv) / s[0] / 1125899906842624.0);
+        o.sx2 = 1.2676506002282294e30f;
+        o.fus = 0.f, o.fvs = 0.f;
+        return TIGRE_OK;
     }
     o.km = (float)((g.dx * g.dy * g.dz) / (g.du * g.dv) / s[0]);
     o.sx2 = (float)(s[0] * s[0]);
