@@ -210,6 +210,14 @@ TIGRE_API int tigre_fdk_filter_ex(const float *b, const tigre_geo *geo, const do
                         float *q, void *cuda_stream);
 TIGRE_API int tigre_fdk_weights(const tigre_geo *geo, const double *angles, int nA, int weighting, double *w);
 
+/* Curved detectors ("TIGRE now allows to consider curved detectors by applying a 'flattening' transformation";
+ * DESIGN.md reading P30): curved (dev [nA][nv][nu]) was measured on the cylinder of radius DSD about the axis through the
+ * source parallel to v, pixel pitch du along the arc and dv in height; flat (dev, same shape, must not alias) receives the
+ * image a flat detector of the same pixel counts and pitches would have seen: flat(u, v) = curved(arc length DSD atan(u/DSD),
+ * height v cos(atan(u/DSD))), bilinear, zero outside.  Per-view DSD honoured. */
+TIGRE_API int tigre_flatten_detector(const float *curved, const tigre_geo *geo, const double *angles, int nA, float *flat,
+                           void *cuda_stream);
+
 /* ---- total variation (section 2.2.3 eqs. 7-8; P20-P22) ----------
  * AwTV(x) = sum_p sqrt(w_x dx^2 + w_y dy^2 + w_z dz^2 + eps), backward differences d_a = x[p] - x[p - e_a], weights
  * w_a = exp(-(d_a/delta)^2), over the voxels that have all their backward neighbours (an axis of length 1 drops

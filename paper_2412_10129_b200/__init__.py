@@ -49,7 +49,7 @@ class TigreError(RuntimeError):
 
 _LIB = None
 EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_Ax_slab", "tigre_Atb_slab", "tigre_slab_row_band", "tigre_row_weights", "tigre_col_weights", "tigre_residual",
-           "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_fdk", "tigre_fdk_filter", "tigre_fdk_ex", "tigre_fdk_filter_ex", "tigre_fdk_weights",
+           "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_fdk", "tigre_fdk_filter", "tigre_fdk_ex", "tigre_fdk_filter_ex", "tigre_fdk_weights", "tigre_flatten_detector",
            "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_create_ex", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version"]
@@ -363,6 +363,16 @@ def fdk_filter_ex(b, geo, angles, filt="ram_lak", weighting=None):
     _check(_lib().tigre_fdk_filter_ex(_f32(b, proj_shape(geo, nA), "b"), G.ref, a.ctypes.data_as(_dp), nA, _FILTERS[filt],
                                       _WEIGHTINGS[weighting], _f32(q), _stream(b)), "tigre_fdk_filter_ex")
     return q
+
+
+def flatten_detector(curved, geo, angles):
+    """Projections measured on a curved (cylindrical, radius DSD) detector resampled onto the flat detector of geo."""
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    flat = _new(proj_shape(geo, nA), like=curved)
+    _check(_lib().tigre_flatten_detector(_f32(curved, proj_shape(geo, nA), "curved"), G.ref, a.ctypes.data_as(_dp), nA,
+                                         _f32(flat), _stream(curved)), "tigre_flatten_detector")
+    return flat
 
 
 def fdk_weights(geo, angles, weighting):

@@ -773,6 +773,18 @@ int tigre_fdk_ex(const float* b, const tigre_geo* geo, const double* angles, int
     if (weighting == TIGRE_FDK_PARKER) scale = std::fabs(t.views[nA - 1].ang[0] - t.views[0].ang[0]) / (double)(nA - 1);
     return launch_scale(x, (float)scale, (size_t)g.nx * g.ny * g.nz, st);
 }
+int tigre_flatten_detector(const float* curved, const tigre_geo* geo, const double* angles, int nA, float* flat, void* cuda_stream) {
+    if (!curved || !flat || curved == flat) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    if (mem_kind(curved) != MEM_DEVICE || mem_kind(flat) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    std::vector<double> dd(nA);
+    for (int a = 0; a < nA; ++a) dd[a] = t.views[a].DSD;
+    TempBuf tb;
+    TG_TRY(upload(tb, dd.data(), sizeof(double) * dd.size(), st));
+    return launch_flatten(curved, t.g, tb.as<double>(), nA, flat, st);
+}
 int tigre_fdk_weights(const tigre_geo* geo, const double* angles, int nA, int weighting, double* w) {
     if (!w) return TIGRE_ERR_ARG;
     TG_TRY(validate_geo(geo, angles, nA));      // host arithmetic only: no device needed

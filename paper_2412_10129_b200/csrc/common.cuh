@@ -144,6 +144,7 @@ void fdk_filter_taps(int nu, int filter, std::vector<double>& g);
 int fdk_weights(const Grid& g, const std::vector<ViewH>& views, int weighting, std::vector<double>& w);
 int launch_fdk_filter_taps(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, int nViews, const float* d_taps,
                            const float* d_colw, float* q, cudaStream_t st);
+int launch_flatten(const float* curved, const Grid& g, const double* d_dsd, int nViews, float* flat, cudaStream_t st);
 int launch_count_reduce(const uint32_t* c, size_t n, unsigned long long* d_total, cudaStream_t st);
 
 // TV / AwTV (tv.cu): value and/or gradient in one pass (g, d_val, d_gg may be NULL; accumulators pre-zeroed);

@@ -7,6 +7,7 @@
 // equals the FFT formulation exactly (L >= 2 nu: no wrap) and keeps the kernel free of an FFT dependency.
 // Weights: Parker (short scan) and Wang (displaced detector) are per-view, per-column factors built on the host in
 // fp64 and multiplied into the cosine-weighted row before the convolution.
+#include <algorithm>
 #include <cmath>
 #include <vector>
 #include "common.cuh"
@@ -42,6 +43,38 @@ fdk_filter_taps_kernel(const float* __restrict__ b, int nu, int nv, float du, fl
         for (int n = 1; n <= iu; ++n) s0 = fmaf(row[iu - n], tap[n], s0);
         for (int n = 1; n < nu - iu; ++n) s1 = fmaf(row[iu + n], tap[n], s1);
         q[base + iu] = (s0 + s1) * itau;
+    }
+}
+
+// curved -> flat detector (reading P30): flat pixel (u, v) reads the curved image at arc length DSD atan(u/DSD) and height
+// v cos(atan(u/DSD)), bilinear, zero outside.  One thread per flat pixel; per-column quantities are recomputed (cheap).
+__global__ void __launch_bounds__(256)
+flatten_kernel(const float* __restrict__ curved, int nu, int nv, float du, float dv, const double* __restrict__ dsd_a,
+               float* __restrict__ flat, size_t total) {
+    const size_t per = (size_t)nu * nv;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t ia = i / per;
+        const int r = (int)(i - ia * per), iv = r / nu, iu = r - iv * nu;
+        const float DSD = (float)dsd_a[ia];
+        const float u = ((float)iu + 0.5f) * du - 0.5f * (float)nu * du;
+        const float v = ((float)iv + 0.5f) * dv - 0.5f * (float)nv * dv;
+        const float gamma = atanf(u / DSD);
+        const float fi = (DSD * gamma + 0.5f * (float)nu * du) / du - 0.5f;
+        const float fj = (v * cosf(gamma) + 0.5f * (float)nv * dv) / dv - 0.5f;
+        const float fli = floorf(fi), flj = floorf(fj);
+        const int i0 = (int)fli, j0 = (int)flj;
+        const float ai = fi - fli, aj = fj - flj;
+        const float* src = curved + ia * per;
+        float acc = 0.f;
+#pragma unroll
+        for (int cj = 0; cj < 2; ++cj)
+#pragma unroll
+            for (int ci = 0; ci < 2; ++ci) {
+                const int ii = i0 + ci, jj = j0 + cj;
+                if ((unsigned)ii < (unsigned)nu && (unsigned)jj < (unsigned)nv)
+                    acc = fmaf((ci ? ai : 1.f - ai) * (cj ? aj : 1.f - aj), __ldg(src + (size_t)jj * nu + ii), acc);
+            }
+        flat[i] = acc;
     }
 }
 
@@ -131,6 +164,16 @@ int fdk_weights(const Grid& g, const std::vector<ViewH>& views, int weighting, s
         return TIGRE_OK;
     }
     return TIGRE_ERR_ARG;
+}
+
+int launch_flatten(const float* curved, const Grid& g, const double* d_dsd, int nViews, float* flat, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
+    const size_t total = (size_t)g.nu * g.nv * nViews;
+    if (total == 0) return TIGRE_OK;
+    const int blocks = (int)std::min<size_t>((total + 255) / 256, (size_t)148 * 16);
+    flatten_kernel<<<blocks, 256, 0, st>>>(curved, g.nu, g.nv, (float)g.du, (float)g.dv, d_dsd, flat, total);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
 }
 
 int launch_fdk_filter_taps(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, int nViews, const float* d_taps,

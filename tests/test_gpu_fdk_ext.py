@@ -130,3 +130,21 @@ def test_redundancy_weighting_inside_ossart_matches_oracle(tg):
     assert np.allclose(res, rres, rtol=1e-4)
     plain, _ = orc.ossart(b, geo, ang, subsets, 3)
     assert H.rel_l2(host(x), plain) > 1e-3                             # and it is not the unweighted iteration
+
+
+def test_curved_detector_flattening_matches_oracle(tg):
+    from oracle import curved as ocurved
+    geo = Geometry(nVoxel=(8, 8, 8), dVoxel=(1.0,) * 3, nDetector=(157, 93), dDetector=(1.3, 1.7), DSD=420.0, DSO=300.0)
+    geo.DSD_a = np.array([420.0, 380.0, 505.0])
+    ang = np.stack([np.array([0.0, 1.0, 2.0]), np.zeros(3), np.zeros(3)], 1)
+    img = np.random.default_rng(5).random((3, 93, 157)).astype(np.float32)
+    ref = ocurved.flatten(img, geo)
+    got = host(tg.flatten_detector(dev(img), geo, ang))
+    # fp32 coordinates: a tap index can differ where the continuous index sits on an integer; compare in rel-L2
+    assert H.rel_l2(got, ref) <= 1e-4
+    # C4's detector size, one view: sampled pixels
+    big = Geometry(nVoxel=(8, 8, 8), dVoxel=(1.0,) * 3, nDetector=(1536, 1536), dDetector=(0.2, 0.2), DSD=1536.0, DSO=1000.0)
+    gen = torch.Generator(device="cuda").manual_seed(6)
+    b = torch.rand((2, 1536, 1536), generator=gen, device="cuda")
+    refb = ocurved.flatten(b.cpu().numpy(), big)
+    assert H.rel_l2(host(tg.flatten_detector(b, big, ang[:2])), refb) <= 1e-4
