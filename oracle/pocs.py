@@ -75,3 +75,30 @@ def asd_pocs(b, geo, angles, subsets, n_iter, beta=1.0, beta_red=0.99, ng=20, al
         if (c < -0.99 and dd <= epsilon) or beta < 0.005:
             break
     return x, np.array(hist, dtype=np.float64).reshape(-1, 5)
+
+
+def sart_tv(b, geo, angles, subsets, n_iter, lam=1.0, lam_red=1.0, tv_lambda=0.0, tv_iter=10, ax_mode=orc.SIDDON,
+            atb_mode=orc.MATCHED, x0=None):
+    """SART-TV ("TIGRE also includes the SART-TV algorithm [44] ... can also be interpreted as a proximal
+    method", used at PAPER.md:365): reading P31: per iteration one OS-SART sweep with relaxation lam (single-view subsets:
+    SART), then the TV proximal operator of oracle/prox.py (P24) with weight tv_lambda and tv_iter dual iterations;
+    lam <- lam * lam_red.  Returns (x, resid) with resid[it] the running residual of the sweep (as oracle.ossart)."""
+    from . import prox as oprox
+    angles = np.asarray(angles, dtype=np.float64).reshape(-1, 3)
+    b = np.asarray(b, dtype=np.float64)
+    x = np.zeros(geo.vol_shape) if x0 is None else np.array(x0, dtype=np.float64)
+    subsets = [np.asarray(s, dtype=np.int64) for s in subsets]
+    Ws = [orc.row_weights(orc._sub_geo(geo, s), angles[s], ax_mode) for s in subsets]
+    Vs = [orc.col_weights(orc._sub_geo(geo, s), angles[s], atb_mode) for s in subsets]
+    resid = np.zeros(n_iter)
+    for it in range(n_iter):
+        acc = 0.0
+        for s, W, V in zip(subsets, Ws, Vs):
+            gs = orc._sub_geo(geo, s)
+            d = b[s] - orc.ax(x, gs, angles[s], ax_mode)
+            acc += float(np.sum(d * d))
+            x = np.maximum(x + lam * V * orc.atb(W * d, gs, angles[s], atb_mode), 0.0)
+        resid[it] = np.sqrt(acc)
+        x = oprox.tv_prox(x, tv_lambda, tv_iter)
+        lam *= lam_red
+    return x, resid

@@ -78,3 +78,24 @@ def test_lowers_tv_relative_to_ossart_and_keeps_the_fit(case):
     ref, _ = orc.ossart(b, geo, ang, subsets, 6)
     assert otv.awtv(x) < 0.9 * otv.awtv(ref)
     assert hist[-1, 0] < 1.5 * np.linalg.norm(orc.ax(ref, geo, ang, orc.SIDDON) - b)
+
+
+def test_sart_tv_reductions(case):
+    # SART-TV (reading P31): with tv_lambda = 0 it IS OS-SART (bitwise); one iteration is the hand-written composition
+    # "sweep, then TV prox"; the prox lowers the TV of the iterate
+    from oracle import prox as oprox
+    geo, ang, b, subsets = case
+    x, r = pocs.sart_tv(b, geo, ang, subsets, 3, lam=0.9, tv_lambda=0.0)
+    ref, rr = orc.ossart(b, geo, ang, subsets, 3, lam=0.9)
+    assert np.array_equal(x, ref) and np.array_equal(r, rr)
+    x1, _ = pocs.sart_tv(b, geo, ang, subsets, 1, tv_lambda=2e-3, tv_iter=15)
+    s1, _ = orc.ossart(b, geo, ang, subsets, 1)
+    assert np.allclose(x1, oprox.tv_prox(s1, 2e-3, 15), atol=1e-15)
+    x4, _ = pocs.sart_tv(b, geo, ang, subsets, 4, tv_lambda=2e-3, tv_iter=15)
+    s4, _ = orc.ossart(b, geo, ang, subsets, 4)
+    assert oprox.tv_forward(x4) < 0.9 * oprox.tv_forward(s4)
+    # relaxation reduction: the second sweep runs with lam * lam_red
+    xa, _ = pocs.sart_tv(b, geo, ang, subsets, 2, lam=1.0, lam_red=0.5, tv_lambda=0.0)
+    first, _ = orc.ossart(b, geo, ang, subsets, 1, lam=1.0)
+    second, _ = orc.ossart(b, geo, ang, subsets, 1, lam=0.5, x0=first)
+    assert np.array_equal(xa, second)
