@@ -246,6 +246,12 @@ TIGRE_API int tigre_tv_prox(const float *f, int nx, int ny, int nz, float lambda
 TIGRE_API int tigre_fista(const float *b, const tigre_geo *geo, const double *angles, int nA, int n_iter, float L, float tv_lambda,
                 int tv_iter, float tau, int ax_mode, int atb_mode, float *x_inout, double *resid_hist, void *cuda_stream);
 
+/* SART-TV ("TIGRE also includes the SART-TV algorithm [44]", used at 365; reading P31): per iteration the
+ * plan's OS-SART sweep with relaxation lambda (nonnegativity on; single-view subsets = SART), then x <- tigre_tv_prox(x, tv_lambda,
+ * tv_iter, tau); lambda *= lambda_red.  b, x_inout dev; resid_hist (host, may be NULL) [n_iter] as tigre_plan_ossart. */
+TIGRE_API int tigre_plan_sart_tv(tigre_plan *plan, const float *b, float *x_inout, int n_iter, float lambda, float lambda_red,
+                       float tv_lambda, int tv_iter, float tau, double *resid_hist, void *cuda_stream);
+
 /* ---- measurement helpers -------------------------------------------------------------------
  * Exact count of ray-samples of one tigre_Ax call without marching the data (BASELINE metric:
  * Siddon = non-zero voxel segments; interpolated = samples K inside the grown box).

@@ -861,6 +861,25 @@ static int tv_prox_impl(const float* f, int nx, int ny, int nz, float lam, int n
     return launch_prox_div(px, py, pz, f, lam, true, u, nx, ny, nz, st);
 }
 
+// SART-TV (reading P31; oracle/pocs.py sart_tv): per iteration the plan's OS-SART sweep with relaxation lambda, then the TV prox
+int tigre_plan_sart_tv(tigre_plan* P, const float* b, float* x, int n_iter, float lambda, float lambda_red, float tv_lambda,
+                       int tv_iter, float tau, double* resid_hist, void* cuda_stream) {
+    if (!P || !b || !x || n_iter < 0 || tv_iter < 0 || !(tv_lambda >= 0.f) || !(tau > 0.f)) return TIGRE_ERR_ARG;
+    if (mem_kind(b) != MEM_DEVICE || mem_kind(x) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const Grid& g = P->t.g;
+    const size_t nvox = (size_t)g.nx * g.ny * g.nz;
+    TempBuf p3, dd;
+    TG_TRY(p3.alloc(sizeof(float) * 3 * nvox, st));
+    TG_TRY(dd.alloc(sizeof(float) * nvox, st));
+    for (int it = 0; it < n_iter; ++it) {
+        TG_TRY(tigre_plan_ossart(P, b, x, 1, lambda, 1, resid_hist ? resid_hist + it : nullptr, cuda_stream));
+        TG_TRY(tv_prox_impl(x, g.nx, g.ny, g.nz, tv_lambda, tv_iter, tau, x, p3.as<float>(), dd.as<float>(), st));
+        lambda *= lambda_red;
+    }
+    return TIGRE_OK;
+}
+
 int tigre_tv_prox(const float* f, int nx, int ny, int nz, float lambda, int n_iter, float tau, float* u, void* cuda_stream) {
     if (!f || !u || nx <= 0 || ny <= 0 || nz <= 0 || n_iter < 0 || !(lambda >= 0.f) || !(tau > 0.f)) return TIGRE_ERR_ARG;
     TG_TRY(ensure_device());

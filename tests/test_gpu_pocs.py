@@ -121,6 +121,23 @@ def test_larger_problem_composition_and_tv_drop(tg):
     plan.close()
 
 
+def test_sart_tv_matches_oracle(tg):
+    geo, ang, b = noisy_case(2, 24, 9)
+    subsets = [list(range(s, 24, 4)) for s in range(4)]
+    ref, rref = opocs.sart_tv(b, geo, ang, subsets, 3, lam=1.0, lam_red=0.9, tv_lambda=1e-3, tv_iter=12)
+    plan = tg.OssartPlan(geo, ang, subsets, "siddon", "matched")
+    x = torch.zeros(geo.vol_shape, dtype=torch.float32, device="cuda")
+    res = plan.sart_tv(dev(b), x, 3, lam=1.0, lam_red=0.9, tv_lambda=1e-3, tv_iter=12)
+    assert H.rel_l2(host(x), ref) <= 1e-4
+    assert np.allclose(res, rref, rtol=1e-4)
+    y = torch.zeros_like(x)
+    plan.sart_tv(dev(b), y, 2, lam=0.8, tv_lambda=0.0)                 # no regularisation: the plain sweeps
+    z = torch.zeros_like(x)
+    plan.iterate(dev(b), z, 2, lam=0.8)
+    assert torch.equal(y, z)
+    plan.close()
+
+
 def test_argument_errors(tg):
     geo, ang, b = noisy_case(4, 4, 8)
     plan = tg.OssartPlan(geo, ang, [[0, 1], [2, 3]], "siddon", "matched")
