@@ -16,6 +16,9 @@
 #include <cmath>
 #include "common.cuh"
 
+#ifndef AXMB
+#define AXMB 9
+#endif
 namespace tg {
 
 struct AxP {
@@ -131,7 +134,7 @@ __device__ __forceinline__ void siddon_slab_checked(const float* __restrict__ ba
 }
 
 template <typename IdxT, bool UNIT, bool COUNT, bool SCATTER>
-__global__ void __launch_bounds__(AX_TU* AX_TV, 8)
+__global__ void __launch_bounds__(AX_TU* AX_TV, AXMB)
 ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, const RayView* __restrict__ views,
                  int nViews, AxP p, float* __restrict__ proj, uint32_t* __restrict__ counts) {
     int view, iu, iv;
