@@ -16,6 +16,9 @@
 #include <cmath>
 #include "common.cuh"
 
+#ifndef AXIMB
+#define AXIMB 8
+#endif
 #ifndef AXMB
 #define AXMB 9
 #endif
@@ -305,7 +308,7 @@ struct InterpRay {
 };
 
 template <typename IdxT, bool UNIT, bool COUNT, bool SCATTER>
-__global__ void __launch_bounds__(AX_TU* AX_TV)
+__global__ void __launch_bounds__(AX_TU* AX_TV, AXIMB)
 ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, const RayView* __restrict__ views, int nViews,
                  AxP p, float* __restrict__ proj, uint32_t* __restrict__ counts) {
     int view, iu, iv;
