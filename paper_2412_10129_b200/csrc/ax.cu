@@ -35,7 +35,10 @@ struct AxP {
     int accumulate;
 };
 
-constexpr int AX_TU = 32, AX_TV = 4;
+#ifndef AXTV
+#define AXTV 4
+#endif
+constexpr int AX_TU = 32, AX_TV = AXTV;
 
 __device__ __forceinline__ double sel3(int k, double a, double b, double c) { return k == 0 ? a : (k == 1 ? b : c); }
 
