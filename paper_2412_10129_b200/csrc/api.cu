@@ -700,7 +700,8 @@ static int fdk_filter_impl(const float* b, Tables& t, int nA, float* q, cudaStre
     if (t.views[0].parallel) std::fill(dd.begin(), dd.end(), 1e15);
     TempBuf tb;
     TG_TRY(upload(tb, dd.data(), sizeof(double) * dd.size(), st));
-    return launch_fdk_filter(b, t.g, tb.as<double>(), tb.as<double>() + nA, nA, q, st);
+    // Ram-Lak, no weights: taps formed in the kernel, odd taps only (fdk.cu)
+    return launch_fdk_filter_taps(b, t.g, tb.as<double>(), tb.as<double>() + nA, nA, nullptr, nullptr, q, st, true);
 }
 int tigre_fdk_filter(const float* b, const tigre_geo* geo, const double* angles, int nA, float* q, void* cuda_stream) {
     if (!b || !q) return TIGRE_ERR_ARG;
@@ -747,7 +748,7 @@ static int fdk_filter_ex_impl(const float* b, Tables& t, int nA, int filter, int
         TG_TRY(upload(tw, fw.data(), sizeof(float) * fw.size(), st));
     }
     return launch_fdk_filter_taps(b, t.g, tb.as<double>(), tb.as<double>() + nA, nA, tt.as<float>(),
-                                  weighting != TIGRE_FDK_FULL ? tw.as<float>() : nullptr, q, st);
+                                  weighting != TIGRE_FDK_FULL ? tw.as<float>() : nullptr, q, st, filter == TIGRE_FILTER_RAM_LAK);
 }
 int tigre_fdk_filter_ex(const float* b, const tigre_geo* geo, const double* angles, int nA, int filter, int weighting, float* q,
                         void* cuda_stream) {

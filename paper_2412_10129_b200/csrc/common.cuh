@@ -138,12 +138,10 @@ int launch_xpby(float* p, const float* s, const double* d_num, const double* d_d
 int launch_scale(float* x, float a, size_t n, cudaStream_t st);
 int launch_scale_columns(float* W, const float* colw, int nViews, int nv, int nu, cudaStream_t st);
 int launch_diff_stats(const float* a, const float* b, const float* c, size_t n, double* d_out3, cudaStream_t st);
-int launch_fdk_filter(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, int nViews,
-                      float* q, cudaStream_t st);
 void fdk_filter_taps(int nu, int filter, std::vector<double>& g);
 int fdk_weights(const Grid& g, const std::vector<ViewH>& views, int weighting, std::vector<double>& w);
 int launch_fdk_filter_taps(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, int nViews, const float* d_taps,
-                           const float* d_colw, float* q, cudaStream_t st);
+                           const float* d_colw, float* q, cudaStream_t st, bool odd_only = false);
 int launch_flatten(const float* curved, const Grid& g, const double* d_dsd, int nViews, float* flat, cudaStream_t st);
 int launch_count_reduce(const uint32_t* c, size_t n, unsigned long long* d_total, cudaStream_t st);
 

@@ -1,6 +1,6 @@
 // elementwise.cu — the HBM-bound half of the Kaczmarz family (eq. 6 at 135):
 // residual r = W.*(b - Ax), update x = max(0, x + lambda V.*g), weight inversion, the CGLS
-// vector recurrences and the FDK pre-filter (DESIGN.md O-D).
+// vector recurrences.  (The FDK pre-filter lives in fdk.cu.)
 // Grid-stride kernels, float4 where alignment allows, grids sized as a multiple of the SM count.
 // Reductions: fp32 products accumulated in fp64 per thread, block tree, one fp64 atomic per block.
 #include <cmath>
@@ -262,54 +262,6 @@ int launch_count_reduce(const uint32_t* c, size_t n, unsigned long long* d_total
     TG_CUDA(cudaMemsetAsync(d_total, 0, sizeof(unsigned long long), st));
     if (n == 0) return TIGRE_OK;
     count_reduce_kernel<<<ew_blocks(n), 256, 0, st>>>(c, n, d_total);
-    TG_CUDA(cudaGetLastError());
-    return TIGRE_OK;
-}
-
-// ---------------------------------------------------------------- FDK pre-filter (reading P12)
-// One CTA per detector row: the cosine-weighted row is staged in shared memory, then each thread
-// forms q[iu] = tau * ( row[iu] h[0] + sum_{odd n} row[iu-n] h[n] ),  h[0] = 1/(4 tau^2),
-// h[n] = -1/(pi n tau)^2 (n odd), tau = du*DSO/DSD: a direct linear convolution with zero padding
-// (no FFT, so no circular wrap).  The tap table 1/n^2 is built once per CTA in shared memory.
-__global__ void __launch_bounds__(256)
-fdk_filter_kernel(const float* __restrict__ b, int nu, int nv, float du, float dv, const double* __restrict__ dsd_a,
-                  const double* __restrict__ dso_a, float* __restrict__ q) {
-    extern __shared__ float sm[];
-    float* row = sm;            // [nu]
-    float* tap = sm + nu;       // [nu]  tap[n] = 1/n^2 for odd n, 0 for even n
-    const int iv = blockIdx.x, ia = blockIdx.y;
-    const float DSD = (float)dsd_a[ia], DSO = (float)dso_a[ia];
-    const float tau = du * DSO / DSD;
-    const float v = ((float)iv + 0.5f) * dv - 0.5f * (float)nv * dv;
-    const size_t base = ((size_t)ia * nv + iv) * nu;
-    for (int iu = threadIdx.x; iu < nu; iu += blockDim.x) {
-        const float u = ((float)iu + 0.5f) * du - 0.5f * (float)nu * du;
-        row[iu] = __ldg(b + base + iu) * DSD * rsqrtf(DSD * DSD + u * u + v * v);
-        tap[iu] = (iu & 1) ? 1.0f / ((float)iu * (float)iu) : 0.f;
-    }
-    __syncthreads();
-    const float c0 = 1.0f / (4.0f * tau), c1 = -1.0f / (9.8696044010893586f * tau);   // tau*h[0], tau*h[n]*n^2
-    for (int iu = threadIdx.x; iu < nu; iu += blockDim.x) {
-        float s = 0.f;
-        // odd offsets only: n = 1,3,5,... on both sides
-        for (int n = 1; n < nu; n += 2) {
-            const int l = iu - n, r = iu + n;
-            float t = 0.f;
-            if (l >= 0) t += row[l];
-            if (r < nu) t += row[r];
-            s = fmaf(t, tap[n], s);
-        }
-        q[base + iu] = fmaf(c1, s, c0 * row[iu]);
-    }
-}
-int launch_fdk_filter(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, int nViews,
-                      float* q, cudaStream_t st) {
-    ProfScope ps(PK_EW, st);
-    const size_t smem = 2 * (size_t)g.nu * sizeof(float);
-    if (smem > 200 * 1024) return TIGRE_ERR_ARG;
-    if (smem > 48 * 1024) TG_CUDA(cudaFuncSetAttribute(fdk_filter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    dim3 grid(g.nv, nViews);
-    fdk_filter_kernel<<<grid, 256, smem, st>>>(b, g.nu, g.nv, (float)g.du, (float)g.dv, d_dsd, d_dso, q);
     TG_CUDA(cudaGetLastError());
     return TIGRE_OK;
 }

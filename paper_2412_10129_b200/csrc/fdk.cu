@@ -1,4 +1,4 @@
-// fdk.cu — FDK variants ("various filter types and geometric correction methods,
+// fdk.cu — the FDK pre-filter (reading P12) and the FDK variants (section 8(f).4; "various filter types and geometric correction methods,
 // such as Wang [25] and Parker [26] weights", 281, 359; readings P26-P28).
 //
 // Filters: the Ram-Lak taps (P12) windowed in frequency on L = 2^ceil(log2(2 nu)) samples.  The product of the taps'
@@ -16,33 +16,86 @@ namespace tg {
 
 namespace {
 
-// q[iu] = (1/tau) * sum_n row[iu - n] * taps[|n|],  row = b * cosine weight * colw
-__global__ void __launch_bounds__(256)
-fdk_filter_taps_kernel(const float* __restrict__ b, int nu, int nv, float du, float dv, const double* __restrict__ dsd_a,
-                       const double* __restrict__ dso_a, const float* __restrict__ taps, const float* __restrict__ colw,
-                       float* __restrict__ q) {
-    extern __shared__ float sm[];
-    float* row = sm;            // [nu]
-    float* tap = sm + nu;       // [nu]
+// q[iu] = (1/tau) * sum_m row[m] * taps[|iu - m|],  row = b * cosine weight * colw: one CTA per detector row and view.
+// The convolution is a dense contraction of nu^2 multiply-adds per row (C3: 2.9e11 per FDK), so it is laid out for the FMA
+// pipe: a thread owns FR = 8 consecutive outputs and slides a register window of 8 row values past them, one new value per
+// tap index n on each side, so a tap costs ONE broadcast shared-memory load (two LDS.128 per 8 taps) plus one row load per
+// side for 16 FMAs.  The row sits in shared memory split into FR planes by (index mod FR), zero-padded on both sides: the
+// threads of a warp (consecutive groups of outputs) then read consecutive words of one plane (no bank conflicts) and the
+// row's ends need no tests.  ODD = true: Ram-Lak without a window (taps vanish at even n != 0): even n only shift the window.
+// taps == NULL: the Ram-Lak taps of reading P12 are formed in the kernel.
+constexpr int FR = 8;
+
+template <bool ODD>
+__global__ void __launch_bounds__(128)
+fdk_conv_kernel(const float* __restrict__ b, int nu, int nv, float du, float dv, const double* __restrict__ dsd_a,
+                const double* __restrict__ dso_a, const float* __restrict__ taps, const float* __restrict__ colw,
+                float* __restrict__ q, int PAD, int PL, int NT) {
+    extern __shared__ __align__(16) float sm[];
+    float* tp = sm;              // [NT]  taps, tp[0] = 0 (the centre tap is applied separately), zero beyond nu
+    float* rw = sm + NT;         // [FR][PL]  row value i at plane (i mod FR), offset (i + PAD) / FR
     const int iv = blockIdx.x, ia = blockIdx.y;
     const float DSD = (float)dsd_a[ia], DSO = (float)dso_a[ia];
     const float itau = DSD / (du * DSO);
     const float v = ((float)iv + 0.5f) * dv - 0.5f * (float)nv * dv;
     const size_t base = ((size_t)ia * nv + iv) * nu;
+    for (int i = threadIdx.x; i < FR * PL; i += blockDim.x) rw[i] = 0.f;
+    for (int n = threadIdx.x; n < NT; n += blockDim.x) {
+        float t = 0.f;
+        if (n >= 1 && n < nu) t = taps ? __ldg(taps + n) : ((n & 1) ? -1.0f / (9.8696044010893586f * (float)n * (float)n) : 0.f);
+        tp[n] = t;
+    }
+    const float tap0 = taps ? __ldg(taps) : 0.25f;
+    __syncthreads();
     for (int iu = threadIdx.x; iu < nu; iu += blockDim.x) {
         const float u = ((float)iu + 0.5f) * du - 0.5f * (float)nu * du;
         float r = __ldg(b + base + iu) * DSD * rsqrtf(DSD * DSD + u * u + v * v);
         if (colw) r *= __ldg(colw + (size_t)ia * nu + iu);
-        row[iu] = r;
-        tap[iu] = __ldg(taps + iu);
+        rw[(iu % FR) * PL + (iu + PAD) / FR] = r;
     }
     __syncthreads();
-    for (int iu = threadIdx.x; iu < nu; iu += blockDim.x) {
-        float s0 = row[iu] * tap[0], s1 = 0.f;
-        // left side: row[iu - n], n = 1..iu;  right side: row[iu + n], n = 1..nu-1-iu  (two chains for ILP)
-        for (int n = 1; n <= iu; ++n) s0 = fmaf(row[iu - n], tap[n], s0);
-        for (int n = 1; n < nu - iu; ++n) s1 = fmaf(row[iu + n], tap[n], s1);
-        q[base + iu] = (s0 + s1) * itau;
+    for (int c = threadIdx.x; c * FR < nu; c += blockDim.x) {
+        const int i0 = c * FR, ob = (i0 + PAD) / FR;
+        float acc[FR], L[FR], R[FR];
+#pragma unroll
+        for (int j = 0; j < FR; ++j) {
+            L[j] = rw[j * PL + ob];          // window at n = 0: row[i0 + j]
+            R[j] = L[j];
+            acc[j] = tap0 * L[j];
+        }
+        // left side: row[i0 + j - n]; taps with n > i0 + FR - 1 meet only the zero padding
+        const int mL = (i0 + FR - 1) / FR, mR = (nu - 1 - i0) / FR;
+        for (int m = 0; m <= mL; ++m) {
+            const float4 ta = *reinterpret_cast<const float4*>(tp + FR * m), tb = *reinterpret_cast<const float4*>(tp + FR * m + 4);
+            const float t[FR] = {ta.x, ta.y, ta.z, ta.w, tb.x, tb.y, tb.z, tb.w};
+#pragma unroll
+            for (int k = 0; k < FR; ++k) {   // n = FR * m + k
+                if (!ODD || (k & 1)) {
+#pragma unroll
+                    for (int j = 0; j < FR; ++j) acc[j] = fmaf(t[k], L[j], acc[j]);
+                }
+#pragma unroll
+                for (int j = FR - 1; j > 0; --j) L[j] = L[j - 1];
+                L[0] = rw[((FR - 1 - k) % FR) * PL + ob - m - 1];      // row[i0 - (n + 1)]
+            }
+        }
+        for (int m = 0; m <= mR; ++m) {
+            const float4 ta = *reinterpret_cast<const float4*>(tp + FR * m), tb = *reinterpret_cast<const float4*>(tp + FR * m + 4);
+            const float t[FR] = {ta.x, ta.y, ta.z, ta.w, tb.x, tb.y, tb.z, tb.w};
+#pragma unroll
+            for (int k = 0; k < FR; ++k) {
+                if (!ODD || (k & 1)) {
+#pragma unroll
+                    for (int j = 0; j < FR; ++j) acc[j] = fmaf(t[k], R[j], acc[j]);
+                }
+#pragma unroll
+                for (int j = 0; j < FR - 1; ++j) R[j] = R[j + 1];
+                R[FR - 1] = rw[k * PL + ob + m + 1];                     // row[i0 + FR - 1 + (n + 1)]
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < FR; ++j)
+            if (i0 + j < nu) q[base + i0 + j] = acc[j] * itau;
     }
 }
 
@@ -176,14 +229,21 @@ int launch_flatten(const float* curved, const Grid& g, const double* d_dsd, int 
     return TIGRE_OK;
 }
 
+// d_taps: nu taps for tau = 1 (device) or NULL for the Ram-Lak taps of P12; odd_only: the taps vanish at even n != 0
 int launch_fdk_filter_taps(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, int nViews, const float* d_taps,
-                           const float* d_colw, float* q, cudaStream_t st) {
+                           const float* d_colw, float* q, cudaStream_t st, bool odd_only) {
     ProfScope ps(PK_EW, st);
-    const size_t smem = 2 * (size_t)g.nu * sizeof(float);
+    const int nuC = (g.nu + FR - 1) / FR * FR;
+    const int PAD = nuC + 2 * FR;                   // zero padding on each side (multiple of FR)
+    int PL = (nuC + 2 * PAD) / FR;                  // words per plane
+    PL += (PL % 32 == 1) ? 0 : ((33 - PL % 32) % 32);   // = 1 mod 32: the fill of the planes is then conflict-free as well
+    const int NT = nuC + 2 * FR;                    // taps incl. the overshoot of the last block, multiple of 4
+    const size_t smem = ((size_t)NT + (size_t)FR * PL) * sizeof(float);
     if (smem > 200 * 1024) return TIGRE_ERR_ARG;
-    if (smem > 48 * 1024) TG_CUDA(cudaFuncSetAttribute(fdk_filter_taps_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    auto kern = odd_only ? fdk_conv_kernel<true> : fdk_conv_kernel<false>;
+    if (smem > 48 * 1024) TG_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid(g.nv, nViews);
-    fdk_filter_taps_kernel<<<grid, 256, smem, st>>>(b, g.nu, g.nv, (float)g.du, (float)g.dv, d_dsd, d_dso, d_taps, d_colw, q);
+    kern<<<grid, 128, smem, st>>>(b, g.nu, g.nv, (float)g.du, (float)g.dv, d_dsd, d_dso, d_taps, d_colw, q, PAD, PL, NT);
     TG_CUDA(cudaGetLastError());
     return TIGRE_OK;
 }
