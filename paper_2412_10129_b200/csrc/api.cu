@@ -530,19 +530,27 @@ int tigre_plan_ossart(tigre_plan* P, const float* b, float* x, int n_iter, float
     } else if (kb != MEM_DEVICE || kx != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
     TG_TRY(P->d_acc.alloc(sizeof(double) * std::max(n_iter, 1), st));
     TG_CUDA(cudaMemsetAsync(P->d_acc.p, 0, sizeof(double) * std::max(n_iter, 1), st));
+    // the (x,y)-transposed copy of the iterate that the Ax kernels read for x-dominant rays is kept up to date by the
+    // update kernel (one pass over the volume per subset instead of two)
+    TempBuf xT;
+    float* xTd = nullptr;
+    if (n_iter > 0 && g.nx > 1 && g.ny > 1 && xT.alloc(sizeof(float) * nvox, st) == TIGRE_OK &&
+        launch_transpose_xy(xd, xT.as<float>(), g, st) == TIGRE_OK)
+        xTd = xT.as<float>();
     for (int it = 0; it < n_iter; ++it) {
         for (int s = 0; s < P->nSubsets; ++s) {
             const int n = P->off[s + 1] - P->off[s];
             float* Ws = P->W.as<float>() + per * P->off[s];
             float* Vs = P->V.as<float>() + nvox * s;
             float* A = P->Axb.as<float>();
-            TG_TRY(launch_ax(xd, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st));
+            TG_TRY(launch_ax(xd, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st, nullptr, xTd));
             if (up && it == 0) TG_CUDA(cudaStreamWaitEvent(st, ev[1 + s], 0));   // this subset's projections have arrived
             // r = W_s .* (b_s - A_s x) in place over A; b is gathered through the subset's view list
             TG_TRY(launch_residual(bd, P->d_idx.as<int32_t>() + P->off[s], A, Ws, A, per, n, P->d_acc.as<double>() + it, st));
             TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>(), 0, g.nz, false, 0, g.nv, P->clamp, st,
                               P->hvox[s].data()));
-            TG_TRY(launch_update(xd, P->grad.as<float>(), Vs, lambda, nonneg, nvox, st));
+            if (xTd) TG_TRY(launch_update_t(xd, xTd, P->grad.as<float>(), Vs, lambda, nonneg, g.nx, g.ny, g.nz, st));
+            else TG_TRY(launch_update(xd, P->grad.as<float>(), Vs, lambda, nonneg, nvox, st));
         }
     }
     if (xd != x) TG_CUDA(cudaMemcpyAsync(x, xd, sizeof(float) * nvox, cudaMemcpyDeviceToHost, st));

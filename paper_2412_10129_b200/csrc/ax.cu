@@ -559,7 +559,7 @@ static void ax_dispatch(const float* vol, const float* volT, const RayView* v, i
 }
 
 int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nViews, int mode, bool unit_vol,
-              bool accumulate, float* proj, uint32_t* count_out, cudaStream_t st, const AxSub* sub) {
+              bool accumulate, float* proj, uint32_t* count_out, cudaStream_t st, const AxSub* sub, const float* volT_in) {
     if (mode != TIGRE_AX_SIDDON && mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
     if (sub && (sub->row0 < 0 || sub->row0 + sub->nrows > g.nv || sub->zs0 < 0 || sub->zs0 + sub->nzs > g.nz)) return TIGRE_ERR_ARG;
     if (sub && (sub->nrows <= 0 || sub->nzs <= 0)) return TIGRE_OK;   // nothing of this slab reaches the detector
@@ -582,15 +582,26 @@ int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nView
     // an (x,y)-transposed copy of the volume (of the slab present, in the chunked path) serves the x-dominant rays
     const int nzT = p.zs1 - p.zs0;
     const bool wantT = !unit_vol && !count_out && vol && g.nx > 1 && g.ny > 1;
-    if (wantT && vt.alloc((size_t)g.nx * g.ny * nzT * sizeof(float), st) == TIGRE_OK) volT = vt.as<float>(), launches = 2;
+    if (wantT && volT_in) volT = volT_in;            // the caller keeps a transposed copy up to date (OS-SART plan)
+    else if (wantT && vt.alloc((size_t)g.nx * g.ny * nzT * sizeof(float), st) == TIGRE_OK) volT = vt.as<float>(), launches = 2;
     ProfScope ps(PK_AX, st, launches);
-    if (volT) {
+    if (volT && !volT_in) {
         dim3 tb(32, 8), tg_((g.nx + 31) / 32, (g.ny + 31) / 32, nzT);
         if (tg_.y > 65535 || tg_.z > 65535) volT = nullptr;
         else transpose_xy_kernel<<<tg_, tb, 0, st>>>(vol, vt.as<float>(), g.nx, g.ny);
     }
     if (nvox < (1ull << 31)) ax_dispatch<int>(vol, volT, d_views, nViews, p, mode, unit_vol, proj, count_out, st);
     else ax_dispatch<long long>(vol, volT, d_views, nViews, p, mode, unit_vol, proj, count_out, st);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+
+// the transposed copy alone (for callers that maintain it themselves); returns TIGRE_ERR_ARG if the grid does not fit
+int launch_transpose_xy(const float* vol, float* volT, const Grid& g, cudaStream_t st) {
+    dim3 tb(32, 8), tg_((g.nx + 31) / 32, (g.ny + 31) / 32, g.nz);
+    if (tg_.y > 65535 || tg_.z > 65535) return TIGRE_ERR_ARG;
+    ProfScope ps(PK_AX, st);
+    transpose_xy_kernel<<<tg_, tb, 0, st>>>(vol, volT, g.nx, g.ny);
     TG_CUDA(cudaGetLastError());
     return TIGRE_OK;
 }

@@ -108,7 +108,9 @@ struct AxSub {
     int row0, nrows, zs0, nzs;
 };
 int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nViews, int mode, bool unit_vol,
-              bool accumulate, float* proj, uint32_t* count_out, cudaStream_t st, const AxSub* sub = nullptr);
+              bool accumulate, float* proj, uint32_t* count_out, cudaStream_t st, const AxSub* sub = nullptr,
+              const float* volT_in = nullptr);   // volT_in: an up-to-date (x,y)-transposed copy of vol, if the caller has one
+int launch_transpose_xy(const float* vol, float* volT, const Grid& g, cudaStream_t st);
 // exact adjoint of launch_ax (ray-driven scatter of the same weights); vol [nz][ny][nx] is overwritten
 int launch_ax_adjoint(const float* proj, const Grid& g, const RayView* d_views, int nViews, int mode, float* vol,
                       cudaStream_t st);
@@ -128,6 +130,9 @@ bool vox_needs_clamp(const Grid& g, const VoxView* host_views, int n);
 int launch_residual(const float* b, const int32_t* view_idx, const float* Ax, const float* W, float* r,
                     size_t per_view, int nViews, double* d_nrm2_accum, cudaStream_t st);
 int launch_update(float* x, const float* g, const float* V, float lambda, int nonneg, size_t n, cudaStream_t st);
+// the same update, which also writes the (x,y)-transposed copy xT[z][x][y] of the new iterate (tiles through shared memory)
+int launch_update_t(float* x, float* xT, const float* g, const float* V, float lambda, int nonneg, int nx, int ny, int nz,
+                    cudaStream_t st);
 int launch_invert_rows(float* w, size_t n, float eps, cudaStream_t st);                 // w = w>eps ? 1/w : 0
 int launch_invert_cols(float* v, size_t n, float rel_eps, cudaStream_t st);             // eps = rel_eps*max(v)
 int launch_dot(const float* a, const float* b, size_t n, double* d_out, cudaStream_t st);   // *d_out = sum a*b

@@ -128,6 +128,40 @@ int launch_update(float* x, const float* g, const float* V, float lambda, int no
     return TIGRE_OK;
 }
 
+// x <- max(0, x + lambda V g) (as update_kernel) AND xT[z][x][y] <- the new x: the Siddon / interpolated Ax kernels read an
+// (x,y)-transposed copy for x-dominant rays; writing it here saves re-reading the volume in a separate transpose pass.
+__global__ void __launch_bounds__(256)
+update_t_kernel(float* __restrict__ x, float* __restrict__ xT, const float* __restrict__ g, const float* __restrict__ V,
+                float lambda, int nonneg, int nx, int ny) {
+    __shared__ float tile[32][33];
+    const size_t slice = (size_t)nx * ny * blockIdx.z;
+    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
+    for (int j = threadIdx.y; j < 32; j += 8) {
+        const int ix = x0 + threadIdx.x, iy = y0 + j;
+        if (ix < nx && iy < ny) {
+            const size_t i = slice + (size_t)iy * nx + ix;
+            float v = fmaf(lambda * (V ? __ldg(V + i) : 1.f), __ldg(g + i), x[i]);
+            if (nonneg) v = fmaxf(v, 0.f);
+            x[i] = v;
+            tile[j][threadIdx.x] = v;
+        }
+    }
+    __syncthreads();
+    for (int j = threadIdx.y; j < 32; j += 8) {
+        const int iy = y0 + threadIdx.x, ix = x0 + j;
+        if (ix < nx && iy < ny) xT[slice + (size_t)ix * ny + iy] = tile[threadIdx.x][j];
+    }
+}
+int launch_update_t(float* x, float* xT, const float* g, const float* V, float lambda, int nonneg, int nx, int ny, int nz,
+                    cudaStream_t st) {
+    dim3 tb(32, 8), grid((nx + 31) / 32, (ny + 31) / 32, nz);
+    if (grid.y > 65535 || grid.z > 65535) return TIGRE_ERR_ARG;
+    ProfScope ps(PK_EW, st);
+    update_t_kernel<<<grid, tb, 0, st>>>(x, xT, g, V, lambda, nonneg, nx, ny);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+
 __global__ void __launch_bounds__(256) invert_kernel(float* __restrict__ w, size_t n, float eps, const float* __restrict__ d_max, float rel) {
     const float e = d_max ? rel * (*d_max) : eps;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
