@@ -16,6 +16,11 @@
 #include <cmath>
 #include "common.cuh"
 
+// Launch configuration, overridable with -D for sweeps (measured on C3 / C2 / C4):
+//   AXMB   CTAs per SM of the Siddon kernel: 9 (56 registers); 5-6 / 7 / 8 / 10 / 12 / 16 give 986 / 1093 / 1139 / 1149 / 1130 / 1071
+//          against 1165 G samples/s
+//   AXIMB  CTAs per SM of the interpolated kernel: 8 (64 registers); 9 the same, 10 and 12 spill and lose 9-12 %
+//   AXTV   detector rows per CTA (tile = 32 x AXTV pixels): 4; 1, 2 and 8 lose 0.3-4 %
 #ifndef AXIMB
 #define AXIMB 8
 #endif
