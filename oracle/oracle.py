@@ -300,3 +300,18 @@ def cgls(b, geo, angles, n_iter, ax_mode=SIDDON, atb_mode=MATCHED, exact_adjoint
         gamma = gamma_new
         resid[it] = np.sqrt(float(np.sum(r * r)))
     return x, resid
+
+
+# ------------------------------------------------------------------ gradient descent, eq. (4)
+def gradient_descent(b, geo, angles, n_iter, lam, ax_mode=SIDDON, atb_mode=MATCHED, exact_adjoint=False, x0=None):
+    """x^k = x^{k-1} + lam A^T (b - A x^{k-1}) (eq. 4; the paper prints the residual as (Ax - b): with that sign the
+    iteration ascends, so the descent sign is taken: reading P32).  resid[k] = ||b - A x^{k-1}||_2."""
+    AT = (lambda y: atb_exact(y, geo, angles, ax_mode)) if exact_adjoint else (lambda y: atb(y, geo, angles, atb_mode))
+    b = np.asarray(b, dtype=np.float64)
+    x = np.zeros(geo.vol_shape) if x0 is None else np.array(x0, dtype=np.float64)
+    resid = np.zeros(n_iter)
+    for k in range(n_iter):
+        r = b - ax(x, geo, angles, ax_mode)
+        resid[k] = np.sqrt(float(np.sum(r * r)))
+        x = x + lam * AT(r)
+    return x, resid

@@ -130,3 +130,25 @@ def test_fista_first_iterates_by_hand(tiny_system):
     y2 = x2_ref + (t1 - 1) / t2 * (x2_ref - x1_ref)
     x3_ref = prox.tv_prox(y2 + (2.0 / L) * At(b - orc.ax(y2, geo, ang, orc.SIDDON)), lam, nit)
     assert np.allclose(x3, x3_ref, atol=1e-14)
+
+
+def test_gradient_descent_is_fista_without_momentum_and_converges(tiny_system):
+    # eq. (4) (reading P32): one FISTA iteration with lam_tv = 0 IS a gradient step of length 2/L; iterating it from its own
+    # result reproduces gradient descent with lam = 2/L; with lam < 2/sigma_max^2 the residual decreases monotonically to
+    # the least-squares residual
+    geo, ang, A, b = tiny_system
+    smax = np.linalg.svd(A, compute_uv=False)[0]
+    lam = 1.0 / smax ** 2
+    x, resid = orc.gradient_descent(b, geo, ang, 4, lam, exact_adjoint=True)
+    xi = np.zeros(geo.vol_shape)
+    for _ in range(4):
+        xi, _ = prox.fista(b, geo, ang, 1, 2.0 / lam, 0.0, 0, exact_adjoint=True, x0=xi)
+    assert np.allclose(x, xi, rtol=1e-13, atol=1e-15)
+    _, resid = orc.gradient_descent(b, geo, ang, 300, lam, exact_adjoint=True)
+    assert np.all(np.diff(resid) <= 1e-12)
+    xs, *_ = np.linalg.lstsq(A, b.ravel(), rcond=None)
+    assert resid[-1] >= np.linalg.norm(A @ xs - b.ravel()) - 1e-12
+    # and by hand: the first step from zero is lam A^T b
+    x1, r1 = orc.gradient_descent(b, geo, ang, 1, lam, exact_adjoint=True)
+    assert np.allclose(x1.ravel(), lam * (A.T @ b.ravel()), rtol=1e-12, atol=1e-15)
+    assert r1[0] == pytest.approx(np.linalg.norm(b), rel=1e-14)
