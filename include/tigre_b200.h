@@ -187,6 +187,11 @@ TIGRE_API int tigre_plan_asd_pocs(tigre_plan *plan, const float *b, float *x_ino
  * four tigre_Atb modes (the exact ones must match ax_mode); tigre_ossart / tigre_plan_* take the voxel-driven two. */
 TIGRE_API int tigre_cgls(const float *b, const tigre_geo *geo, const double *angles, int nA, int n_iter,
                int ax_mode, int atb_mode, float *x_out, double *resid_hist, void *cuda_stream);
+/* Gradient descent (eq. 4; reading P32): x^k = x^{k-1} + lambda A^T (b - A x^{k-1}), all views per
+ * step, no weights, no constraint (the paper prints the residual as (Ax - b); the descent sign is used).  x_inout dev (start in,
+ * result out); resid_hist[k] (host, may be NULL) = ||b - A x^{k-1}||_2.  atb_mode: any of the four tigre_Atb modes. */
+TIGRE_API int tigre_gradient_descent(const float *b, const tigre_geo *geo, const double *angles, int nA, int n_iter, float lambda,
+                           int ax_mode, int atb_mode, float *x_inout, double *resid_hist, void *cuda_stream);
 /* FDK (DESIGN.md O-D): cosine weight, Ram-Lak ramp filter along u, FDK-weighted
  * backprojection scaled by pi/nA (full 2 pi orbit).  b dev, x_out dev. */
 TIGRE_API int tigre_fdk(const float *b, const tigre_geo *geo, const double *angles, int nA, float *x_out,

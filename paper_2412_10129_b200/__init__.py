@@ -49,7 +49,7 @@ class TigreError(RuntimeError):
 
 _LIB = None
 EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_Ax_slab", "tigre_Atb_slab", "tigre_slab_row_band", "tigre_row_weights", "tigre_col_weights", "tigre_residual",
-           "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_fdk", "tigre_fdk_filter", "tigre_fdk_ex", "tigre_fdk_filter_ex", "tigre_fdk_weights", "tigre_flatten_detector",
+           "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_gradient_descent", "tigre_fdk", "tigre_fdk_filter", "tigre_fdk_ex", "tigre_fdk_filter_ex", "tigre_fdk_weights", "tigre_flatten_detector",
            "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_create_ex", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_sart_tv", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version"]
@@ -353,6 +353,22 @@ def cgls(b, geo, angles, n_iter, ax_mode="siddon", atb_mode="matched"):
 
 _FILTERS = {"ram_lak": 0, "shepp_logan": 1, "cosine": 2, "hamming": 3, "hann": 4}
 _WEIGHTINGS = {None: 0, "full": 0, "parker": 1, "wang": 2}
+
+
+def gradient_descent(b, geo, angles, n_iter, lam, ax_mode="siddon", atb_mode="matched", x0=None):
+    """Eq. (4): x += lam A^T (b - A x); returns (x, resid)."""
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    x = _new(vol_shape(geo), like=b)
+    if x0 is None:
+        x.zero_()
+    else:
+        x.copy_(x0)
+    hist = np.zeros(max(n_iter, 1), dtype=np.float64)
+    _check(_lib().tigre_gradient_descent(_f32(b, proj_shape(geo, nA), "b"), G.ref, a.ctypes.data_as(_dp), nA, int(n_iter),
+                                         C.c_float(lam), _AX_MODES[ax_mode], _ATB_MODES[atb_mode], _f32(x),
+                                         hist.ctypes.data_as(_dp), _stream(b)), "tigre_gradient_descent")
+    return x, hist[:n_iter]
 
 
 def fdk_ex(b, geo, angles, filt="ram_lak", weighting=None):

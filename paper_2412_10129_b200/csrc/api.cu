@@ -700,6 +700,44 @@ int tigre_cgls(const float* b, const tigre_geo* geo, const double* angles, int n
     return TIGRE_OK;
 }
 
+// ---------------------------------------------------------------- gradient descent, eq. (4) (reading P32)
+int tigre_gradient_descent(const float* b, const tigre_geo* geo, const double* angles, int nA, int n_iter, float lambda, int ax_mode,
+                           int atb_mode, float* x, double* resid_hist, void* cuda_stream) {
+    if (!b || !x || n_iter < 0) return TIGRE_ERR_ARG;
+    if (ax_mode != TIGRE_AX_SIDDON && ax_mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
+    if (atb_mode < TIGRE_ATB_MATCHED || atb_mode > TIGRE_ATB_EXACT_INTERP) return TIGRE_ERR_ARG;
+    const bool exact = atb_mode >= TIGRE_ATB_EXACT_SIDDON;
+    if (exact && atb_mode - TIGRE_ATB_EXACT_SIDDON != ax_mode) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    if (mem_kind(b) != MEM_DEVICE || mem_kind(x) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const Grid& g = t.g;
+    const size_t np = (size_t)nA * g.nu * g.nv, nvox = (size_t)g.nx * g.ny * g.nz;
+    TempBuf r, grad, sc;
+    TG_TRY(r.alloc(sizeof(float) * np, st));
+    TG_TRY(grad.alloc(sizeof(float) * nvox, st));
+    TG_TRY(sc.alloc(sizeof(double) * std::max(n_iter, 1), st));
+    TG_CUDA(cudaMemsetAsync(sc.p, 0, sizeof(double) * std::max(n_iter, 1), st));
+    TG_TRY(t.build_ray(nullptr, nA, st));
+    if (!exact) TG_TRY(t.build_vox(nullptr, nA, st));
+    for (int it = 0; it < n_iter; ++it) {
+        TG_TRY(launch_ax(x, g, t.ray.as<RayView>(), nA, ax_mode, false, false, r.as<float>(), nullptr, st));
+        TG_TRY(launch_residual(b, nullptr, r.as<float>(), nullptr, r.as<float>(), (size_t)g.nu * g.nv, nA, sc.as<double>() + it, st));
+        if (exact) TG_TRY(launch_ax_adjoint(r.as<float>(), g, t.ray.as<RayView>(), nA, ax_mode, grad.as<float>(), st));
+        else TG_TRY(launch_atb(r.as<float>(), g, t.vox.as<VoxView>(), nA, atb_mode, false, grad.as<float>(), 0, g.nz, false, 0, g.nv, t.clamp, st,
+                               t.hvox.data()));
+        TG_TRY(launch_update(x, grad.as<float>(), nullptr, lambda, 0, nvox, st));
+    }
+    if (resid_hist && n_iter > 0) {
+        std::vector<double> h(n_iter);
+        TG_CUDA(cudaMemcpyAsync(h.data(), sc.p, sizeof(double) * n_iter, cudaMemcpyDeviceToHost, st));
+        TG_CUDA(cudaStreamSynchronize(st));
+        for (int it = 0; it < n_iter; ++it) resid_hist[it] = std::sqrt(h[it]);
+    }
+    return TIGRE_OK;
+}
+
 // ---------------------------------------------------------------- FDK (O-D)
 static int fdk_filter_impl(const float* b, Tables& t, int nA, float* q, cudaStream_t st) {
     std::vector<double> dd(2 * (size_t)nA);

@@ -95,6 +95,18 @@ def test_fista_matches_oracle(tg, modes):
     assert rref[-1] < rref[0]
 
 
+def test_gradient_descent_eq4_matches_oracle(tg):
+    geo, ang, rec = make_config("C1", scale=2, n_angles=16)
+    vol = phantom_for(rec, geo).astype(np.float64)
+    b = orc.ax(vol, geo, ang, orc.SIDDON).astype(np.float32)
+    lam = 1.0 / float(orc.atb(orc.ax(np.ones(geo.vol_shape), geo, ang, orc.SIDDON), geo, ang, orc.MATCHED).max())
+    for atm, exact in (("matched", False), ("exact_siddon", True)):
+        ref, rref = orc.gradient_descent(b, geo, ang, 5, lam, exact_adjoint=exact)
+        x, resid = tg.gradient_descent(dev(b), geo, ang, 5, lam, atb_mode=atm)
+        assert H.rel_l2(host(x), ref) <= 1e-4 and np.allclose(resid, rref, rtol=1e-4)
+        assert resid[-1] < resid[0]
+
+
 def test_fista_init_and_argument_errors(tg):
     geo, ang, rec = make_config("C1", scale=4, n_angles=6)
     vol = phantom_for(rec, geo).astype(np.float32)
