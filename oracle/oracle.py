@@ -315,3 +315,38 @@ def gradient_descent(b, geo, angles, n_iter, lam, ax_mode=SIDDON, atb_mode=MATCH
         resid[k] = np.sqrt(float(np.sum(r * r)))
         x = x + lam * AT(r)
     return x, resid
+
+
+# ------------------------------------------------------------------ MLEM / OSEM, eq. (5); 118-120, 139
+def osem(b, geo, angles, subsets, n_iter, ax_mode=SIDDON, atb_mode=MATCHED, exact_adjoint=False, x0=None):
+    """x <- x / (A_s^T 1) * A_s^T (b_s / (A_s x)) for every subset s in turn (one subset holding all views: MLEM, eq. 5).
+    Reading P33: the quotient is 0 where A_s x <= 0 (rays that miss the support), the column normalisation 1/(A_s^T 1) is
+    0 where A_s^T 1 <= 1e-6 max (as V in P13); x0 = ones unless given."""
+    angles = np.asarray(angles, dtype=np.float64).reshape(-1, 3)
+    b = np.asarray(b, dtype=np.float64)
+    x = np.ones(geo.vol_shape) if x0 is None else np.array(x0, dtype=np.float64)
+    subsets = [np.asarray(s, dtype=np.int64) for s in subsets]
+
+    def AT(y, gs, a):
+        return atb_exact(y, gs, a, ax_mode) if exact_adjoint else atb(y, gs, a, atb_mode)
+
+    Vs = []
+    for s in subsets:
+        gs = _sub_geo(geo, s)
+        at1 = AT(np.ones((len(s),) + geo.proj_shape), gs, angles[s])
+        V = np.zeros_like(at1)
+        np.divide(1.0, at1, out=V, where=at1 > 1e-6 * at1.max())
+        Vs.append(V)
+    for _ in range(n_iter):
+        for s, V in zip(subsets, Vs):
+            gs = _sub_geo(geo, s)
+            p = ax(x, gs, angles[s], ax_mode)
+            ratio = np.zeros_like(p)
+            np.divide(b[s], p, out=ratio, where=p > 0.0)
+            x = x * V * AT(ratio, gs, angles[s])
+    return x
+
+
+def mlem(b, geo, angles, n_iter, **kw):
+    nA = np.asarray(angles).reshape(-1, 3).shape[0]
+    return osem(b, geo, angles, [np.arange(nA)], n_iter, **kw)

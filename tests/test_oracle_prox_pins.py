@@ -152,3 +152,34 @@ def test_gradient_descent_is_fista_without_momentum_and_converges(tiny_system):
     x1, r1 = orc.gradient_descent(b, geo, ang, 1, lam, exact_adjoint=True)
     assert np.allclose(x1.ravel(), lam * (A.T @ b.ravel()), rtol=1e-12, atol=1e-15)
     assert r1[0] == pytest.approx(np.linalg.norm(b), rel=1e-14)
+
+
+def test_mlem_eq5_by_hand_fixed_point_and_kl_descent(tiny_system):
+    # eq. (5): the first iterate from x = 1 written with the explicit matrix; a consistent solution is a fixed point; with
+    # the exact adjoint the Kullback-Leibler distance KL(b, Ax) never increases (the classical EM property); one subset of
+    # all views = MLEM, and OSEM with the subsets visited in turn equals chained single-subset calls
+    geo, ang, A, b = tiny_system
+    b = np.abs(b) + 0.05
+    bv = b.ravel()
+    x1 = orc.mlem(b, geo, ang, 1, exact_adjoint=True)
+    hit = (A @ np.ones(A.shape[1])) > 0                      # rays that meet the volume (the others have a zero row)
+    q = np.zeros_like(bv)
+    q[hit] = bv[hit] / (A @ np.ones(A.shape[1]))[hit]
+    ref = (1.0 / (A.T @ np.ones(A.shape[0]))) * (A.T @ q)
+    assert np.allclose(x1.ravel(), ref, rtol=1e-12)
+    xs = np.random.default_rng(5).random(A.shape[1]) + 0.1
+    bc = (A @ xs).reshape(b.shape)
+    keep = orc.mlem(bc, geo, ang, 3, exact_adjoint=True, x0=xs.reshape(geo.vol_shape))
+    assert np.allclose(keep.ravel(), xs, rtol=1e-12)
+
+    def kl(x):
+        p = (A @ x.ravel())[hit]
+        return float(np.sum(bv[hit] * np.log(bv[hit] / p) - bv[hit] + p))
+
+    vals = [kl(orc.mlem(b, geo, ang, k, exact_adjoint=True)) for k in range(1, 9)]
+    assert all(vals[i + 1] <= vals[i] + 1e-12 for i in range(7)) and vals[-1] < 0.5 * vals[0]
+    subs = [[0, 2, 4], [1, 3, 5]]
+    full = orc.osem(b, geo, ang, subs, 1, exact_adjoint=True)
+    step = orc.osem(b, geo, ang, [subs[0]], 1, exact_adjoint=True)
+    step = orc.osem(b, geo, ang, [subs[1]], 1, exact_adjoint=True, x0=step)
+    assert np.allclose(full, step, rtol=1e-13)
