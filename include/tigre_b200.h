@@ -170,6 +170,11 @@ TIGRE_API int tigre_plan_ossart(tigre_plan *plan, const float *b, float *x_inout
                       int nonneg, double *resid_hist, void *cuda_stream);
 TIGRE_API int tigre_plan_destroy(tigre_plan *plan);
 TIGRE_API size_t tigre_plan_bytes(const tigre_plan *plan);
+/* MLEM / OSEM (eq. 5 "x^k = x^{k-1}/(A1) A^T (b / (A x^{k-1}))"; 118-120, 139 OS counterpart; DESIGN.md reading
+ * P33): for every subset s of the plan in turn  x <- x * V_s * A_s^T(b_s / (A_s x)),  V_s = the plan's column weights 1/(A_s^T 1),
+ * quotient 0 where A_s x <= 0.  One subset holding all views is MLEM.  b, x_inout dev (x_inout: positive start, e.g. ones).
+ * Asynchronous. */
+TIGRE_API int tigre_plan_osem(tigre_plan *plan, const float *b, float *x_inout, int n_iter, void *cuda_stream);
 /* ASD-POCS / OS-ASD-POCS / AwASD-POCS ("Projection Onto Convex Sets ... ASD-POCS [30] ... Adaptive weighed TV
  * norm [32, 33] ... OS versions", 141-149 Snippet 1, 169; reading P23 spells the loop out).  Per iteration:
  *   x0 = x;  one OS-SART sweep of the plan's subsets with relaxation beta (nonnegativity on);  beta *= beta_red;

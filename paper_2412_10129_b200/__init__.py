@@ -50,7 +50,7 @@ class TigreError(RuntimeError):
 _LIB = None
 EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_Ax_slab", "tigre_Atb_slab", "tigre_slab_row_band", "tigre_row_weights", "tigre_col_weights", "tigre_residual",
            "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_gradient_descent", "tigre_fdk", "tigre_fdk_filter", "tigre_fdk_ex", "tigre_fdk_filter_ex", "tigre_fdk_weights", "tigre_flatten_detector",
-           "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_create_ex", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_sart_tv", "tigre_plan_destroy",
+           "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_create_ex", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_osem", "tigre_plan_sart_tv", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version"]
 
@@ -313,6 +313,12 @@ class OssartPlan:
                                           C.c_float(r_max), C.c_float(epsilon), _delta(delta), C.c_float(tv_eps),
                                           hist.ctypes.data_as(_dp), C.byref(done), _stream(b)), "tigre_plan_asd_pocs")
         return hist[:done.value]
+
+    def osem(self, b, x, n_iter):
+        """MLEM (one subset of all views) / OSEM in place on x (positive start)."""
+        _check(_lib().tigre_plan_osem(self._h, _f32(b, proj_shape(self.geo, self.nA), "b"), _f32(x, vol_shape(self.geo), "x"),
+                                      int(n_iter), _stream(b)), "tigre_plan_osem")
+        return x
 
     def sart_tv(self, b, x, n_iter, lam=1.0, lam_red=1.0, tv_lambda=0.0, tv_iter=10, tau=1.0 / 12.0):
         """SART-TV in place on x: OS-SART sweep + TV prox per iteration; returns the residual history."""

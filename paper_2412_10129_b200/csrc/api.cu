@@ -576,6 +576,27 @@ int tigre_ossart(const float* b, const tigre_geo* geo, const double* angles, int
     return rc;
 }
 
+// ---------------------------------------------------------------- MLEM / OSEM (eq. 5; reading P33)
+int tigre_plan_osem(tigre_plan* P, const float* b, float* x, int n_iter, void* cuda_stream) {
+    if (!P || !b || !x || n_iter < 0) return TIGRE_ERR_ARG;
+    if (mem_kind(b) != MEM_DEVICE || mem_kind(x) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const Grid& g = P->t.g;
+    const size_t per = (size_t)g.nu * g.nv, nvox = (size_t)g.nx * g.ny * g.nz;
+    for (int it = 0; it < n_iter; ++it) {
+        for (int s = 0; s < P->nSubsets; ++s) {
+            const int n = P->off[s + 1] - P->off[s];
+            float* A = P->Axb.as<float>();
+            TG_TRY(launch_ax(x, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st));
+            TG_TRY(launch_ratio(b, P->d_idx.as<int32_t>() + P->off[s], A, A, per, n, st));
+            TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>(), 0, g.nz, false, 0, g.nv, P->clamp,
+                              st, P->hvox[s].data()));
+            TG_TRY(launch_mul_update(x, P->grad.as<float>(), P->V.as<float>() + nvox * s, nvox, st));
+        }
+    }
+    return TIGRE_OK;
+}
+
 // ---------------------------------------------------------------- ASD-POCS family (reading P23; oracle/pocs.py)
 // Data step = one OS-SART sweep of the plan with relaxation beta; regulariser step = ng normalised steepest-descent
 // steps on (Aw)TV.  The control scalars (dd, dp, dg) decide the next step length on the host: two stream

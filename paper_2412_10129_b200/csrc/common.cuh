@@ -142,6 +142,8 @@ int launch_xpby(float* p, const float* s, const double* d_num, const double* d_d
                 cudaStream_t st);                                                       // p = s + (num/den)*p
 int launch_scale(float* x, float a, size_t n, cudaStream_t st);
 int launch_scale_columns(float* W, const float* colw, int nViews, int nv, int nu, cudaStream_t st);
+int launch_ratio(const float* b, const int32_t* view_idx, const float* Ax, float* q, size_t per_view, int nViews, cudaStream_t st);
+int launch_mul_update(float* x, const float* g, const float* V, size_t n, cudaStream_t st);
 int launch_diff_stats(const float* a, const float* b, const float* c, size_t n, double* d_out3, cudaStream_t st);
 void fdk_filter_taps(int nu, int filter, std::vector<double>& g);
 int fdk_weights(const Grid& g, const std::vector<ViewH>& views, int weighting, std::vector<double>& w);

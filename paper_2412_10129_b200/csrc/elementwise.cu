@@ -195,6 +195,38 @@ int launch_invert_cols(float* v, size_t n, float rel_eps, cudaStream_t st) {
     return TIGRE_OK;
 }
 
+// MLEM / OSEM (eq. 5; reading P33): q[j][i] = b[view_idx[j]][i] / Ax[j][i] where Ax > 0, else 0 (in place over Ax is fine)
+__global__ void __launch_bounds__(256) ratio_kernel(const float* __restrict__ b, const int32_t* __restrict__ view_idx,
+                                                    const float* __restrict__ Ax, float* __restrict__ q, size_t per_view, size_t total) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t j = i / per_view;
+        const size_t src = (size_t)(view_idx ? view_idx[j] : (int32_t)j) * per_view + (i - j * per_view);
+        const float p = Ax[i];
+        q[i] = p > 0.f ? __ldg(b + src) / p : 0.f;
+    }
+}
+int launch_ratio(const float* b, const int32_t* view_idx, const float* Ax, float* q, size_t per_view, int nViews, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
+    const size_t total = per_view * nViews;
+    if (total == 0) return TIGRE_OK;
+    ratio_kernel<<<ew_blocks(total), 256, 0, st>>>(b, view_idx, Ax, q, per_view, total);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+// x <- x * V * g   (the multiplicative update of eq. 5; V = 1/(A^T 1))
+__global__ void __launch_bounds__(256) mul_update_kernel(float* __restrict__ x, const float* __restrict__ g, const float* __restrict__ V,
+                                                         size_t n) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        x[i] = x[i] * __ldg(V + i) * __ldg(g + i);
+}
+int launch_mul_update(float* x, const float* g, const float* V, size_t n, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
+    if (n == 0) return TIGRE_OK;
+    mul_update_kernel<<<ew_blocks(n), 256, 0, st>>>(x, g, V, n);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+
 // W[j][iv][iu] *= colw[j][iu]   (data-redundancy weighting of the row weights, reading P17)
 __global__ void __launch_bounds__(256) scale_columns_kernel(float* __restrict__ W, const float* __restrict__ colw, int nu, size_t per,
                                                             size_t total) {

@@ -138,6 +138,19 @@ def test_sart_tv_matches_oracle(tg):
     plan.close()
 
 
+def test_mlem_and_osem_match_oracle(tg):
+    geo, ang, b = noisy_case(2, 24, 10)
+    b = np.abs(b) + 0.01
+    for subsets in ([list(range(24))], [list(range(s, 24, 4)) for s in range(4)]):       # MLEM, OSEM
+        ref = orc.osem(b, geo, ang, subsets, 3)
+        plan = tg.OssartPlan(geo, ang, subsets, "siddon", "matched")
+        x = torch.ones(geo.vol_shape, dtype=torch.float32, device="cuda")
+        plan.osem(dev(b), x, 3)
+        plan.close()
+        assert H.rel_l2(host(x), ref) <= 1e-4
+        assert float(x.min()) >= 0.0
+
+
 def test_argument_errors(tg):
     geo, ang, b = noisy_case(4, 4, 8)
     plan = tg.OssartPlan(geo, ang, [[0, 1], [2, 3]], "siddon", "matched")
