@@ -546,6 +546,34 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     }
 }
 
+// Row sums A 1 of the Siddon projector in closed form: the intersection lengths of a ray with
+// the voxels add up to the length of its segment inside the volume box, so a unit volume needs no march: clip the
+// segment S -> P (parameter [0,1]) against the box [0,n]^3 in voxel-index coordinates, in fp64.
+__global__ void __launch_bounds__(AX_TU* AX_TV)
+ax_siddon_unit_kernel(const RayView* __restrict__ views, int nViews, AxP p, float* __restrict__ proj) {
+    int view, iu, iv;
+    if (!ax_decode(p, nViews, view, iu, iv)) return;
+    const RayView& rv = views[view];
+    const size_t out = ((size_t)view * p.nv + iv) * p.nu + iu;
+    const double n[3] = {(double)p.nx, (double)p.ny, (double)p.nz};
+    const double h[3] = {p.hxd, p.hyd, p.hzd};
+    double t0 = 0.0, t1 = 1.0, L2 = 0.0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const double S = rv.S[k] + iu * rv.dSU[k] + iv * rv.dSV[k];
+        const double d = rv.P0[k] + iu * rv.dU[k] + iv * rv.dV[k] - S;
+        L2 += d * h[k] * d * h[k];
+        if (d != 0.0) {
+            const double a = (0.0 - S) / d, b = (n[k] - S) / d;
+            t0 = fmax(t0, fmin(a, b)), t1 = fmin(t1, fmax(a, b));
+        } else if (S < 0.0 || S >= n[k]) {
+            t1 = -1.0;   // parallel to this pair of faces and outside (a ray IN a face goes to the upper voxel, reading P8)
+        }
+    }
+    const float result = t1 > t0 ? (float)((t1 - t0) * sqrt(L2)) : 0.f;
+    proj[out] = p.accumulate ? proj[out] + result : result;
+}
+
 template <typename IdxT>
 static void ax_dispatch(const float* vol, const float* volT, const RayView* v, int nViews, const AxP& p, int mode, bool unit,
                         float* proj, uint32_t* counts, cudaStream_t st) {
@@ -554,7 +582,7 @@ static void ax_dispatch(const float* vol, const float* volT, const RayView* v, i
     dim3 grid((unsigned)nblk);
     if (mode == TIGRE_AX_SIDDON) {
         if (counts) ax_siddon_kernel<IdxT, false, true, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
-        else if (unit) ax_siddon_kernel<IdxT, true, false, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
+        else if (unit) ax_siddon_unit_kernel<<<grid, block, 0, st>>>(v, nViews, p, proj);
         else ax_siddon_kernel<IdxT, false, false, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
     } else {
         if (counts) ax_interp_kernel<IdxT, false, true, false><<<grid, block, 0, st>>>(vol, volT, v, nViews, p, proj, counts);
