@@ -8,6 +8,7 @@ configs[2] "C3" (512^3, 720 views of 1024x768, half-fan, Poisson noise, 20 order
 Siddon Ax / matched A^T b) — the configuration north_star's target is quoted on.
 
   python bench.py --gpus N --steps K --warmup W [--config C3] [--impl reference]
+  python bench.py --mode tv [--tv-op prox] | --mode chunked | --mode drivers     (the other measured rows)
 
 N > 1 (torchrun): the path does not shard in this build (north_star: one GPU, no collectives),
 so every rank runs an independent replica of the same workload; value = N * units / max time.
@@ -339,6 +340,48 @@ def run_tv(args, tg, geo, rec, K, W, rank, world, local_rank):
     print(json.dumps(line))
 
 
+def run_drivers(args, tg, geo, ang, rec, subsets, rank):
+    """One iteration of every reconstruction driver on the config's workload, device-resident:
+    the extra rows' measurement.  One JSON line: ms per iteration (CUDA events, second of two runs)."""
+    import torch
+    vol = torch.from_numpy(phantom_for(rec, geo)).cuda()
+    b = tg.Ax(vol, geo, ang, rec["ax"])
+    del vol
+    plan = tg.OssartPlan(geo, ang, subsets, rec["ax"], rec["atb"])
+
+    def timed(f):
+        f()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        f()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1)
+
+    x = torch.zeros(geo.vol_shape, dtype=torch.float32, device="cuda")
+    out = {}
+    out["os_sart"] = timed(lambda: plan.iterate(b, x, 1, want_resid=False))
+    x.zero_()
+    out["os_asd_pocs_ng20"] = timed(lambda: plan.asd_pocs(b, x, 1, ng=20))
+    x.zero_()
+    out["sart_tv_tviter50"] = timed(lambda: plan.sart_tv(b, x, 1, tv_lambda=1e-3, tv_iter=50))
+    x.fill_(1.0)
+    out["osem"] = timed(lambda: plan.osem(b, x, 1))
+    plan.close()
+    del x
+    out["fista_tviter50"] = timed(lambda: tg.fista(b, geo, ang, 1, 2e5, 1e-3, 50, rec["ax"], rec["atb"]))
+    out["cgls"] = timed(lambda: tg.cgls(b, geo, ang, 1, rec["ax"], rec["atb"]))
+    out["gradient_descent"] = timed(lambda: tg.gradient_descent(b, geo, ang, 1, 1e-6, rec["ax"], rec["atb"]))
+    out["fdk_ram_lak"] = timed(lambda: tg.fdk(b, geo, ang))
+    out["fdk_hann"] = timed(lambda: tg.fdk_ex(b, geo, ang, "hann"))
+    if rank == 0:
+        print(json.dumps({"metric": "ms per iteration of each driver", "unit": "ms", "n_gpus": 1, "data": "synthetic", "dtype": "f32",
+                          "config": {"workload": f"{rec['name']}: {geo.nVoxel[0]}^3, {len(ang)} views of {geo.nDetector[0]}x"
+                                                 f"{geo.nDetector[1]}, {rec['ax']} Ax / {rec['atb']} A^T b, {len(subsets)} subsets"},
+                          "ms_per_iteration": {k: round(v, 2) for k, v in out.items()}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -352,7 +395,7 @@ def main():
     ap.add_argument("--tv-delta", type=float, default=0.0, help="tv mode: AwTV delta (0 = plain TV)")
     ap.add_argument("--tv-op", default="minimise", choices=["minimise", "prox"],
                     help="tv mode: the gradient-descent minimiser (tigre_minimize_awtv) or the TV proximal operator of FISTA (tigre_tv_prox)")
-    ap.add_argument("--mode", default="plan", choices=["plan", "chunked", "tv"],
+    ap.add_argument("--mode", default="plan", choices=["plan", "chunked", "tv", "drivers"],
                     help="plan: OS-SART iteration in HBM (default); chunked: Ax + A^T b with all arrays in pinned host memory (S8)")
     ap.add_argument("--budget-gb", type=float, default=0.0, help="chunked mode: device bytes the chunked path may use (0 = 3/4 of free)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -410,6 +453,11 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
+    if args.mode == "drivers":
+        run_drivers(args, tg, geo, ang, rec, subsets, rank)
+        if world > 1:
+            dist.destroy_process_group()
+        return
     if args.mode == "tv":
         run_tv(args, tg, geo, rec, K, W, rank, world, local_rank)
         if world > 1:
