@@ -26,23 +26,74 @@ namespace {
 // taps == NULL: the Ram-Lak taps of reading P12 are formed in the kernel.
 constexpr int FR = 8;
 
+__host__ __device__ constexpr int mod8(int x) { return ((x % FR) + FR) % FR; }
+__host__ __device__ constexpr int fdiv8(int x) { return (x - mod8(x)) / FR; }
+
+// acc[j] += sum_{d >= 0} T[d] * (src[i0 + A + j - d] + src[i0 + AR + j + d]),  j = 0..7, for an 8-aligned i0: the left window
+// runs over taps d <= 8 mL + 7, the right one over d <= 8 mR + 7 (negative: side absent).  src is stored in FR planes by
+// (index mod FR), element e at plane e mod FR, offset (e + PAD) / FR; ob = (i0 + PAD) / FR.  A, AR are compile-time so that every
+// plane index is: each tap costs one row load per side (consecutive words across the threads of a warp: no bank
+// conflict), one broadcast tap (two LDS.128 per 8 taps) and 16 FMAs.
+template <int A, int AR>
+__device__ __forceinline__ void conv8(const float* __restrict__ src, int PL, int ob, const float* __restrict__ T, int mL, int mR,
+                                      float (&acc)[FR]) {
+    float L[FR], R[FR];
+#pragma unroll
+    for (int j = 0; j < FR; ++j) {
+        L[j] = src[mod8(A + j) * PL + ob + fdiv8(A + j)];
+        R[j] = src[mod8(AR + j) * PL + ob + fdiv8(AR + j)];
+    }
+    for (int m = 0; m <= mL; ++m) {
+        const float4 ta = *reinterpret_cast<const float4*>(T + FR * m), tb = *reinterpret_cast<const float4*>(T + FR * m + 4);
+        const float t[FR] = {ta.x, ta.y, ta.z, ta.w, tb.x, tb.y, tb.z, tb.w};
+#pragma unroll
+        for (int k = 0; k < FR; ++k) {   // tap d = FR * m + k
+#pragma unroll
+            for (int j = 0; j < FR; ++j) acc[j] = fmaf(t[k], L[j], acc[j]);
+#pragma unroll
+            for (int j = FR - 1; j > 0; --j) L[j] = L[j - 1];
+            L[0] = src[mod8(A - k - 1) * PL + ob - m + fdiv8(A - k - 1)];          // src[i0 + A - (d + 1)]
+        }
+    }
+    for (int m = 0; m <= mR; ++m) {
+        const float4 ta = *reinterpret_cast<const float4*>(T + FR * m), tb = *reinterpret_cast<const float4*>(T + FR * m + 4);
+        const float t[FR] = {ta.x, ta.y, ta.z, ta.w, tb.x, tb.y, tb.z, tb.w};
+#pragma unroll
+        for (int k = 0; k < FR; ++k) {
+#pragma unroll
+            for (int j = 0; j < FR; ++j) acc[j] = fmaf(t[k], R[j], acc[j]);
+#pragma unroll
+            for (int j = 0; j < FR - 1; ++j) R[j] = R[j + 1];
+            R[FR - 1] = src[mod8(AR + k) * PL + ob + m + 1 + fdiv8(AR + k)];       // src[i0 + AR + FR - 1 + (d + 1)]
+        }
+    }
+}
+
+// ODD = false: every tap (windowed filters).  The centre tap is applied separately and T[0] = 0, so both windows start at the
+//              output's own position (A = AR = 0).
+// ODD = true:  Ram-Lak without a window: the taps vanish at even n != 0, so an output of one parity reads only row elements of
+//              the other parity.  The row is stored as two half-rows X0[m] = row[2m], X1[m] = row[2m + 1] and the taps as
+//              T[d] = tap[2d + 1]: output 2j reads X1[j - 1 - d] and X1[j + d], output 2j + 1 reads X0[j - d] and X0[j + 1 + d]:
+//              two dense half-length convolutions (no skipped taps).
 template <bool ODD>
 __global__ void __launch_bounds__(128)
 fdk_conv_kernel(const float* __restrict__ b, int nu, int nv, float du, float dv, const double* __restrict__ dsd_a,
                 const double* __restrict__ dso_a, const float* __restrict__ taps, const float* __restrict__ colw,
                 float* __restrict__ q, int PAD, int PL, int NT) {
     extern __shared__ __align__(16) float sm[];
-    float* tp = sm;              // [NT]  taps, tp[0] = 0 (the centre tap is applied separately), zero beyond nu
-    float* rw = sm + NT;         // [FR][PL]  row value i at plane (i mod FR), offset (i + PAD) / FR
+    float* tp = sm;              // [NT]  taps (ODD: T[d] = tap[2d + 1]; else tap[n] with tp[0] = 0), zero beyond the row
+    float* rw = sm + NT;         // [FR][PL] planes of the row (ODD: [2][FR][PL], the two half-rows)
     const int iv = blockIdx.x, ia = blockIdx.y;
     const float DSD = (float)dsd_a[ia], DSO = (float)dso_a[ia];
     const float itau = DSD / (du * DSO);
     const float v = ((float)iv + 0.5f) * dv - 0.5f * (float)nv * dv;
     const size_t base = ((size_t)ia * nv + iv) * nu;
-    for (int i = threadIdx.x; i < FR * PL; i += blockDim.x) rw[i] = 0.f;
+    const int nplanes = (ODD ? 2 : 1) * FR * PL;
+    for (int i = threadIdx.x; i < nplanes; i += blockDim.x) rw[i] = 0.f;
     for (int n = threadIdx.x; n < NT; n += blockDim.x) {
+        const int src = ODD ? 2 * n + 1 : n;
         float t = 0.f;
-        if (n >= 1 && n < nu) t = taps ? __ldg(taps + n) : ((n & 1) ? -1.0f / (9.8696044010893586f * (float)n * (float)n) : 0.f);
+        if (src >= 1 && src < nu) t = taps ? __ldg(taps + src) : ((src & 1) ? -1.0f / (9.8696044010893586f * (float)src * (float)src) : 0.f);
         tp[n] = t;
     }
     const float tap0 = taps ? __ldg(taps) : 0.25f;
@@ -51,51 +102,50 @@ fdk_conv_kernel(const float* __restrict__ b, int nu, int nv, float du, float dv,
         const float u = ((float)iu + 0.5f) * du - 0.5f * (float)nu * du;
         float r = __ldg(b + base + iu) * DSD * rsqrtf(DSD * DSD + u * u + v * v);
         if (colw) r *= __ldg(colw + (size_t)ia * nu + iu);
-        rw[(iu % FR) * PL + (iu + PAD) / FR] = r;
+        if (ODD) {
+            const int m = iu >> 1;
+            rw[(iu & 1) * FR * PL + (m % FR) * PL + (m + PAD) / FR] = r;
+        } else {
+            rw[(iu % FR) * PL + (iu + PAD) / FR] = r;
+        }
     }
     __syncthreads();
-    for (int c = threadIdx.x; c * FR < nu; c += blockDim.x) {
-        const int i0 = c * FR, ob = (i0 + PAD) / FR;
-        float acc[FR], L[FR], R[FR];
+    if (!ODD) {
+        for (int c = threadIdx.x; c * FR < nu; c += blockDim.x) {
+            const int i0 = c * FR, ob = (i0 + PAD) / FR;
+            float acc[FR];
 #pragma unroll
-        for (int j = 0; j < FR; ++j) {
-            L[j] = rw[j * PL + ob];          // window at n = 0: row[i0 + j]
-            R[j] = L[j];
-            acc[j] = tap0 * L[j];
+            for (int j = 0; j < FR; ++j) acc[j] = tap0 * rw[j * PL + ob];
+            conv8<0, 0>(rw, PL, ob, tp, (i0 + FR - 1) / FR, (nu - 1 - i0) / FR, acc);
+#pragma unroll
+            for (int j = 0; j < FR; ++j)
+                if (i0 + j < nu) q[base + i0 + j] = acc[j] * itau;
         }
-        // left side: row[i0 + j - n]; taps with n > i0 + FR - 1 meet only the zero padding
-        const int mL = (i0 + FR - 1) / FR, mR = (nu - 1 - i0) / FR;
-        for (int m = 0; m <= mL; ++m) {
-            const float4 ta = *reinterpret_cast<const float4*>(tp + FR * m), tb = *reinterpret_cast<const float4*>(tp + FR * m + 4);
-            const float t[FR] = {ta.x, ta.y, ta.z, ta.w, tb.x, tb.y, tb.z, tb.w};
+    } else {
+        const int n0 = (nu + 1) >> 1, n1 = nu >> 1;          // lengths of X0 (even elements) and X1 (odd elements)
+        const int C0 = (n0 + FR - 1) / FR, C1 = (n1 + FR - 1) / FR;
+        const float* X0 = rw;
+        const float* X1 = rw + FR * PL;
+        for (int id = threadIdx.x; id < C0 + C1; id += blockDim.x) {
+            const int par = id >= C0, j0 = (par ? id - C0 : id) * FR, ob = (j0 + PAD) / FR;
+            float acc[FR];
+            if (!par) {   // outputs 2j: own half-row X0, neighbours in X1 at j - 1 - d and j + d
 #pragma unroll
-            for (int k = 0; k < FR; ++k) {   // n = FR * m + k
-                if (!ODD || (k & 1)) {
+                for (int j = 0; j < FR; ++j) acc[j] = tap0 * X0[j * PL + ob];
+                const int last = n1 - 1 - j0;
+                conv8<-1, 0>(X1, PL, ob, tp, (j0 + FR - 2) / FR, last >= 0 ? last / FR : -1, acc);
+            } else {      // outputs 2j + 1: own half-row X1, neighbours in X0 at j - d and j + 1 + d
 #pragma unroll
-                    for (int j = 0; j < FR; ++j) acc[j] = fmaf(t[k], L[j], acc[j]);
-                }
+                for (int j = 0; j < FR; ++j) acc[j] = tap0 * X1[j * PL + ob];
+                const int last = n0 - 2 - j0;
+                conv8<0, 1>(X0, PL, ob, tp, (j0 + FR - 1) / FR, last >= 0 ? last / FR : -1, acc);
+            }
 #pragma unroll
-                for (int j = FR - 1; j > 0; --j) L[j] = L[j - 1];
-                L[0] = rw[((FR - 1 - k) % FR) * PL + ob - m - 1];      // row[i0 - (n + 1)]
+            for (int j = 0; j < FR; ++j) {
+                const int i = 2 * (j0 + j) + par;
+                if (i < nu) q[base + i] = acc[j] * itau;
             }
         }
-        for (int m = 0; m <= mR; ++m) {
-            const float4 ta = *reinterpret_cast<const float4*>(tp + FR * m), tb = *reinterpret_cast<const float4*>(tp + FR * m + 4);
-            const float t[FR] = {ta.x, ta.y, ta.z, ta.w, tb.x, tb.y, tb.z, tb.w};
-#pragma unroll
-            for (int k = 0; k < FR; ++k) {
-                if (!ODD || (k & 1)) {
-#pragma unroll
-                    for (int j = 0; j < FR; ++j) acc[j] = fmaf(t[k], R[j], acc[j]);
-                }
-#pragma unroll
-                for (int j = 0; j < FR - 1; ++j) R[j] = R[j + 1];
-                R[FR - 1] = rw[k * PL + ob + m + 1];                     // row[i0 + FR - 1 + (n + 1)]
-            }
-        }
-#pragma unroll
-        for (int j = 0; j < FR; ++j)
-            if (i0 + j < nu) q[base + i0 + j] = acc[j] * itau;
     }
 }
 
@@ -233,12 +283,14 @@ int launch_flatten(const float* curved, const Grid& g, const double* d_dsd, int 
 int launch_fdk_filter_taps(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, int nViews, const float* d_taps,
                            const float* d_colw, float* q, cudaStream_t st, bool odd_only) {
     ProfScope ps(PK_EW, st);
-    const int nuC = (g.nu + FR - 1) / FR * FR;
-    const int PAD = nuC + 2 * FR;                   // zero padding on each side (multiple of FR)
+    // odd_only: two half-rows of ceil(nu / 2) elements; otherwise one row of nu
+    const int len = odd_only ? (g.nu + 1) / 2 : g.nu;
+    const int nuC = (len + FR - 1) / FR * FR;
+    const int PAD = nuC + 3 * FR;                   // zero padding on each side (multiple of FR)
     int PL = (nuC + 2 * PAD) / FR;                  // words per plane
     PL += (PL % 32 == 1) ? 0 : ((33 - PL % 32) % 32);   // = 1 mod 32: the fill of the planes is then conflict-free as well
     const int NT = nuC + 2 * FR;                    // taps incl. the overshoot of the last block, multiple of 4
-    const size_t smem = ((size_t)NT + (size_t)FR * PL) * sizeof(float);
+    const size_t smem = ((size_t)NT + (size_t)(odd_only ? 2 : 1) * FR * PL) * sizeof(float);
     if (smem > 200 * 1024) return TIGRE_ERR_ARG;
     auto kern = odd_only ? fdk_conv_kernel<true> : fdk_conv_kernel<false>;
     if (smem > 48 * 1024) TG_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
