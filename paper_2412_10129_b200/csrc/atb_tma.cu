@@ -166,7 +166,6 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
         const float V0 = fmaf(rV.x, cxf, fmaf(rV.y, cyf, fmaf(rV.z, czf, rV.w)));
         const float W0 = fmaf(rW.x, cxf, fmaf(rW.y, cyf, fmaf(rW.z, czf, rW.w)));
         const float G0 = fmaf(rG.x, cxf, fmaf(rG.y, cyf, fmaf(rG.z, czf, rG.w)));
-        const float* tile = tiles + (size_t)s * stageElems;
         if (!fits) {
             // footprint larger than the staged box: gather this view through L1/L2 (bounds-checked, clamped)
             if (active) {
@@ -232,16 +231,52 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
                 }
             }
         } else {
-            const int ushift = -c0, vshift = -c1;   // voxel_view returns absolute detector indices
+            // general view (tilted detector): U, V, W all vary along the z-run, so each voxel has its own reciprocal.
+            // (1) the -1/2 of floor_magic is folded into the rows: fu - 1/2 = (U - W/2) t, so round(fu - 1/2) + magic is ONE
+            //     FFMA, and au = (U - W/2) t + (1/2 - round) another;
+            // (2) both tap indices enter the address as the raw bits of those sums (two integer multiply-adds; the biases
+            //     are folded into `col` as in the branch above);
+            // (3) matched weight: eu = fu - fus = Eu t with Eu = U - fus W linear in k, so
+            //     sx2 + du^2 eu^2 + dv^2 ev^2 = t^2 Q(k), Q = sx2 W^2 + du^2 Eu^2 + dv^2 Ev^2 quadratic in k (Horner), w = km t^3 sqrt(Q).
+            const float Uh = fmaf(-0.5f, W0, U0), Vh = fmaf(-0.5f, W0, V0);
+            const float dUh = fmaf(-0.5f, rW.z, rU.z), dVh = fmaf(-0.5f, rW.z, rV.z);
+            float qA = 0.f, qB = 0.f, qC = 0.f;
+            if (MODE != TIGRE_ATB_FDK) {
+                const float Eu = fmaf(-cst.z, W0, U0), Ev = fmaf(-cst.w, W0, V0);
+                const float dEu = fmaf(-cst.z, rW.z, rU.z), dEv = fmaf(-cst.w, rW.z, rV.z);
+                const float sW = cst.y * W0, sdW = cst.y * rW.z;
+                qA = fmaf(p.du2 * Eu, Eu, fmaf(p.dv2 * Ev, Ev, sW * W0));
+                qB = 2.f * fmaf(p.du2 * Eu, dEu, fmaf(p.dv2 * Ev, dEv, sW * rW.z));
+                qC = fmaf(p.du2 * dEu, dEu, fmaf(p.dv2 * dEv, dEv, sdW * rW.z));
+            }
+            const uint32_t col = tiles_s + (uint32_t)(s * stageElems + (p.hu - c0) + (p.hv - c1) * BU) * 4u -
+                                 (uint32_t)p.magic * (uint32_t)(BU * 4 + 4);
 #pragma unroll
             for (int k = 0; k < ZR; ++k) {
                 const float kf = (float)k;
-                const TapW tw = voxel_view<MODE, false>(fmaf(kf, rU.z, U0), fmaf(kf, rV.z, V0), fmaf(kf, rW.z, W0),
-                                                        fmaf(kf, rG.z, G0), cst, p);
-                const float* q = tile + (tw.iv + vshift) * BU + (tw.iu + ushift);
-                const float p00 = q[0], p10 = q[1], p01 = q[BU], p11 = q[BU + 1];
-                const float r0 = fmaf(tw.au, p10 - p00, p00), r1 = fmaf(tw.au, p11 - p01, p01);
-                acc[k] = fmaf(tw.w, fmaf(tw.av, r1 - r0, r0), acc[k]);
+                const float t = rcp_fast(fmaf(kf, rW.z, W0));
+                const float Uk = fmaf(kf, dUh, Uh), Vk = fmaf(kf, dVh, Vh);
+                const float tmu = fmaf(Uk, t, 12582912.0f), tmv = fmaf(Vk, t, 12582912.0f);
+                const float au = fmaf(Uk, t, 0.5f - (tmu - 12582912.0f)), av = fmaf(Vk, t, 0.5f - (tmv - 12582912.0f));
+                const uint32_t q = col + __float_as_uint(tmv) * (uint32_t)(BU * 4) + __float_as_uint(tmu) * 4u;
+                float p00, p10, p01, p11;
+                asm volatile(
+                    "ld.shared.f32 %0, [%4];\n\t"
+                    "ld.shared.f32 %1, [%4+4];\n\t"
+                    "ld.shared.f32 %2, [%4+%5];\n\t"
+                    "ld.shared.f32 %3, [%4+%6];"
+                    : "=f"(p00), "=f"(p10), "=f"(p01), "=f"(p11)
+                    : "r"(q), "n"(BU * 4), "n"(BU * 4 + 4));
+                const float r0 = fmaf(au, p10 - p00, p00), r1 = fmaf(au, p11 - p01, p01);
+                const float val = fmaf(av, r1 - r0, r0);
+                float w;
+                if (MODE == TIGRE_ATB_FDK) {
+                    const float ig = rcp_fast(fmaf(kf, rG.z, G0));
+                    w = ig * ig;
+                } else {
+                    w = ((cst.x * t) * (t * t)) * sqrt_fast(fmaf(fmaf(qC, kf, qB), kf, qA));
+                }
+                acc[k] = fmaf(w, val, acc[k]);
             }
         }
         __syncwarp();
