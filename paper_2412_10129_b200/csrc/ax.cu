@@ -493,53 +493,82 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
         atomicAdd(q + pitchZ, (1.f - ax) * w01), atomicAdd(q + pitchZ + 1, ax * w01);
         atomicAdd(q + pitchZ + pitchY, (1.f - ax) * w11), atomicAdd(q + pitchZ + pitchY + 1, ax * w11);
     };
-    // samples [k, kend): the checked ends of the ray around the unchecked interior [kA, kB)
-    auto run = [&](int& k, int kend) {
-        if (UNIT) {
-            for (; k < kend; ++k) checked(k);
-            return;
-        }
-        const int e1 = min(kend, r.kA);
-        for (; k < e1; ++k) checked(k);
-        const int e2 = min(kend, r.kB);
-        if (k < e2) {
+    // bounds-checked sample without branches (gather only): every tap index is tested once per axis; an outside tap gets
+    // weight zero and a clamped (valid) address
+    auto edge = [&](int k) {
+        const float t = (float)k + 0.5f;
+        const float x = fmaf(t, r.sx, r.x0), y = fmaf(t, r.sy, r.y0), z = fmaf(t, r.sz, r.z0);
+        const float mx = (x - 0.5f) + 12582912.0f, my = (y - 0.5f) + 12582912.0f, mz = (z - 0.5f) + 12582912.0f;
+        const float ax = x - (mx - 12582912.0f), ay = y - (my - 12582912.0f), az = z - (mz - 12582912.0f);
+        // array indices of the lower taps (relative to the first slice present; may be out of range)
+        const int jx = __float_as_int(mx) - 0x4B400000 + hx, jy = __float_as_int(my) - 0x4B400000 + hy,
+                  jz = __float_as_int(mz) - 0x4B400000 + hz - p.zs0;
+        const unsigned ex = (unsigned)(nX - 1), ey = (unsigned)(nY - 1), ez = (unsigned)(p.zs1 - p.zs0 - 1);
+        const bool x0 = (unsigned)jx <= ex, x1 = (unsigned)(jx + 1) <= ex;
+        const bool y0 = (unsigned)jy <= ey, y1 = (unsigned)(jy + 1) <= ey;
+        const bool z0 = (unsigned)jz <= ez, z1 = (unsigned)(jz + 1) <= ez;
+        const float wx0 = x0 ? 1.f - ax : 0.f, wx1 = x1 ? ax : 0.f;
+        const float wy0 = y0 ? 1.f - ay : 0.f, wy1 = y1 ? ay : 0.f;
+        const float wz0 = z0 ? 1.f - az : 0.f, wz1 = z1 ? az : 0.f;
+        const int cx0 = x0 ? jx : 0, cx1 = x1 ? jx + 1 : 0;
+        const IdxT oy0 = (IdxT)(y0 ? jy : 0) * pitchY, oy1 = (IdxT)(y1 ? jy + 1 : 0) * pitchY;
+        const IdxT oz0 = (IdxT)(z0 ? jz : 0) * pitchZ, oz1 = (IdxT)(z1 ? jz + 1 : 0) * pitchZ;
+        const float *r00 = base + (oz0 + oy0), *r10 = base + (oz0 + oy1), *r01 = base + (oz1 + oy0), *r11 = base + (oz1 + oy1);
+        const float c00 = fmaf(wx1, __ldg(r00 + cx1), wx0 * __ldg(r00 + cx0)), c10 = fmaf(wx1, __ldg(r10 + cx1), wx0 * __ldg(r10 + cx0));
+        const float c01 = fmaf(wx1, __ldg(r01 + cx1), wx0 * __ldg(r01 + cx0)), c11 = fmaf(wx1, __ldg(r11 + cx1), wx0 * __ldg(r11 + cx0));
+        const float c0 = fmaf(wy1, c10, wy0 * c00), c1 = fmaf(wy1, c11, wy0 * c01);
+        acc += fmaf(wz1, c1, wz0 * c0);
+    };
+    // unchecked samples [k, kend) of the interior [kA, kB)
+    auto inner = [&](int& k, int kend) {
+        if (k < kend) {
             float t = (float)k + 0.5f;
-            for (; k < e2; ++k, t += 1.f) {
+            for (; k < kend; ++k, t += 1.f) {
                 if (SCATTER) interior_scatter(t);
                 else interior(t);
             }
         }
-        for (; k < kend; ++k) checked(k);
     };
 
     // The samples of a ray are fixed by the definition (l_in + (k+1/2) delta from ITS entry point), but the
     // order in which a warp visits them is free.  Neighbouring rays enter the volume at different depths, so
     // visiting sample k of every lane together scatters the warp over many rows of the volume.  Instead the
     // warp advances along Y (the in-plane axis the rays run along) two rows at a time: in each step every
-    // lane takes the samples of its own ray that fall into the current pair of rows (4 or 5 of them at a
+    // lane takes the INTERIOR samples of its own ray that fall into the current pair of rows (4 or 5 of them at a
     // step of half a voxel, so the lanes' trip counts differ by at most one in five), and all lanes stay
-    // within three adjacent rows of the (transposed) volume.
-    int k = r.k0;
-    const bool live = r.Kuse > r.k0, up = r.sy >= 0.f;
+    // within three adjacent rows of the (transposed) volume.  The few bounds-checked samples at the two ends of each ray
+    // ([k0, kA) and [kB, Kuse)) are left out of the march and taken afterwards by all lanes together: inside the march
+    // they ran a lane or three at a time (rays of one warp enter and leave the volume in different rows) and cost a
+    // quarter of the kernel's issue slots.
+    int k = r.kA;
+    const bool live = r.kB > r.kA, up = r.sy >= 0.f;
     const unsigned liveM = __ballot_sync(wmask, live), upM = __ballot_sync(wmask, live && up);
     const bool steep = fabsf(r.sy) > 0.05f * (fabsf(r.sx) + fabsf(r.sz));
     const bool lock = liveM != 0 && (upM == liveM || upM == 0) && __ballot_sync(wmask, live && !steep) == 0;
     if (lock) {
         const bool wup = upM != 0;
         const float isy = live ? 1.0f / r.sy : 0.f, cc = live ? fmaf(-r.y0, isy, -0.5f) : 0.f;
-        const int j0 = live ? (int)floorf(fmaf((float)r.k0 + 0.5f, r.sy, r.y0)) : (wup ? 0x7fffffff : (int)0x80000000);
+        const int j0 = live ? (int)floorf(fmaf((float)r.kA + 0.5f, r.sy, r.y0)) : (wup ? 0x7fffffff : (int)0x80000000);
         const int jw = wup ? __reduce_min_sync(wmask, j0) : __reduce_max_sync(wmask, j0);
         float Yb = wup ? (float)jw + 2.f : (float)jw - 1.f;   // far side of the current rows in the direction of travel
         const float dY = wup ? 2.f : -2.f;
         for (int it = 0; it < nY / 2 + 8; ++it) {
             const float kf = ceilf(fmaf(Yb, isy, cc));
-            const int kend = live ? (int)fminf(fmaxf(kf, (float)k), (float)r.Kuse) : k;
-            run(k, kend);
+            const int kend = live ? (int)fminf(fmaxf(kf, (float)k), (float)r.kB) : k;
+            inner(k, kend);
             Yb += dY;
-            if (!__any_sync(wmask, k < r.Kuse)) break;
+            if (!__any_sync(wmask, k < r.kB)) break;
         }
     }
-    run(k, r.Kuse);   // rays not marched in lockstep (mixed directions, rays across Y), leftovers
+    inner(k, r.kB);   // rays not marched in lockstep (mixed directions, rays across Y), leftovers
+    for (int q = r.k0; q < r.kA; ++q) {
+        if (UNIT || SCATTER) checked(q);
+        else edge(q);
+    }
+    for (int q = r.kB; q < r.Kuse; ++q) {
+        if (UNIT || SCATTER) checked(q);
+        else edge(q);
+    }
     if (!SCATTER) {
         const float result = acc * (float)p.delta;
         proj[out] = p.accumulate ? proj[out] + result : result;
