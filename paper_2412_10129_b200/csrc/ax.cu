@@ -20,6 +20,8 @@
 //   AXMB   CTAs per SM of the Siddon kernel: 9 (56 registers); 5-6 / 7 / 8 / 10 / 12 / 16 give 986 / 1093 / 1139 / 1149 / 1130 / 1071
 //          against 1165 G samples/s
 //   AXIMB  CTAs per SM of the interpolated kernel: 8 (64 registers); 9 the same, 10 and 12 spill and lose 9-12 %
+//   AXI_ROWS  rows of the volume per lockstep step of the interpolated kernel: 8; 2 / 3 / 4 / 6 / 12 / 16 / 32 give 318 / 323 / 342 / 342 /
+//          345 / 347 / 318 against 352 G samples/s on C2 (C3-sized: 405 / 411 / 443 / 452 / 465 / 464 / 455 against 459)
 //   AXTV   detector rows per CTA (tile = 32 x AXTV pixels): 4; 1, 2 and 8 lose 0.3-4 %
 #ifndef AXIMB
 #define AXIMB 8
@@ -44,6 +46,7 @@ struct AxP {
 #define AXTV 4
 #endif
 constexpr int AX_TU = 32, AX_TV = AXTV;
+constexpr int AXI_ROWS = 8;
 
 __device__ __forceinline__ double sel3(int k, double a, double b, double c) { return k == 0 ? a : (k == 1 ? b : c); }
 
@@ -533,10 +536,11 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     // The samples of a ray are fixed by the definition (l_in + (k+1/2) delta from ITS entry point), but the
     // order in which a warp visits them is free.  Neighbouring rays enter the volume at different depths, so
     // visiting sample k of every lane together scatters the warp over many rows of the volume.  Instead the
-    // warp advances along Y (the in-plane axis the rays run along) two rows at a time: in each step every
-    // lane takes the INTERIOR samples of its own ray that fall into the current pair of rows (4 or 5 of them at a
-    // step of half a voxel, so the lanes' trip counts differ by at most one in five), and all lanes stay
-    // within three adjacent rows of the (transposed) volume.  The few bounds-checked samples at the two ends of each ray
+    // warp advances along Y (the in-plane axis the rays run along) AXI_ROWS rows at a time: in each step every
+    // lane takes the INTERIOR samples of its own ray that fall into the current rows (16 to 23 of them at a
+    // step of half a voxel; the lanes' trip counts differ by at most one), and all lanes stay within AXI_ROWS + 1
+    // adjacent rows of the (transposed) volume.  (Two rows per step, the first design, kept the footprint smallest but
+    // lost one trip in five to the uneven counts and paid the step's overhead every 4-5 samples.)  The few bounds-checked samples at the two ends of each ray
     // ([k0, kA) and [kB, Kuse)) are left out of the march and taken afterwards by all lanes together: inside the march
     // they ran a lane or three at a time (rays of one warp enter and leave the volume in different rows) and cost a
     // quarter of the kernel's issue slots.
@@ -550,9 +554,9 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
         const float isy = live ? 1.0f / r.sy : 0.f, cc = live ? fmaf(-r.y0, isy, -0.5f) : 0.f;
         const int j0 = live ? (int)floorf(fmaf((float)r.kA + 0.5f, r.sy, r.y0)) : (wup ? 0x7fffffff : (int)0x80000000);
         const int jw = wup ? __reduce_min_sync(wmask, j0) : __reduce_max_sync(wmask, j0);
-        float Yb = wup ? (float)jw + 2.f : (float)jw - 1.f;   // far side of the current rows in the direction of travel
-        const float dY = wup ? 2.f : -2.f;
-        for (int it = 0; it < nY / 2 + 8; ++it) {
+        float Yb = wup ? (float)(jw + AXI_ROWS) : (float)(jw + 1 - AXI_ROWS);   // far side of the current rows in the direction of travel
+        const float dY = wup ? (float)AXI_ROWS : -(float)AXI_ROWS;
+        for (int it = 0; it < nY / AXI_ROWS + 8; ++it) {
             const float kf = ceilf(fmaf(Yb, isy, cc));
             const int kend = live ? (int)fminf(fmaxf(kf, (float)k), (float)r.kB) : k;
             inner(k, kend);
