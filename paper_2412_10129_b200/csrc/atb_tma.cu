@@ -2,8 +2,9 @@
 // TMA (BASELINE.json north_star: "each batch's detector footprint is staged into shared memory by TMA,
 // and accumulation stays in registers"; DESIGN.md O-C for what is computed).
 //
-// A CTA owns a tile of 32 x 16 x 16 voxels: 4 x 4 consumer warps, each 8 (x) x 4 (y) columns of voxels, every
-// thread the 16 voxels along z of one column, their sums in registers over all views.  One extra PRODUCER
+// A CTA owns a tile of 32 x 12 x 32 voxels: 4 x 3 consumer warps, each 8 (x) x 4 (y) columns of voxels, every
+// thread the 32 voxels along z of one column, their sums in registers over all views (thin slabs: 4 x 4 warps,
+// 16 voxels along z).  One extra PRODUCER
 // warp walks the views ahead of the consumers: for each view it projects the 8 corner voxels of the tile (the
 // projective map is quasi-linear, so they bound the footprint), and issues ONE cp.async.bulk.tensor load of
 // the BU x BV pixel box around it into a ring of shared-memory stages (mbarrier full/empty pairs), together
@@ -73,7 +74,7 @@ extern int g_atb_path;   // atb.cu
 // launcher picks the smallest of 48, 80, ... 240 (all = 16 mod 32: with the 8 x 4 lane layout below, the taps
 // of one warp span < 16 columns of at most a few adjacent rows, and rows 16 banks apart do not collide).
 template <int MODE, int WX, int WY, int ZR, int BU>
-__global__ void __launch_bounds__(32 * (WX * WY + 1), (WX * WY >= 16 ? 2 : 3))
+__global__ void __launch_bounds__(32 * (WX * WY + 1), 2)
 atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict__ proj, const VoxView* __restrict__ views,
                int nViews, AtbP p, int BV, int nStages, float* __restrict__ vol) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -426,8 +427,16 @@ int launch_atb_tma(const float* proj, const Grid& g, const VoxView* d_views, con
     EncodeTiledFn enc = encode_fn();
     if (!enc || !h_views || !proj) return 1;
     if ((g.nu & 3) || (reinterpret_cast<uintptr_t>(proj) & 15) || p.nrows < 1) return 1;   // TMA: 16-byte rows and base
-    // tile = 4 x 4 consumer warps of 8 x 4 voxel columns, 16 voxels along z per thread (32 x 16 x 16 voxels per CTA,
-    // 2 CTAs per SM): the best of the configurations measured on C2, C3 and C4 (profiles/r1_atb_tma.md)
+    // tile = 4 x 3 consumer warps of 8 x 4 voxel columns, 32 voxels along z per thread (32 x 12 x 32 voxels per CTA, 13 warps,
+    // 2 CTAs per SM): the per-view work of a thread (table entry, projective map of its column, weights, barrier round trip) is
+    // spread over 32 voxels instead of 16.  Measured on C3 / C2 / C4 (profiles/r1_atb_tma.md): 1160 / 1204 / 861 GUPS against
+    // 950 / 918 / 818 for the former 4 x 4 x 16 tile, which stays for thin slabs: there a 32-voxel run would be mostly empty
+    // (chosen when the z-extent rounded up to 32 exceeds 1.2 x the z-extent rounded up to 16).
+    const int up32 = (p.nzs + 31) / 32 * 32, up16 = (p.nzs + 15) / 16 * 16;
+    if (up32 * 10 <= up16 * 12) {
+        const int rc = tma_config<4, 3, 32>(enc, proj, g, d_views, h_views, nViews, mode, p, vol, st);
+        if (rc != 1) return rc;   // launched, or a CUDA error; 1 = the taller footprint does not fit a stage: try the flatter tile
+    }
     return tma_config<4, 4, 16>(enc, proj, g, d_views, h_views, nViews, mode, p, vol, st);
 }
 

@@ -317,10 +317,15 @@ def _tma_geometries():
                   rotDetector=(0.05, -0.04, 0.08))
     ab = np.stack([rng.uniform(0, 2 * np.pi, nA), rng.uniform(-0.4, 0.4, nA), rng.uniform(-0.5, 0.5, nA)], 1)
     gb.rotDetector_a = np.asarray(gb.rotDetector) + 0.03 * rng.standard_normal((nA, 3))
-    return [(ga, aa), (gb, ab)]
+    # (c), (d) z-extents 16 and 40: the thin-slab tile (16 voxels along z per thread) instead of the 32-voxel one of (a), (b);
+    #     (d) with a ragged last z-block and the tilted views of (b)
+    gc = Geometry(nVoxel=(40, 36, 16), dVoxel=(1.0, 1.0, 1.1), nDetector=(64, 28), dDetector=(1.5, 1.5),
+                  DSD=600.0, DSO=380.0, offDetector=(-4.0, 2.0))
+    gd = gb.copy(nVoxel=(41, 33, 40))
+    return [(ga, aa), (gb, ab), (gc, circular_angles(9, start=0.4)), (gd, ab)]
 
 
-@pytest.mark.parametrize("case", [0, 1])
+@pytest.mark.parametrize("case", [0, 1, 2, 3])
 @pytest.mark.parametrize("mode,tol", [("matched", 1e-5), ("fdk", 1e-4)])
 def test_atb_tma_and_gather_kernels_match_oracle(tg, case, mode, tol):
     geo, ang = _tma_geometries()[case]
