@@ -8,6 +8,9 @@
 //  of a slab are formed branch-free.  This keeps the 32 lanes of a warp in lock step (same slab
 //  index, neighbouring voxels -> few L1 wavefronts per gather) and makes the trip count uniform.
 //  The sum of the lengths is exactly the Siddon sum: only the order of summation differs.
+//  The lanes of a warp share a detector row, so they cross the z-planes (rarely, and) in nearly the same slabs: the
+//  interior runs in warp-uniform groups of AXG slabs, and a group in which no lane crosses a z-plane (one vote) takes
+//  a two-voxel slab step with a third fewer instructions and bitwise the same sum.
 //  Per-ray set-up (entry/exit, slopes, first slab) is fp64; the march is fp32 with positions
 //  recomputed from the integer slab counter (never accumulated) in volume-centred coordinates.
 //
@@ -19,6 +22,9 @@
 // Launch configuration, overridable with -D for sweeps (measured on C3 / C2 / C4):
 //   AXMB   CTAs per SM of the Siddon kernel: 9 (56 registers); 5-6 / 7 / 8 / 10 / 12 / 16 give 986 / 1093 / 1139 / 1149 / 1130 / 1071
 //          against 1165 G samples/s
+//          (before the voted groups below); with them 8 / 9 / 10 give 1364 / 1359 / 1337 at AXG 4 and 7 / 8 / 9 give 1327 / 1347 / 1397 at AXG 6
+//   AXG    slabs per warp-voted group of the Siddon march (see the kernel): 6; 2 / 3 / 4 / 8 gave 1224 / 1252 / 1293 / 1245 before the
+//          second load of a slab was predicated, 4 / 5 / 6 / 7 / 8 give 1359 / 1346 / 1397 / 1342 / 1361 G samples/s with it (C3)
 //   AXIMB  CTAs per SM of the interpolated kernel: 8 (64 registers); 9 the same, 10 and 12 spill and lose 9-12 %
 //   AXI_ROWS  rows of the volume per lockstep step of the interpolated kernel: 8; 2 / 3 / 4 / 6 / 12 / 16 / 32 give 318 / 323 / 342 / 342 /
 //          345 / 347 / 318 against 352 G samples/s on C2 (C3-sized: 405 / 411 / 443 / 452 / 465 / 464 / 455 against 459)
@@ -28,6 +34,9 @@
 #endif
 #ifndef AXMB
 #define AXMB 9
+#endif
+#ifndef AXG
+#define AXG 6
 #endif
 namespace tg {
 
@@ -99,7 +108,8 @@ __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base,
         atomicAdd(out + offC, (1.0f - s2) * r.ys);
     } else {
         const float vA = UNIT ? 1.f : __ldg(base + r.off);
-        const float vC = UNIT ? 1.f : __ldg(base + offC);
+        float vC = vA;   // a lane that stays in its voxel does not load it twice
+        if (!UNIT && (cE || cF)) vC = __ldg(base + offC);
         r.acc = fmaf(s1, vA, r.acc);
         // (the middle weight multiplies the last value loaded when this lane has no middle voxel: times zero)
         if (both && !UNIT) r.vB = __ldg(base + (r.off + ((se < sf) ? r.stE : r.stF)));
@@ -108,6 +118,29 @@ __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base,
     }
     if (cE) r.hE += r.sgE;
     if (cF) r.hF += r.sgF;
+    r.off = offC + r.sD;
+}
+
+// One interior D-slab of a ray that is known not to cross an F-plane in it (sf = 1 in siddon_slab_fast): the same two
+// lengths and the same operations on them as there, without the middle voxel and the F bookkeeping (bitwise the same sum).
+template <typename IdxT, bool UNIT, bool SCATTER>
+__device__ __forceinline__ void siddon_slab_e_only(const float* __restrict__ base, SidRay<IdxT>& r) {
+    const float se = __saturatef(fmaf(r.hE, r.imE, -r.kf));
+    r.kf += 1.0f;
+    const bool cE = se < 1.0f;
+    const IdxT offC = r.off + (cE ? r.stE : (IdxT)0);
+    if (SCATTER) {
+        float* out = const_cast<float*>(base);
+        atomicAdd(out + r.off, se * r.ys);
+        atomicAdd(out + offC, (1.0f - se) * r.ys);
+    } else {
+        const float vA = UNIT ? 1.f : __ldg(base + r.off);
+        float vC = vA;   // a lane that stays in its voxel does not load it twice (the L1 data pipe is co-critical)
+        if (!UNIT && cE) vC = __ldg(base + offC);
+        r.acc = fmaf(se, vA, r.acc);
+        r.acc = fmaf(1.0f - se, vC, r.acc);
+    }
+    if (cE) r.hE += r.sgE;
     r.off = offC + r.sD;
 }
 
@@ -167,7 +200,9 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     const double Lmm = sqrt(d[0] * p.hxd * d[0] * p.hxd + d[1] * p.hyd * d[1] * p.hyd + d[2] * p.hzd * d[2] * p.hzd);
     const double a0 = fabs(d[0]), a1 = fabs(d[1]), a2 = fabs(d[2]);
     const int D = (a0 >= a1 && a0 >= a2) ? 0 : (a1 >= a2 ? 1 : 2);
-    const int E = (D + 1) % 3, F = (D + 2) % 3;
+    // F is the z axis unless the ray itself runs along z: along a detector row (= a warp) the rays cross the z-planes in nearly
+    // the same slabs, which the march below uses
+    const int E = D == 0 ? 1 : 0, F = D == 2 ? 1 : 2;
     const double dD = sel3(D, d[0], d[1], d[2]), dE = sel3(E, d[0], d[1], d[2]), dF = sel3(F, d[0], d[1], d[2]);
     const double SD = sel3(D, S[0], S[1], S[2]), SE = sel3(E, S[0], S[1], S[2]), SF = sel3(F, S[0], S[1], S[2]);
     const int nD = D == 0 ? p.nx : (D == 1 ? p.ny : p.nz);
@@ -267,9 +302,10 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     // unchecked slabs at its own first one, the warp would be spread over many rows of the volume.  So the head
     // (clipped, bounds-checked slabs) of each lane is stretched to the deepest start in the warp: from there on
     // all lanes are in the SAME absolute slab in every iteration of the interior loop.
+    int jmax;
     {
         const bool any = kB > kA;
-        const int jmax = __reduce_max_sync(wmask, any ? i0 + kA : (int)0x80000000);
+        jmax = __reduce_max_sync(wmask, any ? i0 + kA : (int)0x80000000);
         if (any) kA = min(max(kA, jmax - i0), kB);
     }
     const int last = nslab - 1;
@@ -277,6 +313,28 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     for (; k < kA; ++k)
         siddon_slab_checked<IdxT, UNIT, SCATTER>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
     const bool ranFast = kB > k;
+    {
+        // Warp-uniform part of the interior: groups of AXG slabs up to the shallowest end in the warp.  The lanes of a warp share a
+        // detector row, so they meet the (rare) z-plane crossings in nearly the same slabs: one vote per group tells whether ANY
+        // lane crosses an F-plane in its next AXG slabs (next crossing at hF/mF - k <= AXG slabs ahead; "<=" is conservative under the
+        // rounding of that FFMA); if none does, the group runs the two-voxel slab.  All lanes with interior slabs are at absolute
+        // slab jmax here.
+        const int jendmin = __reduce_min_sync(wmask, ranFast ? i0 + kB : 0x7fffffff);
+        const int groups = jendmin == 0x7fffffff ? 0 : (jendmin - jmax) / AXG;
+        for (int g = 0; g < groups; ++g) {
+            const bool nearF = ranFast && fmaf(r.hF, r.imF, -r.kf) <= (float)AXG;
+            if (__any_sync(wmask, nearF)) {
+                if (ranFast) {
+#pragma unroll
+                    for (int j = 0; j < AXG; ++j) siddon_slab_fast<IdxT, UNIT, SCATTER>(base, r);
+                }
+            } else if (ranFast) {
+#pragma unroll
+                for (int j = 0; j < AXG; ++j) siddon_slab_e_only<IdxT, UNIT, SCATTER>(base, r);
+            }
+        }
+        if (ranFast) k += AXG * groups;
+    }
     for (; k < kB; ++k) siddon_slab_fast<IdxT, UNIT, SCATTER>(base, r);
     if (k < nslab) {
         // recover the cell indices from the plane state for the checked tail: hE has moved by one per crossing
