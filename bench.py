@@ -56,7 +56,7 @@ def model_peak(kname, sm_mhz):
 
 # dram__bytes_read+write per launch of the dominant kernel from the committed ncu captures (profiles/), for
 # the default workload only (C3, one ordered subset = 36 views per launch)
-NCU_TRAFFIC_PER_LAUNCH = {("C3", "ax_siddon"): 2.557e9, ("C3", "atb"): 5.97e8, ("C2", "ax_interp"): 4.58e8}
+NCU_TRAFFIC_PER_LAUNCH = {("C3", "ax_siddon"): 2.338e9, ("C3", "atb"): 6.11e8, ("C2", "ax_interp"): 4.58e8}
 
 
 def max_over_ranks(ms, device="cpu"):
