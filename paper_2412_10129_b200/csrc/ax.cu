@@ -28,7 +28,7 @@
 //   AXIMB  CTAs per SM of the interpolated kernel: 8 (64 registers); 9 the same, 10 and 12 spill and lose 9-12 %
 //   AXI_ROWS  rows of the volume per lockstep step of the interpolated kernel: 8; 2 / 3 / 4 / 6 / 12 / 16 / 32 give 318 / 323 / 342 / 342 /
 //          345 / 347 / 318 against 352 G samples/s on C2 (C3-sized: 405 / 411 / 443 / 452 / 465 / 464 / 455 against 459)
-//   AXTV   detector rows per CTA (tile = 32 x AXTV pixels): 4; 1, 2 and 8 lose 0.3-4 %
+//   AXTV   detector rows per CTA (tile = 32 x AXTV pixels): 4; 1, 2 and 8 lose 0.3-4 % (with the voted groups: 2 rows x 18 CTAs 1390, 8 rows x 4 / 5 CTAs 1331 / 1339 against 1397)
 #ifndef AXIMB
 #define AXIMB 8
 #endif
