@@ -133,13 +133,16 @@ def fdk_filter(proj, geo, angles, filt="ram_lak", colw=None):
     DSO = _per_view(geo, "DSO", geo.DSO, nA)
     u = (np.arange(nu) + 0.5) * du - 0.5 * nu * du
     v = (np.arange(nv) + 0.5) * dv - 0.5 * nv * dv
+    offa = getattr(geo, "offDetector_a", None)
+    offD = np.broadcast_to(np.asarray(geo.offDetector, dtype=np.float64), (nA, 2)) if offa is None else np.asarray(offa, dtype=np.float64).reshape(nA, 2)
     p = np.asarray(proj, dtype=np.float64).reshape(nA, nv, nu)
     out = np.zeros_like(p)
     L = pad_length(nu)
     par = getattr(geo, "mode", "cone") == "parallel"       # P29: no magnification, no cosine weight
     for a in range(nA):
         tau = du if par else du * DSO[a] / DSD[a]
-        cosw = 1.0 if par else DSD[a] / np.sqrt(DSD[a] ** 2 + u[None, :] ** 2 + v[:, None] ** 2)
+        # P34: (u, v) of the cosine weight are measured from the principal ray, i.e. include offDetector
+        cosw = 1.0 if par else DSD[a] / np.sqrt(DSD[a] ** 2 + (u[None, :] + offD[a, 0]) ** 2 + (v[:, None] + offD[a, 1]) ** 2)
         row = p[a] * cosw
         if colw is not None:
             row = row * colw[a][None, :]

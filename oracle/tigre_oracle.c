@@ -23,7 +23,8 @@
  *   atb (fdk / matched)  pinned: proj==1 closed form of the weights, linear projections,
  *                          delta-pixel brute force, normalisation against the exact transpose.
  *   atb_exact_*    pinned: <Ax,y> = <x,A^T y> to 1e-12.
- *   fdk_filter     pinned: reconstruction of an analytic ball returns rho.
+ *   fdk_filter     pinned: reconstruction of an analytic ball returns rho; impulse response = tau * cos * Ram-Lak taps with
+ *                          the cosine from independent geometry (also with a displaced detector); wide-fan ball needs it.
  *
  * Layout: vol[iz][iy][ix] (x fastest), proj[ia][iv][iu] (u fastest).  Inputs may be
  * float32 or float64 (flag); all arithmetic and all outputs are float64.
@@ -525,7 +526,9 @@ int orc_atb(const void *proj, int proj_f32, int unit_proj, const orc_grid *g, co
 /* ---------------------------------------------------------------- O-D  FDK pre-filter (P12) */
 /* per projection: p1 = p * DSD/sqrt(DSD^2+u^2+v^2); q = tau * (p1 * h) along u, direct linear
  * convolution with zero padding, tau = du*DSO/DSD, h[0]=1/(4 tau^2), h[odd n] = -1/(pi n tau)^2.
- * (u,v) are the detector-local pixel-centre coordinates. */
+ * (u,v) are measured from the foot of the source's perpendicular on the detector plane (the principal ray of the
+ * textbook derivation [24]): detector-local pixel-centre coordinates PLUS offDetector (reading P34; the weight is the
+ * cosine between the ray and the detector normal; rotDetector is not taken into it). */
 int orc_fdk_filter(const void *proj, int proj_f32, const orc_grid *g, const orc_view *views, int nA,
                    double *out) {
     arr_t Y = {proj, proj_f32};
@@ -538,10 +541,10 @@ int orc_fdk_filter(const void *proj, int proj_f32, const orc_grid *g, const orc_
             for (int iv = 0; iv < nv; iv++) {
                 const orc_view *w = &views[ia];
                 double tau = g->parallel ? g->du : g->du * w->DSO / w->DSD; /* P29: no magnification */
-                double v = (iv + 0.5) * g->dv - 0.5 * nv * g->dv;
+                double v = (iv + 0.5) * g->dv - 0.5 * nv * g->dv + w->offD[1];
                 size_t base = ((size_t)ia * nv + iv) * nu;
                 for (int iu = 0; iu < nu; iu++) {
-                    double u = (iu + 0.5) * g->du - 0.5 * nu * g->du;
+                    double u = (iu + 0.5) * g->du - 0.5 * nu * g->du + w->offD[0];
                     row[iu] = LD(Y, base + iu) * (g->parallel ? 1.0 : w->DSD / sqrt(w->DSD * w->DSD + u * u + v * v));
                 }
                 for (int iu = 0; iu < nu; iu++) {

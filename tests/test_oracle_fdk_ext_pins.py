@@ -152,3 +152,85 @@ def test_displaced_detector_fdk_with_wang_weights_reconstructs_the_ball():
     assert abs(outside) < 0.1 * rho
     plain_in, _ = _ball_levels(fx.fdk(proj, geo, ang, "ram_lak", None), geo, rad, cen)
     assert abs(plain_in / rho - 1.0) > 0.1                       # truncated rows through the ramp filter: wrong level
+
+
+# ------------------------------------------------------------------ the cosine pre-weight of P12 / P34
+def _cosine_weight_from_geometry(geo, ang, ia, iu, iv):
+    """cos of the angle between the ray source -> pixel and the detector normal, from the independent WORLD-frame geometry of
+    tests/helpers.py: for an unrotated detector this is the textbook FDK pre-weight DSD / sqrt(DSD^2 + u^2 + v^2) with (u, v)
+    measured from the foot of the source's perpendicular on the detector."""
+    S, Dc, eu, ev, n, p = H.world_frame(geo, ang, ia)
+    _, P = H.pixel_world(geo, ang, ia, np.array([iu]), np.array([iv]))
+    d = P[0] - S
+    return abs(d @ n) / np.linalg.norm(d)
+
+
+@pytest.mark.parametrize("offD", [(0.0, 0.0), (25.0, -10.0)])
+def test_fdk_filter_impulse_response_pins_the_cosine_weight(offD):
+    """A single bright pixel far off the axis of a SHORT geometry (weight ~ 0.85): the filtered row is
+    tau * cos * h[n] (h the Ram-Lak taps of P12), every other row stays zero.  With a displaced detector the weight is
+    centred on the principal ray, not on the detector (reading P34)."""
+    nu, nv, du, dv = 40, 30, 4.0, 4.0
+    geo = Geometry(nVoxel=(8, 8, 8), dVoxel=(1.0,) * 3, nDetector=(nu, nv), dDetector=(du, dv), DSD=150.0, DSO=100.0,
+                   offDetector=offD)
+    ang = circular_angles(3, start=0.4)
+    tau = du * geo.DSO / geo.DSD
+    for ia, iu0, iv0 in ((1, 29, 26), (2, 2, 3), (0, 20, 15)):
+        p = np.zeros((3, nv, nu))
+        p[ia, iv0, iu0] = 1.0
+        cosw = _cosine_weight_from_geometry(geo, ang, ia, iu0, iv0)
+        u0 = (iu0 + 0.5) * du - 0.5 * nu * du + offD[0]
+        v0 = (iv0 + 0.5) * dv - 0.5 * nv * dv + offD[1]
+        assert cosw == pytest.approx(geo.DSD / np.sqrt(geo.DSD ** 2 + u0 ** 2 + v0 ** 2), rel=1e-13)
+        if (iu0, iv0) != (20, 15):
+            assert cosw < 0.95                                      # far from 1: a dropped weight is a >5 % error here
+        n = np.arange(nu) - iu0
+        h = np.where(n == 0, 1.0 / (4 * tau * tau), np.where(n % 2 != 0, -1.0 / (np.pi * np.where(n == 0, 1, n) * tau) ** 2, 0.0))
+        want = np.zeros((3, nv, nu))
+        want[ia, iv0] = tau * cosw * h
+        for got in (orc.fdk_filter(p, geo, ang), fx.fdk_filter(p, geo, ang, "ram_lak")):
+            assert np.allclose(got, want, rtol=0, atol=1e-12 * abs(want).max())
+
+
+def _wide_fan_problem(offu=0.0, nu=168):
+    # source 200 mm from the axis: short geometry, wide fan
+    geo = Geometry(nVoxel=(96, 96, 2), dVoxel=(1.5, 1.5, 1.0), nDetector=(nu, 4), dDetector=(2.5, 2.5), DSD=300.0, DSO=200.0,
+                   offDetector=(offu, 0.0))
+    ang = circular_angles(240)
+    rho, rad, cen = 0.02, 12.0, np.array([52.0, -25.0, 0.0])       # a small ball far off the axis: seen at fan angles up to 20 deg
+    return geo, ang, rho, rad, cen
+
+
+def _wide_levels(x, geo, rad, cen):
+    c = H.voxel_centres(geo, (0, 0, 0))
+    d = np.linalg.norm(c - cen, axis=-1)
+    return x[d < rad - 4.0].mean(), x[(d > rad + 4.0) & (d < rad + 9.0)].mean()
+
+
+def test_wide_fan_fdk_needs_the_cosine_weight():
+    """Mid-plane FDK is exact fan-beam FBP: an analytic ball seen under fan angles up to 20 degrees comes back at rho; without
+    the cosine pre-weight the level is 2 % off (the pin that a 1536 mm geometry cannot give: there the weight
+    is 0.999)."""
+    geo, ang, rho, rad, cen = _wide_fan_problem()
+    proj = _ball_projections(geo, ang, rho, rad, cen)
+    inside, outside = _wide_levels(orc.fdk(proj, geo, ang), geo, rad, cen)
+    assert abs(inside / rho - 1.0) < 0.005, inside / rho
+    assert abs(outside) < 0.01 * rho
+    # the same reconstruction with the weight divided out again
+    nu, nv = geo.nDetector
+    u = (np.arange(nu) + 0.5) * 2.5 - 0.5 * nu * 2.5
+    v = (np.arange(nv) + 0.5) * 2.5 - 0.5 * nv * 2.5
+    cosw = geo.DSD / np.sqrt(geo.DSD ** 2 + u[None, :] ** 2 + v[:, None] ** 2)
+    naive, _ = _wide_levels(orc.fdk(proj / cosw[None], geo, ang), geo, rad, cen)
+    assert abs(naive / rho - 1.0) > 0.015, naive / rho            # 2.1 %: four times the tolerance above
+
+
+def test_displaced_wide_fan_fdk_centres_the_cosine_weight_on_the_principal_ray():
+    """Detector displaced by a quarter of its width (the case Wang weights exist for): the level inside the ball
+    is right to 0.5 % only if the cosine weight is centred on the principal ray (u + offDetector_u), reading P34."""
+    nu = 120
+    geo, ang, rho, rad, cen = _wide_fan_problem(offu=0.25 * nu * 2.5, nu=nu)
+    proj = _ball_projections(geo, ang, rho, rad, cen)
+    inside, outside = _wide_levels(fx.fdk(proj, geo, ang, "ram_lak", "wang"), geo, rad, cen)
+    assert abs(inside / rho - 1.0) < 0.005, inside / rho
+    assert abs(outside) < 0.02 * rho
