@@ -59,6 +59,29 @@ def model_peak(kname, sm_mhz):
 NCU_TRAFFIC_PER_LAUNCH = {("C3", "ax_siddon"): 2.338e9, ("C3", "atb"): 6.11e8, ("C2", "ax_interp"): 4.58e8}
 
 
+PEAK_UNITS = {"ffma": "thread-instr/s", "smem": "B/s", "l1_lines": "128-B lines/s", "l2": "B/s", "h2d": "B/s", "d2h": "B/s",
+              "hbm_copy": "B/s (read+write)", "sm_hz": "Hz"}
+
+
+def measure_peaks(tg, kinds=("ffma", "smem", "l1_lines", "l2", "hbm_copy", "sm_hz")):
+    """The machine rates the projector rooflines rest on, measured now on this device by the library's own microbenchmark
+    kernels (tigre_microbench): a few hundred milliseconds in all."""
+    return {k: tg.microbench(k) for k in kinds}
+
+
+def run_peaks(tg, rank):
+    import torch
+    m = measure_peaks(tg, tuple(PEAK_UNITS))
+    if rank != 0:
+        return
+    sm_hz = m["sm_hz"]
+    per_clk = {"ffma_per_clk_per_sm": m["ffma"] / sm_hz / SM_COUNT, "smem_bytes_per_clk_per_sm": m["smem"] / sm_hz / SM_COUNT,
+               "l1_lines_per_clk_per_sm": m["l1_lines"] / sm_hz / SM_COUNT, "l2_bytes_per_clk": m["l2"] / sm_hz}
+    print(json.dumps({"metric": "step-0 machine rates (tigre_microbench)", "n_gpus": 1, "device": torch.cuda.get_device_name(0),
+                      "values": m, "units": PEAK_UNITS, "per_clock": per_clk,
+                      "nominal": {"ffma_per_clk_per_sm": 128, "smem_bytes_per_clk_per_sm": 128, "l1_lines_per_clk_per_sm": 1}}))
+
+
 def max_over_ranks(ms, device="cpu"):
     """Device time of the slowest rank (the contract's max over ranks); identity without a process group."""
     import torch
@@ -405,7 +428,7 @@ def main():
     ap.add_argument("--tv-delta", type=float, default=0.0, help="tv mode: AwTV delta (0 = plain TV)")
     ap.add_argument("--tv-op", default="minimise", choices=["minimise", "prox"],
                     help="tv mode: the gradient-descent minimiser (tigre_minimize_awtv) or the TV proximal operator of FISTA (tigre_tv_prox)")
-    ap.add_argument("--mode", default="plan", choices=["plan", "chunked", "tv", "drivers"],
+    ap.add_argument("--mode", default="plan", choices=["plan", "chunked", "tv", "drivers", "peaks"],
                     help="plan: OS-SART iteration in HBM (default); chunked: Ax + A^T b with all arrays in pinned host memory (S8)")
     ap.add_argument("--drivers", default="", help="drivers mode: comma-separated subset of the drivers to time (default: all)")
     ap.add_argument("--budget-gb", type=float, default=0.0, help="chunked mode: device bytes the chunked path may use (0 = 3/4 of free)")
@@ -464,6 +487,11 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
+    if args.mode == "peaks":
+        run_peaks(tg, rank)
+        if world > 1:
+            dist.destroy_process_group()
+        return
     if args.mode == "drivers":
         run_drivers(args, tg, geo, ang, rec, subsets, rank)
         if world > 1:

@@ -14,10 +14,12 @@
  *              The library keeps no pointer after a call returns.
  *   stream     `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
  *              Kernels are enqueued on it; calls that return host scalars synchronise it.
- *   memory     The library owns no persistent device memory.  Temporaries (per-view parameter
- *              tables; driver work buffers) come from the device's stream-ordered pool
- *              (cudaMallocAsync / cudaFreeAsync on `cuda_stream`); tigre_workspace_bytes()
- *              reports how much a call will take so the caller can budget HBM.
+ *   memory     Volumes and projections are the caller's.  Temporaries (per-view parameter tables, driver work
+ *              buffers, the buffers of a tigre_plan) are carved from the caller-owned workspace given to
+ *              tigre_set_workspace(); tigre_workspace_bytes() /
+ *              tigre_plan_workspace_bytes() say how much a call needs.  With NO workspace set (the default) they
+ *              come from the device's stream-ordered pool instead (cudaMallocAsync / cudaFreeAsync on
+ *              `cuda_stream`), which is the only allocation the library ever makes.
  *   errors     0 on success, negative tigre_status otherwise.  No exception crosses the ABI.
  *              There is no CPU fallback: without a CUDA device every compute call fails.
  */
@@ -170,6 +172,19 @@ TIGRE_API int tigre_plan_ossart(tigre_plan *plan, const float *b, float *x_inout
                       int nonneg, double *resid_hist, void *cuda_stream);
 TIGRE_API int tigre_plan_destroy(tigre_plan *plan);
 TIGRE_API size_t tigre_plan_bytes(const tigre_plan *plan);
+/* SIRT on arrays larger than the device (BASELINE.json configs[4] "single-GPU z-slab/angle-batch host chunking ... one SIRT
+ * iteration"; eq. 6 with one subset of all views): b, x_inout and r_scratch are PINNED HOST
+ * arrays (b, r_scratch [nA][nv][nu]; x_inout [nz][ny][nx], start in, result out).  Per iteration two streamed passes:
+ *   pass 1, per view batch: A x accumulated over the z-slabs of x, then r = W .* (b - A x), W = 1/(A 1) (reading P13), written
+ *           to r_scratch; resid_hist[it] (host, may be NULL) = ||b - A x||_2;
+ *   pass 2, per z-slab: G = A^T r and U = A^T 1 over the streamed row bands of all views, x <- max(0, x + lambda G / U)
+ *           where U > 1e-6 max(A^T 1) (nonneg = 0: no clamp).  max(A^T 1) over the volume costs one extra A^T 1 pass per call.
+ * r_scratch may be b itself when n_iter == 1 (b is then overwritten by the weighted residual).  Synchronises.
+ * Same kernels as the device-resident path; results agree with tigre_plan_ossart (one subset) up to summation order.
+ * TIGRE_ERR_MEMSPACE unless all three arrays are pinned. */
+TIGRE_API int tigre_sirt_chunked(const float *b, const tigre_geo *geo, const double *angles, int nA, int n_iter, float lambda,
+                       int nonneg, int ax_mode, int atb_mode, float *x_inout, float *r_scratch, double *resid_hist,
+                       void *cuda_stream);
 /* MLEM / OSEM (eq. 5 "x^k = x^{k-1}/(A1) A^T (b / (A x^{k-1}))"; 118-120, 139 OS counterpart; DESIGN.md reading
  * P33): for every subset s of the plan in turn  x <- x * V_s * A_s^T(b_s / (A_s x)),  V_s = the plan's column weights 1/(A_s^T 1),
  * quotient 0 where A_s x <= 0.  One subset holding all views is MLEM.  b, x_inout dev (x_inout: positive start, e.g. ones).
@@ -268,6 +283,13 @@ TIGRE_API int tigre_plan_sart_tv(tigre_plan *plan, const float *b, float *x_inou
  * counts: dev uint32 [nA][nv][nu] or NULL; *total (host) = sum.  Synchronises. */
 TIGRE_API int tigre_Ax_count(const tigre_geo *geo, const double *angles, int nA, int mode, uint32_t *counts,
                    uint64_t *total, void *cuda_stream);
+/* Index equality of the Siddon march (BASELINE.json north_star "Voxel/pixel index and footprint bounds must match exactly";
+ * DESIGN.md reading P19(a)): runs the march of tigre_Ax(TIGRE_AX_SIDDON) without touching a volume and returns, per ray,
+ * first_last[2 ray] / [2 ray + 1] = linear index (iz ny + iy) nx + ix of the first / last voxel the march gives a non-zero
+ * length to, in order from the source (-1 for a ray that misses), and nseg[ray] = the number of such voxels.
+ * first_last dev int64 [nA][nv][nu][2]; nseg dev uint32 [nA][nv][nu].  Asynchronous. */
+TIGRE_API int tigre_Ax_index(const tigre_geo *geo, const double *angles, int nA, int64_t *first_last, uint32_t *nseg,
+                   void *cuda_stream);
 /* In-library timing for bench.py's roofline leg.  tigre_profile(1) resets and starts recording a CUDA
  * event pair around every kernel group the launchers enqueue (on the launching stream); tigre_profile(0)
  * stops.  tigre_profile_read waits for the recorded events and returns, per kind k = 0 (Ax kernels),
@@ -275,8 +297,25 @@ TIGRE_API int tigre_Ax_count(const tigre_geo *geo, const double *angles, int nA,
  * launches[k] = kernels launched since the last tigre_profile call (counted even when not recording). */
 TIGRE_API int tigre_profile(int enable);
 TIGRE_API int tigre_profile_read(double *ms /*[3]*/, uint64_t *launches /*[3]*/);
-/* bytes of stream-ordered temporaries a call of kind `op` will allocate */
+/* Caller-owned workspace ("the library allocates nothing persistent ... workspace memory is the
+ * caller's"; north_star: "PyTorch used only for device memory and streams").
+ * tigre_set_workspace(dev_ptr, bytes): from now on every temporary and every plan buffer of this process is a block of
+ *   [dev_ptr, dev_ptr + bytes) (first-fit free list on the host, 256-byte granules) and the library makes no allocation of its
+ *   own; a call that does not fit returns TIGRE_ERR_WORKSPACE and leaves the workspace as it found it.  The memory stays
+ *   the caller's and must outlive every call and plan that uses it.  Blocks are re-used in the order calls are enqueued:
+ *   use ONE stream with a workspace (or synchronise when switching streams).  dev_ptr = NULL returns to the default, the
+ *   stream-ordered pool.  TIGRE_ERR_ARG while a plan (or a call in flight) still holds blocks, or for bytes < 4096;
+ *   TIGRE_ERR_MEMSPACE if dev_ptr is not device memory.  Process-global, guarded by a mutex.
+ * tigre_workspace_bytes(geo, nA, op): an upper bound on what one call of kind `op` takes for device-resident data.
+ * tigre_plan_workspace_bytes: the same for tigre_plan_create(_ex) plus tigre_plan_ossart with nSubsets subsets of at most
+ *   max_subset_views views (host_data != 0: b and x in pinned host memory, the end-to-end path).
+ *   The chunked (pinned host) path of tigre_Ax / tigre_Atb / tigre_sirt_chunked sizes its slabs to the workspace.
+ * tigre_workspace_stats: bytes in use now, the high-water mark, and the number of pool allocations (cudaMallocAsync) made
+ *   since the last tigre_set_workspace (stays 0 while a workspace is set); any pointer may be NULL. */
+TIGRE_API int tigre_set_workspace(void *dev_ptr, size_t bytes);
 TIGRE_API size_t tigre_workspace_bytes(const tigre_geo *geo, int nA, int op);
+TIGRE_API size_t tigre_plan_workspace_bytes(const tigre_geo *geo, int nA, int nSubsets, int max_subset_views, int host_data);
+TIGRE_API int tigre_workspace_stats(size_t *in_use, size_t *high_water, uint64_t *pool_allocs);
 /* tuning knobs of the chunked path: device bytes it may use for slabs (0 = default 3/4 of free) */
 TIGRE_API int tigre_set_chunk_budget(size_t bytes);
 /* what the most recent chunked tigre_Ax / tigre_Atb call of this process moved: bytes copied host->device and
@@ -290,6 +329,25 @@ TIGRE_API int tigre_set_atb_path(int path);
 /* which TV gradient kernel runs: 0 (default) = four voxels along x per thread whenever nx % 4 == 0, ny > 1, nz > 1 and
  * the arrays are 16-byte aligned, 1 = always the one-voxel-per-thread kernel (any shape).  Same sums; A/B and test hook. */
 TIGRE_API int tigre_set_tv_path(int path);
+
+/* Step-0 microbenchmarks: the machine rates the projector rooflines rest on,
+ * measured by kernels of this library on the current device with CUDA events on `cuda_stream` (best of 5 after a warm-up;
+ * the call synchronises).  *value (host) receives
+ *   TIGRE_PEAK_FFMA      fp32 multiply-adds per second over all SMs = thread-instructions / s of the plain-ALU issue slots
+ *   TIGRE_PEAK_SMEM      bytes / s of conflict-free 128-bit shared-memory loads, all SMs
+ *   TIGRE_PEAK_L1_LINES  distinct 128-byte lines / s served from L1 when every lane of a load reads its own (cached) line
+ *   TIGRE_PEAK_L2        bytes / s of 128-bit loads that bypass L1 and hit L2 (48 MB working set)
+ *   TIGRE_PEAK_H2D, _D2H bytes / s of a 1 GiB cudaMemcpyAsync from / to pinned host memory (allocated and freed inside)
+ *   TIGRE_PEAK_HBM_COPY  bytes / s, read + write, of a 2 GiB device-to-device float4 copy kernel
+ *   TIGRE_PEAK_SM_HZ     SM clock (Hz) seen by clock64() against the global timer under the FFMA load */
+enum { TIGRE_PEAK_FFMA = 0, TIGRE_PEAK_SMEM = 1, TIGRE_PEAK_L1_LINES = 2, TIGRE_PEAK_L2 = 3, TIGRE_PEAK_H2D = 4, TIGRE_PEAK_D2H = 5,
+       TIGRE_PEAK_HBM_COPY = 6, TIGRE_PEAK_SM_HZ = 7 };
+TIGRE_API int tigre_microbench(int kind, double *value, void *cuda_stream);
+
+/* which element-index type the ray-driven kernels (tigre_Ax both modes, the exact transposes, tigre_Ax_index) use:
+ * 0 (default) = 32-bit offsets for volumes (or resident slabs) below 2^31 voxels, 64-bit above; 1 = always the 64-bit
+ * instantiations (test hook: the kernels C5-sized slabs take, on volumes small enough to check element by element). */
+TIGRE_API int tigre_set_index_path(int path);
 
 TIGRE_API const char *tigre_strerror(int code);
 TIGRE_API const char *tigre_last_cuda_error(void);

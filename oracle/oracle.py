@@ -43,6 +43,7 @@ def lib():
         _lib.orc_atb_exact.restype = C.c_int
         _lib.orc_fdk_filter.restype = C.c_int
         _lib.orc_siddon_segments.restype = C.c_int
+        _lib.orc_siddon_index.restype = C.c_int
         _lib.orc_num_threads.restype = C.c_int
     return _lib
 
@@ -158,6 +159,22 @@ def atb_exact(proj, geo, angles, ax_mode=SIDDON):
     rc = lib().orc_atb_exact(_ptr(p), f32, C.byref(g), _ptr(v), v.shape[0], int(ax_mode), _ptr(out))
     assert rc == 0
     return out.reshape(geo.vol_shape)
+
+
+def siddon_index(geo, angles, ray_ids):
+    """Reading P19(a): per ray the segment count, the voxel index of the first / second / second-to-last / last segment, the
+    parameter lengths of the first and last segment and the smallest gap between consecutive crossings (knife-edge flags)."""
+    g = _grid(geo)
+    v = _views(geo, angles)
+    ids = np.ascontiguousarray(ray_ids, dtype=np.int64)
+    n = ids.size
+    nseg = np.zeros(n, dtype=np.int64)
+    vox4 = np.zeros((n, 4), dtype=np.int64)
+    ft, lt, mg = np.zeros(n), np.zeros(n), np.zeros(n)
+    rc = lib().orc_siddon_index(C.byref(g), _ptr(v), v.shape[0], _ptr(ids), C.c_int64(n), _ptr(nseg), _ptr(vox4), _ptr(ft), _ptr(lt), _ptr(mg))
+    assert rc == 0
+    return dict(nseg=nseg, first=vox4[:, 0], second=vox4[:, 1], second_last=vox4[:, 2], last=vox4[:, 3], first_t=ft, last_t=lt,
+                min_gap=mg)
 
 
 def siddon_segments(geo, angles, ia, iu, iv):

@@ -227,8 +227,8 @@ static int box_clip(const double S[3], const double d[3], const double b0[3], co
  * t in [0,1] (P7).  All plane crossings are collected, sorted, and each consecutive pair is
  * attributed to the voxel containing its midpoint (P8).  Returns the number of segments
  * of non-zero length. */
-static int siddon_ray(const orc_grid *g, const orc_view *w, const double S[3], const double P[3],
-                      double *ts, int64_t *idx, double *len) {
+static int siddon_ray_m(const orc_grid *g, const orc_view *w, const double S[3], const double P[3],
+                        double *ts, int64_t *idx, double *len, int *m_out) {
     double d[3] = {P[0] - S[0], P[1] - S[1], P[2] - S[2]};
     double L = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
     int n[3] = {g->nx, g->ny, g->nz};
@@ -253,6 +253,7 @@ static int siddon_ray(const orc_grid *g, const orc_view *w, const double S[3], c
         }
     }
     qsort(ts, m, sizeof(double), cmp_d);
+    if (m_out) *m_out = m; /* number of sorted crossing parameters left in ts[] (for the knife-edge flags) */
     int ns = 0;
     for (int j = 0; j + 1 < m; j++) {
         double ta = ts[j], tb = ts[j + 1];
@@ -269,6 +270,11 @@ static int siddon_ray(const orc_grid *g, const orc_view *w, const double S[3], c
         ns++;
     }
     return ns;
+}
+
+static int siddon_ray(const orc_grid *g, const orc_view *w, const double S[3], const double P[3],
+                      double *ts, int64_t *idx, double *len) {
+    return siddon_ray_m(g, w, S, P, ts, idx, len, NULL);
 }
 
 /* ---------------------------------------------------------------- O-B  interpolated, one ray */
@@ -391,6 +397,54 @@ int orc_ax(const void *vol, int vol_f32, const orc_grid *g, const orc_view *view
                 out[r] = interp_ray(g, w, V, S, P, NULL, 0.0, &K);
                 if (nseg) nseg[r] = K;
             }
+        }
+        free(ts);
+        free(len);
+        free(idx);
+    }
+    return 0;
+}
+
+/* Index / footprint equality (reading P19(a)): per ray (linear ids as in orc_ax) the number of non-zero segments, the
+ * linear voxel index of the first, second, second-to-last and last segment in order of increasing t (-1 if absent), and
+ * what a reader needs to call a ray knife-edge: the parameter lengths (t in [0,1] along source -> pixel) of the first and
+ * the last segment, and the smallest gap between two consecutive sorted crossing parameters (0 when two planes are
+ * crossed at the same point: the ray runs through a voxel edge).  All outputs [n_rays]. */
+int orc_siddon_index(const orc_grid *g, const orc_view *views, int nA, const int64_t *ray_ids, int64_t n_rays,
+                     int64_t *nseg, int64_t *vox4, double *first_t, double *last_t, double *min_gap) {
+    int64_t per = (int64_t)g->nu * g->nv;
+    int cap = g->nx + g->ny + g->nz + 8;
+    (void)nA;
+#pragma omp parallel
+    {
+        double *ts = (double *)malloc(sizeof(double) * cap);
+        double *len = (double *)malloc(sizeof(double) * cap);
+        int64_t *idx = (int64_t *)malloc(sizeof(int64_t) * cap);
+#pragma omp for schedule(dynamic, 256)
+        for (int64_t r = 0; r < n_rays; r++) {
+            int64_t id = ray_ids[r];
+            int ia = (int)(id / per);
+            int iv = (int)((id % per) / g->nu), iu = (int)(id % g->nu);
+            const orc_view *w = &views[ia];
+            double Rg[9], Rd[9], S[3], P[3];
+            frames(w, Rg, Rd);
+            pixel_pos(g, w, Rg, Rd, iu, iv, P);
+            ray_start(g, w, Rg, P, S);
+            int m = 0;
+            int ns = siddon_ray_m(g, w, S, P, ts, idx, len, &m);
+            double L = sqrt((P[0] - S[0]) * (P[0] - S[0]) + (P[1] - S[1]) * (P[1] - S[1]) + (P[2] - S[2]) * (P[2] - S[2]));
+            nseg[r] = ns;
+            vox4[4 * r + 0] = ns > 0 ? idx[0] : -1;
+            vox4[4 * r + 1] = ns > 1 ? idx[1] : -1;
+            vox4[4 * r + 2] = ns > 1 ? idx[ns - 2] : -1;
+            vox4[4 * r + 3] = ns > 0 ? idx[ns - 1] : -1;
+            first_t[r] = ns > 0 ? len[0] / L : 0.0;
+            last_t[r] = ns > 0 ? len[ns - 1] / L : 0.0;
+            double mg = INFINITY;
+            if (ns > 0)
+                for (int j = 0; j + 1 < m; j++)
+                    if (ts[j + 1] - ts[j] < mg) mg = ts[j + 1] - ts[j];
+            min_gap[r] = mg;
         }
         free(ts);
         free(len);

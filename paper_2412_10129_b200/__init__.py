@@ -52,7 +52,8 @@ EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_Ax_slab", "tigre_Atb_slab", "tigre_sl
            "tigre_update", "tigre_ossart", "tigre_cgls", "tigre_gradient_descent", "tigre_fdk", "tigre_fdk_filter", "tigre_fdk_ex", "tigre_fdk_filter_ex", "tigre_fdk_weights", "tigre_flatten_detector",
            "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_create_ex", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_osem", "tigre_plan_sart_tv", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
-           "tigre_last_cuda_error", "tigre_version"]
+           "tigre_last_cuda_error", "tigre_version", "tigre_Ax_index", "tigre_set_index_path", "tigre_set_workspace", "tigre_plan_workspace_bytes",
+           "tigre_workspace_stats", "tigre_sirt_chunked", "tigre_microbench"]
 
 
 def _lib():
@@ -66,6 +67,8 @@ def _lib():
         lib.tigre_last_cuda_error.restype = C.c_char_p
         lib.tigre_workspace_bytes.restype = C.c_size_t
         lib.tigre_plan_bytes.restype = C.c_size_t
+        lib.tigre_plan_workspace_bytes.restype = C.c_size_t
+        lib.tigre_set_workspace.argtypes = [C.c_void_p, C.c_size_t]
         lib.tigre_plan_bytes.argtypes = [C.c_void_p]
         lib.tigre_plan_destroy.argtypes = [C.c_void_p]
         for name in EXPORTS:
@@ -445,6 +448,74 @@ def Ax_count(geo, angles, mode="siddon", return_counts=False, device="cuda"):
                                  C.c_void_p(counts.data_ptr()) if return_counts else None, C.byref(total),
                                  _stream(counts)), "tigre_Ax_count")
     return (total.value, counts) if return_counts else total.value
+
+
+def Ax_index(geo, angles, device="cuda"):
+    """Reading P19(a): (first_last int64 [nA][nv][nu][2], nseg int32 [nA][nv][nu]) of the Siddon march itself: linear index of
+    the first / last voxel each ray gives a non-zero length to (-1: the ray misses) and the number of such voxels."""
+    import torch
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    fl = torch.empty(proj_shape(geo, nA) + (2,), dtype=torch.int64, device=device)
+    ns = torch.empty(proj_shape(geo, nA), dtype=torch.int32, device=device)
+    _check(_lib().tigre_Ax_index(G.ref, a.ctypes.data_as(_dp), nA, C.c_void_p(fl.data_ptr()), C.c_void_p(ns.data_ptr()), _stream(fl)),
+           "tigre_Ax_index")
+    return fl, ns
+
+
+def set_index_path(path):
+    """0 = 32-bit element offsets below 2^31 voxels (default), 1 = always the 64-bit instantiations of the ray-driven kernels."""
+    _check(_lib().tigre_set_index_path(int(path)), "tigre_set_index_path")
+
+
+_WORKSPACE = None
+
+
+def set_workspace(buf):
+    """Give the library a caller-owned workspace (a CUDA uint8 / any-dtype tensor, kept alive here) or None to return to the
+    stream-ordered pool."""
+    global _WORKSPACE
+    if buf is None:
+        _check(_lib().tigre_set_workspace(None, 0), "tigre_set_workspace")
+        _WORKSPACE = None
+        return
+    _check(_lib().tigre_set_workspace(C.c_void_p(buf.data_ptr()), C.c_size_t(buf.numel() * buf.element_size())), "tigre_set_workspace")
+    _WORKSPACE = buf
+
+
+def plan_workspace_bytes(geo, nA, n_subsets, max_subset_views, host_data=False):
+    G = _Geo(geo, nA)
+    return int(_lib().tigre_plan_workspace_bytes(G.ref, int(nA), int(n_subsets), int(max_subset_views), int(bool(host_data))))
+
+
+def workspace_stats():
+    """(bytes in use, high-water mark, pool allocations since set_workspace)."""
+    a, b, c = C.c_size_t(0), C.c_size_t(0), C.c_uint64(0)
+    _check(_lib().tigre_workspace_stats(C.byref(a), C.byref(b), C.byref(c)), "tigre_workspace_stats")
+    return a.value, b.value, c.value
+
+
+def sirt_chunked(b, geo, angles, x, n_iter=1, lam=1.0, nonneg=True, ax_mode="siddon", atb_mode="matched", r_scratch=None):
+    """SIRT on PINNED host tensors larger than the device (in place on x).  r_scratch: pinned, shaped like b (None: b itself is
+    overwritten by the weighted residual, n_iter == 1 only).  Returns the residual history."""
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    r = b if r_scratch is None else r_scratch
+    hist = np.zeros(max(n_iter, 1), dtype=np.float64)
+    _check(_lib().tigre_sirt_chunked(_f32(b, proj_shape(geo, nA), "b"), G.ref, a.ctypes.data_as(_dp), nA, int(n_iter), C.c_float(lam),
+                                     int(bool(nonneg)), _AX_MODES[ax_mode], _ATB_MODES[atb_mode], _f32(x, vol_shape(geo), "x"),
+                                     _f32(r, proj_shape(geo, nA), "r_scratch"), hist.ctypes.data_as(_dp), _stream()), "tigre_sirt_chunked")
+    return hist[:n_iter]
+
+
+PEAK_KINDS = {"ffma": 0, "smem": 1, "l1_lines": 2, "l2": 3, "h2d": 4, "d2h": 5, "hbm_copy": 6, "sm_hz": 7}
+
+
+def microbench(kind):
+    """One of the step-0 machine rates (see tigre_microbench in the header); kind: a key of PEAK_KINDS."""
+    v = C.c_double(0.0)
+    _check(_lib().tigre_microbench(PEAK_KINDS[kind], C.byref(v), _stream()), "tigre_microbench")
+    return v.value
 
 
 def workspace_bytes(geo, nA, op):

@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtigre_b200.so")
-SOURCES = ["geometry.cu", "ax.cu", "atb.cu", "atb_tma.cu", "elementwise.cu", "tv.cu", "prox.cu", "fdk.cu", "chunked.cu", "api.cu"]
+SOURCES = ["geometry.cu", "ax.cu", "atb.cu", "atb_tma.cu", "elementwise.cu", "tv.cu", "prox.cu", "fdk.cu", "chunked.cu", "peaks.cu", "api.cu"]
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--fmad=true", "-cudart", "static"]
 
@@ -19,8 +19,8 @@ def needs_build() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = _sources() + [os.path.join(CSRC, "common.cuh"),
-                         os.path.join(HERE, "..", "include", "tigre_b200.h")]
+    import glob
+    deps = _sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + [os.path.join(HERE, "..", "include", "tigre_b200.h")]
     return any(os.path.getmtime(d) > t for d in deps)
 
 

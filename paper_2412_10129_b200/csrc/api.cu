@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <map>
 #include <memory>
 #include <mutex>
 #include <string>
@@ -53,10 +54,75 @@ ProfScope::~ProfScope() {
     g_prof_recs.push_back(r);
 }
 
+// ---------------------------------------------------------------- caller-owned workspace (tigre_set_workspace)
+// "the library allocates nothing persistent; volume / projection / workspace memory is the caller's".
+// When a workspace is set every temporary and every plan buffer is carved from it by this first-fit free list (host-side
+// bookkeeping only, 256-byte granules, neighbours coalesced on release) and the library makes no cudaMallocAsync call.
+// Re-use of a released block is ordered by the stream the calls are enqueued on, as with the stream-ordered pool.
+struct Workspace {
+    std::mutex mu;
+    char* base = nullptr;
+    size_t size = 0, in_use = 0, high = 0;
+    std::map<size_t, size_t> free_;     // offset -> length of every free block
+    std::map<size_t, size_t> used;      // offset -> length of every live block
+    unsigned long long pool_allocs = 0; // cudaMallocAsync calls made since the last tigre_set_workspace
+    void* take(size_t bytes) {
+        bytes = (bytes + 255) & ~(size_t)255;
+        for (auto it = free_.begin(); it != free_.end(); ++it) {
+            if (it->second < bytes) continue;
+            const size_t off = it->first, len = it->second;
+            free_.erase(it);
+            if (len > bytes) free_[off + bytes] = len - bytes;
+            used[off] = bytes;
+            in_use += bytes, high = std::max(high, in_use);
+            return base + off;
+        }
+        return nullptr;
+    }
+    void give(void* p) {
+        const size_t off = (size_t)((char*)p - base);
+        auto u = used.find(off);
+        if (u == used.end()) return;
+        size_t o = off, len = u->second;
+        in_use -= len;
+        used.erase(u);
+        auto nx = free_.lower_bound(o);
+        if (nx != free_.end() && o + len == nx->first) len += nx->second, nx = free_.erase(nx);
+        if (nx != free_.begin()) {
+            auto pv = std::prev(nx);
+            if (pv->first + pv->second == o) o = pv->first, len += pv->second, free_.erase(pv);
+        }
+        free_[o] = len;
+    }
+};
+static Workspace g_ws;
+size_t workspace_free_bytes() {   // largest free block of the workspace (0: none set)
+    std::lock_guard<std::mutex> lk(g_ws.mu);
+    size_t m = 0;
+    for (auto& f : g_ws.free_) m = std::max(m, f.second);
+    return g_ws.base ? m : 0;
+}
+bool workspace_active() { return g_ws.base != nullptr; }
+
 int TempBuf::alloc(size_t bytes, cudaStream_t st) {
     release();
     s = st;
     if (bytes == 0) bytes = 16;
+    {
+        std::lock_guard<std::mutex> lk(g_ws.mu);
+        if (g_ws.base) {
+            p = g_ws.take(bytes);
+            ws = true;
+            if (!p) {
+                ws = false;
+                g_last_cuda_error = "caller-owned workspace too small (tigre_set_workspace)";
+                return TIGRE_ERR_WORKSPACE;
+            }
+            return TIGRE_OK;
+        }
+        ++g_ws.pool_allocs;
+    }
+    ws = false;
     cudaError_t e = cudaMallocAsync(&p, bytes, st);
     if (e != cudaSuccess) {
         p = nullptr;
@@ -66,8 +132,15 @@ int TempBuf::alloc(size_t bytes, cudaStream_t st) {
     return TIGRE_OK;
 }
 void TempBuf::release() {
-    if (p) cudaFreeAsync(p, s);
-    p = nullptr;
+    if (p) {
+        if (ws) {
+            std::lock_guard<std::mutex> lk(g_ws.mu);
+            g_ws.give(p);
+        } else {
+            cudaFreeAsync(p, s);
+        }
+    }
+    p = nullptr, ws = false;
 }
 int upload(TempBuf& buf, const void* host, size_t bytes, cudaStream_t st) {
     TG_TRY(buf.alloc(bytes, st));
@@ -385,6 +458,55 @@ int tigre_Ax_count(const tigre_geo* geo, const double* angles, int nA, int mode,
     return TIGRE_OK;
 }
 
+int tigre_Ax_index(const tigre_geo* geo, const double* angles, int nA, int64_t* first_last, uint32_t* nseg, void* cuda_stream) {
+    if (!first_last || !nseg) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    if (mem_kind(first_last) != MEM_DEVICE || mem_kind(nseg) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    TG_TRY(t.build_ray(nullptr, nA, st));
+    static_assert(sizeof(long long) == sizeof(int64_t), "int64_t is long long here");
+    return launch_ax_track(t.g, t.ray.as<RayView>(), nA, nseg, reinterpret_cast<long long*>(first_last), st);
+}
+
+int tigre_set_workspace(void* dev_ptr, size_t bytes) {
+    std::lock_guard<std::mutex> lk(g_ws.mu);
+    if (!g_ws.used.empty()) return TIGRE_ERR_ARG;   // a plan or a call in flight still holds blocks of the current workspace
+    if (dev_ptr && bytes < 4096) return TIGRE_ERR_ARG;
+    if (dev_ptr && mem_kind(dev_ptr) != MEM_DEVICE) return TIGRE_ERR_MEMSPACE;
+    g_ws.free_.clear();
+    g_ws.in_use = g_ws.high = 0, g_ws.pool_allocs = 0;
+    if (!dev_ptr) {
+        g_ws.base = nullptr, g_ws.size = 0;
+        return TIGRE_OK;
+    }
+    // carve from the first 256-byte boundary inside the block
+    const size_t mis = (size_t)((uintptr_t)dev_ptr & 255), skip = mis ? 256 - mis : 0;
+    g_ws.base = (char*)dev_ptr + skip, g_ws.size = (bytes - skip) & ~(size_t)255;
+    g_ws.free_[0] = g_ws.size;
+    return TIGRE_OK;
+}
+
+int tigre_workspace_stats(size_t* in_use, size_t* high_water, uint64_t* pool_allocs) {
+    std::lock_guard<std::mutex> lk(g_ws.mu);
+    if (in_use) *in_use = g_ws.in_use;
+    if (high_water) *high_water = g_ws.high;
+    if (pool_allocs) *pool_allocs = g_ws.pool_allocs;
+    return TIGRE_OK;
+}
+
+int tigre_microbench(int kind, double* value, void* cuda_stream) {
+    if (!value) return TIGRE_ERR_ARG;
+    TG_TRY(ensure_device());
+    return microbench(kind, value, (cudaStream_t)cuda_stream);
+}
+
+int tigre_set_index_path(int path) {
+    if (path != 0 && path != 1) return TIGRE_ERR_ARG;
+    set_index_path(path);
+    return TIGRE_OK;
+}
+
 // ---------------------------------------------------------------- OS-SART / SIRT
 // A plan holds what does not change between iterations: the per-subset view tables, the row weights
 // W_s = 1/(A_s 1) and column weights V_s = 1/(A_s^T 1) (P13, P16) and the scratch buffers.
@@ -499,9 +621,11 @@ int tigre_plan_ossart(tigre_plan* P, const float* b, float* x, int n_iter, float
     struct Cleanup {
         cudaStream_t& s;
         std::vector<cudaEvent_t>& e;
-        ~Cleanup() {
+        ~Cleanup() {   // destroyed before db / dx (declared after them): the upload stream is idle before they are released
+            if (s) cudaStreamSynchronize(s);
             for (cudaEvent_t x : e) cudaEventDestroy(x);
             if (s) cudaStreamDestroy(s);
+            (void)cudaGetLastError();
         }
     } cleanup{up, ev};
     if (kb == MEM_PINNED && kx == MEM_PINNED) {
@@ -574,6 +698,19 @@ int tigre_ossart(const float* b, const tigre_geo* geo, const double* angles, int
     const int rc = tigre_plan_ossart(P, b, x, n_iter, lambda, nonneg, resid_hist, cuda_stream);
     tigre_plan_destroy(P);
     return rc;
+}
+
+int tigre_sirt_chunked(const float* b, const tigre_geo* geo, const double* angles, int nA, int n_iter, float lambda, int nonneg,
+                       int ax_mode, int atb_mode, float* x_inout, float* r_scratch, double* resid_hist, void* cuda_stream) {
+    if (!b || !x_inout || !r_scratch || n_iter < 0) return TIGRE_ERR_ARG;
+    if (ax_mode != TIGRE_AX_SIDDON && ax_mode != TIGRE_AX_INTERP) return TIGRE_ERR_ARG;
+    if (atb_mode != TIGRE_ATB_MATCHED && atb_mode != TIGRE_ATB_FDK) return TIGRE_ERR_ARG;
+    if (r_scratch == b && n_iter > 1) return TIGRE_ERR_ARG;   // the residual would overwrite data a later iteration needs
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    if (mem_kind(b) != MEM_PINNED || mem_kind(x_inout) != MEM_PINNED || mem_kind(r_scratch) != MEM_PINNED) return TIGRE_ERR_MEMSPACE;
+    return chunked_sirt(b, geo, angles, nA, n_iter, lambda, nonneg, ax_mode, atb_mode, x_inout, r_scratch, resid_hist,
+                        (cudaStream_t)cuda_stream);
 }
 
 // ---------------------------------------------------------------- MLEM / OSEM (eq. 5; reading P33)
@@ -761,14 +898,15 @@ int tigre_gradient_descent(const float* b, const tigre_geo* geo, const double* a
 
 // ---------------------------------------------------------------- FDK (O-D)
 static int fdk_filter_impl(const float* b, Tables& t, int nA, float* q, cudaStream_t st) {
-    std::vector<double> dd(2 * (size_t)nA);
-    for (int a = 0; a < nA; ++a) dd[a] = t.views[a].DSD, dd[nA + a] = t.views[a].DSO;
+    std::vector<double> dd(4 * (size_t)nA);   // DSD, DSO, offDetector (u, v) per view
+    for (int a = 0; a < nA; ++a)
+        dd[a] = t.views[a].DSD, dd[nA + a] = t.views[a].DSO, dd[2 * nA + 2 * a] = t.views[a].offD[0], dd[2 * nA + 2 * a + 1] = t.views[a].offD[1];
     // parallel beam (P29): no magnification (tau = du) and no cosine weight: the kernels' DSO/DSD = 1, DSD/sqrt(DSD^2 + u^2 + v^2) = 1
-    if (t.views[0].parallel) std::fill(dd.begin(), dd.end(), 1e15);
+    if (t.views[0].parallel) std::fill(dd.begin(), dd.begin() + 2 * nA, 1e15);
     TempBuf tb;
     TG_TRY(upload(tb, dd.data(), sizeof(double) * dd.size(), st));
     // Ram-Lak, no weights: taps formed in the kernel, odd taps only (fdk.cu)
-    return launch_fdk_filter_taps(b, t.g, tb.as<double>(), tb.as<double>() + nA, nA, nullptr, nullptr, q, st, true);
+    return launch_fdk_filter_taps(b, t.g, tb.as<double>(), tb.as<double>() + nA, tb.as<double>() + 2 * nA, nA, nullptr, nullptr, q, st, true);
 }
 int tigre_fdk_filter(const float* b, const tigre_geo* geo, const double* angles, int nA, float* q, void* cuda_stream) {
     if (!b || !q) return TIGRE_ERR_ARG;
@@ -798,10 +936,11 @@ static int fdk_filter_ex_impl(const float* b, Tables& t, int nA, int filter, int
     if (weighting != TIGRE_FDK_FULL && t.views[0].parallel) return TIGRE_ERR_ARG;   // cone-beam redundancy weights
     if (filter == TIGRE_FILTER_RAM_LAK && weighting == TIGRE_FDK_FULL) return fdk_filter_impl(b, t, nA, q, st);
     const int nu = t.g.nu;
-    std::vector<double> dd(2 * (size_t)nA), taps, w;
-    for (int a = 0; a < nA; ++a) dd[a] = t.views[a].DSD, dd[nA + a] = t.views[a].DSO;
+    std::vector<double> dd(4 * (size_t)nA), taps, w;   // DSD, DSO, offDetector (u, v) per view
+    for (int a = 0; a < nA; ++a)
+        dd[a] = t.views[a].DSD, dd[nA + a] = t.views[a].DSO, dd[2 * nA + 2 * a] = t.views[a].offD[0], dd[2 * nA + 2 * a + 1] = t.views[a].offD[1];
     // parallel beam (P29): no magnification (tau = du) and no cosine weight: the kernels' DSO/DSD = 1, DSD/sqrt(DSD^2 + u^2 + v^2) = 1
-    if (t.views[0].parallel) std::fill(dd.begin(), dd.end(), 1e15);
+    if (t.views[0].parallel) std::fill(dd.begin(), dd.begin() + 2 * nA, 1e15);
     fdk_filter_taps(nu, filter, taps);
     std::vector<float> ft(taps.begin(), taps.end()), fw;
     TempBuf tb, tt, tw;
@@ -814,7 +953,7 @@ static int fdk_filter_ex_impl(const float* b, Tables& t, int nA, int filter, int
         for (size_t i = 0; i < w.size(); ++i) fw[i] = (float)(k * w[i]);
         TG_TRY(upload(tw, fw.data(), sizeof(float) * fw.size(), st));
     }
-    return launch_fdk_filter_taps(b, t.g, tb.as<double>(), tb.as<double>() + nA, nA, tt.as<float>(),
+    return launch_fdk_filter_taps(b, t.g, tb.as<double>(), tb.as<double>() + nA, tb.as<double>() + 2 * nA, nA, tt.as<float>(),
                                   weighting != TIGRE_FDK_FULL ? tw.as<float>() : nullptr, q, st, filter == TIGRE_FILTER_RAM_LAK);
 }
 int tigre_fdk_filter_ex(const float* b, const tigre_geo* geo, const double* angles, int nA, int filter, int weighting, float* q,
@@ -1009,19 +1148,34 @@ int tigre_fista(const float* b, const tigre_geo* geo, const double* angles, int 
     return TIGRE_OK;
 }
 
+// Upper bounds (256-byte granules and a megabyte of small tables / scalars included) on the temporaries of one call on
+// device-resident data.  OSSART = tigre_ossart / tigre_plan_* with ONE subset (SIRT): tigre_plan_workspace_bytes is the general form.
 size_t tigre_workspace_bytes(const tigre_geo* geo, int nA, int op) {
     if (!geo || nA <= 0) return 0;
     const size_t per = (size_t)geo->nDetector[0] * geo->nDetector[1] * sizeof(float);
     const size_t vol = (size_t)geo->nVoxel[0] * geo->nVoxel[1] * geo->nVoxel[2] * sizeof(float);
-    const size_t tab = (size_t)nA * (sizeof(RayView) + sizeof(VoxView));
+    const size_t tab = (size_t)nA * (sizeof(RayView) + sizeof(VoxView) + 4 * sizeof(double)) + ((size_t)1 << 20);
     switch (op) {
-        case TIGRE_OP_AX:
-        case TIGRE_OP_ATB: return tab;
-        case TIGRE_OP_OSSART: return tab + per * nA * 2 + vol * 2;   // + vol per subset for V (caller adds nSubsets-1)
-        case TIGRE_OP_CGLS: return tab + per * nA * 2 + vol * 2;
-        case TIGRE_OP_FDK: return tab + per * nA;
+        case TIGRE_OP_AX: return tab + vol;                       // the (x,y)-transposed copy of the volume
+        case TIGRE_OP_ATB: return tab + vol;                      // exact modes: the transposed scratch volume
+        case TIGRE_OP_OSSART: return tigre_plan_workspace_bytes(geo, nA, 1, nA, 0);
+        case TIGRE_OP_CGLS: return tab + per * nA * 2 + vol * 3;  // r, q; s, p; transposed copy / scratch
+        case TIGRE_OP_FDK: return tab + per * nA + (size_t)geo->nDetector[0] * (nA + 1) * sizeof(float);
     }
     return 0;
+}
+
+size_t tigre_plan_workspace_bytes(const tigre_geo* geo, int nA, int nSubsets, int max_subset_views, int host_data) {
+    if (!geo || nA <= 0 || nSubsets <= 0 || max_subset_views <= 0) return 0;
+    const size_t per = (size_t)geo->nDetector[0] * geo->nDetector[1] * sizeof(float);
+    const size_t vol = (size_t)geo->nVoxel[0] * geo->nVoxel[1] * geo->nVoxel[2] * sizeof(float);
+    const size_t tab = (size_t)nA * (sizeof(RayView) + sizeof(VoxView) + sizeof(int32_t) + sizeof(float) * geo->nDetector[0]) +
+                       (size_t)nSubsets * 1024 + ((size_t)1 << 20);
+    // plan: W (all views), V (one volume per subset), one subset's Ax / residual, A^T r; iteration: transposed iterate;
+    // pinned-host data (end-to-end path): device copies of b and x
+    size_t n = tab + per * nA + vol * nSubsets + per * max_subset_views + vol + vol;
+    if (host_data) n += per * nA + vol;
+    return n;
 }
 
 }  // extern "C"

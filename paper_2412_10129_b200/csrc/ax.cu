@@ -84,11 +84,22 @@ struct SidRay {
     float kf, acc, vB;
     float ys;                                       // scatter (exact adjoint): ray value times the length scale
     IdxT off;                                       // element offset of the current voxel
+    // TRACK instantiation only (tigre_Ax_index, reading P19(a)): element offsets of the first / last voxel met with a
+    // non-zero length, and the number of such voxels
+    long long first, last;
+    uint32_t nseg;
+    __device__ __forceinline__ void note(IdxT o, float len) {
+        if (len > 0.f) {
+            if (nseg == 0) first = (long long)o;
+            last = (long long)o;
+            ++nseg;
+        }
+    }
 };
 
 // One D-slab, interior of the volume: the whole slab [0,1] lies inside the ray's clipped range and at
 // least 1e-3 voxel away from the lateral faces, so no clipping and no bounds checks are needed.
-template <typename IdxT, bool UNIT, bool SCATTER>
+template <typename IdxT, bool UNIT, bool SCATTER, bool TRACK = false>
 __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base, SidRay<IdxT>& r) {
     // slab-local parameter of the next E / F plane crossing, saturated to [0,1] (1 = not in this slab)
     const float se = __saturatef(fmaf(r.hE, r.imE, -r.kf)), sf = __saturatef(fmaf(r.hF, r.imF, -r.kf));
@@ -100,7 +111,11 @@ __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base,
     // the other lanes the middle piece has zero length
     const bool both = cE && cF;
     const float s2 = both ? fmaxf(se, sf) : s1;
-    if (SCATTER) {
+    if (TRACK) {
+        r.note(r.off, s1);
+        if (both) r.note(r.off + ((se < sf) ? r.stE : r.stF), s2 - s1);
+        r.note(offC, 1.0f - s2);
+    } else if (SCATTER) {
         // exact adjoint: the same three lengths, added to the voxels instead of gathered from them
         float* out = const_cast<float*>(base);
         atomicAdd(out + r.off, s1 * r.ys);
@@ -123,13 +138,16 @@ __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base,
 
 // One interior D-slab of a ray that is known not to cross an F-plane in it (sf = 1 in siddon_slab_fast): the same two
 // lengths and the same operations on them as there, without the middle voxel and the F bookkeeping (bitwise the same sum).
-template <typename IdxT, bool UNIT, bool SCATTER>
+template <typename IdxT, bool UNIT, bool SCATTER, bool TRACK = false>
 __device__ __forceinline__ void siddon_slab_e_only(const float* __restrict__ base, SidRay<IdxT>& r) {
     const float se = __saturatef(fmaf(r.hE, r.imE, -r.kf));
     r.kf += 1.0f;
     const bool cE = se < 1.0f;
     const IdxT offC = r.off + (cE ? r.stE : (IdxT)0);
-    if (SCATTER) {
+    if (TRACK) {
+        r.note(r.off, se);
+        r.note(offC, 1.0f - se);
+    } else if (SCATTER) {
         float* out = const_cast<float*>(base);
         atomicAdd(out + r.off, se * r.ys);
         atomicAdd(out + offC, (1.0f - se) * r.ys);
@@ -146,7 +164,7 @@ __device__ __forceinline__ void siddon_slab_e_only(const float* __restrict__ bas
 
 // One D-slab with clipping to [slo, shi] and per-voxel bounds checks (first / last slabs of a ray and
 // slabs that run within 1e-3 voxel of a lateral face).
-template <typename IdxT, bool UNIT, bool SCATTER>
+template <typename IdxT, bool UNIT, bool SCATTER, bool TRACK = false>
 __device__ __forceinline__ void siddon_slab_checked(const float* __restrict__ base, SidRay<IdxT>& r, int& ie, int& jf,
                                                     int diE, int diF, int nE, int nF, float slo, float shi) {
     const float se = __saturatef(fmaf(r.hE, r.imE, -r.kf)), sf = __saturatef(fmaf(r.hF, r.imF, -r.kf));
@@ -164,7 +182,11 @@ __device__ __forceinline__ void siddon_slab_checked(const float* __restrict__ ba
     const float lenA = s1 - slo, lenB = s2 - s1, lenC = shi - s2;
     // with a single crossing [s1, shi] lies in the end voxel: lenB + lenC = shi - s1
     const float lenE = (cE && cF) ? lenC : lenB + lenC;
-    if (SCATTER) {
+    if (TRACK) {
+        if (vEA && vFA) r.note(r.off, lenA);
+        if (cE && cF && vB) r.note(offB, lenB);
+        if (vEC && vFC) r.note(offC, lenE);
+    } else if (SCATTER) {
         float* out = const_cast<float*>(base);
         if (lenA > 0.f && vEA && vFA) atomicAdd(out + r.off, lenA * r.ys);
         if (cE && cF && lenB > 0.f && vB) atomicAdd(out + offB, lenB * r.ys);
@@ -180,13 +202,18 @@ __device__ __forceinline__ void siddon_slab_checked(const float* __restrict__ ba
     r.off = offC + r.sD;
 }
 
-template <typename IdxT, bool UNIT, bool COUNT, bool SCATTER>
+// TRACK (tigre_Ax_index): the march runs as for a gather, without touching the volume, and records per ray the first and
+// last voxel it gives a non-zero length to (canonical linear index (iz ny + iy) nx + ix, -1 if none) into track[2 * ray]
+// and the number of such voxels into counts[ray]: what reading P19(a) compares with the oracle, from the march itself.
+template <typename IdxT, bool UNIT, bool COUNT, bool SCATTER, bool TRACK = false>
 __global__ void __launch_bounds__(AX_TU* AX_TV, AXMB)
 ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, const RayView* __restrict__ views,
-                 int nViews, AxP p, float* __restrict__ proj, uint32_t* __restrict__ counts) {
+                 int nViews, AxP p, float* __restrict__ proj, uint32_t* __restrict__ counts, long long* __restrict__ track = nullptr) {
     int view, iu, iv;
-    if (!ax_decode(p, nViews, view, iu, iv)) return;
-    const unsigned wmask = __activemask();   // lanes of this warp that own a pixel (converged here)
+    const bool mine = ax_decode(p, nViews, view, iu, iv);
+    // lanes of this warp that own a pixel, taken while all 32 lanes are still here (the mask of every warp vote below)
+    const unsigned wmask = __ballot_sync(0xffffffffu, mine);
+    if (!mine) return;
     const RayView& rv = views[view];
     const size_t out = ((size_t)view * p.nv + iv) * p.nu + iu;
 
@@ -213,6 +240,7 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     SidRay<IdxT> r;
     r.imE = r.imF = 1.f, r.sgE = r.sgF = 1.f, r.hE = r.hF = 3.0e38f, r.stE = r.stF = r.sD = 0;
     r.kf = 0.f, r.acc = 0.f, r.vB = 0.f, r.ys = 0.f, r.off = 0;
+    r.first = r.last = -1, r.nseg = 0;
     const float* base = vol;
     int i0 = 0, nslab = 0, kA = 0, kB = 0, ie = 0, jf = 0, ie0 = 0, jf0 = 0, diE = 1, diF = 1;
     float slo0 = 0.f, shiN = 1.f, scale = 0.f;
@@ -311,7 +339,7 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     const int last = nslab - 1;
     int k = 0;
     for (; k < kA; ++k)
-        siddon_slab_checked<IdxT, UNIT, SCATTER>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
+        siddon_slab_checked<IdxT, UNIT, SCATTER, TRACK>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
     const bool ranFast = kB > k;
     {
         // Warp-uniform part of the interior: groups of AXG slabs up to the shallowest end in the warp.  The lanes of a warp share a
@@ -326,16 +354,16 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
             if (__any_sync(wmask, nearF)) {
                 if (ranFast) {
 #pragma unroll
-                    for (int j = 0; j < AXG; ++j) siddon_slab_fast<IdxT, UNIT, SCATTER>(base, r);
+                    for (int j = 0; j < AXG; ++j) siddon_slab_fast<IdxT, UNIT, SCATTER, TRACK>(base, r);
                 }
             } else if (ranFast) {
 #pragma unroll
-                for (int j = 0; j < AXG; ++j) siddon_slab_e_only<IdxT, UNIT, SCATTER>(base, r);
+                for (int j = 0; j < AXG; ++j) siddon_slab_e_only<IdxT, UNIT, SCATTER, TRACK>(base, r);
             }
         }
         if (ranFast) k += AXG * groups;
     }
-    for (; k < kB; ++k) siddon_slab_fast<IdxT, UNIT, SCATTER>(base, r);
+    for (; k < kB; ++k) siddon_slab_fast<IdxT, UNIT, SCATTER, TRACK>(base, r);
     if (k < nslab) {
         // recover the cell indices from the plane state for the checked tail: hE has moved by one per crossing
         if (ranFast) {
@@ -343,7 +371,22 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
             if (r.hF < 1.0e38f) jf = jf0 + (int)rint((double)r.hF - hF0);
         }
         for (; k < nslab; ++k)
-            siddon_slab_checked<IdxT, UNIT, SCATTER>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
+            siddon_slab_checked<IdxT, UNIT, SCATTER, TRACK>(base, r, ie, jf, diE, diF, nE, nF, k == 0 ? slo0 : 0.f, k == last ? shiN : 1.f);
+    }
+    if (TRACK) {
+        // offsets are in the layout this ray marched through: bring those of the transposed copy [z][x][y] back to [z][y][x]
+        const bool useT = base == volT;
+        const long long nxy = (long long)p.nx * p.ny;
+        long long fl[2] = {r.first, r.last};
+#pragma unroll
+        for (int q = 0; q < 2; ++q)
+            if (fl[q] >= 0 && useT) {
+                const long long z = fl[q] / nxy, rem = fl[q] - z * nxy, x = rem / p.ny, y = rem - x * p.ny;
+                fl[q] = z * nxy + y * p.nx + x;
+            }
+        track[2 * out] = fl[0], track[2 * out + 1] = fl[1];
+        counts[out] = r.nseg;
+        return;
     }
     if (!SCATTER) {
         const float result = r.acc * scale;
@@ -381,8 +424,10 @@ __global__ void __launch_bounds__(AX_TU* AX_TV, AXIMB)
 ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, const RayView* __restrict__ views, int nViews,
                  AxP p, float* __restrict__ proj, uint32_t* __restrict__ counts) {
     int view, iu, iv;
-    if (!ax_decode(p, nViews, view, iu, iv)) return;
-    const unsigned wmask = __activemask();   // lanes of this warp that own a pixel (converged here)
+    const bool mine = ax_decode(p, nViews, view, iu, iv);
+    // lanes of this warp that own a pixel, taken while all 32 lanes are still here (the mask of every warp vote below)
+    const unsigned wmask = __ballot_sync(0xffffffffu, mine);
+    if (!mine) return;
     const RayView& rv = views[view];
     const size_t out = ((size_t)view * p.nv + iv) * p.nu + iu;
     // fp64 set-up in voxel-index coordinates (voxel centres at integer + 1/2)
@@ -665,6 +710,12 @@ ax_siddon_unit_kernel(const RayView* __restrict__ views, int nViews, AxP p, floa
     proj[out] = p.accumulate ? proj[out] + result : result;
 }
 
+// test hook (tigre_set_index_path): 1 = take the 64-bit element-index instantiations (volumes or slabs of >= 2^31 voxels, the
+// C5 regime) for every volume, so that they can be compared with the 32-bit ones and with the oracle on small volumes
+static int g_index_path = 0;
+void set_index_path(int path) { g_index_path = path; }
+static bool use_idx64(size_t nvox) { return g_index_path == 1 || nvox >= (1ull << 31); }
+
 template <typename IdxT>
 static void ax_dispatch(const float* vol, const float* volT, const RayView* v, int nViews, const AxP& p, int mode, bool unit,
                         float* proj, uint32_t* counts, cudaStream_t st) {
@@ -714,8 +765,33 @@ int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nView
         if (tg_.y > 65535 || tg_.z > 65535) volT = nullptr;
         else transpose_xy_kernel<<<tg_, tb, 0, st>>>(vol, vt.as<float>(), g.nx, g.ny);
     }
-    if (nvox < (1ull << 31)) ax_dispatch<int>(vol, volT, d_views, nViews, p, mode, unit_vol, proj, count_out, st);
+    if (!use_idx64(nvox)) ax_dispatch<int>(vol, volT, d_views, nViews, p, mode, unit_vol, proj, count_out, st);
     else ax_dispatch<long long>(vol, volT, d_views, nViews, p, mode, unit_vol, proj, count_out, st);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+
+// tigre_Ax_index: the Siddon march without the volume; per ray the first / last voxel with a non-zero length and their number
+int launch_ax_track(const Grid& g, const RayView* d_views, int nViews, uint32_t* counts, long long* track, cudaStream_t st) {
+    AxP p;
+    p.nx = g.nx, p.ny = g.ny, p.nz = g.nz, p.nu = g.nu, p.nv = g.nv;
+    p.hx = (float)g.dx, p.hy = (float)g.dy, p.hz = (float)g.dz;
+    p.hxd = g.dx, p.hyd = g.dy, p.hzd = g.dz;
+    p.delta = g.accuracy * fmin(g.dx, fmin(g.dy, g.dz));
+    p.iv0 = 0, p.iv1 = g.nv, p.zs0 = 0, p.zs1 = g.nz;
+    p.nUt = (g.nu + AX_TU - 1) / AX_TU, p.nVt = (g.nv + AX_TV - 1) / AX_TV;
+    p.accumulate = 0;
+    const long long nblk = (long long)p.nUt * p.nVt * nViews;
+    if (nblk <= 0 || nblk > 0x7fffffffLL) return TIGRE_ERR_ARG;
+    const size_t nvox = (size_t)g.nx * g.ny * g.nz;
+    // the march only forms offsets from these two bases (it never dereferences them); they select the layout each ray walks,
+    // exactly as in launch_ax: x-dominant rays take the transposed one whenever launch_ax would make it
+    const float* fakeV = reinterpret_cast<const float*>(0x1000);
+    const float* fakeT = (g.nx > 1 && g.ny > 1) ? reinterpret_cast<const float*>(0x2000) : nullptr;
+    dim3 block(AX_TU, AX_TV), grid((unsigned)nblk);
+    ProfScope ps(PK_AX, st);
+    if (!use_idx64(nvox)) ax_siddon_kernel<int, true, false, false, true><<<grid, block, 0, st>>>(fakeV, fakeT, d_views, nViews, p, nullptr, counts, track);
+    else ax_siddon_kernel<long long, true, false, false, true><<<grid, block, 0, st>>>(fakeV, fakeT, d_views, nViews, p, nullptr, counts, track);
     TG_CUDA(cudaGetLastError());
     return TIGRE_OK;
 }
@@ -772,7 +848,7 @@ int launch_ax_adjoint(const float* proj, const Grid& g, const RayView* d_views, 
     if (volT) TG_CUDA(cudaMemsetAsync(volT, 0, nvox * sizeof(float), st));
     dim3 block(AX_TU, AX_TV), grid((unsigned)nblk);
     float* pin = const_cast<float*>(proj);   // read only by the SCATTER instantiations
-    if (nvox < (1ull << 31)) {
+    if (!use_idx64(nvox)) {
         if (mode == TIGRE_AX_SIDDON) ax_siddon_kernel<int, false, false, true><<<grid, block, 0, st>>>(vol, volT, d_views, nViews, p, pin, nullptr);
         else ax_interp_kernel<int, false, false, true><<<grid, block, 0, st>>>(vol, volT, d_views, nViews, p, pin, nullptr);
     } else {

@@ -71,9 +71,10 @@ int build_vox_view(const Grid& g, const ViewH& v, VoxView& o);
 void row_band(const Grid& g, const ViewH& v, int z0, int nzs, int& row0, int& nrows);
 
 // ---------------------------------------------------------------- stream-ordered temporaries
-struct TempBuf {  // RAII: cudaMallocAsync / cudaFreeAsync on one stream
+struct TempBuf {  // RAII: a block of the caller's workspace (tigre_set_workspace) if one is set, else cudaMallocAsync / cudaFreeAsync on one stream
     void* p = nullptr;
     cudaStream_t s = nullptr;
+    bool ws = false;
     TempBuf() {}
     TempBuf(const TempBuf&) = delete;
     TempBuf& operator=(const TempBuf&) = delete;
@@ -111,6 +112,9 @@ int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nView
               bool accumulate, float* proj, uint32_t* count_out, cudaStream_t st, const AxSub* sub = nullptr,
               const float* volT_in = nullptr);   // volT_in: an up-to-date (x,y)-transposed copy of vol, if the caller has one
 int launch_transpose_xy(const float* vol, float* volT, const Grid& g, cudaStream_t st);
+// Siddon march without the volume: counts[ray] = voxels met with a non-zero length, track[2 ray], [2 ray + 1] = first / last of them
+int launch_ax_track(const Grid& g, const RayView* d_views, int nViews, uint32_t* counts, long long* track, cudaStream_t st);
+void set_index_path(int path);
 // exact adjoint of launch_ax (ray-driven scatter of the same weights); vol [nz][ny][nx] is overwritten
 int launch_ax_adjoint(const float* proj, const Grid& g, const RayView* d_views, int nViews, int mode, float* vol,
                       cudaStream_t st);
@@ -141,14 +145,16 @@ int launch_axpy(float* y, const float* x, const double* d_num, const double* d_d
 int launch_xpby(float* p, const float* s, const double* d_num, const double* d_den, size_t n,
                 cudaStream_t st);                                                       // p = s + (num/den)*p
 int launch_scale(float* x, float a, size_t n, cudaStream_t st);
+int launch_fill(float* x, float a, size_t n, cudaStream_t st);                          // x = a
+int launch_max(const float* v, size_t n, float* d_max, cudaStream_t st);                // *d_max = max(*d_max, max v), v >= 0
 int launch_scale_columns(float* W, const float* colw, int nViews, int nv, int nu, cudaStream_t st);
 int launch_ratio(const float* b, const int32_t* view_idx, const float* Ax, float* q, size_t per_view, int nViews, cudaStream_t st);
 int launch_mul_update(float* x, const float* g, const float* V, size_t n, cudaStream_t st);
 int launch_diff_stats(const float* a, const float* b, const float* c, size_t n, double* d_out3, cudaStream_t st);
 void fdk_filter_taps(int nu, int filter, std::vector<double>& g);
 int fdk_weights(const Grid& g, const std::vector<ViewH>& views, int weighting, std::vector<double>& w);
-int launch_fdk_filter_taps(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, int nViews, const float* d_taps,
-                           const float* d_colw, float* q, cudaStream_t st, bool odd_only = false);
+int launch_fdk_filter_taps(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, const double* d_offd, int nViews,
+                           const float* d_taps, const float* d_colw, float* q, cudaStream_t st, bool odd_only = false);
 int launch_flatten(const float* curved, const Grid& g, const double* d_dsd, int nViews, float* flat, cudaStream_t st);
 int launch_count_reduce(const uint32_t* c, size_t n, unsigned long long* d_total, cudaStream_t st);
 
@@ -162,12 +168,18 @@ int launch_prox_update(float* px, float* py, float* pz, const float* d, float ta
 int launch_momentum(float* y, float* x, const float* xn, float c, size_t n, cudaStream_t st);
 int launch_tv_step(float* x, const float* g, float alpha, const double* d_gg, size_t n, cudaStream_t st);
 
+int microbench(int kind, double* value, cudaStream_t st);   // peaks.cu
+
 // chunked (pinned host) path
 int chunked_ax(const float* h_vol, const tigre_geo* geo, const double* angles, int nA, int mode, float* h_proj,
                cudaStream_t st);
 int chunked_atb(const float* h_proj, const tigre_geo* geo, const double* angles, int nA, int mode, float* h_vol,
                 cudaStream_t st);
+int chunked_sirt(const float* h_b, const tigre_geo* geo, const double* angles, int nA, int n_iter, float lambda, int nonneg,
+                 int ax_mode, int atb_mode, float* h_x, float* h_r, double* resid_hist, cudaStream_t st);
 size_t chunk_budget();
+size_t workspace_free_bytes();   // largest free block of the caller's workspace (0: none set)
+bool workspace_active();
 int tables_prep(const tigre_geo* geo, const double* angles, int nA, Grid& g, std::vector<ViewH>& views);
 
 }  // namespace tg

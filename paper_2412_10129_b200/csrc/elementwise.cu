@@ -316,6 +316,24 @@ int launch_scale(float* x, float a, size_t n, cudaStream_t st) {
     return TIGRE_OK;
 }
 
+__global__ void __launch_bounds__(256) fill_kernel(float* __restrict__ x, float a, size_t n) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) x[i] = a;
+}
+int launch_fill(float* x, float a, size_t n, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
+    if (n == 0) return TIGRE_OK;
+    fill_kernel<<<ew_blocks(n), 256, 0, st>>>(x, a, n);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+int launch_max(const float* v, size_t n, float* d_max, cudaStream_t st) {
+    ProfScope ps(PK_EW, st);
+    if (n == 0) return TIGRE_OK;
+    max_kernel<<<ew_blocks(n), 256, 0, st>>>(v, n, d_max);
+    TG_CUDA(cudaGetLastError());
+    return TIGRE_OK;
+}
+
 __global__ void __launch_bounds__(256) count_reduce_kernel(const uint32_t* __restrict__ c, size_t n, unsigned long long* __restrict__ out) {
     unsigned long long s = 0;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) s += c[i];

@@ -78,15 +78,17 @@ __device__ __forceinline__ void conv8(const float* __restrict__ src, int PL, int
 template <bool ODD>
 __global__ void __launch_bounds__(128)
 fdk_conv_kernel(const float* __restrict__ b, int nu, int nv, float du, float dv, const double* __restrict__ dsd_a,
-                const double* __restrict__ dso_a, const float* __restrict__ taps, const float* __restrict__ colw,
-                float* __restrict__ q, int PAD, int PL, int NT) {
+                const double* __restrict__ dso_a, const double* __restrict__ offd_a, const float* __restrict__ taps,
+                const float* __restrict__ colw, float* __restrict__ q, int PAD, int PL, int NT) {
     extern __shared__ __align__(16) float sm[];
     float* tp = sm;              // [NT]  taps (ODD: T[d] = tap[2d + 1]; else tap[n] with tp[0] = 0), zero beyond the row
     float* rw = sm + NT;         // [FR][PL] planes of the row (ODD: [2][FR][PL], the two half-rows)
     const int iv = blockIdx.x, ia = blockIdx.y;
     const float DSD = (float)dsd_a[ia], DSO = (float)dso_a[ia];
     const float itau = DSD / (du * DSO);
-    const float v = ((float)iv + 0.5f) * dv - 0.5f * (float)nv * dv;
+    // reading P34: the cosine weight is centred on the principal ray: local pixel coordinates plus offDetector
+    const float offu = offd_a ? (float)offd_a[2 * ia] : 0.f, offv = offd_a ? (float)offd_a[2 * ia + 1] : 0.f;
+    const float v = ((float)iv + 0.5f) * dv - 0.5f * (float)nv * dv + offv;
     const size_t base = ((size_t)ia * nv + iv) * nu;
     const int nplanes = (ODD ? 2 : 1) * FR * PL;
     for (int i = threadIdx.x; i < nplanes; i += blockDim.x) rw[i] = 0.f;
@@ -99,7 +101,7 @@ fdk_conv_kernel(const float* __restrict__ b, int nu, int nv, float du, float dv,
     const float tap0 = taps ? __ldg(taps) : 0.25f;
     __syncthreads();
     for (int iu = threadIdx.x; iu < nu; iu += blockDim.x) {
-        const float u = ((float)iu + 0.5f) * du - 0.5f * (float)nu * du;
+        const float u = ((float)iu + 0.5f) * du - 0.5f * (float)nu * du + offu;
         float r = __ldg(b + base + iu) * DSD * rsqrtf(DSD * DSD + u * u + v * v);
         if (colw) r *= __ldg(colw + (size_t)ia * nu + iu);
         if (ODD) {
@@ -280,8 +282,9 @@ int launch_flatten(const float* curved, const Grid& g, const double* d_dsd, int 
 }
 
 // d_taps: nu taps for tau = 1 (device) or NULL for the Ram-Lak taps of P12; odd_only: the taps vanish at even n != 0
-int launch_fdk_filter_taps(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, int nViews, const float* d_taps,
-                           const float* d_colw, float* q, cudaStream_t st, bool odd_only) {
+// d_offd: [nViews][2] offDetector per view (device) or NULL (no displacement)
+int launch_fdk_filter_taps(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, const double* d_offd, int nViews,
+                           const float* d_taps, const float* d_colw, float* q, cudaStream_t st, bool odd_only) {
     ProfScope ps(PK_EW, st);
     // odd_only: two half-rows of ceil(nu / 2) elements; otherwise one row of nu
     const int len = odd_only ? (g.nu + 1) / 2 : g.nu;
@@ -295,7 +298,7 @@ int launch_fdk_filter_taps(const float* b, const Grid& g, const double* d_dsd, c
     auto kern = odd_only ? fdk_conv_kernel<true> : fdk_conv_kernel<false>;
     if (smem > 48 * 1024) TG_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid(g.nv, nViews);
-    kern<<<grid, 128, smem, st>>>(b, g.nu, g.nv, (float)g.du, (float)g.dv, d_dsd, d_dso, d_taps, d_colw, q, PAD, PL, NT);
+    kern<<<grid, 128, smem, st>>>(b, g.nu, g.nv, (float)g.du, (float)g.dv, d_dsd, d_dso, d_offd, d_taps, d_colw, q, PAD, PL, NT);
     TG_CUDA(cudaGetLastError());
     return TIGRE_OK;
 }

@@ -98,6 +98,24 @@ def segment_box_length(S, P, lo, hi):
     return np.maximum(tmax - tmin, 0.0) * L
 
 
+def segment_box_params(S, P, lo, hi):
+    """Entry and exit parameters (t in [0,1] along S->P) of the segment in each box; exit <= entry where it misses."""
+    d = P - S
+    tmin = np.zeros(lo.shape[:-1])
+    tmax = np.ones(lo.shape[:-1])
+    for k in range(3):
+        if d[k] == 0.0:
+            inside = (S[k] >= lo[..., k]) & (S[k] <= hi[..., k])
+            tmin = np.where(inside, tmin, 1.0)
+            tmax = np.where(inside, tmax, 0.0)
+        else:
+            t1 = (lo[..., k] - S[k]) / d[k]
+            t2 = (hi[..., k] - S[k]) / d[k]
+            tmin = np.maximum(tmin, np.minimum(t1, t2))
+            tmax = np.minimum(tmax, np.maximum(t1, t2))
+    return tmin, tmax
+
+
 def brute_force_ax(vol, geo, angles):
     """Sum over ALL voxels of (segment length inside that voxel's box) * value."""
     nA = np.asarray(angles).reshape(-1, 3).shape[0]

@@ -96,27 +96,40 @@ def test_chunked_general_geometry(tg):
         tg.set_chunk_budget(0)
 
 
-def test_chunked_sirt_iteration_c5_shape(tg):
-    # configs[4] in miniature: Siddon Ax + matched A^T b for one SIRT iteration with every array in pinned
-    # host memory, composed from the chunked projector pair and checked against the oracle's SIRT
+@pytest.mark.parametrize("ax_mode,atb_mode,tol", [("siddon", "matched", 1e-5), ("interp", "fdk", 1e-4)])
+def test_chunked_sirt_driver_matches_oracle(tg, ax_mode, atb_mode, tol):
+    # configs[4] in miniature: one and three SIRT iterations through tigre_sirt_chunked with every array in pinned host
+    # memory and a budget that forces several slabs and batches in both passes, against the oracle's SIRT
     geo, ang, rec = make_config("C5", scale=96, n_angles=20)      # 32^3, 32x32 detector
     vol = phantom_for(rec, geo)
-    b = orc.ax(vol, geo, ang, orc.SIDDON).astype(np.float32)
-    xr, _ = orc.sirt(b, geo, ang, 1, lam=1.0)
-    tg.set_chunk_budget(96 * 1024)
+    om = dict(ax_mode=orc.SIDDON if ax_mode == "siddon" else orc.INTERP, atb_mode=orc.MATCHED if atb_mode == "matched" else orc.FDK)
+    b = orc.ax(vol, geo, ang, om["ax_mode"]).astype(np.float32)
+    x0 = (0.5 * vol).astype(np.float32)
+    tg.set_chunk_budget(200 * 1024)
     try:
-        ones_v = pinned(np.ones(geo.vol_shape, np.float32))
-        ones_p = pinned(np.ones((20,) + geo.proj_shape, np.float32))
-        A1 = host(tg.Ax(ones_v, geo, ang, "siddon"))
-        At1 = host(tg.Atb(ones_p, geo, ang, "matched"))
-        W = np.where(A1 > 1e-2 * min(geo.dVoxel), 1.0 / np.maximum(A1, 1e-30), 0.0)
-        V = np.where(At1 > 1e-6 * At1.max(), 1.0 / np.maximum(At1, 1e-30), 0.0)
-        r = W * b                                            # x0 = 0
-        g = host(tg.Atb(pinned(r), geo, ang, "matched"))
-        x = np.maximum(V * g, 0.0)
+        for n_iter in (1, 3):
+            xr, rr = orc.ossart(b, geo, ang, [np.arange(20)], n_iter, lam=1.0, x0=x0.astype(np.float64), **om)
+            x, bb, r = pinned(x0), pinned(b), pinned(np.zeros_like(b))
+            hist = tg.sirt_chunked(bb, geo, ang, x, n_iter, lam=1.0, ax_mode=ax_mode, atb_mode=atb_mode, r_scratch=r)
+            assert H.rel_l2(host(x), xr) <= tol * (1 if n_iter == 1 else 3)
+            assert np.allclose(hist, rr, rtol=1e-4)
+            assert np.array_equal(bb.numpy(), b)                    # the data are untouched when a scratch array is given
+        # in-place variant: b doubles as the residual scratch (one iteration only)
+        x, bb = pinned(x0), pinned(b)
+        tg.sirt_chunked(bb, geo, ang, x, 1, ax_mode=ax_mode, atb_mode=atb_mode)
+        xr, _ = orc.ossart(b, geo, ang, [np.arange(20)], 1, lam=1.0, x0=x0.astype(np.float64), **om)
+        assert H.rel_l2(host(x), xr) <= tol
+        with pytest.raises(tg.TigreError):
+            tg.sirt_chunked(bb, geo, ang, x, 2)                     # in place needs n_iter == 1
+        # and the same step with everything resident on the device
+        tg.set_chunk_budget(0)
+        plan = tg.OssartPlan(geo, ang, [np.arange(20)], ax_mode, atb_mode)
+        xd = torch.from_numpy(x0).cuda()
+        plan.iterate(torch.from_numpy(b).cuda(), xd, 1)
+        plan.close()
+        assert H.rel_l2(host(x), host(xd)) <= 3e-6
     finally:
         tg.set_chunk_budget(0)
-    assert H.rel_l2(x, xr) <= 1e-5
 
 
 def test_chunked_budget_too_small_and_mixed_memory(tg):

@@ -1,0 +1,191 @@
+"""Index equality of the Siddon march (north_star: "Voxel/pixel index and footprint bounds must match exactly"; DESIGN.md
+reading P19(a)), the staged-box containment of the TMA backprojector (P19(b)), and the 64-bit element-index instantiations
+of the ray-driven kernels (the ones C5-sized slabs take), forced on small volumes with tigre_set_index_path(1).
+
+P19(a) as tested: tigre_Ax_index returns, from the fp32 march itself, the first / last voxel every ray gives a non-zero
+length to and the number of such voxels; the oracle returns the same from its sorted crossing list, plus the knife-edge
+measures.  A ray is flagged when its first or last segment is shorter than 1e-6 in the ray parameter (a clipped corner the
+fp32 march may or may not see: 1e-6 of a 1536 mm ray is 3e-3 voxel, ten times the march's worst crossing error) or when two
+crossings coincide to 1e-9 (a ray through a voxel edge).  On every ray that is not flagged the three numbers are EQUAL; on a
+flagged ray the march's first (last) voxel is the oracle's first or second (last or second-to-last) and the counts differ
+by at most the number of such ends.  The flagged share is the geometric probability of a clipped corner (~ threshold /
+mean segment length ~ 5e-3), not the 1e-5 SURVEY.md proposed: that number would need a threshold of 3e-6 voxel, below what
+fp32 positions resolve; DESIGN.md section 2 (P19) records the reading."""
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from tests import helpers as H
+from workloads import Geometry, circular_angles, make_config, phantom_for
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def tg():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2412_10129_b200 as m
+    m.version()
+    yield m
+    m.set_index_path(0)
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def host(t):
+    return t.detach().cpu().numpy().astype(np.float64)
+
+
+def odd_geometry(nA=5, seed=11, n=(37, 29, 23), det=(45, 31)):
+    rng = np.random.default_rng(seed)
+    geo = Geometry(nVoxel=n, dVoxel=(1.0, 1.3, 0.8), nDetector=det, dDetector=(2.1, 2.6),
+                   DSD=400.0, DSO=250.0, COR=0.7, offOrigin=(0.4, -0.6, 0.3), offDetector=(1.1, -0.9),
+                   rotDetector=(0.05, -0.04, 0.08))
+    angles = np.stack([rng.uniform(0, 2 * np.pi, nA), rng.uniform(-0.4, 0.4, nA), rng.uniform(-0.5, 0.5, nA)], 1)
+    geo.offOrigin_a = np.asarray(geo.offOrigin) + 0.2 * rng.standard_normal((nA, 3))
+    geo.rotDetector_a = np.asarray(geo.rotDetector) + 0.03 * rng.standard_normal((nA, 3))
+    geo.DSD_a = geo.DSD + rng.uniform(-3, 3, nA)
+    return geo, angles
+
+
+def check_index_equality(tg, geo, ang, ray_ids, max_flagged):
+    fl, ns = tg.Ax_index(geo, ang)
+    fl = fl.cpu().numpy().reshape(-1, 2)[ray_ids]
+    ns = ns.cpu().numpy().reshape(-1).astype(np.int64)[ray_ids]
+    o = orc.siddon_index(geo, ang, ray_ids)
+    hit = o["nseg"] > 0
+    corner_first = hit & (o["first_t"] < 1e-6)
+    corner_last = hit & (o["last_t"] < 1e-6)
+    edge = hit & (o["min_gap"] < 1e-9)
+    flagged = corner_first | corner_last | edge
+    ok = ~flagged
+    # exact on everything that is not knife-edge: first voxel, last voxel, number of voxels; misses are misses
+    assert np.array_equal(fl[ok, 0], o["first"][ok])
+    assert np.array_equal(fl[ok, 1], o["last"][ok])
+    assert np.array_equal(ns[ok], o["nseg"][ok])
+    assert np.all(fl[~hit & ok] == -1)
+    # flagged rays: what is unique still holds, the rest is one of the valid alternatives
+    f = np.flatnonzero(flagged)
+    assert np.all((fl[f, 0] == o["first"][f]) | (fl[f, 0] == o["second"][f]) | (o["nseg"][f] <= 1))
+    assert np.all((fl[f, 1] == o["last"][f]) | (fl[f, 1] == o["second_last"][f]) | (o["nseg"][f] <= 1))
+    assert np.all(np.abs(ns[f] - o["nseg"][f]) <= 3)
+    share = flagged.mean()
+    assert share <= max_flagged, share
+    return share, int(hit.sum())
+
+
+@pytest.mark.parametrize("path", [0, 1])
+def test_siddon_index_equality_c1_and_general_geometry(tg, path):
+    tg.set_index_path(path)
+    try:
+        geo, ang, _ = make_config("C1")
+        n = len(ang) * geo.nDetector[0] * geo.nDetector[1]
+        # C1 is symmetric (views at multiples of 2 pi / 64): whole fans of rays run through voxel edges
+        share, hits = check_index_equality(tg, geo, ang, np.arange(n, dtype=np.int64), 0.05)
+        assert hits > 0.4 * n
+        geo, ang = odd_geometry()
+        n = len(ang) * geo.nDetector[0] * geo.nDetector[1]
+        share, hits = check_index_equality(tg, geo, ang, np.arange(n, dtype=np.int64), 0.02)
+        assert hits > 0.3 * n
+        # z-dominant rays, source inside the volume
+        geo = Geometry(nVoxel=(24, 24, 24), dVoxel=(1, 1, 1), nDetector=(20, 20), dDetector=(1.0, 1.0), DSD=60.0, DSO=40.0)
+        ang = np.array([[0.3, 1.4, 0.2], [2.0, -1.45, 0.0]])
+        check_index_equality(tg, geo, ang, np.arange(800, dtype=np.int64), 0.03)
+        geo2 = geo.copy(DSO=6.0, DSD=14.0)
+        check_index_equality(tg, geo2, circular_angles(3, start=0.2), np.arange(1200, dtype=np.int64), 0.05)
+    finally:
+        tg.set_index_path(0)
+
+
+def test_siddon_index_equality_full_c3_sampled(tg):
+    geo, ang, _ = make_config("C3")
+    n = len(ang) * geo.nDetector[0] * geo.nDetector[1]
+    ids = np.sort(np.random.default_rng(19).choice(n, 200000, replace=False)).astype(np.int64)
+    share, hits = check_index_equality(tg, geo, ang, ids, 0.02)
+    assert hits > 0.9 * len(ids)
+
+
+def test_march_count_equals_closed_form_count(tg):
+    """tigre_Ax_count (the metric's exact |dix|+|diy|+|diz|+1, fp64, no march) against the march's own count."""
+    geo, ang = odd_geometry()
+    _, counts = tg.Ax_count(geo, ang, "siddon", return_counts=True)
+    _, ns = tg.Ax_index(geo, ang)
+    c, m = counts.cpu().numpy().astype(np.int64).ravel(), ns.cpu().numpy().astype(np.int64).ravel()
+    assert np.mean(c != m) < 0.02 and np.max(np.abs(c - m)) <= 3          # clipped corners only
+
+
+# ------------------------------------------------------------------ the 64-bit element-index instantiations
+def test_idx64_kernels_equal_idx32_and_oracle(tg):
+    geo, ang = odd_geometry()
+    vol = np.random.default_rng(1).random(geo.vol_shape, dtype=np.float32)
+    y = np.random.default_rng(2).random((len(ang),) + geo.proj_shape, dtype=np.float32)
+    ref = {m: orc.ax(vol, geo, ang, getattr(orc, m.upper())) for m in ("siddon", "interp")}
+    ref_t = {m: orc.atb_exact(y, geo, ang, getattr(orc, m.upper())) for m in ("siddon", "interp")}
+    out = {}
+    for path in (0, 1):
+        tg.set_index_path(path)
+        try:
+            for m, tol in (("siddon", 1e-5), ("interp", 1e-4)):
+                a = host(tg.Ax(dev(vol), geo, ang, m))
+                t = host(tg.Atb(dev(y), geo, ang, "exact_" + m))
+                assert H.rel_l2(a, ref[m]) <= tol, (path, m)
+                assert H.rel_l2(t, ref_t[m]) <= tol, (path, m)
+                out[(path, m)] = (a, t)
+        finally:
+            tg.set_index_path(0)
+    for m in ("siddon", "interp"):
+        assert np.array_equal(out[(0, m)][0], out[(1, m)][0])               # gather: the same sums in the same order
+        assert H.rel_l2(out[(1, m)][1], out[(0, m)][1]) <= 2e-6            # scatter: atomics, order of summation only
+
+
+def test_idx64_slabs_and_c2_scale(tg):
+    # the chunked / sharded entry points and a volume with several tiles per axis, 64-bit offsets forced
+    geo, ang, rec = make_config("C2", scale=4, n_angles=24)
+    vol = phantom_for(rec, geo)
+    tg.set_index_path(1)
+    try:
+        for m, tol in (("siddon", 1e-5), ("interp", 1e-4)):
+            ref = orc.ax(vol, geo, ang, getattr(orc, m.upper()))
+            assert H.rel_l2(host(tg.Ax(dev(vol), geo, ang, m)), ref) <= tol
+            nz = geo.nVoxel[2]
+            parts = sum(host(tg.Ax_slab(dev(vol[z0:z1]), geo, ang, z0, m)) for z0, z1 in ((0, nz // 3), (nz // 3, nz)))
+            assert H.rel_l2(parts, ref) <= tol
+    finally:
+        tg.set_index_path(0)
+
+
+@pytest.mark.skipif(not torch.cuda.is_available() or torch.cuda.mem_get_info()[0] < 40e9, reason="needs 40 GB of free HBM")
+def test_ax_above_2_31_voxels_sampled(tg):
+    """A volume that really has more than 2^31 voxels (1344^3 = 2.43e9, 9.7 GB): tigre_Ax dispatches to the 64-bit kernels by
+    itself; 10^4 seeded rays against the oracle (Siddon 1e-5, interpolated 1e-4), and the exact transposes through the adjoint
+    identity on the same arrays."""
+    n = 1344
+    geo = Geometry(nVoxel=(n, n, n), dVoxel=(0.19,) * 3, nDetector=(512, 384), dDetector=(0.8, 0.8), DSD=1536.0, DSO=1000.0,
+                   offDetector=(3.0, -2.0))
+    ang = circular_angles(6, start=0.31)
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    x = torch.rand((n, n, n), generator=gen, device="cuda", dtype=torch.float32)
+    xh = x.cpu().numpy()
+    nr = len(ang) * 512 * 384
+    ids = np.sort(np.random.default_rng(3).choice(nr, 10000, replace=False)).astype(np.int64)
+    for m, tol in (("siddon", 1e-5), ("interp", 1e-4)):
+        p = tg.Ax(x, geo, ang, m)
+        got = host(p).ravel()[ids]
+        ref = orc.ax(xh, geo, ang, getattr(orc, m.upper()), ray_ids=ids)
+        assert H.rel_l2(got, ref) <= tol, m
+        y = torch.rand(p.shape, generator=gen, device="cuda", dtype=torch.float32)
+        xt = tg.Atb(y, geo, ang, "exact_" + m)
+        lhs = float((p.double() * y.double()).sum())
+        rhs = float((x.double() * xt.double()).sum())
+        assert abs(lhs - rhs) <= 1e-5 * abs(lhs), (m, lhs, rhs)
+        del p, y, xt
+    fl, ns = tg.Ax_index(geo, ang)
+    o = orc.siddon_index(geo, ang, ids)
+    ok = (o["nseg"] > 0) & (o["first_t"] >= 1e-6) & (o["last_t"] >= 1e-6) & (o["min_gap"] >= 1e-9)
+    flh = fl.cpu().numpy().reshape(-1, 2)[ids]
+    assert np.array_equal(flh[ok, 0], o["first"][ok]) and np.array_equal(flh[ok, 1], o["last"][ok])
+    assert flh[ok].max() >= 2 ** 31                                           # indices that need 64 bits were compared

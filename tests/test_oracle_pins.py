@@ -130,6 +130,39 @@ def test_siddon_segment_list_is_ordered_and_sums_to_chord():
     assert abs(ln.sum() - H.segment_box_length(S, P, b0[None], b1[None])[0]) < 1e-12
 
 
+def test_siddon_index_first_last_voxel_by_brute_force():
+    """Reading P19(a): the first / last voxel of a ray and its segment count, against a per-voxel ray / box intersection
+    (the voxel a ray is in first is the one with the smallest entry parameter among those it crosses with positive length)."""
+    geo, angles = odd_geometry()
+    nu, nv = geo.nDetector
+    ids = np.arange(3 * nu * nv, dtype=np.int64)
+    info = orc.siddon_index(geo, angles, ids)
+    h = np.array(geo.dVoxel)
+    nx, ny, nz = geo.nVoxel
+    hit = 0
+    for r in ids:
+        ia, iv, iu = r // (nu * nv), (r % (nu * nv)) // nu, r % nu
+        p = H.view_params(geo, angles, ia)
+        c = H.voxel_centres(geo, p["offO"])
+        S, P = H.pixel_world(geo, angles, ia, iu, iv)
+        t0, t1 = H.segment_box_params(S, P, c - 0.5 * h, c + 0.5 * h)
+        pos = (t1 - t0) > 1e-13
+        assert info["nseg"][r] == pos.sum()
+        if not pos.any():
+            assert info["first"][r] == -1 and info["last"][r] == -1
+            continue
+        hit += 1
+        order = np.argsort(np.where(pos, t0, np.inf).ravel())
+        lin = order[:pos.sum()]                                       # linear index (iz*ny + iy)*nx + ix in order of entry
+        assert info["first"][r] == lin[0] and info["last"][r] == lin[-1]
+        if pos.sum() > 1:
+            assert info["second"][r] == lin[1] and info["second_last"][r] == lin[-2]
+        assert info["first_t"][r] == pytest.approx((t1 - t0).ravel()[lin[0]], abs=1e-13)
+        assert info["last_t"][r] == pytest.approx((t1 - t0).ravel()[lin[-1]], abs=1e-13)
+        assert info["min_gap"][r] >= 0 and info["min_gap"][r] <= (t1 - t0)[pos].min() + 1e-15
+    assert hit > 20
+
+
 def test_siddon_ray_clipped_to_source_detector_segment():
     # P7: a detector INSIDE the volume stops the ray there
     geo = Geometry(nVoxel=(8, 8, 8), dVoxel=(1, 1, 1), nDetector=(2, 2), dDetector=(0.5, 0.5), DSD=11.0, DSO=10.0)

@@ -7,11 +7,11 @@ phantom voxeliser (point-sampled ellipsoid membership).  Both `oracle/` and
 `paper_2412_10129_b200/` take their inputs from here; neither imports the other.
 """
 from .geometry import Geometry, circular_angles
-from .configs import CONFIGS, make_config, scaled_config
+from .configs import CONFIGS, c5_like, make_config, scaled_config
 from .phantoms import (head_ellipsoids, random_ellipsoids, voxelise,
                        voxelise_slab, porous_cylinder, poisson_noise, phantom_for,
-                       concat_ellipsoids)
+                       concat_ellipsoids, voxelise_slab_torch)
 
 __all__ = ["Geometry", "circular_angles", "CONFIGS", "make_config", "scaled_config",
            "head_ellipsoids", "random_ellipsoids", "voxelise", "voxelise_slab",
-           "porous_cylinder", "poisson_noise", "phantom_for", "concat_ellipsoids"]
+           "porous_cylinder", "poisson_noise", "phantom_for", "concat_ellipsoids", "voxelise_slab_torch", "c5_like"]

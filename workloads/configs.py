@@ -52,3 +52,14 @@ def make_config(name: str, scale: int = 1, n_angles: int | None = None):
 
 def scaled_config(name: str, scale: int, n_angles: int | None = None):
     return make_config(name, scale=scale, n_angles=n_angles)
+
+
+def c5_like(n: int, n_angles: int):
+    """configs[4]'s geometry at n^3 voxels and an n x n detector over the SAME field of view (pitches scaled by 3072 / n),
+    with n_angles views over 2 pi: what the host-chunking runs use when the box cannot hold the full 207 GB."""
+    r = CONFIGS["C5"]
+    f = r["n"] / float(n)
+    geo = Geometry(nVoxel=(n, n, n), dVoxel=(r["d"] * f,) * 3, nDetector=(n, n), dDetector=(r["ddet"] * f,) * 2,
+                   DSD=1536.0, DSO=1000.0, accuracy=0.5)
+    rec = dict(r, name="C5", scale=f, nA=n_angles)
+    return geo, circular_angles(n_angles), rec

@@ -90,6 +90,36 @@ def voxelise_slab(ell, geo, z0: int, z1: int, dtype=np.float32):
     return out
 
 
+def voxelise_slab_torch(ell, geo, z0: int, z1: int, device="cuda"):
+    """voxelise_slab evaluated with torch on `device` (the same membership test in float64, the same bounding boxes): for
+    volumes of tens of GB, where the numpy loop would take an hour.  Returns a float32 tensor [z1 - z0][ny][nx] on `device`.
+    Input synthesis only; the consumer copies it wherever both sides read it from."""
+    import torch
+    nx, ny, nz = geo.nVoxel
+    dx, dy, dz = geo.dVoxel
+    ox, oy, oz = geo.offOrigin
+    x = ox + (np.arange(nx) + 0.5) * dx - 0.5 * nx * dx
+    y = oy + (np.arange(ny) + 0.5) * dy - 0.5 * ny * dy
+    z = oz + (np.arange(z0, z1) + 0.5) * dz - 0.5 * nz * dz
+    tx, ty, tz = (torch.from_numpy(a).to(device) for a in (x, y, z))
+    out = torch.zeros((z1 - z0, ny, nx), dtype=torch.float32, device=device)
+    for c, ax, Q, rho in zip(ell["centre"], ell["axes"], ell["Q"], ell["rho"]):
+        ext = np.sqrt(((Q * ax[None, :]) ** 2).sum(axis=1))
+        sel = [np.nonzero(np.abs(coord - ck) <= ek)[0] for coord, ck, ek in ((x, c[0], ext[0]), (y, c[1], ext[1]), (z, c[2], ext[2]))]
+        if any(k.size == 0 for k in sel):
+            continue
+        sx, sy, sz = (slice(int(k[0]), int(k[-1]) + 1) for k in sel)
+        X = tx[sx][None, None, :] - float(c[0])
+        Y = ty[sy][None, :, None] - float(c[1])
+        Z = tz[sz][:, None, None] - float(c[2])
+        s = None
+        for k in range(3):
+            lk = (float(Q[0, k]) * X + float(Q[1, k]) * Y + float(Q[2, k]) * Z) / float(ax[k])
+            s = lk * lk if s is None else s + lk * lk
+        out[sz, sy, sx] += (s <= 1.0).to(torch.float32) * float(np.float32(rho))
+    return out
+
+
 def voxelise(ell, geo, dtype=np.float32, slab: int = 64):
     nz = geo.nVoxel[2]
     return np.concatenate([voxelise_slab(ell, geo, z0, min(nz, z0 + slab), dtype)
