@@ -384,7 +384,9 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
                 const long long z = fl[q] / nxy, rem = fl[q] - z * nxy, x = rem / p.ny, y = rem - x * p.ny;
                 fl[q] = z * nxy + y * p.nx + x;
             }
-        track[2 * out] = fl[0], track[2 * out + 1] = fl[1];
+        // the march runs towards increasing D whichever way the ray points: "first" is the voxel nearest the source
+        const bool rev = dD < 0.0;
+        track[2 * out] = rev ? fl[1] : fl[0], track[2 * out + 1] = rev ? fl[0] : fl[1];
         counts[out] = r.nseg;
         return;
     }

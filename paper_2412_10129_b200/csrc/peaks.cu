@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(PK_THREADS) pk_smem_kernel(float* out, int ite
     int idx = threadIdx.x;
     for (int i = 0; i < iters; ++i) {
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
+        for (int u = 0; u < 4; ++u) {   // four DISTINCT 16-byte words per thread and iteration (the array holds 4 per thread)
             const float4 v = sm[(idx + u * PK_THREADS) & (PK_THREADS * 4 - 1)];   // consecutive lanes, consecutive 16-byte words
             acc.x += v.x, acc.y += v.y, acc.z += v.z, acc.w += v.w;
         }
@@ -68,12 +68,15 @@ __global__ void __launch_bounds__(PK_THREADS) pk_smem_kernel(float* out, int ite
 __global__ void __launch_bounds__(PK_THREADS) pk_l1_kernel(const float* __restrict__ buf, float* out, int iters) {
     const int warp = (blockIdx.x * PK_THREADS + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     const float* p = buf + (size_t)warp * 1024 + lane * 32;
+    // the word each lane reads within ITS line depends on the value just loaded (the buffer holds zeros, which the compiler
+    // cannot know): a loop-invariant address would be hoisted out of the loop.  64 resident warps per SM hide the chain.
     float acc = 0.f;
+    int off = lane;
     for (int i = 0; i < iters; ++i) {
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-            float v;
-            asm volatile("ld.global.ca.f32 %0, [%1];" : "=f"(v) : "l"(p + ((i * 8 + u) & 31)));
+            const float v = __ldca(p + (off & 31));
+            off += 1 + __float_as_int(v);
             acc += v;
         }
     }
@@ -148,7 +151,7 @@ int microbench(int kind, double* value, cudaStream_t st) {
         case TIGRE_PEAK_SMEM: {
             const int iters = 1 << 13;
             TG_TRY(best_ms([&] { pk_smem_kernel<<<ctas, PK_THREADS, 0, st>>>(out, iters); return TIGRE_OK; }, st, ms));
-            *value = (double)ctas * PK_THREADS * (double)iters * 8.0 * 16.0 / (ms * 1e-3);
+            *value = (double)ctas * PK_THREADS * (double)iters * 4.0 * 16.0 / (ms * 1e-3);
             return TIGRE_OK;
         }
         case TIGRE_PEAK_L1_LINES: {

@@ -52,7 +52,7 @@ def test_ossart_cgls_fdk_bitwise_with_and_without_workspace(tg):
     torch.cuda.synchronize()
     for a, r in zip(got[:1] + got[2:5], ref[:1] + ref[2:5]):
         assert torch.equal(a, r)                     # same kernels, same order: bitwise
-    assert np.array_equal(got[1], ref[1])
+    assert np.allclose(got[1], ref[1], rtol=1e-12, atol=0)     # the norm is summed with fp64 atomics: block order only
     assert float((got[5] - ref[5]).norm() / ref[5].norm()) < 2e-6   # atomics: order of summation only
 
 
@@ -64,7 +64,7 @@ def test_workspace_too_small_fails_cleanly_and_plans_pin_it(tg):
     tg.set_workspace(small)
     try:
         with pytest.raises(tg.TigreError) as e:
-            tg.Atb(b, geo, ang, "exact_siddon")      # needs a scratch volume
+            tg.cgls(b, geo, ang, 1)                  # needs two projection-sized and two volume-sized buffers
         assert e.value.code == -4
         assert tg.workspace_stats()[0] == 0          # the failed call left nothing behind
     finally:
@@ -89,7 +89,7 @@ def test_chunked_path_sizes_itself_to_the_workspace(tg):
     geo, ang, rec = make_config("C5", scale=96)
     vol = phantom_for(rec, geo)
     hv = torch.from_numpy(vol).pin_memory()
-    ws = torch.empty(3 << 20, dtype=torch.uint8, device="cuda")
+    ws = torch.empty(400 << 10, dtype=torch.uint8, device="cuda")      # budget = half of it: several slabs and batches
     tg.set_workspace(ws)
     try:
         p = tg.Ax(hv, geo, ang, "siddon")
