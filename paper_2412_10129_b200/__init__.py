@@ -151,6 +151,33 @@ def _new(shape, like=None, device=None):
     return torch.empty(shape, dtype=torch.float32, device=device or "cuda")
 
 
+class _Registered:
+    """Keeps a cudaHostRegister'ed range registered for as long as the tensor that owns it lives."""
+
+    def __init__(self, ptr):
+        self.ptr = ptr
+
+    def __del__(self):
+        try:
+            import torch
+            torch.cuda.cudart().cudaHostUnregister(self.ptr)
+        except Exception:
+            pass
+
+
+def pinned_empty(shape):
+    """A float32 host tensor of exactly prod(shape) * 4 bytes, page-locked with cudaHostRegister: what the chunked path wants
+    for arrays of tens of GB (torch's own pinned allocator rounds every request up to a power of two: 116 GB would take 128 GiB)."""
+    import torch
+    t = torch.empty(shape, dtype=torch.float32)
+    if t.numel():
+        rc = torch.cuda.cudart().cudaHostRegister(t.data_ptr(), t.numel() * 4, 0)
+        if int(rc) != 0:
+            raise RuntimeError(f"cudaHostRegister failed ({rc}) for {t.numel() * 4} bytes")
+        t._tigre_registration = _Registered(t.data_ptr())
+    return t
+
+
 def vol_shape(geo):
     return (geo.nVoxel[2], geo.nVoxel[1], geo.nVoxel[0])
 

@@ -2,9 +2,10 @@
 projections together EXCEED the library's default device budget (3/4 of free HBM; no tigre_set_chunk_budget), in pinned
 host memory, through tigre_Ax and one tigre_sirt_chunked iteration, with the oracle on 10^4 seeded rays and 10^4 seeded
 voxels as configs[4] prescribes.  Full C5 (207 GB) does not fit the box's host RAM, so the volume and detector keep C5's
-full size (3072^3 voxels, 3072^2 pixels) and the views are thinned to what the host holds (512 of them: 116 + 19 GB).
+full size (3072^3 voxels, 3072^2 pixels) and the views are thinned to the fewest that still exceed the budget
+(on a 183 GB B200: 147 GB of budget, 1024 views: 116 + 39 GB of pinned host arrays).
 Slabs of 768 x 3072^2 = 7.2e9 voxels take the 64-bit element-index kernels.  Size-gated by free host RAM; smaller boxes
-run the largest n that still exceeds the budget, or skip."""
+skip."""
 import os
 
 import numpy as np
@@ -23,10 +24,12 @@ def _pick_size():
     avail = psutil.virtual_memory().available
     free = torch.cuda.mem_get_info()[0]
     budget = free // 4 * 3
-    for n, nA in ((3072, 512), (2816, 768), (2560, 1200)):
-        need = 4 * (n ** 3 + nA * n * n)
-        if need > budget and need + (24 << 30) < avail:
-            return n, nA, need, budget
+    n = 3072
+    # as few views as make volume + projections exceed the budget by 3 % (a multiple of 64; never fewer than 512)
+    nA = max(512, -(-int(1.03 * budget - 4 * n ** 3) // (4 * n * n * 64)) * 64)
+    need = 4 * (n ** 3 + nA * n * n)
+    if need > budget and need + (24 << 30) < avail and nA <= 2400:
+        return n, nA, need, budget
     return None
 
 
@@ -38,17 +41,26 @@ def test_c5_shaped_run_beyond_the_default_budget():
         pytest.skip("TIGRE_SKIP_BIG set")
     pick = _pick_size()
     if pick is None:
-        pytest.skip("host RAM cannot hold a problem larger than the device budget")
+        pytest.skip("host RAM cannot hold a C5-sized volume plus enough views to exceed the device budget")
+    import time
     import paper_2412_10129_b200 as tg
+    t_start = time.time()
+
+    def log(msg):
+        print(f"[big {time.time() - t_start:6.1f}s] {msg}", flush=True)
+
     n, nA, need, budget = pick
+    log(f"n={n} nA={nA} host arrays {need / 1e9:.1f} GB, default device budget {budget / 1e9:.1f} GB")
     tg.set_chunk_budget(0)
     geo, ang, rec = c5_like(n, nA)
     ell = random_ellipsoids(64, geo.nVoxel[0] * geo.dVoxel[0], rec["seed"])
-    x = torch.empty(geo.vol_shape, dtype=torch.float32, pin_memory=True)
-    b = torch.empty((nA,) + geo.proj_shape, dtype=torch.float32, pin_memory=True)
+    x = tg.pinned_empty(geo.vol_shape)                  # exact-size page-locked arrays (torch's pinned allocator rounds up to 2^k)
+    b = tg.pinned_empty((nA,) + geo.proj_shape)
+    log("pinned arrays allocated")
     for z0 in range(0, n, 64):
         x[z0:z0 + 64].copy_(voxelise_slab_torch(ell, geo, z0, min(n, z0 + 64)))
     torch.cuda.synchronize()
+    log("phantom voxelised")
     torch.cuda.empty_cache()
     xn, bn = x.numpy(), b.numpy()
     rng = np.random.default_rng(4)
@@ -58,19 +70,24 @@ def test_c5_shaped_run_beyond_the_default_budget():
     # ---- tigre_Ax from pinned memory, default budget
     tg.Ax(x, geo, ang, "siddon", out=b)
     h2d, d2h, n_slabs, n_batches = tg.chunk_stats()
+    log(f"tigre_Ax done: {n_slabs} z-slabs x {n_batches} view batches, H2D {h2d / 1e9:.1f} GB, D2H {d2h / 1e9:.1f} GB")
     assert n_slabs >= 2 and n_batches >= 2 and h2d >= n_batches * 4 * n ** 3          # the volume went up once per batch
     assert (n // n_slabs) * n * n >= 2 ** 31                                          # slabs beyond 32-bit element offsets
     ax_true = orc.ax(xn, geo, ang, orc.SIDDON, ray_ids=rays)
     assert H.rel_l2(bn.ravel()[rays].astype(np.float64), ax_true) <= 1e-5
     assert np.count_nonzero(ax_true) > 3000
+    log("Ax checked on 10^4 rays")
 
     # ---- one SIRT iteration from x0 = x / 2 (library driver; b doubles as the residual scratch)
     x.mul_(0.5)
     x0_v = xn.ravel()[vox].astype(np.float64)
     b_r = bn.ravel()[rays].astype(np.float64)
     ax0 = orc.ax(xn, geo, ang, orc.SIDDON, ray_ids=rays)
-    bnorm = float(torch.linalg.vector_norm(b.view(-1)[::1], dtype=torch.float64))
+    # ||b|| in fp64, 16 views at a time (an upcast of the whole array would need another 60 GB of host memory)
+    bnorm = float(np.sqrt(sum(float((b[a:a + 16].double() ** 2).sum()) for a in range(0, nA, 16))))
+    log("oracle A x0 on the sampled rays, ||b|| done")
     hist = tg.sirt_chunked(b, geo, ang, x, 1, lam=1.0)
+    log(f"tigre_sirt_chunked done, residual {hist[0]:.6e}")
     # pass 1: r = W (b - A x0), W = 1 / (chord of the ray through the volume box) (closed form, independent geometry)
     per = n * n
     chord = np.zeros(len(rays))
@@ -94,3 +111,4 @@ def test_c5_shaped_run_beyond_the_default_budget():
     assert np.all(got[U == 0.0] == np.maximum(x0_v[U == 0.0], 0.0))              # voxels no ray sees keep their value
     upd = got[seen] - x0_v[seen]
     assert H.rel_l2(upd, x1_ref - x0_v[seen]) <= 1e-4 and np.linalg.norm(upd) > 0.01 * np.linalg.norm(x0_v[seen])
+    log("SIRT iteration checked on 10^4 rays and 10^4 voxels")
