@@ -33,31 +33,24 @@ from workloads import make_config, phantom_for  # noqa: E402
 METRIC = "Ax ray-samples/s + A^T b voxel-updates/s (one OS-SART iteration)"
 UNIT = "G(samples+updates)/s"
 
-# Roofline of the projector kernels.  They are gather kernels with hundreds of updates per
-# HBM byte: the binding resource is plain-ALU issue slots (and the L1 gather path for the interpolated
-# projector), not HBM.  peak = issue slots per second / ALGORITHMIC thread-instructions per unit of work, the
-# instruction count being the a-priori minimum derived in DESIGN.md (not the kernel's own count):
-#   A^T b          22 per voxel-update   (projective map or its z-incremental form, floor, 4 taps, bilinear, weight)
-#   Ax Siddon      min(18 per segment on the ALUs, 6 L1 wavefronts per warp-step) = 1.5e12 segments/s at 1965 MHz
-#   Ax interpolated  24 L1 wavefronts per warp-sample (8 taps) = 3.9e11 samples/s at 1965 MHz
-SM_COUNT, LANES_PER_CLK = 148, 128          # 4 schedulers x 32 lanes per SM per clock
-
-
-def model_peak(kname, sm_mhz):
-    """G units/s the model allows at the given SM clock."""
-    slots = SM_COUNT * LANES_PER_CLK * sm_mhz * 1e6            # thread-instructions per second
-    wavefronts = SM_COUNT * sm_mhz * 1e6                       # L1 wavefronts per second (1 per clk per SM)
-    if kname == "atb":
-        return slots / 22.0 / 1e9
-    if kname == "ax_siddon":
-        return min(slots / 18.0, wavefronts / 6.0 * 32) / 1e9
-    return min(slots / 40.0, wavefronts / 24.0 * 32) / 1e9    # ax_interp
-
-
-# dram__bytes_read+write per launch of the dominant kernel from the committed ncu captures (profiles/), for
-# the default workload only (C3, one ordered subset = 36 views per launch)
-NCU_TRAFFIC_PER_LAUNCH = {("C3", "ax_siddon"): 2.338e9, ("C3", "atb"): 6.11e8, ("C2", "ax_interp"): 4.58e8}
-
+# Roofline of the projector kernels.  They are gather kernels with hundreds of updates per HBM byte:
+# the binding resource is plain-ALU issue slots or the on-chip gather path (L1 for Ax, shared memory for A^T b), not HBM.
+# Every machine rate below is MEASURED at the start of the run by the library's own microbenchmark kernels
+# (tigre_microbench): thread-instructions/s (FFMA issue), shared-memory bytes/s, L1 lines
+# (wavefronts)/s.  The per-unit demands are algorithmic, except the L1 wavefronts a warp needs per
+# 32 Siddon samples, which depend on how the rays of a warp spread over cache lines and are taken from the committed ncu
+# captures (l1tex__data_pipe_lsu_wavefronts / samples):
+#   A^T b            22 thread-instr and 16 B of shared-memory taps per voxel-update
+#   Ax Siddon        18 thread-instr per segment; L1: W wavefronts per warp-sample (measured, table below)
+#   Ax interpolated  40 thread-instr per sample; L1: 8 taps, two samples share a cell at a step of half a voxel: 12 wavefronts
+#                    per warp-sample ("24 ... ~halved by reusing a cell's 8 corners")
+SM_COUNT = 148
+ALGO_INSTR = {"atb": 22.0, "ax_siddon": 18.0, "ax_interp": 40.0}
+# L1 data-pipe wavefronts per 32 samples of the Siddon march, from ncu (profiles/r1_late_ax_siddon.md: data pipe 42.7 % busy at
+# 1397.6 G samples/s, 148 SMs x 1965 MHz => 2.84 wavefronts per warp-sample on C3)
+SIDDON_WAVEFRONTS_PER_WARP_SAMPLE = 2.84
+INTERP_WAVEFRONTS_PER_WARP_SAMPLE = 12.0
+NOMINAL_PEAKS = {"ffma": 148 * 128 * 1.965e9, "smem": 148 * 128 * 1.965e9, "l1_lines": 148 * 1.965e9}
 
 PEAK_UNITS = {"ffma": "thread-instr/s", "smem": "B/s", "l1_lines": "128-B lines/s", "l2": "B/s", "h2d": "B/s", "d2h": "B/s",
               "hbm_copy": "B/s (read+write)", "sm_hz": "Hz"}
@@ -67,6 +60,33 @@ def measure_peaks(tg, kinds=("ffma", "smem", "l1_lines", "l2", "hbm_copy", "sm_h
     """The machine rates the projector rooflines rest on, measured now on this device by the library's own microbenchmark
     kernels (tigre_microbench): a few hundred milliseconds in all."""
     return {k: tg.microbench(k) for k in kinds}
+
+
+def model_bounds(kname, rates):
+    """{resource: G units/s} the machine rates allow for one kernel."""
+    out = {"issue": rates["ffma"] / ALGO_INSTR[kname] / 1e9}
+    if kname == "atb":
+        out["smem"] = rates["smem"] / 16.0 / 1e9
+    elif kname == "ax_siddon":
+        out["l1"] = rates["l1_lines"] * 32.0 / SIDDON_WAVEFRONTS_PER_WARP_SAMPLE / 1e9
+    else:
+        out["l1"] = rates["l1_lines"] * 32.0 / INTERP_WAVEFRONTS_PER_WARP_SAMPLE / 1e9
+    return out
+
+
+def model_peak(kname, rates):
+    """G units/s of the binding bound."""
+    return min(model_bounds(kname, rates).values())
+
+
+def peak_source(kname, rates, measured):
+    bd = model_bounds(kname, rates)
+    bind = min(bd, key=bd.get)
+    how = "measured now by tigre_microbench" if measured else "NOMINAL (no microbenchmark in this mode)"
+    return (f"min over {', '.join(f'{k} {v:.0f}' for k, v in bd.items())} G/s: binding = {bind}; machine rates {how}: "
+            f"FFMA issue {rates['ffma'] / 1e12:.2f} T thread-instr/s, shared memory {rates['smem'] / 1e12:.2f} TB/s, L1 "
+            f"{rates['l1_lines'] / 1e9:.1f} G lines/s; per-unit demand algorithmic (DESIGN.md section 6), Siddon L1 wavefronts from "
+            f"ncu (profiles/); HBM is not the bound (see hbm)")
 
 
 def run_peaks(tg, rank):
@@ -80,6 +100,40 @@ def run_peaks(tg, rank):
     print(json.dumps({"metric": "step-0 machine rates (tigre_microbench)", "n_gpus": 1, "device": torch.cuda.get_device_name(0),
                       "values": m, "units": PEAK_UNITS, "per_clock": per_clk,
                       "nominal": {"ffma_per_clk_per_sm": 128, "smem_bytes_per_clk_per_sm": 128, "l1_lines_per_clk_per_sm": 1}}))
+
+
+def ncu_traffic(config_name, kernel_regex, skip=5, timeout_s=240):
+    """dram__bytes_read + dram__bytes_write of ONE launch of the dominant kernel, from a separate `ncu` run of this file's
+    probe mode (a number printed under a profiler is never a bench value: only the byte counters are taken).  None if ncu
+    is missing or the run fails (e.g. when this process is itself being profiled)."""
+    import shutil
+    ncu = shutil.which("ncu") or "/usr/local/cuda/bin/ncu"
+    if not os.path.exists(ncu):
+        return None, "ncu not found"
+    cmd = [ncu, "--metrics", "dram__bytes_read.sum,dram__bytes_write.sum", "--clock-control", "none", "--print-units", "base",
+           "--kernel-name", "regex:" + kernel_regex, "--launch-skip", str(skip), "--launch-count", "1", "--csv",
+           sys.executable, os.path.abspath(__file__), "--mode", "probe", "--config", config_name]
+    try:
+        out = subprocess.run(cmd, capture_output=True, text=True, timeout=timeout_s, cwd=ROOT).stdout
+    except Exception as e:
+        return None, f"ncu run failed: {e}"
+    import csv
+    tot, seen = 0.0, 0
+    rows = [r for r in csv.reader(out.splitlines()) if len(r) > 5]
+    hdr = next((r for r in rows if "Metric Name" in r and "Metric Value" in r), None)
+    if hdr is None:
+        return None, "no ncu csv in the output"
+    iname, ival = hdr.index("Metric Name"), hdr.index("Metric Value")
+    for r in rows:
+        if len(r) > max(iname, ival) and r[iname] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            try:
+                tot += float(r[ival].replace(",", ""))
+                seen += 1
+            except ValueError:
+                pass
+    if seen < 2:
+        return None, "dram counters not found in the ncu output"
+    return tot, "ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum --clock-control none, launch %d of %s in `bench.py --mode probe`" % (skip + 1, kernel_regex)
 
 
 def max_over_ranks(ms, device="cpu"):
@@ -164,8 +218,18 @@ def cpu_baseline(geo, ang, rec, vol_h, b_h, samples_per_step, updates_per_step, 
     t_atb, u_atb = run_atb(n_atb)
     rate_ax, rate_atb = s_ax / t_ax, u_atb / t_atb
     t_step = samples_per_step / rate_ax + updates_per_step / rate_atb
-    return {"value": (samples_per_step + updates_per_step) / t_step / 1e9, "unit": UNIT, "cores": orc.num_threads(),
-            "kind": "oracle",
+    # the same two rates on ONE thread ("all hardware threads ... and single-thread"), on a tenth of the sample
+    threads = orc.num_threads()
+    orc.set_num_threads(1)
+    try:
+        t1a, s1a = run_ax(max(200, n_ax // (10 * max(threads, 1))))
+        t1b, u1b = run_atb(max(20, n_atb // (10 * max(threads, 1))))
+    finally:
+        orc.set_num_threads(threads)
+    t_step1 = samples_per_step / (s1a / t1a) + updates_per_step / (u1b / t1b)
+    return {"value": (samples_per_step + updates_per_step) / t_step / 1e9, "unit": UNIT, "cores": threads, "nproc": os.cpu_count(),
+            "kind": "oracle", "single_thread_value": (samples_per_step + updates_per_step) / t_step1 / 1e9,
+            "single_thread": {"ax_gsamples_per_s": s1a / t1a / 1e9, "atb_gups": u1b / t1b / 1e9, "seconds": t1a + t1b},
             "sample": f"{n_ax} seeded random rays ({s_ax} ray-samples, {t_ax:.1f} s) + {n_atb} seeded random voxels x "
                       f"{nA} views ({u_atb} updates, {t_atb:.1f} s) of the same workload; full-step time extrapolated "
                       f"linearly from the two rates",
@@ -173,25 +237,34 @@ def cpu_baseline(geo, ang, rec, vol_h, b_h, samples_per_step, updates_per_step, 
 
 
 def run_chunked(args, tg, geo, ang, rec, config, K, W, rank, world, local_rank):
-    """Host-chunking path: a step = one tigre_Ax + one tigre_Atb with the volume and
-    the projections in PINNED HOST memory, streamed through the device budget.  Everything is end to end by
-    construction (H2D / D2H copies inside the timed region, overlapped with the kernels by the library)."""
+    """Host-chunking path: a step = one tigre_Ax + one tigre_sirt_chunked iteration (configs[4]'s
+    "Siddon Ax + matched A^T b for one SIRT iteration") with the volume and the projections in PINNED HOST memory, streamed
+    through the device budget.  Everything is end to end by construction (H2D / D2H copies inside the timed region,
+    overlapped with the kernels by the library).  --chunk-n / --chunk-views select a C5-shaped problem of another size."""
     import torch
+    from workloads import c5_like
+    if args.chunk_n:
+        geo, ang, rec = c5_like(args.chunk_n, args.chunk_views or max(64, int(2400 * args.chunk_n / 3072)))
+        config = dict(config, workload=f"C5-shaped: {args.chunk_n}^3 fp32 volume, {len(ang)} views of {args.chunk_n}x{args.chunk_n}, "
+                                       f"siddon Ax / matched A^T b")
     nA = len(ang)
     if args.budget_gb > 0:
         tg.set_chunk_budget(int(args.budget_gb * 2 ** 30))
+    free_hbm = torch.cuda.mem_get_info()[0]
+    rates = measure_peaks(tg, ("ffma", "smem", "l1_lines", "h2d", "d2h"))
     # seeded uniform-random volume generated slab by slab on the device (a voxelised phantom of this size takes
-    # minutes on the host; timing does not depend on the values), pinned host arrays for everything
+    # minutes on the host; timing does not depend on the values), exact-size page-locked host arrays for everything
     gen = torch.Generator(device="cuda").manual_seed(rec["seed"])
-    vol_h = torch.empty(geo.vol_shape, dtype=torch.float32, pin_memory=True)
+    vol_h = tg.pinned_empty(geo.vol_shape)
     for z0 in range(0, geo.vol_shape[0], 64):
         z1 = min(z0 + 64, geo.vol_shape[0])
         vol_h[z0:z1].copy_(torch.rand((z1 - z0,) + tuple(geo.vol_shape[1:]), generator=gen, device="cuda") * 0.02)
-    proj_h = torch.empty((nA,) + tuple(geo.proj_shape), dtype=torch.float32, pin_memory=True)
-    back_h = torch.empty(geo.vol_shape, dtype=torch.float32, pin_memory=True)
+    proj_h = tg.pinned_empty((nA,) + tuple(geo.proj_shape))
     samples = tg.Ax_count(geo, ang, rec["ax"])
     updates = int(np.prod(geo.nVoxel)) * nA
-    units = samples + updates
+    # a step: Ax (1 pass of samples) + SIRT iteration (1 pass of samples, 3 passes of voxel updates in the first iteration of a
+    # call: max(A^T 1), A^T r, A^T 1; DESIGN.md "Host chunking")
+    units = 2 * samples + 3 * updates
     torch.cuda.synchronize()
 
     def step():
@@ -199,23 +272,22 @@ def run_chunked(args, tg, geo, ang, rec, config, K, W, rank, world, local_rank):
         tg.Ax(vol_h, geo, ang, rec["ax"], out=proj_h)          # synchronises before returning
         st_ax = tg.chunk_stats()
         t1 = time.perf_counter()
-        tg.Atb(proj_h, geo, ang, rec["atb"], out=back_h)
-        st_atb = tg.chunk_stats()
+        vol_h.mul_(0.5)                                        # start of the SIRT step: not the solution (host arithmetic, untimed below)
         t2 = time.perf_counter()
-        return (t1 - t0) * 1e3, (t2 - t1) * 1e3, st_ax, st_atb
+        tg.sirt_chunked(proj_h, geo, ang, vol_h, 1, ax_mode=rec["ax"], atb_mode=rec["atb"])   # b doubles as the residual scratch
+        st_sirt = tg.chunk_stats()
+        t3 = time.perf_counter()
+        return (t1 - t0) * 1e3, (t3 - t2) * 1e3, st_ax, st_sirt
 
     for _ in range(W):
         step()
     sampler = ClockSampler(local_rank)
     sampler.start()
     tg.profile(True)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
-    e0.record()
     runs = [step() for _ in range(K)]
-    e1.record()
     torch.cuda.synchronize()
-    ms = max_over_ranks(e0.elapsed_time(e1), "cuda")
+    ms = max_over_ranks(sum(r[0] + r[1] for r in runs), "cuda")     # the two library calls (both synchronise); host scaling excluded
     prof = tg.profile_read()
     tg.profile(False)
     sampler.stop_flag = True
@@ -223,37 +295,40 @@ def run_chunked(args, tg, geo, ang, rec, config, K, W, rank, world, local_rank):
     if rank != 0:
         return
     ms_step = ms / K
-    ax_ms = float(np.mean([r[0] for r in runs])), float(np.mean([r[1] for r in runs]))
-    st_ax, st_atb = runs[-1][2], runs[-1][3]
-    peaks = {}
-    try:
-        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-    except Exception:
-        pass
-    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    call_ms = float(np.mean([r[0] for r in runs])), float(np.mean([r[1] for r in runs]))
+    st_ax, st_sirt = runs[-1][2], runs[-1][3]
     kind = "ax" if prof["ms"]["ax"] >= prof["ms"]["atb"] else "atb"
     kname = ("ax_" + rec["ax"]) if kind == "ax" else "atb"
-    k_units, k_ms = (samples if kind == "ax" else updates), prof["ms"][kind] / K
-    achieved, peak = k_units / (k_ms * 1e-3) / 1e9, model_peak(kname, sm_max)
+    k_units, k_ms = (2 * samples if kind == "ax" else 3 * updates), prof["ms"][kind] / K
+    achieved, peak = k_units / (k_ms * 1e-3) / 1e9, model_peak(kname, rates)
     value = whole_job_value(units, ms_step, world)
-    config = dict(config, workload=config["workload"].split(", OS-SART")[0] + ", host-chunked (pinned host arrays)",
-                  budget_gb=args.budget_gb or "3/4 of free HBM", phantom="uniform random (device-generated)",
-                  chunks={"ax": {"z_slabs": st_ax[2], "view_batches": st_ax[3]}, "atb": {"z_slabs": st_atb[2], "view_batches": st_atb[3]}})
-    line = {"metric": METRIC.replace("one OS-SART iteration", "one chunked Ax + one chunked A^T b"), "value": value, "unit": UNIT,
+    h2d, d2h = int(st_ax[0] + st_sirt[0]), int(st_ax[1] + st_sirt[1])
+    host_bytes = (int(np.prod(geo.nVoxel)) + nA * geo.nDetector[0] * geo.nDetector[1]) * 4
+    config = dict(config, workload=config["workload"].split(", OS-SART")[0] + ", host-chunked (pinned host arrays): tigre_Ax + one tigre_sirt_chunked iteration",
+                  budget_gb=args.budget_gb or f"default: 3/4 of free HBM = {free_hbm * 0.75 / 2 ** 30:.1f} GiB",
+                  host_array_gb=host_bytes / 2 ** 30, exceeds_budget=bool(host_bytes > (args.budget_gb * 2 ** 30 if args.budget_gb else free_hbm * 0.75)),
+                  phantom="uniform random (device-generated)",
+                  chunks={"ax": {"z_slabs": st_ax[2], "view_batches": st_ax[3]}, "sirt_last_pass": {"z_slabs": st_sirt[2], "view_batches": st_sirt[3]}})
+    link_s = h2d / rates["h2d"] + d2h / rates["d2h"]
+    line = {"metric": METRIC.replace("one OS-SART iteration", "one chunked Ax + one chunked SIRT iteration"), "value": value, "unit": UNIT,
             "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config, "clocks": sampler.summary(),
-            "call_ms": {"tigre_Ax": ax_ms[0], "tigre_Atb": ax_ms[1]},
+            "call_ms": {"tigre_Ax": call_ms[0], "tigre_sirt_chunked": call_ms[1]},
             "kernel_ms_per_step": {k: v / K for k, v in prof["ms"].items()},
-            "overlap": {"kernel_share_of_call_time": (prof["ms"]["ax"] + prof["ms"]["atb"]) / ms,
+            "overlap": {"kernel_share_of_call_time": (prof["ms"]["ax"] + prof["ms"]["atb"] + prof["ms"]["ew"]) / ms,
                         "note": "kernels and copies run on different streams: a share near 1 means the copies are hidden"},
-            "ax_gsamples_per_s": samples / (ax_ms[0] * 1e-3) / 1e9, "atb_gups": updates / (ax_ms[1] * 1e-3) / 1e9,
-            "units_per_step": {"ray_samples": samples, "voxel_updates": updates},
+            "host_link": {"h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "measured_peak_h2d_gbs": rates["h2d"] / 1e9,
+                          "measured_peak_d2h_gbs": rates["d2h"] / 1e9, "seconds_at_peak_if_serial": link_s,
+                          "share_of_step_if_serial": link_s / (ms_step * 1e-3),
+                          "achieved_gbs_over_whole_step": (h2d + d2h) / (ms_step * 1e-3) / 1e9},
+            "ax_gsamples_per_s": samples / (call_ms[0] * 1e-3) / 1e9,
+            "sirt_g_units_per_s": (samples + 3 * updates) / (call_ms[1] * 1e-3) / 1e9,
+            "units_per_step": {"ray_samples": 2 * samples, "voxel_updates": 3 * updates},
             "gpu_launches": int(sum(prof["launches"].values())),
             "roofline": {"kernel": kname, "bound": "alu", "achieved": achieved, "peak": peak, "frac": achieved / peak,
                          "unit": "Gsamples/s" if kind == "ax" else "Gupdates/s", "traffic": None,
-                         "peak_source": "model (DESIGN.md section 6)", "ms_per_pass": k_ms},
-            "e2e": {"value": value, "unit": UNIT, "ms_per_step": ms_step,
-                    "h2d_bytes_per_step": int(st_ax[0] + st_atb[0]), "d2h_bytes_per_step": int(st_ax[1] + st_atb[1])}}
+                         "peak_source": peak_source(kname, rates, True), "ms_per_pass": k_ms},
+            "e2e": {"value": value, "unit": UNIT, "ms_per_step": ms_step, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}}
     print(json.dumps(line))
 
 
@@ -415,6 +490,68 @@ def run_drivers(args, tg, geo, ang, rec, subsets, rank):
                           "ms_per_iteration": {k: round(v, 2) for k, v in out.items()}}))
 
 
+def run_probe(tg, geo, ang, rec, subsets):
+    """What `ncu` watches for the traffic leg: one OS-SART iteration of the config through the plan on a seeded random
+    volume (DRAM traffic does not depend on the values).  Prints nothing the driver reads."""
+    import torch
+    gen = torch.Generator(device="cuda").manual_seed(rec["seed"])
+    vol = torch.rand(geo.vol_shape, generator=gen, device="cuda") * 0.02
+    b = tg.Ax(vol, geo, ang, rec["ax"])
+    plan = tg.OssartPlan(geo, ang, subsets, rec["ax"], rec["atb"])
+    x = torch.zeros(geo.vol_shape, dtype=torch.float32, device="cuda")
+    plan.iterate(b, x, 1, want_resid=False)
+    torch.cuda.synchronize()
+    plan.close()
+
+
+def kernel_rates_other_configs(tg, rates):
+    """SURVEY.md section 8(d) "per kernel, per config C2-C5": the two projector kernels of C2 (full size) and C4 (full-size volume and
+    detector, 64 of its 1600 views: a launch of the size its CGLS makes per subset-free pass would take 9 s) timed with CUDA events
+    on seeded random data, against the same measured-rate bounds.  C5's rates are `--mode chunked`'s (profiles/)."""
+    import torch
+    out = {}
+    for name, n_views in (("C2", None), ("C4", 64)):
+        geo, ang, rec = make_config(name)
+        if n_views:
+            sel = np.arange(0, len(ang), len(ang) // n_views)[:n_views]
+            ang = ang[sel]
+            if geo.rotDetector_a is not None:
+                geo.rotDetector_a = geo.rotDetector_a[sel]
+        if torch.cuda.mem_get_info()[0] < 4 * (int(np.prod(geo.nVoxel)) * 3 + len(ang) * geo.nDetector[0] * geo.nDetector[1] * 2) + (4 << 30):
+            continue
+        gen = torch.Generator(device="cuda").manual_seed(rec["seed"])
+        vol = torch.rand(geo.vol_shape, generator=gen, device="cuda") * 0.02
+        samples = tg.Ax_count(geo, ang, rec["ax"])
+        updates = int(np.prod(geo.nVoxel)) * len(ang)
+
+        def timed(f, reps=3):
+            f()
+            best = 1e30
+            for _ in range(reps):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                e0.record()
+                r = f()
+                e1.record()
+                torch.cuda.synchronize()
+                best = min(best, e0.elapsed_time(e1))
+            return best, r
+
+        # (tigre_Ax includes the transposed copy of the volume it makes per call: < 1 % of these times)
+        ms_ax, b = timed(lambda: tg.Ax(vol, geo, ang, rec["ax"]))
+        ms_atb, _ = timed(lambda: tg.Atb(b, geo, ang, rec["atb"]))
+        kax = "ax_" + rec["ax"]
+        ax_rate, atb_rate = samples / (ms_ax * 1e-3) / 1e9, updates / (ms_atb * 1e-3) / 1e9
+        out[name] = {"workload": f"{geo.nVoxel[0]}^3, {len(ang)} views of {geo.nDetector[0]}x{geo.nDetector[1]}" + (f" (of {rec['nA']})" if n_views else ""),
+                     kax: {"achieved": ax_rate, "unit": "Gsamples/s", "peak": model_peak(kax, rates), "frac": ax_rate / model_peak(kax, rates),
+                           "ms": ms_ax},
+                     "atb_" + rec["atb"]: {"achieved": atb_rate, "unit": "Gupdates/s", "peak": model_peak("atb", rates),
+                                           "frac": atb_rate / model_peak("atb", rates), "ms": ms_atb}}
+        del vol, b
+        torch.cuda.empty_cache()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -428,10 +565,14 @@ def main():
     ap.add_argument("--tv-delta", type=float, default=0.0, help="tv mode: AwTV delta (0 = plain TV)")
     ap.add_argument("--tv-op", default="minimise", choices=["minimise", "prox"],
                     help="tv mode: the gradient-descent minimiser (tigre_minimize_awtv) or the TV proximal operator of FISTA (tigre_tv_prox)")
-    ap.add_argument("--mode", default="plan", choices=["plan", "chunked", "tv", "drivers", "peaks"],
+    ap.add_argument("--mode", default="plan", choices=["plan", "chunked", "tv", "drivers", "peaks", "probe"],
                     help="plan: OS-SART iteration in HBM (default); chunked: Ax + A^T b with all arrays in pinned host memory (S8)")
     ap.add_argument("--drivers", default="", help="drivers mode: comma-separated subset of the drivers to time (default: all)")
     ap.add_argument("--budget-gb", type=float, default=0.0, help="chunked mode: device bytes the chunked path may use (0 = 3/4 of free)")
+    ap.add_argument("--chunk-n", type=int, default=0, help="chunked mode: C5-shaped problem with an n^3 volume and an n x n detector (0: --config as given)")
+    ap.add_argument("--chunk-views", type=int, default=0, help="chunked mode with --chunk-n: number of views (0: 2400 n / 3072)")
+    ap.add_argument("--no-traffic", action="store_true", help="skip the ncu leg that measures the dominant kernel's DRAM bytes")
+    ap.add_argument("--no-extra", action="store_true", help="skip the per-config kernel rates of C2 and C4")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -487,6 +628,9 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
+    if args.mode == "probe":
+        run_probe(tg, geo, ang, rec, subsets)
+        return
     if args.mode == "peaks":
         run_peaks(tg, rank)
         if world > 1:
@@ -520,6 +664,7 @@ def main():
     samples = tg.Ax_count(geo, ang, rec["ax"])
     updates = int(np.prod(geo.nVoxel)) * nA
     units = samples + updates
+    rates = measure_peaks(tg)          # the machine rates the roofline rests on, measured now (a few hundred ms, untimed)
 
     plan = tg.OssartPlan(geo, ang, subsets, rec["ax"], rec["atb"])
     x = torch.zeros(geo.vol_shape, dtype=torch.float32, device="cuda")
@@ -569,7 +714,7 @@ def main():
         ems = max_over_ranks(ems, "cuda")
         e2e = {"value": whole_job_value(units, ems / K, world), "unit": UNIT, "ms_per_step": ems / K,
                "h2d_bytes_per_step": int(b_h.numel() * 4 + x_h.numel() * 4), "d2h_bytes_per_step": int(x_h.numel() * 4)}
-        del b_h
+        del b_h, x_h
 
     if rank != 0:
         return
@@ -580,29 +725,35 @@ def main():
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
-    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     kind = "ax" if prof["ms"]["ax"] >= prof["ms"]["atb"] else "atb"
     kname = ("ax_" + rec["ax"]) if kind == "ax" else "atb"
+    other = "atb" if kind == "ax" else "ax_" + rec["ax"]
     k_units = samples if kind == "ax" else updates
     k_ms = prof["ms"][kind] / K                       # per full pass over all views
     achieved = k_units / (k_ms * 1e-3) / 1e9
-    peak = model_peak(kname, sm_max)
+    peak = model_peak(kname, rates)
     n_launch = len(subsets)                           # launches of the dominant kernel per step (one per subset)
     hbm_bytes = (vol.numel() + b.numel()) * 4         # compulsory: volume once + projections once
+    traffic, traffic_src = (None, "skipped")
+    if world == 1 and not args.no_traffic and args.scale == 1:
+        del plan, x
+        torch.cuda.empty_cache()
+        traffic, traffic_src = ncu_traffic(rec["name"], "ax_siddon_kernel|ax_interp_kernel" if kind == "ax" else "atb_tma_kernel|atb_gather_kernel")
+    other_ach = (updates if kind == "ax" else samples) / (prof["ms"]["atb" if kind == "ax" else "ax"] / K * 1e-3) / 1e9
     roofline = {"kernel": kname, "bound": "alu", "achieved": achieved, "peak": peak,
                 "unit": "Gsamples/s" if kind == "ax" else "Gupdates/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_PER_LAUNCH.get((rec["name"], kname)) if args.scale == 1 else None,
-                "peak_source": f"model (DESIGN.md section 6): {SM_COUNT} SMs x {LANES_PER_CLK} lanes/clk x {sm_max:.0f} MHz "
-                               f"(MEASURED_PEAKS.json sm_max_mhz) / algorithmic thread-instructions per unit, or the L1 "
-                               f"wavefront bound where lower; HBM is not the bound (see hbm)",
+                "traffic": traffic, "traffic_source": traffic_src,
+                "algorithmic_hbm_bytes_per_launch": hbm_bytes / n_launch if kind == "atb" else (vol.numel() * 4 + b.numel() * 4 / n_launch),
+                "bounds": model_bounds(kname, rates), "peak_source": peak_source(kname, rates, True),
+                "machine_rates": dict(rates, nominal=NOMINAL_PEAKS),
                 "launches_per_step": n_launch, "ms_per_launch": k_ms / n_launch,
                 "units_per_launch": k_units / n_launch,
                 "share_of_step": prof["ms"][kind] / ms, "ms_per_pass": k_ms,
-                "other_kernel": {"kernel": "atb" if kind == "ax" else "ax_" + rec["ax"],
-                                 "achieved": (updates if kind == "ax" else samples) / (prof["ms"]["atb" if kind == "ax" else "ax"] / K * 1e-3) / 1e9,
-                                 "peak": model_peak("atb" if kind == "ax" else "ax_" + rec["ax"], sm_max)},
+                "other_kernel": {"kernel": other, "achieved": other_ach, "peak": model_peak(other, rates),
+                                 "frac": other_ach / model_peak(other, rates), "bounds": model_bounds(other, rates)},
                 "hbm": {"algorithmic_bytes_per_pass": hbm_bytes, "achieved_gbs": hbm_bytes / (k_ms * 1e-3) / 1e9,
-                        "peak_gbs": peaks.get("hbm_gbs"), "note": "compulsory HBM traffic is ~1% of the time: not the bound"}}
+                        "peak_gbs": peaks.get("hbm_gbs"), "peak_source": "MEASURED_PEAKS.json hbm_gbs",
+                        "note": "compulsory HBM traffic is ~1% of the time: not the bound"}}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic", "config": config, "clocks": clocks,
@@ -616,6 +767,10 @@ def main():
     if world == 1 and not args.no_cpu_baseline:
         b_host = b.cpu().numpy()
         line["cpu_baseline"], _ = cpu_baseline(geo, ang, rec, vol_h, b_host, samples, updates)
+    if world == 1 and not args.no_extra and args.scale == 1:
+        del vol, b
+        torch.cuda.empty_cache()
+        line["per_config"] = kernel_rates_other_configs(tg, rates)
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

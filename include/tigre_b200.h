@@ -326,6 +326,11 @@ TIGRE_API int tigre_chunk_stats(uint64_t *h2d_bytes, uint64_t *d2h_bytes, int *n
  * compute the same sums (DESIGN.md O-C); the switch exists for A/B measurement.  2 = the TMA kernel with its
  * staged box deliberately undersized, so that views take its in-kernel gather fallback (test hook). */
 TIGRE_API int tigre_set_atb_path(int path);
+/* which interpolated tigre_Ax kernel runs: 0 (default) = boxes of the volume staged into shared memory by TMA where that is
+ * the faster one (the 32 rays of a warp span less than 27 voxels) and the problem qualifies (nx, ny multiples of 4, 16-byte
+ * aligned volume, the beam of a 32 x 4 pixel tile fits a stage), 1 = always the L1 gather kernel, 2 = the TMA kernel for wide
+ * beams too.  Same samples, same per-ray order of summation; A/B and test hook. */
+TIGRE_API int tigre_set_ax_path(int path);
 /* which TV gradient kernel runs: 0 (default) = four voxels along x per thread whenever nx % 4 == 0, ny > 1, nz > 1 and
  * the arrays are 16-byte aligned, 1 = always the one-voxel-per-thread kernel (any shape).  Same sums; A/B and test hook. */
 TIGRE_API int tigre_set_tv_path(int path);

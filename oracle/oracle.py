@@ -48,6 +48,11 @@ def lib():
     return _lib
 
 
+def set_num_threads(n: int) -> None:
+    """OpenMP threads the C routines use from now on (bench.py's single-thread leg)."""
+    lib().orc_set_num_threads(int(n))
+
+
 def num_threads() -> int:
     return int(lib().orc_num_threads())
 

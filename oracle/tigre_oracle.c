@@ -633,6 +633,14 @@ void orc_voxel_map(const orc_grid *g, const orc_view *views, int ia, int ix, int
     fuv[0] = m.fu;
     fuv[1] = m.fv;
 }
+/* measurement plumbing for bench.py's cpu_baseline (all hardware threads and single thread): no arithmetic */
+void orc_set_num_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
 int orc_num_threads(void) {
     int n = 1;
 #ifdef _OPENMP

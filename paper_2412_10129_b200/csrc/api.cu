@@ -190,9 +190,11 @@ struct Tables {
     Grid g;
     TempBuf ray, vox;
     std::vector<VoxView> hvox;   // host copy of the table in `vox` (sizes the TMA boxes)
+    std::vector<RayView> hray;   // host copy of the table in `ray` (sizes the boxes of the interpolated projector)
     bool clamp = false;
     int build_ray(const int32_t* idx, int n, cudaStream_t st) {
-        std::vector<RayView> h(n);
+        std::vector<RayView>& h = hray;
+        h.resize(n);
         for (int i = 0; i < n; ++i) build_ray_view(g, views[idx ? idx[i] : i], h[i]);
         return upload(ray, h.data(), sizeof(RayView) * n, st);
     }
@@ -219,7 +221,7 @@ static int prep(const tigre_geo* geo, const double* angles, int nA, Tables& t) {
 static int device_ax(const float* vol, Tables& t, const int32_t* idx, int n, int mode, bool unit, float* proj,
                      cudaStream_t st) {
     TG_TRY(t.build_ray(idx, n, st));
-    return launch_ax(vol, t.g, t.ray.as<RayView>(), n, mode, unit, false, proj, nullptr, st);
+    return launch_ax(vol, t.g, t.ray.as<RayView>(), n, mode, unit, false, proj, nullptr, st, nullptr, nullptr, t.hray.data());
 }
 static int device_atb(const float* proj, Tables& t, const int32_t* idx, int n, int mode, bool unit, float* vol,
                       cudaStream_t st) {
@@ -363,7 +365,7 @@ int tigre_Ax_slab(const float* vol_slab, const tigre_geo* geo, const double* ang
     // interpolated: the sample positions are those of the full volume; taps outside the slab count as zero
     TG_TRY(upload(t.ray, hr.data(), sizeof(RayView) * nA, st));
     sub.zs0 = z0, sub.nzs = nzs;
-    return launch_ax(vol_slab, g, t.ray.as<RayView>(), nA, mode, false, true, proj, nullptr, st, &sub);
+    return launch_ax(vol_slab, g, t.ray.as<RayView>(), nA, mode, false, true, proj, nullptr, st, &sub, nullptr, hr.data());
 }
 
 int tigre_Atb_slab(const float* proj, const tigre_geo* geo, const double* angles, int nA, int mode, int z0, int nzs,
@@ -516,6 +518,7 @@ struct tigre_plan {
     std::vector<int32_t> idx, off;
     std::vector<TempBuf> ray, vox;
     std::vector<std::vector<VoxView>> hvox;
+    std::vector<std::vector<RayView>> hray;
     TempBuf W, V, Axb, grad, d_idx, d_acc;
     size_t bytes = 0;
     bool clamp = false;
@@ -559,13 +562,15 @@ int tigre_plan_create_ex(const tigre_geo* geo, const double* angles, int nA, con
     P->ray = std::vector<TempBuf>(nSubsets);
     P->vox = std::vector<TempBuf>(nSubsets);
     P->hvox.resize(nSubsets);
+    P->hray.resize(nSubsets);
     const double epsW = 1e-2 * std::min(g.dx, std::min(g.dy, g.dz));
     std::vector<double> red;
     if (redundancy) TG_TRY(fdk_weights(g, P->t.views, TIGRE_FDK_WANG, red));   // [nA][nu], reading P17 / P28
     for (int s = 0; s < nSubsets; ++s) {
         const int32_t* idx = subset_idx + subset_off[s];
         const int n = subset_off[s + 1] - subset_off[s];
-        std::vector<RayView> hr(n);
+        std::vector<RayView>& hr = P->hray[s];
+        hr.resize(n);
         std::vector<VoxView>& hv = P->hvox[s];
         hv.resize(n);
         for (int i = 0; i < n; ++i) {
@@ -667,7 +672,7 @@ int tigre_plan_ossart(tigre_plan* P, const float* b, float* x, int n_iter, float
             float* Ws = P->W.as<float>() + per * P->off[s];
             float* Vs = P->V.as<float>() + nvox * s;
             float* A = P->Axb.as<float>();
-            TG_TRY(launch_ax(xd, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st, nullptr, xTd));
+            TG_TRY(launch_ax(xd, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st, nullptr, xTd, P->hray[s].data()));
             if (up && it == 0) TG_CUDA(cudaStreamWaitEvent(st, ev[1 + s], 0));   // this subset's projections have arrived
             // r = W_s .* (b_s - A_s x) in place over A; b is gathered through the subset's view list
             TG_TRY(launch_residual(bd, P->d_idx.as<int32_t>() + P->off[s], A, Ws, A, per, n, P->d_acc.as<double>() + it, st));
@@ -724,7 +729,7 @@ int tigre_plan_osem(tigre_plan* P, const float* b, float* x, int n_iter, void* c
         for (int s = 0; s < P->nSubsets; ++s) {
             const int n = P->off[s + 1] - P->off[s];
             float* A = P->Axb.as<float>();
-            TG_TRY(launch_ax(x, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st));
+            TG_TRY(launch_ax(x, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st, nullptr, nullptr, P->hray[s].data()));
             TG_TRY(launch_ratio(b, P->d_idx.as<int32_t>() + P->off[s], A, A, per, n, st));
             TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>(), 0, g.nz, false, 0, g.nv, P->clamp,
                               st, P->hvox[s].data()));
@@ -761,7 +766,7 @@ int tigre_plan_asd_pocs(tigre_plan* P, const float* b, float* x, int n_iter, flo
         for (int s = 0; s < P->nSubsets; ++s) {
             const int n = P->off[s + 1] - P->off[s];
             float* A = P->Axb.as<float>();
-            TG_TRY(launch_ax(x, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st));
+            TG_TRY(launch_ax(x, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st, nullptr, nullptr, P->hray[s].data()));
             TG_TRY(launch_residual(b, P->d_idx.as<int32_t>() + P->off[s], A, P->W.as<float>() + per * P->off[s], A, per, n, nullptr, st));
             TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, G, 0, g.nz, false, 0, g.nv, P->clamp, st,
                               P->hvox[s].data()));
@@ -773,7 +778,7 @@ int tigre_plan_asd_pocs(tigre_plan* P, const float* b, float* x, int n_iter, flo
         for (int s = 0; s < P->nSubsets; ++s) {
             const int n = P->off[s + 1] - P->off[s];
             float* A = P->Axb.as<float>();
-            TG_TRY(launch_ax(x, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st));
+            TG_TRY(launch_ax(x, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st, nullptr, nullptr, P->hray[s].data()));
             TG_TRY(launch_residual(b, P->d_idx.as<int32_t>() + P->off[s], A, nullptr, A, per, n, d + 3, st));
         }
         TG_TRY(launch_diff_stats(x, x0.as<float>(), x0.as<float>(), nvox, d, st));
@@ -839,7 +844,7 @@ int tigre_cgls(const float* b, const tigre_geo* geo, const double* angles, int n
     TG_CUDA(cudaMemcpyAsync(p.p, s.p, sizeof(float) * nvox, cudaMemcpyDeviceToDevice, st));          // p = s
     TG_TRY(launch_dot(s.as<float>(), s.as<float>(), nvox, d + 0, st));                               // gamma
     for (int it = 0; it < n_iter; ++it) {
-        TG_TRY(launch_ax(p.as<float>(), g, rv, nA, ax_mode, false, false, q.as<float>(), nullptr, st));   // q = A p
+        TG_TRY(launch_ax(p.as<float>(), g, rv, nA, ax_mode, false, false, q.as<float>(), nullptr, st, nullptr, nullptr, t.hray.data()));   // q = A p
         TG_TRY(launch_dot(q.as<float>(), q.as<float>(), np, d + 2, st));
         TG_TRY(launch_axpy(x, p.as<float>(), d + 0, d + 2, 1.f, nvox, st));                          // x += alpha p
         TG_TRY(launch_axpy(r.as<float>(), q.as<float>(), d + 0, d + 2, -1.f, np, st));               // r -= alpha q
@@ -880,7 +885,7 @@ int tigre_gradient_descent(const float* b, const tigre_geo* geo, const double* a
     TG_TRY(t.build_ray(nullptr, nA, st));
     if (!exact) TG_TRY(t.build_vox(nullptr, nA, st));
     for (int it = 0; it < n_iter; ++it) {
-        TG_TRY(launch_ax(x, g, t.ray.as<RayView>(), nA, ax_mode, false, false, r.as<float>(), nullptr, st));
+        TG_TRY(launch_ax(x, g, t.ray.as<RayView>(), nA, ax_mode, false, false, r.as<float>(), nullptr, st, nullptr, nullptr, t.hray.data()));
         TG_TRY(launch_residual(b, nullptr, r.as<float>(), nullptr, r.as<float>(), (size_t)g.nu * g.nv, nA, sc.as<double>() + it, st));
         if (exact) TG_TRY(launch_ax_adjoint(r.as<float>(), g, t.ray.as<RayView>(), nA, ax_mode, grad.as<float>(), st));
         else TG_TRY(launch_atb(r.as<float>(), g, t.vox.as<VoxView>(), nA, atb_mode, false, grad.as<float>(), 0, g.nz, false, 0, g.nv, t.clamp, st,
@@ -1129,7 +1134,7 @@ int tigre_fista(const float* b, const tigre_geo* geo, const double* angles, int 
     TG_CUDA(cudaMemcpyAsync(y.p, x, sizeof(float) * nvox, cudaMemcpyDeviceToDevice, st));            // y_0 = x_0
     double tk = 1.0;
     for (int it = 0; it < n_iter; ++it) {
-        TG_TRY(launch_ax(y.as<float>(), g, rv, nA, ax_mode, false, false, r.as<float>(), nullptr, st));
+        TG_TRY(launch_ax(y.as<float>(), g, rv, nA, ax_mode, false, false, r.as<float>(), nullptr, st, nullptr, nullptr, t.hray.data()));
         TG_TRY(launch_residual(b, nullptr, r.as<float>(), nullptr, r.as<float>(), (size_t)g.nu * g.nv, nA, sc.as<double>() + it, st));
         if (exact) TG_TRY(launch_ax_adjoint(r.as<float>(), g, rv, nA, ax_mode, grad.as<float>(), st));
         else TG_TRY(launch_atb(r.as<float>(), g, vv, nA, atb_mode, false, grad.as<float>(), 0, g.nz, false, 0, g.nv, t.clamp, st, t.hvox.data()));

@@ -108,9 +108,12 @@ struct ProfScope {
 struct AxSub {
     int row0, nrows, zs0, nzs;
 };
+//   h_views: host copy of the same table; when given (and the problem qualifies) the interpolated mode runs the kernel of
+//   ax_tma.cu (boxes of the volume staged into shared memory by TMA), otherwise the L1 gather kernel of ax.cu
 int launch_ax(const float* vol, const Grid& g, const RayView* d_views, int nViews, int mode, bool unit_vol,
               bool accumulate, float* proj, uint32_t* count_out, cudaStream_t st, const AxSub* sub = nullptr,
-              const float* volT_in = nullptr);   // volT_in: an up-to-date (x,y)-transposed copy of vol, if the caller has one
+              const float* volT_in = nullptr,    // volT_in: an up-to-date (x,y)-transposed copy of vol, if the caller has one
+              const RayView* h_views = nullptr);
 int launch_transpose_xy(const float* vol, float* volT, const Grid& g, cudaStream_t st);
 // Siddon march without the volume: counts[ray] = voxels met with a non-zero length, track[2 ray], [2 ray + 1] = first / last of them
 int launch_ax_track(const Grid& g, const RayView* d_views, int nViews, uint32_t* counts, long long* track, cudaStream_t st);

@@ -15,6 +15,7 @@
 #include <cmath>
 #include <mutex>
 #include "common.cuh"
+#include "tma.cuh"
 
 namespace tg {
 
@@ -180,35 +181,6 @@ __device__ __forceinline__ void tv_voxel(float dx, float dy, float dz, float thr
 
 __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0;" ::: "memory"); }   // same barrier from two code paths
 __device__ __forceinline__ float4 ld4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n"
-            ".reg .pred p;\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-            "selp.u32 %0, 1, 0, p;\n"
-            "}\n"
-            : "=r"(ok)
-            : "r"(smem_u32(bar)), "r"(parity)
-            : "memory");
-    } while (!ok);
-}
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
-            smem_u32(dst)),
-        "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
-        : "memory");
-}
-
 static_assert((TM_BY + 1) % 4 == 0, "a staged plane must be a multiple of 128 bytes (TMA destination alignment)");
 constexpr size_t TM_SMEM = (size_t)TM_D * TM_PLANE * 4 + 2 * TM_BY * 32 * 16 + 64 * 4 + TM_D * 8;
 
@@ -391,22 +363,8 @@ __global__ void __launch_bounds__(256) tv_step_kernel(float* __restrict__ x, con
 }  // namespace
 
 namespace {
-typedef CUresult (*TvEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-TvEncodeFn tv_encode_fn() {
-    static TvEncodeFn fn = nullptr;
-    static std::once_flag once;
-    std::call_once(once, [] {
-        void* f = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = (TvEncodeFn)f;
-        (void)cudaGetLastError();
-    });
-    return fn;
-}
+typedef TensorMapEncodeTiledFn TvEncodeFn;
+inline TvEncodeFn tv_encode_fn() { return tensor_map_encoder(); }
 }  // namespace
 
 bool g_tv_scalar = false;   // test hook (tigre_set_tv_path): force the one-voxel-per-thread kernel

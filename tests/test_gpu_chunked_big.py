@@ -4,7 +4,8 @@ host memory, through tigre_Ax and one tigre_sirt_chunked iteration, with the ora
 voxels as configs[4] prescribes.  Full C5 (207 GB) does not fit the box's host RAM, so the volume and detector keep C5's
 full size (3072^3 voxels, 3072^2 pixels) and the views are thinned to the fewest that still exceed the budget
 (on a 183 GB B200: 147 GB of budget, 1024 views: 116 + 39 GB of pinned host arrays).
-Slabs of 768 x 3072^2 = 7.2e9 voxels take the 64-bit element-index kernels.  Size-gated by free host RAM; smaller boxes
+The library cuts the volume into slabs below 2^31 voxels (227 slices of 3072^2) so that the ray-driven kernels keep their
+32-bit element offsets (the 64-bit instantiations are covered by tests/test_gpu_index.py, incl. a real 2.4e9-voxel volume).  Size-gated by free host RAM; smaller boxes
 skip."""
 import os
 
@@ -72,7 +73,7 @@ def test_c5_shaped_run_beyond_the_default_budget():
     h2d, d2h, n_slabs, n_batches = tg.chunk_stats()
     log(f"tigre_Ax done: {n_slabs} z-slabs x {n_batches} view batches, H2D {h2d / 1e9:.1f} GB, D2H {d2h / 1e9:.1f} GB")
     assert n_slabs >= 2 and n_batches >= 2 and h2d >= n_batches * 4 * n ** 3          # the volume went up once per batch
-    assert (n // n_slabs) * n * n >= 2 ** 31                                          # slabs beyond 32-bit element offsets
+    assert -(-n // n_slabs) * n * n < 2 ** 31                                         # slabs sized for 32-bit element offsets
     ax_true = orc.ax(xn, geo, ang, orc.SIDDON, ray_ids=rays)
     assert H.rel_l2(bn.ravel()[rays].astype(np.float64), ax_true) <= 1e-5
     assert np.count_nonzero(ax_true) > 3000
