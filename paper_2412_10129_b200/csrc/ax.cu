@@ -69,9 +69,9 @@ __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base,
     } else if (SCATTER) {
         // exact adjoint: the same three lengths, added to the voxels instead of gathered from them
         float* out = const_cast<float*>(base);
-        atomicAdd(out + r.off, s1 * r.ys);
-        if (both) atomicAdd(out + (r.off + ((se < sf) ? r.stE : r.stF)), (s2 - s1) * r.ys);
-        atomicAdd(out + offC, (1.0f - s2) * r.ys);
+        red_add_global(out + r.off, s1 * r.ys);
+        if (both) red_add_global(out + (r.off + ((se < sf) ? r.stE : r.stF)), (s2 - s1) * r.ys);
+        red_add_global(out + offC, (1.0f - s2) * r.ys);
     } else {
         const float vA = UNIT ? 1.f : __ldg(base + r.off);
         float vC = vA;   // a lane that stays in its voxel does not load it twice
@@ -100,8 +100,8 @@ __device__ __forceinline__ void siddon_slab_e_only(const float* __restrict__ bas
         r.note(offC, 1.0f - se);
     } else if (SCATTER) {
         float* out = const_cast<float*>(base);
-        atomicAdd(out + r.off, se * r.ys);
-        atomicAdd(out + offC, (1.0f - se) * r.ys);
+        red_add_global(out + r.off, se * r.ys);
+        red_add_global(out + offC, (1.0f - se) * r.ys);
     } else {
         const float vA = UNIT ? 1.f : __ldg(base + r.off);
         float vC = vA;   // a lane that stays in its voxel does not load it twice (the L1 data pipe is co-critical)
@@ -139,9 +139,9 @@ __device__ __forceinline__ void siddon_slab_checked(const float* __restrict__ ba
         if (vEC && vFC) r.note(offC, lenE);
     } else if (SCATTER) {
         float* out = const_cast<float*>(base);
-        if (lenA > 0.f && vEA && vFA) atomicAdd(out + r.off, lenA * r.ys);
-        if (cE && cF && lenB > 0.f && vB) atomicAdd(out + offB, lenB * r.ys);
-        if (lenE > 0.f && vEC && vFC) atomicAdd(out + offC, lenE * r.ys);
+        if (lenA > 0.f && vEA && vFA) red_add_global(out + r.off, lenA * r.ys);
+        if (cE && cF && lenB > 0.f && vB) red_add_global(out + offB, lenB * r.ys);
+        if (lenE > 0.f && vEC && vFC) red_add_global(out + offC, lenE * r.ys);
     } else {
         if (lenA > 0.f && vEA && vFA) r.acc = fmaf(lenA, UNIT ? 1.f : __ldg(base + r.off), r.acc);
         if (cE && cF && lenB > 0.f && vB) r.acc = fmaf(lenB, UNIT ? 1.f : __ldg(base + offB), r.acc);
@@ -411,7 +411,7 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
                 if ((unsigned)jx < (unsigned)nX && (unsigned)jy < (unsigned)nY && (unsigned)(jz - p.zs0) < (unsigned)(p.zs1 - p.zs0)) {
                     const float w = ((c & 1) ? ax : 1.f - ax) * ((c & 2) ? ay : 1.f - ay) * ((c & 4) ? az : 1.f - az);
                     const IdxT at = (IdxT)(jz - p.zs0) * pitchZ + (IdxT)jy * pitchY + jx;
-                    if (SCATTER) atomicAdd(const_cast<float*>(base) + at, w * ys);   // exact adjoint: same weight, added
+                    if (SCATTER) red_add_global(const_cast<float*>(base) + at, w * ys);   // exact adjoint: same weight, added
                     else v = fmaf(w, __ldg(base + at), v);
                 }
             }
@@ -459,10 +459,10 @@ ax_interp_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
         float* q = const_cast<float*>(org) + ((IdxT)iz * pitchZ + (IdxT)iy * pitchY + (IdxT)ix);
         const float w0 = (1.f - az) * ys, w1 = az * ys;
         const float w00 = (1.f - ay) * w0, w10 = ay * w0, w01 = (1.f - ay) * w1, w11 = ay * w1;
-        atomicAdd(q, (1.f - ax) * w00), atomicAdd(q + 1, ax * w00);
-        atomicAdd(q + pitchY, (1.f - ax) * w10), atomicAdd(q + pitchY + 1, ax * w10);
-        atomicAdd(q + pitchZ, (1.f - ax) * w01), atomicAdd(q + pitchZ + 1, ax * w01);
-        atomicAdd(q + pitchZ + pitchY, (1.f - ax) * w11), atomicAdd(q + pitchZ + pitchY + 1, ax * w11);
+        red_add_global(q, (1.f - ax) * w00), red_add_global(q + 1, ax * w00);
+        red_add_global(q + pitchY, (1.f - ax) * w10), red_add_global(q + pitchY + 1, ax * w10);
+        red_add_global(q + pitchZ, (1.f - ax) * w01), red_add_global(q + pitchZ + 1, ax * w01);
+        red_add_global(q + pitchZ + pitchY, (1.f - ax) * w11), red_add_global(q + pitchZ + pitchY + 1, ax * w11);
     };
     // bounds-checked sample without branches (gather only): every tap index is tested once per axis; an outside tap gets
     // weight zero and a clamped (valid) address

@@ -43,6 +43,13 @@ struct AxP {
 constexpr int AX_TU = 32, AX_TV = AXTV;
 constexpr int AXI_ROWS = 8;
 
+// a[i] += v without a return value, on GLOBAL memory, said so explicitly: through a generic pointer (the scatter kernels pick
+// vol or volT at run time) atomicAdd compiles to a generic ATOM with a shared-memory CAS fall-back path behind a branch
+// (ncu: 24 long-scoreboard stall cycles per issue, issue slots 29 % busy on C3) instead of one RED.E.ADD.F32
+__device__ __forceinline__ void red_add_global(float* a, float v) {
+    asm volatile("red.global.add.f32 [%0], %1;" ::"l"(__cvta_generic_to_global(a)), "f"(v) : "memory");
+}
+
 __device__ __forceinline__ double sel3(int k, double a, double b, double c) { return k == 0 ? a : (k == 1 ? b : c); }
 
 // tile order: u-tile fastest, then view, then v-band slowest: all views of one detector-row band
