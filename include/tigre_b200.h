@@ -171,7 +171,13 @@ TIGRE_API int tigre_plan_create_ex(const tigre_geo *geo, const double *angles, i
 TIGRE_API int tigre_plan_ossart(tigre_plan *plan, const float *b, float *x_inout, int n_iter, float lambda,
                       int nonneg, double *resid_hist, void *cuda_stream);
 TIGRE_API int tigre_plan_destroy(tigre_plan *plan);
+/* device bytes the plan holds.  The column weights V_s take one volume PER SUBSET while all of them fit half of the free device
+ * memory (or of the workspace) at creation; otherwise (single-view subsets on large volumes: SART on 512^3 would need 386 GB)
+ * the plan keeps ONE volume and every subset step recomputes its V_s first (one more backprojection per subset).
+ * tigre_set_plan_v_path: 0 = that rule (default), 1 = always stored, 2 = always recomputed (test hook; applies to plans
+ * created afterwards). */
 TIGRE_API size_t tigre_plan_bytes(const tigre_plan *plan);
+TIGRE_API int tigre_set_plan_v_path(int path);
 /* SIRT on arrays larger than the device (BASELINE.json configs[4] "single-GPU z-slab/angle-batch host chunking ... one SIRT
  * iteration"; eq. 6 with one subset of all views): b, x_inout and r_scratch are PINNED HOST
  * arrays (b, r_scratch [nA][nv][nu]; x_inout [nz][ny][nx], start in, result out).  Per iteration two streamed passes:

@@ -503,6 +503,14 @@ int tigre_microbench(int kind, double* value, void* cuda_stream) {
     return microbench(kind, value, (cudaStream_t)cuda_stream);
 }
 
+// test hook (tigre_set_plan_v_path): 0 = store V_s per subset when they fit (default), 1 = always store, 2 = always recompute
+static int g_plan_v_path = 0;
+int tigre_set_plan_v_path(int path) {
+    if (path < 0 || path > 2) return TIGRE_ERR_ARG;
+    g_plan_v_path = path;
+    return TIGRE_OK;
+}
+
 int tigre_set_index_path(int path) {
     if (path != 0 && path != 1) return TIGRE_ERR_ARG;
     set_index_path(path);
@@ -522,6 +530,26 @@ struct tigre_plan {
     TempBuf W, V, Axb, grad, d_idx, d_acc;
     size_t bytes = 0;
     bool clamp = false;
+    // Column weights: one volume per subset while nSubsets volumes fit the plan's share of the device (C3: 20 x 537 MB), else
+    // ONE volume that every subset step refills (A_s^T 1 through the same TMA kernel, from a buffer of ones: one more
+    // backprojection per subset).  Single-view subsets (SART, ASD-POCS, SART-TV) of a 512^3 problem would need 386 GB stored.
+    bool v_stored = true;
+    // V_s of subset s, ready to use on the stream (stored: a pointer; otherwise computed now into the one volume)
+    int col_weights(int s, float** out, cudaStream_t st) {
+        const Grid& g = t.g;
+        const size_t nvox = (size_t)g.nx * g.ny * g.nz, per = (size_t)g.nu * g.nv;
+        if (v_stored) {
+            *out = V.as<float>() + nvox * s;
+            return TIGRE_OK;
+        }
+        const int n = off[s + 1] - off[s];
+        float* ones = Axb.as<float>();   // free between two subset steps
+        TG_TRY(launch_fill(ones, 1.0f, per * n, st));
+        TG_TRY(launch_atb(ones, g, vox[s].as<VoxView>(), n, atb_mode, false, V.as<float>(), 0, g.nz, false, 0, g.nv, clamp, st, hvox[s].data()));
+        TG_TRY(launch_invert_cols(V.as<float>(), nvox, 1e-6f, st));
+        *out = V.as<float>();
+        return TIGRE_OK;
+    }
 };
 
 int tigre_plan_create(const tigre_geo* geo, const double* angles, int nA, const int32_t* subset_idx,
@@ -554,11 +582,20 @@ int tigre_plan_create_ex(const tigre_geo* geo, const double* angles, int nA, con
     const Grid& g = P->t.g;
     const size_t per = (size_t)g.nu * g.nv, nvox = (size_t)g.nx * g.ny * g.nz;
     TG_TRY(P->W.alloc(sizeof(float) * per * nIdx, st));
-    TG_TRY(P->V.alloc(sizeof(float) * nvox * nSubsets, st));
+    {
+        // store V_s per subset if that takes at most half of what is free now (or of the caller's workspace)
+        size_t fr = 0, tot = 0;
+        if (workspace_active()) fr = workspace_free_bytes();
+        else if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) fr = 0, (void)cudaGetLastError();
+        P->v_stored = nSubsets == 1 || sizeof(float) * nvox * (size_t)nSubsets <= fr / 2;
+        if (g_plan_v_path == 1) P->v_stored = true;
+        if (g_plan_v_path == 2) P->v_stored = false;
+    }
+    TG_TRY(P->V.alloc(sizeof(float) * nvox * (P->v_stored ? nSubsets : 1), st));
     TG_TRY(P->Axb.alloc(sizeof(float) * per * P->maxs, st));
     TG_TRY(P->grad.alloc(sizeof(float) * nvox, st));
     TG_TRY(upload(P->d_idx, subset_idx, sizeof(int32_t) * nIdx, st));
-    P->bytes = sizeof(float) * (per * nIdx + nvox * nSubsets + per * P->maxs + nvox);
+    P->bytes = sizeof(float) * (per * nIdx + nvox * (P->v_stored ? nSubsets : 1) + per * P->maxs + nvox);
     P->ray = std::vector<TempBuf>(nSubsets);
     P->vox = std::vector<TempBuf>(nSubsets);
     P->hvox.resize(nSubsets);
@@ -581,7 +618,6 @@ int tigre_plan_create_ex(const tigre_geo* geo, const double* angles, int nA, con
         P->clamp = P->clamp || vox_needs_clamp(g, hv.data(), n);
         TG_TRY(upload(P->vox[s], hv.data(), sizeof(VoxView) * n, st));
         float* Ws = P->W.as<float>() + per * subset_off[s];
-        float* Vs = P->V.as<float>() + nvox * s;
         TG_TRY(launch_ax(nullptr, g, P->ray[s].as<RayView>(), n, ax_mode, true, false, Ws, nullptr, st));
         TG_TRY(launch_invert_rows(Ws, per * n, (float)epsW, st));
         if (redundancy) {
@@ -592,8 +628,15 @@ int tigre_plan_create_ex(const tigre_geo* geo, const double* angles, int nA, con
             TG_TRY(upload(tc, cw.data(), sizeof(float) * cw.size(), st));
             TG_TRY(launch_scale_columns(Ws, tc.as<float>(), n, g.nv, g.nu, st));
         }
-        TG_TRY(launch_atb(nullptr, g, P->vox[s].as<VoxView>(), n, atb_mode, true, Vs, 0, g.nz, false, 0, g.nv, P->clamp, st));
-        TG_TRY(launch_invert_cols(Vs, nvox, 1e-6f, st));
+        if (P->v_stored) {
+            // A_s^T 1 as the backprojection of a buffer of ones through the TMA kernel (4 ms per C3 subset; the gather kernel's
+            // unit-projection variant, which it replaces here, took 6)
+            float* Vs = P->V.as<float>() + nvox * s;
+            TG_TRY(launch_fill(P->Axb.as<float>(), 1.0f, per * n, st));
+            TG_TRY(launch_atb(P->Axb.as<float>(), g, P->vox[s].as<VoxView>(), n, atb_mode, false, Vs, 0, g.nz, false, 0, g.nv, P->clamp, st,
+                              hv.data()));
+            TG_TRY(launch_invert_cols(Vs, nvox, 1e-6f, st));
+        }
     }
     *out = P.release();
     return TIGRE_OK;
@@ -670,8 +713,9 @@ int tigre_plan_ossart(tigre_plan* P, const float* b, float* x, int n_iter, float
         for (int s = 0; s < P->nSubsets; ++s) {
             const int n = P->off[s + 1] - P->off[s];
             float* Ws = P->W.as<float>() + per * P->off[s];
-            float* Vs = P->V.as<float>() + nvox * s;
+            float* Vs = nullptr;
             float* A = P->Axb.as<float>();
+            TG_TRY(P->col_weights(s, &Vs, st));   // (when V_s is not stored this uses A as scratch: before this subset's projection)
             TG_TRY(launch_ax(xd, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st, nullptr, xTd, P->hray[s].data()));
             if (up && it == 0) TG_CUDA(cudaStreamWaitEvent(st, ev[1 + s], 0));   // this subset's projections have arrived
             // r = W_s .* (b_s - A_s x) in place over A; b is gathered through the subset's view list
@@ -729,11 +773,13 @@ int tigre_plan_osem(tigre_plan* P, const float* b, float* x, int n_iter, void* c
         for (int s = 0; s < P->nSubsets; ++s) {
             const int n = P->off[s + 1] - P->off[s];
             float* A = P->Axb.as<float>();
+            float* Vs = nullptr;
+            TG_TRY(P->col_weights(s, &Vs, st));
             TG_TRY(launch_ax(x, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st, nullptr, nullptr, P->hray[s].data()));
             TG_TRY(launch_ratio(b, P->d_idx.as<int32_t>() + P->off[s], A, A, per, n, st));
             TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>(), 0, g.nz, false, 0, g.nv, P->clamp,
                               st, P->hvox[s].data()));
-            TG_TRY(launch_mul_update(x, P->grad.as<float>(), P->V.as<float>() + nvox * s, nvox, st));
+            TG_TRY(launch_mul_update(x, P->grad.as<float>(), Vs, nvox, st));
         }
     }
     return TIGRE_OK;
@@ -766,11 +812,13 @@ int tigre_plan_asd_pocs(tigre_plan* P, const float* b, float* x, int n_iter, flo
         for (int s = 0; s < P->nSubsets; ++s) {
             const int n = P->off[s + 1] - P->off[s];
             float* A = P->Axb.as<float>();
+            float* Vs = nullptr;
+            TG_TRY(P->col_weights(s, &Vs, st));
             TG_TRY(launch_ax(x, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st, nullptr, nullptr, P->hray[s].data()));
             TG_TRY(launch_residual(b, P->d_idx.as<int32_t>() + P->off[s], A, P->W.as<float>() + per * P->off[s], A, per, n, nullptr, st));
             TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, G, 0, g.nz, false, 0, g.nv, P->clamp, st,
                               P->hvox[s].data()));
-            TG_TRY(launch_update(x, G, P->V.as<float>() + nvox * s, beta, 1, nvox, st));
+            TG_TRY(launch_update(x, G, Vs, beta, 1, nvox, st));
         }
         beta *= beta_red;
         // ---- dd = ||A x - b||, dp = ||x - x0||

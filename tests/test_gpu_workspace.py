@@ -99,3 +99,33 @@ def test_chunked_path_sizes_itself_to_the_workspace(tg):
         tg.set_workspace(None)
     ref = orc.ax(vol, geo, ang, orc.SIDDON)
     assert np.linalg.norm(p.numpy().astype(np.float64) - ref) <= 1e-5 * np.linalg.norm(ref)
+
+
+def test_plan_recomputes_column_weights_when_they_do_not_fit(tg):
+    """Single-view subsets (SART, the data step of ASD-POCS / SART-TV): the plan keeps one volume of column weights and refills it
+    per subset step instead of nSubsets volumes; same kernels, same numbers as the stored variant, and the oracle's SART."""
+    from oracle import oracle as orc
+    geo, ang, rec = make_config("C3", scale=16, n_angles=24)
+    vol = phantom_for(rec, geo)
+    b = tg.Ax(torch.from_numpy(vol).cuda(), geo, ang, "siddon")
+    subsets = [np.array([a]) for a in range(len(ang))]
+    out = {}
+    for path in (1, 2):
+        tg.set_plan_v_path(path)
+        try:
+            plan = tg.OssartPlan(geo, ang, subsets)
+            out[path] = (plan.nbytes, torch.zeros_like(b[0, :1, :1]))
+            x = torch.zeros(tg.vol_shape(geo), dtype=torch.float32, device="cuda")
+            plan.iterate(b, x, 2, lam=0.5)
+            xo = torch.ones_like(x)
+            plan.osem(b, xo, 1)
+            out[path] = (plan.nbytes, x, xo)
+            plan.close()
+        finally:
+            tg.set_plan_v_path(0)
+    nvox = int(np.prod(geo.nVoxel))
+    assert out[1][0] - out[2][0] == 4 * nvox * (len(subsets) - 1)
+    assert torch.equal(out[1][1], out[2][1]) and torch.equal(out[1][2], out[2][2])
+    xr, _ = orc.ossart(b.cpu().numpy(), geo, ang, subsets, 2, lam=0.5)
+    got = out[2][1].cpu().numpy().astype(np.float64)
+    assert np.linalg.norm(got - xr) <= 3e-5 * np.linalg.norm(xr)
