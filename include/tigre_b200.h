@@ -170,6 +170,11 @@ TIGRE_API int tigre_plan_create_ex(const tigre_geo *geo, const double *angles, i
                          void *cuda_stream, tigre_plan **plan_out);
 TIGRE_API int tigre_plan_ossart(tigre_plan *plan, const float *b, float *x_inout, int n_iter, float lambda,
                       int nonneg, double *resid_hist, void *cuda_stream);
+/* The subset steps [s_begin, s_end) of ONE sweep of tigre_plan_ossart, in order, with the plan's own W_s, V_s and view lists
+ * (what a caller needs to interleave other work between subsets, and what the tests use to check a single ordered-subset
+ * update of the very plan a long run advances).  b, x_inout dev, or both pinned host.  Asynchronous for device data. */
+TIGRE_API int tigre_plan_ossart_subsets(tigre_plan *plan, const float *b, float *x_inout, int s_begin, int s_end, float lambda,
+                              int nonneg, void *cuda_stream);
 TIGRE_API int tigre_plan_destroy(tigre_plan *plan);
 /* device bytes the plan holds.  The column weights V_s take one volume PER SUBSET while all of them fit half of the free device
  * memory (or of the workspace) at creation; otherwise (single-view subsets on large volumes: SART on 512^3 would need 386 GB)

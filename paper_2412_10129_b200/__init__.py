@@ -53,7 +53,7 @@ EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_Ax_slab", "tigre_Atb_slab", "tigre_sl
            "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_create_ex", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_osem", "tigre_plan_sart_tv", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version", "tigre_Ax_index", "tigre_set_index_path", "tigre_set_workspace", "tigre_plan_workspace_bytes",
-           "tigre_workspace_stats", "tigre_sirt_chunked", "tigre_microbench", "tigre_set_ax_path", "tigre_set_plan_v_path"]
+           "tigre_workspace_stats", "tigre_sirt_chunked", "tigre_microbench", "tigre_set_ax_path", "tigre_set_plan_v_path", "tigre_plan_ossart_subsets"]
 
 
 def _lib():
@@ -330,6 +330,13 @@ class OssartPlan:
                                         int(bool(nonneg)), hist.ctypes.data_as(_dp) if want_resid else None,
                                         _stream(b)), "tigre_plan_ossart")
         return hist[:n_iter]
+
+    def iterate_subsets(self, b, x, s_begin, s_end, lam=1.0, nonneg=True):
+        """The subset steps [s_begin, s_end) of one sweep, in place on x."""
+        _check(_lib().tigre_plan_ossart_subsets(self._h, _f32(b, proj_shape(self.geo, self.nA), "b"), _f32(x, vol_shape(self.geo), "x"),
+                                                int(s_begin), int(s_end), C.c_float(lam), int(bool(nonneg)), _stream(b)),
+               "tigre_plan_ossart_subsets")
+        return x
 
     def asd_pocs(self, b, x, n_iter, beta=1.0, beta_red=0.99, ng=20, alpha=0.002, alpha_red=0.95, r_max=0.95,
                  epsilon=0.0, delta=None, tv_eps=1e-8):

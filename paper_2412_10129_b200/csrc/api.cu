@@ -649,8 +649,24 @@ int tigre_plan_destroy(tigre_plan* plan) {
 
 size_t tigre_plan_bytes(const tigre_plan* plan) { return plan ? plan->bytes : 0; }
 
+static int plan_ossart_impl(tigre_plan* P, const float* b, float* x, int n_iter, float lambda, int nonneg, double* resid_hist,
+                            void* cuda_stream, int s_begin, int s_end);
+
 int tigre_plan_ossart(tigre_plan* P, const float* b, float* x, int n_iter, float lambda, int nonneg,
                       double* resid_hist, void* cuda_stream) {
+    if (!P) return TIGRE_ERR_ARG;
+    return plan_ossart_impl(P, b, x, n_iter, lambda, nonneg, resid_hist, cuda_stream, 0, P->nSubsets);
+}
+
+int tigre_plan_ossart_subsets(tigre_plan* P, const float* b, float* x, int s_begin, int s_end, float lambda, int nonneg,
+                              void* cuda_stream) {
+    if (!P || s_begin < 0 || s_end > P->nSubsets || s_begin > s_end) return TIGRE_ERR_ARG;
+    if (s_begin == s_end) return TIGRE_OK;
+    return plan_ossart_impl(P, b, x, 1, lambda, nonneg, nullptr, cuda_stream, s_begin, s_end);
+}
+
+static int plan_ossart_impl(tigre_plan* P, const float* b, float* x, int n_iter, float lambda, int nonneg, double* resid_hist,
+                            void* cuda_stream, int s_begin, int s_end) {
     if (!P || !b || !x || n_iter < 0) return TIGRE_ERR_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const Grid& g = P->t.g;
@@ -688,7 +704,7 @@ int tigre_plan_ossart(tigre_plan* P, const float* b, float* x, int n_iter, float
             ev.push_back(start);
             TG_CUDA(cudaEventRecord(start, st));               // the buffer exists from here on in stream order
             TG_CUDA(cudaStreamWaitEvent(up, start, 0));
-            for (int s = 0; s < P->nSubsets; ++s) {
+            for (int s = s_begin; s < s_end; ++s) {
                 for (int k = P->off[s]; k < P->off[s + 1]; ++k) {
                     const size_t o = per * (size_t)P->idx[k];
                     TG_CUDA(cudaMemcpyAsync(db.as<float>() + o, b + o, sizeof(float) * per, cudaMemcpyHostToDevice, up));
@@ -710,14 +726,14 @@ int tigre_plan_ossart(tigre_plan* P, const float* b, float* x, int n_iter, float
         launch_transpose_xy(xd, xT.as<float>(), g, st) == TIGRE_OK)
         xTd = xT.as<float>();
     for (int it = 0; it < n_iter; ++it) {
-        for (int s = 0; s < P->nSubsets; ++s) {
+        for (int s = s_begin; s < s_end; ++s) {
             const int n = P->off[s + 1] - P->off[s];
             float* Ws = P->W.as<float>() + per * P->off[s];
             float* Vs = nullptr;
             float* A = P->Axb.as<float>();
             TG_TRY(P->col_weights(s, &Vs, st));   // (when V_s is not stored this uses A as scratch: before this subset's projection)
             TG_TRY(launch_ax(xd, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st, nullptr, xTd, P->hray[s].data()));
-            if (up && it == 0) TG_CUDA(cudaStreamWaitEvent(st, ev[1 + s], 0));   // this subset's projections have arrived
+            if (up && it == 0) TG_CUDA(cudaStreamWaitEvent(st, ev[1 + s - s_begin], 0));   // this subset's projections have arrived
             // r = W_s .* (b_s - A_s x) in place over A; b is gathered through the subset's view list
             TG_TRY(launch_residual(bd, P->d_idx.as<int32_t>() + P->off[s], A, Ws, A, per, n, P->d_acc.as<double>() + it, st));
             TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>(), 0, g.nz, false, 0, g.nv, P->clamp, st,

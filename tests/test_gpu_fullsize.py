@@ -10,7 +10,7 @@ import pytest
 
 from oracle import oracle as orc
 from tests import helpers as H
-from workloads import make_config
+from workloads import make_config, phantom_for
 
 pytestmark = pytest.mark.gpu
 
@@ -126,68 +126,69 @@ def test_c4_full_size_tilted_detectors(tg):
 
 
 def test_c3_full_size_ossart_teacher_forced(tg):
-    """north_star's target run, 20 iterations x 20 ordered subsets of OS-SART on the full C3 problem through the plan path
-    that bench.py times, checked against the oracle by teacher forcing: at iterations 1, 10 and 20 the
-    GPU's iterate is handed to the oracle, which applies ONE ordered-subset update of reading P13 / PAPER.md:115 to sampled
-    voxels, x_j <- max(0, x_j + V_j (A_s^T W (b_s - A_s x))_j); the GPU applies the same update through a one-subset plan of
-    those 36 views (the bench's launch configuration).  The oracle evaluates A_s x and A_s 1 only at the detector pixels the
-    sampled voxels' bilinear taps touch (their indices come from the oracle's own voxel map), so the step costs seconds.
-    b is seeded uniform noise: an inconsistent system, the residual never gets small, no cancellation for errors to hide in."""
+    """north_star's target run, 20 iterations x 20 ordered subsets of OS-SART on the full C3 problem (its phantom, Poisson noise on
+    I0 = 1e5, half-fan detector) through the plan bench.py times, checked against the oracle by teacher forcing (SURVEY.md section
+    8(d)): before subset 0 of iteration 1, subset 7 of iteration 10 and subset 19 of iteration 20 the GPU's iterate is handed to
+    the oracle, which applies ONE ordered-subset update of reading P13 / PAPER.md:115 to 20 000 sampled voxels,
+    x_j <- max(0, x_j + V_j (A_s^T W (b_s - A_s x))_j); the GPU takes the same step through THE 20-SUBSET PLAN ITSELF
+    (tigre_plan_ossart_subsets: its own W_s, V_s, view lists and offsets).  The oracle evaluates A_s x and A_s 1 only at the
+    detector pixels the sampled voxels' bilinear taps touch (their indices come from the oracle's own voxel map)."""
     geo, ang, rec = make_config("C3")
     nA, (nu, nv) = len(ang), geo.nDetector
     subsets = [np.arange(s, nA, 20) for s in range(20)]
-    b_d, b_h = random_projections(geo, nA, 401)
-    s0 = subsets[0]
-    geo_s, ang_s, _ = subset_geometry("C3", s0)
-    nS = len(s0)
-    b_s_d = b_d[torch.from_numpy(s0).cuda()].contiguous()
-    b_s_h = b_h[s0].astype(np.float64)
-    del b_h
-    # oracle quantities that do not depend on the iterate: taps, A 1 at the tap pixels, A^T 1 at the voxels
-    n_vox = 4000
+    vol_h = phantom_for(rec, geo)
+    b_d = tg.Ax(torch.from_numpy(vol_h).cuda(), geo, ang, "siddon")
+    gen = torch.Generator(device="cuda").manual_seed(rec["seed"])
+    b_d = -torch.log(torch.clamp(torch.poisson(1e5 * torch.exp(-b_d), generator=gen), min=1.0) / 1e5)    # reading P18, drawn once
+    b_h = b_d.cpu().numpy()
+    del vol_h
+    n_vox = 20000
     ids = np.random.default_rng(402).integers(0, int(np.prod(geo.vol_shape)), n_vox)
-    at1, fuv = orc.atb(None, geo_s, ang_s, orc.MATCHED, vox_ids=ids, return_fuv=True)
-    iu0, iv0 = np.floor(fuv[..., 0]).astype(np.int64), np.floor(fuv[..., 1]).astype(np.int64)     # [n_vox][nS]
-    ia = np.broadcast_to(np.arange(nS)[None, :], iu0.shape)
-    rays = []
-    for du in (0, 1):
-        for dv in (0, 1):
-            u, v = iu0 + du, iv0 + dv
-            ok = (u >= 0) & (u < nu) & (v >= 0) & (v < nv)
-            rays.append(((ia * nv + v) * nu + u)[ok])
-    rid = np.unique(np.concatenate(rays))
-    a1 = orc.ax(np.ones(geo.vol_shape, np.float32), geo_s, ang_s, orc.SIDDON, ray_ids=rid)
+    ids_d = torch.from_numpy(ids).cuda()
     eps_w = 1e-2 * min(geo.dVoxel)
-    W = np.where(a1 > eps_w, 1.0 / np.maximum(a1, 1e-300), 0.0)
-    seen = at1 > 1e-4 * at1.max()              # V's own threshold is 1e-6 max_j (A^T 1)_j over the volume: stay clear of it
-    assert np.count_nonzero(seen) > n_vox // 2
-    V = np.where(seen, 1.0 / np.maximum(at1, 1e-300), 0.0)
+    ones = np.ones(geo.vol_shape, np.float32)
 
     plan = tg.OssartPlan(geo, ang, subsets, "siddon", "matched")
-    plan_s = tg.OssartPlan(geo_s, ang_s, [np.arange(nS)], "siddon", "matched")
     x = torch.zeros(geo.vol_shape, dtype=torch.float32, device="cuda")
-    ids_d = torch.from_numpy(ids).cuda()
-    done = 0
+    done = 0                                                           # full iterations applied to x
     try:
-        for it in (1, 10, 20):
+        for it, s in ((1, 0), (10, 7), (20, 19)):
             if it - 1 > done:
                 plan.iterate(b_d, x, it - 1 - done, want_resid=False)
                 done = it - 1
+            plan.iterate_subsets(b_d, x, 0, s)                          # subsets 0 .. s-1 of iteration `it`
             x_prev = x.cpu().numpy()
-            x1 = x.clone()
-            plan_s.iterate(b_s_d, x1, 1, want_resid=False)         # first ordered subset of iteration `it`
-            got = x1.reshape(-1)[ids_d].cpu().numpy().astype(np.float64)
-            del x1
-            # the oracle's update of the sampled voxels
+            plan.iterate_subsets(b_d, x, s, s + 1)                      # the step under test
+            got = x.reshape(-1)[ids_d].cpu().numpy().astype(np.float64)
+            plan.iterate_subsets(b_d, x, s + 1, len(subsets))           # finish the iteration
+            done = it
+            # ---- the oracle's update of the sampled voxels with subset s
+            geo_s, ang_s, _ = subset_geometry("C3", subsets[s])
+            nS = len(subsets[s])
+            b_s = b_h[subsets[s]].astype(np.float64)
+            at1, fuv = orc.atb(None, geo_s, ang_s, orc.MATCHED, vox_ids=ids, return_fuv=True)
+            iu0, iv0 = np.floor(fuv[..., 0]).astype(np.int64), np.floor(fuv[..., 1]).astype(np.int64)     # [n_vox][nS]
+            ia = np.broadcast_to(np.arange(nS)[None, :], iu0.shape)
+            rays = []
+            for du in (0, 1):
+                for dv in (0, 1):
+                    u, v = iu0 + du, iv0 + dv
+                    ok = (u >= 0) & (u < nu) & (v >= 0) & (v < nv)
+                    rays.append(((ia * nv + v) * nu + u)[ok])
+            rid = np.unique(np.concatenate(rays))
+            a1 = orc.ax(ones, geo_s, ang_s, orc.SIDDON, ray_ids=rid)
+            W = np.where(a1 > eps_w, 1.0 / np.maximum(a1, 1e-300), 0.0)
+            seen = at1 > 1e-4 * at1.max()          # V's own threshold is 1e-6 max_j (A^T 1)_j over the volume: stay clear of it
+            assert np.count_nonzero(seen) > n_vox // 2
+            V = np.where(seen, 1.0 / np.maximum(at1, 1e-300), 0.0)
             r = np.zeros(nS * nv * nu)
-            r[rid] = W * (b_s_h.reshape(-1)[rid] - orc.ax(x_prev, geo_s, ang_s, orc.SIDDON, ray_ids=rid))
+            r[rid] = W * (b_s.reshape(-1)[rid] - orc.ax(x_prev, geo_s, ang_s, orc.SIDDON, ray_ids=rid))
             g = orc.atb(r.reshape(nS, nv, nu), geo_s, ang_s, orc.MATCHED, vox_ids=ids)
             xp = x_prev.reshape(-1)[ids].astype(np.float64)
             ref = np.maximum(xp + V * g, 0.0)
-            assert H.rel_l2(got[seen], ref[seen]) <= 1e-5, it
+            assert H.rel_l2(got[seen], ref[seen]) <= 1e-5, (it, s)
             moved = seen & ((ref > 0) | (got > 0))
-            assert H.rel_l2((got - xp)[moved], (ref - xp)[moved]) <= 1e-4, it      # the update itself
+            assert H.rel_l2((got - xp)[moved], (ref - xp)[moved]) <= 1e-4, (it, s)      # the update itself
             assert np.isfinite(got).all()
     finally:
         plan.close()
-        plan_s.close()
