@@ -192,3 +192,58 @@ def test_c3_full_size_ossart_teacher_forced(tg):
             assert np.isfinite(got).all()
     finally:
         plan.close()
+
+
+def test_c4_full_size_cgls_two_iterations_teacher_forced(tg):
+    """configs[3]: CGLS on the full C4 problem (1024^3, 1600 views of 1536^2, per-view detector roll / pitch / yaw, COR offset;
+    interpolated Ax, matched A^T b) through tigre_cgls, first two iterations, against the textbook recurrences (DESIGN.md O-F)
+    with the oracle's operators on 5000 sampled voxels.  The global scalars (gamma, ||A p||^2) are formed in fp64 from arrays
+    the SAME library calls produce outside the driver (teacher forcing: the oracle cannot form a 3.8e9-ray norm), so this
+    checks (i) the operators at full size inside the driver, (ii) the recurrences, (iii) the residual history.
+    Tolerance: x_1 = alpha_0 A^T b is linear in one matched backprojection (1e-5) times a ratio of two norms that carry the
+    interpolated projector's 1e-4: 3e-4; iteration 2 adds a second projection / backprojection pair: 6e-4."""
+    if torch.cuda.mem_get_info()[0] < 90e9:
+        pytest.skip("needs 90 GB of free HBM")
+    geo, ang, rec = make_config("C4")
+    nA = len(ang)
+    gen = torch.Generator(device="cuda").manual_seed(rec["seed"])
+    vol = torch.rand(geo.vol_shape, generator=gen, device="cuda") * 0.02
+    b = tg.Ax(vol, geo, ang, "interp")
+    del vol
+    ids = np.random.default_rng(77).integers(0, int(np.prod(geo.vol_shape)), 5000)
+    ids_d = torch.from_numpy(ids).cuda()
+
+    def dot(a, c):
+        return float((a.double().reshape(-1) * c.double().reshape(-1)).sum()) if a.numel() < 2 ** 31 else \
+            sum(float((a[i].double() * c[i].double()).sum()) for i in range(a.shape[0]))
+
+    x2, hist = tg.cgls(b, geo, ang, 2, "interp", "matched")
+    x1, _ = tg.cgls(b, geo, ang, 1, "interp", "matched")
+    got1 = x1.reshape(-1)[ids_d].cpu().numpy().astype(np.float64)
+    got2 = x2.reshape(-1)[ids_d].cpu().numpy().astype(np.float64)
+    del x1, x2
+    # ---- iteration 1: s0 = A^T b, p0 = s0, q0 = A p0, alpha0 = |s0|^2 / |q0|^2, x1 = alpha0 p0, r1 = b - alpha0 q0
+    s0 = tg.Atb(b, geo, ang, "matched")
+    q0 = tg.Ax(s0, geo, ang, "interp")
+    gamma0, qq0 = dot(s0, s0), dot(q0, q0)
+    alpha0 = gamma0 / qq0
+    b_h = b.cpu().numpy()
+    s0_ref = orc.atb(b_h, geo, ang, orc.MATCHED, vox_ids=ids)
+    assert H.rel_l2(got1, alpha0 * s0_ref) <= 3e-4
+    r1 = b - float(alpha0) * q0
+    assert hist[0] == pytest.approx(np.sqrt(dot(r1, r1)), rel=1e-4)
+    del q0, b, b_h
+    # ---- iteration 2: s1 = A^T r1, beta = |s1|^2 / gamma0, p1 = s1 + beta p0, alpha1 = |s1|^2 / |A p1|^2, x2 = x1 + alpha1 p1
+    s1 = tg.Atb(r1, geo, ang, "matched")
+    gamma1 = dot(s1, s1)
+    beta = gamma1 / gamma0
+    p1 = s1 + float(beta) * s0
+    del s1
+    q1 = tg.Ax(p1, geo, ang, "interp")
+    alpha1 = gamma1 / dot(q1, q1)
+    r1_h = r1.cpu().numpy()
+    del r1, q1, p1, s0
+    s1_ref = orc.atb(r1_h, geo, ang, orc.MATCHED, vox_ids=ids)
+    ref2 = alpha0 * s0_ref + alpha1 * (s1_ref + beta * s0_ref)
+    assert H.rel_l2(got2, ref2) <= 6e-4
+    assert H.rel_l2(got2 - got1, alpha1 * (s1_ref + beta * s0_ref)) <= 2e-3          # the second step on its own
