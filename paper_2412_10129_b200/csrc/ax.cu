@@ -287,6 +287,9 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
         jmax = __reduce_max_sync(wmask, any ? i0 + kA : (int)0x80000000);
         if (any) kA = min(max(kA, jmax - i0), kB);
     }
+#ifdef AX_PREFETCH
+    const IdxT pfo = (IdxT)AXG * r.sD + (IdxT)(int)((float)AXG * 1.5f * fabsf(1.0f / r.imE) + 0.5f) * r.stE;
+#endif
     const int last = nslab - 1;
     int k = 0;
     for (; k < kA; ++k)
@@ -301,6 +304,15 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
         const int jendmin = __reduce_min_sync(wmask, ranFast ? i0 + kB : 0x7fffffff);
         const int groups = jendmin == 0x7fffffff ? 0 : (jendmin - jmax) / AXG;
         for (int g = 0; g < groups; ++g) {
+#ifdef AX_PREFETCH
+            if (!UNIT && !SCATTER && !TRACK && ranFast) {
+                // the rows the next group will read, one L1 prefetch per row (a line holds 32 voxels along E: the drift of the
+                // ray over the group is folded into pfo)
+                const float* pf = base + (r.off + pfo);
+#pragma unroll
+                for (int j = 0; j < AXG; ++j) asm volatile("prefetch.global.L1 [%0];" ::"l"(pf + (IdxT)j * r.sD));
+            }
+#endif
             const bool nearF = ranFast && fmaf(r.hF, r.imF, -r.kf) <= (float)AXG;
             if (__any_sync(wmask, nearF)) {
                 if (ranFast) {
