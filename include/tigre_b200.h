@@ -301,6 +301,15 @@ TIGRE_API int tigre_Ax_count(const tigre_geo *geo, const double *angles, int nA,
  * first_last dev int64 [nA][nv][nu][2]; nseg dev uint32 [nA][nv][nu].  Asynchronous. */
 TIGRE_API int tigre_Ax_index(const tigre_geo *geo, const double *angles, int nA, int64_t *first_last, uint32_t *nseg,
                    void *cuda_stream);
+/* Footprint bounds of the TMA-staged backprojector (north_star "footprint bounds must match exactly"; reading P19(b)):
+ * tigre_Atb with the kernel reporting, per (voxel tile, view), the detector box it staged into shared memory.
+ * meta (host int32[8]) receives the tiling: tile size in voxels (x, y, z), box size in pixels (u, v), number of tiles (x, y, z);
+ * all zero if this problem does not take the TMA kernel.  boxes (dev int32 [tiles_z][tiles_y][tiles_x][nA][4], or NULL to
+ * query meta only: nothing is launched then) receives (u0, v0, fits, 0): the absolute detector index of the box origin and
+ * whether the view's footprint fitted the box (0: the kernel gathered that view through L1 / L2 with bounds checks).
+ * vol is written as by tigre_Atb.  Voxel-driven modes only. */
+TIGRE_API int tigre_Atb_boxes(const float *proj, const tigre_geo *geo, const double *angles, int nA, int mode, float *vol,
+                    int32_t *meta, int32_t *boxes, void *cuda_stream);
 /* In-library timing for bench.py's roofline leg.  tigre_profile(1) resets and starts recording a CUDA
  * event pair around every kernel group the launchers enqueue (on the launching stream); tigre_profile(0)
  * stops.  tigre_profile_read waits for the recorded events and returns, per kind k = 0 (Ax kernels),

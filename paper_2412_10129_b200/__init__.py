@@ -53,7 +53,7 @@ EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_Ax_slab", "tigre_Atb_slab", "tigre_sl
            "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_create_ex", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_osem", "tigre_plan_sart_tv", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version", "tigre_Ax_index", "tigre_set_index_path", "tigre_set_workspace", "tigre_plan_workspace_bytes",
-           "tigre_workspace_stats", "tigre_sirt_chunked", "tigre_microbench", "tigre_set_ax_path", "tigre_set_plan_v_path", "tigre_plan_ossart_subsets"]
+           "tigre_workspace_stats", "tigre_sirt_chunked", "tigre_microbench", "tigre_set_ax_path", "tigre_set_plan_v_path", "tigre_plan_ossart_subsets", "tigre_Atb_boxes"]
 
 
 def _lib():
@@ -482,6 +482,26 @@ def Ax_count(geo, angles, mode="siddon", return_counts=False, device="cuda"):
                                  C.c_void_p(counts.data_ptr()) if return_counts else None, C.byref(total),
                                  _stream(counts)), "tigre_Ax_count")
     return (total.value, counts) if return_counts else total.value
+
+
+def Atb_boxes(proj, geo, angles, mode="matched"):
+    """Reading P19(b): (vol, meta, boxes) of the TMA-staged backprojector: meta = dict(tile=(x, y, z), box=(u, v), tiles=(x, y, z)) or
+    None when the problem takes the gather kernel; boxes int32 [tz][ty][tx][nA][4] = (u0, v0, fits, 0)."""
+    import torch
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    pp = _f32(proj, proj_shape(geo, nA), "proj")
+    vol = _new(vol_shape(geo), like=proj)
+    meta = (C.c_int32 * 8)()
+    _check(_lib().tigre_Atb_boxes(pp, G.ref, a.ctypes.data_as(_dp), nA, _ATB_MODES[mode], _f32(vol), meta, None, _stream(proj)),
+           "tigre_Atb_boxes")
+    m = [int(v) for v in meta]
+    if m[0] == 0:
+        return Atb(proj, geo, angles, mode), None, None
+    boxes = torch.empty((m[7], m[6], m[5], nA, 4), dtype=torch.int32, device=proj.device)
+    _check(_lib().tigre_Atb_boxes(pp, G.ref, a.ctypes.data_as(_dp), nA, _ATB_MODES[mode], _f32(vol), meta,
+                                  C.c_void_p(boxes.data_ptr()), _stream(proj)), "tigre_Atb_boxes")
+    return vol, dict(tile=tuple(m[0:3]), box=tuple(m[3:5]), tiles=tuple(m[5:8])), boxes
 
 
 def Ax_index(geo, angles, device="cuda"):

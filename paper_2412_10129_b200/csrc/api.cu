@@ -505,6 +505,26 @@ int tigre_microbench(int kind, double* value, void* cuda_stream) {
 
 // test hook (tigre_set_plan_v_path): 0 = store V_s per subset when they fit (default), 1 = always store, 2 = always recompute
 static int g_plan_v_path = 0;
+}  // extern "C"
+namespace tg {
+extern int* g_atb_box_meta;
+extern int32_t* g_atb_boxes;
+}
+extern "C" {
+int tigre_Atb_boxes(const float* proj, const tigre_geo* geo, const double* angles, int nA, int mode, float* vol, int32_t* meta,
+                    int32_t* boxes, void* cuda_stream) {
+    if (!proj || !vol || !meta) return TIGRE_ERR_ARG;
+    if (mode != TIGRE_ATB_MATCHED && mode != TIGRE_ATB_FDK) return TIGRE_ERR_ARG;
+    Tables t;
+    TG_TRY(prep(geo, angles, nA, t));
+    if (mem_kind(proj) != MEM_DEVICE || mem_kind(vol) != MEM_DEVICE || (boxes && mem_kind(boxes) != MEM_DEVICE)) return TIGRE_ERR_MEMSPACE;
+    for (int i = 0; i < 8; ++i) meta[i] = 0;
+    g_atb_box_meta = meta, g_atb_boxes = boxes;
+    const int rc = device_atb(proj, t, nullptr, nA, mode, false, vol, (cudaStream_t)cuda_stream);
+    g_atb_box_meta = nullptr, g_atb_boxes = nullptr;
+    return rc;
+}
+
 int tigre_set_plan_v_path(int path) {
     if (path < 0 || path > 2) return TIGRE_ERR_ARG;
     g_plan_v_path = path;

@@ -38,6 +38,8 @@ struct StageInfo {   // written by the producer before it arms the stage's full 
 }  // namespace
 
 extern int g_atb_path;   // atb.cu
+int* g_atb_box_meta = nullptr;   // tigre_Atb_boxes (api.cu): host int[8] to fill, and the device buffer for the boxes
+int32_t* g_atb_boxes = nullptr;
 
 // BU (box width, pixels) is a template parameter so that the second tap row is an immediate offset; the
 // launcher picks the smallest of 48, 80, ... 240 (all = 16 mod 32: with the 8 x 4 lane layout below, the taps
@@ -45,7 +47,7 @@ extern int g_atb_path;   // atb.cu
 template <int MODE, int WX, int WY, int ZR, int BU>
 __global__ void __launch_bounds__(32 * (WX * WY + 1), 2)
 atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict__ proj, const VoxView* __restrict__ views,
-               int nViews, AtbP p, int BV, int nStages, float* __restrict__ vol) {
+               int nViews, AtbP p, int BV, int nStages, float* __restrict__ vol, int4* __restrict__ boxes) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int stageElems = (BU * BV + 31) & ~31;   // 128-byte multiple
     float* tiles = reinterpret_cast<float*>(smem_raw);
@@ -99,6 +101,8 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
                 }
                 if (a >= nStages) mbar_wait(empty + s, ph);
                 info[s].c0 = c0, info[s].c1 = c1, info[s].fits = fits;
+                if (boxes)   // tigre_Atb_boxes (reading P19(b)): the staged box of this (tile, view), absolute detector indices
+                    boxes[((size_t)(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * nViews + a] = make_int4(c0, c1, fits, 0);
                 info[s].rU = rU, info[s].rV = rV, info[s].rW = rW, info[s].rG = rG, info[s].cst = cst;
                 if (fits) {
                     mbar_arrive_expect_tx(full + s, (uint32_t)(BU * BV * sizeof(float)));
@@ -307,7 +311,14 @@ int tma_launch(const TmaArgs& A) {
     TG_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 block(32, WX * WY + 1), grid((A.p.nx + 8 * WX - 1) / (8 * WX), (A.p.ny + 4 * WY - 1) / (4 * WY), (A.p.nzs + ZR - 1) / ZR);
     if (grid.y > 65535 || grid.z > 65535) return TIGRE_ERR_ARG;
-    kern<<<grid, block, smem, A.st>>>(A.map, A.proj, A.d_views, A.nViews, A.p, A.BV, A.nStages, A.vol);
+    int4* boxes = nullptr;
+    if (g_atb_box_meta) {   // tigre_Atb_boxes: report the tiling; write the boxes if the caller's buffer is there
+        int* m = g_atb_box_meta;
+        m[0] = 8 * WX, m[1] = 4 * WY, m[2] = ZR, m[3] = BU, m[4] = A.BV, m[5] = (int)grid.x, m[6] = (int)grid.y, m[7] = (int)grid.z;
+        boxes = reinterpret_cast<int4*>(g_atb_boxes);
+        if (!boxes) return TIGRE_OK;   // size query only
+    }
+    kern<<<grid, block, smem, A.st>>>(A.map, A.proj, A.d_views, A.nViews, A.p, A.BV, A.nStages, A.vol, boxes);
     TG_CUDA(cudaGetLastError());
     return TIGRE_OK;
 }

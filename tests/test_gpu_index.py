@@ -199,3 +199,55 @@ def test_ax_above_2_31_voxels_sampled(tg):
     flh = fl.cpu().numpy().reshape(-1, 2)[ids]
     assert np.array_equal(flh[ok, 0], o["first"][ok]) and np.array_equal(flh[ok, 1], o["last"][ok])
     assert flh[ok].max() >= 2 ** 31                                           # indices that need 64 bits were compared
+
+
+# ------------------------------------------------------------------ P19(b): staged boxes of the TMA backprojector
+def _box_geometries():
+    ga = Geometry(nVoxel=(75, 50, 29), dVoxel=(1.0, 1.0, 1.2), nDetector=(96, 44), dDetector=(1.5, 1.5),
+                  DSD=600.0, DSO=380.0, offDetector=(7.0, -3.0))
+    aa = circular_angles(13, start=0.05)
+    rng = np.random.default_rng(5)
+    gb = Geometry(nVoxel=(64, 48, 40), dVoxel=(1.0, 1.0, 1.0), nDetector=(112, 80), dDetector=(1.2, 1.2), DSD=500.0, DSO=320.0,
+                  COR=0.4, rotDetector=(0.02, -0.03, 0.05))
+    ab = np.stack([rng.uniform(0, 2 * np.pi, 9), rng.uniform(-0.1, 0.1, 9), rng.uniform(-0.1, 0.1, 9)], 1)
+    gb.rotDetector_a = np.asarray(gb.rotDetector) + 0.01 * rng.standard_normal((9, 3))
+    return [(ga, aa), (gb, ab)]
+
+
+@pytest.mark.parametrize("case", [0, 1])
+def test_staged_boxes_contain_the_exact_footprint(tg, case):
+    """Per (voxel tile, view): the detector box the kernel stages holds every bilinear tap of every voxel of the tile (the oracle's
+    voxel map gives the taps), and its origin sits at most 5 pixels below the lowest tap (one pixel of slack, up to three for
+    the 16-byte alignment TMA demands of the row, one for fp32 rounding of the corner projections).  The box has ONE size
+    per launch (the largest footprint over tiles and views), so the upper slack is whatever that leaves: "at most one pixel per
+    side" holds for the origin, not for a fixed-size box.  Views flagged as not fitting are gathered with
+    bounds checks by the kernel instead and are exempt; there must be none in these geometries."""
+    geo, ang = _box_geometries()[case]
+    nA = len(ang)
+    proj = np.random.default_rng(case).random((nA,) + geo.proj_shape, dtype=np.float32)
+    vol, meta, boxes = tg.Atb_boxes(dev(proj), geo, ang, "matched")
+    assert meta is not None, "this geometry must take the TMA kernel"
+    ref, fuv = orc.atb(proj, geo, ang, orc.MATCHED, return_fuv=True)
+    assert H.rel_l2(host(vol), ref) <= 1e-5
+    nx, ny, nz = geo.nVoxel
+    fu = np.floor(fuv[..., 0]).astype(np.int64).reshape(nz, ny, nx, nA)
+    fv = np.floor(fuv[..., 1]).astype(np.int64).reshape(nz, ny, nx, nA)
+    bx, by, bz = meta["tile"]
+    BU, BV = meta["box"]
+    tx, ty, tz = meta["tiles"]
+    b = boxes.cpu().numpy()
+    assert b.shape == (tz, ty, tx, nA, 4) and np.all(b[..., 2] == 1)
+    worst_lo, checked = 0, 0
+    for kz in range(tz):
+        for ky in range(ty):
+            for kx in range(tx):
+                sl = (slice(kz * bz, min(nz, (kz + 1) * bz)), slice(ky * by, min(ny, (ky + 1) * by)), slice(kx * bx, min(nx, (kx + 1) * bx)))
+                ulo, uhi = fu[sl].min(axis=(0, 1, 2)), fu[sl].max(axis=(0, 1, 2)) + 1
+                vlo, vhi = fv[sl].min(axis=(0, 1, 2)), fv[sl].max(axis=(0, 1, 2)) + 1
+                u0, v0 = b[kz, ky, kx, :, 0], b[kz, ky, kx, :, 1]
+                assert np.all(u0 <= ulo) and np.all(uhi < u0 + BU), (kz, ky, kx)
+                assert np.all(v0 <= vlo) and np.all(vhi < v0 + BV), (kz, ky, kx)
+                if (kx + 1) * bx <= nx and (ky + 1) * by <= ny and (kz + 1) * bz <= nz:   # (a ragged tile's box is placed for the whole tile)
+                    worst_lo = max(worst_lo, int((ulo - u0).max()), int((vlo - v0).max()))
+                checked += nA
+    assert worst_lo <= 5 and checked == tx * ty * tz * nA
