@@ -351,6 +351,10 @@ TIGRE_API int tigre_set_atb_path(int path);
  * aligned volume, the beam of a 32 x 4 pixel tile fits a stage), 1 = always the L1 gather kernel, 2 = the TMA kernel for wide
  * beams too.  Same samples, same per-ray order of summation; A/B and test hook. */
 TIGRE_API int tigre_set_ax_path(int path);
+/* which FDK pre-filter kernel runs: 0 (default) = the Toeplitz GEMM on the tensor cores (tcgen05, 3 x tf32 split products into an fp32
+ * accumulator in tensor memory) whenever nDetector_u is a multiple of 4 and input and output are distinct 16-byte aligned arrays,
+ * 1 = always the CUDA-core convolution.  Same taps, same weights; A/B and test hook. */
+TIGRE_API int tigre_set_fdk_path(int path);
 /* which TV gradient kernel runs: 0 (default) = four voxels along x per thread whenever nx % 4 == 0, ny > 1, nz > 1 and
  * the arrays are 16-byte aligned, 1 = always the one-voxel-per-thread kernel (any shape).  Same sums; A/B and test hook. */
 TIGRE_API int tigre_set_tv_path(int path);

@@ -992,6 +992,15 @@ static int fdk_filter_impl(const float* b, Tables& t, int nA, float* q, cudaStre
         dd[a] = t.views[a].DSD, dd[nA + a] = t.views[a].DSO, dd[2 * nA + 2 * a] = t.views[a].offD[0], dd[2 * nA + 2 * a + 1] = t.views[a].offD[1];
     // parallel beam (P29): no magnification (tau = du) and no cosine weight: the kernels' DSO/DSD = 1, DSD/sqrt(DSD^2 + u^2 + v^2) = 1
     if (t.views[0].parallel) std::fill(dd.begin(), dd.begin() + 2 * nA, 1e15);
+    {
+        // tensor-core filter (fdk_tc.cu) where the problem qualifies
+        std::vector<double> taps;
+        fdk_filter_taps(t.g.nu, TIGRE_FILTER_RAM_LAK, taps);
+        const std::vector<float> ft(taps.begin(), taps.end());
+        const std::vector<double> dsd(dd.begin(), dd.begin() + nA), dso(dd.begin() + nA, dd.begin() + 2 * nA), offd(dd.begin() + 2 * nA, dd.end());
+        const int rc = launch_fdk_filter_tc(b, t.g, dsd, dso, offd, nA, ft, nullptr, q, st);
+        if (rc <= 0) return rc;
+    }
     TempBuf tb;
     TG_TRY(upload(tb, dd.data(), sizeof(double) * dd.size(), st));
     // Ram-Lak, no weights: taps formed in the kernel, odd taps only (fdk.cu)
@@ -1041,6 +1050,11 @@ static int fdk_filter_ex_impl(const float* b, Tables& t, int nA, int filter, int
         const double k = weighting == TIGRE_FDK_WANG ? 2.0 : 1.0;
         for (size_t i = 0; i < w.size(); ++i) fw[i] = (float)(k * w[i]);
         TG_TRY(upload(tw, fw.data(), sizeof(float) * fw.size(), st));
+    }
+    {
+        const std::vector<double> dsd(dd.begin(), dd.begin() + nA), dso(dd.begin() + nA, dd.begin() + 2 * nA), offd(dd.begin() + 2 * nA, dd.end());
+        const int rc = launch_fdk_filter_tc(b, t.g, dsd, dso, offd, nA, ft, weighting != TIGRE_FDK_FULL ? tw.as<float>() : nullptr, q, st);
+        if (rc <= 0) return rc;
     }
     return launch_fdk_filter_taps(b, t.g, tb.as<double>(), tb.as<double>() + nA, tb.as<double>() + 2 * nA, nA, tt.as<float>(),
                                   weighting != TIGRE_FDK_FULL ? tw.as<float>() : nullptr, q, st, filter == TIGRE_FILTER_RAM_LAK);

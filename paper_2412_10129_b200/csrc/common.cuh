@@ -158,6 +158,10 @@ void fdk_filter_taps(int nu, int filter, std::vector<double>& g);
 int fdk_weights(const Grid& g, const std::vector<ViewH>& views, int weighting, std::vector<double>& w);
 int launch_fdk_filter_taps(const float* b, const Grid& g, const double* d_dsd, const double* d_dso, const double* d_offd, int nViews,
                            const float* d_taps, const float* d_colw, float* q, cudaStream_t st, bool odd_only = false);
+// the same filter on the tensor cores (fdk_tc.cu); returns 1 if the problem does not qualify (then the kernel above runs)
+int launch_fdk_filter_tc(const float* b, const Grid& g, const std::vector<double>& dsd, const std::vector<double>& dso,
+                         const std::vector<double>& offd, int nViews, const std::vector<float>& h_taps, const float* d_colw, float* q,
+                         cudaStream_t st);
 int launch_flatten(const float* curved, const Grid& g, const double* d_dsd, int nViews, float* flat, cudaStream_t st);
 int launch_count_reduce(const uint32_t* c, size_t n, unsigned long long* d_total, cudaStream_t st);
 

@@ -9,6 +9,7 @@
 // fp64 and multiplied into the cosine-weighted row before the convolution.
 #include <algorithm>
 #include <cmath>
+#include <mutex>
 #include <vector>
 #include "common.cuh"
 
@@ -195,8 +196,22 @@ double window_at(int filter, double om) {
 
 }  // namespace
 
-// taps for tau = 1 (the kernel scales by 1/tau: h ~ 1/tau^2, times the tau of the quadrature)
+// taps for tau = 1 (the kernel scales by 1/tau: h ~ 1/tau^2, times the tau of the quadrature).  The windowed taps cost two
+// O(nu L) cosine sums on the host (4 ms for nu = 1024, while the tensor-core filter of a whole C3 scan takes 7): the last
+// (nu, filter) pair is kept.
+static void fdk_filter_taps_compute(int nu, int filter, std::vector<double>& g);
 void fdk_filter_taps(int nu, int filter, std::vector<double>& g) {
+    static std::mutex mu;
+    static int c_nu = -1, c_filter = -1;
+    static std::vector<double> cache;
+    std::lock_guard<std::mutex> lk(mu);
+    if (nu != c_nu || filter != c_filter) {
+        fdk_filter_taps_compute(nu, filter, cache);
+        c_nu = nu, c_filter = filter;
+    }
+    g = cache;
+}
+static void fdk_filter_taps_compute(int nu, int filter, std::vector<double>& g) {
     g.assign(nu, 0.0);
     if (filter == TIGRE_FILTER_RAM_LAK) {
         g[0] = 0.25;

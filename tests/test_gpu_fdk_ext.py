@@ -148,3 +148,36 @@ def test_curved_detector_flattening_matches_oracle(tg):
     b = torch.rand((2, 1536, 1536), generator=gen, device="cuda")
     refb = ocurved.flatten(b.cpu().numpy(), big)
     assert H.rel_l2(host(tg.flatten_detector(b, big, ang[:2])), refb) <= 1e-4
+
+
+# ------------------------------------------------------------------ the tensor-core pre-filter (fdk_tc.cu) against the CUDA-core one
+@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("nu,nv,nA", [(96, 9, 5), (332, 37, 7), (1024, 6, 3)])
+def test_fdk_filter_kernel_paths_match_oracle(tg, path, nu, nv, nA):
+    """tigre_set_fdk_path: 0 = Toeplitz GEMM on tcgen05 (3 x tf32 split products, fp32 accumulator in tensor memory), 1 = CUDA-core
+    convolution.  Widths below one N tile (96), ragged in every tile dimension (332 = 256 + 76 columns, 7 x 37 = 259 rows = 2 row
+    tiles + 3), C3's width (1024: 4 passes x 32 K blocks), displaced detector + per-view distances, every filter, Wang and
+    Parker column weights: both kernels within 1e-5 of the oracle's fp64 filter."""
+    rng = np.random.default_rng(nu)
+    geo = Geometry(nVoxel=(8, 8, 8), dVoxel=(1.0,) * 3, nDetector=(nu, nv), dDetector=(0.4 * 1024 / nu, 1.1), DSD=700.0, DSO=450.0,
+                   offDetector=(0.11 * nu * 0.4 * 1024 / nu, -1.7))
+    geo.DSD_a = 700.0 + rng.uniform(-40, 40, nA)
+    ang = np.stack([np.linspace(0.1, 2 * np.pi, nA, endpoint=False), np.zeros(nA), np.zeros(nA)], 1)
+    p = rng.random((nA, nv, nu)).astype(np.float32)
+    tg.set_fdk_path(path)
+    try:
+        for filt in ("ram_lak", "hann", "shepp_logan"):
+            assert H.rel_l2(host(tg.fdk_filter_ex(dev(p), geo, ang, filt)), fx.fdk_filter(p, geo, ang, filt)) <= 1e-5, filt
+        assert H.rel_l2(host(tg.fdk_filter(dev(p), geo, ang)), orc.fdk_filter(p, geo, ang)) <= 1e-5
+        w = 2.0 * fx.wang_weights(geo, nA)
+        assert H.rel_l2(host(tg.fdk_filter_ex(dev(p), geo, ang, "hamming", "wang")), fx.fdk_filter(p, geo, ang, "hamming", w)) <= 1e-5
+        # smooth data: the ramp filter cancels two to three digits of the sum, so the fp32 rounding of the taps and of the
+        # accumulation (6e-8 of the terms) shows as up to 1e-4 of the RESULT in either kernel: north_star's FDK tolerance
+        u = np.linspace(-1, 1, nu)[None, None, :]
+        smooth = (np.sqrt(np.maximum(1.0 - u * u, 0.0)) * (1.0 + 0.1 * rng.random((nA, nv, 1)))).astype(np.float32)
+        ref = orc.fdk_filter(smooth, geo, ang)
+        got = host(tg.fdk_filter(dev(smooth), geo, ang))
+        assert np.linalg.norm(ref) < 0.2 * np.linalg.norm(smooth) / (4 * (geo.dDetector[0] * 450 / 700) ** 1)    # cancellation is real
+        assert H.rel_l2(got, ref) <= 2e-4
+    finally:
+        tg.set_fdk_path(0)
