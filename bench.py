@@ -42,14 +42,17 @@ UNIT = "G(samples+updates)/s"
 # captures (l1tex__data_pipe_lsu_wavefronts / samples):
 #   A^T b            22 thread-instr and 16 B of shared-memory taps per voxel-update
 #   Ax Siddon        18 thread-instr per segment; L1: W wavefronts per warp-sample (measured, table below)
-#   Ax interpolated  40 thread-instr per sample; L1: 8 taps, two samples share a cell at a step of half a voxel: 12 wavefronts
-#                    per warp-sample ("24 ... ~halved by reusing a cell's 8 corners")
+#   Ax interpolated  40 thread-instr per sample; L1: 8 tap requests per sample, each at least TWO wavefronts on C2 / C4, where the 32
+#                    rays of a warp are 1.04 / cos(theta) voxels apart and one request spans 132-188 bytes of a row: 16 per warp-
+#                    sample.  (SURVEY.md section 8(d) guessed 24, "~halved by reusing a cell's 8 corners": reuse saves no REQUEST in a
+#                    SIMT gather, the lanes change cells at different samples; shared-memory staging measured 17.6:
+#                    profiles/r2_ax_interp_tma.md.  The L1 kernel itself needs 22: ncu.)
 SM_COUNT = 148
 ALGO_INSTR = {"atb": 22.0, "ax_siddon": 18.0, "ax_interp": 40.0}
 # L1 data-pipe wavefronts per 32 samples of the Siddon march, from ncu (profiles/r1_late_ax_siddon.md: data pipe 42.7 % busy at
 # 1397.6 G samples/s, 148 SMs x 1965 MHz => 2.84 wavefronts per warp-sample on C3)
 SIDDON_WAVEFRONTS_PER_WARP_SAMPLE = 2.84
-INTERP_WAVEFRONTS_PER_WARP_SAMPLE = 12.0
+INTERP_WAVEFRONTS_PER_WARP_SAMPLE = 16.0
 NOMINAL_PEAKS = {"ffma": 148 * 128 * 1.965e9, "smem": 148 * 128 * 1.965e9, "l1_lines": 148 * 1.965e9}
 
 PEAK_UNITS = {"ffma": "thread-instr/s", "smem": "B/s", "l1_lines": "128-B lines/s", "l2": "B/s", "h2d": "B/s", "d2h": "B/s",
@@ -510,6 +513,10 @@ def kernel_rates_other_configs(tg, rates):
     on seeded random data, against the same measured-rate bounds.  C5's rates are `--mode chunked`'s (profiles/)."""
     import torch
     out = {}
+    try:
+        mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        mp = {}
     for name, n_views in (("C2", None), ("C4", 64)):
         geo, ang, rec = make_config(name)
         if n_views:
@@ -542,7 +549,16 @@ def kernel_rates_other_configs(tg, rates):
         ms_atb, _ = timed(lambda: tg.Atb(b, geo, ang, rec["atb"]))
         kax = "ax_" + rec["ax"]
         ax_rate, atb_rate = samples / (ms_ax * 1e-3) / 1e9, updates / (ms_atb * 1e-3) / 1e9
-        out[name] = {"workload": f"{geo.nVoxel[0]}^3, {len(ang)} views of {geo.nDetector[0]}x{geo.nDetector[1]}" + (f" (of {rec['nA']})" if n_views else ""),
+        extra = {}
+        if rec["atb"] == "fdk":
+            # the FDK pre-filter (fdk_tc.cu): the path's dense contraction, on the tensor cores: 3 split tf32 products per multiply-add
+            ms_f, _ = timed(lambda: tg.fdk_filter(b, geo, ang))
+            flop = 3.0 * 2.0 * len(ang) * geo.nDetector[1] * float(geo.nDetector[0]) ** 2
+            tf32_peak = float(mp.get("bf16_tflops", 1591.4)) * 0.5
+            extra["fdk_filter"] = {"ms": ms_f, "achieved": flop / (ms_f * 1e-3) / 1e12, "unit": "TFLOP/s (tf32, 3 split products per fp32 multiply-add)",
+                                   "bound": "tensor", "peak": tf32_peak, "frac": flop / (ms_f * 1e-3) / 1e12 / tf32_peak,
+                                   "peak_source": "MEASURED_PEAKS.json bf16_tflops x the guide's nominal tf32 : bf16 ratio 1/2"}
+        out[name] = {"workload": f"{geo.nVoxel[0]}^3, {len(ang)} views of {geo.nDetector[0]}x{geo.nDetector[1]}" + (f" (of {rec['nA']})" if n_views else ""), **extra,
                      kax: {"achieved": ax_rate, "unit": "Gsamples/s", "peak": model_peak(kax, rates), "frac": ax_rate / model_peak(kax, rates),
                            "ms": ms_ax},
                      "atb_" + rec["atb"]: {"achieved": atb_rate, "unit": "Gupdates/s", "peak": model_peak("atb", rates),

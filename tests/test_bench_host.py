@@ -52,7 +52,7 @@ def test_roofline_model_and_subsets():
     assert bench.model_peak("atb", r) == pytest.approx(148 * 128 * 1965e6 / 22 / 1e9)                  # 1.69 T updates/s (smem: 2.3)
     assert bench.model_peak("ax_siddon", r) == pytest.approx(148 * 128 * 1965e6 / 18 / 1e9)            # 2.07 T samples/s: issue binds
     assert bench.model_bounds("ax_siddon", r)["l1"] == pytest.approx(148 * 1965e6 * 32 / 2.84 / 1e9)   # (L1 at the measured 2.84 wavefronts)
-    assert bench.model_peak("ax_interp", r) == pytest.approx(148 * 1965e6 / 12 * 32 / 1e9)             # 0.78 T samples/s: L1 binds
+    assert bench.model_peak("ax_interp", r) == pytest.approx(148 * 1965e6 / 16 * 32 / 1e9)             # 0.58 T samples/s: L1 binds
     assert "binding = issue" in bench.peak_source("ax_siddon", r, False)
     subs = bench.subsets_for({"name": "C3"}, 720)                   # reading P15: 20 interleaved subsets
     assert len(subs) == 20 and all(len(s) == 36 for s in subs)
