@@ -251,6 +251,13 @@ ax_interp_tma_kernel(const __grid_constant__ CUtensorMap mapV, const __grid_cons
                     const float mx = (x - 0.5f) + 12582912.0f, my = (y - 0.5f) + 12582912.0f, mz = (z - 0.5f) + 12582912.0f;
                     const float ax = x - (mx - 12582912.0f), ay = y - (my - 12582912.0f), az = z - (mz - 12582912.0f);
                     const uint32_t q = qb + 4u * (__float_as_uint(mz) * (uint32_t)PLANE + __float_as_uint(my) * (uint32_t)BX + __float_as_uint(mx));
+#ifdef AXT_CHECK   // debug build (nvcc -DAXT_CHECK): every tap of every staged sample must lie inside the box the producer loaded
+                    {
+                        const int cx = __float_as_int(mx) - 0x4B400000 - info[s].bx, cy = __float_as_int(my) - 0x4B400000 - info[s].by,
+                                  cz = __float_as_int(mz) - 0x4B400000 - info[s].bz;
+                        if (cx < 0 || cx + 1 >= BX || cy < 0 || cy + 1 >= AXT_BY || cz < 0 || cz + 1 >= BZ) __trap();
+                    }
+#endif
                     float v000, v100, v010, v110, v001, v101, v011, v111;
                     asm volatile(
                         "ld.shared.f32 %0, [%8];\n\t"
