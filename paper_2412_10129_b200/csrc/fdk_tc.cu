@@ -33,8 +33,17 @@ namespace {
 constexpr int FT_M = 128, FT_N = 256, FT_K = 32, FT_STAGES = 2;
 constexpr int FT_A_BYTES = FT_M * FT_K * 4;                          // 16 KB
 constexpr int FT_B_BYTES = FT_N * FT_K * 4;                          // 32 KB
-constexpr int FT_STAGE_BYTES = 2 * FT_A_BYTES + 2 * FT_B_BYTES;      // A (-> a_hi), a_lo, B_hi, B_lo = 96 KB
-constexpr int FT_SMEM = FT_STAGES * FT_STAGE_BYTES + 1024 /* alignment */ + 256 /* barriers, tmem slot */;
+constexpr int FT_STAGE_BYTES = 2 * FT_A_BYTES;                       // A (-> a_hi), a_lo = 32 KB per stage
+// The Toeplitz operand is a RING of rows in shared memory.  B_kb[n][k] = g[|(n0 + n) - (32 kb + k)|] = H[n0 + n - 32 kb][k] with
+// H[m][k] = g[|m - k|]: the 256 x 32 tiles of consecutive K blocks are the SAME rows of H shifted by 32, so a K block brings 32 new
+// rows (2 x 4 KB) instead of a whole tile (2 x 32 KB).  288 = 256 + 32 rows: the new rows of K block kb take the slots that left the
+// window after K block kb - 2, the very tensor-core reads whose completion frees A's stage; the window wraps around the ring, so the
+// N = 256 product is issued as two tcgen05.mma (N1 and 256 - N1 columns of the accumulator).  Two rings alternate between passes.
+constexpr int FT_RING_ROWS = FT_N + FT_K;                            // 288 rows of 128 bytes = 36 swizzle atoms
+constexpr int FT_RING_BYTES = FT_RING_ROWS * 128;                    // 36 KB
+constexpr int FT_RINGS_OFF = FT_STAGES * FT_STAGE_BYTES;             // [A stages][ring 0: hi, lo][ring 1: hi, lo]
+constexpr int FT_BAR_OFF = FT_RINGS_OFF + 4 * FT_RING_BYTES;
+constexpr int FT_SMEM = FT_BAR_OFF + 1024 /* alignment */ + 256 /* barriers, tmem slot */;
 constexpr int FT_THREADS = 192;
 
 __device__ __forceinline__ float rn_tf32(float x) {
@@ -54,17 +63,19 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, i
 __device__ __forceinline__ uint64_t umma_desc_k128(uint32_t smem_addr) {
     return (uint64_t)((smem_addr & 0x3FFFFu) >> 4) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
 }
-// kind::tf32, fp32 accumulator, both operands K-major, M 128, N 256 (cute::UMMA::InstrDescriptor)
-constexpr uint32_t FT_IDESC = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(FT_N >> 3) << 17) | ((uint32_t)(FT_M >> 4) << 24);
+// kind::tf32, fp32 accumulator, both operands K-major, M 128, N columns (cute::UMMA::InstrDescriptor)
+__device__ __forceinline__ constexpr uint32_t ft_idesc(int n) {
+    return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(FT_M >> 4) << 24);
+}
 
-__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t accumulate) {
+__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
     asm volatile(
         "{\n\t"
         ".reg .pred p;\n\t"
         "setp.ne.b32 p, %4, 0;\n\t"
         "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t"
         "}\n" ::"r"(tmem_d),
-        "l"(da), "l"(db), "r"(FT_IDESC), "r"(accumulate)
+        "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
         : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint64_t* bar) {
@@ -75,15 +86,17 @@ struct FtRow {       // per-view quantities the transform and the epilogue need 
     float dsd, itau, offu, offv;
 };
 
-// T_hi / T_lo [nu][nu]: the symmetric Toeplitz matrix of the taps, split into two tf32 parts
-__global__ void __launch_bounds__(256) ft_toeplitz_kernel(const float* __restrict__ taps, int nu, float* __restrict__ thi, float* __restrict__ tlo) {
-    const size_t total = (size_t)nu * nu;
-    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
-        const int n = (int)(i / nu), k = (int)(i - (size_t)n * nu);
-        const float t = __ldg(taps + abs(n - k));
+// H_hi / H_lo [rowsH][32]: H[j][k] = g[|j - shift - k|] (0 beyond the taps), split into two tf32 parts; shift = 32 nKb
+__global__ void __launch_bounds__(256) ft_toeplitz_kernel(const float* __restrict__ taps, int nu, int rowsH, int shift, float* __restrict__ hhi,
+                                                          float* __restrict__ hlo) {
+    const int total = rowsH * FT_K;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < total; i += gridDim.x * blockDim.x) {
+        const int j = i / FT_K, k = i - j * FT_K;
+        const int m = abs(j - shift - k);
+        const float t = m < nu ? __ldg(taps + m) : 0.f;
         const float hi = rn_tf32(t);
-        thi[i] = hi;
-        tlo[i] = rn_tf32(t - hi);
+        hhi[i] = hi;
+        hlo[i] = rn_tf32(t - hi);
     }
 }
 
@@ -93,7 +106,7 @@ fdk_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ 
               float du, float dv, int nTiles) {
     extern __shared__ unsigned char smem_raw[];
     unsigned char* sm = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(sm + FT_STAGES * FT_STAGE_BYTES);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(sm + FT_BAR_OFF);
     uint64_t *full = bars, *ready = bars + FT_STAGES, *empty = bars + 2 * FT_STAGES, *accfull = bars + 3 * FT_STAGES,
              *accempty = bars + 3 * FT_STAGES + 1;
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 3 * FT_STAGES + 2);
@@ -123,17 +136,24 @@ fdk_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ 
     if (warp == 4) {
         // ------------------------------------------------------------ TMA producer
         if (lane == 0) {
-            uint32_t it = 0;
+            uint32_t it = 0, pc = 0;
             for (int tile = blockIdx.x; tile < nTiles; tile += gridDim.x)
-                for (int ps = 0; ps < nPass; ++ps)
+                for (int ps = 0; ps < nPass; ++ps, ++pc)
                     for (int kb = 0; kb < nKb; ++kb, ++it) {
                         const int s = it % FT_STAGES;
                         mbar_wait(empty + s, ((it / FT_STAGES) & 1) ^ 1);
                         unsigned char* st = sm + s * FT_STAGE_BYTES;
-                        mbar_arrive_expect_tx(full + s, FT_A_BYTES + 2 * FT_B_BYTES);
+                        // rows of H this K block adds to the ring (all 256 + nothing at the start of a pass: 8 boxes of 32 rows)
+                        unsigned char* ring = sm + FT_RINGS_OFF + (pc & 1) * 2 * FT_RING_BYTES;
+                        const int nbox = kb == 0 ? FT_N / FT_K : 1;
+                        mbar_arrive_expect_tx(full + s, FT_A_BYTES + 2 * nbox * FT_K * 128);
                         tma_load_2d(st, &mapA, kb * FT_K, tile * FT_M, full + s);
-                        tma_load_2d(st + 2 * FT_A_BYTES, &mapBh, kb * FT_K, ps * FT_N, full + s);
-                        tma_load_2d(st + 2 * FT_A_BYTES + FT_B_BYTES, &mapBl, kb * FT_K, ps * FT_N, full + s);
+                        for (int bx = 0; bx < nbox; ++bx) {
+                            const int slot = kb == 0 ? bx * FT_K : (FT_RING_ROWS - (FT_K * kb) % FT_RING_ROWS) % FT_RING_ROWS;   // ring row
+                            const int j = ps * FT_N + FT_K * (nKb - kb) + bx * FT_K;                                                // row of H
+                            tma_load_2d(ring + slot * 128, &mapBh, 0, j, full + s);
+                            tma_load_2d(ring + FT_RING_BYTES + slot * 128, &mapBl, 0, j, full + s);
+                        }
                     }
         }
     } else if (warp == 5) {
@@ -150,13 +170,25 @@ fdk_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ 
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                         const uint32_t a0 = smem_u32(sm + s * FT_STAGE_BYTES);
                         const uint64_t dAh = umma_desc_k128(a0), dAl = umma_desc_k128(a0 + FT_A_BYTES);
-                        const uint64_t dBh = umma_desc_k128(a0 + 2 * FT_A_BYTES), dBl = umma_desc_k128(a0 + 2 * FT_A_BYTES + FT_B_BYTES);
+                        // the window of this K block starts at ring row P and wraps: columns [0, N1) from rows [P, 288), the rest from row 0
+                        const uint32_t ring = smem_u32(sm + FT_RINGS_OFF + (pc & 1) * 2 * FT_RING_BYTES);
+                        const int P = (FT_RING_ROWS - (FT_K * kb) % FT_RING_ROWS) % FT_RING_ROWS;
+                        const int N1 = min(FT_N, FT_RING_ROWS - P), N2 = FT_N - N1;
+                        const uint64_t dBh1 = umma_desc_k128(ring + P * 128), dBl1 = umma_desc_k128(ring + FT_RING_BYTES + P * 128);
+                        const uint64_t dBh2 = umma_desc_k128(ring), dBl2 = umma_desc_k128(ring + FT_RING_BYTES);
+                        const uint32_t id1 = ft_idesc(N1), id2 = ft_idesc(N2);
 #pragma unroll
                         for (int kk = 0; kk < FT_K / 8; ++kk) {   // K step of 8 tf32 = 32 bytes inside the swizzle row: +2 in 16-byte units
                             const uint64_t o = (uint64_t)(kk * 2);
-                            umma_tf32(tmem, dAh + o, dBh + o, (kb | kk) != 0);
-                            umma_tf32(tmem, dAh + o, dBl + o, 1);
-                            umma_tf32(tmem, dAl + o, dBh + o, 1);
+                            const uint32_t acc = (kb | kk) != 0;
+                            umma_tf32(tmem, dAh + o, dBh1 + o, id1, acc);
+                            umma_tf32(tmem, dAh + o, dBl1 + o, id1, 1);
+                            umma_tf32(tmem, dAl + o, dBh1 + o, id1, 1);
+                            if (N2 > 0) {
+                                umma_tf32(tmem + (uint32_t)N1, dAh + o, dBh2 + o, id2, acc);
+                                umma_tf32(tmem + (uint32_t)N1, dAh + o, dBl2 + o, id2, 1);
+                                umma_tf32(tmem + (uint32_t)N1, dAl + o, dBh2 + o, id2, 1);
+                            }
                         }
                         umma_commit(empty + s);            // the stage is free once these have read it
                     }
@@ -274,8 +306,10 @@ int launch_fdk_filter_tc(const float* b, const Grid& g, const std::vector<double
     const int nTiles = (int)((mTotal + FT_M - 1) / FT_M);
     TempBuf taps, thi, tlo, rows;
     TG_TRY(upload(taps, h_taps.data(), sizeof(float) * nu, st));
-    TG_TRY(thi.alloc(sizeof(float) * (size_t)nu * nu, st));
-    TG_TRY(tlo.alloc(sizeof(float) * (size_t)nu * nu, st));
+    const int nPass = (nu + FT_N - 1) / FT_N, nKb = (nu + FT_K - 1) / FT_K;
+    const int rowsH = FT_K * nKb + FT_N * nPass;   // rows of H any (pass, K block) can ask for
+    TG_TRY(thi.alloc(sizeof(float) * (size_t)rowsH * FT_K, st));
+    TG_TRY(tlo.alloc(sizeof(float) * (size_t)rowsH * FT_K, st));
     std::vector<FtRow> hr(nViews);
     for (int a = 0; a < nViews; ++a) {
         hr[a].dsd = (float)dsd[a];
@@ -284,10 +318,10 @@ int launch_fdk_filter_tc(const float* b, const Grid& g, const std::vector<double
     }
     TG_TRY(upload(rows, hr.data(), sizeof(FtRow) * nViews, st));
     ProfScope ps(PK_EW, st, 2);
-    ft_toeplitz_kernel<<<sms * 4, 256, 0, st>>>(taps.as<float>(), nu, thi.as<float>(), tlo.as<float>());
+    ft_toeplitz_kernel<<<std::min(sms * 4, (rowsH * FT_K + 255) / 256), 256, 0, st>>>(taps.as<float>(), nu, rowsH, FT_K * nKb, thi.as<float>(), tlo.as<float>());
     CUtensorMap mA, mBh, mBl;
-    if (!encode_2d_sw128(&mA, b, (uint64_t)nu, (uint64_t)mTotal, FT_M) || !encode_2d_sw128(&mBh, thi.p, (uint64_t)nu, (uint64_t)nu, FT_N) ||
-        !encode_2d_sw128(&mBl, tlo.p, (uint64_t)nu, (uint64_t)nu, FT_N))
+    if (!encode_2d_sw128(&mA, b, (uint64_t)nu, (uint64_t)mTotal, FT_M) || !encode_2d_sw128(&mBh, thi.p, (uint64_t)FT_K, (uint64_t)rowsH, FT_K) ||
+        !encode_2d_sw128(&mBl, tlo.p, (uint64_t)FT_K, (uint64_t)rowsH, FT_K))
         return 1;
     TG_CUDA(cudaFuncSetAttribute(fdk_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM));
     fdk_tc_kernel<<<std::min(sms, nTiles), FT_THREADS, FT_SMEM, st>>>(mA, mBh, mBl, rows.as<FtRow>(), d_colw, q, nu, nv, mTotal, (float)g.du,
