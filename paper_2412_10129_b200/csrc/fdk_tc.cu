@@ -10,14 +10,15 @@
 //
 // One CTA per SM, persistent over tiles of 128 detector rows; per tile four passes of 256 output columns; per pass a ring of
 // K blocks of 32 (one 128-byte swizzle row of tf32):
-//   warp 4 (one lane)   TMA producer: A = 128 raw detector rows x 32 columns, B_hi / B_lo = 256 x 32 tiles of the Toeplitz
-//                       matrix (precomputed once per call in global memory, L2-resident), 128-byte swizzled, into a 2-stage ring
-//   warps 0-3           transform: a thread owns one row of the A tile; it multiplies the raw values by the cosine pre-weight
-//                       (and the Parker / Wang column weight), rounds to a_hi in place and writes a_lo beside it (the swizzle
-//                       only permutes 16-byte chunks inside the thread's own 128-byte row), then fences the async proxy
-//   warp 5 (one lane)   issues the 12 tcgen05.mma of the K block (4 K steps of 8 x 3 products, M 128 x N 256), commits the
-//                       stage back to the producer and, after the last K block, the accumulator to the epilogue
-//   warps 0-3 again     epilogue: tcgen05.ld of the thread's accumulator row, times 1/tau of its view, stored to q
+//   warp 8 (one lane)   TMA producer: A = 128 raw detector rows x 32 columns into a 4-stage ring, and the 32 new rows of the
+//                       Toeplitz operand's row ring (see FT_RING_ROWS), 128-byte swizzled
+//   warps 0-7           transform: two threads per row of the A tile; they multiply the raw values by the cosine pre-weight
+//                       (and the Parker / Wang column weight), round to a_hi in place and write a_lo beside it (the swizzle
+//                       only permutes 16-byte chunks inside the row's own 128 bytes), then fence the async proxy
+//   warp 9 (one lane)   issues the tcgen05.mma of the K block (4 K steps of 8 x 3 products, M 128 x N 256 in two column
+//                       segments around the ring's wrap), commits the stage back to the producer and, after the last K
+//                       block, the accumulator to the epilogue
+//   warps 0-7 again     epilogue: tcgen05.ld of the thread's half of its accumulator row, times 1/tau of its view, stored to q
 // Detector widths that are not a multiple of 4 (TMA row pitch) and drivers without the tensor-map encoder keep fdk.cu's kernel.
 #include <cuda.h>
 #include <algorithm>
@@ -30,7 +31,8 @@ namespace tg {
 
 namespace {
 
-constexpr int FT_M = 128, FT_N = 256, FT_K = 32, FT_STAGES = 2;
+constexpr int FT_M = 128, FT_N = 256, FT_K = 32, FT_STAGES = 4;
+constexpr int FT_TW = 8;   // transform / epilogue warps: two threads per row of the A tile (warp w: rows 32 (w & 3).., column half w >> 2)
 constexpr int FT_A_BYTES = FT_M * FT_K * 4;                          // 16 KB
 constexpr int FT_B_BYTES = FT_N * FT_K * 4;                          // 32 KB
 constexpr int FT_STAGE_BYTES = 2 * FT_A_BYTES;                       // A (-> a_hi), a_lo = 32 KB per stage
@@ -38,13 +40,15 @@ constexpr int FT_STAGE_BYTES = 2 * FT_A_BYTES;                       // A (-> a_
 // H[m][k] = g[|m - k|]: the 256 x 32 tiles of consecutive K blocks are the SAME rows of H shifted by 32, so a K block brings 32 new
 // rows (2 x 4 KB) instead of a whole tile (2 x 32 KB).  288 = 256 + 32 rows: the new rows of K block kb take the slots that left the
 // window after K block kb - 2, the very tensor-core reads whose completion frees A's stage; the window wraps around the ring, so the
-// N = 256 product is issued as two tcgen05.mma (N1 and 256 - N1 columns of the accumulator).  Two rings alternate between passes.
-constexpr int FT_RING_ROWS = FT_N + FT_K;                            // 288 rows of 128 bytes = 36 swizzle atoms
-constexpr int FT_RING_BYTES = FT_RING_ROWS * 128;                    // 36 KB
-constexpr int FT_RINGS_OFF = FT_STAGES * FT_STAGE_BYTES;             // [A stages][ring 0: hi, lo][ring 1: hi, lo]
-constexpr int FT_BAR_OFF = FT_RINGS_OFF + 4 * FT_RING_BYTES;
+// N = 256 product is issued as two tcgen05.mma (N1 and 256 - N1 columns of the accumulator).  With S stages of A in flight the
+// producer runs up to S K blocks ahead of the tensor core, so the ring holds 256 + 32 (S - 1) rows; at the start of a pass the
+// whole window is reloaded, after the previous pass's products have finished (one pipeline drain per 32 K blocks).
+constexpr int FT_RING_ROWS = FT_N + FT_K * (FT_STAGES - 1);          // 352 rows of 128 bytes = 44 swizzle atoms
+constexpr int FT_RING_BYTES = FT_RING_ROWS * 128;                    // 44 KB
+constexpr int FT_RINGS_OFF = FT_STAGES * FT_STAGE_BYTES;             // [A stages][ring: hi, lo]
+constexpr int FT_BAR_OFF = FT_RINGS_OFF + 2 * FT_RING_BYTES;
 constexpr int FT_SMEM = FT_BAR_OFF + 1024 /* alignment */ + 256 /* barriers, tmem slot */;
-constexpr int FT_THREADS = 192;
+constexpr int FT_THREADS = 32 * (FT_TW + 2);   // + the TMA warp and the MMA warp
 
 __device__ __forceinline__ float rn_tf32(float x) {
     uint32_t r;
@@ -115,14 +119,14 @@ fdk_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ 
     if (threadIdx.x == 0) {
         for (int s = 0; s < FT_STAGES; ++s) {
             mbar_init(full + s, 1);
-            mbar_init(ready + s, 128);
+            mbar_init(ready + s, 32 * FT_TW);
             mbar_init(empty + s, 1);
         }
         mbar_init(accfull, 1);
-        mbar_init(accempty, 128);
+        mbar_init(accempty, 32 * FT_TW);
         mbar_fence_init();
     }
-    if (warp == 4) {   // one warp allocates (and later frees) the accumulator's 256 columns of tensor memory
+    if (warp == FT_TW) {   // one warp allocates (and later frees) the accumulator's 256 columns of tensor memory
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(FT_N) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
@@ -133,7 +137,7 @@ fdk_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ 
 
     const int nPass = (nu + FT_N - 1) / FT_N, nKb = (nu + FT_K - 1) / FT_K;
 
-    if (warp == 4) {
+    if (warp == FT_TW) {
         // ------------------------------------------------------------ TMA producer
         if (lane == 0) {
             uint32_t it = 0, pc = 0;
@@ -144,8 +148,9 @@ fdk_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ 
                         mbar_wait(empty + s, ((it / FT_STAGES) & 1) ^ 1);
                         unsigned char* st = sm + s * FT_STAGE_BYTES;
                         // rows of H this K block adds to the ring (all 256 + nothing at the start of a pass: 8 boxes of 32 rows)
-                        unsigned char* ring = sm + FT_RINGS_OFF + (pc & 1) * 2 * FT_RING_BYTES;
+                        unsigned char* ring = sm + FT_RINGS_OFF;
                         const int nbox = kb == 0 ? FT_N / FT_K : 1;
+                        if (kb == 0 && pc > 0) mbar_wait(accfull, (pc - 1) & 1);   // the previous pass's products no longer read the ring
                         mbar_arrive_expect_tx(full + s, FT_A_BYTES + 2 * nbox * FT_K * 128);
                         tma_load_2d(st, &mapA, kb * FT_K, tile * FT_M, full + s);
                         for (int bx = 0; bx < nbox; ++bx) {
@@ -156,7 +161,7 @@ fdk_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ 
                         }
                     }
         }
-    } else if (warp == 5) {
+    } else if (warp == FT_TW + 1) {
         // ------------------------------------------------------------ MMA issuer
         if (lane == 0) {
             uint32_t it = 0, pc = 0;
@@ -171,7 +176,7 @@ fdk_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ 
                         const uint32_t a0 = smem_u32(sm + s * FT_STAGE_BYTES);
                         const uint64_t dAh = umma_desc_k128(a0), dAl = umma_desc_k128(a0 + FT_A_BYTES);
                         // the window of this K block starts at ring row P and wraps: columns [0, N1) from rows [P, 288), the rest from row 0
-                        const uint32_t ring = smem_u32(sm + FT_RINGS_OFF + (pc & 1) * 2 * FT_RING_BYTES);
+                        const uint32_t ring = smem_u32(sm + FT_RINGS_OFF);
                         const int P = (FT_RING_ROWS - (FT_K * kb) % FT_RING_ROWS) % FT_RING_ROWS;
                         const int N1 = min(FT_N, FT_RING_ROWS - P), N2 = FT_N - N1;
                         const uint64_t dBh1 = umma_desc_k128(ring + P * 128), dBl1 = umma_desc_k128(ring + FT_RING_BYTES + P * 128);
@@ -196,8 +201,9 @@ fdk_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ 
                 }
         }
     } else {
-        // ------------------------------------------------------------ transform + epilogue (warps 0-3: thread t <-> row t of the tile)
-        const int t = threadIdx.x;
+        // ------------------------------------------------------------ transform + epilogue (8 warps: two threads per row of the tile,
+        // each half of its chunks and, in the epilogue, half of its columns)
+        const int t = threadIdx.x & 127, half = threadIdx.x >> 7;
         uint32_t it = 0, pc = 0;
         for (int tile = blockIdx.x; tile < nTiles; tile += gridDim.x) {
             const long long gr = (long long)tile * FT_M + t;     // global detector row (view * nv + iv)
@@ -214,7 +220,8 @@ fdk_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ 
                     mbar_wait(full + s, (it / FT_STAGES) & 1);
                     unsigned char* rowA = sm + s * FT_STAGE_BYTES + t * 128;
 #pragma unroll
-                    for (int c = 0; c < 8; ++c) {
+                    for (int cc = 0; cc < 4; ++cc) {
+                        const int c = 4 * half + cc;
                         const int p = (c + t) & 7;                 // physical 16-byte chunk (rotated per lane: no bank conflicts)
                         const int k = kb * FT_K + 4 * (p ^ (t & 7));   // logical column of its first element (128-byte swizzle)
                         float4 a = *reinterpret_cast<float4*>(rowA + p * 16);
@@ -238,10 +245,10 @@ fdk_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ 
                 // ---- epilogue of this pass
                 mbar_wait(accfull, pc & 1);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const uint32_t trow = tmem + ((uint32_t)(warp * 32) << 16);
+                const uint32_t trow = tmem + ((uint32_t)((warp & 3) * 32) << 16);
                 float* qrow = q + (size_t)(rowok ? gr : 0) * nu + (size_t)ps * FT_N;
 #pragma unroll 1
-                for (int c0 = 0; c0 < FT_N; c0 += 32) {
+                for (int c0 = half * (FT_N / 2); c0 < (half + 1) * (FT_N / 2); c0 += 32) {
                     uint32_t r[32];
                     asm volatile(
                         "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, "
@@ -271,7 +278,7 @@ fdk_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ 
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     __syncwarp();
-    if (warp == 4) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(FT_N) : "memory");
+    if (warp == FT_TW) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(FT_N) : "memory");
 }
 
 bool encode_2d_sw128(CUtensorMap* map, const void* base, uint64_t cols, uint64_t rowsN, uint32_t boxRows) {
