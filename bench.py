@@ -507,6 +507,61 @@ def run_probe(tg, geo, ang, rec, subsets):
     plan.close()
 
 
+def run_kernel(args, tg, geo, ang, rec, rank):
+    """One kernel of the library on one config, timed alone with CUDA events (best of 3 after a warm-up) on seeded random data:
+    the command the per-kernel ncu captures under profiles/ profile, and the A/B switch of the kernel-path hooks.
+      --kernel ax:siddon | ax:interp | atb:matched | atb:fdk | atb:exact_siddon | atb:exact_interp | fdk_filter[:hann]
+      --views N (a subset of N views, evenly spaced)   --ax-path / --fdk-path / --index-path (the library's test hooks)"""
+    import torch
+    if args.views:
+        sel = np.arange(0, len(ang), max(1, len(ang) // args.views))[:args.views]
+        ang = ang[sel]
+        if geo.rotDetector_a is not None:
+            geo.rotDetector_a = geo.rotDetector_a[sel]
+    tg.set_ax_path(args.ax_path)
+    tg.set_fdk_path(args.fdk_path)
+    tg.set_index_path(args.index_path)
+    kind, _, mode = args.kernel.partition(":")
+    gen = torch.Generator(device="cuda").manual_seed(rec["seed"])
+
+    def timed(f, reps=3):
+        f()
+        best = 1e30
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            f()
+            e1.record()
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        return best
+
+    nA = len(ang)
+    if kind == "ax":
+        vol = torch.rand(geo.vol_shape, generator=gen, device="cuda") * 0.02
+        units, unit = tg.Ax_count(geo, ang, mode), "Gsamples/s"
+        ms = timed(lambda: tg.Ax(vol, geo, ang, mode))
+    elif kind == "atb":
+        b = torch.rand((nA,) + tuple(geo.proj_shape), generator=gen, device="cuda")
+        if mode.startswith("exact_"):
+            units, unit = tg.Ax_count(geo, ang, mode[6:]), "Gsamples/s"
+        else:
+            units, unit = int(np.prod(geo.nVoxel)) * nA, "Gupdates/s"
+        ms = timed(lambda: tg.Atb(b, geo, ang, mode))
+    elif kind == "fdk_filter":
+        b = torch.rand((nA,) + tuple(geo.proj_shape), generator=gen, device="cuda")
+        units, unit = 3.0 * 2.0 * nA * geo.nDetector[1] * float(geo.nDetector[0]) ** 2 / 1e3, "TFLOP/s (tf32-equivalent: 6 per multiply-add of the row convolution)"
+        ms = timed((lambda: tg.fdk_filter_ex(b, geo, ang, mode)) if mode else (lambda: tg.fdk_filter(b, geo, ang)))
+    else:
+        raise SystemExit("unknown --kernel " + args.kernel)
+    if rank == 0:
+        print(json.dumps({"metric": "one kernel, timed alone", "kernel": args.kernel, "ms": ms, "value": units / (ms * 1e-3) / 1e9, "unit": unit,
+                          "n_gpus": 1, "dtype": "f32", "data": "synthetic (seeded uniform random)",
+                          "config": {"workload": f"{rec['name']}: {geo.nVoxel[0]}^3, {nA} views of {geo.nDetector[0]}x{geo.nDetector[1]}",
+                                     "ax_path": args.ax_path, "fdk_path": args.fdk_path, "index_path": args.index_path}}))
+
+
 def kernel_rates_other_configs(tg, rates):
     """SURVEY.md section 8(d) "per kernel, per config C2-C5": the two projector kernels of C2 (full size) and C4 (full-size volume and
     detector, 64 of its 1600 views: a launch of the size its CGLS makes per subset-free pass would take 9 s) timed with CUDA events
@@ -581,8 +636,13 @@ def main():
     ap.add_argument("--tv-delta", type=float, default=0.0, help="tv mode: AwTV delta (0 = plain TV)")
     ap.add_argument("--tv-op", default="minimise", choices=["minimise", "prox"],
                     help="tv mode: the gradient-descent minimiser (tigre_minimize_awtv) or the TV proximal operator of FISTA (tigre_tv_prox)")
-    ap.add_argument("--mode", default="plan", choices=["plan", "chunked", "tv", "drivers", "peaks", "probe"],
+    ap.add_argument("--mode", default="plan", choices=["plan", "chunked", "tv", "drivers", "peaks", "probe", "kernel"],
                     help="plan: OS-SART iteration in HBM (default); chunked: Ax + A^T b with all arrays in pinned host memory (S8)")
+    ap.add_argument("--kernel", default="ax:siddon", help="kernel mode: ax:siddon | ax:interp | atb:matched | atb:fdk | atb:exact_siddon | atb:exact_interp | fdk_filter[:window]")
+    ap.add_argument("--views", type=int, default=0, help="kernel mode: use N evenly spaced views of the config (0 = all)")
+    ap.add_argument("--ax-path", type=int, default=0, help="kernel mode: tigre_set_ax_path (0 default, 1 L1 kernel, 2 TMA kernel also for wide beams)")
+    ap.add_argument("--fdk-path", type=int, default=0, help="kernel mode: tigre_set_fdk_path (0 tensor cores, 1 CUDA cores)")
+    ap.add_argument("--index-path", type=int, default=0, help="kernel mode: tigre_set_index_path (1 = 64-bit element offsets)")
     ap.add_argument("--drivers", default="", help="drivers mode: comma-separated subset of the drivers to time (default: all)")
     ap.add_argument("--budget-gb", type=float, default=0.0, help="chunked mode: device bytes the chunked path may use (0 = 3/4 of free)")
     ap.add_argument("--chunk-n", type=int, default=0, help="chunked mode: C5-shaped problem with an n^3 volume and an n x n detector (0: --config as given)")
@@ -646,6 +706,9 @@ def main():
 
     if args.mode == "probe":
         run_probe(tg, geo, ang, rec, subsets)
+        return
+    if args.mode == "kernel":
+        run_kernel(args, tg, geo, ang, rec, rank)
         return
     if args.mode == "peaks":
         run_peaks(tg, rank)
