@@ -39,6 +39,8 @@ struct SidRay {
     // non-zero length, and the number of such voxels
     long long first, last;
     uint32_t nseg;
+    bool pok;      // SCATTER only: lane ^ 1 is in fm and scatters into the same array
+    unsigned fm;   // SCATTER only: the lanes of the warp that run the warp-uniform groups of the interior together
     __device__ __forceinline__ void note(IdxT o, float len) {
         if (len > 0.f) {
             if (nseg == 0) first = (long long)o;
@@ -48,9 +50,30 @@ struct SidRay {
     }
 };
 
+// Exact-adjoint scatter inside the warp-uniform groups: the lanes named in fm execute this together and are in the same slab.
+// Neighbouring rays are less than a voxel apart on most geometries, so lanes 2j and 2j + 1 often add to the SAME voxel; then the
+// even lane adds both values in one REDG (the L1 -> L2 reduction path, not the issue slots, is what binds the scatter kernels:
+// profiles/r2_scatter.md).  Any pairing is correct; runs that straddle a pair boundary just stay two operations.  pok: the
+// partner lane runs the groups too AND adds into the same array (vol or its transposed copy) -- equal offsets then mean one voxel.
+// (Merging runs of up to three lanes at any alignment -- 3 shuffles, a vote and a CLZ per REDG -- was measured slower than no
+// merging at all: 582 against 700 G samples/s on C3; this two-shuffle pairing gives 785.)
+#ifndef AX_NO_PAIR
+template <typename IdxT>
+__device__ __forceinline__ void red_pair(float* out, IdxT off, float v, unsigned fm, bool pok) {
+    const IdxT o2 = __shfl_xor_sync(fm, off, 1);
+    const float v2 = __shfl_xor_sync(fm, v, 1);
+    const bool same = pok && o2 == off;
+    if (same && (threadIdx.x & 1u)) return;   // blockDim.x == 32: threadIdx.x is the lane
+    red_add_global(out + off, same ? v + v2 : v);
+}
+#else
+template <typename IdxT>
+__device__ __forceinline__ void red_pair(float* out, IdxT off, float v, unsigned, bool) { red_add_global(out + off, v); }
+#endif
+
 // One D-slab, interior of the volume: the whole slab [0,1] lies inside the ray's clipped range and at
 // least 1e-3 voxel away from the lateral faces, so no clipping and no bounds checks are needed.
-template <typename IdxT, bool UNIT, bool SCATTER, bool TRACK = false>
+template <typename IdxT, bool UNIT, bool SCATTER, bool TRACK = false, bool PAIR = false>
 __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base, SidRay<IdxT>& r) {
     // slab-local parameter of the next E / F plane crossing, saturated to [0,1] (1 = not in this slab)
     const float se = __saturatef(fmaf(r.hE, r.imE, -r.kf)), sf = __saturatef(fmaf(r.hF, r.imF, -r.kf));
@@ -69,9 +92,11 @@ __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base,
     } else if (SCATTER) {
         // exact adjoint: the same three lengths, added to the voxels instead of gathered from them
         float* out = const_cast<float*>(base);
-        red_add_global(out + r.off, s1 * r.ys);
+        if (PAIR) red_pair(out, r.off, s1 * r.ys, r.fm, r.pok);
+        else red_add_global(out + r.off, s1 * r.ys);
         if (both) red_add_global(out + (r.off + ((se < sf) ? r.stE : r.stF)), (s2 - s1) * r.ys);
-        red_add_global(out + offC, (1.0f - s2) * r.ys);
+        if (PAIR) red_pair(out, offC, (1.0f - s2) * r.ys, r.fm, r.pok);
+        else red_add_global(out + offC, (1.0f - s2) * r.ys);
     } else {
         const float vA = UNIT ? 1.f : __ldg(base + r.off);
         float vC = vA;   // a lane that stays in its voxel does not load it twice
@@ -89,7 +114,7 @@ __device__ __forceinline__ void siddon_slab_fast(const float* __restrict__ base,
 
 // One interior D-slab of a ray that is known not to cross an F-plane in it (sf = 1 in siddon_slab_fast): the same two
 // lengths and the same operations on them as there, without the middle voxel and the F bookkeeping (bitwise the same sum).
-template <typename IdxT, bool UNIT, bool SCATTER, bool TRACK = false>
+template <typename IdxT, bool UNIT, bool SCATTER, bool TRACK = false, bool PAIR = false>
 __device__ __forceinline__ void siddon_slab_e_only(const float* __restrict__ base, SidRay<IdxT>& r) {
     const float se = __saturatef(fmaf(r.hE, r.imE, -r.kf));
     r.kf += 1.0f;
@@ -100,8 +125,8 @@ __device__ __forceinline__ void siddon_slab_e_only(const float* __restrict__ bas
         r.note(offC, 1.0f - se);
     } else if (SCATTER) {
         float* out = const_cast<float*>(base);
-        red_add_global(out + r.off, se * r.ys);
-        red_add_global(out + offC, (1.0f - se) * r.ys);
+        if (PAIR) red_pair(out, r.off, se * r.ys, r.fm, r.pok), red_pair(out, offC, (1.0f - se) * r.ys, r.fm, r.pok);
+        else red_add_global(out + r.off, se * r.ys), red_add_global(out + offC, (1.0f - se) * r.ys);
     } else {
         const float vA = UNIT ? 1.f : __ldg(base + r.off);
         float vC = vA;   // a lane that stays in its voxel does not load it twice (the L1 data pipe is co-critical)
@@ -191,7 +216,7 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
     SidRay<IdxT> r;
     r.imE = r.imF = 1.f, r.sgE = r.sgF = 1.f, r.hE = r.hF = 3.0e38f, r.stE = r.stF = r.sD = 0;
     r.kf = 0.f, r.acc = 0.f, r.vB = 0.f, r.ys = 0.f, r.off = 0;
-    r.first = r.last = -1, r.nseg = 0;
+    r.first = r.last = -1, r.nseg = 0, r.fm = 0, r.pok = false;
     const float* base = vol;
     int i0 = 0, nslab = 0, kA = 0, kB = 0, ie = 0, jf = 0, ie0 = 0, jf0 = 0, diE = 1, diF = 1;
     float slo0 = 0.f, shiN = 1.f, scale = 0.f;
@@ -303,6 +328,11 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
         // slab jmax here.
         const int jendmin = __reduce_min_sync(wmask, ranFast ? i0 + kB : 0x7fffffff);
         const int groups = jendmin == 0x7fffffff ? 0 : (jendmin - jmax) / AXG;
+        if (SCATTER) {
+            r.fm = __ballot_sync(wmask, ranFast);
+            const unsigned tm = __ballot_sync(wmask, base == volT), q = threadIdx.x ^ 1u;
+            r.pok = ((r.fm >> q) & 1u) && ((tm >> q) & 1u) == ((tm >> threadIdx.x) & 1u);
+        }
         for (int g = 0; g < groups; ++g) {
 #ifdef AX_PREFETCH
             if (!UNIT && !SCATTER && !TRACK && ranFast) {
@@ -317,11 +347,11 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
             if (__any_sync(wmask, nearF)) {
                 if (ranFast) {
 #pragma unroll
-                    for (int j = 0; j < AXG; ++j) siddon_slab_fast<IdxT, UNIT, SCATTER, TRACK>(base, r);
+                    for (int j = 0; j < AXG; ++j) siddon_slab_fast<IdxT, UNIT, SCATTER, TRACK, SCATTER>(base, r);
                 }
             } else if (ranFast) {
 #pragma unroll
-                for (int j = 0; j < AXG; ++j) siddon_slab_e_only<IdxT, UNIT, SCATTER, TRACK>(base, r);
+                for (int j = 0; j < AXG; ++j) siddon_slab_e_only<IdxT, UNIT, SCATTER, TRACK, SCATTER>(base, r);
             }
         }
         if (ranFast) k += AXG * groups;

@@ -94,3 +94,20 @@ def test_cgls_with_exact_adjoint(tg):
     with pytest.raises(tg.TigreError) as e:                   # the transpose must be that of the Ax in use
         tg.cgls(dev(b), geo, ang, 1, "siddon", "exact_interp")
     assert e.value.code == -1
+
+
+def test_exact_siddon_scatter_across_the_dominance_boundary(tg):
+    """Lanes of one warp on both sides of |dx| = |dy| scatter into different arrays (the volume and its (x,y)-transposed
+    copy), where EQUAL offsets are different voxels (on the diagonal x = y they coincide numerically): the pairwise merge
+    of the scatter must not join such lanes.  Views at and around 45 degrees, the boundary moved pixel by pixel over the
+    detector row so that it falls inside an (even, odd) lane pair as well as between pairs."""
+    for offu in (0.0, 1.0, 2.0, 0.5):
+        geo = Geometry(nVoxel=(64, 64, 40), dVoxel=(1.0, 1.0, 1.0), nDetector=(96, 48), dDetector=(1.0, 1.0),
+                       DSD=500.0, DSO=300.0, offDetector=(offu, 0.0))
+        ang = np.zeros((5, 3))
+        ang[:, 0] = [np.pi / 4, np.pi / 4 + 1e-3, 3 * np.pi / 4 - 2e-3, 5 * np.pi / 4, 7 * np.pi / 4 + 5e-4]
+        y = np.random.default_rng(7).random((len(ang),) + geo.proj_shape, dtype=np.float32)
+        ref = orc.atb_exact(y, geo, ang, orc.SIDDON)
+        got = host(tg.Atb(dev(y), geo, ang, "exact_siddon"))
+        assert H.rel_l2(got, ref) <= 1e-5
+        assert np.abs(got - ref).max() <= 1e-4 * np.abs(ref).max()
