@@ -1,4 +1,7 @@
-"""Build libtigre_b200.so in-tree with nvcc for sm_100a (run: python -m paper_2412_10129_b200.build)."""
+"""Build libtigre_b200.so in-tree with nvcc for sm_100a (run: python -m paper_2412_10129_b200.build).
+
+TIGRE_NVCC_EXTRA="-DAXTU=64 -DAXTV=2" python -m paper_2412_10129_b200.build --force   builds a tuning variant (the macros are
+listed at the top of csrc/ax_common.cuh, csrc/ax_tma.cu, csrc/fdk_tc.cu); profiles/ names such builds by this command line."""
 import os
 import subprocess
 import sys
@@ -32,7 +35,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
     for src in _sources():
         obj = os.path.join(HERE, "build", os.path.basename(src) + ".o")
-        cmd = ["nvcc", "-c", src, "-o", obj] + FLAGS + (["-Xptxas", "-v"] if verbose else [])
+        cmd = ["nvcc", "-c", src, "-o", obj] + FLAGS + os.environ.get("TIGRE_NVCC_EXTRA", "").split() + (["-Xptxas", "-v"] if verbose else [])
         procs.append((cmd, subprocess.Popen(cmd)))
         objs.append(obj)
     for cmd, p in procs:

@@ -63,7 +63,7 @@ __device__ __forceinline__ void red_pair(float* out, IdxT off, float v, unsigned
     const IdxT o2 = __shfl_xor_sync(fm, off, 1);
     const float v2 = __shfl_xor_sync(fm, v, 1);
     const bool same = pok && o2 == off;
-    if (same && (threadIdx.x & 1u)) return;   // blockDim.x == 32: threadIdx.x is the lane
+    if (same && (threadIdx.x & 1u)) return;   // blockDim.x is a multiple of 32: the parity of threadIdx.x is the lane's
     red_add_global(out + off, same ? v + v2 : v);
 }
 #else
@@ -330,8 +330,8 @@ ax_siddon_kernel(const float* __restrict__ vol, const float* __restrict__ volT, 
         const int groups = jendmin == 0x7fffffff ? 0 : (jendmin - jmax) / AXG;
         if (SCATTER) {
             r.fm = __ballot_sync(wmask, ranFast);
-            const unsigned tm = __ballot_sync(wmask, base == volT), q = threadIdx.x ^ 1u;
-            r.pok = ((r.fm >> q) & 1u) && ((tm >> q) & 1u) == ((tm >> threadIdx.x) & 1u);
+            const unsigned tm = __ballot_sync(wmask, base == volT), ln = threadIdx.x & 31u, q = ln ^ 1u;
+            r.pok = ((r.fm >> q) & 1u) && ((tm >> q) & 1u) == ((tm >> ln) & 1u);
         }
         for (int g = 0; g < groups; ++g) {
 #ifdef AX_PREFETCH

@@ -16,6 +16,9 @@ namespace tg {
 //   AXI_ROWS  rows of the volume per lockstep step of the interpolated kernel: 8; 2 / 3 / 4 / 6 / 12 / 16 / 32 give 318 / 323 / 342 / 342 /
 //          345 / 347 / 318 against 352 G samples/s on C2 (C3-sized: 405 / 411 / 443 / 452 / 465 / 464 / 455 against 459)
 //   AXTV   detector rows per CTA (tile = 32 x AXTV pixels): 4; 1, 2 and 8 lose 0.3-4 % (with the voted groups: 2 rows x 18 CTAs 1390, 8 rows x 4 / 5 CTAs 1331 / 1339 against 1397)
+//   AXTU   detector columns per CTA (a multiple of 32; one warp = 32 consecutive pixels of a row): 32 x 4 rows; 64 x 2 / 64 x 4 (4 CTAs) /
+//          128 x 1 / 64 x 1 (18 CTAs) give 1347 / 1288 / 1325 / 1328 against 1352 G samples/s (C3, one launch through tigre_Ax):
+//          sharing L1 lines between the two warps of a row does not pay (ax.cu only: ax_tma.cu wants 32)
 #ifndef AXIMB
 #define AXIMB 8
 #endif
@@ -40,7 +43,10 @@ struct AxP {
 #ifndef AXTV
 #define AXTV 4
 #endif
-constexpr int AX_TU = 32, AX_TV = AXTV;
+#ifndef AXTU
+#define AXTU 32
+#endif
+constexpr int AX_TU = AXTU, AX_TV = AXTV;   // AX_TU: a multiple of 32 (a warp is 32 consecutive pixels of one detector row)
 constexpr int AXI_ROWS = 8;
 
 // a[i] += v without a return value, on GLOBAL memory, said so explicitly: through a generic pointer (the scatter kernels pick
