@@ -178,9 +178,10 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
             // byte address (shared window) of the tap column in row 0 of the stage, minus the magic-number
             // bias of floor_magic times the row pitch (mod 2^32): the row address is then ONE integer
             // multiply-add of the raw bits of (fv - 1/2) + 1.5*2^23
-            const uint32_t col = tiles_s + (uint32_t)(s * stageElems + (iu + p.hu - c0) + (p.hv - c1) * BU) * 4u -
+            uint32_t col = tiles_s + (uint32_t)(s * stageElems + (iu + p.hu - c0) + (p.hv - c1) * BU) * 4u -
                            (uint32_t)p.magic * (uint32_t)(BU * 4);   // p.magic = 0x4B400000, opaque to the compiler
                                                                       // (as a literal it is re-added before every load)
+            asm volatile("" : "+r"(col));   // ... and so is the sum: nvcc factors it back into (bits - magic) * pitch, an IADD3 per update
 #pragma unroll
             for (int k = 0; k < ZR; ++k) {
                 const float fv = fmaf((float)k, dfv, fv0);
