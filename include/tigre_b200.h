@@ -73,7 +73,9 @@ typedef enum tigre_status {
     TIGRE_ERR_MEMSPACE = -3,  /* a data pointer is in the wrong memory space                   */
     TIGRE_ERR_WORKSPACE = -4, /* a temporary allocation failed                                 */
     TIGRE_ERR_CUDA = -5,      /* any other CUDA error (tigre_last_cuda_error() gives the text) */
-    TIGRE_ERR_NO_DEVICE = -6  /* no CUDA device: there is no CPU fallback                      */
+    TIGRE_ERR_NO_DEVICE = -6, /* no CUDA device: there is no CPU fallback                      */
+    TIGRE_ERR_TOO_LARGE = -7  /* a size exceeds the fixed scratch of a no-allocation entry     */
+                              /* point (tigre_residual_noalloc); nothing was launched          */
 } tigre_status;
 
 enum { TIGRE_AX_SIDDON = 0, TIGRE_AX_INTERP = 1 };
@@ -139,6 +141,23 @@ TIGRE_API int tigre_col_weights(const tigre_geo *geo, const double *angles, int 
  * All arrays dev, n elements.  Synchronises only when nrm2 != NULL. */
 TIGRE_API int tigre_residual(const float *b, const float *Ax, const float *W, float *r, size_t n, double *nrm2,
                    void *cuda_stream);
+/* tigre_residual for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): the same r = W .* (b - Ax) (bitwise) and ||b - Ax||_2^2 (eq. 2), but
+ *   - it calls no cudaMalloc / cudaFree / cudaMallocAsync or allocating library routine, creates no stream or event and never
+ *     synchronises: its scratch (one fp64 partial sum per CTA) is a file-scope 128 KiB array in device memory that every GPU
+ *     which loads the library holds until the process exits (csrc/noalloc.cu);
+ *   - that array bounds the size: n <= TIGRE_RESIDUAL_NOALLOC_MAX_N elements (2^28 = 1 GiB per array), else
+ *     TIGRE_ERR_TOO_LARGE and nothing is launched or written (split the call);
+ *   - nrm2_dev is a DEVICE pointer (may be NULL: then only r is formed), written in stream order; the sum is formed in a fixed
+ *     order, so it is bitwise reproducible (it agrees with tigre_residual's to fp64 rounding, not bitwise);
+ *   - all calls on a device share the scratch array, which keeps the last call's contents; nothing in it has to start at zero
+ *     (each call overwrites the slots it then reads).  Calls that OVERLAP on the GPU (different streams without an event
+ *     between them, graphs replayed concurrently) race on it: their nrm2 is undefined.  Calls on one stream are safe;
+ *   - the device that is current at the call is the one whose scratch is used (its address is looked up on the first call on
+ *     that device: make that first call outside graph capture); b, Ax, W (may be NULL), r: dev, n elements, r may alias Ax. */
+#define TIGRE_RESIDUAL_NOALLOC_MAX_N 268435456ull
+TIGRE_API int tigre_residual_noalloc(const float *b, const float *Ax, const float *W, float *r, size_t n, double *nrm2_dev,
+                           void *cuda_stream);
 /* x <- x + lambda * V .* g, then x <- max(x,0) if nonneg  (V may be NULL = ones).  dev, n elements */
 TIGRE_API int tigre_update(float *x, const float *g, const float *V, float lambda, int nonneg, size_t n,
                  void *cuda_stream);

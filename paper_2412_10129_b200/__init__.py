@@ -53,7 +53,7 @@ EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_Ax_slab", "tigre_Atb_slab", "tigre_sl
            "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_create_ex", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_osem", "tigre_plan_sart_tv", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version", "tigre_Ax_index", "tigre_set_index_path", "tigre_set_workspace", "tigre_plan_workspace_bytes",
-           "tigre_workspace_stats", "tigre_sirt_chunked", "tigre_microbench", "tigre_set_ax_path", "tigre_set_plan_v_path", "tigre_plan_ossart_subsets", "tigre_Atb_boxes", "tigre_set_fdk_path"]
+           "tigre_workspace_stats", "tigre_sirt_chunked", "tigre_microbench", "tigre_set_ax_path", "tigre_set_plan_v_path", "tigre_plan_ossart_subsets", "tigre_Atb_boxes", "tigre_set_fdk_path", "tigre_residual_noalloc"]
 
 
 def _lib():
@@ -275,6 +275,23 @@ def residual(b, ax, W=None, return_norm=False):
                                  _f32(r), C.c_size_t(b.numel()), C.byref(nrm) if return_norm else None, _stream(b)),
            "tigre_residual")
     return (r, nrm.value) if return_norm else r
+
+
+RESIDUAL_NOALLOC_MAX_N = 1 << 28   # TIGRE_RESIDUAL_NOALLOC_MAX_N
+
+
+def residual_noalloc(b, ax, r, W=None, nrm2=None):
+    """tigre_residual_noalloc: r <- W .* (b - ax), nrm2[0] <- ||b - ax||^2, with no allocation and no synchronisation inside the
+    library (scratch: a file-scope device array, so numel <= RESIDUAL_NOALLOC_MAX_N; calls that overlap on the GPU race on it).
+    The caller passes the outputs: r (float32, b's shape) and, optionally, nrm2 (a float64 device tensor of one element)."""
+    import torch
+    if nrm2 is not None and (not isinstance(nrm2, torch.Tensor) or nrm2.dtype != torch.float64 or not nrm2.is_cuda or nrm2.numel() != 1):
+        raise ValueError("nrm2: need a float64 device tensor of one element")
+    _check(_lib().tigre_residual_noalloc(_f32(b), _f32(ax, b.shape, "Ax"), _f32(W, b.shape, "W") if W is not None else None,
+                                         _f32(r, b.shape, "r"), C.c_size_t(b.numel()),
+                                         C.c_void_p(nrm2.data_ptr()) if nrm2 is not None else None, _stream(b)),
+           "tigre_residual_noalloc")
+    return r
 
 
 def update(x, g, V=None, lam=1.0, nonneg=True):

@@ -275,6 +275,7 @@ const char* tigre_strerror(int code) {
         case TIGRE_ERR_WORKSPACE: return "temporary device allocation failed";
         case TIGRE_ERR_CUDA: return "CUDA error (see tigre_last_cuda_error)";
         case TIGRE_ERR_NO_DEVICE: return "no CUDA device (libtigre_b200 has no CPU fallback)";
+        case TIGRE_ERR_TOO_LARGE: return "size exceeds the fixed scratch array of a no-allocation entry point (tigre_residual_noalloc: n > TIGRE_RESIDUAL_NOALLOC_MAX_N = 2^28 elements); nothing was launched";
     }
     return "unknown error";
 }
