@@ -370,6 +370,11 @@ TIGRE_API int tigre_set_atb_path(int path);
  * aligned volume, the beam of a 32 x 4 pixel tile fits a stage), 1 = always the L1 gather kernel, 2 = the TMA kernel for wide
  * beams too.  Same samples, same per-ray order of summation; A/B and test hook. */
 TIGRE_API int tigre_set_ax_path(int path);
+/* which Siddon tigre_Ax kernel runs: 0 (default) = the L1 gather kernel, 1 = the kernel that stages the interior of the march
+ * into shared memory by TMA (csrc/ax_siddon_tma.cu) where the problem qualifies (nx, ny multiples of 4, 16-byte aligned
+ * volume, whole detector, 32-bit offsets).  Bitwise the same projections; the staged kernel is the slower one on B200
+ * (profiles/r2_ax_siddon.md) and is kept for A/B measurement and its test. */
+TIGRE_API int tigre_set_siddon_path(int path);
 /* which FDK pre-filter kernel runs: 0 (default) = the Toeplitz GEMM on the tensor cores (tcgen05, 3 x tf32 split products into an fp32
  * accumulator in tensor memory) whenever nDetector_u is a multiple of 4 and input and output are distinct 16-byte aligned arrays,
  * 1 = always the CUDA-core convolution.  Same taps, same weights; A/B and test hook. */

@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtigre_b200.so")
-SOURCES = ["geometry.cu", "ax.cu", "ax_tma.cu", "atb.cu", "atb_tma.cu", "elementwise.cu", "tv.cu", "prox.cu", "fdk.cu", "fdk_tc.cu", "chunked.cu", "peaks.cu", "noalloc.cu", "api.cu"]
+SOURCES = ["geometry.cu", "ax.cu", "ax_tma.cu", "ax_siddon_tma.cu", "atb.cu", "atb_tma.cu", "elementwise.cu", "tv.cu", "prox.cu", "fdk.cu", "fdk_tc.cu", "chunked.cu", "peaks.cu", "noalloc.cu", "api.cu"]
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--fmad=true", "-cudart", "static"]
 

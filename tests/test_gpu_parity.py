@@ -383,6 +383,36 @@ def test_plan_pinned_host_path_equals_device_path(tg):
     plan.close(), plan2.close()
 
 
+# ------------------------------------------------------------------ the TMA-staged Siddon projector (ax_siddon_tma.cu)
+def test_siddon_ax_staged_kernel_is_bitwise_the_l1_kernel(tg):
+    """tigre_set_siddon_path(1): the interior of the march read from shared-memory boxes.  Same lengths, same order of
+    summation per ray: the projections are bitwise those of the default kernel (and so within 1e-5 of the oracle).  C3's
+    half-fan detector at 1/4 scale (windows on most tiles, all view angles incl. 45 degrees where the tile's rays change
+    their dominant axis), C4's tilted detectors, a volume wider than deep, and sizes that do not qualify."""
+    cases = []
+    geo, ang, rec = make_config("C3", scale=4, n_angles=24)
+    ang = np.array(ang, dtype=np.float64)
+    ang[:, 0] += 0.01   # (at 1/4 scale pixel column 115 sits at u = 0: at 90, 180, 270 degrees its rays would lie IN a voxel-face plane, reading P19's tie)
+    cases.append((geo, ang, phantom_for(rec, geo), True))
+    geo, ang, rec = make_config("C4", scale=8, n_angles=12)
+    cases.append((geo, ang, np.random.default_rng(7).random(geo.vol_shape, dtype=np.float32), True))
+    geo = Geometry(nVoxel=(160, 96, 40), dVoxel=(0.5, 0.5, 0.5), nDetector=(256, 96), dDetector=(0.4, 0.4), DSD=400.0, DSO=250.0,
+                   offDetector=(3.0, -1.1))
+    cases.append((geo, circular_angles(10, start=0.3), np.random.default_rng(8).random(geo.vol_shape, dtype=np.float32), True))
+    geo, ang = odd_geometry()
+    cases.append((geo, ang, np.random.default_rng(3).random(geo.vol_shape, dtype=np.float32), False))
+    for geo, ang, vol, check_oracle in cases:
+        base = host(tg.Ax(dev(vol), geo, ang, "siddon"))
+        tg.set_siddon_path(1)
+        try:
+            got = host(tg.Ax(dev(vol), geo, ang, "siddon"))
+        finally:
+            tg.set_siddon_path(0)
+        assert np.array_equal(got, base)
+        if check_oracle:
+            assert H.rel_l2(got, orc.ax(vol, geo, ang, orc.SIDDON)) <= 1e-5
+
+
 # ------------------------------------------------------------------ the TMA-staged interpolated projector (ax_tma.cu)
 @pytest.mark.parametrize("path", [0, 1, 2])
 def test_interp_ax_kernel_paths_agree_with_the_oracle(tg, path):
