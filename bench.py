@@ -511,7 +511,7 @@ def run_kernel(args, tg, geo, ang, rec, rank):
     """One kernel of the library on one config, timed alone with CUDA events (best of 3 after a warm-up) on seeded random data:
     the command the per-kernel ncu captures under profiles/ profile, and the A/B switch of the kernel-path hooks.
       --kernel ax:siddon | ax:interp | atb:matched | atb:fdk | atb:exact_siddon | atb:exact_interp | fdk_filter[:hann]
-      --views N (a subset of N views, evenly spaced)   --ax-path / --siddon-path / --fdk-path / --index-path (the library's test hooks)"""
+      --views N (a subset of N views, evenly spaced)   --ax-path / --siddon-path / --atb-path / --fdk-path / --index-path (the library's test hooks)"""
     import torch
     if args.views:
         sel = np.arange(0, len(ang), max(1, len(ang) // args.views))[:args.views]
@@ -520,6 +520,7 @@ def run_kernel(args, tg, geo, ang, rec, rank):
             geo.rotDetector_a = geo.rotDetector_a[sel]
     tg.set_ax_path(args.ax_path)
     tg.set_siddon_path(args.siddon_path)
+    tg.set_atb_path(args.atb_path)
     tg.set_fdk_path(args.fdk_path)
     tg.set_index_path(args.index_path)
     kind, _, mode = args.kernel.partition(":")
@@ -560,7 +561,7 @@ def run_kernel(args, tg, geo, ang, rec, rank):
         print(json.dumps({"metric": "one kernel, timed alone", "kernel": args.kernel, "ms": ms, "value": units / (ms * 1e-3) / 1e9, "unit": unit,
                           "n_gpus": 1, "dtype": "f32", "data": "synthetic (seeded uniform random)",
                           "config": {"workload": f"{rec['name']}: {geo.nVoxel[0]}^3, {nA} views of {geo.nDetector[0]}x{geo.nDetector[1]}",
-                                     "ax_path": args.ax_path, "siddon_path": args.siddon_path, "fdk_path": args.fdk_path, "index_path": args.index_path}}))
+                                     "ax_path": args.ax_path, "siddon_path": args.siddon_path, "atb_path": args.atb_path, "fdk_path": args.fdk_path, "index_path": args.index_path}}))
 
 
 def kernel_rates_other_configs(tg, rates):
@@ -641,6 +642,7 @@ def main():
                     help="plan: OS-SART iteration in HBM (default); chunked: Ax + A^T b with all arrays in pinned host memory (S8)")
     ap.add_argument("--kernel", default="ax:siddon", help="kernel mode: ax:siddon | ax:interp | atb:matched | atb:fdk | atb:exact_siddon | atb:exact_interp | fdk_filter[:window]")
     ap.add_argument("--views", type=int, default=0, help="kernel mode: use N evenly spaced views of the config (0 = all)")
+    ap.add_argument("--atb-path", type=int, default=0, help="kernel mode: tigre_set_atb_path (0 default, 1 gather kernel, 3 TMA kernel without the linearised z-runs of tilted views)")
     ap.add_argument("--siddon-path", type=int, default=0, help="kernel mode: tigre_set_siddon_path (0 L1 kernel, 1 TMA-staged kernel)")
     ap.add_argument("--ax-path", type=int, default=0, help="kernel mode: tigre_set_ax_path (0 default, 1 L1 kernel, 2 TMA kernel also for wide beams)")
     ap.add_argument("--fdk-path", type=int, default=0, help="kernel mode: tigre_set_fdk_path (0 tensor cores, 1 CUDA cores)")

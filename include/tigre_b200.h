@@ -363,7 +363,8 @@ TIGRE_API int tigre_chunk_stats(uint64_t *h2d_bytes, uint64_t *d2h_bytes, int *n
 /* which A^T b kernel runs: 0 (default) = detector footprints staged into shared memory by TMA whenever the
  * problem qualifies (16-byte aligned rows, tiles >= 32x16 voxels), 1 = always the L1/L2 gather kernel.  Both
  * compute the same sums (DESIGN.md O-C); the switch exists for A/B measurement.  2 = the TMA kernel with its
- * staged box deliberately undersized, so that views take its in-kernel gather fallback (test hook). */
+ * staged box deliberately undersized, so that views take its in-kernel gather fallback (test hook).  3 = the TMA kernel with
+ * the per-voxel reciprocal and square root on tilted views instead of the linearised z-run (A/B and test hook). */
 TIGRE_API int tigre_set_atb_path(int path);
 /* which interpolated tigre_Ax kernel runs: 0 (default) = boxes of the volume staged into shared memory by TMA where that is
  * the faster one (the 32 rays of a warp span less than 27 voxels) and the problem qualifies (nx, ny multiples of 4, 16-byte

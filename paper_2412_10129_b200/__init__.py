@@ -642,7 +642,8 @@ def set_siddon_path(path):
 
 
 def set_atb_path(path):
-    """0 = TMA-staged A^T b kernel when the problem qualifies (default), 1 = gather kernel only."""
+    """0 = TMA-staged A^T b kernel when the problem qualifies (default), 1 = gather kernel only, 2 = TMA kernel with an undersized box
+    (test hook), 3 = TMA kernel without the linearised z-runs of tilted views."""
     _check(_lib().tigre_set_atb_path(int(path)), "tigre_set_atb_path")
 
 

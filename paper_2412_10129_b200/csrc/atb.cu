@@ -105,7 +105,7 @@ static void atb_gather_launch(dim3 grid, dim3 block, cudaStream_t st, bool clamp
 
 int launch_atb_tma(const float* proj, const Grid& g, const VoxView* d_views, const VoxView* h_views, int nViews, int mode,
                    const AtbP& p, float* vol, cudaStream_t st);   // atb_tma.cu
-int g_atb_path = 0;   // 0 = TMA-staged kernel when the problem qualifies, 1 = gather kernel only, 2 = TMA, box undersized
+int g_atb_path = 0;   // 0 = TMA-staged kernel when the problem qualifies, 1 = gather kernel only, 2 = TMA, box undersized, 3 = TMA without the linearised z-runs
 
 int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nViews, int mode, bool unit_proj,
                float* vol, int z0, int nzs, bool accumulate, int row0, int nrows, bool clamp, cudaStream_t st,
@@ -119,6 +119,7 @@ int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nVi
     p.hu = g.nu / 2, p.hv = g.nv / 2;
     p.accumulate = accumulate ? 1 : 0;
     p.magic = 0x4B400000;
+    p.lin_ok = g_atb_path != 3;
     constexpr int ZR = 8;
     dim3 block(ATB_BX, ATB_BY);
     dim3 grid((g.nx + ATB_BX - 1) / ATB_BX, (g.ny + ATB_BY - 1) / ATB_BY, (nzs + ZR - 1) / ZR);
@@ -142,7 +143,7 @@ int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nVi
 }  // namespace tg
 
 extern "C" int tigre_set_atb_path(int path) {
-    if (path < 0 || path > 2) return TIGRE_ERR_ARG;
+    if (path < 0 || path > 3) return TIGRE_ERR_ARG;
     tg::g_atb_path = path;
     return TIGRE_OK;
 }

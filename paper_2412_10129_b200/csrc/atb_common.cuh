@@ -18,6 +18,7 @@ struct AtbP {
     int hu, hv;           // nu/2, nv/2
     int accumulate;
     int magic;            // 0x4B400000 = bits of 1.5*2^23 (floor_magic), passed as data (see atb_tma.cu)
+    int lin_ok;           // atb_tma.cu: tilted views may take the linearised z-run (0 = always the per-voxel reciprocal: tigre_set_atb_path(3))
 };
 
 constexpr int ATB_BX = 32, ATB_BY = 8;

@@ -31,7 +31,8 @@ constexpr int TMA_STAGES_MAX = 8;
 
 struct StageInfo {   // written by the producer before it arms the stage's full barrier
     int c0, c1;      // absolute detector index of the box origin (u, v)
-    int fits, pad;
+    int fits;
+    int lin;         // tilted view: over this tile's z-runs 1/W is linear and the weight quadratic in k to 2e-7 (see the general branch)
     float4 rU, rV, rW, rG, cst;   // the view's table entry: consumers read it here (shared-memory latency, broadcast)
 };
 
@@ -83,10 +84,13 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
             const float W = fmaf(rW.x, cxf, fmaf(rW.y, cyf, fmaf(rW.z, czf, rW.w)));
             const float t = rcp_fast(W);
             float ulo = U * t, vlo = V * t, uhi = ulo, vhi = vlo;
+            // smallest depth of the tile's corners (W, and the FDK weight's G): what the bounds of the general branch divide by
+            float dmin = MODE == TIGRE_ATB_FDK ? fminf(W, fmaf(rG.x, cxf, fmaf(rG.y, cyf, fmaf(rG.z, czf, rG.w)))) : W;
 #pragma unroll
             for (int o = 4; o > 0; o >>= 1) {
                 ulo = fminf(ulo, __shfl_xor_sync(0xffffffffu, ulo, o)), uhi = fmaxf(uhi, __shfl_xor_sync(0xffffffffu, uhi, o));
                 vlo = fminf(vlo, __shfl_xor_sync(0xffffffffu, vlo, o)), vhi = fmaxf(vhi, __shfl_xor_sync(0xffffffffu, vhi, o));
+                dmin = fminf(dmin, __shfl_xor_sync(0xffffffffu, dmin, o));
             }
             if (lane == 0) {
                 // box origin one pixel below the smallest tap; taps reach floor(max)+1, one more of slack for
@@ -101,6 +105,21 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
                 }
                 if (a >= nStages) mbar_wait(empty + s, ph);
                 info[s].c0 = c0, info[s].c1 = c1, info[s].fits = fits;
+                {
+                    // General (tilted) views: along a z-run of ZR voxels W(k) = W0 + k rW.z and the matched weight is km N(k) / W(k)^3 with
+                    // N = |(sx W, du Eu, dv Ev)| the norm of a vector linear in k (slope b, |b|^2 = qC below); FDK: 1 / G(k)^2.  With
+                    // rho = max(|rW.z| / Wmin, |b| / (sx Wmin), |rG.z| / Gmin) the third logarithmic derivative of the weight is below
+                    // 60 rho^3, so the quadratic through its values at k = 0, h, 2h (h = (ZR-1)/2) is off by < 0.064 * 60 (rho h)^3, and
+                    // 1/W expanded to first order about the middle of the run by (|rW.z| h / W)^2.  Both below 2e-7 / 1e-8: the consumers
+                    // take one reciprocal and three exact weights per run instead of a reciprocal and a square root per voxel.
+                    const float dEu = fmaf(-cst.z, rW.z, rU.z), dEv = fmaf(-cst.w, rW.z, rV.z);
+                    const float b2 = MODE == TIGRE_ATB_FDK ? 0.f : fmaf(p.du2 * dEu, dEu, fmaf(p.dv2 * dEv, dEv, cst.y * rW.z * rW.z));
+                    const float h = 0.5f * (float)(ZR - 1), inv = dmin > 0.f ? 1.0f / dmin : 3.0e38f;
+                    const float rhoW = fabsf(rW.z) * inv;
+                    const float rho = fmaxf(fmaxf(rhoW, fabsf(rG.z) * inv), MODE == TIGRE_ATB_FDK ? 0.f : sqrtf(b2 / fmaxf(cst.y, 1e-30f)) * inv);
+                    const float e = rho * h, eW = rhoW * h;
+                    info[s].lin = (3.84f * e * e * e < 2.0e-7f && eW * eW < 1.0e-8f) ? 1 : 0;
+                }
                 if (boxes)   // tigre_Atb_boxes (reading P19(b)): the staged box of this (tile, view), absolute detector indices
                     boxes[((size_t)(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * nViews + a] = make_int4(c0, c1, fits, 0);
                 info[s].rU = rU, info[s].rV = rV, info[s].rW = rW, info[s].rG = rG, info[s].cst = cst;
@@ -204,6 +223,65 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
                     const float kf = (float)k;
                     acc[k] = fmaf(sqrt_fast(fmaf(fmaf(qC, kf, qB), kf, qA)), val, acc[k]);
                 }
+            }
+        } else if (info[s].lin && p.lin_ok) {
+            // general view whose z-runs are short against the depth (the producer's bound): 1/W to first order about the middle of
+            // the run (one reciprocal, Newton-refined), the weight as the quadratic through its exact values at k = 0, h, 2h
+            constexpr float H = 0.5f * (float)(ZR - 1);
+            const float Wm = fmaf(H, rW.z, W0);
+            float tm_ = rcp_fast(Wm);
+            tm_ = tm_ * fmaf(-Wm, tm_, 2.0f);
+            const float dt = -rW.z * tm_ * tm_, t0 = fmaf(-H, dt, tm_);
+            float wq0, wq1, wq2;
+            {
+                float qA = 0.f, qB = 0.f, qC = 0.f;
+                if (MODE != TIGRE_ATB_FDK) {
+                    const float Eu = fmaf(-cst.z, W0, U0), Ev = fmaf(-cst.w, W0, V0);
+                    const float dEu = fmaf(-cst.z, rW.z, rU.z), dEv = fmaf(-cst.w, rW.z, rV.z);
+                    const float sW = cst.y * W0, sdW = cst.y * rW.z;
+                    qA = fmaf(p.du2 * Eu, Eu, fmaf(p.dv2 * Ev, Ev, sW * W0));
+                    qB = 2.f * fmaf(p.du2 * Eu, dEu, fmaf(p.dv2 * Ev, dEv, sW * rW.z));
+                    qC = fmaf(p.du2 * dEu, dEu, fmaf(p.dv2 * dEv, dEv, sdW * rW.z));
+                }
+                float wn[3];
+#pragma unroll
+                for (int n = 0; n < 3; ++n) {
+                    const float kf = H * (float)n;
+                    if (MODE == TIGRE_ATB_FDK) {
+                        const float ig = rcp_fast(fmaf(kf, rG.z, G0));
+                        wn[n] = ig * ig;
+                    } else {
+                        const float t = rcp_fast(fmaf(kf, rW.z, W0));
+                        wn[n] = ((cst.x * t) * (t * t)) * sqrt_fast(fmaf(fmaf(qC, kf, qB), kf, qA));
+                    }
+                }
+                wq0 = wn[0];
+                wq2 = ((wn[2] - wn[1]) - (wn[1] - wn[0])) * (0.5f / (H * H));
+                wq1 = fmaf(-wq2, H, (wn[1] - wn[0]) * (1.0f / H));
+            }
+            const float Uh = fmaf(-0.5f, W0, U0), Vh = fmaf(-0.5f, W0, V0);
+            const float dUh = fmaf(-0.5f, rW.z, rU.z), dVh = fmaf(-0.5f, rW.z, rV.z);
+            const uint32_t col = tiles_s + (uint32_t)(s * stageElems + (p.hu - c0) + (p.hv - c1) * BU) * 4u -
+                                 (uint32_t)p.magic * (uint32_t)(BU * 4 + 4);
+#pragma unroll
+            for (int k = 0; k < ZR; ++k) {
+                const float kf = (float)k;
+                const float t = fmaf(kf, dt, t0);
+                const float Uk = fmaf(kf, dUh, Uh), Vk = fmaf(kf, dVh, Vh);
+                const float tmu = fmaf(Uk, t, 12582912.0f), tmv = fmaf(Vk, t, 12582912.0f);
+                const float au = fmaf(Uk, t, 0.5f - (tmu - 12582912.0f)), av = fmaf(Vk, t, 0.5f - (tmv - 12582912.0f));
+                const uint32_t q = col + __float_as_uint(tmv) * (uint32_t)(BU * 4) + __float_as_uint(tmu) * 4u;
+                float p00, p10, p01, p11;
+                asm volatile(
+                    "ld.shared.f32 %0, [%4];\n\t"
+                    "ld.shared.f32 %1, [%4+4];\n\t"
+                    "ld.shared.f32 %2, [%4+%5];\n\t"
+                    "ld.shared.f32 %3, [%4+%6];"
+                    : "=f"(p00), "=f"(p10), "=f"(p01), "=f"(p11)
+                    : "r"(q), "n"(BU * 4), "n"(BU * 4 + 4));
+                const float r0 = fmaf(au, p10 - p00, p00), r1 = fmaf(au, p11 - p01, p01);
+                const float val = fmaf(av, r1 - r0, r0);
+                acc[k] = fmaf(fmaf(fmaf(wq2, kf, wq1), kf, wq0), val, acc[k]);
             }
         } else {
             // general view (tilted detector): U, V, W all vary along the z-run, so each voxel has its own reciprocal.

@@ -20,19 +20,22 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+// Spin on a phase of the barrier.  The loop is INSIDE the asm block with the address in a register: as a C++ do-while around a
+// try_wait the "memory" clobber made nvcc re-form the barrier's address (and whatever else it had rematerialised) after every
+// failed try -- 11 instructions per poll in the consumers of atb_tma.cu, which compete for issue slots with the warps that have
+// work (labels in a { } block are local to it, so the block may be inlined any number of times).
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n"
-            ".reg .pred p;\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-            "selp.u32 %0, 1, 0, p;\n"
-            "}\n"
-            : "=r"(ok)
-            : "r"(smem_u32(bar)), "r"(parity)
-            : "memory");
-    } while (!ok);
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "MBAR_WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra MBAR_WAIT_DONE;\n"
+        "bra MBAR_WAIT_LOOP;\n"
+        "MBAR_WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
 }
 // one box of a 3-D tensor (coordinates fastest dimension first; whatever lies outside the tensor arrives as zeros)
 __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
