@@ -20,6 +20,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <mutex>
+#include <type_traits>
 #include "atb_common.cuh"
 #include "tma.cuh"
 
@@ -118,7 +119,12 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
                     const float rhoW = fabsf(rW.z) * inv;
                     const float rho = fmaxf(fmaxf(rhoW, fabsf(rG.z) * inv), MODE == TIGRE_ATB_FDK ? 0.f : sqrtf(b2 / fmaxf(cst.y, 1e-30f)) * inv);
                     const float e = rho * h, eW = rhoW * h;
-                    info[s].lin = (3.84f * e * e * e < 2.0e-7f && eW * eW < 1.0e-8f) ? 1 : 0;
+                    // z-aligned views (the branch below with one reciprocal per run): the matched weight is wk sqrt(q(k)) = wk |a + b k| with
+                    // |b| = dv |rV.z| t and |a + b k| >= sx; the third derivative of such a norm N is below 1.155 |b|^3 / N^2, so the quadratic
+                    // through sqrt(q) at k = 0, h, 2h is off by < 0.064 * 1.155 (rhoZ h)^3 relative (bit 1 of the flag)
+                    const float rhoZ = MODE == TIGRE_ATB_FDK ? 0.f : sqrtf(p.dv2 / fmaxf(cst.y, 1e-30f)) * fabsf(rV.z) * inv;
+                    const float eZ = rhoZ * h;
+                    info[s].lin = ((3.84f * e * e * e < 2.0e-7f && eW * eW < 1.0e-8f) ? 1 : 0) | ((0.074f * eZ * eZ * eZ < 1.0e-7f) ? 2 : 0);
                 }
                 if (boxes)   // tigre_Atb_boxes (reading P19(b)): the staged box of this (tile, view), absolute detector indices
                     boxes[((size_t)(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * nViews + a] = make_int4(c0, c1, fits, 0);
@@ -193,6 +199,16 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
                 qA = fmaf(p.dv2 * ev0, ev0, fmaf(p.du2 * eu, eu, cst.y));
                 qB = 2.f * p.dv2 * ev0 * dfv, qC = p.dv2 * dfv * dfv;
             }
+            // where the producer's bound holds the square root itself is replaced by the quadratic through its values at k = 0, h, 2h
+            // (three MUFU.SQRT per run instead of one per voxel; the Horner form below then yields sqrt(q) directly)
+            const bool surrogate = MODE != TIGRE_ATB_FDK && (info[s].lin & 2) && p.lin_ok;
+            if (surrogate) {
+                constexpr float H = 0.5f * (float)(ZR - 1);
+                const float s0 = sqrt_fast(qA), s1 = sqrt_fast(fmaf(fmaf(qC, H, qB), H, qA)), s2 = sqrt_fast(fmaf(fmaf(qC, 2.f * H, qB), 2.f * H, qA));
+                qA = s0;
+                qC = ((s2 - s1) - (s1 - s0)) * (0.5f / (H * H));
+                qB = fmaf(-qC, H, (s1 - s0) * (1.0f / H));
+            }
             const float wa = wk * (1.f - au), wb = wk * au;
             // byte address (shared window) of the tap column in row 0 of the stage, minus the magic-number
             // bias of floor_magic times the row pitch (mod 2^32): the row address is then ONE integer
@@ -201,6 +217,9 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
                            (uint32_t)p.magic * (uint32_t)(BU * 4);   // p.magic = 0x4B400000, opaque to the compiler
                                                                       // (as a literal it is re-added before every load)
             asm volatile("" : "+r"(col));   // ... and so is the sum: nvcc factors it back into (bits - magic) * pitch, an IADD3 per update
+            // (the loop is instantiated twice so that the choice is a branch around it, not a predicated MUFU in it)
+            auto zrun = [&](auto sur_tag) {
+            constexpr bool SUR = decltype(sur_tag)::value;
 #pragma unroll
             for (int k = 0; k < ZR; ++k) {
                 const float fv = fmaf((float)k, dfv, fv0);
@@ -221,10 +240,14 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
                     acc[k] += val;
                 } else {
                     const float kf = (float)k;
-                    acc[k] = fmaf(sqrt_fast(fmaf(fmaf(qC, kf, qB), kf, qA)), val, acc[k]);
+                    const float qk = fmaf(fmaf(qC, kf, qB), kf, qA);
+                    acc[k] = fmaf(SUR ? qk : sqrt_fast(qk), val, acc[k]);
                 }
             }
-        } else if (info[s].lin && p.lin_ok) {
+            };
+            if (surrogate) zrun(std::true_type{});
+            else zrun(std::false_type{});
+        } else if ((info[s].lin & 1) && p.lin_ok) {
             // general view whose z-runs are short against the depth (the producer's bound): 1/W to first order about the middle of
             // the run (one reciprocal, Newton-refined), the weight as the quadratic through its exact values at k = 0, h, 2h
             constexpr float H = 0.5f * (float)(ZR - 1);
