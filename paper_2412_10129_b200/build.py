@@ -23,7 +23,7 @@ def needs_build() -> bool:
         return True
     t = os.path.getmtime(LIB)
     import glob
-    deps = _sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + [os.path.join(HERE, "..", "include", "tigre_b200.h")]
+    deps = _sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.inc")) + [os.path.join(HERE, "..", "include", "tigre_b200.h")]
     return any(os.path.getmtime(d) > t for d in deps)
 
 

@@ -1,7 +1,6 @@
 // ax_siddon.cuh — the Siddon march shared by ax.cu (volume gathered through L1) and ax_siddon_tma.cu (interior of the march staged
 // into shared memory by TMA): per-ray state, the three slab steps, and the fp64 per-ray set-up as a function.  See the head of
-// ax.cu for the method.  (ax_siddon_kernel of ax.cu keeps its own inline copy of the set-up below: handing the twenty values
-// through a struct costs that kernel 1-2 % in spills at its 56-register budget; the two texts must stay the same.)
+// ax.cu for the method.  (The set-up's text lives in ax_siddon_setup.inc and is included by ax_siddon_kernel directly and by siddon_setup() here.)
 #pragma once
 #include <cmath>
 #include "ax_common.cuh"
@@ -177,112 +176,17 @@ struct SidSetup {
 };
 
 template <typename IdxT, bool COUNT>
-__device__ __forceinline__ void siddon_setup(const RayView& rv, const AxP& p, int iu, int iv, bool haveT, SidRay<IdxT>& r, SidSetup& q) {
-    q.useT = false;
-    // ---- per-ray set-up, fp64
-    double S[3], d[3];
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        S[k] = rv.S[k] + iu * rv.dSU[k] + iv * rv.dSV[k];   // parallel beam: every ray has its own start (P29)
-        d[k] = rv.P0[k] + iu * rv.dU[k] + iv * rv.dV[k] - S[k];
-    }
-    const double Lmm = sqrt(d[0] * p.hxd * d[0] * p.hxd + d[1] * p.hyd * d[1] * p.hyd + d[2] * p.hzd * d[2] * p.hzd);
-    const double a0 = fabs(d[0]), a1 = fabs(d[1]), a2 = fabs(d[2]);
-    const int D = (a0 >= a1 && a0 >= a2) ? 0 : (a1 >= a2 ? 1 : 2);
-    q.D = D;
-    // F is the z axis unless the ray itself runs along z: along a detector row (= a warp) the rays cross the z-planes in nearly
-    // the same slabs, which the march below uses
-    const int E = D == 0 ? 1 : 0, F = D == 2 ? 1 : 2;
-    const double dD = sel3(D, d[0], d[1], d[2]), dE = sel3(E, d[0], d[1], d[2]), dF = sel3(F, d[0], d[1], d[2]);
-    q.rev = dD < 0.0;
-    const double SD = sel3(D, S[0], S[1], S[2]), SE = sel3(E, S[0], S[1], S[2]), SF = sel3(F, S[0], S[1], S[2]);
+__device__ __forceinline__ void siddon_setup(const RayView& rv, const AxP& p, int iu, int iv, bool haveT, SidRay<IdxT>& rout, SidSetup& q) {
+    // stand-ins for the two volume pointers the text selects `base` from (never dereferenced here)
+    const float* const vol = nullptr;
+    const float* const volT = haveT ? reinterpret_cast<const float*>(sizeof(float)) : nullptr;
+#include "ax_siddon_setup.inc"
+    rout = r;
+    q.D = D, q.i0 = i0, q.nslab = nslab, q.kA = kA, q.kB = kB, q.ie = ie, q.jf = jf, q.ie0 = ie0, q.jf0 = jf0, q.diE = diE, q.diF = diF;
+    q.nE = nE, q.nF = nF, q.slo0 = slo0, q.shiN = shiN, q.scale = scale, q.hE0 = hE0, q.hF0 = hF0;
     q.SD = SD, q.SE = SE, q.SF = SF, q.mE = dD != 0.0 ? dE / dD : 0.0, q.mF = dD != 0.0 ? dF / dD : 0.0;
-    const int nD = D == 0 ? p.nx : (D == 1 ? p.ny : p.nz);
-    const int nE = q.nE = E == 0 ? p.nx : (E == 1 ? p.ny : p.nz);
-    const int nF = q.nF = F == 0 ? p.nx : (F == 1 ? p.ny : p.nz);
-    uint32_t& cnt = q.cnt;
-    cnt = 0;
-    // marching state, filled by the set-up below; a ray that misses the volume keeps nslab = 0
-    r.imE = r.imF = 1.f, r.sgE = r.sgF = 1.f, r.hE = r.hF = 3.0e38f, r.stE = r.stF = r.sD = 0;
-    r.kf = 0.f, r.acc = 0.f, r.vB = 0.f, r.ys = 0.f, r.off = 0;
-    r.first = r.last = -1, r.nseg = 0, r.fm = 0, r.pok = false;
-    int &i0 = q.i0, &nslab = q.nslab, &kA = q.kA, &kB = q.kB, &ie = q.ie, &jf = q.jf, &ie0 = q.ie0, &jf0 = q.jf0, &diE = q.diE, &diF = q.diF;
-    i0 = 0, nslab = 0, kA = 0, kB = 0, ie = 0, jf = 0, ie0 = 0, jf0 = 0, diE = 1, diF = 1;
-    float &slo0 = q.slo0, &shiN = q.shiN, &scale = q.scale;
-    slo0 = 0.f, shiN = 1.f, scale = 0.f;
-    double &hE0 = q.hE0, &hF0 = q.hF0;   // fp64 values r.hE / r.hF start from (0 for a ray that never crosses)
-    hE0 = 0.0, hF0 = 0.0;
-    if (dD != 0.0) {
-        const double mE = dE / dD, mF = dF / dD;
-        // range of xi_D covered by the segment S->P, clipped to the volume box on all three axes;
-        // [sa, sb]: sub-range that also stays >= margin away from the lateral faces (unchecked slabs)
-        const double margin = 1e-3;
-        double lo = fmin(SD, SD + dD), hi = fmax(SD, SD + dD);
-        lo = fmax(lo, 0.0), hi = fmin(hi, (double)nD);
-        double sa = lo, sb = hi;
-        bool miss = false;
-        if (mE != 0.0) {
-            const double t1 = SD + (0.0 - SE) / mE, t2 = SD + ((double)nE - SE) / mE;
-            lo = fmax(lo, fmin(t1, t2)), hi = fmin(hi, fmax(t1, t2));
-            const double u1 = SD + (margin - SE) / mE, u2 = SD + ((double)nE - margin - SE) / mE;
-            sa = fmax(sa, fmin(u1, u2)), sb = fmin(sb, fmax(u1, u2));
-        } else {
-            if (SE < 0.0 || SE > (double)nE) miss = true;
-            if (SE < margin || SE > (double)nE - margin) sb = sa - 1.0;
-        }
-        if (mF != 0.0) {
-            const double t1 = SD + (0.0 - SF) / mF, t2 = SD + ((double)nF - SF) / mF;
-            lo = fmax(lo, fmin(t1, t2)), hi = fmin(hi, fmax(t1, t2));
-            const double u1 = SD + (margin - SF) / mF, u2 = SD + ((double)nF - margin - SF) / mF;
-            sa = fmax(sa, fmin(u1, u2)), sb = fmin(sb, fmax(u1, u2));
-        } else {
-            if (SF < 0.0 || SF > (double)nF) miss = true;
-            if (SF < margin || SF > (double)nF - margin) sb = sa - 1.0;
-        }
-        if (!miss && hi > lo) {
-            if (COUNT) {
-                // exact number of voxels met = |dix|+|diy|+|diz|+1 between entry and exit voxel
-                const double eps = 1e-9 * (hi - lo);
-                const double l0 = lo + eps, l1 = hi - eps;
-                int c = 1;
-                c += abs((int)floor(l1) - (int)floor(l0));
-                c += abs((int)floor(SE + (l1 - SD) * mE) - (int)floor(SE + (l0 - SD) * mE));
-                c += abs((int)floor(SF + (l1 - SD) * mF) - (int)floor(SF + (l0 - SD) * mF));
-                cnt = (uint32_t)c;
-            } else {
-                int i1 = (int)ceil(hi);
-                i0 = max((int)floor(lo), 0), i1 = min(i1, nD);
-                nslab = i1 - i0;
-                // unchecked slabs: k in [kA, kB), each fully inside [max(lo,sa), min(hi,sb)]
-                kA = (int)ceil(fmax(lo, sa)) - i0, kB = (int)floor(fmin(hi, sb)) - i0;
-                kA = min(max(kA, 0), nslab), kB = min(max(kB, kA), nslab);
-                // state at the START of slab i0 (s = 0), fp64: position, cell index, next plane ahead
-                const double eS = SE + ((double)i0 - SD) * mE, fS = SF + ((double)i0 - SD) * mF;
-                ie0 = (int)floor(eS), jf0 = (int)floor(fS);
-                ie = ie0, jf = jf0;
-                const bool upE = mE > 0.0, upF = mF > 0.0;
-                // x-dominant rays read the (x,y)-transposed copy so that neighbouring lanes (which differ
-                // mostly in y) touch neighbouring addresses
-                const bool useT = (D == 0) && haveT;
-                q.useT = useT;
-                const IdxT pX = useT ? (IdxT)p.ny : (IdxT)1, pY = useT ? (IdxT)1 : (IdxT)p.nx, pZ = (IdxT)p.nx * p.ny;
-                const IdxT sD = D == 0 ? pX : (D == 1 ? pY : pZ);
-                const IdxT sE = E == 0 ? pX : (E == 1 ? pY : pZ);
-                const IdxT sF = F == 0 ? pX : (F == 1 ? pY : pZ);
-                // a ray parallel to the planes (m = 0) never crosses: next plane at +huge, 1/m := 1
-                r.imE = mE != 0.0 ? (float)(1.0 / mE) : 1.f, r.imF = mF != 0.0 ? (float)(1.0 / mF) : 1.f;
-                hE0 = mE != 0.0 ? (double)(upE ? ie0 + 1 : ie0) - eS : 0.0;
-                hF0 = mF != 0.0 ? (double)(upF ? jf0 + 1 : jf0) - fS : 0.0;
-                r.hE = mE != 0.0 ? (float)hE0 : 3.0e38f, r.hF = mF != 0.0 ? (float)hF0 : 3.0e38f;
-                r.sgE = upE ? 1.f : -1.f, r.sgF = upF ? 1.f : -1.f;
-                r.stE = upE ? sE : -sE, r.stF = upF ? sF : -sF, r.sD = sD;
-                r.off = (IdxT)i0 * sD + (IdxT)ie * sE + (IdxT)jf * sF;   // may be out of range in checked slabs
-                diE = upE ? 1 : -1, diF = upF ? 1 : -1;
-                slo0 = (float)(lo - (double)i0), shiN = (float)(hi - (double)(i1 - 1));
-                scale = (float)(Lmm / fabs(dD));
-            }
-        }
-    }
+    q.useT = haveT && base == volT, q.rev = dD < 0.0, q.cnt = cnt;
+    (void)Lmm, (void)nD;
 }
 
 }  // namespace tg
