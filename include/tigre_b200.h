@@ -189,6 +189,12 @@ TIGRE_API int tigre_plan_create_ex(const tigre_geo *geo, const double *angles, i
                          void *cuda_stream, tigre_plan **plan_out);
 TIGRE_API int tigre_plan_ossart(tigre_plan *plan, const float *b, float *x_inout, int n_iter, float lambda,
                       int nonneg, double *resid_hist, void *cuda_stream);
+/* Host only (no device needed): the z-slices [*zlo, *zhi] of the volume that rays of detector rows [row0, row1) of the given views
+ * can meet, with three slices of margin (zlo > zhi: none).  Returns 1 when no bound is formed (parallel beam; source or detector
+ * over the volume's (x,y) footprint).  tigre_plan_ossart with pinned host arrays uses it to send the iterate up in the order the
+ * first projection's row bands need it (e2e); exported for its test against the oracle's first / last
+ * voxel per ray (reading P19(a)). */
+TIGRE_API int tigre_band_z_range(const tigre_geo *geo, const double *angles, int nA, int row0, int row1, int32_t *zlo, int32_t *zhi);
 /* The subset steps [s_begin, s_end) of ONE sweep of tigre_plan_ossart, in order, with the plan's own W_s, V_s and view lists
  * (what a caller needs to interleave other work between subsets, and what the tests use to check a single ordered-subset
  * update of the very plan a long run advances).  b, x_inout dev, or both pinned host.  Asynchronous for device data. */

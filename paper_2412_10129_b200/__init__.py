@@ -53,7 +53,7 @@ EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_Ax_slab", "tigre_Atb_slab", "tigre_sl
            "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_create_ex", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_osem", "tigre_plan_sart_tv", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version", "tigre_Ax_index", "tigre_set_index_path", "tigre_set_workspace", "tigre_plan_workspace_bytes",
-           "tigre_workspace_stats", "tigre_sirt_chunked", "tigre_microbench", "tigre_set_ax_path", "tigre_set_plan_v_path", "tigre_plan_ossart_subsets", "tigre_Atb_boxes", "tigre_set_fdk_path", "tigre_residual_noalloc", "tigre_set_siddon_path"]
+           "tigre_workspace_stats", "tigre_sirt_chunked", "tigre_microbench", "tigre_set_ax_path", "tigre_set_plan_v_path", "tigre_plan_ossart_subsets", "tigre_Atb_boxes", "tigre_set_fdk_path", "tigre_residual_noalloc", "tigre_set_siddon_path", "tigre_band_z_range"]
 
 
 def _lib():
@@ -634,6 +634,19 @@ def set_ax_path(path):
     """0 = TMA-staged interpolated Ax kernel for narrow beams that qualify (default), 1 = L1 gather kernel only, 2 = TMA kernel
     for wide beams too."""
     _check(_lib().tigre_set_ax_path(int(path)), "tigre_set_ax_path")
+
+
+def band_z_range(geo, angles, row0, row1):
+    """(zlo, zhi): z-slices that rays of detector rows [row0, row1) of these views can meet (zlo > zhi: none); None if no bound is
+    formed.  Host only."""
+    a, nA = _angles(angles)
+    G = _Geo(geo, nA)
+    lo, hi = C.c_int32(0), C.c_int32(-1)
+    rc = _lib().tigre_band_z_range(C.byref(G.c), a.ctypes.data_as(_dp), nA, int(row0), int(row1), C.byref(lo), C.byref(hi))
+    if rc == 1:
+        return None
+    _check(rc, "tigre_band_z_range")
+    return lo.value, hi.value
 
 
 def set_siddon_path(path):

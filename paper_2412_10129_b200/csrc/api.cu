@@ -9,6 +9,7 @@
 #include <memory>
 #include <mutex>
 #include <string>
+#include <array>
 #include <vector>
 #include "common.cuh"
 
@@ -686,6 +687,76 @@ int tigre_plan_ossart_subsets(tigre_plan* P, const float* b, float* x, int s_beg
     return plan_ossart_impl(P, b, x, 1, lambda, nonneg, nullptr, cuda_stream, s_begin, s_end);
 }
 
+// z-slices [zlo, zhi] of the volume that rays of detector rows [r0, r1) of these cone-beam views can meet (zlo > zhi: none), or
+// false if no bound is formed (parallel beam, source or detector over the volume's (x,y) footprint).  The points such rays reach
+// inside the footprint are (pyramid over the band from the source) n (footprint x all z), a convex polytope: its z-extremes are at
+// corner rays clipped to the footprint, or where a vertical edge of the footprint meets one of the pyramid's four side planes
+// (all eight taken, whether or not inside the face: a superset).  RayView is in voxel-index coordinates.  Three slices of margin.
+static bool band_z_range(const RayView* hv, int nViews, const Grid& g, int r0, int r1, int& zlo, int& zhi) {
+    double lo = 1e300, hi = -1e300;
+    const double bx[2] = {0.0, (double)g.nx}, by[2] = {0.0, (double)g.ny};
+    for (int a = 0; a < nViews; ++a) {
+        const RayView& rv = hv[a];
+        for (int k = 0; k < 3; ++k)
+            if (rv.dSU[k] != 0.0 || rv.dSV[k] != 0.0) return false;
+        const double* S = rv.S;
+        if (S[0] >= bx[0] && S[0] <= bx[1] && S[1] >= by[0] && S[1] <= by[1]) return false;
+        double d[4][3];
+        for (int c = 0; c < 4; ++c) {
+            const double iu = (c & 1) ? g.nu - 1 : 0, iv = (c & 2) ? r1 - 1 : r0;
+            for (int k = 0; k < 3; ++k) d[c][k] = rv.P0[k] + iu * rv.dU[k] + iv * rv.dV[k] - S[k];
+            double t0 = 0.0, t1 = 1.0;
+            for (int k = 0; k < 2; ++k) {
+                const double n = k == 0 ? bx[1] : by[1];
+                if (d[c][k] != 0.0) {
+                    const double ta = (0.0 - S[k]) / d[c][k], tb = (n - S[k]) / d[c][k];
+                    t0 = std::max(t0, std::min(ta, tb)), t1 = std::min(t1, std::max(ta, tb));
+                } else if (S[k] < 0.0 || S[k] > n) {
+                    t1 = -1.0;
+                }
+            }
+            if (t1 >= t0) {
+                if (t1 >= 1.0) return false;   // the detector pixel itself lies over the footprint
+                const double za = S[2] + t0 * d[c][2], zb = S[2] + t1 * d[c][2];
+                lo = std::min(lo, std::min(za, zb)), hi = std::max(hi, std::max(za, zb));
+            }
+        }
+        const int face[4][2] = {{0, 1}, {2, 3}, {0, 2}, {1, 3}};   // bottom row, top row, first column, last column
+        for (int f = 0; f < 4; ++f) {
+            const double* p = d[face[f][0]];
+            const double* q = d[face[f][1]];
+            const double n[3] = {p[1] * q[2] - p[2] * q[1], p[2] * q[0] - p[0] * q[2], p[0] * q[1] - p[1] * q[0]};
+            const double nn = std::sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
+            if (!(std::fabs(n[2]) > 1e-9 * nn)) continue;   // a vertical face holds no isolated point of a vertical edge
+            for (int e = 0; e < 4; ++e) {
+                const double z = S[2] - (n[0] * (bx[e & 1] - S[0]) + n[1] * (by[e >> 1] - S[1])) / n[2];
+                lo = std::min(lo, z), hi = std::max(hi, z);
+            }
+        }
+    }
+    if (hi < lo) {
+        zlo = 0, zhi = -1;
+        return true;
+    }
+    zlo = (int)std::max(0.0, std::floor(std::max(lo, -1e8)) - 3.0), zhi = (int)std::min((double)g.nz - 1.0, std::floor(std::min(hi, 1e8)) + 3.0);
+    return true;
+}
+
+int tigre_band_z_range(const tigre_geo* geo, const double* angles, int nA, int row0, int row1, int32_t* zlo, int32_t* zhi) {
+    if (!zlo || !zhi) return TIGRE_ERR_ARG;
+    TG_TRY(validate_geo(geo, angles, nA));
+    const Grid g = make_grid(geo);
+    if (row0 < 0 || row1 > g.nv || row0 >= row1) return TIGRE_ERR_ARG;
+    std::vector<ViewH> views;
+    resolve_views(geo, angles, nA, views);
+    std::vector<RayView> h(nA);
+    for (int i = 0; i < nA; ++i) build_ray_view(g, views[i], h[i]);
+    int lo = 0, hi = -1;
+    if (!band_z_range(h.data(), nA, g, row0, row1, lo, hi)) return 1;
+    *zlo = lo, *zhi = hi;
+    return TIGRE_OK;
+}
+
 static int plan_ossart_impl(tigre_plan* P, const float* b, float* x, int n_iter, float lambda, int nonneg, double* resid_hist,
                             void* cuda_stream, int s_begin, int s_end) {
     if (!P || !b || !x || n_iter < 0) return TIGRE_ERR_ARG;
@@ -695,9 +766,14 @@ static int plan_ossart_impl(tigre_plan* P, const float* b, float* x, int n_iter,
     // b and x may live in device memory, or both in pinned host memory (end-to-end path: the
     // projections and the iterate are copied in, the iterate is copied back, all on `st`)
     const MemKind kb = mem_kind(b), kx = mem_kind(x);
-    TempBuf db, dx;
+    TempBuf db, dx, xT;
     const float* bd = b;
     float* xd = x;
+    constexpr int X_BANDS = 4, AX_ROW_ALIGN = 4;   // bands of detector rows of the first projection (multiples of the Ax kernels' 4-row tiles)
+    bool banded = false, downloaded = false;
+    std::vector<std::vector<std::array<size_t, 2>>> bandRuns;   // per band (and one more for the rest): runs {first slice, count} of the iterate
+    std::vector<int> bandRow0, bandRows;
+    int sbase = 1;
     // end-to-end path: the projections go up on a side stream in the order the subsets need them (one event per subset:
     // the first sweep's residual of subset s waits for its views only), so all but the first subset's upload hides
     // behind the kernels; the iterate goes up first on the caller's stream
@@ -717,7 +793,43 @@ static int plan_ossart_impl(tigre_plan* P, const float* b, float* x, int n_iter,
         TG_TRY(db.alloc(sizeof(float) * per * P->nA, st));
         TG_TRY(dx.alloc(sizeof(float) * nvox, st));
         bd = db.as<float>(), xd = dx.as<float>();
-        TG_CUDA(cudaMemcpyAsync(dx.p, x, sizeof(float) * nvox, cudaMemcpyHostToDevice, st));
+        // The iterate: the first subset's projection is cut into bands of detector rows, each of which meets only a range of z-slices
+        // (band_z_range); the slices go up on the side stream in the order the bands need them, one event per band, so the first
+        // band's rays start when a quarter of the volume has arrived instead of all of it.  Without a bound (or without the
+        // transposed copy, which the bands fill slice range by slice range) the iterate goes up whole on the caller's stream.
+        const size_t slice = (size_t)g.nx * g.ny;
+        if (n_iter > 0 && g.nz >= 4 * X_BANDS && g.nx > 1 && g.ny > 1 && xT.alloc(sizeof(float) * nvox, st) == TIGRE_OK) {
+            const int rows = ((g.nv + X_BANDS - 1) / X_BANDS + AX_ROW_ALIGN - 1) / AX_ROW_ALIGN * AX_ROW_ALIGN;
+            std::vector<char> sent(g.nz, 0);
+            banded = true;
+            for (int bnd = 0; bnd < X_BANDS && banded; ++bnd) {
+                const int r0 = std::min(bnd * rows, g.nv), r1 = std::min(r0 + rows, g.nv);
+                int zlo = 0, zhi = -1;
+                if (r1 > r0 && !band_z_range(P->hray[s_begin].data(), P->off[s_begin + 1] - P->off[s_begin], g, r0, r1, zlo, zhi)) banded = false;
+                bandRow0.push_back(r0), bandRows.push_back(r1 - r0);
+                bandRuns.emplace_back();
+                for (int z = zlo; z <= zhi; ++z) {
+                    if (sent[z]) continue;
+                    int z1 = z;
+                    while (z1 <= zhi && !sent[z1]) sent[z1++] = 1;
+                    bandRuns.back().push_back(std::array<size_t, 2>{(size_t)z, (size_t)(z1 - z)});
+                    z = z1 - 1;
+                }
+            }
+            if (banded) {
+                bandRuns.emplace_back();   // the slices no band asked for
+                for (int z = 0; z < g.nz; ++z) {
+                    if (sent[z]) continue;
+                    int z1 = z;
+                    while (z1 < g.nz && !sent[z1]) sent[z1++] = 1;
+                    bandRuns.back().push_back(std::array<size_t, 2>{(size_t)z, (size_t)(z1 - z)});
+                    z = z1 - 1;
+                }
+            } else {
+                bandRuns.clear(), bandRow0.clear(), bandRows.clear();
+            }
+        }
+        if (!banded) TG_CUDA(cudaMemcpyAsync(dx.p, x, sizeof(float) * nvox, cudaMemcpyHostToDevice, st));
         if (n_iter > 0) {
             TG_CUDA(cudaStreamCreateWithFlags(&up, cudaStreamNonBlocking));
             cudaEvent_t start;
@@ -725,6 +837,15 @@ static int plan_ossart_impl(tigre_plan* P, const float* b, float* x, int n_iter,
             ev.push_back(start);
             TG_CUDA(cudaEventRecord(start, st));               // the buffer exists from here on in stream order
             TG_CUDA(cudaStreamWaitEvent(up, start, 0));
+            for (size_t bnd = 0; bnd < bandRuns.size(); ++bnd) {
+                for (const auto& run : bandRuns[bnd])
+                    TG_CUDA(cudaMemcpyAsync(dx.as<float>() + run[0] * slice, x + run[0] * slice, sizeof(float) * slice * run[1], cudaMemcpyHostToDevice, up));
+                cudaEvent_t e;
+                TG_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+                ev.push_back(e);
+                TG_CUDA(cudaEventRecord(e, up));
+            }
+            sbase = (int)ev.size();   // ev[sbase + s - s_begin]: subset s's projections have arrived
             for (int s = s_begin; s < s_end; ++s) {
                 for (int k = P->off[s]; k < P->off[s + 1]; ++k) {
                     const size_t o = per * (size_t)P->idx[k];
@@ -741,10 +862,10 @@ static int plan_ossart_impl(tigre_plan* P, const float* b, float* x, int n_iter,
     TG_CUDA(cudaMemsetAsync(P->d_acc.p, 0, sizeof(double) * std::max(n_iter, 1), st));
     // the (x,y)-transposed copy of the iterate that the Ax kernels read for x-dominant rays is kept up to date by the
     // update kernel (one pass over the volume per subset instead of two)
-    TempBuf xT;
     float* xTd = nullptr;
-    if (n_iter > 0 && g.nx > 1 && g.ny > 1 && xT.alloc(sizeof(float) * nvox, st) == TIGRE_OK &&
-        launch_transpose_xy(xd, xT.as<float>(), g, st) == TIGRE_OK)
+    if (banded) xTd = xT.as<float>();   // filled band by band below
+    else if (n_iter > 0 && g.nx > 1 && g.ny > 1 && (xT.p || xT.alloc(sizeof(float) * nvox, st) == TIGRE_OK) &&
+             launch_transpose_xy(xd, xT.as<float>(), g, st) == TIGRE_OK)
         xTd = xT.as<float>();
     for (int it = 0; it < n_iter; ++it) {
         for (int s = s_begin; s < s_end; ++s) {
@@ -753,17 +874,60 @@ static int plan_ossart_impl(tigre_plan* P, const float* b, float* x, int n_iter,
             float* Vs = nullptr;
             float* A = P->Axb.as<float>();
             TG_TRY(P->col_weights(s, &Vs, st));   // (when V_s is not stored this uses A as scratch: before this subset's projection)
-            TG_TRY(launch_ax(xd, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st, nullptr, xTd, P->hray[s].data()));
-            if (up && it == 0) TG_CUDA(cudaStreamWaitEvent(st, ev[1 + s - s_begin], 0));   // this subset's projections have arrived
+            if (banded && it == 0 && s == s_begin) {
+                const size_t slice = (size_t)g.nx * g.ny;
+                for (size_t bnd = 0; bnd < bandRuns.size(); ++bnd) {
+                    TG_CUDA(cudaStreamWaitEvent(st, ev[1 + bnd], 0));   // this band's slices of the iterate have arrived
+                    for (const auto& run : bandRuns[bnd]) {
+                        Grid gs = g;
+                        gs.nz = (int)run[1];
+                        TG_TRY(launch_transpose_xy(xd + run[0] * slice, xTd + run[0] * slice, gs, st));
+                    }
+                    if (bnd < bandRows.size() && bandRows[bnd] > 0) {
+                        const AxSub sub{bandRow0[bnd], bandRows[bnd], 0, g.nz};
+                        TG_TRY(launch_ax(xd, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st, &sub, xTd, P->hray[s].data()));
+                    }
+                }
+            } else {
+                TG_TRY(launch_ax(xd, g, P->ray[s].as<RayView>(), n, P->ax_mode, false, false, A, nullptr, st, nullptr, xTd, P->hray[s].data()));
+            }
+            if (up && it == 0) TG_CUDA(cudaStreamWaitEvent(st, ev[sbase + s - s_begin], 0));   // this subset's projections have arrived
             // r = W_s .* (b_s - A_s x) in place over A; b is gathered through the subset's view list
             TG_TRY(launch_residual(bd, P->d_idx.as<int32_t>() + P->off[s], A, Ws, A, per, n, P->d_acc.as<double>() + it, st));
+            if (up && xTd && it == n_iter - 1 && s == s_end - 1 && g.nz >= 32 * X_BANDS) {
+                // last update of an end-to-end call: backprojection and update go range by range of z-slices (whole 32-slice blocks of
+                // the backprojector), and each range of the new iterate starts for the host on the side stream as soon as it is final,
+                // behind the ranges still being computed (the same kernels on the same data: the same bits)
+                const size_t slice = (size_t)g.nx * g.ny;
+                const int step = (g.nz / X_BANDS + 31) / 32 * 32;
+                for (int z0 = 0; z0 < g.nz; z0 += step) {
+                    const int nzs = std::min(step, g.nz - z0);
+                    const size_t o = (size_t)z0 * slice;
+                    TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>() + o, z0, nzs, false, 0, g.nv, P->clamp, st,
+                                      P->hvox[s].data()));
+                    TG_TRY(launch_update_t(xd + o, xTd + o, P->grad.as<float>() + o, Vs ? Vs + o : nullptr, lambda, nonneg, g.nx, g.ny, nzs, st));
+                    cudaEvent_t e;
+                    TG_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+                    ev.push_back(e);
+                    TG_CUDA(cudaEventRecord(e, st));
+                    TG_CUDA(cudaStreamWaitEvent(up, e, 0));
+                    TG_CUDA(cudaMemcpyAsync(x + o, xd + o, sizeof(float) * slice * nzs, cudaMemcpyDeviceToHost, up));
+                }
+                cudaEvent_t e;
+                TG_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+                ev.push_back(e);
+                TG_CUDA(cudaEventRecord(e, up));
+                TG_CUDA(cudaStreamWaitEvent(st, e, 0));   // the caller's stream is done when the iterate is on the host
+                downloaded = true;
+                continue;
+            }
             TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>(), 0, g.nz, false, 0, g.nv, P->clamp, st,
                               P->hvox[s].data()));
             if (xTd) TG_TRY(launch_update_t(xd, xTd, P->grad.as<float>(), Vs, lambda, nonneg, g.nx, g.ny, g.nz, st));
             else TG_TRY(launch_update(xd, P->grad.as<float>(), Vs, lambda, nonneg, nvox, st));
         }
     }
-    if (xd != x) TG_CUDA(cudaMemcpyAsync(x, xd, sizeof(float) * nvox, cudaMemcpyDeviceToHost, st));
+    if (xd != x && !downloaded) TG_CUDA(cudaMemcpyAsync(x, xd, sizeof(float) * nvox, cudaMemcpyDeviceToHost, st));
     if (resid_hist && n_iter > 0) {
         std::vector<double> h(n_iter);
         TG_CUDA(cudaMemcpyAsync(h.data(), P->d_acc.p, sizeof(double) * n_iter, cudaMemcpyDeviceToHost, st));

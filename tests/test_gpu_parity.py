@@ -414,6 +414,40 @@ def test_plan_pinned_host_path_equals_device_path(tg):
     plan.close(), plan2.close()
 
 
+@pytest.mark.parametrize("ax_mode", ["siddon", "interp"])
+def test_plan_pinned_host_path_with_a_nonzero_iterate(tg, ax_mode):
+    """The end-to-end path sends the iterate up slice range by slice range, in the order the row bands of the first projection need
+    it (tigre_band_z_range), and starts each band when its slices are there.  With a non-zero starting iterate a band that read a
+    slice before it arrived would change the result: the bits must be those of the device-resident path.  C3's geometry, a rolled
+    and offset detector (rows do not map to z), parallel beam (no bound: the iterate goes up whole), and a 128-slice volume, where
+    the last backprojection + update of the call runs in four z-ranges whose download overlaps the ranges still being computed."""
+    rng = np.random.default_rng(61)
+    cases = []
+    geo, ang, rec = make_config("C3", scale=8, n_angles=24)
+    cases.append((geo, ang))
+    g2 = Geometry(nVoxel=(48, 40, 56), dVoxel=(1.0, 1.0, 0.8), nDetector=(64, 72), dDetector=(1.5, 1.2), DSD=600.0, DSO=380.0,
+                  offDetector=(3.0, -4.0), rotDetector=(0.6, 0.05, -0.04))
+    cases.append((g2, circular_angles(12, start=0.1)))
+    cases.append((geo.copy(mode="parallel"), ang))
+    g4, a4, _ = make_config("C3", scale=4, n_angles=12)           # 128 slices: the last update's download goes range by range as well
+    cases.append((g4, a4))
+    for geo, ang in cases:
+        nA = len(ang)
+        subsets = [np.arange(s, nA, 3) for s in range(3)]
+        plan = tg.OssartPlan(geo, ang, subsets, ax_mode, "matched")
+        x0 = rng.random(geo.vol_shape, dtype=np.float32)
+        b = rng.random((nA,) + geo.proj_shape, dtype=np.float32) * 50.0
+        x = dev(x0)
+        plan.iterate(dev(b), x, 1, want_resid=False)
+        b_h = torch.from_numpy(b).pin_memory()
+        x_h = torch.from_numpy(x0.copy()).pin_memory()
+        for _ in range(2):                                   # twice: the second call finds the pool's buffers holding the first call's data
+            x_h.copy_(torch.from_numpy(x0))
+            plan.iterate(b_h, x_h, 1, want_resid=False)
+            assert torch.equal(x_h, x.cpu())
+        plan.close()
+
+
 # ------------------------------------------------------------------ the TMA-staged Siddon projector (ax_siddon_tma.cu)
 def test_siddon_ax_staged_kernel_is_bitwise_the_l1_kernel(tg):
     """tigre_set_siddon_path(1): the interior of the march read from shared-memory boxes.  Same lengths, same order of
