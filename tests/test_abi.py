@@ -94,3 +94,21 @@ def test_product_does_not_import_oracle():
             txt = open(os.path.join(ROOT, "oracle", fn)).read()
             assert not re.search(r"^\s*(import|from)\s+paper_2412_10129_b200", txt, flags=re.M), fn
             assert "libtigre_b200" not in txt and "#include \"../" not in txt, fn
+
+
+def test_no_alloc_entry_point_rejects_oversize_without_a_device(lib_path):
+    """tigre_residual_noalloc: the size limit of its fixed scratch array is checked before anything else (no device needed), the
+    header's constant is the binding's, and the error has its own code and text."""
+    import paper_2412_10129_b200 as tg
+    hdr = open(os.path.join(ROOT, "include", "tigre_b200.h")).read()
+    m = re.search(r"#define\s+TIGRE_RESIDUAL_NOALLOC_MAX_N\s+(\d+)ull", hdr)
+    assert m and int(m.group(1)) == tg.RESIDUAL_NOALLOC_MAX_N == 1 << 28
+    lib = ctypes.CDLL(lib_path)
+    lib.tigre_strerror.restype = ctypes.c_char_p
+    code = lib.tigre_residual_noalloc(None, None, None, None, ctypes.c_size_t(tg.RESIDUAL_NOALLOC_MAX_N + 1), None, None)
+    assert code == -7 and b"no-allocation" in lib.tigre_strerror(code)
+    src = open(os.path.join(ROOT, "paper_2412_10129_b200", "csrc", "noalloc.cu")).read()
+    body = src[src.index('extern "C"'):]
+    for banned in ("cudaMalloc", "cudaFree", "cudaHostAlloc", "TempBuf", "cudaStreamCreate", "cudaEventCreate", "Synchronize"):
+        assert banned not in body, banned                     # the entry point allocates nothing and never synchronises
+    assert "static __device__ __align__(256)" in src and "cudaGetSymbolAddress" in src
