@@ -833,7 +833,9 @@ def main():
                 "units_per_launch": k_units / n_launch,
                 "share_of_step": prof["ms"][kind] / ms, "ms_per_pass": k_ms,
                 "other_kernel": {"kernel": other, "achieved": other_ach, "peak": model_peak(other, rates),
-                                 "frac": other_ach / model_peak(other, rates), "bounds": model_bounds(other, rates)},
+                                 "frac": other_ach / model_peak(other, rates), "bounds": model_bounds(other, rates),
+                                 "note": "in the plan's OS-SART step this kernel also forms the update x <- max(0, x + lambda V .* A^T r) in its epilogue "
+                                         "(fusion F2: no separate update kernel, no gradient volume); the kernel with a plain store: per_config / --mode kernel"},
                 "hbm": {"algorithmic_bytes_per_pass": hbm_bytes, "achieved_gbs": hbm_bytes / (k_ms * 1e-3) / 1e9,
                         "peak_gbs": peaks.get("hbm_gbs"), "peak_source": "MEASURED_PEAKS.json hbm_gbs",
                         "note": "compulsory HBM traffic is ~1% of the time: not the bound"}}

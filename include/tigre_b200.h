@@ -382,6 +382,10 @@ TIGRE_API int tigre_set_ax_path(int path);
  * volume, whole detector, 32-bit offsets).  Bitwise the same projections; the staged kernel is the slower one on B200
  * (profiles/r2_ax_siddon.md) and is kept for A/B measurement and its test. */
 TIGRE_API int tigre_set_siddon_path(int path);
+/* fusion F2 in the plan drivers' OS-SART step: 1 (default) = the update x <- max(0, x + lambda V .* A^T r) is formed in the epilogue of
+ * the TMA backprojection kernel (no gradient volume written or read; the same arithmetic, bitwise the same iterate), 0 = backprojection
+ * and update as two kernels.  Problems the TMA kernel does not take run the two kernels either way.  A/B and test hook. */
+TIGRE_API int tigre_set_plan_fuse(int on);
 /* which FDK pre-filter kernel runs: 0 (default) = the Toeplitz GEMM on the tensor cores (tcgen05, 3 x tf32 split products into an fp32
  * accumulator in tensor memory) whenever nDetector_u is a multiple of 4 and input and output are distinct 16-byte aligned arrays,
  * 1 = always the CUDA-core convolution.  Same taps, same weights; A/B and test hook. */

@@ -53,7 +53,7 @@ EXPORTS = ["tigre_Ax", "tigre_Atb", "tigre_Ax_slab", "tigre_Atb_slab", "tigre_sl
            "tigre_awtv", "tigre_awtv_gradient", "tigre_minimize_awtv", "tigre_tv_prox", "tigre_fista", "tigre_Ax_count", "tigre_plan_create", "tigre_plan_create_ex", "tigre_plan_ossart", "tigre_plan_asd_pocs", "tigre_plan_osem", "tigre_plan_sart_tv", "tigre_plan_destroy",
            "tigre_plan_bytes", "tigre_profile", "tigre_profile_read", "tigre_workspace_bytes", "tigre_set_chunk_budget", "tigre_chunk_stats", "tigre_set_atb_path", "tigre_set_tv_path", "tigre_strerror",
            "tigre_last_cuda_error", "tigre_version", "tigre_Ax_index", "tigre_set_index_path", "tigre_set_workspace", "tigre_plan_workspace_bytes",
-           "tigre_workspace_stats", "tigre_sirt_chunked", "tigre_microbench", "tigre_set_ax_path", "tigre_set_plan_v_path", "tigre_plan_ossart_subsets", "tigre_Atb_boxes", "tigre_set_fdk_path", "tigre_residual_noalloc", "tigre_set_siddon_path", "tigre_band_z_range"]
+           "tigre_workspace_stats", "tigre_sirt_chunked", "tigre_microbench", "tigre_set_ax_path", "tigre_set_plan_v_path", "tigre_plan_ossart_subsets", "tigre_Atb_boxes", "tigre_set_fdk_path", "tigre_residual_noalloc", "tigre_set_siddon_path", "tigre_band_z_range", "tigre_set_plan_fuse"]
 
 
 def _lib():
@@ -647,6 +647,11 @@ def band_z_range(geo, angles, row0, row1):
         return None
     _check(rc, "tigre_band_z_range")
     return lo.value, hi.value
+
+
+def set_plan_fuse(on):
+    """1 = OS-SART update in the backprojector's epilogue where the TMA kernel runs (default), 0 = as its own kernel."""
+    _check(_lib().tigre_set_plan_fuse(int(bool(on))), "tigre_set_plan_fuse")
 
 
 def set_siddon_path(path):

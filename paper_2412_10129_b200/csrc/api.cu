@@ -507,6 +507,7 @@ int tigre_microbench(int kind, double* value, void* cuda_stream) {
 
 // test hook (tigre_set_plan_v_path): 0 = store V_s per subset when they fit (default), 1 = always store, 2 = always recompute
 static int g_plan_v_path = 0;
+static int g_plan_fuse = 1;   // 1 = the OS-SART update runs in the backprojector's epilogue where it can (fusion F2), 0 = always as its own kernel (tigre_set_plan_fuse)
 }  // extern "C"
 namespace tg {
 extern int* g_atb_box_meta;
@@ -530,6 +531,12 @@ int tigre_Atb_boxes(const float* proj, const tigre_geo* geo, const double* angle
 int tigre_set_plan_v_path(int path) {
     if (path < 0 || path > 2) return TIGRE_ERR_ARG;
     g_plan_v_path = path;
+    return TIGRE_OK;
+}
+
+int tigre_set_plan_fuse(int on) {
+    if (on != 0 && on != 1) return TIGRE_ERR_ARG;
+    g_plan_fuse = on;
     return TIGRE_OK;
 }
 
@@ -904,9 +911,15 @@ static int plan_ossart_impl(tigre_plan* P, const float* b, float* x, int n_iter,
                 for (int z0 = 0; z0 < g.nz; z0 += step) {
                     const int nzs = std::min(step, g.nz - z0);
                     const size_t o = (size_t)z0 * slice;
-                    TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>() + o, z0, nzs, false, 0, g.nv, P->clamp, st,
-                                      P->hvox[s].data()));
-                    TG_TRY(launch_update_t(xd + o, xTd + o, P->grad.as<float>() + o, Vs ? Vs + o : nullptr, lambda, nonneg, g.nx, g.ny, nzs, st));
+                    const AtbFuse fz{xTd + o, Vs ? Vs + o : nullptr, lambda, nonneg};
+                    const int frc = g_plan_fuse ? launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, xd + o, z0, nzs, false, 0, g.nv, P->clamp, st,
+                                                             P->hvox[s].data(), &fz) : 2;
+                    if (frc < 0) return frc;
+                    if (frc == 2) {
+                        TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>() + o, z0, nzs, false, 0, g.nv, P->clamp, st,
+                                          P->hvox[s].data()));
+                        TG_TRY(launch_update_t(xd + o, xTd + o, P->grad.as<float>() + o, Vs ? Vs + o : nullptr, lambda, nonneg, g.nx, g.ny, nzs, st));
+                    }
                     cudaEvent_t e;
                     TG_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
                     ev.push_back(e);
@@ -921,6 +934,12 @@ static int plan_ossart_impl(tigre_plan* P, const float* b, float* x, int n_iter,
                 TG_CUDA(cudaStreamWaitEvent(st, e, 0));   // the caller's stream is done when the iterate is on the host
                 downloaded = true;
                 continue;
+            }
+            if (xTd && g_plan_fuse) {   // F2: the update in the backprojector's epilogue (where the TMA kernel takes the problem)
+                const AtbFuse fz{xTd, Vs, lambda, nonneg};
+                const int frc = launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, xd, 0, g.nz, false, 0, g.nv, P->clamp, st, P->hvox[s].data(), &fz);
+                if (frc < 0) return frc;
+                if (frc == TIGRE_OK) continue;
             }
             TG_TRY(launch_atb(A, g, P->vox[s].as<VoxView>(), n, P->atb_mode, false, P->grad.as<float>(), 0, g.nz, false, 0, g.nv, P->clamp, st,
                               P->hvox[s].data()));

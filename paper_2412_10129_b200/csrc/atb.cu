@@ -109,7 +109,7 @@ int g_atb_path = 0;   // 0 = TMA-staged kernel when the problem qualifies, 1 = g
 
 int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nViews, int mode, bool unit_proj,
                float* vol, int z0, int nzs, bool accumulate, int row0, int nrows, bool clamp, cudaStream_t st,
-               const VoxView* h_views) {
+               const VoxView* h_views, const AtbFuse* fuse) {
     if (mode != TIGRE_ATB_MATCHED && mode != TIGRE_ATB_FDK) return TIGRE_ERR_ARG;
     AtbP p;
     p.nx = g.nx, p.ny = g.ny, p.nz = g.nz, p.nu = g.nu, p.nv = g.nv;
@@ -120,6 +120,8 @@ int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nVi
     p.accumulate = accumulate ? 1 : 0;
     p.magic = 0x4B400000;
     p.lin_ok = g_atb_path != 3;
+    p.fuse = fuse ? 1 : 0, p.nonneg = fuse ? fuse->nonneg : 0, p.lambda = fuse ? fuse->lambda : 0.f, p.V = fuse ? fuse->V : nullptr, p.xT = fuse ? fuse->xT : nullptr;
+    if (fuse && (unit_proj || accumulate || !h_views || g_atb_path == 1)) return 2;
     constexpr int ZR = 8;
     dim3 block(ATB_BX, ATB_BY);
     dim3 grid((g.nx + ATB_BX - 1) / ATB_BX, (g.ny + ATB_BY - 1) / ATB_BY, (nzs + ZR - 1) / ZR);
@@ -129,6 +131,7 @@ int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nVi
         const int rc = launch_atb_tma(proj, g, d_views, h_views, nViews, mode, p, vol, st);
         if (rc <= 0) return rc;   // launched, or a CUDA error; rc > 0: does not qualify
     }
+    if (fuse) return 2;   // the gather kernel has no fused epilogue
     if (unit_proj) {
         if (mode == TIGRE_ATB_FDK) atb_gather_launch<TIGRE_ATB_FDK, true>(grid, block, st, clamp, proj, d_views, nViews, p, vol);
         else atb_gather_launch<TIGRE_ATB_MATCHED, true>(grid, block, st, clamp, proj, d_views, nViews, p, vol);

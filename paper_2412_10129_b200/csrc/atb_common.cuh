@@ -19,6 +19,14 @@ struct AtbP {
     int accumulate;
     int magic;            // 0x4B400000 = bits of 1.5*2^23 (floor_magic), passed as data (see atb_tma.cu)
     int lin_ok;           // atb_tma.cu: tilted views may take the linearised z-run (0 = always the per-voxel reciprocal: tigre_set_atb_path(3))
+    // fusion F2: the kernel's output IS the SART update.  With fuse != 0, `vol` is the iterate x (slab pointer, like
+    // the output otherwise): x <- max(0, x + lambda V .* (A^T r)) is formed in the epilogue from the accumulators, and the (x,y)-transposed
+    // copy xT gets the new value too; V and xT are slab pointers like vol.  The backprojector is issue-bound and leaves HBM idle, so the
+    // update's traffic hides behind the other CTAs' arithmetic, and the gradient volume is neither written nor read.
+    int fuse, nonneg;
+    float lambda;
+    const float* V;
+    float* xT;
 };
 
 constexpr int ATB_BX = 32, ATB_BY = 8;

@@ -364,8 +364,15 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
 #pragma unroll
         for (int k = 0; k < ZR; ++k) {
             if (zb + k < p.nzs) {
-                float* o = vol + (size_t)(zb + k) * slice + (size_t)iy * p.nx + ix;
-                *o = p.accumulate ? *o + acc[k] : acc[k];
+                const size_t i = (size_t)(zb + k) * slice + (size_t)iy * p.nx + ix;
+                if (p.fuse) {   // F2: the same arithmetic as update_t_kernel, on the accumulator instead of a stored gradient
+                    float v = fmaf(p.lambda * (p.V ? __ldg(p.V + i) : 1.f), acc[k], vol[i]);
+                    if (p.nonneg) v = fmaxf(v, 0.f);
+                    vol[i] = v;
+                    p.xT[(size_t)(zb + k) * slice + (size_t)ix * p.ny + iy] = v;
+                } else {
+                    vol[i] = p.accumulate ? vol[i] + acc[k] : acc[k];
+                }
             }
         }
     }

@@ -127,9 +127,16 @@ int launch_ax_adjoint(const float* proj, const Grid& g, const RayView* d_views, 
 //   row0/nrows: the projection buffer holds detector rows [row0,row0+nrows) only (chunked path)
 //   h_views: host copy of the same table; when given (and the problem qualifies) the TMA-staged kernel of
 //   atb_tma.cu runs, otherwise the L1/L2 gather kernel of atb.cu
+struct AtbFuse {   // launch_atb with the SART update in the backprojector's epilogue (atb_common.cuh, AtbP::fuse): vol = the iterate's slab
+    float* xT;     // slab of the (x,y)-transposed copy of the iterate, updated too
+    const float* V;   // slab of the column weights (may be null = ones)
+    float lambda;
+    int nonneg;
+};
+// Returns 2 (nothing launched) when `fuse` is given and the TMA kernel does not take the problem: the caller then runs the two steps.
 int launch_atb(const float* proj, const Grid& g, const VoxView* d_views, int nViews, int mode, bool unit_proj,
                float* vol, int z0, int nzs, bool accumulate, int row0, int nrows, bool clamp, cudaStream_t st,
-               const VoxView* h_views = nullptr);
+               const VoxView* h_views = nullptr, const AtbFuse* fuse = nullptr);
 // true if some voxel of the box can project beyond |index| 1e6 in some view (then the kernels clamp)
 bool vox_needs_clamp(const Grid& g, const VoxView* host_views, int n);
 

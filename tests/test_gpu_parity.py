@@ -414,6 +414,43 @@ def test_plan_pinned_host_path_equals_device_path(tg):
     plan.close(), plan2.close()
 
 
+@pytest.mark.parametrize("atb_mode", ["matched", "fdk"])
+def test_plan_update_fused_into_the_backprojector_is_bitwise_the_two_kernels(tg, atb_mode):
+    """Fusion F2 (tigre_set_plan_fuse): the OS-SART update formed in the epilogue of the TMA backprojection kernel from its
+    accumulators, against backprojection + update kernel: the same arithmetic on the same values, so the same bits, for the iterate
+    (and hence for every later residual).  C3's geometry with 16- and 32-voxel z-runs and ragged tiles, tilted views, lambda != 1,
+    with and without the non-negativity clamp; a geometry the TMA kernel does not take (nu % 4 != 0) runs the two kernels either way."""
+    rng = np.random.default_rng(71)
+    cases = []
+    geo, ang, rec = make_config("C3", scale=8, n_angles=24)
+    cases.append((geo.copy(nVoxel=(61, 50, 64)), ang))
+    cases.append((geo.copy(nVoxel=(64, 64, 40)), ang))
+    g2, a2, _ = make_config("C4", scale=16, n_angles=12)
+    cases.append((g2, a2))
+    godd, aodd = odd_geometry()
+    cases.append((godd, aodd))
+    for geo, ang in cases:
+        nA = len(ang)
+        subsets = [np.arange(s, nA, 3) for s in range(3)]
+        plan = tg.OssartPlan(geo, ang, subsets, "siddon", atb_mode)
+        x0 = rng.standard_normal(geo.vol_shape).astype(np.float32)
+        b = dev(rng.random((nA,) + geo.proj_shape, dtype=np.float32) * 40.0)
+        out = {}
+        try:
+            for fuse in (1, 0):
+                tg.set_plan_fuse(fuse)
+                for nonneg in (True, False):
+                    x = dev(x0)
+                    res = plan.iterate(b, x, 2, lam=0.7, nonneg=nonneg)
+                    out[(fuse, nonneg)] = (x.cpu(), np.asarray(res))
+        finally:
+            tg.set_plan_fuse(1)
+        for nonneg in (True, False):
+            assert torch.equal(out[(1, nonneg)][0], out[(0, nonneg)][0])
+            assert np.allclose(out[(1, nonneg)][1], out[(0, nonneg)][1], rtol=1e-12)
+        plan.close()
+
+
 @pytest.mark.parametrize("ax_mode", ["siddon", "interp"])
 def test_plan_pinned_host_path_with_a_nonzero_iterate(tg, ax_mode):
     """The end-to-end path sends the iterate up slice range by slice range, in the order the row bands of the first projection need
