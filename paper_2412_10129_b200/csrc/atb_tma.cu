@@ -223,8 +223,11 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
 #pragma unroll
             for (int k = 0; k < ZR; ++k) {
                 const float fv = fmaf((float)k, dfv, fv0);
-                const float tm = (fv - 0.5f) + 12582912.0f;
-                const float av = fv - (tm - 12582912.0f);
+                // row index and fraction: FRND.FLOOR on the conversion pipe (idle since the square root left this loop) and two adds; the
+                // magic-number floor of atb_common.cuh takes four adds on the FMA / ALU pipes (C3 1210 -> 1230 GUPS, C2 FDK 1112 -> 1140)
+                const float fl = floorf(fv);
+                const float av = fv - fl;
+                const float tm = fl + 12582912.0f;   // exact: the integer in the low mantissa bits
                 const uint32_t q = col + __float_as_uint(tm) * (uint32_t)(BU * 4);
                 float p00, p10, p01, p11;
                 asm volatile(
