@@ -482,6 +482,16 @@ def test_plan_pinned_host_path_with_a_nonzero_iterate(tg, ax_mode):
             x_h.copy_(torch.from_numpy(x0))
             plan.iterate(b_h, x_h, 1, want_resid=False)
             assert torch.equal(x_h, x.cpu())
+        # a sub-range of the subsets (the teacher-forcing entry): the bands are those of ITS first subset
+        y = dev(x0)
+        plan.iterate_subsets(dev(b), y, 1, 3)
+        x_h.copy_(torch.from_numpy(x0))
+        plan.iterate_subsets(b_h, x_h, 1, 3)
+        assert torch.equal(x_h, y.cpu())
+        # and no iteration at all: the iterate comes back as it went up
+        x_h.copy_(torch.from_numpy(x0))
+        plan.iterate(b_h, x_h, 0, want_resid=False)
+        assert torch.equal(x_h, torch.from_numpy(x0))
         plan.close()
 
 
