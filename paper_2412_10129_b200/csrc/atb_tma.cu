@@ -46,7 +46,9 @@ int32_t* g_atb_boxes = nullptr;
 // BU (box width, pixels) is a template parameter so that the second tap row is an immediate offset; the
 // launcher picks the smallest of 48, 80, ... 240 (all = 16 mod 32: with the 8 x 4 lane layout below, the taps
 // of one warp span < 16 columns of at most a few adjacent rows, and rows 16 banks apart do not collide).
-template <int MODE, int WX, int WY, int ZR, int BU>
+// FUSE: the OS-SART update in the epilogue (AtbP::fuse).  A template flag, not a branch on p.fuse: the branch alone cost the plain
+// kernel's tilted-view loop 4 % (C4 999 -> 962 GUPS: a different register allocation in the loops above it).
+template <int MODE, int WX, int WY, int ZR, int BU, bool FUSE = false>
 __global__ void __launch_bounds__(32 * (WX * WY + 1), 2)
 atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict__ proj, const VoxView* __restrict__ views,
                int nViews, AtbP p, int BV, int nStages, float* __restrict__ vol, int4* __restrict__ boxes) {
@@ -368,7 +370,7 @@ atb_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float* __restrict
         for (int k = 0; k < ZR; ++k) {
             if (zb + k < p.nzs) {
                 const size_t i = (size_t)(zb + k) * slice + (size_t)iy * p.nx + ix;
-                if (p.fuse) {   // F2: the same arithmetic as update_t_kernel, on the accumulator instead of a stored gradient
+                if (FUSE) {   // F2: the same arithmetic as update_t_kernel, on the accumulator instead of a stored gradient
                     float v = fmaf(p.lambda * (p.V ? __ldg(p.V + i) : 1.f), acc[k], vol[i]);
                     if (p.nonneg) v = fmaxf(v, 0.f);
                     vol[i] = v;
@@ -419,7 +421,7 @@ template <int MODE, int WX, int WY, int ZR, int BU>
 int tma_launch(const TmaArgs& A) {
     const size_t stageElems = ((size_t)BU * A.BV + 31) & ~(size_t)31;
     const size_t smem = A.nStages * stageElems * sizeof(float) + 2 * TMA_STAGES_MAX * sizeof(uint64_t) + TMA_STAGES_MAX * sizeof(StageInfo);
-    auto kern = atb_tma_kernel<MODE, WX, WY, ZR, BU>;
+    auto kern = A.p.fuse ? atb_tma_kernel<MODE, WX, WY, ZR, BU, true> : atb_tma_kernel<MODE, WX, WY, ZR, BU, false>;
     TG_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 block(32, WX * WY + 1), grid((A.p.nx + 8 * WX - 1) / (8 * WX), (A.p.ny + 4 * WY - 1) / (4 * WY), (A.p.nzs + ZR - 1) / ZR);
     if (grid.y > 65535 || grid.z > 65535) return TIGRE_ERR_ARG;
